@@ -1,0 +1,408 @@
+#!/usr/bin/env python
+"""bench.py — coarse-op apply throughput on B200 (BASELINE.json metric: coarse-op site-updates/s
+and effective HBM GB/s).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl ours|reference]
+
+Workload (default C2 = BASELINE.json configs[1], the configuration the metric is quoted on):
+16^3 x 24 periodic lattice, Nc = 48, complex64 links and vectors, 1 RHS, seeded Gamma-Hermitian
+generator, "run with dagger=0 and dagger=1".  One STEP = one pass of the whole hot path over the
+lattice in both modes: out = A.in followed by out2 = A^H.in (what one CGNE normal-equation
+application does), i.e. 2 V site-updates.  `value` is device-timed with all inputs resident in HBM;
+`e2e` goes through coarse_op_apply_host with pinned HOST vectors (H2D of the input vector and D2H
+of the result inside the timed region; the links are operator state, set once, like weights).
+
+N > 1 (torchrun): the path does not shard (north_star: single GPU, no inter-GPU communication), so
+each rank runs an independent replica of the same workload; the timed region is bracketed by a
+barrier + synchronize and the MAX over ranks is reported ("scaling": "weak").
+
+`--impl reference`: there is no reference implementation for this paper (no code exists); the
+reference arm times the CPU oracle (oracle/, fp64, as it stands) on the host cores on a bounded
+sample of the same workload.  This and the `cpu_baseline` leg are the only places that execute
+oracle/ outside tests.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import torch
+
+import synth
+
+METRIC = "coarse-op site-updates/s"
+UNIT = "site-updates/s"
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+# `ncu --set full` captures summarised under profiles/ (None until a capture exists).
+NCU_TRAFFIC_BYTES = {}
+
+
+def compulsory_bytes_per_site(Nc: int, links: str, nrhs: int) -> int:
+    """SURVEY.md §8(d) / north_star: 9 Nc^2 link entries + 9 input vectors + 1 output vector."""
+    link = 9 * Nc * Nc * (8 if links == "c64" else 4) + (36 if links == "i16" else 0)
+    return link + 10 * Nc * nrhs * 8
+
+
+def measured_peak_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        self._period = period_s
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _loop(self):
+        nv = self._nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for k, bit in names.items():
+                    if mask & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self._period)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thread = threading.Thread(target=self._loop, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def dist_env():
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return world, rank, local
+
+
+def reduce_max_sum(local_ms: float, local_units: float, device=None):
+    """(max over ranks of the elapsed time, sum over ranks of the units processed)."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return local_ms, local_units
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def barrier():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.barrier()
+
+
+# ------------------------------------------------------------------------------- CPU oracle legs
+def oracle_sample_dims(cfg):
+    """Bounded sample of the workload for the CPU oracle: a slab of the same lattice (same Nc, same
+    generator, same per-site work), periodic on its own."""
+    d = list(cfg["dims"])
+    per_site = 9 * cfg["Nc"] ** 2 * cfg["nrhs"]
+    budget = 4.0e7 * 1.0            # complex MACs per apply (~0.05-0.5 s on 8-64 host cores)
+    while d[0] * d[1] * d[2] * d[3] * per_site > budget and d[3] > 2:
+        d[3] = max(2, d[3] // 2)
+    while d[0] * d[1] * d[2] * d[3] * per_site > budget and d[2] > 2:
+        d[2] = max(2, d[2] // 2)
+    while d[0] * d[1] * d[2] * d[3] * per_site > budget and d[1] > 2:
+        d[1] = max(2, d[1] // 2)
+    return tuple(d)
+
+
+def make_oracle_sample(cfg, device):
+    import oracle
+    dims = oracle_sample_dims(cfg)
+    Nc, nrhs = cfg["Nc"], cfg["nrhs"]
+    links = synth.make_gamma_hermitian_links(dims, Nc, cfg["seed"], device=device).cpu().numpy()
+    scales, prec = None, oracle.LINK_C64
+    if cfg["links"] == "i16":
+        q, scales = oracle.quantize_i16(links, Nc)
+        links, prec = q.reshape(-1, 9, Nc, Nc, 2), oracle.LINK_I16
+    vin = synth.make_vectors(dims, Nc, nrhs, cfg["seed"] + 1, device=device).cpu().numpy()
+    return dims, links, scales, prec, vin
+
+
+def oracle_step(sample, cfg, daggers):
+    import oracle
+    dims, links, scales, prec, vin = sample
+    for dg in daggers:
+        oracle.coarse_apply(dims, cfg["Nc"], links, vin, nrhs=cfg["nrhs"], dagger=dg,
+                            link_precision=prec, scales=scales)
+
+
+def time_oracle(cfg, daggers, device, min_seconds=10.0, max_steps=200):
+    import oracle
+    oracle.build()
+    sample = make_oracle_sample(cfg, device)
+    V = synth.lattice_volume(sample[0])
+    oracle_step(sample, cfg, daggers)                      # warm-up (page-in, thread pool)
+    t0 = time.perf_counter()
+    n = 0
+    while n < max_steps and (time.perf_counter() - t0 < min_seconds or n < 3):
+        oracle_step(sample, cfg, daggers)
+        n += 1
+    dt = time.perf_counter() - t0
+    return {
+        "value": V * len(daggers) * n / dt,
+        "unit": UNIT,
+        "cores": oracle.max_threads(),
+        "kind": "oracle",
+        "sample": f"{n} steps on a {'x'.join(map(str, sample[0]))} slab of the workload lattice "
+                  f"({V} sites, same Nc/links/nrhs/generator, periodic on its own), {dt:.1f} s of CPU time",
+    }
+
+
+def run_reference(args, cfg, daggers):
+    """--impl reference: the CPU oracle as it stands, on the host cores (rank 0 only)."""
+    world, rank, _ = dist_env()
+    if rank != 0:
+        return 0
+    import oracle
+    oracle.build()
+    device = "cuda" if torch.cuda.is_available() else "cpu"
+    sample = make_oracle_sample(cfg, device)
+    V = synth.lattice_volume(sample[0])
+    for _ in range(args.warmup):
+        oracle_step(sample, cfg, daggers)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(sample, cfg, daggers)
+    dt = time.perf_counter() - t0
+    value = V * len(daggers) * args.steps / dt
+    sample_desc = (f"each step = dagger {daggers} applies on a {'x'.join(map(str, sample[0]))} slab "
+                   f"({V} sites) of the workload lattice, same Nc/links/nrhs/generator")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": workload_name(args.config, cfg), "sample": sample_desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+                         "sample": sample_desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_name(name, cfg):
+    return (f"{name}: coarse-op apply, {'x'.join(map(str, cfg['dims']))} periodic lattice, Nc={cfg['Nc']}, "
+            f"{cfg['links']} links, complex64 vectors, nrhs={cfg['nrhs']}")
+
+
+# ------------------------------------------------------------------------------- GPU arm
+def run_ours(args, cfg, daggers):
+    import paper_2212_12559_b200 as cop
+
+    world, rank, local = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the coarse-op library has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    dims, Nc, nrhs = cfg["dims"], cfg["Nc"], cfg["nrhs"]
+    V = synth.lattice_volume(dims)
+    prec = cop.LINK_I16 if cfg["links"] == "i16" else cop.LINK_C64
+
+    links = synth.make_gamma_hermitian_links(dims, Nc, cfg["seed"], device=dev)
+    scales = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device=dev)
+        scales = torch.empty((V, 9), dtype=torch.float32, device=dev)
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        torch.cuda.synchronize()
+        links = q
+    vin = synth.make_vectors(dims, Nc, nrhs, cfg["seed"] + 1, device=dev)
+    vouts = [torch.empty_like(vin) for _ in daggers]
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    if args.path:
+        op.set_option(cop.OPT_PATH, args.path)
+
+    stream = torch.cuda.current_stream()
+    launches = 0
+
+    def step(record=None):
+        nonlocal launches
+        for k, dg in enumerate(daggers):
+            if record is not None:
+                e0 = torch.cuda.Event(enable_timing=True)
+                e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+            op.apply(vin, vouts[k], nrhs=nrhs, dagger=dg)
+            launches += op.last_launches
+            if record is not None:
+                e1.record(stream)
+                record[dg].append((e0, e1))
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    barrier()
+    launches = 0
+    per_launch = {dg: [] for dg in daggers}
+    t_start = torch.cuda.Event(enable_timing=True)
+    t_end = torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        torch.cuda.synchronize()
+        t_start.record(stream)
+        for _ in range(args.steps):
+            step(per_launch)
+        t_end.record(stream)
+        torch.cuda.synchronize()
+    barrier()
+    local_ms = t_start.elapsed_time(t_end)
+    units_local = float(V) * len(daggers) * args.steps
+    total_ms, units = reduce_max_sum(local_ms, units_local, device=dev)
+    value = units / (total_ms * 1e-3)
+    gpu_launches = launches
+
+    kernel_ms = {dg: sum(a.elapsed_time(b) for a, b in per_launch[dg]) / max(1, len(per_launch[dg]))
+                 for dg in daggers}
+
+    # ---- end to end: host vectors through coarse_op_apply_host
+    vin_h = vin.cpu().pin_memory()
+    vout_h = torch.empty_like(vin_h).pin_memory()
+    e2e_steps = max(3, min(args.steps, 20))
+    for dg in daggers:
+        op.apply_host(vin_h, vout_h, nrhs=nrhs, dagger=dg)
+    torch.cuda.synchronize()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        for dg in daggers:
+            op.apply_host(vin_h, vout_h, nrhs=nrhs, dagger=dg)      # synchronises the stream itself
+    torch.cuda.synchronize()
+    e2e_ms_local = 1e3 * (time.perf_counter() - t0)
+    barrier()
+    e2e_ms, e2e_units = reduce_max_sum(e2e_ms_local, float(V) * len(daggers) * e2e_steps, device=dev)
+    vec_bytes = V * Nc * nrhs * 8
+
+    if rank != 0:
+        return 0
+
+    peak, peak_src = measured_peak_gbs()
+    bps = compulsory_bytes_per_site(Nc, cfg["links"], nrhs)
+    dom = daggers[0]
+    achieved = bps * V / (kernel_ms[dom] * 1e-3) / 1e9
+    roofline = {
+        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "traffic": NCU_TRAFFIC_BYTES.get((args.config, dom)),
+        "kernel": f"coarse_apply_stream<{Nc},{'i16' if prec else 'c64'},dagger={dom}>" if op.last_path == cop.PATH_STREAM
+                  else f"path {op.last_path}",
+        "kernel_ms": kernel_ms[dom],
+        "algorithmic_bytes_per_launch": bps * V,
+        "peak_source": peak_src,
+        "frac_of_nominal_8000": achieved / 8000.0,
+    }
+    for dg in daggers[1:]:
+        roofline[f"dagger{dg}_achieved"] = bps * V / (kernel_ms[dg] * 1e-3) / 1e9
+        roofline[f"dagger{dg}_kernel_ms"] = kernel_ms[dg]
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {
+            "workload": workload_name(args.config, cfg),
+            "step": f"one apply per dagger in {daggers} (2V site-updates)" if len(daggers) == 2 else f"one apply, dagger={daggers[0]}",
+            "l2": "inputs larger than L2 (links %.2f GB per apply, no flush needed)" % (links.numel() * links.element_size() / 1e9)
+                  if links.numel() * links.element_size() > 4 * 126e6 else "working set fits L2: warm-L2 number",
+            "multi_gpu": "replicas only (the path does not shard; no collective)",
+            "seed": cfg["seed"],
+        },
+        "effective_gbs": value * bps / 1e9,
+        "clocks": clocks.summary(),
+        "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": vec_bytes * len(daggers),
+                "d2h_bytes_per_step": vec_bytes * len(daggers), "steps": e2e_steps,
+                "note": "vectors from/to pinned host memory every apply; links are resident operator state"},
+        "gpu_launches": gpu_launches,
+        "roofline": roofline,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        del links, vin, vouts
+        line["cpu_baseline"] = time_oracle(cfg, daggers, dev, min_seconds=args.cpu_seconds)
+    print(json.dumps(line), flush=True)
+    op.close()
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C2", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--dagger", default="both", choices=["0", "1", "both"])
+    ap.add_argument("--path", type=int, default=0, help="COARSE_PATH_* override (0 = auto)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0)
+    args = ap.parse_args()
+    cfg = synth.config(args.config)
+    daggers = [0, 1] if args.dagger == "both" else [int(args.dagger)]
+    if args.impl == "reference":
+        return run_reference(args, cfg, daggers)
+    return run_ours(args, cfg, daggers)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,132 @@
+/* coarse_op.h — C ABI of libcoarseop: the coarse-grid Dirac operator apply on one B200.
+ *
+ * The operation (BASELINE.json north_star; the paper names it "the coarse stencil operator",
+ * PAPER.md:L99 §3.1, stored as "nine 48^2 matrices per super-site: eight for the hopping terms
+ * and one for the [local] term", §3.1):
+ *
+ *   dagger = 0:  out(x) = X(x).in(x) + sum_{mu=0..3} [ Y_{+mu}(x).in(x+mu^) + Y_{-mu}(x).in(x-mu^) ]
+ *   dagger = 1:  out(x) = X(x)^H.in(x) + sum_mu [ Y_{+mu}(x-mu^)^H.in(x-mu^) + Y_{-mu}(x+mu^)^H.in(x+mu^) ]
+ *                (the true adjoint for arbitrary links; needed by the CGNE setup solver,
+ *                 PAPER.md:L123 Table 1)
+ *
+ * on a periodic 4-D lattice, X and Y dense Nc x Nc complex matrices, Nc = 2 N_vec after the
+ * chiral doubling of PAPER.md:L41/L87, applied to nrhs vectors at once (block variant;
+ * multi-RHS is the paper's future work).  Links are stored either as complex64
+ * or in the paper's "16-bit fixed point format": int16 (re,im) pairs with one
+ * fp32 scale per matrix, scale = max|component|/32767 (BASELINE.json config 4).
+ *
+ * Everything runs in hand-written sm_100a kernels.  There is no CPU fallback: every entry point
+ * that needs the GPU returns COARSE_ECUDA when no usable device is present.
+ *
+ * LAYOUTS (all device pointers unless a name ends in _host; all 16-byte aligned)
+ *   site index      s(x) = x0 + L0*(x1 + L1*(x2 + L2*x3)), dims = {L0,L1,L2,L3}; neighbours wrap
+ *                   periodically (extent 2: both hops come from the same site and both are added;
+ *                   extent 1: both come from the site itself).
+ *   links           links[s][m][i][j], m = 0:X, 1+mu:Y_{+mu}, 5+mu:Y_{-mu}; row-major,
+ *                   out_i = sum_j M_ij in_j.
+ *                   COARSE_LINK_C64: float[2] = (re,im) per entry.
+ *                   COARSE_LINK_I16: int16_t[2] = (re,im) per entry, entry = scales[s][m]*(re + i im).
+ *   scales          float scales[s][m] (COARSE_LINK_I16 only).
+ *   vectors         v[s][a][r], float[2] = (re,im), a in [0,Nc) colour-spin (a = chi*N_vec + k),
+ *                   r in [0,nrhs) innermost.
+ *
+ * OWNERSHIP  The handle owns metadata and (only if coarse_op_apply_host is used) two vector-sized
+ *   staging buffers.  Link, scale, in and out buffers are the caller's; coarse_op_set_links borrows
+ *   the pointers, which must stay valid and unchanged until destroy or the next set_links.
+ *
+ * ERRORS  int-returning calls return COARSE_OK (0) or a negative code; coarse_op_create returns
+ *   NULL.  coarse_op_last_error() gives a thread-local message.  No exception crosses the ABI.
+ *   Asynchronous device faults surface at the caller's next synchronisation.
+ *
+ * STREAMS  `stream` is a cudaStream_t passed as void* (0 = legacy default stream).  coarse_op_apply
+ *   enqueues and returns; it never synchronises and never allocates.  Results are bit-identical
+ *   from run to run (no floating-point atomics).
+ */
+#ifndef COARSE_OP_H
+#define COARSE_OP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct coarse_op coarse_op_t; /* opaque */
+
+enum { COARSE_LINK_C64 = 0, COARSE_LINK_I16 = 1 };
+
+enum {
+    COARSE_OK = 0,
+    COARSE_EINVAL = -1,       /* bad argument (NULL, misaligned, overlapping in/out, nrhs < 1, ...) */
+    COARSE_EUNSUPPORTED = -2, /* valid but not compiled in (see coarse_op_set_option)              */
+    COARSE_ENOTREADY = -3,    /* apply before set_links                                            */
+    COARSE_ECUDA = -4,        /* CUDA runtime error, or no sm_100 device                           */
+    COARSE_ENOMEM = -5
+};
+
+/* Kernel families.  AUTO picks STREAM when (Nc, precision, nrhs) is in its compiled set, else
+ * SIMPLE.  Every family computes the same operation; tests run parity on each. */
+enum {
+    COARSE_PATH_AUTO = 0,
+    COARSE_PATH_SIMPLE = 1,  /* one thread per output element, any even Nc, any nrhs             */
+    COARSE_PATH_STREAM = 2,  /* persistent TMA-bulk -> smem ring -> CUDA-core consumers           */
+    COARSE_PATH_TENSOR = 3   /* block apply on tcgen05 tensor cores (3xTF32), nrhs >= 8           */
+};
+
+enum {
+    COARSE_OPT_PATH = 0,     /* one of COARSE_PATH_*                                              */
+    COARSE_OPT_GRID = 1      /* persistent grid size for STREAM/TENSOR; 0 = one CTA per SM        */
+};
+
+/* Create an operator descriptor for a periodic lattice dims[0..3] (each >= 1), Nc even and
+ * >= 2, link_precision one of COARSE_LINK_*.  Returns NULL on error (see coarse_op_last_error). */
+coarse_op_t* coarse_op_create(const int dims[4], int Nc, int link_precision);
+
+/* V*9*Nc*Nc*8 bytes (C64) or V*9*Nc*Nc*4 bytes (I16); 0 for NULL. */
+size_t coarse_op_link_bytes(const coarse_op_t* op);
+/* V*9*4 bytes for I16, 0 for C64. */
+size_t coarse_op_scale_bytes(const coarse_op_t* op);
+/* V*Nc*nrhs*8 bytes. */
+size_t coarse_op_vector_bytes(const coarse_op_t* op, int nrhs);
+
+/* Borrow the device link array (layout above) and, for I16, the device scale array.
+ * scales_dev must be NULL for C64 and non-NULL for I16. */
+int coarse_op_set_links(coarse_op_t* op, const void* links_dev, const float* scales_dev);
+
+/* Select a kernel family / tuning knob (COARSE_OPT_*).  COARSE_EUNSUPPORTED if the requested
+ * family cannot run this operator's (Nc, precision); the nrhs-dependent check happens in apply. */
+int coarse_op_set_option(coarse_op_t* op, int option, int value);
+
+/* out = A.in (dagger = 0) or A^H.in (dagger = 1) for nrhs >= 1 right-hand sides.
+ * in_dev and out_dev are device vectors [V][Nc][nrhs] complex64 and must not overlap. */
+int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs, int dagger,
+                    void* stream);
+
+/* Same operation on HOST vectors: copies in_host to a device staging buffer owned by the handle
+ * (allocated on first use, grown when nrhs grows), applies, copies the result to out_host and
+ * synchronises the stream before returning.  Pinned host memory gives full PCIe rate. */
+int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, int nrhs, int dagger,
+                         void* stream);
+
+/* Kernel launches the most recent coarse_op_apply / coarse_op_apply_host on this handle enqueued. */
+int coarse_op_last_launches(const coarse_op_t* op);
+/* Family (COARSE_PATH_*) the most recent apply actually ran; 0 before the first apply. */
+int coarse_op_last_path(const coarse_op_t* op);
+
+/* The paper's reduced-precision link storage (BASELINE.json config 4), on the device:
+ * for each of n_matrices Nc x Nc complex64 matrices, scale = max|component|/32767 (fp32 division)
+ * and q = clamp(rint(component/scale), -32767, 32767) (fp32, round-half-to-even); an all-zero
+ * matrix gets scale 0 and q = 0.  links_c64_dev: float[n][Nc][Nc][2]; q_dev: int16[n][Nc][Nc][2];
+ * scales_dev: float[n]. */
+int coarse_op_quantize_i16(const void* links_c64_dev, int64_t n_matrices, int Nc, void* q_dev,
+                           float* scales_dev, void* stream);
+
+void coarse_op_destroy(coarse_op_t* op); /* NULL is a no-op */
+
+const char* coarse_op_last_error(void); /* thread-local, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COARSE_OP_H */

@@ -1,0 +1,231 @@
+"""paper_2212_12559_b200 — B200-native coarse-grid Dirac operator apply (arXiv:2212.12559 §3.1).
+
+Thin Python binding over libcoarseop.so (include/coarse_op.h).  The functions carry the C ABI's
+names and only marshal arguments: torch is used for device memory and streams, every step of the
+apply runs in the library's sm_100a kernels.  There is no CPU fallback: if the shared library is
+missing and cannot be built, importing `lib()` raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+from . import build as _build
+
+LINK_C64 = 0
+LINK_I16 = 1
+
+OK, EINVAL, EUNSUPPORTED, ENOTREADY, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
+
+PATH_AUTO, PATH_SIMPLE, PATH_STREAM, PATH_TENSOR = 0, 1, 2, 3
+OPT_PATH, OPT_GRID = 0, 1
+
+EXPORTS = (
+    "coarse_op_create", "coarse_op_link_bytes", "coarse_op_scale_bytes", "coarse_op_vector_bytes",
+    "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_host",
+    "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_destroy",
+    "coarse_op_last_error",
+)
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+class CoarseOpError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"libcoarseop error {code}: {message}")
+        self.code = code
+
+
+def lib() -> ctypes.CDLL:
+    """Load (building if needed) libcoarseop.so and declare its prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB_PATH
+    if _build.is_stale():
+        path = _build.build_library()          # raises if nvcc is missing: no silent fallback
+    L = ctypes.CDLL(path)
+    vp, ci, ci64, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_size_t
+    L.coarse_op_create.restype = vp
+    L.coarse_op_create.argtypes = [ctypes.POINTER(ci), ci, ci]
+    L.coarse_op_link_bytes.restype = sz
+    L.coarse_op_link_bytes.argtypes = [vp]
+    L.coarse_op_scale_bytes.restype = sz
+    L.coarse_op_scale_bytes.argtypes = [vp]
+    L.coarse_op_vector_bytes.restype = sz
+    L.coarse_op_vector_bytes.argtypes = [vp, ci]
+    L.coarse_op_set_links.restype = ci
+    L.coarse_op_set_links.argtypes = [vp, vp, vp]
+    L.coarse_op_set_option.restype = ci
+    L.coarse_op_set_option.argtypes = [vp, ci, ci]
+    L.coarse_op_apply.restype = ci
+    L.coarse_op_apply.argtypes = [vp, vp, vp, ci, ci, vp]
+    L.coarse_op_apply_host.restype = ci
+    L.coarse_op_apply_host.argtypes = [vp, vp, vp, ci, ci, vp]
+    L.coarse_op_last_launches.restype = ci
+    L.coarse_op_last_launches.argtypes = [vp]
+    L.coarse_op_last_path.restype = ci
+    L.coarse_op_last_path.argtypes = [vp]
+    L.coarse_op_quantize_i16.restype = ci
+    L.coarse_op_quantize_i16.argtypes = [vp, ci64, ci, vp, vp, vp]
+    L.coarse_op_destroy.restype = None
+    L.coarse_op_destroy.argtypes = [vp]
+    L.coarse_op_last_error.restype = ctypes.c_char_p
+    L.coarse_op_last_error.argtypes = []
+    _lib = L
+    return L
+
+
+def coarse_op_last_error() -> str:
+    return lib().coarse_op_last_error().decode()
+
+
+def _check(rc: int) -> None:
+    if rc != OK:
+        raise CoarseOpError(rc, coarse_op_last_error())
+
+
+def _ptr(t) -> Optional[int]:
+    return None if t is None else int(t.data_ptr())
+
+
+def _stream_handle(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return int(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)
+
+
+def coarse_op_create(dims: Sequence[int], Nc: int, link_precision: int) -> int:
+    arr = (ctypes.c_int * 4)(*[int(d) for d in dims])
+    h = lib().coarse_op_create(arr, int(Nc), int(link_precision))
+    if not h:
+        raise CoarseOpError(EINVAL, coarse_op_last_error())
+    return h
+
+
+def coarse_op_link_bytes(op: int) -> int:
+    return int(lib().coarse_op_link_bytes(op))
+
+
+def coarse_op_scale_bytes(op: int) -> int:
+    return int(lib().coarse_op_scale_bytes(op))
+
+
+def coarse_op_vector_bytes(op: int, nrhs: int) -> int:
+    return int(lib().coarse_op_vector_bytes(op, int(nrhs)))
+
+
+def coarse_op_set_links(op: int, links, scales=None) -> None:
+    """links / scales: CUDA tensors in the ABI layouts (borrowed: keep them alive)."""
+    for t in (links, scales):
+        if t is not None and (not t.is_cuda or not t.is_contiguous()):
+            raise ValueError("links/scales must be contiguous CUDA tensors")
+    if links.numel() * links.element_size() != coarse_op_link_bytes(op):
+        raise ValueError("links tensor has the wrong number of bytes for this operator")
+    if scales is not None and scales.numel() * scales.element_size() != coarse_op_scale_bytes(op):
+        raise ValueError("scales tensor has the wrong number of bytes for this operator")
+    _check(lib().coarse_op_set_links(op, _ptr(links), _ptr(scales)))
+
+
+def coarse_op_set_option(op: int, option: int, value: int) -> None:
+    _check(lib().coarse_op_set_option(op, int(option), int(value)))
+
+
+def coarse_op_apply(op: int, vin, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+    """vin / vout: contiguous CUDA complex64 tensors [V][Nc][nrhs]; enqueues on `stream`
+    (default: torch's current stream) and returns without synchronising."""
+    for t in (vin, vout):
+        if not t.is_cuda or not t.is_contiguous():
+            raise ValueError("vectors must be contiguous CUDA tensors")
+        if t.numel() * t.element_size() != coarse_op_vector_bytes(op, nrhs):
+            raise ValueError("vector tensor has the wrong number of bytes for this operator/nrhs")
+    _check(lib().coarse_op_apply(op, _ptr(vin), _ptr(vout), int(nrhs), int(dagger), _stream_handle(stream)))
+
+
+def coarse_op_apply_host(op: int, vin_host, vout_host, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+    """vin_host / vout_host: contiguous CPU complex64 tensors (pinned for full PCIe rate).
+    Copies in, applies, copies out and synchronises the stream."""
+    for t in (vin_host, vout_host):
+        if t.is_cuda or not t.is_contiguous():
+            raise ValueError("host vectors must be contiguous CPU tensors")
+        if t.numel() * t.element_size() != coarse_op_vector_bytes(op, nrhs):
+            raise ValueError("vector tensor has the wrong number of bytes for this operator/nrhs")
+    _check(lib().coarse_op_apply_host(op, _ptr(vin_host), _ptr(vout_host), int(nrhs), int(dagger),
+                                      _stream_handle(stream)))
+
+
+def coarse_op_last_launches(op: int) -> int:
+    return int(lib().coarse_op_last_launches(op))
+
+
+def coarse_op_last_path(op: int) -> int:
+    return int(lib().coarse_op_last_path(op))
+
+
+def coarse_op_quantize_i16(links_c64, Nc: int, q_out, scales_out, stream=None) -> None:
+    """links_c64: CUDA complex64 [...][Nc][Nc]; q_out: CUDA int16 [...][Nc][Nc][2]; scales_out: CUDA
+    float32 [...] (one per matrix)."""
+    n = links_c64.numel() // (Nc * Nc)
+    if q_out.numel() != 2 * links_c64.numel() or scales_out.numel() != n:
+        raise ValueError("quantize_i16: output tensors have the wrong size")
+    for t in (links_c64, q_out, scales_out):
+        if not t.is_cuda or not t.is_contiguous():
+            raise ValueError("quantize_i16 needs contiguous CUDA tensors")
+    _check(lib().coarse_op_quantize_i16(_ptr(links_c64), n, int(Nc), _ptr(q_out), _ptr(scales_out),
+                                        _stream_handle(stream)))
+
+
+def coarse_op_destroy(op: int) -> None:
+    if op:
+        lib().coarse_op_destroy(op)
+
+
+class CoarseOp:
+    """Owning convenience wrapper: keeps the borrowed link tensors alive with the handle."""
+
+    def __init__(self, dims: Sequence[int], Nc: int, link_precision: int = LINK_C64):
+        self.dims = tuple(int(d) for d in dims)
+        self.Nc = int(Nc)
+        self.link_precision = int(link_precision)
+        self.V = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
+        self._h = coarse_op_create(self.dims, self.Nc, self.link_precision)
+        self._links = None
+        self._scales = None
+
+    def set_links(self, links, scales=None) -> "CoarseOp":
+        coarse_op_set_links(self._h, links, scales)
+        self._links, self._scales = links, scales
+        return self
+
+    def set_option(self, option: int, value: int) -> "CoarseOp":
+        coarse_op_set_option(self._h, option, value)
+        return self
+
+    def apply(self, vin, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+        coarse_op_apply(self._h, vin, vout, nrhs, dagger, stream)
+
+    def apply_host(self, vin_host, vout_host, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+        coarse_op_apply_host(self._h, vin_host, vout_host, nrhs, dagger, stream)
+
+    @property
+    def last_launches(self) -> int:
+        return coarse_op_last_launches(self._h)
+
+    @property
+    def last_path(self) -> int:
+        return coarse_op_last_path(self._h)
+
+    def close(self) -> None:
+        if self._h:
+            coarse_op_destroy(self._h)
+            self._h = 0
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,341 @@
+// coarse_op.cu — C ABI of libcoarseop (include/coarse_op.h): argument checking, kernel selection
+// and launches.  All arithmetic of the coarse-op apply lives in the kernels included below.
+#include "../../include/coarse_op.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "common.cuh"
+#include "quantize_kernel.cuh"
+#include "simple_kernel.cuh"
+#include "stream_kernel.cuh"
+
+using namespace coarse;
+
+namespace {
+
+thread_local std::string g_last_error = "";
+
+int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    g_last_error = buf;
+    return code;
+}
+
+int cuda_fail(cudaError_t e, const char* what) {
+    return fail(COARSE_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace
+
+struct coarse_op {
+    Lat lat;
+    int Nc;
+    int prec;
+    const void* links;
+    const float* scales;
+    int path_opt;
+    int grid_opt;
+    int last_launches;
+    int last_path;
+    int device;
+    int num_sms;
+    int max_smem;
+    void* stage_in;
+    void* stage_out;
+    size_t stage_bytes;
+};
+
+namespace {
+
+// ---------------------------------------------------------------- STREAM dispatch
+template <int NC, bool I16, bool DAG>
+int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
+    using Gm = StreamGeom<NC, I16>;
+    static_assert(Gm::OK, "unsupported STREAM geometry");
+    StreamParams p = base;
+    p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
+    int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (Gm::stage_bytes(DAG) + 16);
+    if (stages > 12) stages = 12;
+    if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM: shared memory too small for Nc=%d", NC);
+    p.stages = stages;
+    const int smem = Gm::smem_bytes(DAG, stages);
+    auto kern = coarse_apply_stream<NC, I16, DAG>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
+    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
+    if (grid > p.n_items) grid = p.n_items;
+    kern<<<grid, Gm::THREADS, smem, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch");
+    return COARSE_OK;
+}
+
+template <int NC>
+int launch_stream_nc(const coarse_op* op, const StreamParams& p, int dagger, cudaStream_t stream) {
+    if (op->prec == COARSE_LINK_I16)
+        return dagger ? launch_stream_t<NC, true, true>(op, p, stream) : launch_stream_t<NC, true, false>(op, p, stream);
+    return dagger ? launch_stream_t<NC, false, true>(op, p, stream) : launch_stream_t<NC, false, false>(op, p, stream);
+}
+
+bool stream_supports(int Nc, int nrhs) {
+    if (nrhs != 1) return false;
+    switch (Nc) {
+        case 32: case 48: case 64: case 96: case 128: case 192: return true;
+        default: return false;
+    }
+}
+
+int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, cudaStream_t stream) {
+    StreamParams p;
+    p.lat = op->lat;
+    p.links = static_cast<const unsigned char*>(op->links);
+    p.scales = op->scales;
+    p.in = static_cast<const float2*>(in);
+    p.out = static_cast<float2*>(out);
+    p.n_items = 0;
+    p.stages = 0;
+    switch (op->Nc) {
+        case 32: return launch_stream_nc<32>(op, p, dagger, stream);
+        case 48: return launch_stream_nc<48>(op, p, dagger, stream);
+        case 64: return launch_stream_nc<64>(op, p, dagger, stream);
+        case 96: return launch_stream_nc<96>(op, p, dagger, stream);
+        case 128: return launch_stream_nc<128>(op, p, dagger, stream);
+        case 192: return launch_stream_nc<192>(op, p, dagger, stream);
+        default: return fail(COARSE_EUNSUPPORTED, "STREAM path is not compiled for Nc=%d", op->Nc);
+    }
+}
+
+int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, cudaStream_t stream) {
+    SimpleParams p;
+    p.lat = op->lat;
+    p.Nc = op->Nc;
+    p.nrhs = nrhs;
+    p.dagger = dagger;
+    p.links = op->links;
+    p.scales = op->scales;
+    p.in = static_cast<const float2*>(in);
+    p.out = static_cast<float2*>(out);
+    const int64_t total = (int64_t)op->lat.V * op->Nc * nrhs;
+    const int64_t blocks = (total + 255) / 256;
+    if (blocks > 0x7fffffffLL) return fail(COARSE_EUNSUPPORTED, "SIMPLE path: problem too large");
+    if (op->prec == COARSE_LINK_I16)
+        coarse_apply_simple<true><<<(unsigned)blocks, 256, 0, stream>>>(p);
+    else
+        coarse_apply_simple<false><<<(unsigned)blocks, 256, 0, stream>>>(p);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "simple kernel launch");
+    return COARSE_OK;
+}
+
+int check_apply_args(const coarse_op* op, const void* in, const void* out, int nrhs, int dagger) {
+    if (!op) return fail(COARSE_EINVAL, "apply: op is NULL");
+    if (!op->links) return fail(COARSE_ENOTREADY, "apply: coarse_op_set_links has not been called");
+    if (!in || !out) return fail(COARSE_EINVAL, "apply: in/out is NULL");
+    if (nrhs < 1) return fail(COARSE_EINVAL, "apply: nrhs must be >= 1 (got %d)", nrhs);
+    if (dagger != 0 && dagger != 1) return fail(COARSE_EINVAL, "apply: dagger must be 0 or 1 (got %d)", dagger);
+    return COARSE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+coarse_op_t* coarse_op_create(const int dims[4], int Nc, int link_precision) {
+    if (!dims) { fail(COARSE_EINVAL, "create: dims is NULL"); return nullptr; }
+    int64_t V = 1;
+    for (int mu = 0; mu < 4; ++mu) {
+        if (dims[mu] < 1) { fail(COARSE_EINVAL, "create: dims[%d] = %d must be >= 1", mu, dims[mu]); return nullptr; }
+        V *= dims[mu];
+        if (V > 0x7fffffffLL) { fail(COARSE_EINVAL, "create: lattice volume exceeds 2^31-1 sites"); return nullptr; }
+    }
+    if (Nc < 2 || (Nc & 1)) { fail(COARSE_EINVAL, "create: Nc = %d must be even and >= 2", Nc); return nullptr; }
+    if (link_precision != COARSE_LINK_C64 && link_precision != COARSE_LINK_I16) {
+        fail(COARSE_EINVAL, "create: unknown link_precision %d", link_precision);
+        return nullptr;
+    }
+    int dev = 0, count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess || count < 1) {
+        cudaGetLastError();
+        fail(COARSE_ECUDA, "create: no CUDA device (libcoarseop has no CPU fallback)");
+        return nullptr;
+    }
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) { cuda_fail(e, "cudaGetDevice"); return nullptr; }
+    int major = 0, sms = 0, smem = 0;
+    cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (major != 10) {
+        fail(COARSE_ECUDA, "create: device %d has compute capability %d.x; this library is built for sm_100a only", dev, major);
+        return nullptr;
+    }
+    coarse_op* op = new (std::nothrow) coarse_op();
+    if (!op) { fail(COARSE_ENOMEM, "create: out of host memory"); return nullptr; }
+    for (int mu = 0; mu < 4; ++mu) op->lat.L[mu] = dims[mu];
+    op->lat.V = (int)V;
+    op->Nc = Nc;
+    op->prec = link_precision;
+    op->links = nullptr;
+    op->scales = nullptr;
+    op->path_opt = COARSE_PATH_AUTO;
+    op->grid_opt = 0;
+    op->last_launches = 0;
+    op->last_path = 0;
+    op->device = dev;
+    op->num_sms = sms;
+    op->max_smem = smem;
+    op->stage_in = op->stage_out = nullptr;
+    op->stage_bytes = 0;
+    g_last_error = "";
+    return op;
+}
+
+size_t coarse_op_link_bytes(const coarse_op_t* op) {
+    if (!op) return 0;
+    return (size_t)op->lat.V * 9 * op->Nc * op->Nc * (op->prec == COARSE_LINK_I16 ? 4 : 8);
+}
+
+size_t coarse_op_scale_bytes(const coarse_op_t* op) {
+    if (!op || op->prec != COARSE_LINK_I16) return 0;
+    return (size_t)op->lat.V * 9 * 4;
+}
+
+size_t coarse_op_vector_bytes(const coarse_op_t* op, int nrhs) {
+    if (!op || nrhs < 1) return 0;
+    return (size_t)op->lat.V * op->Nc * nrhs * 8;
+}
+
+int coarse_op_set_links(coarse_op_t* op, const void* links_dev, const float* scales_dev) {
+    if (!op) return fail(COARSE_EINVAL, "set_links: op is NULL");
+    if (!links_dev) return fail(COARSE_EINVAL, "set_links: links_dev is NULL");
+    if (!aligned16(links_dev)) return fail(COARSE_EINVAL, "set_links: links_dev must be 16-byte aligned");
+    if (op->prec == COARSE_LINK_I16) {
+        if (!scales_dev) return fail(COARSE_EINVAL, "set_links: I16 links need scales_dev");
+        if ((reinterpret_cast<uintptr_t>(scales_dev) & 3u) != 0)
+            return fail(COARSE_EINVAL, "set_links: scales_dev must be 4-byte aligned");
+    } else if (scales_dev) {
+        return fail(COARSE_EINVAL, "set_links: scales_dev must be NULL for C64 links");
+    }
+    op->links = links_dev;
+    op->scales = scales_dev;
+    return COARSE_OK;
+}
+
+int coarse_op_set_option(coarse_op_t* op, int option, int value) {
+    if (!op) return fail(COARSE_EINVAL, "set_option: op is NULL");
+    switch (option) {
+        case COARSE_OPT_PATH:
+            if (value == COARSE_PATH_AUTO || value == COARSE_PATH_SIMPLE) { op->path_opt = value; return COARSE_OK; }
+            if (value == COARSE_PATH_STREAM) {
+                if (!stream_supports(op->Nc, 1))
+                    return fail(COARSE_EUNSUPPORTED, "set_option: STREAM path is not compiled for Nc=%d", op->Nc);
+                op->path_opt = value;
+                return COARSE_OK;
+            }
+            if (value == COARSE_PATH_TENSOR)
+                return fail(COARSE_EUNSUPPORTED, "set_option: TENSOR path is not available in this build");
+            return fail(COARSE_EINVAL, "set_option: unknown path %d", value);
+        case COARSE_OPT_GRID:
+            if (value < 0) return fail(COARSE_EINVAL, "set_option: grid must be >= 0");
+            op->grid_opt = value;
+            return COARSE_OK;
+        default:
+            return fail(COARSE_EINVAL, "set_option: unknown option %d", option);
+    }
+}
+
+int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs, int dagger, void* stream) {
+    int rc = check_apply_args(op, in_dev, out_dev, nrhs, dagger);
+    if (rc != COARSE_OK) return rc;
+    if (!aligned16(in_dev) || !aligned16(out_dev))
+        return fail(COARSE_EINVAL, "apply: in_dev/out_dev must be 16-byte aligned");
+    const size_t vb = coarse_op_vector_bytes(op, nrhs);
+    const uintptr_t a = reinterpret_cast<uintptr_t>(in_dev), b = reinterpret_cast<uintptr_t>(out_dev);
+    if (a < b + vb && b < a + vb) return fail(COARSE_EINVAL, "apply: in and out overlap (the stencil reads neighbours)");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int path = op->path_opt;
+    if (path == COARSE_PATH_AUTO) path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM : COARSE_PATH_SIMPLE;
+    op->last_launches = 0;
+    if (path == COARSE_PATH_STREAM) {
+        if (!stream_supports(op->Nc, nrhs))
+            return fail(COARSE_EUNSUPPORTED, "apply: STREAM path does not cover Nc=%d nrhs=%d", op->Nc, nrhs);
+        rc = launch_stream(op, in_dev, out_dev, dagger, st);
+    } else {
+        rc = launch_simple(op, in_dev, out_dev, nrhs, dagger, st);
+    }
+    if (rc != COARSE_OK) return rc;
+    op->last_launches = 1;
+    op->last_path = path;
+    return COARSE_OK;
+}
+
+int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, int nrhs, int dagger, void* stream) {
+    int rc = check_apply_args(op, in_host, out_host, nrhs, dagger);
+    if (rc != COARSE_OK) return rc;
+    const size_t vb = coarse_op_vector_bytes(op, nrhs);
+    if (op->stage_bytes < vb) {
+        if (op->stage_in) cudaFree(op->stage_in);
+        if (op->stage_out) cudaFree(op->stage_out);
+        op->stage_in = op->stage_out = nullptr;
+        op->stage_bytes = 0;
+        cudaError_t e = cudaMalloc(&op->stage_in, vb);
+        if (e == cudaSuccess) e = cudaMalloc(&op->stage_out, vb);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            if (op->stage_in) cudaFree(op->stage_in);
+            op->stage_in = nullptr;
+            return fail(COARSE_ENOMEM, "apply_host: cannot allocate %zu-byte staging buffers", vb);
+        }
+        op->stage_bytes = vb;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaMemcpyAsync(op->stage_in, in_host, vb, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e, "apply_host: H2D copy");
+    rc = coarse_op_apply(op, op->stage_in, op->stage_out, nrhs, dagger, stream);
+    if (rc != COARSE_OK) return rc;
+    e = cudaMemcpyAsync(out_host, op->stage_out, vb, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return cuda_fail(e, "apply_host: D2H copy");
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(e, "apply_host: stream synchronize");
+    return COARSE_OK;
+}
+
+int coarse_op_last_launches(const coarse_op_t* op) { return op ? op->last_launches : 0; }
+int coarse_op_last_path(const coarse_op_t* op) { return op ? op->last_path : 0; }
+
+int coarse_op_quantize_i16(const void* links_c64_dev, int64_t n_matrices, int Nc, void* q_dev, float* scales_dev,
+                           void* stream) {
+    if (!links_c64_dev || !q_dev || !scales_dev) return fail(COARSE_EINVAL, "quantize_i16: NULL pointer");
+    if (n_matrices < 0 || Nc < 1) return fail(COARSE_EINVAL, "quantize_i16: bad sizes");
+    if (n_matrices == 0) return COARSE_OK;
+    if ((int64_t)2 * Nc * Nc > 0x7fffffffLL) return fail(COARSE_EINVAL, "quantize_i16: Nc too large");
+    const unsigned grid = (unsigned)(n_matrices < 148 * 16 ? n_matrices : 148 * 16);
+    quantize_i16_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(
+        static_cast<const float*>(links_c64_dev), n_matrices, Nc, static_cast<short*>(q_dev), scales_dev);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "quantize kernel launch");
+    return COARSE_OK;
+}
+
+void coarse_op_destroy(coarse_op_t* op) {
+    if (!op) return;
+    if (op->stage_in) cudaFree(op->stage_in);
+    if (op->stage_out) cudaFree(op->stage_out);
+    delete op;
+}
+
+const char* coarse_op_last_error(void) { return g_last_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,115 @@
+// common.cuh — lattice indexing and PTX helpers shared by the coarse-op kernels (sm_100a).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace coarse {
+
+// Periodic 4-D lattice, site index s(x) = x0 + L0*(x1 + L1*(x2 + L2*x3))  (include/coarse_op.h).
+struct Lat {
+    int L[4];
+    int V;
+};
+
+// Site whose data stage m of output site s needs:
+//   m = 0           -> s
+//   dagger = 0      -> vector from x+mu^ (m = 1+mu) / x-mu^ (m = 5+mu); the link matrix is at s itself
+//   dagger = 1      -> link AND vector from x-mu^ (m = 1+mu) / x+mu^ (m = 5+mu)
+__device__ __forceinline__ int stencil_site(const Lat& lat, int s, int m, int dagger) {
+    if (m == 0) return s;
+    const int mu = (m - 1) & 3;
+    int sign = (m <= 4) ? 1 : -1;
+    if (dagger) sign = -sign;
+    int stride = 1;
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+        if (d < mu) stride *= lat.L[d];
+    const int Lmu = mu == 0 ? lat.L[0] : mu == 1 ? lat.L[1] : mu == 2 ? lat.L[2] : lat.L[3];
+    const int x = (s / stride) % Lmu;
+    int xn = x + sign;
+    if (xn == Lmu) xn = 0;
+    if (xn < 0) xn = Lmu - 1;
+    return s + (xn - x) * stride;
+}
+
+namespace ptx {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {
+    }
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+// 1-D TMA bulk copy global -> shared, completion counted in bytes on an mbarrier.
+// dst, src 16-byte aligned; bytes a multiple of 16.
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar,
+                                         uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int threads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint4 lds128u(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float2 lds64(uint32_t addr) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+
+}  // namespace ptx
+
+// int16 (re,im) packed in one 32-bit word -> two floats (exact).
+__device__ __forceinline__ float2 unpack_i16x2(uint32_t w) {
+    return make_float2((float)(short)(w & 0xffffu), (float)(short)(w >> 16));
+}
+
+}  // namespace coarse

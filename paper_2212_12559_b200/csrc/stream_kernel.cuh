@@ -1,0 +1,319 @@
+// stream_kernel.cuh — COARSE_PATH_STREAM: the single-RHS coarse-op apply as an HBM streaming kernel.
+//
+// 97-99 % of the bytes of one apply are the nine Nc x Nc link matrices per site (SURVEY.md §8(a)
+// row a3), each read exactly once, and in the C-ABI layout links[s][m][i][j] every (site, matrix,
+// row range) is one contiguous run of bytes.  So the kernel is a persistent producer/consumer
+// pipeline per SM:
+//
+//   producer (1 elected thread)  walks its work items and, per pipeline stage, issues two 1-D TMA
+//       bulk copies (cp.async.bulk, SASS UBLKCP) into a ring of S shared-memory slots: the link rows
+//       of one (site, matrix, row range) with an L2 evict_first hint, and the neighbour vector
+//       entries that those rows multiply with an evict_last hint (the vector field is re-read 9x
+//       and stays L2-resident).  Completion is counted in bytes on the slot's `full` mbarrier.
+//       With S x ~18 KB per SM the chip keeps > 20 MB of loads in flight, far beyond the
+//       latency x bandwidth product of HBM3e, with no registers tied up.
+//   consumers (W = 8 warps)      wait on `full`, read the slot with conflict-free LDS.128 (lane <->
+//       16-byte column quad, warp <-> rows), accumulate in fp32 registers across all nine matrices
+//       of the item, release the slot through its `empty` mbarrier, and combine partial sums ONCE
+//       per item (not per matrix): warp shuffles over the column slices (dagger = 0) or a
+//       shared-memory sum over the row slices (dagger = 1).
+//
+// dagger = 0: item = (site, row block of RS rows), 9 stages (one per matrix m); lane holds the
+//             vector entries of its columns, accumulators are per row.
+// dagger = 1: item = site, 9 * Nc/RS stages (matrix m of the dagger-neighbour, row chunk c);
+//             rows are the contraction index, lane <-> OUTPUT columns, the vector entry of a row is
+//             a shared-memory broadcast.  The same row-major layout serves both (no transposed copy).
+// int16 links: a 16-byte quad holds 4 complex entries; decode is in registers, the per-matrix fp32
+//             scale is folded into the (short) vector operand once per stage, never per entry.
+//
+// Summation order is fixed by the static schedule: results are bit-identical run to run.
+#pragma once
+#include "common.cuh"
+
+namespace coarse {
+
+struct StreamParams {
+    Lat lat;
+    const unsigned char* links;
+    const float* scales;
+    const float2* in;
+    float2* out;
+    int n_items;
+    int stages;
+};
+
+constexpr int stream_pow2ceil(int v) { return v <= 1 ? 1 : v <= 2 ? 2 : v <= 4 ? 4 : v <= 8 ? 8 : v <= 16 ? 16 : 32; }
+constexpr int stream_passes(int q) {
+    for (int p = 1; p <= 8; ++p)
+        if (q % p == 0 && q / p <= 32) return p;
+    return 0;
+}
+constexpr int stream_rows_per_stage(int nc, int rowbytes, int unit, int max_bytes) {
+    int best = 0;
+    for (int d = unit; d <= nc; d += unit)
+        if (nc % d == 0 && d * rowbytes <= max_bytes) best = d;
+    return best;
+}
+
+template <int NC, bool I16>
+struct StreamGeom {
+    static constexpr int W = 8;                                // consumer warps
+    static constexpr int ENTRY_BYTES = I16 ? 4 : 8;            // one complex link entry
+    static constexpr int ROWBYTES = NC * ENTRY_BYTES;
+    static constexpr int Q = ROWBYTES / 16;                    // 16-byte quads per row
+    static constexpr int CPQ = 16 / ENTRY_BYTES;               // complex entries per quad
+    static constexpr int PASSES = stream_passes(Q);
+    static constexpr int QP = Q / PASSES;                      // quads per row per pass (<= 32)
+    static constexpr int G = stream_pow2ceil(QP);              // lanes that share one row
+    static constexpr int RPL = 32 / G;                         // rows per warp-wide load
+    static constexpr int RS = stream_rows_per_stage(NC, ROWBYTES, W * RPL, 24576);
+    static constexpr int NB = NC / RS;                         // row blocks per matrix
+    static constexpr int WL = RS / (W * RPL);                  // warp-wide loads per warp, stage, pass
+    static constexpr int LINK_STAGE = RS * ROWBYTES;
+    static constexpr int VEC_STAGE_N = NC * 8;                 // dagger = 0: whole neighbour vector
+    static constexpr int VEC_STAGE_D = RS * 8;                 // dagger = 1: the RS entries of the chunk
+    static constexpr int RED_BYTES = 2 * W * RPL * NC * 8;     // dagger = 1: double-buffered partial sums
+    static constexpr bool OK = (ROWBYTES % 16 == 0) && PASSES > 0 && RS > 0 && (QP * PASSES == Q);
+    static constexpr int THREADS = (W + 1) * 32;
+
+    static constexpr int stage_bytes(bool dag) { return LINK_STAGE + (dag ? VEC_STAGE_D : VEC_STAGE_N); }
+    static constexpr int fixed_bytes(bool dag) { return (dag ? RED_BYTES : 0) + 128; }
+    static int smem_bytes(bool dag, int stages) { return stages * (stage_bytes(dag) + 16) + fixed_bytes(dag); }
+};
+
+// acc += M * v   (conj = false)   |   acc += conj(M) * v   (conj = true)
+template <bool CONJ>
+__device__ __forceinline__ void cmac(float2& acc, float mre, float mim, const float2 v) {
+    if (!CONJ) {
+        acc.x = fmaf(mre, v.x, acc.x);
+        acc.x = fmaf(-mim, v.y, acc.x);
+        acc.y = fmaf(mre, v.y, acc.y);
+        acc.y = fmaf(mim, v.x, acc.y);
+    } else {
+        acc.x = fmaf(mre, v.x, acc.x);
+        acc.x = fmaf(mim, v.y, acc.x);
+        acc.y = fmaf(mre, v.y, acc.y);
+        acc.y = fmaf(-mim, v.x, acc.y);
+    }
+}
+
+template <int NC, bool I16, bool DAG>
+__global__ void __launch_bounds__(StreamGeom<NC, I16>::THREADS, 1) coarse_apply_stream(StreamParams p) {
+    using Gm = StreamGeom<NC, I16>;
+    constexpr int W = Gm::W, RS = Gm::RS, NB = Gm::NB, WL = Gm::WL, QP = Gm::QP, G = Gm::G, RPL = Gm::RPL;
+    constexpr int PASSES = Gm::PASSES, CPQ = Gm::CPQ, ROWBYTES = Gm::ROWBYTES;
+    constexpr int LINK_STAGE = Gm::LINK_STAGE;
+    constexpr int VEC_STAGE = DAG ? Gm::VEC_STAGE_D : Gm::VEC_STAGE_N;
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int S = p.stages;
+    unsigned char* link_smem = smem;
+    unsigned char* vec_smem = link_smem + (size_t)S * LINK_STAGE;
+    unsigned char* red_smem = vec_smem + (size_t)S * VEC_STAGE;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(red_smem + (DAG ? Gm::RED_BYTES : 0));
+    const uint32_t full0 = ptx::smem_u32(bars);
+    const uint32_t empty0 = full0 + 8u * S;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < S; ++i) {
+            ptx::mbar_init(full0 + 8u * i, 1);
+            ptx::mbar_init(empty0 + 8u * i, W);
+        }
+        ptx::fence_mbar_init();
+    }
+    __syncthreads();
+
+    if (warp == W) {
+        // ------------------------------------------------------------------ producer
+        if (lane != 0) return;
+        const uint64_t pol_links = ptx::policy_evict_first();
+        const uint64_t pol_vec = ptx::policy_evict_last();
+        const uint32_t link_u32 = ptx::smem_u32(link_smem), vec_u32 = ptx::smem_u32(vec_smem);
+        int slot = 0;
+        uint32_t phase = 0;
+        for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+            const int s = DAG ? item : item / NB;
+            const int rb = DAG ? 0 : item % NB;
+            for (int m = 0; m < 9; ++m) {
+                const int sv = stencil_site(p.lat, s, m, DAG ? 1 : 0);
+                const int sm = DAG ? sv : s;
+                const unsigned char* mat = p.links + ((int64_t)sm * 9 + m) * ((int64_t)NC * ROWBYTES);
+                const float2* vec = p.in + (int64_t)sv * NC;
+#pragma unroll 1
+                for (int c = 0; c < (DAG ? NB : 1); ++c) {
+                    const int r0 = DAG ? c * RS : rb * RS;
+                    ptx::mbar_wait(empty0 + 8u * slot, phase ^ 1u);
+                    ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE + VEC_STAGE);
+                    ptx::bulk_g2s(link_u32 + slot * LINK_STAGE, mat + (int64_t)r0 * ROWBYTES, LINK_STAGE,
+                                  full0 + 8u * slot, pol_links);
+                    ptx::bulk_g2s(vec_u32 + slot * VEC_STAGE, DAG ? (vec + r0) : vec, VEC_STAGE,
+                                  full0 + 8u * slot, pol_vec);
+                    if (++slot == S) { slot = 0; phase ^= 1u; }
+                }
+            }
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------------- consumers
+    const int grp = lane / G;          // which of the RPL rows of a warp-wide load
+    const int qi = lane % G;           // quad index inside the pass
+    const bool active = qi < QP;
+    const uint32_t link_u32 = ptx::smem_u32(link_smem), vec_u32 = ptx::smem_u32(vec_smem);
+    int slot = 0;
+    uint32_t phase = 0;
+    int red_parity = 0;
+
+    // int16: lane m (< 9) carries the fp32 scale of matrix m of the current item; the next item's
+    // scales are fetched one item ahead so the global-load latency never sits on the critical path.
+    float cur_scale = 1.f, next_scale = 1.f;
+    auto fetch_scale = [&](int item) -> float {
+        if (!I16 || lane >= 9 || item >= p.n_items) return 1.f;
+        const int s = DAG ? item : item / NB;
+        const int sm = DAG ? stencil_site(p.lat, s, lane, 1) : s;
+        return __ldg(p.scales + (int64_t)sm * 9 + lane);
+    };
+    next_scale = fetch_scale(blockIdx.x);
+
+    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+        const int s = DAG ? item : item / NB;
+        const int rb = DAG ? 0 : item % NB;
+        cur_scale = next_scale;
+        next_scale = fetch_scale(item + gridDim.x);
+
+        if (!DAG) {
+            float2 acc[WL];
+#pragma unroll
+            for (int k = 0; k < WL; ++k) acc[k] = make_float2(0.f, 0.f);
+#pragma unroll 1
+            for (int m = 0; m < 9; ++m) {
+                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                ptx::mbar_wait(full0 + 8u * slot, phase);
+                const uint32_t lbase = link_u32 + slot * LINK_STAGE + qi * 16;
+                const uint32_t vbase = vec_u32 + slot * VEC_STAGE;
+                float2 v[PASSES][CPQ];
+                if (active) {
+#pragma unroll
+                    for (int ps = 0; ps < PASSES; ++ps) {
+                        const int col0 = (ps * QP + qi) * CPQ;
+#pragma unroll
+                        for (int h = 0; h < CPQ / 2; ++h) {
+                            const float4 t = ptx::lds128(vbase + (col0 + 2 * h) * 8);
+                            v[ps][2 * h] = make_float2(t.x, t.y);
+                            v[ps][2 * h + 1] = make_float2(t.z, t.w);
+                        }
+                        if constexpr (I16) {
+#pragma unroll
+                            for (int e = 0; e < CPQ; ++e) { v[ps][e].x *= sc; v[ps][e].y *= sc; }
+                        }
+                    }
+#pragma unroll
+                    for (int k = 0; k < WL; ++k) {
+                        const int rl = (k * W + warp) * RPL + grp;
+#pragma unroll
+                        for (int ps = 0; ps < PASSES; ++ps) {
+                            const uint32_t a = lbase + rl * ROWBYTES + ps * QP * 16;
+                            if constexpr (I16) {
+                                const uint4 t = ptx::lds128u(a);
+                                const float2 m0 = unpack_i16x2(t.x), m1 = unpack_i16x2(t.y);
+                                const float2 m2 = unpack_i16x2(t.z), m3 = unpack_i16x2(t.w);
+                                cmac<false>(acc[k], m0.x, m0.y, v[ps][0]);
+                                cmac<false>(acc[k], m1.x, m1.y, v[ps][1]);
+                                cmac<false>(acc[k], m2.x, m2.y, v[ps][2]);
+                                cmac<false>(acc[k], m3.x, m3.y, v[ps][3]);
+                            } else {
+                                const float4 t = ptx::lds128(a);
+                                cmac<false>(acc[k], t.x, t.y, v[ps][0]);
+                                cmac<false>(acc[k], t.z, t.w, v[ps][1]);
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
+                if (++slot == S) { slot = 0; phase ^= 1u; }
+            }
+            // a6: combine the column-slice partial sums, once per item
+#pragma unroll
+            for (int k = 0; k < WL; ++k) {
+#pragma unroll
+                for (int o = G / 2; o > 0; o >>= 1) {
+                    acc[k].x += __shfl_xor_sync(0xffffffffu, acc[k].x, o);
+                    acc[k].y += __shfl_xor_sync(0xffffffffu, acc[k].y, o);
+                }
+                if (qi == 0) {
+                    const int row = rb * RS + (k * W + warp) * RPL + grp;
+                    p.out[(int64_t)s * NC + row] = acc[k];
+                }
+            }
+        } else {
+            float2 acc[PASSES][CPQ];
+#pragma unroll
+            for (int ps = 0; ps < PASSES; ++ps)
+#pragma unroll
+                for (int e = 0; e < CPQ; ++e) acc[ps][e] = make_float2(0.f, 0.f);
+#pragma unroll 1
+            for (int m = 0; m < 9; ++m) {
+                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+#pragma unroll 1
+                for (int c = 0; c < NB; ++c) {
+                    ptx::mbar_wait(full0 + 8u * slot, phase);
+                    const uint32_t lbase = link_u32 + slot * LINK_STAGE + qi * 16;
+                    const uint32_t vbase = vec_u32 + slot * VEC_STAGE;
+                    if (active) {
+#pragma unroll
+                        for (int k = 0; k < WL; ++k) {
+                            const int rl = (k * W + warp) * RPL + grp;
+                            float2 vj = ptx::lds64(vbase + rl * 8);
+                            if constexpr (I16) { vj.x *= sc; vj.y *= sc; }
+#pragma unroll
+                            for (int ps = 0; ps < PASSES; ++ps) {
+                                const uint32_t a = lbase + rl * ROWBYTES + ps * QP * 16;
+                                if constexpr (I16) {
+                                    const uint4 t = ptx::lds128u(a);
+                                    const float2 m0 = unpack_i16x2(t.x), m1 = unpack_i16x2(t.y);
+                                    const float2 m2 = unpack_i16x2(t.z), m3 = unpack_i16x2(t.w);
+                                    cmac<true>(acc[ps][0], m0.x, m0.y, vj);
+                                    cmac<true>(acc[ps][1], m1.x, m1.y, vj);
+                                    cmac<true>(acc[ps][2], m2.x, m2.y, vj);
+                                    cmac<true>(acc[ps][3], m3.x, m3.y, vj);
+                                } else {
+                                    const float4 t = ptx::lds128(a);
+                                    cmac<true>(acc[ps][0], t.x, t.y, vj);
+                                    cmac<true>(acc[ps][1], t.z, t.w, vj);
+                                }
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
+                    if (++slot == S) { slot = 0; phase ^= 1u; }
+                }
+            }
+            // a6: combine the row-slice partial sums (W warps x RPL row groups), once per item
+            float2* red = reinterpret_cast<float2*>(red_smem) + red_parity * (W * RPL * NC);
+            if (active) {
+#pragma unroll
+                for (int ps = 0; ps < PASSES; ++ps)
+#pragma unroll
+                    for (int e = 0; e < CPQ; ++e)
+                        red[(warp * RPL + grp) * NC + (ps * QP + qi) * CPQ + e] = acc[ps][e];
+            }
+            ptx::named_bar_sync(1, W * 32);
+            for (int t = threadIdx.x; t < NC; t += W * 32) {
+                float2 sum = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int g = 0; g < W * RPL; ++g) {
+                    const float2 x = red[g * NC + t];
+                    sum.x += x.x;
+                    sum.y += x.y;
+                }
+                p.out[(int64_t)s * NC + t] = sum;
+            }
+            red_parity ^= 1;
+        }
+    }
+}
+
+}  // namespace coarse

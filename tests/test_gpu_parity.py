@@ -1,0 +1,189 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerance (BASELINE.json north_star, written here as asked): relative L2 error per output vector
+<= 1e-5 for complex64 links, and <= 1e-5 against the oracle run on the SAME int16 + scale arrays
+(i.e. on the dequantised links) for int16 storage.  The quantiser is integer work: bit-exact.
+"""
+import numpy as np
+import pytest
+import torch
+
+import synth
+import paper_2212_12559_b200 as cop
+from tests.helpers import rel_l2, rel_l2_per_rhs
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_cuda():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests selected but no CUDA device is visible (there is no CPU fallback)")
+    torch.cuda.set_device(0)
+
+
+def _links_for(dims, Nc, prec, seed, hermitian, oracle_lib):
+    """Returns (device link tensor, device scales or None, host links for the oracle, host scales)."""
+    gen = synth.make_gamma_hermitian_links if hermitian else synth.make_arbitrary_links
+    links = gen(dims, Nc, seed, device="cuda")
+    if prec == cop.LINK_C64:
+        return links, None, links.cpu().numpy(), None
+    V = synth.lattice_volume(dims)
+    q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+    sc = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+    cop.coarse_op_quantize_i16(links, Nc, q, sc)
+    torch.cuda.synchronize()
+    # the integers handed to BOTH sides come from the oracle's quantiser; the CUDA quantiser
+    # must reproduce them bit for bit (checked here on every int16 case)
+    q_ref, sc_ref = oracle_lib.quantize_i16(links.cpu().numpy(), Nc)
+    assert np.array_equal(sc.cpu().numpy().reshape(-1), sc_ref)
+    assert np.array_equal(q.cpu().numpy().reshape(q_ref.shape), q_ref)
+    return q, sc, q_ref.reshape(V, 9, Nc, Nc, 2), sc_ref
+
+
+def _run(oracle_lib, dims, Nc, prec, nrhs, dagger, path, seed=1234, hermitian=True, grid=0):
+    V = synth.lattice_volume(dims)
+    links, scales, links_h, scales_h = _links_for(dims, Nc, prec, seed, hermitian, oracle_lib)
+    vin = synth.make_vectors(dims, Nc, nrhs, seed + 1, device="cuda")
+    vout = torch.full((V, Nc, nrhs), float("nan"), dtype=torch.complex64, device="cuda")
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    op.set_option(cop.OPT_PATH, path)
+    if grid:
+        op.set_option(cop.OPT_GRID, grid)
+    op.apply(vin, vout, nrhs=nrhs, dagger=dagger)
+    torch.cuda.synchronize()
+    assert op.last_launches >= 1
+    if path != cop.PATH_AUTO:
+        assert op.last_path == path
+    got = vout.cpu().numpy()
+    ref = oracle_lib.coarse_apply(dims, Nc, links_h, vin.cpu().numpy(), nrhs=nrhs, dagger=dagger,
+                                  link_precision=prec, scales=scales_h)
+    assert np.isfinite(got.view(np.float32)).all()
+    err = rel_l2_per_rhs(got, ref)
+    assert err <= TOL, f"rel-L2 {err:.3e} > {TOL} for dims={dims} Nc={Nc} prec={prec} nrhs={nrhs} dagger={dagger} path={path}"
+    op.close()
+    return err
+
+
+SMALL_LATTICES = [(4, 4, 4, 4), (3, 2, 1, 4), (2, 2, 2, 2), (1, 1, 1, 1), (5, 3, 4, 7)]
+
+
+@pytest.mark.parametrize("dims", SMALL_LATTICES)
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_stream_path_single_rhs(oracle_lib, dims, Nc, prec, dagger):
+    if Nc >= 128 and dims == (5, 3, 4, 7):
+        dims = (5, 3, 2, 3)               # keep the oracle's run time in seconds
+    _run(oracle_lib, dims, Nc, prec, 1, dagger, cop.PATH_STREAM)
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (1, 1, 1, 1)])
+@pytest.mark.parametrize("Nc", [6, 8, 48, 64])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("nrhs", [1, 3, 16])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_simple_path(oracle_lib, dims, Nc, prec, nrhs, dagger):
+    _run(oracle_lib, dims, Nc, prec, nrhs, dagger, cop.PATH_SIMPLE)
+
+
+@pytest.mark.parametrize("dagger", [0, 1])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+def test_arbitrary_links_not_gamma_hermitian(oracle_lib, prec, dagger):
+    """The dagger must be the true adjoint for ANY links (no Gamma shortcut in the library)."""
+    _run(oracle_lib, (3, 4, 2, 5), 48, prec, 1, dagger, cop.PATH_STREAM, hermitian=False)
+    _run(oracle_lib, (3, 4, 2, 5), 128, prec, 1, dagger, cop.PATH_STREAM, hermitian=False)
+
+
+@pytest.mark.parametrize("grid", [1, 7, 148, 1000])
+def test_stream_path_any_grid(oracle_lib, grid):
+    """Several items per CTA, a ragged tail, and more CTAs than items."""
+    for dagger in (0, 1):
+        _run(oracle_lib, (5, 3, 4, 7), 48, cop.LINK_C64, 1, dagger, cop.PATH_STREAM, grid=grid)
+        _run(oracle_lib, (3, 3, 2, 2), 128, cop.LINK_I16, 1, dagger, cop.PATH_STREAM, grid=grid)
+
+
+def test_bit_reproducible():
+    dims, Nc = (4, 4, 4, 6), 64
+    links = synth.make_gamma_hermitian_links(dims, Nc, 5, device="cuda")
+    vin = synth.make_vectors(dims, Nc, 1, 6, device="cuda")
+    op = cop.CoarseOp(dims, Nc).set_links(links)
+    outs = []
+    for _ in range(3):
+        vout = torch.empty_like(vin)
+        op.apply(vin, vout)
+        torch.cuda.synchronize()
+        outs.append(vout.clone())
+    assert torch.equal(torch.view_as_real(outs[0]), torch.view_as_real(outs[1]))
+    assert torch.equal(torch.view_as_real(outs[0]), torch.view_as_real(outs[2]))
+
+
+def test_apply_host_matches_device_apply(oracle_lib):
+    dims, Nc = (4, 3, 2, 5), 48
+    V = synth.lattice_volume(dims)
+    links = synth.make_gamma_hermitian_links(dims, Nc, 8, device="cuda")
+    vin = synth.make_vectors(dims, Nc, 1, 9, device="cpu").pin_memory()
+    vout = torch.empty((V, Nc, 1), dtype=torch.complex64).pin_memory()
+    op = cop.CoarseOp(dims, Nc).set_links(links)
+    for dagger in (0, 1):
+        op.apply_host(vin, vout, dagger=dagger)
+        ref = oracle_lib.coarse_apply(dims, Nc, links.cpu().numpy(), vin.numpy(), dagger=dagger)
+        assert rel_l2_per_rhs(vout.numpy(), ref) <= TOL
+
+
+# ------------------------------------------------------------------ ABI behaviour
+def test_error_codes():
+    dims, Nc = (2, 2, 2, 2), 48
+    V = 16
+    with pytest.raises(cop.CoarseOpError):
+        cop.coarse_op_create((2, 2, 0, 2), Nc, cop.LINK_C64)
+    with pytest.raises(cop.CoarseOpError):
+        cop.coarse_op_create(dims, 7, cop.LINK_C64)
+    with pytest.raises(cop.CoarseOpError):
+        cop.coarse_op_create(dims, Nc, 5)
+    h = cop.coarse_op_create(dims, Nc, cop.LINK_C64)
+    assert cop.coarse_op_link_bytes(h) == V * 9 * Nc * Nc * 8
+    assert cop.coarse_op_scale_bytes(h) == 0
+    assert cop.coarse_op_vector_bytes(h, 3) == V * Nc * 3 * 8
+    vin = torch.zeros((V, Nc, 1), dtype=torch.complex64, device="cuda")
+    vout = torch.zeros_like(vin)
+    L = cop.lib()
+    assert L.coarse_op_apply(h, vin.data_ptr(), vout.data_ptr(), 1, 0, None) == cop.ENOTREADY
+    links = torch.zeros((V, 9, Nc, Nc), dtype=torch.complex64, device="cuda")
+    assert L.coarse_op_set_links(h, links.data_ptr(), vin.data_ptr()) == cop.EINVAL      # scales with C64
+    assert L.coarse_op_set_links(h, links.data_ptr() + 8, None) == cop.EINVAL            # misaligned
+    assert L.coarse_op_set_links(h, links.data_ptr(), None) == cop.OK
+    assert L.coarse_op_apply(h, vin.data_ptr(), vin.data_ptr(), 1, 0, None) == cop.EINVAL      # overlap
+    assert L.coarse_op_apply(h, vin.data_ptr(), vout.data_ptr(), 0, 0, None) == cop.EINVAL     # nrhs
+    assert L.coarse_op_apply(h, vin.data_ptr(), vout.data_ptr(), 1, 2, None) == cop.EINVAL     # dagger
+    assert L.coarse_op_apply(h, None, vout.data_ptr(), 1, 0, None) == cop.EINVAL
+    assert "dagger" in cop.coarse_op_last_error() or "NULL" in cop.coarse_op_last_error()
+    assert L.coarse_op_set_option(h, cop.OPT_PATH, 99) == cop.EINVAL
+    assert L.coarse_op_apply(h, vin.data_ptr(), vout.data_ptr(), 1, 0, None) == cop.OK
+    cop.coarse_op_destroy(h)
+    cop.coarse_op_destroy(0)
+    h16 = cop.coarse_op_create(dims, Nc, cop.LINK_I16)
+    assert cop.coarse_op_link_bytes(h16) == V * 9 * Nc * Nc * 4
+    assert cop.coarse_op_scale_bytes(h16) == V * 9 * 4
+    assert L.coarse_op_set_links(h16, links.data_ptr(), None) == cop.EINVAL              # I16 needs scales
+    cop.coarse_op_destroy(h16)
+    h6 = cop.coarse_op_create(dims, 6, cop.LINK_C64)
+    assert L.coarse_op_set_option(h6, cop.OPT_PATH, cop.PATH_STREAM) == cop.EUNSUPPORTED
+    cop.coarse_op_destroy(h6)
+
+
+def test_quantiser_edge_cases_bit_exact(oracle_lib):
+    Nc = 16
+    links = synth.make_gamma_hermitian_links((2, 2, 1, 2), Nc, 77, device="cuda")
+    links[1, 3] = 0
+    links[2, 5] *= 1e-30
+    links[3, 0, 0, 0] = 1e30
+    q = torch.empty(links.shape + (2,), dtype=torch.int16, device="cuda")
+    sc = torch.empty(links.shape[:2], dtype=torch.float32, device="cuda")
+    cop.coarse_op_quantize_i16(links, Nc, q, sc)
+    torch.cuda.synchronize()
+    q_ref, sc_ref = oracle_lib.quantize_i16(links.cpu().numpy(), Nc)
+    assert np.array_equal(sc.cpu().numpy().reshape(-1), sc_ref)
+    assert np.array_equal(q.cpu().numpy().reshape(q_ref.shape), q_ref)
