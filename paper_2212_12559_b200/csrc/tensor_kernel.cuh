@@ -23,7 +23,7 @@
 //                           bytes cross shared memory exactly twice (TMA write + one LDS read);
 //                           build B hi/lo in shared memory in the canonical K-major UMMA layout.
 //   MMA issuer (1 thread)   tcgen05.mma kind::tf32, A from TMEM, B from smem, D (128 x 2nrhs fp32)
-//                           in TMEM, 12 MMAs (4 k-steps x 3 split terms) per stage, one accumulator
+//                           in TMEM, 8 MMAs per stage (4 k-steps x {A_hi.[B_hi|B_lo], A_lo.B_hi}), one accumulator
 //                           slot per link matrix; tcgen05.commit releases the operand slot / publishes D.
 //   epilogue (4 warps)      tcgen05.ld D -> registers, adds the nine per-matrix partial results in
 //                           round-to-nearest fp32 -> out[s][i][r]; a ring of 4 accumulator slots lets
@@ -116,6 +116,7 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
         : "r"(taddr)
         : "memory");
 }
+__device__ __forceinline__ void fence_cta() { asm volatile("fence.acq_rel.cta;" ::: "memory"); }
 __device__ __forceinline__ void sts64(uint32_t addr, float a, float b) {
     asm volatile("st.shared.v2.f32 [%0], {%1,%2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
 }
@@ -149,6 +150,8 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
     constexpr int STAGES_PER_SITE = 9 * CHUNKS;
     // instruction descriptor: D fp32, A/B tf32, both K-major, N, M = 128
     constexpr uint32_t IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
+    constexpr uint32_t IDESC2 = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(2 * N >> 3) << 17) | ((128u >> 4) << 24);
+    static_assert(B_HALF == (N / 8) * B_SBO, "B lo must continue B hi's n groups");
 
     extern __shared__ unsigned char smem_raw[];
     const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -240,15 +243,14 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
                     ptx::mbar_wait(abfull0 + 8u * as, aph);
                     ptx::tc_fence_after();
                     const uint32_t a_hi = tmem_base + as * Gm::A_COLS, a_lo = a_hi + Gm::KSTAGE;
-                    const uint32_t b_hi = b_u32 + as * 2 * B_HALF, b_lo = b_hi + B_HALF;
+                    const uint32_t b_hi = b_u32 + as * 2 * B_HALF;
 #pragma unroll
                     for (int kk = 0; kk < Gm::KSTAGE / 8; ++kk) {
+                        // B hi and B lo are adjacent 8-wide n groups of one K-major tile, so
+                        // A_hi . [B_hi | B_lo] is ONE N = 2N MMA writing [main | small]
                         const uint64_t dbh = umma_desc_kmajor(b_hi + kk * 256, 128, B_SBO);
-                        const uint64_t dbl = umma_desc_kmajor(b_lo + kk * 256, 128, B_SBO);
-                        const uint32_t first = (c | kk) != 0 ? 1u : 0u;
-                        ptx::mma_tf32_ts(d_small, a_lo + kk * 8, dbh, IDESC, first);
-                        ptx::mma_tf32_ts(d_small, a_hi + kk * 8, dbl, IDESC, 1u);
-                        ptx::mma_tf32_ts(d_main, a_hi + kk * 8, dbh, IDESC, first);
+                        ptx::mma_tf32_ts(d_main, a_hi + kk * 8, dbh, IDESC2, (c | kk) != 0 ? 1u : 0u);
+                        ptx::mma_tf32_ts(d_small, a_lo + kk * 8, dbh, IDESC, 1u);
                     }
                     ptx::tc_commit(abempty0 + 8u * as);
                 }
@@ -291,8 +293,14 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
             float2 v[NRHS / 8];
 #pragma unroll
             for (int x = 0; x < NRHS / 8; ++x) v[x] = ptx::lds64(vec_u32 + slot * VEC_STAGE + (gtid + 128 * x) * 8);
+#ifndef COARSE_EXP_LATE_RELEASE
+            // The loaded values are not consumed before the release below, and SYNCS.ARRIVE does not wait
+            // for in-flight LDS: without this fence the producer's next TMA write into the slot can overtake
+            // the reads (seen on B200 as sporadic stale 512-byte runs).  The fence completes the loads.
+            ptx::fence_cta();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);      // link slot back to the producer
+#endif
 
             ptx::mbar_wait(abempty0 + 8u * as, aph ^ 1u);            // MMAs that read this operand slot are done
             ptx::tc_fence_after();
@@ -331,6 +339,9 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(abfull0 + 8u * as);
+#ifdef COARSE_EXP_LATE_RELEASE
+            if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
+#endif
         }
     } else if (warp >= 12) {
         // ---------------------------------------------------------------- epilogue

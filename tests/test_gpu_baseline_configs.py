@@ -88,6 +88,8 @@ def test_baseline_config_parity(oracle_lib, name):
         outs[dagger] = vout
     if nrhs == 1:
         assert op.last_path == cop.PATH_STREAM          # the configuration bench.py times
+    else:
+        assert op.last_path == cop.PATH_TENSOR          # C5: block apply on the tensor cores
 
     work = V * 9.0 * Nc * Nc * nrhs
     vin_h = vin.cpu().numpy()

@@ -89,6 +89,59 @@ def test_simple_path(oracle_lib, dims, Nc, prec, nrhs, dagger):
     _run(oracle_lib, dims, Nc, prec, nrhs, dagger, cop.PATH_SIMPLE)
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (2, 2, 2, 2), (1, 1, 1, 1), (5, 3, 2, 3)])
+@pytest.mark.parametrize("Nc", [48, 64, 128])
+@pytest.mark.parametrize("nrhs", [8, 16])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_tensor_path_block_apply(oracle_lib, dims, Nc, nrhs, dagger):
+    """tcgen05 3xTF32 block apply: same 1e-5 bound as the CUDA-core paths (north_star (4))."""
+    err = _run(oracle_lib, dims, Nc, cop.LINK_C64, nrhs, dagger, cop.PATH_TENSOR)
+    assert err <= 3e-6, f"3xTF32 with per-matrix accumulator chains should sit near 1e-6, got {err:.2e}"
+
+
+@pytest.mark.parametrize("grid", [1, 7, 1000])
+def test_tensor_path_any_grid(oracle_lib, grid):
+    """Several sites per CTA (accumulator/operand rings wrap many times), ragged tail, idle CTAs."""
+    for dagger in (0, 1):
+        _run(oracle_lib, (5, 3, 2, 3), 128, cop.LINK_C64, 16, dagger, cop.PATH_TENSOR, grid=grid)
+        _run(oracle_lib, (5, 3, 4, 7), 48, cop.LINK_C64, 8, dagger, cop.PATH_TENSOR, grid=grid, hermitian=False)
+
+
+def test_tensor_path_matches_cuda_core_path_and_is_reproducible():
+    dims, Nc, nrhs = (4, 3, 2, 5), 128, 16
+    links = synth.make_arbitrary_links(dims, Nc, 21, device="cuda")
+    vin = synth.make_vectors(dims, Nc, nrhs, 22, device="cuda")
+    op = cop.CoarseOp(dims, Nc).set_links(links)
+    outs = {}
+    for path in (cop.PATH_SIMPLE, cop.PATH_TENSOR, cop.PATH_TENSOR):
+        op.set_option(cop.OPT_PATH, path)
+        vout = torch.empty_like(vin)
+        op.apply(vin, vout, nrhs=nrhs, dagger=1)
+        torch.cuda.synchronize()
+        outs.setdefault(path, []).append(vout)
+    a, b = outs[cop.PATH_TENSOR]
+    assert torch.equal(torch.view_as_real(a), torch.view_as_real(b))
+    ref = outs[cop.PATH_SIMPLE][0].cpu().numpy()
+    assert rel_l2_per_rhs(a.cpu().numpy(), ref) <= 3e-6
+    op.close()
+
+
+def test_tensor_path_unsupported_shapes():
+    L = cop.lib()
+    h = cop.coarse_op_create((2, 2, 2, 2), 128, cop.LINK_I16)
+    assert L.coarse_op_set_option(h, cop.OPT_PATH, cop.PATH_TENSOR) == cop.EUNSUPPORTED
+    cop.coarse_op_destroy(h)
+    dims, Nc = (2, 2, 2, 2), 64
+    links = synth.make_arbitrary_links(dims, Nc, 3, device="cuda")
+    vin = synth.make_vectors(dims, Nc, 3, 4, device="cuda")
+    vout = torch.empty_like(vin)
+    op = cop.CoarseOp(dims, Nc).set_links(links).set_option(cop.OPT_PATH, cop.PATH_TENSOR)
+    with pytest.raises(cop.CoarseOpError) as e:
+        op.apply(vin, vout, nrhs=3)
+    assert e.value.code == cop.EUNSUPPORTED
+    op.close()
+
+
 @pytest.mark.parametrize("dagger", [0, 1])
 @pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
 def test_arbitrary_links_not_gamma_hermitian(oracle_lib, prec, dagger):
