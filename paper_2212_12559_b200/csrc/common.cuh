@@ -32,6 +32,41 @@ __device__ __forceinline__ int stencil_site(const Lat& lat, int s, int m, int da
     return s + (xn - x) * stride;
 }
 
+// The same neighbour with the site's coordinates already known (one set of divisions per ITEM
+// instead of two per pipeline stage: the TMA producer is a single thread and its instruction
+// latency, not HBM, was what capped the int16 path).  m is a compile-time constant at every call
+// site, so x[mu] and the stride fold into registers.
+struct SiteX {
+    int x0, x1, x2, x3;
+    int st1, st2, st3;   // strides L0, L0*L1, L0*L1*L2
+};
+__device__ __forceinline__ SiteX site_coords(const Lat& lat, int s) {
+    SiteX c;
+    c.st1 = lat.L[0];
+    c.st2 = lat.L[0] * lat.L[1];
+    c.st3 = c.st2 * lat.L[2];
+    const unsigned us = (unsigned)s;
+    const unsigned q1 = us / (unsigned)lat.L[0];
+    c.x0 = (int)(us - q1 * (unsigned)lat.L[0]);
+    const unsigned q2 = q1 / (unsigned)lat.L[1];
+    c.x1 = (int)(q1 - q2 * (unsigned)lat.L[1]);
+    const unsigned q3 = q2 / (unsigned)lat.L[2];
+    c.x2 = (int)(q2 - q3 * (unsigned)lat.L[2]);
+    c.x3 = (int)q3;
+    return c;
+}
+__device__ __forceinline__ int stencil_site_x(const Lat& lat, int s, const SiteX& c, int m, int dagger) {
+    if (m == 0) return s;
+    const int mu = (m - 1) & 3;
+    bool fwd = (m <= 4);
+    if (dagger) fwd = !fwd;
+    const int x = mu == 0 ? c.x0 : mu == 1 ? c.x1 : mu == 2 ? c.x2 : c.x3;
+    const int Lmu = mu == 0 ? lat.L[0] : mu == 1 ? lat.L[1] : mu == 2 ? lat.L[2] : lat.L[3];
+    const int stride = mu == 0 ? 1 : mu == 1 ? c.st1 : mu == 2 ? c.st2 : c.st3;
+    if (fwd) return (x + 1 == Lmu) ? s - x * stride : s + stride;
+    return (x == 0) ? s + (Lmu - 1) * stride : s - stride;
+}
+
 namespace ptx {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -86,6 +121,15 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
         ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy)
         : "memory");
 }
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
@@ -107,9 +151,18 @@ __device__ __forceinline__ float2 lds64(uint32_t addr) {
 
 }  // namespace ptx
 
-// int16 (re,im) packed in one 32-bit word -> two floats (exact).
+// int16 (re,im) packed in one 32-bit word -> two floats (exact), without the int->float
+// conversion instruction: I2F issues on the quarter-rate XU pipe, and at HBM rate the int16 path
+// needs ~13 conversions per clock per SM of the 16 that pipe can do (ncu: XU 70 % busy, the
+// limiter of config C4).  Instead: q ^ 0x8000 = q + 32768 as an unsigned 16-bit number u; placing
+// u in the low mantissa bits of 2^23 gives the float 2^23 + u exactly; subtracting 2^23 + 32768
+// (exact: all three are integers below 2^24) leaves q.  One LOP3 per word, one PRMT and one FADD
+// per value, all on the full-rate ALU/FMA pipes.
 __device__ __forceinline__ float2 unpack_i16x2(uint32_t w) {
-    return make_float2((float)(short)(w & 0xffffu), (float)(short)(w >> 16));
+    const uint32_t u = w ^ 0x80008000u;
+    const uint32_t lo = __byte_perm(u, 0x4B000000u, 0x7610);
+    const uint32_t hi = __byte_perm(u, 0x4B000000u, 0x7632);
+    return make_float2(__uint_as_float(lo) - 8421376.0f, __uint_as_float(hi) - 8421376.0f);
 }
 
 }  // namespace coarse

@@ -126,7 +126,8 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16>::THREADS, 1) coarse_apply_
 
     if (warp == W) {
         // ------------------------------------------------------------------ producer
-        if (lane != 0) return;
+        // The whole warp walks the loop (uniform control flow, so the bulk copies are not wrapped
+        // in per-lane replay loops) and one elected lane issues the copies.
         const uint64_t pol_links = ptx::policy_evict_first();
         const uint64_t pol_vec = ptx::policy_evict_last();
         const uint32_t link_u32 = ptx::smem_u32(link_smem), vec_u32 = ptx::smem_u32(vec_smem);
@@ -135,8 +136,10 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16>::THREADS, 1) coarse_apply_
         for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
             const int s = DAG ? item : item / NB;
             const int rb = DAG ? 0 : item % NB;
+            const SiteX cx = site_coords(p.lat, s);
+#pragma unroll
             for (int m = 0; m < 9; ++m) {
-                const int sv = stencil_site(p.lat, s, m, DAG ? 1 : 0);
+                const int sv = stencil_site_x(p.lat, s, cx, m, DAG ? 1 : 0);
                 const int sm = DAG ? sv : s;
                 const unsigned char* mat = p.links + ((int64_t)sm * 9 + m) * ((int64_t)NC * ROWBYTES);
                 const float2* vec = p.in + (int64_t)sv * NC;
@@ -144,11 +147,14 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16>::THREADS, 1) coarse_apply_
                 for (int c = 0; c < (DAG ? NB : 1); ++c) {
                     const int r0 = DAG ? c * RS : rb * RS;
                     ptx::mbar_wait(empty0 + 8u * slot, phase ^ 1u);
-                    ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE + VEC_STAGE);
-                    ptx::bulk_g2s(link_u32 + slot * LINK_STAGE, mat + (int64_t)r0 * ROWBYTES, LINK_STAGE,
-                                  full0 + 8u * slot, pol_links);
-                    ptx::bulk_g2s(vec_u32 + slot * VEC_STAGE, DAG ? (vec + r0) : vec, VEC_STAGE,
-                                  full0 + 8u * slot, pol_vec);
+                    if (ptx::elect_one()) {
+                        ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE + VEC_STAGE);
+                        ptx::bulk_g2s(link_u32 + slot * LINK_STAGE, mat + (int64_t)r0 * ROWBYTES, LINK_STAGE,
+                                      full0 + 8u * slot, pol_links);
+                        ptx::bulk_g2s(vec_u32 + slot * VEC_STAGE, DAG ? (vec + r0) : vec, VEC_STAGE,
+                                      full0 + 8u * slot, pol_vec);
+                    }
+                    __syncwarp();
                     if (++slot == S) { slot = 0; phase ^= 1u; }
                 }
             }

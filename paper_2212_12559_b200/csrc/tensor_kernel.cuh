@@ -192,21 +192,24 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
 
     if (warp == 0) {
         // ---------------------------------------------------------------- TMA producer
-        if (lane == 0) {
-            const uint64_t pol_links = ptx::policy_evict_first();
-            const uint64_t pol_vec = ptx::policy_evict_last();
-            uint32_t t = 0;
-            for (int it = 0; it < n_my; ++it) {
-                const int s = blockIdx.x + it * gridDim.x;
-                for (int m = 0; m < 9; ++m) {
-                    const int sv = stencil_site(p.lat, s, m, DAG ? 1 : 0);
-                    const int sm = DAG ? sv : s;
-                    const int64_t mat_row0 = ((int64_t)sm * 9 + m) * NC;
-                    const float2* vec = p.in + (int64_t)sv * NC * NRHS;
+        // (whole warp in uniform control flow, one elected lane issues: see the MMA issuer below)
+        const uint64_t pol_links = ptx::policy_evict_first();
+        const uint64_t pol_vec = ptx::policy_evict_last();
+        uint32_t t = 0;
+        for (int it = 0; it < n_my; ++it) {
+            const int s = blockIdx.x + it * gridDim.x;
+            const SiteX cx = site_coords(p.lat, s);
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const int sv = stencil_site_x(p.lat, s, cx, m, DAG ? 1 : 0);
+                const int sm = DAG ? sv : s;
+                const int64_t mat_row0 = ((int64_t)sm * 9 + m) * NC;
+                const float2* vec = p.in + (int64_t)sv * NC * NRHS;
 #pragma unroll 1
-                    for (int c = 0; c < CHUNKS; ++c, ++t) {
-                        const uint32_t slot = t % LS, ph = (t / LS) & 1u;
-                        ptx::mbar_wait(empty0 + 8u * slot, ph ^ 1u);
+                for (int c = 0; c < CHUNKS; ++c, ++t) {
+                    const uint32_t slot = t % LS, ph = (t / LS) & 1u;
+                    ptx::mbar_wait(empty0 + 8u * slot, ph ^ 1u);
+                    if (ptx::elect_one()) {
                         ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE + VEC_STAGE);
                         if (!DAG) {
                             ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, c * 32, (int)mat_row0,
@@ -219,42 +222,49 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
                         ptx::bulk_g2s(vec_u32 + slot * VEC_STAGE, vec + (int64_t)16 * c * NRHS, VEC_STAGE,
                                       full0 + 8u * slot, pol_vec);
                     }
+                    __syncwarp();
                 }
             }
         }
     } else if (warp == 1) {
         // ---------------------------------------------------------------- MMA issuer
-        if (lane == 0) {
-            // One accumulator slot per link matrix: the tensor core truncates (rounds toward zero) when it
-            // adds into the fp32 accumulator, a bias that grows linearly with the chain length, so the
-            // chains are kept short (32 MMAs for hi.hi, 64 for the two cross terms, which are 2^-11
-            // smaller and live in their own columns) and the nine partial results are added with
-            // round-to-nearest fp32 in the epilogue.
-            uint32_t t = 0;
-            const uint32_t n_mat = (uint32_t)n_my * 9u;
-            for (uint32_t tm = 0; tm < n_mat; ++tm) {
-                const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
-                ptx::mbar_wait(dempty0 + 8u * ds, dph ^ 1u);
-                ptx::tc_fence_after();
-                const uint32_t d_main = tmem_base + Gm::D_COL0 + ds * Gm::D_COLS, d_small = d_main + N;
+        // The whole warp walks the loop (uniform control flow) and ONE elected lane issues the MMAs:
+        // tcgen05.mma/commit read uniform registers, and inside a divergent `if (lane == 0)` the
+        // compiler wraps every one of them in a per-lane replay loop (~100 issue cycles per MMA,
+        // which made this warp the bottleneck of the kernel; profiles/r01_ncu_full_c5_tensor.md).
+        //
+        // One accumulator slot per link matrix: the tensor core truncates (rounds toward zero) when it
+        // adds into the fp32 accumulator, a bias that grows linearly with the chain length, so the
+        // chains are kept short (32 MMAs for hi.hi, 64 for the two cross terms, which are 2^-11
+        // smaller and live in their own columns) and the nine partial results are added with
+        // round-to-nearest fp32 in the epilogue.
+        uint32_t t = 0;
+        const uint32_t n_mat = (uint32_t)n_my * 9u;
+        for (uint32_t tm = 0; tm < n_mat; ++tm) {
+            const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
+            ptx::mbar_wait(dempty0 + 8u * ds, dph ^ 1u);
+            ptx::tc_fence_after();
+            const uint32_t d_main = tmem_base + Gm::D_COL0 + ds * Gm::D_COLS, d_small = d_main + N;
 #pragma unroll 1
-                for (int c = 0; c < CHUNKS; ++c, ++t) {
-                    const uint32_t as = t % AS, aph = (t / AS) & 1u;
-                    ptx::mbar_wait(abfull0 + 8u * as, aph);
-                    ptx::tc_fence_after();
+            for (int c = 0; c < CHUNKS; ++c, ++t) {
+                const uint32_t as = t % AS, aph = (t / AS) & 1u;
+                ptx::mbar_wait(abfull0 + 8u * as, aph);
+                ptx::tc_fence_after();
+                if (ptx::elect_one()) {
                     const uint32_t a_hi = tmem_base + as * Gm::A_COLS, a_lo = a_hi + Gm::KSTAGE;
-                    const uint32_t b_hi = b_u32 + as * 2 * B_HALF;
+                    // B hi and B lo are adjacent 8-wide n groups of one K-major tile, so
+                    // A_hi . [B_hi | B_lo] is ONE N = 2N MMA writing [main | small]
+                    const uint64_t dbh0 = umma_desc_kmajor(b_u32 + as * 2 * B_HALF, 128, B_SBO);
 #pragma unroll
                     for (int kk = 0; kk < Gm::KSTAGE / 8; ++kk) {
-                        // B hi and B lo are adjacent 8-wide n groups of one K-major tile, so
-                        // A_hi . [B_hi | B_lo] is ONE N = 2N MMA writing [main | small]
-                        const uint64_t dbh = umma_desc_kmajor(b_hi + kk * 256, 128, B_SBO);
+                        const uint64_t dbh = dbh0 + (uint64_t)(kk * 256 >> 4);
                         ptx::mma_tf32_ts(d_main, a_hi + kk * 8, dbh, IDESC2, (c | kk) != 0 ? 1u : 0u);
                         ptx::mma_tf32_ts(d_small, a_lo + kk * 8, dbh, IDESC, 1u);
                     }
                     ptx::tc_commit(abempty0 + 8u * as);
+                    if (c == CHUNKS - 1) ptx::tc_commit(dfull0 + 8u * ds);
                 }
-                ptx::tc_commit(dfull0 + 8u * ds);
+                __syncwarp();
             }
         }
     } else if (warp >= 4 && warp < 12) {
