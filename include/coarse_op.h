@@ -76,7 +76,10 @@ enum {
 
 enum {
     COARSE_OPT_PATH = 0,     /* one of COARSE_PATH_*                                              */
-    COARSE_OPT_GRID = 1      /* persistent grid size for STREAM/TENSOR; 0 = one CTA per SM        */
+    COARSE_OPT_GRID = 1,     /* persistent grid size for STREAM/TENSOR; 0 = one CTA per SM        */
+    COARSE_OPT_STAGES = 2,   /* cap on the STREAM shared-memory ring depth; 0 = library default   */
+    COARSE_OPT_FINE = 3,     /* STREAM dagger=0 small-lattice row-block split: 0 auto, 1 never, 2 always */
+    COARSE_OPT_KEEP_LINKS = 4 /* L2 policy of the link stream: 0 auto (keep if links <= L2/2), 1 evict_first, 2 keep */
 };
 
 /* Create an operator descriptor for a periodic lattice dims[0..3] (each >= 1), Nc even and

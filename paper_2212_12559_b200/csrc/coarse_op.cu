@@ -48,6 +48,10 @@ struct coarse_op {
     const float* scales;
     int path_opt;
     int grid_opt;
+    int stages_opt;
+    int fine_opt;
+    int keep_opt;
+    int l2_bytes;
     int last_launches;
     int last_path;
     int device;
@@ -63,18 +67,24 @@ struct coarse_op {
 namespace {
 
 // ---------------------------------------------------------------- STREAM dispatch
-template <int NC, bool I16, bool DAG>
+template <int NC, bool I16, bool DAG, bool FINE>
 int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
-    using Gm = StreamGeom<NC, I16>;
+    using Gm = StreamGeom<NC, I16, FINE>;
     static_assert(Gm::OK, "unsupported STREAM geometry");
     StreamParams p = base;
     p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
     int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (Gm::stage_bytes(DAG) + 16);
     if (stages > 12) stages = 12;
     if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM: shared memory too small for Nc=%d", NC);
+    // Default depth: ~112 KB in flight per SM (the measured optimum, see stream_kernel.cuh), at
+    // least 4 stages; COARSE_OPT_STAGES overrides.
+    int want = (114688 + Gm::stage_bytes(DAG) / 2) / Gm::stage_bytes(DAG);
+    if (want < 4) want = 4;
+    if (op->stages_opt > 0) want = op->stages_opt;
+    if (stages > want) stages = want;
     p.stages = stages;
     const int smem = Gm::smem_bytes(DAG, stages);
-    auto kern = coarse_apply_stream<NC, I16, DAG>;
+    auto kern = coarse_apply_stream<NC, I16, DAG, FINE>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
@@ -85,11 +95,26 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     return COARSE_OK;
 }
 
+// dagger = 0 on a tiny lattice: switch to the fine row-block geometry when the regular one gives
+// fewer work items than SMs (COARSE_OPT_FINE: 0 auto, 1 never, 2 always).  Measured on C1
+// (256 sites, Nc = 48: 256 regular items on 148 SMs) the regular geometry is 2.8x faster (5.6 us
+// vs 15.4 us warm): 3 KB stages pay the per-stage handshake 6x more often, so the fine split only
+// pays when SMs would otherwise sit idle.
+template <int NC, bool I16>
+int launch_stream_n(const coarse_op* op, const StreamParams& p, cudaStream_t stream) {
+    constexpr bool HAS_FINE = StreamGeom<NC, I16, true>::NB > StreamGeom<NC, I16, false>::NB;
+    if constexpr (HAS_FINE) {
+        const bool few = (int64_t)op->lat.V * StreamGeom<NC, I16, false>::NB < (int64_t)op->num_sms;
+        if (op->fine_opt == 2 || (op->fine_opt == 0 && few)) return launch_stream_t<NC, I16, false, true>(op, p, stream);
+    }
+    return launch_stream_t<NC, I16, false, false>(op, p, stream);
+}
+
 template <int NC>
 int launch_stream_nc(const coarse_op* op, const StreamParams& p, int dagger, cudaStream_t stream) {
     if (op->prec == COARSE_LINK_I16)
-        return dagger ? launch_stream_t<NC, true, true>(op, p, stream) : launch_stream_t<NC, true, false>(op, p, stream);
-    return dagger ? launch_stream_t<NC, false, true>(op, p, stream) : launch_stream_t<NC, false, false>(op, p, stream);
+        return dagger ? launch_stream_t<NC, true, true, false>(op, p, stream) : launch_stream_n<NC, true>(op, p, stream);
+    return dagger ? launch_stream_t<NC, false, true, false>(op, p, stream) : launch_stream_n<NC, false>(op, p, stream);
 }
 
 bool stream_supports(int Nc, int nrhs) {
@@ -109,6 +134,8 @@ int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, cu
     p.out = static_cast<float2*>(out);
     p.n_items = 0;
     p.stages = 0;
+    // links that fit L2 (with room for the vectors) are re-read from L2 by the next apply: keep them
+    p.keep_links = op->keep_opt == 2 || (op->keep_opt == 0 && coarse_op_link_bytes(op) <= (size_t)op->l2_bytes / 2);
     switch (op->Nc) {
         case 32: return launch_stream_nc<32>(op, p, dagger, stream);
         case 48: return launch_stream_nc<48>(op, p, dagger, stream);
@@ -274,6 +301,10 @@ coarse_op_t* coarse_op_create(const int dims[4], int Nc, int link_precision) {
     op->scales = nullptr;
     op->path_opt = COARSE_PATH_AUTO;
     op->grid_opt = 0;
+    op->stages_opt = 0;
+    op->fine_opt = 0;
+    op->keep_opt = 0;
+    { int l2 = 0; cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev); op->l2_bytes = l2; }
     op->last_launches = 0;
     op->last_path = 0;
     op->device = dev;
@@ -338,6 +369,18 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value) {
         case COARSE_OPT_GRID:
             if (value < 0) return fail(COARSE_EINVAL, "set_option: grid must be >= 0");
             op->grid_opt = value;
+            return COARSE_OK;
+        case COARSE_OPT_FINE:
+            if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: fine must be 0 (auto), 1 (never) or 2 (always)");
+            op->fine_opt = value;
+            return COARSE_OK;
+        case COARSE_OPT_KEEP_LINKS:
+            if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: keep_links must be 0 (auto), 1 (never) or 2 (always)");
+            op->keep_opt = value;
+            return COARSE_OK;
+        case COARSE_OPT_STAGES:
+            if (value < 0 || value == 1) return fail(COARSE_EINVAL, "set_option: stages must be 0 (default) or >= 2");
+            op->stages_opt = value;
             return COARSE_OK;
         default:
             return fail(COARSE_EINVAL, "set_option: unknown option %d", option);

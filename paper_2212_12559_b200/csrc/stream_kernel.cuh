@@ -10,8 +10,11 @@
 //       of one (site, matrix, row range) with an L2 evict_first hint, and the neighbour vector
 //       entries that those rows multiply with an evict_last hint (the vector field is re-read 9x
 //       and stays L2-resident).  Completion is counted in bytes on the slot's `full` mbarrier.
-//       With S x ~18 KB per SM the chip keeps > 20 MB of loads in flight, far beyond the
-//       latency x bandwidth product of HBM3e, with no registers tied up.
+//       The ring depth S is chosen by the host so that ~112 KB per SM (~16 MB chip-wide) is in
+//       flight: measured on B200, throughput peaks there (S = 6-7 at 16-19 KB stages, 7.3-7.4 TB/s)
+//       and DROPS by 5 % when the ring is deepened to the 227 KB that would fit (12 stages): past
+//       the latency x bandwidth product more outstanding requests only lengthen the DRAM queues.
+//       No registers are tied up by loads in flight.
 //   consumers (W = 8 warps)      wait on `full`, read the slot with conflict-free LDS.128 (lane <->
 //       16-byte column quad, warp <-> rows), accumulate in fp32 registers across all nine matrices
 //       of the item, release the slot through its `empty` mbarrier, and combine partial sums ONCE
@@ -40,6 +43,7 @@ struct StreamParams {
     float2* out;
     int n_items;
     int stages;
+    int keep_links;   // 1: the whole link field fits L2 and is re-read every apply -> do not mark it evict_first
 };
 
 constexpr int stream_pow2ceil(int v) { return v <= 1 ? 1 : v <= 2 ? 2 : v <= 4 ? 4 : v <= 8 ? 8 : v <= 16 ? 16 : 32; }
@@ -55,7 +59,11 @@ constexpr int stream_rows_per_stage(int nc, int rowbytes, int unit, int max_byte
     return best;
 }
 
-template <int NC, bool I16>
+// FINE = the small-lattice geometry (dagger = 0 only): as few rows per stage as the warp layout
+// allows, so that V * NB work items still fill 148 SMs when the local volume is a few hundred
+// sites or less ("additional parallelism is exposed in the matrix-vector application
+// to compensate for reduction in parallelism possible by the size of the local volume alone").
+template <int NC, bool I16, bool FINE = false>
 struct StreamGeom {
     static constexpr int W = 8;                                // consumer warps
     static constexpr int ENTRY_BYTES = I16 ? 4 : 8;            // one complex link entry
@@ -66,7 +74,7 @@ struct StreamGeom {
     static constexpr int QP = Q / PASSES;                      // quads per row per pass (<= 32)
     static constexpr int G = stream_pow2ceil(QP);              // lanes that share one row
     static constexpr int RPL = 32 / G;                         // rows per warp-wide load
-    static constexpr int RS = stream_rows_per_stage(NC, ROWBYTES, W * RPL, 24576);
+    static constexpr int RS = stream_rows_per_stage(NC, ROWBYTES, W * RPL, FINE ? (W * RPL * ROWBYTES) : 24576);
     static constexpr int NB = NC / RS;                         // row blocks per matrix
     static constexpr int WL = RS / (W * RPL);                  // warp-wide loads per warp, stage, pass
     static constexpr int LINK_STAGE = RS * ROWBYTES;
@@ -97,9 +105,10 @@ __device__ __forceinline__ void cmac(float2& acc, float mre, float mim, const fl
     }
 }
 
-template <int NC, bool I16, bool DAG>
-__global__ void __launch_bounds__(StreamGeom<NC, I16>::THREADS, 1) coarse_apply_stream(StreamParams p) {
-    using Gm = StreamGeom<NC, I16>;
+template <int NC, bool I16, bool DAG, bool FINE = false>
+__global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_apply_stream(StreamParams p) {
+    static_assert(!(DAG && FINE), "the fine geometry splits output rows: dagger = 0 only");
+    using Gm = StreamGeom<NC, I16, FINE>;
     constexpr int W = Gm::W, RS = Gm::RS, NB = Gm::NB, WL = Gm::WL, QP = Gm::QP, G = Gm::G, RPL = Gm::RPL;
     constexpr int PASSES = Gm::PASSES, CPQ = Gm::CPQ, ROWBYTES = Gm::ROWBYTES;
     constexpr int LINK_STAGE = Gm::LINK_STAGE;
@@ -128,8 +137,8 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16>::THREADS, 1) coarse_apply_
         // ------------------------------------------------------------------ producer
         // The whole warp walks the loop (uniform control flow, so the bulk copies are not wrapped
         // in per-lane replay loops) and one elected lane issues the copies.
-        const uint64_t pol_links = ptx::policy_evict_first();
         const uint64_t pol_vec = ptx::policy_evict_last();
+        const uint64_t pol_links = p.keep_links ? pol_vec : ptx::policy_evict_first();
         const uint32_t link_u32 = ptx::smem_u32(link_smem), vec_u32 = ptx::smem_u32(vec_smem);
         int slot = 0;
         uint32_t phase = 0;

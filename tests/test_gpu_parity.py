@@ -43,7 +43,7 @@ def _links_for(dims, Nc, prec, seed, hermitian, oracle_lib):
     return q, sc, q_ref.reshape(V, 9, Nc, Nc, 2), sc_ref
 
 
-def _run(oracle_lib, dims, Nc, prec, nrhs, dagger, path, seed=1234, hermitian=True, grid=0):
+def _run(oracle_lib, dims, Nc, prec, nrhs, dagger, path, seed=1234, hermitian=True, grid=0, opts=None):
     V = synth.lattice_volume(dims)
     links, scales, links_h, scales_h = _links_for(dims, Nc, prec, seed, hermitian, oracle_lib)
     vin = synth.make_vectors(dims, Nc, nrhs, seed + 1, device="cuda")
@@ -52,6 +52,8 @@ def _run(oracle_lib, dims, Nc, prec, nrhs, dagger, path, seed=1234, hermitian=Tr
     op.set_option(cop.OPT_PATH, path)
     if grid:
         op.set_option(cop.OPT_GRID, grid)
+    for k, v in (opts or {}).items():
+        op.set_option(k, v)
     op.apply(vin, vout, nrhs=nrhs, dagger=dagger)
     torch.cuda.synchronize()
     assert op.last_launches >= 1
@@ -158,6 +160,54 @@ def test_stream_path_any_grid(oracle_lib, grid):
         _run(oracle_lib, (3, 3, 2, 2), 128, cop.LINK_I16, 1, dagger, cop.PATH_STREAM, grid=grid)
 
 
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+def test_stream_fine_geometry(oracle_lib, Nc, prec):
+    """The small-lattice row-block split (PAPER.md:L99 'additional parallelism'), forced on, and the
+    automatic choice on a lattice with fewer regular work items than SMs."""
+    _run(oracle_lib, (3, 2, 1, 4), Nc, prec, 1, 0, cop.PATH_STREAM, opts={cop.OPT_FINE: 2})
+    _run(oracle_lib, (2, 2, 1, 2), Nc, prec, 1, 0, cop.PATH_STREAM, opts={cop.OPT_FINE: 0}, hermitian=False)
+    _run(oracle_lib, (3, 2, 1, 4), Nc, prec, 1, 0, cop.PATH_STREAM, opts={cop.OPT_FINE: 1})
+
+
+@pytest.mark.parametrize("stages", [2, 3, 5, 12, 64])
+@pytest.mark.parametrize("keep", [1, 2])
+def test_stream_ring_depth_and_l2_policy(oracle_lib, stages, keep):
+    for dagger in (0, 1):
+        _run(oracle_lib, (5, 3, 4, 7), 48, cop.LINK_C64, 1, dagger, cop.PATH_STREAM,
+             opts={cop.OPT_STAGES: stages, cop.OPT_KEEP_LINKS: keep})
+        _run(oracle_lib, (3, 3, 2, 2), 192, cop.LINK_I16, 1, dagger, cop.PATH_STREAM,
+             opts={cop.OPT_STAGES: stages, cop.OPT_KEEP_LINKS: keep})
+
+
+def test_apply_is_graph_capturable(oracle_lib):
+    """coarse_op_apply only enqueues: a chain of applies can be captured into one CUDA graph (how
+    bench.py times L2-resident lattices and how a solver would drive it)."""
+    dims, Nc = (4, 4, 4, 4), 48
+    links = synth.make_gamma_hermitian_links(dims, Nc, 31, device="cuda")
+    v0 = synth.make_vectors(dims, Nc, 1, 32, device="cuda")
+    v1, v2 = torch.empty_like(v0), torch.empty_like(v0)
+    op = cop.CoarseOp(dims, Nc).set_links(links)
+    op.apply(v0, v1)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.graph(g, stream=side):
+        op.apply(v0, v1, dagger=0)
+        op.apply(v1, v2, dagger=1)          # A^H A v0: one CGNE normal-equation application
+    torch.cuda.current_stream().wait_stream(side)
+    v1.zero_(); v2.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    links_h = links.cpu().numpy()
+    ref1 = oracle_lib.coarse_apply(dims, Nc, links_h, v0.cpu().numpy(), dagger=0)
+    ref2 = oracle_lib.coarse_apply(dims, Nc, links_h, ref1.astype(np.complex64), dagger=1)
+    assert rel_l2_per_rhs(v1.cpu().numpy(), ref1) <= TOL
+    assert rel_l2_per_rhs(v2.cpu().numpy(), ref2) <= 2 * TOL
+    op.close()
+
+
 def test_bit_reproducible():
     dims, Nc = (4, 4, 4, 6), 64
     links = synth.make_gamma_hermitian_links(dims, Nc, 5, device="cuda")
@@ -214,6 +264,10 @@ def test_error_codes():
     assert L.coarse_op_apply(h, None, vout.data_ptr(), 1, 0, None) == cop.EINVAL
     assert "dagger" in cop.coarse_op_last_error() or "NULL" in cop.coarse_op_last_error()
     assert L.coarse_op_set_option(h, cop.OPT_PATH, 99) == cop.EINVAL
+    assert L.coarse_op_set_option(h, cop.OPT_STAGES, 1) == cop.EINVAL
+    assert L.coarse_op_set_option(h, cop.OPT_FINE, 3) == cop.EINVAL
+    assert L.coarse_op_set_option(h, cop.OPT_KEEP_LINKS, -1) == cop.EINVAL
+    assert L.coarse_op_set_option(h, 77, 0) == cop.EINVAL
     assert L.coarse_op_apply(h, vin.data_ptr(), vout.data_ptr(), 1, 0, None) == cop.OK
     cop.coarse_op_destroy(h)
     cop.coarse_op_destroy(0)
