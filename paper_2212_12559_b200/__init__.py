@@ -18,7 +18,7 @@ LINK_I16 = 1
 
 OK, EINVAL, EUNSUPPORTED, ENOTREADY, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 
-PATH_AUTO, PATH_SIMPLE, PATH_STREAM, PATH_TENSOR = 0, 1, 2, 3
+PATH_AUTO, PATH_SIMPLE, PATH_STREAM, PATH_TENSOR, PATH_BLOCK = 0, 1, 2, 3, 4
 OPT_PATH, OPT_GRID, OPT_STAGES, OPT_FINE, OPT_KEEP_LINKS = 0, 1, 2, 3, 4
 
 EXPORTS = (

@@ -14,6 +14,7 @@
 #include "quantize_kernel.cuh"
 #include "simple_kernel.cuh"
 #include "stream_kernel.cuh"
+#include "block_kernel.cuh"
 #include "tensor_kernel.cuh"
 
 using namespace coarse;
@@ -144,6 +145,68 @@ int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, cu
         case 128: return launch_stream_nc<128>(op, p, dagger, stream);
         case 192: return launch_stream_nc<192>(op, p, dagger, stream);
         default: return fail(COARSE_EUNSUPPORTED, "STREAM path is not compiled for Nc=%d", op->Nc);
+    }
+}
+
+// ---------------------------------------------------------------- BLOCK dispatch
+template <int NC, bool I16, bool DAG, int RP>
+int launch_block_t(const coarse_op* op, const BlockParams& base, cudaStream_t stream) {
+    using Gm = BlockGeom<NC, I16, RP>;
+    BlockParams p = base;
+    p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
+    const int sb = Gm::stage_bytes(DAG, p.nrhs);
+    int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (sb + 16);
+    if (stages < 2) return fail(COARSE_EUNSUPPORTED, "BLOCK: shared memory too small for Nc=%d nrhs=%d", NC, p.nrhs);
+    int want = (114688 + sb / 2) / sb;
+    if (want < 3) want = 3;
+    if (op->stages_opt > 0) want = op->stages_opt;
+    if (stages > want) stages = want;
+    p.stages = stages;
+    const int smem = Gm::smem_bytes(DAG, p.nrhs, stages);
+    auto kern = coarse_apply_block<NC, I16, DAG, RP>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(block kernel)");
+    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
+    if (grid > p.n_items) grid = p.n_items;
+    kern<<<grid, Gm::THREADS, smem, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "block kernel launch");
+    return COARSE_OK;
+}
+
+template <int NC>
+int launch_block_nc(const coarse_op* op, const BlockParams& p, int dagger, cudaStream_t stream) {
+    const bool i16 = op->prec == COARSE_LINK_I16;
+    if (p.nrhs <= 8) {
+        if (i16) return dagger ? launch_block_t<NC, true, true, 8>(op, p, stream) : launch_block_t<NC, true, false, 8>(op, p, stream);
+        return dagger ? launch_block_t<NC, false, true, 8>(op, p, stream) : launch_block_t<NC, false, false, 8>(op, p, stream);
+    }
+    if (i16) return dagger ? launch_block_t<NC, true, true, 16>(op, p, stream) : launch_block_t<NC, true, false, 16>(op, p, stream);
+    return dagger ? launch_block_t<NC, false, true, 16>(op, p, stream) : launch_block_t<NC, false, false, 16>(op, p, stream);
+}
+
+bool block_supports_nc(int Nc) { return stream_supports(Nc, 1); }
+bool block_supports(int Nc, int nrhs) { return block_supports_nc(Nc) && nrhs >= 1 && nrhs <= 16; }
+
+int launch_block(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, cudaStream_t stream) {
+    BlockParams p;
+    p.lat = op->lat;
+    p.links = static_cast<const unsigned char*>(op->links);
+    p.scales = op->scales;
+    p.in = static_cast<const float2*>(in);
+    p.out = static_cast<float2*>(out);
+    p.n_items = 0;
+    p.stages = 0;
+    p.nrhs = nrhs;
+    p.keep_links = op->keep_opt == 2 || (op->keep_opt == 0 && coarse_op_link_bytes(op) <= (size_t)op->l2_bytes / 2);
+    switch (op->Nc) {
+        case 32: return launch_block_nc<32>(op, p, dagger, stream);
+        case 48: return launch_block_nc<48>(op, p, dagger, stream);
+        case 64: return launch_block_nc<64>(op, p, dagger, stream);
+        case 96: return launch_block_nc<96>(op, p, dagger, stream);
+        case 128: return launch_block_nc<128>(op, p, dagger, stream);
+        case 192: return launch_block_nc<192>(op, p, dagger, stream);
+        default: return fail(COARSE_EUNSUPPORTED, "BLOCK path is not compiled for Nc=%d", op->Nc);
     }
 }
 
@@ -359,6 +422,12 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value) {
                 op->path_opt = value;
                 return COARSE_OK;
             }
+            if (value == COARSE_PATH_BLOCK) {
+                if (!block_supports_nc(op->Nc))
+                    return fail(COARSE_EUNSUPPORTED, "set_option: BLOCK path is not compiled for Nc=%d", op->Nc);
+                op->path_opt = value;
+                return COARSE_OK;
+            }
             if (value == COARSE_PATH_TENSOR) {
                 if (!tensor_supports_nc(op->Nc, op->prec))
                     return fail(COARSE_EUNSUPPORTED, "set_option: TENSOR path covers complex64 links with Nc in {48,64,128} (got Nc=%d, precision %d)", op->Nc, op->prec);
@@ -400,12 +469,17 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
     if (path == COARSE_PATH_AUTO)
         path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM
                : (tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok) ? COARSE_PATH_TENSOR
+               : block_supports(op->Nc, nrhs)                                  ? COARSE_PATH_BLOCK
                                                                                : COARSE_PATH_SIMPLE;
     op->last_launches = 0;
     if (path == COARSE_PATH_TENSOR) {
         if (!tensor_supports(op->Nc, op->prec, nrhs))
             return fail(COARSE_EUNSUPPORTED, "apply: TENSOR path covers nrhs in {8,16} (got Nc=%d nrhs=%d)", op->Nc, nrhs);
         rc = launch_tensor(op, in_dev, out_dev, nrhs, dagger, st);
+    } else if (path == COARSE_PATH_BLOCK) {
+        if (!block_supports(op->Nc, nrhs))
+            return fail(COARSE_EUNSUPPORTED, "apply: BLOCK path covers nrhs <= 16 (got Nc=%d nrhs=%d)", op->Nc, nrhs);
+        rc = launch_block(op, in_dev, out_dev, nrhs, dagger, st);
     } else if (path == COARSE_PATH_STREAM) {
         if (!stream_supports(op->Nc, nrhs))
             return fail(COARSE_EUNSUPPORTED, "apply: STREAM path does not cover Nc=%d nrhs=%d", op->Nc, nrhs);

@@ -101,6 +101,49 @@ def test_tensor_path_block_apply(oracle_lib, dims, Nc, nrhs, dagger):
     assert err <= 3e-6, f"3xTF32 with per-matrix accumulator chains should sit near 1e-6, got {err:.2e}"
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (1, 1, 1, 1)])
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("nrhs", [2, 3, 8, 11, 16])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_block_path_cuda_cores(oracle_lib, dims, Nc, prec, nrhs, dagger):
+    """CUDA-core block apply: every compiled Nc, both link formats, ragged nrhs (3 = one propagator,
+    PAPER.md:L188; 11 leaves surplus lanes in the 16-wide mapping)."""
+    if Nc >= 128 and dims == (4, 4, 4, 4):
+        dims = (2, 4, 2, 2)               # keep the oracle's run time in seconds
+    _run(oracle_lib, dims, Nc, prec, nrhs, dagger, cop.PATH_BLOCK)
+
+
+@pytest.mark.parametrize("grid", [1, 7, 1000])
+def test_block_path_any_grid(oracle_lib, grid):
+    for dagger in (0, 1):
+        _run(oracle_lib, (5, 3, 2, 3), 128, cop.LINK_C64, 16, dagger, cop.PATH_BLOCK, grid=grid)
+        _run(oracle_lib, (5, 3, 4, 7), 48, cop.LINK_I16, 3, dagger, cop.PATH_BLOCK, grid=grid, hermitian=False,
+             opts={cop.OPT_STAGES: 2})
+
+
+def test_auto_path_selection():
+    dims = (2, 2, 2, 2)
+    cases = [(48, cop.LINK_C64, 1, cop.PATH_STREAM), (48, cop.LINK_C64, 16, cop.PATH_TENSOR),
+             (48, cop.LINK_C64, 3, cop.PATH_BLOCK), (64, cop.LINK_I16, 16, cop.PATH_BLOCK),
+             (96, cop.LINK_C64, 8, cop.PATH_BLOCK), (48, cop.LINK_C64, 17, cop.PATH_SIMPLE),
+             (6, cop.LINK_C64, 2, cop.PATH_SIMPLE)]
+    for Nc, prec, nrhs, want in cases:
+        V = 16
+        if prec == cop.LINK_C64:
+            links, scales = torch.zeros((V, 9, Nc, Nc), dtype=torch.complex64, device="cuda"), None
+        else:
+            links = torch.zeros((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+            scales = torch.ones((V, 9), dtype=torch.float32, device="cuda")
+        vin = torch.zeros((V, Nc, nrhs), dtype=torch.complex64, device="cuda")
+        vout = torch.empty_like(vin)
+        op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+        op.apply(vin, vout, nrhs=nrhs)
+        torch.cuda.synchronize()
+        assert op.last_path == want, (Nc, prec, nrhs, op.last_path, want)
+        op.close()
+
+
 @pytest.mark.parametrize("grid", [1, 7, 1000])
 def test_tensor_path_any_grid(oracle_lib, grid):
     """Several sites per CTA (accumulator/operand rings wrap many times), ragged tail, idle CTAs."""
