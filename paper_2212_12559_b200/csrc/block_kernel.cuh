@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(BlockGeom<NC, I16, RP>::THREADS, 1) coarse_app
     int slot = 0;
     uint32_t phase = 0;
 
-    float cur_scale = 1.f, next_scale = 1.f;
+    float cur_scale = 1.f, next_scale = 1.f, next2_scale = 1.f;
     auto fetch_scale = [&](int item) -> float {
         if (!I16 || lane >= 9 || item >= p.n_items) return 1.f;
         const int s = DAG ? item : item / NB;
@@ -185,12 +185,14 @@ __global__ void __launch_bounds__(BlockGeom<NC, I16, RP>::THREADS, 1) coarse_app
         return __ldg(p.scales + (int64_t)sm * 9 + lane);
     };
     next_scale = fetch_scale(blockIdx.x);
+    next2_scale = fetch_scale(blockIdx.x + gridDim.x);
 
     for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
         const int s = DAG ? item : item / NB;
         const int rb = DAG ? 0 : item % NB;
         cur_scale = next_scale;
-        next_scale = fetch_scale(item + gridDim.x);
+        next_scale = next2_scale;
+        next2_scale = fetch_scale(item + 2 * gridDim.x);
 
         if (!DAG) {
             float2 acc[RS];

@@ -180,9 +180,10 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
     uint32_t phase = 0;
     int red_parity = 0;
 
-    // int16: lane m (< 9) carries the fp32 scale of matrix m of the current item; the next item's
-    // scales are fetched one item ahead so the global-load latency never sits on the critical path.
-    float cur_scale = 1.f, next_scale = 1.f;
+    // int16: lane m (< 9) carries the fp32 scale of matrix m of the current item.  The scales are
+    // fetched TWO items ahead: under a saturated HBM a DRAM miss takes about as long as a whole
+    // item (~3 us), and with a one-item lead ncu showed 12 % of the dagger = 1 samples waiting on it.
+    float cur_scale = 1.f, next_scale = 1.f, next2_scale = 1.f;
     auto fetch_scale = [&](int item) -> float {
         if (!I16 || lane >= 9 || item >= p.n_items) return 1.f;
         const int s = DAG ? item : item / NB;
@@ -190,12 +191,14 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
         return __ldg(p.scales + (int64_t)sm * 9 + lane);
     };
     next_scale = fetch_scale(blockIdx.x);
+    next2_scale = fetch_scale(blockIdx.x + gridDim.x);
 
     for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
         const int s = DAG ? item : item / NB;
         const int rb = DAG ? 0 : item % NB;
         cur_scale = next_scale;
-        next_scale = fetch_scale(item + gridDim.x);
+        next_scale = next2_scale;
+        next2_scale = fetch_scale(item + 2 * gridDim.x);
 
         if (!DAG) {
             float2 acc[WL];
