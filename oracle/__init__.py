@@ -49,6 +49,9 @@ def _load() -> ctypes.CDLL:
         lib.oracle_coarse_apply.argtypes = [i4, ci, ci, vp, vp, vp, vp, ci, ci, ci]
         lib.oracle_coarse_apply_sites.restype = ci
         lib.oracle_coarse_apply_sites.argtypes = [i4, ci, ci, vp, vp, vp, vp, ci, ci, vp, ci64, ci]
+        lib.oracle_coarse_apply_parts.restype = ci
+        lib.oracle_coarse_apply_parts.argtypes = [i4, ci, ci, vp, vp, vp, vp, vp, ci, ci, ci, ci,
+                                                  ctypes.c_double, ctypes.c_double, ci]
         lib.oracle_neighbours.restype = ci
         lib.oracle_neighbours.argtypes = [i4, ci64, vp]
         lib.oracle_quantize_i16.restype = ci
@@ -165,3 +168,88 @@ def dequantize_i16(q, scales, Nc: int) -> np.ndarray:
     if rc != 0:
         raise ValueError("oracle_dequantize_i16 rejected its arguments")
     return out
+
+
+# ----------------------------------------------------------------------------- even/odd (row f1)
+PARITY_EVEN, PARITY_ODD, PARITY_ALL = 0, 1, 2
+LOCAL_NONE, LOCAL_X, LOCAL_IDENTITY = 0, 1, 2
+
+
+def site_parities(dims) -> np.ndarray:
+    """pi(x) = (x0+x1+x2+x3) mod 2 for every site index s(x) (x0 fastest)."""
+    L0, L1, L2, L3 = (int(d) for d in dims)
+    x3, x2, x1, x0 = np.meshgrid(np.arange(L3), np.arange(L2), np.arange(L1), np.arange(L0), indexing="ij")
+    return ((x0 + x1 + x2 + x3) & 1).reshape(-1)
+
+
+def coarse_apply_parts(dims, Nc: int, links, u, w, nrhs: int = 1, dagger: int = 0, parity: int = PARITY_ALL,
+                       local: int = LOCAL_X, alpha: float = 1.0, beta: float = 1.0,
+                       link_precision: int = LINK_C64, scales=None, nthreads: int = 0) -> np.ndarray:
+    """O7: out(x) = alpha*Loc(x) + beta*Hop(x) on the sites of `parity` (zero elsewhere);
+    Loc = X.u | u | 0, Hop = the eight hopping terms applied to w.  complex128 [V][Nc][nrhs]."""
+    V = int(np.prod([int(d) for d in dims]))
+    L = _as_links(links, link_precision, V, Nc)
+    ww = _as_vec(w, V, Nc, nrhs)
+    uu = None if u is None else _as_vec(u, V, Nc, nrhs)
+    sc = None
+    if link_precision == LINK_I16:
+        sc = np.ascontiguousarray(np.asarray(scales, dtype=np.float32))
+    out = np.empty((V, Nc, nrhs), dtype=np.complex128)
+    rc = _load().oracle_coarse_apply_parts(_dims(dims), Nc, link_precision, L.ctypes.data,
+                                           sc.ctypes.data if sc is not None else None,
+                                           uu.ctypes.data if uu is not None else None,
+                                           ww.ctypes.data, out.ctypes.data, nrhs, dagger, parity, local,
+                                           float(alpha), float(beta), nthreads)
+    if rc != 0:
+        raise ValueError(f"oracle_coarse_apply_parts rejected its arguments (rc={rc})")
+    return out
+
+
+def _even_dims(dims):
+    if any(int(d) % 2 for d in dims):
+        raise ValueError("the even/odd decomposition needs every extent to be even")
+
+
+def schur_apply(dims, Nc: int, links, v, parity: int, nrhs: int = 1) -> np.ndarray:
+    """Textbook Schur complement of the coarse operator on the sites of parity p (q = 1-p):
+        S_p v = X_p v - D_pq X_q^{-1} D_qp v          ("Schur-preconditioned")
+    with D the hopping part.  v lives on parity p (its other-parity entries are ignored).  Steps:
+    O7 hop to parity q, numpy dense solve with X(x) per site of q, O7 X - hop back to p.  The
+    intermediate vectors are rounded to complex64 exactly where the CUDA path stores them."""
+    _even_dims(dims)
+    links = np.asarray(links)
+    V = links.shape[0]
+    q = 1 - parity
+    par = site_parities(dims)
+    vp = np.where((par == parity)[:, None, None], np.asarray(v).reshape(V, Nc, nrhs), 0).astype(np.complex64)
+    t = coarse_apply_parts(dims, Nc, links, None, vp, nrhs, 0, q, LOCAL_NONE, 0.0, 1.0)
+    t2 = np.zeros_like(t)
+    for s in np.nonzero(par == q)[0]:
+        t2[s] = np.linalg.solve(links[s, 0].astype(np.complex128), t[s])
+    return coarse_apply_parts(dims, Nc, links, vp, t2.astype(np.complex64), nrhs, 0, parity, LOCAL_X, 1.0, -1.0)
+
+
+def hat_links(links) -> np.ndarray:
+    """Block-preconditioned links: Yhat_m(x) = X(x)^{-1} Y_m(x), m = 1..8; slot 0
+    holds the identity.  complex128 [V][9][Nc][Nc] (cast to complex64 before use as an input)."""
+    links = np.asarray(links).astype(np.complex128)
+    out = np.empty_like(links)
+    Nc = links.shape[-1]
+    for s in range(links.shape[0]):
+        out[s, 0] = np.eye(Nc)
+        out[s, 1:] = np.linalg.solve(links[s, 0][None, :, :], links[s, 1:])
+    return out
+
+
+def schur_hat_apply(dims, Nc: int, hat, v, parity: int, nrhs: int = 1, dagger: int = 0) -> np.ndarray:
+    """Left-preconditioned Schur operator from block-preconditioned links, two O7 hops:
+        Shat_p v = v - Dhat_pq Dhat_qp v        ( = X_p^{-1} S_p v when hat = hat_links(links) )
+    dagger = 1 gives its adjoint, v - (Dhat^H)_pq (Dhat^H)_qp v."""
+    _even_dims(dims)
+    V = int(np.prod([int(d) for d in dims]))
+    q = 1 - parity
+    par = site_parities(dims)
+    vp = np.where((par == parity)[:, None, None], np.asarray(v).reshape(V, Nc, nrhs), 0).astype(np.complex64)
+    t = coarse_apply_parts(dims, Nc, hat, None, vp, nrhs, dagger, q, LOCAL_NONE, 0.0, 1.0)
+    return coarse_apply_parts(dims, Nc, hat, vp, t.astype(np.complex64), nrhs, dagger, parity,
+                              LOCAL_IDENTITY, 1.0, -1.0)

@@ -27,6 +27,17 @@
 //   O5 (quantiser)   per matrix scale = max|component|/32767 (BASELINE.json config 4;
 //        DESIGN.md readings R7, R8), q = clamp(rint(component/scale)) in fp32.
 //
+//   O7 (parts apply) the building block of the even/odd ("Schur-
+//        preconditioned", Table 1) coarse operators.  With the site parity
+//        pi(x) = (x0+x1+x2+x3) mod 2 and a parity set P (even, odd or all sites), for x in P
+//            out(x) = alpha * Loc(x) + beta * Hop(x)
+//            Loc(x) = X(x).u(x)  |  u(x) (identity)  |  0
+//            Hop(x) = sum_mu [ Y_{+mu}(x).w(x+mu^) + Y_{-mu}(x).w(x-mu^) ]
+//        and for dagger = 1 the same split of O2 (X^H u, and the adjoint hop).  Sites outside P
+//        are not part of the result (returned as zero).  The Schur complement and its
+//        block-preconditioned form are compositions of O7 written out in
+//        oracle/__init__.py (schur_apply, schur_hat_apply) with numpy's dense solve as a step.
+//
 // Layouts (identical to include/coarse_op.h because both take the caller's arrays):
 //   site index s(x) = x0 + L0*(x1 + L1*(x2 + L2*x3)); periodic wrap by modulo, so an
 //   extent-2 direction adds both hops from the same neighbour and an extent-1 direction
@@ -134,6 +145,42 @@ void apply_site(const Lattice& lat, int Nc, int prec, const void* links, const f
     }
 }
 
+// O7 for one output site: out_site = alpha*Loc + beta*Hop (see the header).
+//   local: 0 none, 1 X (X^H for dagger), 2 identity.
+void parts_site(const Lattice& lat, int Nc, int prec, const void* links, const float* scales,
+                const float* u, const float* w, int nrhs, int dagger, int local, double alpha,
+                double beta, int64_t s, double* out_site, double* tmp) {
+    const int64_t n = (int64_t)2 * Nc * nrhs;
+    std::memset(out_site, 0, sizeof(double) * n);
+    // local term
+    std::memset(tmp, 0, sizeof(double) * n);
+    if (local == 1) {
+        accumulate(prec, links, scales, Nc, nrhs, s, 0, dagger, u, s, tmp);
+    } else if (local == 2) {
+        for (int64_t e = 0; e < n; ++e) tmp[e] = (double)u[s * n + e];
+    }
+    for (int64_t e = 0; e < n; ++e) out_site[e] += alpha * tmp[e];
+    // hopping term
+    std::memset(tmp, 0, sizeof(double) * n);
+    for (int mu = 0; mu < 4; ++mu) {
+        const int64_t fwd = neighbour(lat, s, mu, +1), bwd = neighbour(lat, s, mu, -1);
+        if (!dagger) {
+            accumulate(prec, links, scales, Nc, nrhs, s, 1 + mu, 0, w, fwd, tmp);      // Y_{+mu}(x) w(x+mu^)
+            accumulate(prec, links, scales, Nc, nrhs, s, 5 + mu, 0, w, bwd, tmp);      // Y_{-mu}(x) w(x-mu^)
+        } else {
+            accumulate(prec, links, scales, Nc, nrhs, bwd, 1 + mu, 1, w, bwd, tmp);    // Y_{+mu}(x-mu^)^H w(x-mu^)
+            accumulate(prec, links, scales, Nc, nrhs, fwd, 5 + mu, 1, w, fwd, tmp);    // Y_{-mu}(x+mu^)^H w(x+mu^)
+        }
+    }
+    for (int64_t e = 0; e < n; ++e) out_site[e] += beta * tmp[e];
+}
+
+inline int site_parity(const Lattice& lat, int64_t s) {
+    int x[4];
+    coords_of(lat, s, x);
+    return (x[0] + x[1] + x[2] + x[3]) & 1;
+}
+
 bool valid(const int dims[4], int Nc, int prec, int nrhs, int dagger) {
     if (!dims || Nc < 1 || nrhs < 1) return false;
     if (prec != 0 && prec != 1) return false;
@@ -189,6 +236,40 @@ int oracle_coarse_apply_sites(const int dims[4], int Nc, int link_precision, con
     for (int64_t k = 0; k < nsites; ++k)
         apply_site(lat, Nc, link_precision, links, scales, in, nrhs, dagger, sites[k],
                    out + k * 2 * (int64_t)Nc * nrhs);
+    return 0;
+}
+
+// O7: parts apply.  parity: 0 even sites, 1 odd sites, 2 all sites; local: 0 none, 1 X, 2 identity.
+// u may be NULL when local == 0.  out is complex128 [V][Nc][nrhs]; sites outside the parity set are 0.
+int oracle_coarse_apply_parts(const int dims[4], int Nc, int link_precision, const void* links,
+                              const float* scales, const float* u, const float* w, double* out,
+                              int nrhs, int dagger, int parity, int local, double alpha, double beta,
+                              int nthreads) {
+    if (!valid(dims, Nc, link_precision, nrhs, dagger) || !links || !w || !out) return -1;
+    if (link_precision == 1 && !scales) return -1;
+    if (parity < 0 || parity > 2 || local < 0 || local > 2) return -1;
+    if (local != 0 && !u) return -1;
+    Lattice lat{{dims[0], dims[1], dims[2], dims[3]}, (int64_t)dims[0] * dims[1] * dims[2] * dims[3]};
+    const int64_t n = (int64_t)2 * Nc * nrhs;
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#pragma omp parallel num_threads(nthreads)
+#endif
+    {
+        double* tmp = new double[n];
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+        for (int64_t s = 0; s < lat.V; ++s) {
+            if (parity != 2 && site_parity(lat, s) != parity) {
+                std::memset(out + s * n, 0, sizeof(double) * n);
+                continue;
+            }
+            parts_site(lat, Nc, link_precision, links, scales, u, w, nrhs, dagger, local, alpha, beta, s,
+                       out + s * n, tmp);
+        }
+        delete[] tmp;
+    }
     return 0;
 }
 
