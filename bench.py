@@ -42,8 +42,15 @@ METRIC = "coarse-op site-updates/s"
 UNIT = "site-updates/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-# `ncu --set full` captures summarised under profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = {}
+# `ncu --set full` captures summarised under profiles/r01_ncu_full_*.md, keyed by
+# (config, path actually run, dagger); None for combinations that were not captured.
+NCU_TRAFFIC_BYTES = {
+    ("C2", 2, 0): 16362553600, ("C2", 2, 1): 16366406656,
+    ("C3", 2, 0): 7260122880, ("C3", 2, 1): 7261024768,
+    ("C4", 2, 0): 14580251904, ("C4", 2, 1): 14585814272,
+    ("C5", 3, 0): 7475386112, ("C5", 3, 1): 7440746240,
+    ("C5", 4, 0): 7445877248, ("C5", 4, 1): 7445823232,
+}
 
 
 def compulsory_bytes_per_site(Nc: int, links: str, nrhs: int) -> int:
@@ -406,9 +413,11 @@ def run_ours(args, cfg, daggers):
     achieved = bps * V / (kernel_ms[dom] * 1e-3) / 1e9
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": NCU_TRAFFIC_BYTES.get((args.config, dom)),
-        "kernel": f"coarse_apply_stream<{Nc},{'i16' if prec else 'c64'},dagger={dom}>" if op.last_path == cop.PATH_STREAM
-                  else f"path {op.last_path}",
+        "traffic": NCU_TRAFFIC_BYTES.get((args.config, op.last_path, dom)),
+        "kernel": "coarse_apply_%s<Nc=%d,%s,dagger=%d%s>" % (
+            {cop.PATH_SIMPLE: "simple", cop.PATH_STREAM: "stream", cop.PATH_TENSOR: "tensor",
+             cop.PATH_BLOCK: "block"}.get(op.last_path, "?"), Nc, "i16" if prec else "c64", dom,
+            "" if nrhs == 1 else ",nrhs=%d" % nrhs),
         "kernel_ms": kernel_ms[dom],
         "algorithmic_bytes_per_launch": bps * V,
         "peak_source": peak_src,

@@ -107,6 +107,29 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value);
 int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs, int dagger,
                     void* stream);
 
+/* Parts apply: the building block of the even/odd ("Schur-preconditioned", PAPER.md:L127/L135
+ * Table 1) and block-preconditioned coarse operators.  With the site parity
+ * pi(x) = (x0+x1+x2+x3) mod 2, for every site x of `parity` (COARSE_PARITY_*):
+ *
+ *     out(x) = alpha * Loc(x) + beta * Hop(x)
+ *     Loc(x) = X(x).u(x) (COARSE_LOCAL_X) | u(x) (COARSE_LOCAL_IDENTITY) | 0 (COARSE_LOCAL_NONE)
+ *     Hop(x) = sum_mu [ Y_{+mu}(x).w(x+mu^) + Y_{-mu}(x).w(x-mu^) ]
+ *
+ * and for dagger = 1 the same split of the adjoint (X(x)^H.u(x) and the adjoint hop of
+ * coarse_op_apply).  Sites of the other parity are NOT written.  u_dev may be NULL for
+ * COARSE_LOCAL_NONE and may alias out_dev (it is read at x only); w_dev must not overlap out_dev.
+ * COARSE_PARITY_EVEN/ODD need every extent even (COARSE_EINVAL otherwise).
+ * Examples (hat = an operator whose links are Yhat_m = X^{-1} Y_m):
+ *     t_o   = Dhat_oe v_e           : apply_parts(hat, NULL, v, t, .., COARSE_PARITY_ODD, COARSE_LOCAL_NONE, 0, 1)
+ *     out_e = v_e - Dhat_eo t_o     : apply_parts(hat, v, t, out, .., COARSE_PARITY_EVEN, COARSE_LOCAL_IDENTITY, 1, -1)
+ *     out_e = X_e v_e - D_eo t_o    : apply_parts(op, v, t, out, .., COARSE_PARITY_EVEN, COARSE_LOCAL_X, 1, -1)
+ * nrhs = 1 runs on the STREAM kernels (8 or 9 link matrices streamed per site of the parity),
+ * other nrhs on SIMPLE. */
+enum { COARSE_PARITY_EVEN = 0, COARSE_PARITY_ODD = 1, COARSE_PARITY_ALL = 2 };
+enum { COARSE_LOCAL_NONE = 0, COARSE_LOCAL_X = 1, COARSE_LOCAL_IDENTITY = 2 };
+int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev, void* out_dev, int nrhs,
+                          int dagger, int parity, int local, float alpha, float beta, void* stream);
+
 /* Same operation on HOST vectors: copies in_host to a device staging buffer owned by the handle
  * (allocated on first use, grown when nrhs grows), applies, copies the result to out_host and
  * synchronises the stream before returning.  Pinned host memory gives full PCIe rate. */

@@ -20,10 +20,12 @@ OK, EINVAL, EUNSUPPORTED, ENOTREADY, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 
 PATH_AUTO, PATH_SIMPLE, PATH_STREAM, PATH_TENSOR, PATH_BLOCK = 0, 1, 2, 3, 4
 OPT_PATH, OPT_GRID, OPT_STAGES, OPT_FINE, OPT_KEEP_LINKS = 0, 1, 2, 3, 4
+PARITY_EVEN, PARITY_ODD, PARITY_ALL = 0, 1, 2
+LOCAL_NONE, LOCAL_X, LOCAL_IDENTITY = 0, 1, 2
 
 EXPORTS = (
     "coarse_op_create", "coarse_op_link_bytes", "coarse_op_scale_bytes", "coarse_op_vector_bytes",
-    "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_host",
+    "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_parts", "coarse_op_apply_host",
     "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_destroy",
     "coarse_op_last_error",
 )
@@ -61,6 +63,8 @@ def lib() -> ctypes.CDLL:
     L.coarse_op_set_option.argtypes = [vp, ci, ci]
     L.coarse_op_apply.restype = ci
     L.coarse_op_apply.argtypes = [vp, vp, vp, ci, ci, vp]
+    L.coarse_op_apply_parts.restype = ci
+    L.coarse_op_apply_parts.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ctypes.c_float, ctypes.c_float, vp]
     L.coarse_op_apply_host.restype = ci
     L.coarse_op_apply_host.argtypes = [vp, vp, vp, ci, ci, vp]
     L.coarse_op_last_launches.restype = ci
@@ -146,6 +150,21 @@ def coarse_op_apply(op: int, vin, vout, nrhs: int = 1, dagger: int = 0, stream=N
     _check(lib().coarse_op_apply(op, _ptr(vin), _ptr(vout), int(nrhs), int(dagger), _stream_handle(stream)))
 
 
+def coarse_op_apply_parts(op: int, u, w, vout, nrhs: int = 1, dagger: int = 0, parity: int = PARITY_ALL,
+                          local: int = LOCAL_X, alpha: float = 1.0, beta: float = 1.0, stream=None) -> None:
+    """out(x) = alpha*Loc(u)(x) + beta*Hop(w)(x) on the sites of `parity` (include/coarse_op.h).
+    u / w / vout: contiguous CUDA complex64 tensors [V][Nc][nrhs]; u may be None for LOCAL_NONE."""
+    for t in (u, w, vout):
+        if t is None:
+            continue
+        if not t.is_cuda or not t.is_contiguous():
+            raise ValueError("vectors must be contiguous CUDA tensors")
+        if t.numel() * t.element_size() != coarse_op_vector_bytes(op, nrhs):
+            raise ValueError("vector tensor has the wrong number of bytes for this operator/nrhs")
+    _check(lib().coarse_op_apply_parts(op, _ptr(u), _ptr(w), _ptr(vout), int(nrhs), int(dagger), int(parity),
+                                       int(local), float(alpha), float(beta), _stream_handle(stream)))
+
+
 def coarse_op_apply_host(op: int, vin_host, vout_host, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
     """vin_host / vout_host: contiguous CPU complex64 tensors (pinned for full PCIe rate).
     Copies in, applies, copies out and synchronises the stream."""
@@ -207,6 +226,10 @@ class CoarseOp:
 
     def apply(self, vin, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
         coarse_op_apply(self._h, vin, vout, nrhs, dagger, stream)
+
+    def apply_parts(self, u, w, vout, nrhs: int = 1, dagger: int = 0, parity: int = PARITY_ALL,
+                    local: int = LOCAL_X, alpha: float = 1.0, beta: float = 1.0, stream=None) -> None:
+        coarse_op_apply_parts(self._h, u, w, vout, nrhs, dagger, parity, local, alpha, beta, stream)
 
     def apply_host(self, vin_host, vout_host, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
         coarse_op_apply_host(self._h, vin_host, vout_host, nrhs, dagger, stream)

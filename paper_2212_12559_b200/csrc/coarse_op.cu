@@ -67,13 +67,24 @@ struct coarse_op {
 
 namespace {
 
+// Parts apply (coarse_op_apply_parts): out = alpha*Loc(u) + beta*Hop(w) on one parity.  The plain
+// apply is the special case gen = false (u = w, local = X, alpha = beta = 1, all sites).
+struct PartsSpec {
+    bool gen;
+    const void* u;
+    int parity;   // 0 even, 1 odd, 2 all
+    int local;    // 0 none, 1 X, 2 identity
+    float alpha, beta;
+};
+const PartsSpec kPlain = {false, nullptr, 2, 1, 1.f, 1.f};
+
 // ---------------------------------------------------------------- STREAM dispatch
-template <int NC, bool I16, bool DAG, bool FINE>
+template <int NC, bool I16, bool DAG, bool FINE, bool GEN>
 int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
     using Gm = StreamGeom<NC, I16, FINE>;
     static_assert(Gm::OK, "unsupported STREAM geometry");
     StreamParams p = base;
-    p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
+    p.n_items = DAG ? p.n_sites : p.n_sites * Gm::NB;
     int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (Gm::stage_bytes(DAG) + 16);
     if (stages > 12) stages = 12;
     if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM: shared memory too small for Nc=%d", NC);
@@ -85,7 +96,7 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     if (stages > want) stages = want;
     p.stages = stages;
     const int smem = Gm::smem_bytes(DAG, stages);
-    auto kern = coarse_apply_stream<NC, I16, DAG, FINE>;
+    auto kern = coarse_apply_stream<NC, I16, DAG, FINE, GEN>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
@@ -101,21 +112,26 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
 // (256 sites, Nc = 48: 256 regular items on 148 SMs) the regular geometry is 2.8x faster (5.6 us
 // vs 15.4 us warm): 3 KB stages pay the per-stage handshake 6x more often, so the fine split only
 // pays when SMs would otherwise sit idle.
-template <int NC, bool I16>
+template <int NC, bool I16, bool GEN>
 int launch_stream_n(const coarse_op* op, const StreamParams& p, cudaStream_t stream) {
     constexpr bool HAS_FINE = StreamGeom<NC, I16, true>::NB > StreamGeom<NC, I16, false>::NB;
     if constexpr (HAS_FINE) {
-        const bool few = (int64_t)op->lat.V * StreamGeom<NC, I16, false>::NB < (int64_t)op->num_sms;
-        if (op->fine_opt == 2 || (op->fine_opt == 0 && few)) return launch_stream_t<NC, I16, false, true>(op, p, stream);
+        const bool few = (int64_t)p.n_sites * StreamGeom<NC, I16, false>::NB < (int64_t)op->num_sms;
+        if (op->fine_opt == 2 || (op->fine_opt == 0 && few)) return launch_stream_t<NC, I16, false, true, GEN>(op, p, stream);
     }
-    return launch_stream_t<NC, I16, false, false>(op, p, stream);
+    return launch_stream_t<NC, I16, false, false, GEN>(op, p, stream);
+}
+
+template <int NC, bool GEN>
+int launch_stream_nc(const coarse_op* op, const StreamParams& p, int dagger, cudaStream_t stream) {
+    if (op->prec == COARSE_LINK_I16)
+        return dagger ? launch_stream_t<NC, true, true, false, GEN>(op, p, stream) : launch_stream_n<NC, true, GEN>(op, p, stream);
+    return dagger ? launch_stream_t<NC, false, true, false, GEN>(op, p, stream) : launch_stream_n<NC, false, GEN>(op, p, stream);
 }
 
 template <int NC>
-int launch_stream_nc(const coarse_op* op, const StreamParams& p, int dagger, cudaStream_t stream) {
-    if (op->prec == COARSE_LINK_I16)
-        return dagger ? launch_stream_t<NC, true, true, false>(op, p, stream) : launch_stream_n<NC, true>(op, p, stream);
-    return dagger ? launch_stream_t<NC, false, true, false>(op, p, stream) : launch_stream_n<NC, false>(op, p, stream);
+int launch_stream_g(const coarse_op* op, const StreamParams& p, int dagger, bool gen, cudaStream_t stream) {
+    return gen ? launch_stream_nc<NC, true>(op, p, dagger, stream) : launch_stream_nc<NC, false>(op, p, dagger, stream);
 }
 
 bool stream_supports(int Nc, int nrhs) {
@@ -126,7 +142,7 @@ bool stream_supports(int Nc, int nrhs) {
     }
 }
 
-int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, cudaStream_t stream) {
+int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, const PartsSpec& ps, cudaStream_t stream) {
     StreamParams p;
     p.lat = op->lat;
     p.links = static_cast<const unsigned char*>(op->links);
@@ -137,13 +153,20 @@ int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, cu
     p.stages = 0;
     // links that fit L2 (with room for the vectors) are re-read from L2 by the next apply: keep them
     p.keep_links = op->keep_opt == 2 || (op->keep_opt == 0 && coarse_op_link_bytes(op) <= (size_t)op->l2_bytes / 2);
+    p.in_local = static_cast<const float2*>(ps.gen ? ps.u : in);
+    p.alpha = ps.alpha;
+    p.beta = ps.beta;
+    p.m_begin = ps.local == 1 ? 0 : 1;
+    p.identity = ps.local == 2 ? 1 : 0;
+    p.parity = ps.parity;
+    p.n_sites = ps.parity == 2 ? op->lat.V : op->lat.V / 2;
     switch (op->Nc) {
-        case 32: return launch_stream_nc<32>(op, p, dagger, stream);
-        case 48: return launch_stream_nc<48>(op, p, dagger, stream);
-        case 64: return launch_stream_nc<64>(op, p, dagger, stream);
-        case 96: return launch_stream_nc<96>(op, p, dagger, stream);
-        case 128: return launch_stream_nc<128>(op, p, dagger, stream);
-        case 192: return launch_stream_nc<192>(op, p, dagger, stream);
+        case 32: return launch_stream_g<32>(op, p, dagger, ps.gen, stream);
+        case 48: return launch_stream_g<48>(op, p, dagger, ps.gen, stream);
+        case 64: return launch_stream_g<64>(op, p, dagger, ps.gen, stream);
+        case 96: return launch_stream_g<96>(op, p, dagger, ps.gen, stream);
+        case 128: return launch_stream_g<128>(op, p, dagger, ps.gen, stream);
+        case 192: return launch_stream_g<192>(op, p, dagger, ps.gen, stream);
         default: return fail(COARSE_EUNSUPPORTED, "STREAM path is not compiled for Nc=%d", op->Nc);
     }
 }
@@ -290,7 +313,7 @@ int launch_tensor(const coarse_op* op, const void* in, void* out, int nrhs, int 
     }
 }
 
-int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, cudaStream_t stream) {
+int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, const PartsSpec& ps, cudaStream_t stream) {
     SimpleParams p;
     p.lat = op->lat;
     p.Nc = op->Nc;
@@ -300,6 +323,11 @@ int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int 
     p.scales = op->scales;
     p.in = static_cast<const float2*>(in);
     p.out = static_cast<float2*>(out);
+    p.in_local = static_cast<const float2*>(ps.gen ? ps.u : in);
+    p.alpha = ps.alpha;
+    p.beta = ps.beta;
+    p.local = ps.local;
+    p.parity = ps.parity;
     const int64_t total = (int64_t)op->lat.V * op->Nc * nrhs;
     const int64_t blocks = (total + 255) / 256;
     if (blocks > 0x7fffffffLL) return fail(COARSE_EUNSUPPORTED, "SIMPLE path: problem too large");
@@ -483,9 +511,48 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
     } else if (path == COARSE_PATH_STREAM) {
         if (!stream_supports(op->Nc, nrhs))
             return fail(COARSE_EUNSUPPORTED, "apply: STREAM path does not cover Nc=%d nrhs=%d", op->Nc, nrhs);
-        rc = launch_stream(op, in_dev, out_dev, dagger, st);
+        rc = launch_stream(op, in_dev, out_dev, dagger, kPlain, st);
     } else {
-        rc = launch_simple(op, in_dev, out_dev, nrhs, dagger, st);
+        rc = launch_simple(op, in_dev, out_dev, nrhs, dagger, kPlain, st);
+    }
+    if (rc != COARSE_OK) return rc;
+    op->last_launches = 1;
+    op->last_path = path;
+    return COARSE_OK;
+}
+
+int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev, void* out_dev, int nrhs,
+                          int dagger, int parity, int local, float alpha, float beta, void* stream) {
+    int rc = check_apply_args(op, w_dev, out_dev, nrhs, dagger);
+    if (rc != COARSE_OK) return rc;
+    if (parity < 0 || parity > 2) return fail(COARSE_EINVAL, "apply_parts: parity must be 0 (even), 1 (odd) or 2 (all), got %d", parity);
+    if (local < 0 || local > 2) return fail(COARSE_EINVAL, "apply_parts: local must be 0 (none), 1 (X) or 2 (identity), got %d", local);
+    if (local != 0 && !u_dev) return fail(COARSE_EINVAL, "apply_parts: u_dev is NULL but a local term was requested");
+    if (parity != 2)
+        for (int mu = 0; mu < 4; ++mu)
+            if (op->lat.L[mu] & 1)
+                return fail(COARSE_EINVAL, "apply_parts: the even/odd decomposition needs even extents (dims[%d] = %d)", mu, op->lat.L[mu]);
+    if (!aligned16(w_dev) || !aligned16(out_dev) || (u_dev && !aligned16(u_dev)))
+        return fail(COARSE_EINVAL, "apply_parts: device vectors must be 16-byte aligned");
+    const size_t vb = coarse_op_vector_bytes(op, nrhs);
+    const uintptr_t b = reinterpret_cast<uintptr_t>(out_dev);
+    const uintptr_t a = reinterpret_cast<uintptr_t>(w_dev);
+    // w is read at neighbours: it may share a buffer with out only when the two parities are disjoint,
+    // which the caller cannot express here, so overlap is always refused; u is read at x only and
+    // may alias out.
+    if (a < b + vb && b < a + vb) return fail(COARSE_EINVAL, "apply_parts: w and out overlap (the stencil reads neighbours)");
+    PartsSpec ps = {true, local != 0 ? u_dev : w_dev, parity, local, alpha, beta};
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int path = op->path_opt;
+    if (path == COARSE_PATH_AUTO || path == COARSE_PATH_TENSOR || path == COARSE_PATH_BLOCK)
+        path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM : COARSE_PATH_SIMPLE;
+    op->last_launches = 0;
+    if (path == COARSE_PATH_STREAM) {
+        if (!stream_supports(op->Nc, nrhs))
+            return fail(COARSE_EUNSUPPORTED, "apply_parts: STREAM path does not cover Nc=%d nrhs=%d", op->Nc, nrhs);
+        rc = launch_stream(op, w_dev, out_dev, dagger, ps, st);
+    } else {
+        rc = launch_simple(op, w_dev, out_dev, nrhs, dagger, ps, st);
     }
     if (rc != COARSE_OK) return rc;
     op->last_launches = 1;

@@ -44,7 +44,28 @@ struct StreamParams {
     int n_items;
     int stages;
     int keep_links;   // 1: the whole link field fits L2 and is re-read every apply -> do not mark it evict_first
+    // GEN (parts apply, include/coarse_op.h coarse_op_apply_parts): out = alpha*Loc + beta*Hop on one parity
+    const float2* in_local;   // u: operand of the local term (in = w: operand of the hopping term)
+    float alpha, beta;
+    int m_begin;              // 0: the X stage runs (local = X); 1: it is skipped
+    int identity;             // 1: add alpha*u(x) to the result (local = identity)
+    int parity;               // 0 even, 1 odd, 2 all sites
+    int n_sites;              // sites in the parity set
 };
+
+// Site index of the h-th site of a parity (all extents even, checked by the host): consecutive
+// h walk along x0 in steps of 2, the offset in x0 alternates with x1+x2+x3.
+__device__ __forceinline__ int parity_site(const Lat& lat, int h, int parity) {
+    const unsigned half = (unsigned)lat.L[0] >> 1;
+    const unsigned q1 = (unsigned)h / half;            // = x1 + L1*(x2 + L2*x3)
+    const unsigned x0h = (unsigned)h - q1 * half;
+    const unsigned q2 = q1 / (unsigned)lat.L[1];
+    const unsigned x1 = q1 - q2 * (unsigned)lat.L[1];
+    const unsigned x3 = q2 / (unsigned)lat.L[2];
+    const unsigned x2 = q2 - x3 * (unsigned)lat.L[2];
+    const unsigned off = (x1 + x2 + x3 + (unsigned)parity) & 1u;
+    return (int)(q1 * (unsigned)lat.L[0] + 2u * x0h + off);
+}
 
 constexpr int stream_pow2ceil(int v) { return v <= 1 ? 1 : v <= 2 ? 2 : v <= 4 ? 4 : v <= 8 ? 8 : v <= 16 ? 16 : 32; }
 constexpr int stream_passes(int q) {
@@ -105,7 +126,7 @@ __device__ __forceinline__ void cmac(float2& acc, float mre, float mim, const fl
     }
 }
 
-template <int NC, bool I16, bool DAG, bool FINE = false>
+template <int NC, bool I16, bool DAG, bool FINE = false, bool GEN = false>
 __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_apply_stream(StreamParams p) {
     static_assert(!(DAG && FINE), "the fine geometry splits output rows: dagger = 0 only");
     using Gm = StreamGeom<NC, I16, FINE>;
@@ -143,15 +164,17 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
         int slot = 0;
         uint32_t phase = 0;
         for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
-            const int s = DAG ? item : item / NB;
+            const int sidx = DAG ? item : item / NB;
+            const int s = (GEN && p.parity != 2) ? parity_site(p.lat, sidx, p.parity) : sidx;
             const int rb = DAG ? 0 : item % NB;
             const SiteX cx = site_coords(p.lat, s);
 #pragma unroll
             for (int m = 0; m < 9; ++m) {
+                if (GEN && m < p.m_begin) continue;
                 const int sv = stencil_site_x(p.lat, s, cx, m, DAG ? 1 : 0);
                 const int sm = DAG ? sv : s;
                 const unsigned char* mat = p.links + ((int64_t)sm * 9 + m) * ((int64_t)NC * ROWBYTES);
-                const float2* vec = p.in + (int64_t)sv * NC;
+                const float2* vec = ((GEN && m == 0) ? p.in_local : p.in) + (int64_t)sv * NC;
 #pragma unroll 1
                 for (int c = 0; c < (DAG ? NB : 1); ++c) {
                     const int r0 = DAG ? c * RS : rb * RS;
@@ -184,17 +207,22 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
     // fetched TWO items ahead: under a saturated HBM a DRAM miss takes about as long as a whole
     // item (~3 us), and with a one-item lead ncu showed 12 % of the dagger = 1 samples waiting on it.
     float cur_scale = 1.f, next_scale = 1.f, next2_scale = 1.f;
+    auto site_of = [&](int item) -> int {
+        const int sidx = DAG ? item : item / NB;
+        return (GEN && p.parity != 2) ? parity_site(p.lat, sidx, p.parity) : sidx;
+    };
     auto fetch_scale = [&](int item) -> float {
         if (!I16 || lane >= 9 || item >= p.n_items) return 1.f;
-        const int s = DAG ? item : item / NB;
+        const int s = site_of(item);
         const int sm = DAG ? stencil_site(p.lat, s, lane, 1) : s;
         return __ldg(p.scales + (int64_t)sm * 9 + lane);
     };
+    const int M0 = GEN ? p.m_begin : 0;
     next_scale = fetch_scale(blockIdx.x);
     next2_scale = fetch_scale(blockIdx.x + gridDim.x);
 
     for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
-        const int s = DAG ? item : item / NB;
+        const int s = site_of(item);
         const int rb = DAG ? 0 : item % NB;
         cur_scale = next_scale;
         next_scale = next2_scale;
@@ -205,8 +233,9 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
 #pragma unroll
             for (int k = 0; k < WL; ++k) acc[k] = make_float2(0.f, 0.f);
 #pragma unroll 1
-            for (int m = 0; m < 9; ++m) {
-                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+            for (int m = M0; m < 9; ++m) {
+                float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                if constexpr (GEN) sc *= (m == 0) ? p.alpha : p.beta;
                 ptx::mbar_wait(full0 + 8u * slot, phase);
                 const uint32_t lbase = link_u32 + slot * LINK_STAGE + qi * 16;
                 const uint32_t vbase = vec_u32 + slot * VEC_STAGE;
@@ -221,7 +250,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                             v[ps][2 * h] = make_float2(t.x, t.y);
                             v[ps][2 * h + 1] = make_float2(t.z, t.w);
                         }
-                        if constexpr (I16) {
+                        if constexpr (I16 || GEN) {
 #pragma unroll
                             for (int e = 0; e < CPQ; ++e) { v[ps][e].x *= sc; v[ps][e].y *= sc; }
                         }
@@ -262,6 +291,13 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                 }
                 if (qi == 0) {
                     const int row = rb * RS + (k * W + warp) * RPL + grp;
+                    if constexpr (GEN) {
+                        if (p.identity) {
+                            const float2 u = __ldg(p.in_local + (int64_t)s * NC + row);
+                            acc[k].x = fmaf(p.alpha, u.x, acc[k].x);
+                            acc[k].y = fmaf(p.alpha, u.y, acc[k].y);
+                        }
+                    }
                     p.out[(int64_t)s * NC + row] = acc[k];
                 }
             }
@@ -272,8 +308,9 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
 #pragma unroll
                 for (int e = 0; e < CPQ; ++e) acc[ps][e] = make_float2(0.f, 0.f);
 #pragma unroll 1
-            for (int m = 0; m < 9; ++m) {
-                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+            for (int m = M0; m < 9; ++m) {
+                float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                if constexpr (GEN) sc *= (m == 0) ? p.alpha : p.beta;
 #pragma unroll 1
                 for (int c = 0; c < NB; ++c) {
                     ptx::mbar_wait(full0 + 8u * slot, phase);
@@ -284,7 +321,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                         for (int k = 0; k < WL; ++k) {
                             const int rl = (k * W + warp) * RPL + grp;
                             float2 vj = ptx::lds64(vbase + rl * 8);
-                            if constexpr (I16) { vj.x *= sc; vj.y *= sc; }
+                            if constexpr (I16 || GEN) { vj.x *= sc; vj.y *= sc; }
 #pragma unroll
                             for (int ps = 0; ps < PASSES; ++ps) {
                                 const uint32_t a = lbase + rl * ROWBYTES + ps * QP * 16;
@@ -326,6 +363,13 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                     const float2 x = red[g * NC + t];
                     sum.x += x.x;
                     sum.y += x.y;
+                }
+                if constexpr (GEN) {
+                    if (p.identity) {
+                        const float2 u = __ldg(p.in_local + (int64_t)s * NC + t);
+                        sum.x = fmaf(p.alpha, u.x, sum.x);
+                        sum.y = fmaf(p.alpha, u.y, sum.y);
+                    }
                 }
                 p.out[(int64_t)s * NC + t] = sum;
             }
