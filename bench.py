@@ -472,6 +472,70 @@ def run_ours(args, cfg, daggers):
     return 0
 
 
+# ------------------------------------------------------------------------------- even/odd workload
+def run_schur(args, cfg):
+    """--workload schur (not the default bench line): the left-preconditioned
+    Schur operator on block-preconditioned links, Shat_e v = v - Dhat_eo Dhat_oe v, and its adjoint.
+    One step = Shat_e.v then Shat_e^H.v = 4 parity-restricted hop launches of V/2 sites each."""
+    import paper_2212_12559_b200 as cop
+    world, rank, local = dist_env()
+    if world > 1:
+        raise RuntimeError("--workload schur is a single-GPU measurement")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dims, Nc = cfg["dims"], cfg["Nc"]
+    V = synth.lattice_volume(dims)
+    prec = cop.LINK_I16 if cfg["links"] == "i16" else cop.LINK_C64
+    links = synth.make_arbitrary_links(dims, Nc, cfg["seed"], device=dev)      # stands in for Yhat = X^-1 Y
+    scales = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device=dev)
+        scales = torch.empty((V, 9), dtype=torch.float32, device=dev)
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        torch.cuda.synchronize()
+        links = q
+    v = synth.make_vectors(dims, Nc, 1, cfg["seed"] + 1, device=dev)
+    t, out = torch.zeros_like(v), torch.zeros_like(v)
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    stream = torch.cuda.current_stream()
+
+    def schur(dagger):
+        op.apply_parts(None, v, t, dagger=dagger, parity=cop.PARITY_ODD, local=cop.LOCAL_NONE, alpha=0.0, beta=1.0)
+        op.apply_parts(v, t, out, dagger=dagger, parity=cop.PARITY_EVEN, local=cop.LOCAL_IDENTITY, alpha=1.0, beta=-1.0)
+
+    for _ in range(max(args.warmup, 3)):
+        schur(0); schur(1)
+    torch.cuda.synchronize()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    with ClockSampler(local) as clocks:
+        for e in ev:
+            e[0].record(stream); schur(0); e[1].record(stream); schur(1); e[2].record(stream)
+        torch.cuda.synchronize()
+    total_ms = ev[0][0].elapsed_time(ev[-1][2])
+    ms0 = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps
+    ms1 = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps
+    link_site = 8 * Nc * Nc * (8 if prec == cop.LINK_C64 else 4) + (32 if prec == cop.LINK_I16 else 0)
+    bytes_schur = (V // 2) * (2 * link_site + (8 + 1 + 8 + 1 + 1) * Nc * 8)     # hop: 8 reads + 1 write; xpay hop: + u
+    peak, peak_src = measured_peak_gbs()
+    line = {
+        "metric": METRIC, "value": 2.0 * V * args.steps / (total_ms * 1e-3), "unit": UNIT, "n_gpus": 1,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "even/odd Schur-hat operator (v - Dhat_eo Dhat_oe v) and its adjoint on the %s lattice, "
+                               "Nc=%d, %s links: 4 parity-restricted hop launches of V/2 sites per step" %
+                               ("x".join(map(str, dims)), Nc, cfg["links"]), "seed": cfg["seed"]},
+        "clocks": clocks.summary(), "gpu_launches": 4 * args.steps,
+        "roofline": {"bound": "hbm", "achieved": bytes_schur / (ms0 * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": bytes_schur / (ms0 * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                     "kernel": "2 x coarse_apply_stream<GEN> (hop to odd, identity - hop to even)",
+                     "schur_ms": ms0, "schur_dagger_ms": ms1, "algorithmic_bytes_per_schur_apply": bytes_schur,
+                     "dagger_achieved": bytes_schur / (ms1 * 1e-3) / 1e9},
+    }
+    print(json.dumps(line), flush=True)
+    op.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -479,6 +543,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--workload", default="apply", choices=["apply", "schur"],
+                    help="apply: the BASELINE metric (default); schur: the even/odd Schur-hat operator (row f1)")
     ap.add_argument("--dagger", default="both", choices=["0", "1", "both"])
     ap.add_argument("--path", type=int, default=0, help="COARSE_PATH_* override (0 = auto)")
     ap.add_argument("--stages", type=int, default=0, help="COARSE_OPT_STAGES override (0 = library default)")
@@ -492,6 +558,8 @@ def main():
     args = ap.parse_args()
     cfg = synth.config(args.config)
     daggers = [0, 1] if args.dagger == "both" else [int(args.dagger)]
+    if args.workload == "schur":
+        return run_schur(args, cfg)
     if args.impl == "reference":
         return run_reference(args, cfg, daggers)
     return run_ours(args, cfg, daggers)

@@ -232,6 +232,15 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
             float2 acc[WL];
 #pragma unroll
             for (int k = 0; k < WL; ++k) acc[k] = make_float2(0.f, 0.f);
+            // identity local term: fetch u(x) for this lane's rows now, so that the L2 latency hides
+            // behind the item's stages instead of stalling the warp in front of the store
+            float2 uloc[GEN ? WL : 1];
+            if constexpr (GEN) {
+#pragma unroll
+                for (int k = 0; k < WL; ++k)
+                    uloc[k] = p.identity ? __ldg(p.in_local + (int64_t)s * NC + rb * RS + (k * W + warp) * RPL + grp)
+                                         : make_float2(0.f, 0.f);
+            }
 #pragma unroll 1
             for (int m = M0; m < 9; ++m) {
                 float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
@@ -292,16 +301,22 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                 if (qi == 0) {
                     const int row = rb * RS + (k * W + warp) * RPL + grp;
                     if constexpr (GEN) {
-                        if (p.identity) {
-                            const float2 u = __ldg(p.in_local + (int64_t)s * NC + row);
-                            acc[k].x = fmaf(p.alpha, u.x, acc[k].x);
-                            acc[k].y = fmaf(p.alpha, u.y, acc[k].y);
-                        }
+                        acc[k].x = fmaf(p.alpha, uloc[k].x, acc[k].x);
+                        acc[k].y = fmaf(p.alpha, uloc[k].y, acc[k].y);
                     }
                     p.out[(int64_t)s * NC + row] = acc[k];
                 }
             }
         } else {
+            constexpr int UL = (NC + W * 32 - 1) / (W * 32);
+            float2 uloc[GEN ? UL : 1];
+            if constexpr (GEN) {
+#pragma unroll
+                for (int k = 0; k < UL; ++k) {
+                    const int t = threadIdx.x + k * W * 32;
+                    uloc[k] = (p.identity && t < NC) ? __ldg(p.in_local + (int64_t)s * NC + t) : make_float2(0.f, 0.f);
+                }
+            }
             float2 acc[PASSES][CPQ];
 #pragma unroll
             for (int ps = 0; ps < PASSES; ++ps)
@@ -356,7 +371,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                         red[(warp * RPL + grp) * NC + (ps * QP + qi) * CPQ + e] = acc[ps][e];
             }
             ptx::named_bar_sync(1, W * 32);
-            for (int t = threadIdx.x; t < NC; t += W * 32) {
+            for (int t = threadIdx.x, ku = 0; t < NC; t += W * 32, ++ku) {
                 float2 sum = make_float2(0.f, 0.f);
 #pragma unroll
                 for (int g = 0; g < W * RPL; ++g) {
@@ -365,11 +380,8 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                     sum.y += x.y;
                 }
                 if constexpr (GEN) {
-                    if (p.identity) {
-                        const float2 u = __ldg(p.in_local + (int64_t)s * NC + t);
-                        sum.x = fmaf(p.alpha, u.x, sum.x);
-                        sum.y = fmaf(p.alpha, u.y, sum.y);
-                    }
+                    sum.x = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].x, sum.x);
+                    sum.y = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].y, sum.y);
                 }
                 p.out[(int64_t)s * NC + t] = sum;
             }
