@@ -159,6 +159,11 @@ CONFIGS = {
     "C3": dict(dims=(8, 8, 8, 12), Nc=128, links="c64", nrhs=1, seed=20221203),
     "C4": dict(dims=(16, 16, 16, 24), Nc=64, links="i16", nrhs=1, seed=20221204),
     "C5": dict(dims=(8, 8, 8, 12), Nc=128, links="c64", nrhs=16, seed=20221205),
+    # The paper's own per-GPU coarse volumes (not BASELINE configs, derived from
+    # PAPER.md:L117/L125/L133 Table 1): local 24x48x24x36 / aggregate 4x6x6x6 = 6x8x4x6 sites at
+    # level 2 (Nc = 64x2), / 3x2x2x3 = 2x4x2x2 sites at level 3 (Nc = 96x2); int16 links (L99).
+    "P2": dict(dims=(6, 8, 4, 6), Nc=128, links="i16", nrhs=1, seed=20221206),
+    "P3": dict(dims=(2, 4, 2, 2), Nc=192, links="i16", nrhs=1, seed=20221207),
 }
 
 
