@@ -149,6 +149,12 @@ int coarse_op_last_path(const coarse_op_t* op);
 int coarse_op_quantize_i16(const void* links_c64_dev, int64_t n_matrices, int Nc, void* q_dev,
                            float* scales_dev, void* stream);
 
+/* Diagnostic: stream floor(bytes / stage_bytes) * stage_bytes bytes of device memory through the STREAM
+ * kernels' TMA ring (one CTA per SM, `stages` slots of `stage_bytes`, evict_first bulk copies) with an
+ * idle consumer.  Timed by the caller with CUDA events it gives the pure-read ceiling of this GPU for
+ * the access pattern of the apply; bench.py reports it beside the roofline. */
+int coarse_op_probe_read(const void* src_dev, size_t bytes, int stage_bytes, int stages, void* stream);
+
 void coarse_op_destroy(coarse_op_t* op); /* NULL is a no-op */
 
 const char* coarse_op_last_error(void); /* thread-local, never NULL */

@@ -26,7 +26,7 @@ LOCAL_NONE, LOCAL_X, LOCAL_IDENTITY = 0, 1, 2
 EXPORTS = (
     "coarse_op_create", "coarse_op_link_bytes", "coarse_op_scale_bytes", "coarse_op_vector_bytes",
     "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_parts", "coarse_op_apply_host",
-    "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_destroy",
+    "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_probe_read", "coarse_op_destroy",
     "coarse_op_last_error",
 )
 
@@ -73,6 +73,8 @@ def lib() -> ctypes.CDLL:
     L.coarse_op_last_path.argtypes = [vp]
     L.coarse_op_quantize_i16.restype = ci
     L.coarse_op_quantize_i16.argtypes = [vp, ci64, ci, vp, vp, vp]
+    L.coarse_op_probe_read.restype = ci
+    L.coarse_op_probe_read.argtypes = [vp, sz, ci, ci, vp]
     L.coarse_op_destroy.restype = None
     L.coarse_op_destroy.argtypes = [vp]
     L.coarse_op_last_error.restype = ctypes.c_char_p
@@ -196,6 +198,15 @@ def coarse_op_quantize_i16(links_c64, Nc: int, q_out, scales_out, stream=None) -
             raise ValueError("quantize_i16 needs contiguous CUDA tensors")
     _check(lib().coarse_op_quantize_i16(_ptr(links_c64), n, int(Nc), _ptr(q_out), _ptr(scales_out),
                                         _stream_handle(stream)))
+
+
+def coarse_op_probe_read(src, stage_bytes: int = 16384, stages: int = 6, stream=None) -> int:
+    """Enqueue the read-ceiling probe over the CUDA tensor `src`; returns the bytes it reads."""
+    if not src.is_cuda or not src.is_contiguous():
+        raise ValueError("probe_read needs a contiguous CUDA tensor")
+    nbytes = src.numel() * src.element_size()
+    _check(lib().coarse_op_probe_read(_ptr(src), nbytes, int(stage_bytes), int(stages), _stream_handle(stream)))
+    return (nbytes // stage_bytes) * stage_bytes
 
 
 def coarse_op_destroy(op: int) -> None:

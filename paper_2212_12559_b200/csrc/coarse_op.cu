@@ -16,6 +16,7 @@
 #include "stream_kernel.cuh"
 #include "block_kernel.cuh"
 #include "tensor_kernel.cuh"
+#include "probe_kernel.cuh"
 
 using namespace coarse;
 
@@ -605,6 +606,29 @@ int coarse_op_quantize_i16(const void* links_c64_dev, int64_t n_matrices, int Nc
         static_cast<const float*>(links_c64_dev), n_matrices, Nc, static_cast<short*>(q_dev), scales_dev);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "quantize kernel launch");
+    return COARSE_OK;
+}
+
+int coarse_op_probe_read(const void* src_dev, size_t bytes, int stage_bytes, int stages, void* stream) {
+    if (!src_dev || !aligned16(src_dev)) return fail(COARSE_EINVAL, "probe_read: src_dev must be a 16-byte aligned device pointer");
+    if (stage_bytes < 1024 || (stage_bytes & 15) || stages < 2 || stages > 32)
+        return fail(COARSE_EINVAL, "probe_read: stage_bytes must be a multiple of 16 >= 1024 and 2 <= stages <= 32");
+    int dev = 0, sms = 0, max_smem = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "probe_read: cudaGetDevice");
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    const int smem = stages * (stage_bytes + 16) + 64;
+    if (smem > max_smem) return fail(COARSE_EINVAL, "probe_read: %d stages of %d bytes do not fit shared memory", stages, stage_bytes);
+    const unsigned long long n_stages = bytes / (size_t)stage_bytes;
+    if (n_stages < 1) return fail(COARSE_EINVAL, "probe_read: fewer bytes than one stage");
+    e = cudaFuncSetAttribute(probe_read_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(probe kernel)");
+    const int grid = n_stages < (unsigned long long)sms ? (int)n_stages : sms;
+    probe_read_kernel<<<grid, 64, smem, static_cast<cudaStream_t>(stream)>>>(static_cast<const unsigned char*>(src_dev),
+                                                                           n_stages, stage_bytes, stages, nullptr);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "probe kernel launch");
     return COARSE_OK;
 }
 

@@ -251,6 +251,18 @@ def test_apply_is_graph_capturable(oracle_lib):
     op.close()
 
 
+def test_read_probe_runs_and_validates_arguments():
+    buf = torch.zeros(64 << 20, dtype=torch.uint8, device="cuda")
+    assert cop.coarse_op_probe_read(buf, 16384, 6) == 64 << 20
+    assert cop.coarse_op_probe_read(buf[: 100000], 16384, 2) == 6 * 16384
+    torch.cuda.synchronize()
+    L = cop.lib()
+    assert L.coarse_op_probe_read(buf.data_ptr(), 1 << 20, 1000, 6, None) == cop.EINVAL
+    assert L.coarse_op_probe_read(buf.data_ptr(), 1 << 20, 65536, 8, None) == cop.EINVAL     # does not fit smem
+    assert L.coarse_op_probe_read(None, 1 << 20, 16384, 6, None) == cop.EINVAL
+    assert L.coarse_op_probe_read(buf.data_ptr(), 100, 16384, 6, None) == cop.EINVAL
+
+
 def test_bit_reproducible():
     dims, Nc = (4, 4, 4, 6), 64
     links = synth.make_gamma_hermitian_links(dims, Nc, 5, device="cuda")
