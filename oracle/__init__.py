@@ -52,6 +52,10 @@ def _load() -> ctypes.CDLL:
         lib.oracle_coarse_apply_parts.restype = ci
         lib.oracle_coarse_apply_parts.argtypes = [i4, ci, ci, vp, vp, vp, vp, vp, ci, ci, ci, ci,
                                                   ctypes.c_double, ctypes.c_double, ci]
+        lib.oracle_coarse_apply_hvec.restype = ci
+        lib.oracle_coarse_apply_hvec.argtypes = [i4, ci, ci, vp, vp, vp, vp, vp, ci, ci, ci]
+        lib.oracle_quantize_vec_i16.restype = ci
+        lib.oracle_quantize_vec_i16.argtypes = [vp, ci64, ci, ci, vp, vp]
         lib.oracle_neighbours.restype = ci
         lib.oracle_neighbours.argtypes = [i4, ci64, vp]
         lib.oracle_quantize_i16.restype = ci
@@ -253,3 +257,37 @@ def schur_hat_apply(dims, Nc: int, hat, v, parity: int, nrhs: int = 1, dagger: i
     t = coarse_apply_parts(dims, Nc, hat, None, vp, nrhs, dagger, q, LOCAL_NONE, 0.0, 1.0)
     return coarse_apply_parts(dims, Nc, hat, vp, t.astype(np.complex64), nrhs, dagger, parity,
                               LOCAL_IDENTITY, 1.0, -1.0)
+
+
+# ----------------------------------------------------------------------------- half vectors (row f2)
+def quantize_vec_i16(v, Nc: int, nrhs: int = 1):
+    """O8 quantiser. v: complex64 [V][Nc][nrhs]; returns (int16 [V][Nc][nrhs][2], float32 [V][nrhs])."""
+    a = _as_vec(v, np.asarray(v).size // (Nc * nrhs), Nc, nrhs)
+    V = a.size // (2 * Nc * nrhs)
+    q = np.empty((V, Nc, nrhs, 2), dtype=np.int16)
+    norms = np.empty((V, nrhs), dtype=np.float32)
+    rc = _load().oracle_quantize_vec_i16(a.ctypes.data, V, Nc, nrhs, q.ctypes.data, norms.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_quantize_vec_i16 rejected its arguments")
+    return q, norms
+
+
+def coarse_apply_hvec(dims, Nc: int, links, vec_q, vec_norms, nrhs: int = 1, dagger: int = 0,
+                      link_precision: int = LINK_C64, scales=None, nthreads: int = 0) -> np.ndarray:
+    """O8: full apply on half-precision input vectors (int16 + per-(site,rhs) norm); complex128 out."""
+    V = int(np.prod([int(d) for d in dims]))
+    L = _as_links(links, link_precision, V, Nc)
+    q = np.ascontiguousarray(np.asarray(vec_q, dtype=np.int16))
+    nm = np.ascontiguousarray(np.asarray(vec_norms, dtype=np.float32))
+    if q.size != V * Nc * nrhs * 2 or nm.size != V * nrhs:
+        raise ValueError("half vectors must be int16 [V][Nc][nrhs][2] with float32 norms [V][nrhs]")
+    sc = None
+    if link_precision == LINK_I16:
+        sc = np.ascontiguousarray(np.asarray(scales, dtype=np.float32))
+    out = np.empty((V, Nc, nrhs), dtype=np.complex128)
+    rc = _load().oracle_coarse_apply_hvec(_dims(dims), Nc, link_precision, L.ctypes.data,
+                                          sc.ctypes.data if sc is not None else None, q.ctypes.data,
+                                          nm.ctypes.data, out.ctypes.data, nrhs, dagger, nthreads)
+    if rc != 0:
+        raise ValueError(f"oracle_coarse_apply_hvec rejected its arguments (rc={rc})")
+    return out

@@ -38,6 +38,10 @@
 //        block-preconditioned form are compositions of O7 written out in
 //        oracle/__init__.py (schur_apply, schur_hat_apply) with numpy's dense solve as a step.
 //
+//   O8 (half-precision input vectors) PAPER.md:L97: "half precision" =
+//        16-bit fixed point with a per-site fp32 norm.  Entry = norm[s][r] * (q_re + i q_im),
+//        promoted in double before the same loops run; quantiser as O5 with one norm per (site, rhs).
+//
 // Layouts (identical to include/coarse_op.h because both take the caller's arrays):
 //   site index s(x) = x0 + L0*(x1 + L1*(x2 + L2*x3)); periodic wrap by modulo, so an
 //   extent-2 direction adds both hops from the same neighbour and an extent-1 direction
@@ -101,6 +105,27 @@ inline void link_entry(int prec, const void* links, const float* scales, int Nc,
     }
 }
 
+// Half-precision input vectors (O8; "half precision ... 16-bit
+// fixed point with a per-site fp32 norm"): when hv_q is set, the vector entry is
+// (double)q[s][j][r] * (double)norm[s][r] instead of the float array handed to accumulate.
+struct HalfVec {
+    const int16_t* q = nullptr;     // int16 [V][Nc][nrhs][2]
+    const float* norms = nullptr;   // float [V][nrhs]
+};
+thread_local HalfVec g_hv;
+
+inline void vec_entry(const float* in, int Nc, int nrhs, int64_t sv, int j, int r, double& re, double& im) {
+    const int64_t v = ((sv * Nc + j) * nrhs + r) * 2;
+    if (g_hv.q) {
+        const double n = (double)g_hv.norms[sv * nrhs + r];
+        re = (double)g_hv.q[v] * n;
+        im = (double)g_hv.q[v + 1] * n;
+    } else {
+        re = (double)in[v];
+        im = (double)in[v + 1];
+    }
+}
+
 // acc[i][r] += sum_j M(sm,m)_ij * in[sv][j][r]          (conj_transpose == 0)
 // acc[i][r] += sum_j conj(M(sm,m)_ji) * in[sv][j][r]    (conj_transpose == 1)
 void accumulate(int prec, const void* links, const float* scales, int Nc, int nrhs,
@@ -115,8 +140,8 @@ void accumulate(int prec, const void* links, const float* scales, int Nc, int nr
                 mim = -mim;
             }
             for (int r = 0; r < nrhs; ++r) {
-                const int64_t v = ((sv * Nc + j) * nrhs + r) * 2;
-                const double vre = (double)in[v], vim = (double)in[v + 1];
+                double vre, vim;
+                vec_entry(in, Nc, nrhs, sv, j, r, vre, vim);
                 acc[(i * nrhs + r) * 2 + 0] += mre * vre - mim * vim;
                 acc[(i * nrhs + r) * 2 + 1] += mre * vim + mim * vre;
             }
@@ -270,6 +295,57 @@ int oracle_coarse_apply_parts(const int dims[4], int Nc, int link_precision, con
         }
         delete[] tmp;
     }
+    return 0;
+}
+
+// O8: the full apply (O1/O2) on half-precision INPUT vectors: in(x)_jr = q[x][j][r] * norm[x][r].
+// Output complex128 as always.
+int oracle_coarse_apply_hvec(const int dims[4], int Nc, int link_precision, const void* links,
+                             const float* scales, const int16_t* in_q, const float* in_norms, double* out,
+                             int nrhs, int dagger, int nthreads) {
+    if (!valid(dims, Nc, link_precision, nrhs, dagger) || !links || !in_q || !in_norms || !out) return -1;
+    if (link_precision == 1 && !scales) return -1;
+    Lattice lat{{dims[0], dims[1], dims[2], dims[3]}, (int64_t)dims[0] * dims[1] * dims[2] * dims[3]};
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#pragma omp parallel num_threads(nthreads)
+#endif
+    {
+        g_hv.q = in_q;
+        g_hv.norms = in_norms;
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+        for (int64_t s = 0; s < lat.V; ++s)
+            apply_site(lat, Nc, link_precision, links, scales, nullptr, nrhs, dagger, s,
+                       out + s * 2 * (int64_t)Nc * nrhs);
+        g_hv = HalfVec();
+    }
+    return 0;
+}
+
+// O8 quantiser for vectors: one fp32 norm per (site, right-hand side),
+//   amax = max over the 2*Nc real components of |component|, norm = amax / 32767.0f,
+//   q = (int16) clamp(nearbyintf(component / norm), -32767, 32767); amax == 0 => norm = 0, q = 0.
+// v: float [n_sites][Nc][nrhs][2]; q: int16 same shape; norms: float [n_sites][nrhs].
+int oracle_quantize_vec_i16(const float* v, int64_t n_sites, int Nc, int nrhs, int16_t* q, float* norms) {
+    if (!v || !q || !norms || n_sites < 0 || Nc < 1 || nrhs < 1) return -1;
+    for (int64_t s = 0; s < n_sites; ++s)
+        for (int r = 0; r < nrhs; ++r) {
+            float amax = 0.0f;
+            for (int a = 0; a < Nc; ++a)
+                for (int c = 0; c < 2; ++c) amax = std::max(amax, std::fabs(v[((s * Nc + a) * nrhs + r) * 2 + c]));
+            const float norm = amax == 0.0f ? 0.0f : amax / 32767.0f;
+            norms[s * nrhs + r] = norm;
+            for (int a = 0; a < Nc; ++a)
+                for (int c = 0; c < 2; ++c) {
+                    const int64_t e = ((s * Nc + a) * nrhs + r) * 2 + c;
+                    if (amax == 0.0f) { q[e] = 0; continue; }
+                    float t = nearbyintf(v[e] / norm);
+                    t = std::min(32767.0f, std::max(-32767.0f, t));
+                    q[e] = (int16_t)t;
+                }
+        }
     return 0;
 }
 
