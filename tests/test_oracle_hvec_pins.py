@@ -20,7 +20,8 @@ def test_vector_quantiser_properties(oracle_lib):
     assert np.all(q[3] == 0) and np.all(norms[3] == 0)
     assert np.abs(q).max() <= 32767 and q.min() >= -32767
     deq = q.astype(np.float64) * norms[:, None, :, None].astype(np.float64)
-    assert np.all(np.abs(deq - vr) <= 0.503 * norms[:, None, :, None] + 1e-45   # 0.5 + the fp32 division's rounding (32767 * 2^-24))
+    # 0.5 from rounding + the fp32 division's own rounding (32767 * 2^-24 = 0.002)
+    assert np.all(np.abs(deq - vr) <= 0.503 * norms[:, None, :, None] + 1e-45)
     # the largest component of every (site, rhs) maps to +-32767
     assert np.all((np.abs(q).max(axis=(1, 3)) == 32767) | (amax == 0))
     # idempotent on dequantised data
