@@ -53,9 +53,12 @@ NCU_TRAFFIC_BYTES = {
 }
 
 
-def compulsory_bytes_per_site(Nc: int, links: str, nrhs: int) -> int:
-    """SURVEY.md §8(d) / north_star: 9 Nc^2 link entries + 9 input vectors + 1 output vector."""
+def compulsory_bytes_per_site(Nc: int, links: str, nrhs: int, hvec: bool = False) -> int:
+    """SURVEY.md §8(d) / north_star: 9 Nc^2 link entries + 9 input vectors + 1 output vector.
+    hvec: the 9 input vectors are int16 (re,im) + one fp32 norm per (site, rhs)."""
     link = 9 * Nc * Nc * (8 if links == "c64" else 4) + (36 if links == "i16" else 0)
+    if hvec:
+        return link + 9 * (Nc * nrhs * 4 + nrhs * 4) + Nc * nrhs * 8
     return link + 10 * Nc * nrhs * 8
 
 
@@ -245,9 +248,10 @@ def run_reference(args, cfg, daggers):
     return 0
 
 
-def workload_name(name, cfg):
+def workload_name(name, cfg, hvec=False):
     return (f"{name}: coarse-op apply, {'x'.join(map(str, cfg['dims']))} periodic lattice, Nc={cfg['Nc']}, "
-            f"{cfg['links']} links, complex64 vectors, nrhs={cfg['nrhs']}")
+            f"{cfg['links']} links, {'int16+norm input / complex64 output' if hvec else 'complex64'} vectors, "
+            f"nrhs={cfg['nrhs']}")
 
 
 # ------------------------------------------------------------------------------- GPU arm
@@ -289,6 +293,19 @@ def run_ours(args, cfg, daggers):
     if args.keep_links:
         op.set_option(cop.OPT_KEEP_LINKS, args.keep_links)
 
+    vq = vnorm = None
+    if args.hvec:
+        vq = torch.empty((V, Nc, nrhs, 2), dtype=torch.int16, device=dev)
+        vnorm = torch.empty((V, nrhs), dtype=torch.float32, device=dev)
+        cop.coarse_op_quantize_vec_i16(vin, Nc, nrhs, vq, vnorm)
+        torch.cuda.synchronize()
+
+    def apply_one(out, dg):
+        if args.hvec:
+            op.apply_hvec(vq, vnorm, out, nrhs=nrhs, dagger=dg)
+        else:
+            op.apply(vin, out, nrhs=nrhs, dagger=dg)
+
     stream = torch.cuda.current_stream()
     launches = 0
     link_bytes = links.numel() * links.element_size()
@@ -305,7 +322,7 @@ def run_ours(args, cfg, daggers):
                 e0 = torch.cuda.Event(enable_timing=True)
                 e1 = torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
-            op.apply(vin, vouts[k], nrhs=nrhs, dagger=dg)
+            apply_one(vouts[k], dg)
             launches += op.last_launches
             if record is not None:
                 e1.record(stream)
@@ -339,7 +356,7 @@ def run_ours(args, cfg, daggers):
         launches = 0
         g_steps = capture(lambda: [step() for _ in range(args.steps)])
         gpu_launches = launches
-        g_one = {dg: capture(lambda dg=dg: [op.apply(vin, vouts[i], nrhs=nrhs, dagger=dg)
+        g_one = {dg: capture(lambda dg=dg, i=i: [apply_one(vouts[i], dg)
                                              for _ in range(args.steps)])
                  for i, dg in enumerate(daggers)}
         barrier()
@@ -426,12 +443,12 @@ def run_ours(args, cfg, daggers):
         return 0
 
     peak, peak_src = measured_peak_gbs()
-    bps = compulsory_bytes_per_site(Nc, cfg["links"], nrhs)
+    bps = compulsory_bytes_per_site(Nc, cfg["links"], nrhs, args.hvec)
     dom = daggers[0]
     achieved = bps * V / (kernel_ms[dom] * 1e-3) / 1e9
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": NCU_TRAFFIC_BYTES.get((args.config, op.last_path, dom)),
+        "traffic": None if args.hvec else NCU_TRAFFIC_BYTES.get((args.config, op.last_path, dom)),
         "kernel": "coarse_apply_%s<Nc=%d,%s,dagger=%d%s>" % (
             {cop.PATH_SIMPLE: "simple", cop.PATH_STREAM: "stream", cop.PATH_TENSOR: "tensor",
              cop.PATH_BLOCK: "block"}.get(op.last_path, "?"), Nc, "i16" if prec else "c64", dom,
@@ -468,7 +485,7 @@ def run_ours(args, cfg, daggers):
         "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {
-            "workload": workload_name(args.config, cfg),
+            "workload": workload_name(args.config, cfg, args.hvec),
             "step": f"one apply per dagger in {daggers} (2V site-updates)" if len(daggers) == 2 else f"one apply, dagger={daggers[0]}",
             "l2": "inputs larger than L2 (links %.2f GB per apply, no flush needed)" % (links.numel() * links.element_size() / 1e9)
                   if link_bytes > 4 * 126e6 else "working set fits L2: `value` is the warm-L2 number (CUDA graph of all K steps); roofline quotes the cold one",
@@ -576,6 +593,8 @@ def main():
     ap.add_argument("--keep-links", type=int, default=0, help="COARSE_OPT_KEEP_LINKS override (0 auto, 1 never, 2 always)")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="time all K steps as one CUDA graph (auto: when the links fit 2x L2)")
+    ap.add_argument("--hvec", action="store_true",
+                    help="half-precision INPUT vectors (int16 + per-site norm, row f2) through coarse_op_apply_hvec")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     args = ap.parse_args()

@@ -130,6 +130,22 @@ enum { COARSE_LOCAL_NONE = 0, COARSE_LOCAL_X = 1, COARSE_LOCAL_IDENTITY = 2 };
 int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev, void* out_dev, int nrhs,
                           int dagger, int parity, int local, float alpha, float beta, void* stream);
 
+/* The plain apply on HALF-PRECISION input vectors ("half precision" = 16-bit fixed
+ * point with a per-site fp32 norm): in(x)_jr = in_norms[x][r] * (q_re + i q_im), in_q_dev =
+ * int16_t[V][Nc][nrhs][2], in_norms_dev = float[V][nrhs].  The output stays complex64 (a site's rows
+ * are produced by several CTAs, so the per-site norm of the result is taken by a separate
+ * coarse_op_quantize_vec_i16 when a half-precision result is wanted).  Nc % 4 == 0.
+ * nrhs = 1 runs on the STREAM kernels (the norm is folded into the vector operand like the int16
+ * link scale), other nrhs on SIMPLE. */
+int coarse_op_apply_hvec(coarse_op_t* op, const void* in_q_dev, const float* in_norms_dev, void* out_dev, int nrhs,
+                         int dagger, void* stream);
+
+/* Vector quantiser: for each (site, rhs) norm = max|component|/32767 (fp32 division) and
+ * q = clamp(rint(component/norm), -32767, 32767); an all-zero vector gets norm 0 and q = 0.
+ * v_c64_dev: float[n_sites][Nc][nrhs][2]; q_dev: int16_t same shape; norms_dev: float[n_sites][nrhs]. */
+int coarse_op_quantize_vec_i16(const void* v_c64_dev, int64_t n_sites, int Nc, int nrhs, void* q_dev,
+                               float* norms_dev, void* stream);
+
 /* Same operation on HOST vectors: copies in_host to a device staging buffer owned by the handle
  * (allocated on first use, grown when nrhs grows), applies, copies the result to out_host and
  * synchronises the stream before returning.  Pinned host memory gives full PCIe rate. */

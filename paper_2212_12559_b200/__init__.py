@@ -25,7 +25,8 @@ LOCAL_NONE, LOCAL_X, LOCAL_IDENTITY = 0, 1, 2
 
 EXPORTS = (
     "coarse_op_create", "coarse_op_link_bytes", "coarse_op_scale_bytes", "coarse_op_vector_bytes",
-    "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_parts", "coarse_op_apply_host",
+    "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_parts", "coarse_op_apply_hvec",
+    "coarse_op_quantize_vec_i16", "coarse_op_apply_host",
     "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_probe_read", "coarse_op_destroy",
     "coarse_op_last_error",
 )
@@ -65,6 +66,10 @@ def lib() -> ctypes.CDLL:
     L.coarse_op_apply.argtypes = [vp, vp, vp, ci, ci, vp]
     L.coarse_op_apply_parts.restype = ci
     L.coarse_op_apply_parts.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ctypes.c_float, ctypes.c_float, vp]
+    L.coarse_op_apply_hvec.restype = ci
+    L.coarse_op_apply_hvec.argtypes = [vp, vp, vp, vp, ci, ci, vp]
+    L.coarse_op_quantize_vec_i16.restype = ci
+    L.coarse_op_quantize_vec_i16.argtypes = [vp, ci64, ci, ci, vp, vp, vp]
     L.coarse_op_apply_host.restype = ci
     L.coarse_op_apply_host.argtypes = [vp, vp, vp, ci, ci, vp]
     L.coarse_op_last_launches.restype = ci
@@ -167,6 +172,33 @@ def coarse_op_apply_parts(op: int, u, w, vout, nrhs: int = 1, dagger: int = 0, p
                                        int(local), float(alpha), float(beta), _stream_handle(stream)))
 
 
+def coarse_op_apply_hvec(op: int, vin_q, vin_norms, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+    """Plain apply on half-precision input vectors: vin_q CUDA int16 [V][Nc][nrhs][2], vin_norms CUDA
+    float32 [V][nrhs]; vout CUDA complex64 [V][Nc][nrhs]."""
+    for t in (vin_q, vin_norms, vout):
+        if not t.is_cuda or not t.is_contiguous():
+            raise ValueError("apply_hvec needs contiguous CUDA tensors")
+    vb = coarse_op_vector_bytes(op, nrhs)
+    if vout.numel() * vout.element_size() != vb or vin_q.numel() * vin_q.element_size() * 2 != vb:
+        raise ValueError("vector tensors have the wrong number of bytes for this operator/nrhs")
+    if vin_norms.numel() % nrhs or vin_norms.element_size() != 4:
+        raise ValueError("vin_norms must hold one float32 per (site, rhs)")
+    _check(lib().coarse_op_apply_hvec(op, _ptr(vin_q), _ptr(vin_norms), _ptr(vout), int(nrhs), int(dagger),
+                                      _stream_handle(stream)))
+
+
+def coarse_op_quantize_vec_i16(v_c64, Nc: int, nrhs: int, q_out, norms_out, stream=None) -> None:
+    """v_c64: CUDA complex64 [V][Nc][nrhs]; q_out: CUDA int16 [V][Nc][nrhs][2]; norms_out: CUDA float32 [V][nrhs]."""
+    n_sites = v_c64.numel() // (Nc * nrhs)
+    if q_out.numel() != 2 * v_c64.numel() or norms_out.numel() != n_sites * nrhs:
+        raise ValueError("quantize_vec_i16: output tensors have the wrong size")
+    for t in (v_c64, q_out, norms_out):
+        if not t.is_cuda or not t.is_contiguous():
+            raise ValueError("quantize_vec_i16 needs contiguous CUDA tensors")
+    _check(lib().coarse_op_quantize_vec_i16(_ptr(v_c64), n_sites, int(Nc), int(nrhs), _ptr(q_out), _ptr(norms_out),
+                                            _stream_handle(stream)))
+
+
 def coarse_op_apply_host(op: int, vin_host, vout_host, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
     """vin_host / vout_host: contiguous CPU complex64 tensors (pinned for full PCIe rate).
     Copies in, applies, copies out and synchronises the stream."""
@@ -241,6 +273,9 @@ class CoarseOp:
     def apply_parts(self, u, w, vout, nrhs: int = 1, dagger: int = 0, parity: int = PARITY_ALL,
                     local: int = LOCAL_X, alpha: float = 1.0, beta: float = 1.0, stream=None) -> None:
         coarse_op_apply_parts(self._h, u, w, vout, nrhs, dagger, parity, local, alpha, beta, stream)
+
+    def apply_hvec(self, vin_q, vin_norms, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+        coarse_op_apply_hvec(self._h, vin_q, vin_norms, vout, nrhs, dagger, stream)
 
     def apply_host(self, vin_host, vout_host, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
         coarse_op_apply_host(self._h, vin_host, vout_host, nrhs, dagger, stream)

@@ -76,13 +76,14 @@ struct PartsSpec {
     int parity;   // 0 even, 1 odd, 2 all
     int local;    // 0 none, 1 X, 2 identity
     float alpha, beta;
+    const float* vnorms;   // non-NULL: half-precision input vectors (plain apply only)
 };
-const PartsSpec kPlain = {false, nullptr, 2, 1, 1.f, 1.f};
+const PartsSpec kPlain = {false, nullptr, 2, 1, 1.f, 1.f, nullptr};
 
 // ---------------------------------------------------------------- STREAM dispatch
-template <int NC, bool I16, bool DAG, bool FINE, bool GEN>
+template <int NC, bool I16, bool DAG, bool FINE, bool GEN, bool HV = false>
 int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
-    using Gm = StreamGeom<NC, I16, FINE>;
+    using Gm = StreamGeom<NC, I16, FINE, HV>;
     static_assert(Gm::OK, "unsupported STREAM geometry");
     StreamParams p = base;
     p.n_items = DAG ? p.n_sites : p.n_sites * Gm::NB;
@@ -97,7 +98,7 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     if (stages > want) stages = want;
     p.stages = stages;
     const int smem = Gm::smem_bytes(DAG, stages);
-    auto kern = coarse_apply_stream<NC, I16, DAG, FINE, GEN>;
+    auto kern = coarse_apply_stream<NC, I16, DAG, FINE, GEN, HV>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
@@ -132,6 +133,13 @@ int launch_stream_nc(const coarse_op* op, const StreamParams& p, int dagger, cud
 
 template <int NC>
 int launch_stream_g(const coarse_op* op, const StreamParams& p, int dagger, bool gen, cudaStream_t stream) {
+    if (p.vnorms) {   // half-precision input vectors: regular geometry, plain apply
+        if (op->prec == COARSE_LINK_I16)
+            return dagger ? launch_stream_t<NC, true, true, false, false, true>(op, p, stream)
+                          : launch_stream_t<NC, true, false, false, false, true>(op, p, stream);
+        return dagger ? launch_stream_t<NC, false, true, false, false, true>(op, p, stream)
+                      : launch_stream_t<NC, false, false, false, false, true>(op, p, stream);
+    }
     return gen ? launch_stream_nc<NC, true>(op, p, dagger, stream) : launch_stream_nc<NC, false>(op, p, dagger, stream);
 }
 
@@ -161,6 +169,7 @@ int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, co
     p.identity = ps.local == 2 ? 1 : 0;
     p.parity = ps.parity;
     p.n_sites = ps.parity == 2 ? op->lat.V : op->lat.V / 2;
+    p.vnorms = ps.vnorms;
     switch (op->Nc) {
         case 32: return launch_stream_g<32>(op, p, dagger, ps.gen, stream);
         case 48: return launch_stream_g<48>(op, p, dagger, ps.gen, stream);
@@ -329,6 +338,7 @@ int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int 
     p.beta = ps.beta;
     p.local = ps.local;
     p.parity = ps.parity;
+    p.vnorms = ps.vnorms;
     const int64_t total = (int64_t)op->lat.V * op->Nc * nrhs;
     const int64_t blocks = (total + 255) / 256;
     if (blocks > 0x7fffffffLL) return fail(COARSE_EUNSUPPORTED, "SIMPLE path: problem too large");
@@ -542,7 +552,7 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
     // which the caller cannot express here, so overlap is always refused; u is read at x only and
     // may alias out.
     if (a < b + vb && b < a + vb) return fail(COARSE_EINVAL, "apply_parts: w and out overlap (the stencil reads neighbours)");
-    PartsSpec ps = {true, local != 0 ? u_dev : w_dev, parity, local, alpha, beta};
+    PartsSpec ps = {true, local != 0 ? u_dev : w_dev, parity, local, alpha, beta, nullptr};
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int path = op->path_opt;
     if (path == COARSE_PATH_AUTO || path == COARSE_PATH_TENSOR || path == COARSE_PATH_BLOCK)
@@ -558,6 +568,52 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
     if (rc != COARSE_OK) return rc;
     op->last_launches = 1;
     op->last_path = path;
+    return COARSE_OK;
+}
+
+int coarse_op_apply_hvec(coarse_op_t* op, const void* in_q_dev, const float* in_norms_dev, void* out_dev, int nrhs,
+                         int dagger, void* stream) {
+    int rc = check_apply_args(op, in_q_dev, out_dev, nrhs, dagger);
+    if (rc != COARSE_OK) return rc;
+    if (!in_norms_dev) return fail(COARSE_EINVAL, "apply_hvec: in_norms_dev is NULL");
+    if (!aligned16(in_q_dev) || !aligned16(out_dev) || (reinterpret_cast<uintptr_t>(in_norms_dev) & 3u))
+        return fail(COARSE_EINVAL, "apply_hvec: in_q_dev/out_dev must be 16-byte aligned, in_norms_dev 4-byte aligned");
+    if (op->Nc % 4) return fail(COARSE_EUNSUPPORTED, "apply_hvec: Nc must be a multiple of 4 (got %d)", op->Nc);
+    const size_t vb = coarse_op_vector_bytes(op, nrhs);
+    const uintptr_t a = reinterpret_cast<uintptr_t>(in_q_dev), b = reinterpret_cast<uintptr_t>(out_dev);
+    if (a < b + vb && b < a + vb / 2) return fail(COARSE_EINVAL, "apply_hvec: in and out overlap");
+    PartsSpec ps = kPlain;
+    ps.vnorms = in_norms_dev;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int path = op->path_opt;
+    if (path == COARSE_PATH_AUTO || path == COARSE_PATH_TENSOR || path == COARSE_PATH_BLOCK)
+        path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM : COARSE_PATH_SIMPLE;
+    op->last_launches = 0;
+    if (path == COARSE_PATH_STREAM) {
+        if (!stream_supports(op->Nc, nrhs))
+            return fail(COARSE_EUNSUPPORTED, "apply_hvec: STREAM path does not cover Nc=%d nrhs=%d", op->Nc, nrhs);
+        rc = launch_stream(op, in_q_dev, out_dev, dagger, ps, st);
+    } else {
+        rc = launch_simple(op, in_q_dev, out_dev, nrhs, dagger, ps, st);
+    }
+    if (rc != COARSE_OK) return rc;
+    op->last_launches = 1;
+    op->last_path = path;
+    return COARSE_OK;
+}
+
+int coarse_op_quantize_vec_i16(const void* v_c64_dev, int64_t n_sites, int Nc, int nrhs, void* q_dev,
+                               float* norms_dev, void* stream) {
+    if (!v_c64_dev || !q_dev || !norms_dev) return fail(COARSE_EINVAL, "quantize_vec_i16: NULL pointer");
+    if (n_sites < 0 || Nc < 1 || nrhs < 1) return fail(COARSE_EINVAL, "quantize_vec_i16: bad sizes");
+    if (n_sites == 0) return COARSE_OK;
+    const int64_t total = n_sites * nrhs;
+    const int64_t blocks = (total + 127) / 128;
+    if (blocks > 0x7fffffffLL) return fail(COARSE_EINVAL, "quantize_vec_i16: too many vectors");
+    quantize_vec_i16_kernel<<<(unsigned)blocks, 128, 0, static_cast<cudaStream_t>(stream)>>>(
+        static_cast<const float2*>(v_c64_dev), (long long)n_sites, Nc, nrhs, static_cast<short2*>(q_dev), norms_dev);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "vector quantize kernel launch");
     return COARSE_OK;
 }
 

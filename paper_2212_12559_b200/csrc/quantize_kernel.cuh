@@ -43,4 +43,32 @@ __global__ void __launch_bounds__(256) quantize_i16_kernel(const float* __restri
     }
 }
 
+// Half-precision vectors (16-bit fixed point with a per-site fp32 norm): one thread per
+// (site, right-hand side): norm = max|component| / 32767 (fp32), q = clamp(rint(component / norm)).
+// v: float [n_sites][Nc][nrhs][2]; q: int16 same shape; norms: float [n_sites][nrhs].
+__global__ void __launch_bounds__(128) quantize_vec_i16_kernel(const float2* v, long long n_sites, int Nc, int nrhs,
+                                                               short2* q, float* norms) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n_sites * nrhs) return;
+    const long long s = idx / nrhs;
+    const int r = (int)(idx % nrhs);
+    float amax = 0.f;
+    for (int a = 0; a < Nc; ++a) {
+        const float2 x = v[(s * Nc + a) * nrhs + r];
+        amax = fmaxf(amax, fmaxf(fabsf(x.x), fabsf(x.y)));
+    }
+    const float norm = amax == 0.f ? 0.f : __fdiv_rn(amax, 32767.0f);
+    norms[idx] = norm;
+    for (int a = 0; a < Nc; ++a) {
+        const long long e = (s * Nc + a) * nrhs + r;
+        short2 o = make_short2(0, 0);
+        if (amax != 0.f) {
+            const float2 x = v[e];
+            o.x = (short)fminf(32767.f, fmaxf(-32767.f, rintf(__fdiv_rn(x.x, norm))));
+            o.y = (short)fminf(32767.f, fmaxf(-32767.f, rintf(__fdiv_rn(x.y, norm))));
+        }
+        q[e] = o;
+    }
+}
+
 }  // namespace coarse

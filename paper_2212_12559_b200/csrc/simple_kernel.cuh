@@ -23,6 +23,8 @@ struct SimpleParams {
     float alpha, beta;
     int local;               // 0 none, 1 X, 2 identity
     int parity;              // 0 even, 1 odd, 2 all
+    // half-precision input vectors (coarse_op_apply_hvec): in = int16 (re,im) [V][Nc][nrhs], vnorms[V][nrhs]
+    const float* vnorms;     // NULL: complex64 vectors
 };
 
 template <bool I16>
@@ -70,7 +72,15 @@ __global__ void __launch_bounds__(256) coarse_apply_simple(SimpleParams p) {
                 mim = q.y;
             }
             if (p.dagger) mim = -mim;
-            const float2 v = vin[((int64_t)sv * Nc + j) * p.nrhs + r];
+            float2 v;
+            if (p.vnorms) {
+                v = unpack_i16x2(reinterpret_cast<const uint32_t*>(vin)[((int64_t)sv * Nc + j) * p.nrhs + r]);
+                const float n = p.vnorms[(int64_t)sv * p.nrhs + r];
+                v.x *= n;
+                v.y *= n;
+            } else {
+                v = vin[((int64_t)sv * Nc + j) * p.nrhs + r];
+            }
             part_re = fmaf(mre, v.x, part_re);
             part_re = fmaf(-mim, v.y, part_re);
             part_im = fmaf(mre, v.y, part_im);

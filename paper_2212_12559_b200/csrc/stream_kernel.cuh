@@ -51,6 +51,8 @@ struct StreamParams {
     int identity;             // 1: add alpha*u(x) to the result (local = identity)
     int parity;               // 0 even, 1 odd, 2 all sites
     int n_sites;              // sites in the parity set
+    // HV (half-precision input vectors, coarse_op_apply_hvec): `in` points at int16 (re,im) entries
+    const float* vnorms;      // fp32 norm per site (nrhs = 1)
 };
 
 // Site index of the h-th site of a parity (all extents even, checked by the host): consecutive
@@ -84,7 +86,7 @@ constexpr int stream_rows_per_stage(int nc, int rowbytes, int unit, int max_byte
 // allows, so that V * NB work items still fill 148 SMs when the local volume is a few hundred
 // sites or less ("additional parallelism is exposed in the matrix-vector application
 // to compensate for reduction in parallelism possible by the size of the local volume alone").
-template <int NC, bool I16, bool FINE = false>
+template <int NC, bool I16, bool FINE = false, bool HV = false>
 struct StreamGeom {
     static constexpr int W = 8;                                // consumer warps
     static constexpr int ENTRY_BYTES = I16 ? 4 : 8;            // one complex link entry
@@ -99,8 +101,9 @@ struct StreamGeom {
     static constexpr int NB = NC / RS;                         // row blocks per matrix
     static constexpr int WL = RS / (W * RPL);                  // warp-wide loads per warp, stage, pass
     static constexpr int LINK_STAGE = RS * ROWBYTES;
-    static constexpr int VEC_STAGE_N = NC * 8;                 // dagger = 0: whole neighbour vector
-    static constexpr int VEC_STAGE_D = RS * 8;                 // dagger = 1: the RS entries of the chunk
+    static constexpr int VEC_ENTRY = HV ? 4 : 8;               // complex64, or int16 (re,im) half vectors
+    static constexpr int VEC_STAGE_N = NC * VEC_ENTRY;         // dagger = 0: whole neighbour vector
+    static constexpr int VEC_STAGE_D = RS * VEC_ENTRY;         // dagger = 1: the RS entries of the chunk
     static constexpr int RED_BYTES = 2 * W * RPL * NC * 8;     // dagger = 1: double-buffered partial sums
     static constexpr bool OK = (ROWBYTES % 16 == 0) && PASSES > 0 && RS > 0 && (QP * PASSES == Q);
     static constexpr int THREADS = (W + 1) * 32;
@@ -126,10 +129,12 @@ __device__ __forceinline__ void cmac(float2& acc, float mre, float mim, const fl
     }
 }
 
-template <int NC, bool I16, bool DAG, bool FINE = false, bool GEN = false>
-__global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_apply_stream(StreamParams p) {
+template <int NC, bool I16, bool DAG, bool FINE = false, bool GEN = false, bool HV = false>
+__global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coarse_apply_stream(StreamParams p) {
     static_assert(!(DAG && FINE), "the fine geometry splits output rows: dagger = 0 only");
-    using Gm = StreamGeom<NC, I16, FINE>;
+    static_assert(!(GEN && HV), "half-precision input vectors are implemented for the plain apply");
+    using Gm = StreamGeom<NC, I16, FINE, HV>;
+    constexpr int VE = Gm::VEC_ENTRY;
     constexpr int W = Gm::W, RS = Gm::RS, NB = Gm::NB, WL = Gm::WL, QP = Gm::QP, G = Gm::G, RPL = Gm::RPL;
     constexpr int PASSES = Gm::PASSES, CPQ = Gm::CPQ, ROWBYTES = Gm::ROWBYTES;
     constexpr int LINK_STAGE = Gm::LINK_STAGE;
@@ -174,7 +179,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                 const int sv = stencil_site_x(p.lat, s, cx, m, DAG ? 1 : 0);
                 const int sm = DAG ? sv : s;
                 const unsigned char* mat = p.links + ((int64_t)sm * 9 + m) * ((int64_t)NC * ROWBYTES);
-                const float2* vec = ((GEN && m == 0) ? p.in_local : p.in) + (int64_t)sv * NC;
+                const unsigned char* vec = reinterpret_cast<const unsigned char*>((GEN && m == 0) ? p.in_local : p.in) + (int64_t)sv * NC * VE;
 #pragma unroll 1
                 for (int c = 0; c < (DAG ? NB : 1); ++c) {
                     const int r0 = DAG ? c * RS : rb * RS;
@@ -183,7 +188,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                         ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE + VEC_STAGE);
                         ptx::bulk_g2s(link_u32 + slot * LINK_STAGE, mat + (int64_t)r0 * ROWBYTES, LINK_STAGE,
                                       full0 + 8u * slot, pol_links);
-                        ptx::bulk_g2s(vec_u32 + slot * VEC_STAGE, DAG ? (vec + r0) : vec, VEC_STAGE,
+                        ptx::bulk_g2s(vec_u32 + slot * VEC_STAGE, DAG ? (vec + r0 * VE) : vec, VEC_STAGE,
                                       full0 + 8u * slot, pol_vec);
                     }
                     __syncwarp();
@@ -212,10 +217,14 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
         return (GEN && p.parity != 2) ? parity_site(p.lat, sidx, p.parity) : sidx;
     };
     auto fetch_scale = [&](int item) -> float {
-        if (!I16 || lane >= 9 || item >= p.n_items) return 1.f;
+        if (!(I16 || HV) || lane >= 9 || item >= p.n_items) return 1.f;
         const int s = site_of(item);
-        const int sm = DAG ? stencil_site(p.lat, s, lane, 1) : s;
-        return __ldg(p.scales + (int64_t)sm * 9 + lane);
+        const int sv = stencil_site(p.lat, s, lane, DAG ? 1 : 0);   // site of stage `lane`'s vector
+        const int sm = DAG ? sv : s;                                 // site of its link matrix
+        float f = 1.f;
+        if constexpr (I16) f = __ldg(p.scales + (int64_t)sm * 9 + lane);
+        if constexpr (HV) f *= __ldg(p.vnorms + sv);                 // half vectors: per-site norm folded in
+        return f;
     };
     const int M0 = GEN ? p.m_begin : 0;
     next_scale = fetch_scale(blockIdx.x);
@@ -243,7 +252,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
             }
 #pragma unroll 1
             for (int m = M0; m < 9; ++m) {
-                float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                float sc = (I16 || HV) ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
                 if constexpr (GEN) sc *= (m == 0) ? p.alpha : p.beta;
                 ptx::mbar_wait(full0 + 8u * slot, phase);
                 const uint32_t lbase = link_u32 + slot * LINK_STAGE + qi * 16;
@@ -253,13 +262,27 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
 #pragma unroll
                     for (int ps = 0; ps < PASSES; ++ps) {
                         const int col0 = (ps * QP + qi) * CPQ;
+                        if constexpr (HV) {
+                            if constexpr (CPQ == 2) {
+                                const float2 t = ptx::lds64(vbase + col0 * 4);
+                                v[ps][0] = unpack_i16x2(__float_as_uint(t.x));
+                                v[ps][1] = unpack_i16x2(__float_as_uint(t.y));
+                            } else {
+                                const uint4 t = ptx::lds128u(vbase + col0 * 4);
+                                v[ps][0] = unpack_i16x2(t.x);
+                                v[ps][1] = unpack_i16x2(t.y);
+                                v[ps][2] = unpack_i16x2(t.z);
+                                v[ps][3] = unpack_i16x2(t.w);
+                            }
+                        } else {
 #pragma unroll
-                        for (int h = 0; h < CPQ / 2; ++h) {
-                            const float4 t = ptx::lds128(vbase + (col0 + 2 * h) * 8);
-                            v[ps][2 * h] = make_float2(t.x, t.y);
-                            v[ps][2 * h + 1] = make_float2(t.z, t.w);
+                            for (int h = 0; h < CPQ / 2; ++h) {
+                                const float4 t = ptx::lds128(vbase + (col0 + 2 * h) * 8);
+                                v[ps][2 * h] = make_float2(t.x, t.y);
+                                v[ps][2 * h + 1] = make_float2(t.z, t.w);
+                            }
                         }
-                        if constexpr (I16 || GEN) {
+                        if constexpr (I16 || GEN || HV) {
 #pragma unroll
                             for (int e = 0; e < CPQ; ++e) { v[ps][e].x *= sc; v[ps][e].y *= sc; }
                         }
@@ -324,7 +347,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
                 for (int e = 0; e < CPQ; ++e) acc[ps][e] = make_float2(0.f, 0.f);
 #pragma unroll 1
             for (int m = M0; m < 9; ++m) {
-                float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                float sc = (I16 || HV) ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
                 if constexpr (GEN) sc *= (m == 0) ? p.alpha : p.beta;
 #pragma unroll 1
                 for (int c = 0; c < NB; ++c) {
@@ -335,8 +358,15 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE>::THREADS, 1) coarse_
 #pragma unroll
                         for (int k = 0; k < WL; ++k) {
                             const int rl = (k * W + warp) * RPL + grp;
-                            float2 vj = ptx::lds64(vbase + rl * 8);
-                            if constexpr (I16 || GEN) { vj.x *= sc; vj.y *= sc; }
+                            float2 vj;
+                            if constexpr (HV) {
+                                uint32_t w;
+                                asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w) : "r"(vbase + rl * 4));
+                                vj = unpack_i16x2(w);
+                            } else {
+                                vj = ptx::lds64(vbase + rl * 8);
+                            }
+                            if constexpr (I16 || GEN || HV) { vj.x *= sc; vj.y *= sc; }
 #pragma unroll
                             for (int ps = 0; ps < PASSES; ++ps) {
                                 const uint32_t a = lbase + rl * ROWBYTES + ps * QP * 16;
