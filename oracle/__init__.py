@@ -291,3 +291,32 @@ def coarse_apply_hvec(dims, Nc: int, links, vec_q, vec_norms, nrhs: int = 1, dag
     if rc != 0:
         raise ValueError(f"oracle_coarse_apply_hvec rejected its arguments (rc={rc})")
     return out
+
+
+# ----------------------------------------------------------------------------- CA-GCR(s) (row f3)
+def cagcr(apply_fn, b, x0, s: int, cycles: int = 1):
+    """Communication-avoiding GCR(s), the paper's smoother ("CA-GCR(8)", Table 1 L116/L122/
+    L130), power basis (reading R23).  One cycle, by its definition:
+        r0 = b - A x0;   p_k = A^k r0, k = 0..s-1;   q_k = A p_k = p_{k+1}
+        alpha = argmin_a || r0 - sum_k a_k q_k ||_2          (numpy.linalg.lstsq on the tall matrix Q)
+        x = x0 + sum_k alpha_k p_k;   r = r0 - sum_k alpha_k q_k
+    i.e. the residual is minimised over x0 + K_s(A, r0), the iterate GMRES(s)/GCR(s) define.  The s+1
+    basis vectors are rounded to complex64 where the CUDA path stores them; everything else is fp64.
+    apply_fn(v complex64 [n]) -> complex128 [n].  Returns (x complex128, [||r||_2 before each cycle and
+    after the last])."""
+    b = np.asarray(b).reshape(-1).astype(np.complex128)
+    x = np.asarray(x0).reshape(-1).astype(np.complex128)
+    norms = []
+    r = b - apply_fn(x.astype(np.complex64)) if np.any(x != 0) else b.copy()
+    for _ in range(cycles):
+        norms.append(float(np.linalg.norm(r)))
+        P = [r.astype(np.complex64)]
+        for _k in range(s):
+            P.append(apply_fn(P[-1]).astype(np.complex64))
+        Pm = np.stack([p.astype(np.complex128) for p in P], axis=1)       # n x (s+1)
+        Q = Pm[:, 1:]
+        alpha = np.linalg.lstsq(Q, Pm[:, 0], rcond=None)[0]
+        x = x + Pm[:, :s] @ alpha
+        r = Pm[:, 0] - Q @ alpha
+    norms.append(float(np.linalg.norm(r)))
+    return x, norms
