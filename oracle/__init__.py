@@ -298,7 +298,10 @@ def cagcr(apply_fn, b, x0, s: int, cycles: int = 1):
     """Communication-avoiding GCR(s), the paper's smoother ("CA-GCR(8)", Table 1 L116/L122/
     L130), power basis (reading R23).  One cycle, by its definition:
         r0 = b - A x0;   p_k = A^k r0, k = 0..s-1;   q_k = A p_k = p_{k+1}
-        alpha = argmin_a || r0 - sum_k a_k q_k ||_2          (numpy.linalg.lstsq on the tall matrix Q)
+        alpha = argmin_a || r0 - sum_k a_k q_k ||_2          (numpy.linalg.lstsq on the tall matrix Q, columns
+                                                              scaled to unit norm, NO singular-value cut-off:
+                                                              the power basis reaches cond ~1e11 and the
+                                                              default rcond would silently shrink the space)
         x = x0 + sum_k alpha_k p_k;   r = r0 - sum_k alpha_k q_k
     i.e. the residual is minimised over x0 + K_s(A, r0), the iterate GMRES(s)/GCR(s) define.  The s+1
     basis vectors are rounded to complex64 where the CUDA path stores them; everything else is fp64.
@@ -315,7 +318,9 @@ def cagcr(apply_fn, b, x0, s: int, cycles: int = 1):
             P.append(apply_fn(P[-1]).astype(np.complex64))
         Pm = np.stack([p.astype(np.complex128) for p in P], axis=1)       # n x (s+1)
         Q = Pm[:, 1:]
-        alpha = np.linalg.lstsq(Q, Pm[:, 0], rcond=None)[0]
+        d = np.linalg.norm(Q, axis=0)
+        d[d == 0] = 1.0
+        alpha = np.linalg.lstsq(Q / d, Pm[:, 0], rcond=1e-300)[0] / d
         x = x + Pm[:, :s] @ alpha
         r = Pm[:, 0] - Q @ alpha
     norms.append(float(np.linalg.norm(r)))
