@@ -34,6 +34,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+import numpy as np
 import torch
 
 import synth
@@ -576,6 +577,72 @@ def run_schur(args, cfg):
     return 0
 
 
+def run_cagcr(args, cfg):
+    """--workload cagcr: CA-GCR(8) smoother cycles on the config's operator
+    (diagonally shifted so that the smoother converges).  One step = one cycle = 8 chained applies + the
+    fused Gram pass + the 8x8 solve + the fused update = 11 launches."""
+    import paper_2212_12559_b200 as cop
+    world, rank, local = dist_env()
+    if world > 1:
+        raise RuntimeError("--workload cagcr is a single-GPU measurement")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dims, Nc, s = cfg["dims"], cfg["Nc"], 8
+    V = synth.lattice_volume(dims)
+    prec = cop.LINK_I16 if cfg["links"] == "i16" else cop.LINK_C64
+    links = synth.make_gamma_hermitian_links(dims, Nc, cfg["seed"], device=dev)
+    links[:, 0] += 12.0 * torch.eye(Nc, dtype=torch.complex64, device=dev)
+    scales = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device=dev)
+        scales = torch.empty((V, 9), dtype=torch.float32, device=dev)
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        torch.cuda.synchronize()
+        links = q
+    b = synth.make_vectors(dims, Nc, 1, cfg["seed"] + 1, device=dev)
+    x = torch.zeros_like(b)
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    info = torch.zeros((1, 3), dtype=torch.float64, device=dev)
+    work = op.cagcr(b, x, s=s, cycles=1, info=info)
+    stream = torch.cuda.current_stream()
+    for _ in range(max(args.warmup, 3)):
+        op.cagcr(b, x, s=s, cycles=1, work=work, info=info)
+    torch.cuda.synchronize()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        t0.record(stream)
+        for _ in range(args.steps):
+            op.cagcr(b, x, s=s, cycles=1, work=work, info=info)
+        t1.record(stream)
+        tmp = torch.empty_like(b)
+        a0.record(stream)
+        for _ in range(args.steps):
+            for _k in range(s):
+                op.apply(b, tmp)
+        a1.record(stream)
+        torch.cuda.synchronize()
+    ms_cycle = t0.elapsed_time(t1) / args.steps
+    ms_applies = a0.elapsed_time(a1) / args.steps
+    inf = info.cpu().numpy()[0]
+    line = {
+        "metric": METRIC, "value": s * V * args.steps / (t0.elapsed_time(t1) * 1e-3), "unit": UNIT, "n_gpus": 1,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_cycle, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "CA-GCR(8) smoother cycle on the %s lattice, Nc=%d, %s links (X shifted by 12): 8 applies + "
+                               "Gram + solve + update per step" % ("x".join(map(str, dims)), Nc, cfg["links"]),
+                   "seed": cfg["seed"]},
+        "clocks": clocks.summary(), "gpu_launches": (s + 3) * args.steps,
+        "cagcr": {"ms_per_cycle": ms_cycle, "ms_of_8_plain_applies": ms_applies,
+                  "vector_side_share": 1.0 - ms_applies / ms_cycle,
+                  "residual_reduction_one_cycle": float(np.sqrt(max(inf[1], 0.0) / inf[0])) if inf[0] > 0 else None,
+                  "basis_vectors_kept": int(inf[2])},
+    }
+    print(json.dumps(line), flush=True)
+    op.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -583,7 +650,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2", choices=sorted(synth.CONFIGS))
-    ap.add_argument("--workload", default="apply", choices=["apply", "schur"],
+    ap.add_argument("--workload", default="apply", choices=["apply", "schur", "cagcr"],
                     help="apply: the BASELINE metric (default); schur: the even/odd Schur-hat operator (row f1)")
     ap.add_argument("--dagger", default="both", choices=["0", "1", "both"])
     ap.add_argument("--path", type=int, default=0, help="COARSE_PATH_* override (0 = auto)")
@@ -602,6 +669,8 @@ def main():
     daggers = [0, 1] if args.dagger == "both" else [int(args.dagger)]
     if args.workload == "schur":
         return run_schur(args, cfg)
+    if args.workload == "cagcr":
+        return run_cagcr(args, cfg)
     if args.impl == "reference":
         return run_reference(args, cfg, daggers)
     return run_ours(args, cfg, daggers)

@@ -165,6 +165,21 @@ int coarse_op_last_path(const coarse_op_t* op);
 int coarse_op_quantize_i16(const void* links_c64_dev, int64_t n_matrices, int Nc, void* q_dev,
                            float* scales_dev, void* stream);
 
+/* CA-GCR(s), the paper's smoother ("CA-GCR(8)", Table 1 L116/L122/L130), on this operator,
+ * 1 RHS, power basis.  Each of `cycles` cycles: r0 = b - A x; p_k = A^k r0 (s chained coarse_op_apply);
+ * ONE fused pass of block inner products G_jk = <p_j, p_k> (fp64, the single reduction per cycle);
+ * alpha = argmin || r0 - sum_k alpha_k A p_k || from the s x s normal equations (fp64 Cholesky on the
+ * device); x += sum_k alpha_k p_k, r = r0 - sum_k alpha_k A p_k in one fused update pass.
+ *   b_dev, x_dev   complex64 [V][Nc]; x_is_zero != 0: x is cleared first and b is used as r0 directly.
+ *   work_dev       coarse_op_cagcr_work_bytes(op, s) bytes of caller-owned scratch (16-byte aligned).
+ *   info_dev       NULL, or double[3 * cycles]: per cycle ||r0||^2, the predicted ||r||^2 after the
+ *                  cycle, and the number of basis vectors the factorisation kept (s unless the Gram
+ *                  matrix lost positive definiteness).
+ * 1 <= s <= 16.  Enqueues s + 3 kernels per cycle and returns; never synchronises. */
+size_t coarse_op_cagcr_work_bytes(const coarse_op_t* op, int s);
+int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                    void* work_dev, double* info_dev, void* stream);
+
 /* Diagnostic: stream floor(bytes / stage_bytes) * stage_bytes bytes of device memory through the STREAM
  * kernels' TMA ring (one CTA per SM, `stages` slots of `stage_bytes`, evict_first bulk copies) with an
  * idle consumer.  Timed by the caller with CUDA events it gives the pure-read ceiling of this GPU for

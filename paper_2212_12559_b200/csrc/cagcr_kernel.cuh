@@ -1,0 +1,175 @@
+// cagcr_kernel.cuh — the vector side of CA-GCR(s), the paper's smoother ("CA-GCR(8)",
+// Table 1 L116/L122/L130), around s chained coarse-op applies:
+//
+//   p_0 = r0,  p_{k+1} = A p_k  (k < s)          s applies (stream_kernel.cuh), 98 % of the time
+//   G_jk = <p_j, p_k>,  0 <= j <= k <= s          ONE fused pass of block inner products (this file);
+//                                                 on a partitioned lattice this is the single
+//                                                 all-reduce per cycle that makes the method
+//                                                 "communication avoiding"
+//   (Q^H Q) alpha = Q^H r0 with q_k = p_{k+1}     s x s Hermitian solve, fp64 Cholesky, one thread
+//   x += sum_k alpha_k p_k,  r = p_0 - sum_k alpha_k p_{k+1}      one fused update pass
+//
+// The Gram matrix is accumulated in fp64 (the power basis is ill conditioned; the normal equations
+// square that) with a fixed two-level summation order: bit-identical run to run.
+#pragma once
+#include "common.cuh"
+
+namespace coarse {
+
+constexpr int CAGCR_MAX_S = 16;
+constexpr int CAGCR_GRAM_BLOCKS = 148;
+
+struct CagcrVecs {
+    const float2* p[CAGCR_MAX_S + 1];   // p_0 .. p_s
+};
+
+// grid (CAGCR_GRAM_BLOCKS, s+1): block (bx, j) accumulates sum_i conj(p_j[i]) p_k[i] for k = j..s over
+// its slice of i, and writes partial[bx][j][k].
+__global__ void __launch_bounds__(256) cagcr_gram_kernel(CagcrVecs v, long long n, int s, double2* partial) {
+    const int j = blockIdx.y;
+    double2 acc[CAGCR_MAX_S + 1];
+#pragma unroll
+    for (int k = 0; k <= CAGCR_MAX_S; ++k) acc[k] = make_double2(0.0, 0.0);
+    const float2* pj = v.p[j];
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float2 a = pj[i];
+#pragma unroll
+        for (int k = 0; k <= CAGCR_MAX_S; ++k) {
+            if (k + j <= s) {
+                const float2 b = v.p[k + j][i];
+                acc[k].x += (double)a.x * (double)b.x + (double)a.y * (double)b.y;
+                acc[k].y += (double)a.x * (double)b.y - (double)a.y * (double)b.x;
+            }
+        }
+    }
+    __shared__ double2 red[8][CAGCR_MAX_S + 1];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int k = 0; k <= CAGCR_MAX_S; ++k) {
+        if (k + j <= s) {
+            double2 t = acc[k];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                t.x += __shfl_xor_sync(0xffffffffu, t.x, o);
+                t.y += __shfl_xor_sync(0xffffffffu, t.y, o);
+            }
+            if (lane == 0) red[warp][k] = t;
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x <= CAGCR_MAX_S && threadIdx.x + j <= s) {
+        double2 t = make_double2(0.0, 0.0);
+        for (int w = 0; w < 8; ++w) {
+            t.x += red[w][threadIdx.x].x;
+            t.y += red[w][threadIdx.x].y;
+        }
+        const int S1 = s + 1;
+        partial[((long long)blockIdx.x * S1 + j) * S1 + j + threadIdx.x] = t;
+    }
+}
+
+// One CTA: sums the per-block partials in block order, then thread 0 solves the s x s normal equations
+// M alpha = c (M_ab = G[a+1][b+1], c_a = G[a+1][0] = <q_a, r0>) by a complex Cholesky factorisation in
+// fp64.  A pivot that has lost all its digits truncates the basis there (alpha_k = 0 beyond it).
+// info[0] = ||r0||^2, info[1] = predicted ||r||^2 = ||r0||^2 - Re(c^H alpha), info[2] = columns used.
+__global__ void __launch_bounds__(320) cagcr_solve_kernel(const double2* partial, int nblocks, int s, double2* alpha,
+                                                          double* info) {
+    __shared__ double2 G[CAGCR_MAX_S + 1][CAGCR_MAX_S + 1];
+    const int S1 = s + 1;
+    for (int e = threadIdx.x; e < S1 * S1; e += blockDim.x) {
+        const int j = e / S1, k = e % S1;
+        if (k >= j) {
+            double2 t = make_double2(0.0, 0.0);
+            for (int b = 0; b < nblocks; ++b) {
+                const double2 x = partial[((long long)b * S1 + j) * S1 + k];
+                t.x += x.x;
+                t.y += x.y;
+            }
+            G[j][k] = t;
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    double2 L[CAGCR_MAX_S][CAGCR_MAX_S];
+    double2 y[CAGCR_MAX_S];
+    int used = s;
+    // M_ab = G[a+1][b+1] for b >= a, Hermitian: M_ba = conj(M_ab); lower Cholesky M = L L^H
+    for (int k = 0; k < s; ++k) {
+        double d = G[k + 1][k + 1].x;
+        for (int i = 0; i < k; ++i) d -= L[k][i].x * L[k][i].x + L[k][i].y * L[k][i].y;
+        if (!(d > 1e-13 * G[k + 1][k + 1].x)) { used = k; break; }
+        const double lkk = sqrt(d);
+        L[k][k] = make_double2(lkk, 0.0);
+        for (int a = k + 1; a < s; ++a) {
+            // M_ak = conj(G[k+1][a+1])
+            double2 t = make_double2(G[k + 1][a + 1].x, -G[k + 1][a + 1].y);
+            for (int i = 0; i < k; ++i) {   // t -= L[a][i] * conj(L[k][i])
+                t.x -= L[a][i].x * L[k][i].x + L[a][i].y * L[k][i].y;
+                t.y -= L[a][i].y * L[k][i].x - L[a][i].x * L[k][i].y;
+            }
+            L[a][k] = make_double2(t.x / lkk, t.y / lkk);
+        }
+    }
+    // c_a = <q_a, r0> = conj(G[0][a+1]);  forward solve L y = c
+    for (int a = 0; a < used; ++a) {
+        double2 t = make_double2(G[0][a + 1].x, -G[0][a + 1].y);
+        for (int i = 0; i < a; ++i) {       // t -= L[a][i] * y[i]
+            t.x -= L[a][i].x * y[i].x - L[a][i].y * y[i].y;
+            t.y -= L[a][i].x * y[i].y + L[a][i].y * y[i].x;
+        }
+        y[a] = make_double2(t.x / L[a][a].x, t.y / L[a][a].x);
+    }
+    // backward solve L^H alpha = y
+    double gain = 0.0;
+    for (int a = used - 1; a >= 0; --a) {
+        double2 t = y[a];
+        for (int i = a + 1; i < used; ++i) {   // t -= conj(L[i][a]) * alpha[i]
+            const double2 al = alpha[i];
+            t.x -= L[i][a].x * al.x + L[i][a].y * al.y;
+            t.y -= L[i][a].x * al.y - L[i][a].y * al.x;
+        }
+        alpha[a] = make_double2(t.x / L[a][a].x, t.y / L[a][a].x);
+    }
+    for (int a = used; a < s; ++a) alpha[a] = make_double2(0.0, 0.0);
+    for (int a = 0; a < used; ++a) gain += y[a].x * y[a].x + y[a].y * y[a].y;   // c^H M^-1 c = |y|^2
+    if (info) {
+        info[0] = G[0][0].x;
+        info[1] = G[0][0].x - gain;
+        info[2] = (double)used;
+    }
+}
+
+// x += sum_{k<s} alpha_k p_k ;  r_out = p_0 - sum_{k<s} alpha_k p_{k+1}
+__global__ void __launch_bounds__(256) cagcr_update_kernel(CagcrVecs v, long long n, int s, const double2* alpha,
+                                                           float2* x, float2* r_out) {
+    __shared__ float2 al[CAGCR_MAX_S];
+    if (threadIdx.x < s) al[threadIdx.x] = make_float2((float)alpha[threadIdx.x].x, (float)alpha[threadIdx.x].y);
+    __syncthreads();
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        float2 xs = x[i];
+        float2 prev = v.p[0][i];
+        float2 rs = prev;
+#pragma unroll 4
+        for (int k = 0; k < s; ++k) {
+            const float2 a = al[k];
+            xs.x = fmaf(a.x, prev.x, fmaf(-a.y, prev.y, xs.x));
+            xs.y = fmaf(a.x, prev.y, fmaf(a.y, prev.x, xs.y));
+            const float2 next = v.p[k + 1][i];
+            rs.x = fmaf(-a.x, next.x, fmaf(a.y, next.y, rs.x));
+            rs.y = fmaf(-a.x, next.y, fmaf(-a.y, next.x, rs.y));
+            prev = next;
+        }
+        x[i] = xs;
+        r_out[i] = rs;
+    }
+}
+
+// r = b - t
+__global__ void __launch_bounds__(256) cagcr_residual_kernel(const float2* b, const float2* t, long long n, float2* r) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float2 x = b[i], y = t[i];
+        r[i] = make_float2(x.x - y.x, x.y - y.y);
+    }
+}
+
+}  // namespace coarse

@@ -17,6 +17,7 @@
 #include "block_kernel.cuh"
 #include "tensor_kernel.cuh"
 #include "probe_kernel.cuh"
+#include "cagcr_kernel.cuh"
 
 using namespace coarse;
 
@@ -662,6 +663,72 @@ int coarse_op_quantize_i16(const void* links_c64_dev, int64_t n_matrices, int Nc
         static_cast<const float*>(links_c64_dev), n_matrices, Nc, static_cast<short*>(q_dev), scales_dev);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "quantize kernel launch");
+    return COARSE_OK;
+}
+
+size_t coarse_op_cagcr_work_bytes(const coarse_op_t* op, int s) {
+    if (!op || s < 1 || s > CAGCR_MAX_S) return 0;
+    const size_t vec = coarse_op_vector_bytes(op, 1);
+    const size_t S1 = (size_t)s + 1;
+    return (S1 + 1) * vec + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1 * sizeof(double2) + (size_t)CAGCR_MAX_S * sizeof(double2) + 64;
+}
+
+int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                    void* work_dev, double* info_dev, void* stream) {
+    if (!op) return fail(COARSE_EINVAL, "cagcr: op is NULL");
+    if (!op->links) return fail(COARSE_ENOTREADY, "cagcr: coarse_op_set_links has not been called");
+    if (!b_dev || !x_dev || !work_dev) return fail(COARSE_EINVAL, "cagcr: NULL pointer");
+    if (s < 1 || s > CAGCR_MAX_S) return fail(COARSE_EINVAL, "cagcr: 1 <= s <= %d (got %d)", CAGCR_MAX_S, s);
+    if (cycles < 1) return fail(COARSE_EINVAL, "cagcr: cycles must be >= 1");
+    if (!aligned16(b_dev) || !aligned16(x_dev) || !aligned16(work_dev)) return fail(COARSE_EINVAL, "cagcr: pointers must be 16-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t vec = coarse_op_vector_bytes(op, 1);
+    const long long n = (long long)op->lat.V * op->Nc;
+    const int S1 = s + 1;
+    unsigned char* w = static_cast<unsigned char*>(work_dev);
+    float2* slot[CAGCR_MAX_S + 2];
+    for (int k = 0; k < S1 + 1; ++k) slot[k] = reinterpret_cast<float2*>(w + (size_t)k * vec);
+    double2* partial = reinterpret_cast<double2*>(w + (size_t)(S1 + 1) * vec);
+    double2* alpha = partial + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1;
+    const int vgrid = op->num_sms * 4;
+    int launches = 0, rc;
+    // s + 2 slots used as a ring: p_k = slot[(base + k) % (s+2)], k = 0..s, and the update writes the new
+    // residual into slot[(base + s + 1) % (s+2)], which is p_0 of the next cycle.  In the first cycle
+    // with x = 0 the residual is b itself (no copy): p_0 points at b and slot[base] stays unused.
+    const int NS = S1 + 1;
+    int base = 0;
+    bool p0_is_b = false;
+    if (x_is_zero) {
+        cudaError_t e = cudaMemsetAsync(x_dev, 0, vec, st);
+        if (e != cudaSuccess) return cuda_fail(e, "cagcr: memset x");
+        p0_is_b = true;
+    } else {
+        rc = coarse_op_apply(op, x_dev, slot[1], 1, 0, stream);
+        if (rc != COARSE_OK) return rc;
+        ++launches;
+        cagcr_residual_kernel<<<vgrid, 256, 0, st>>>(static_cast<const float2*>(b_dev), slot[1], n, slot[0]);
+        ++launches;
+    }
+    for (int c = 0; c < cycles; ++c) {
+        CagcrVecs v;
+        for (int k = 0; k <= CAGCR_MAX_S; ++k) v.p[k] = k <= s ? slot[(base + k) % NS] : nullptr;
+        if (p0_is_b) v.p[0] = static_cast<const float2*>(b_dev);
+        float2* r_out = slot[(base + s + 1) % NS];
+        for (int k = 0; k < s; ++k) {
+            rc = coarse_op_apply(op, v.p[k], const_cast<float2*>(v.p[k + 1]), 1, 0, stream);
+            if (rc != COARSE_OK) return rc;
+            ++launches;
+        }
+        cagcr_gram_kernel<<<dim3(CAGCR_GRAM_BLOCKS, S1), 256, 0, st>>>(v, n, s, partial);
+        cagcr_solve_kernel<<<1, 320, 0, st>>>(partial, CAGCR_GRAM_BLOCKS, s, alpha, info_dev ? info_dev + 3 * c : nullptr);
+        cagcr_update_kernel<<<vgrid, 256, 0, st>>>(v, n, s, alpha, static_cast<float2*>(x_dev), r_out);
+        launches += 3;
+        base = (base + s + 1) % NS;
+        p0_is_b = false;
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "cagcr kernel launch");
+    op->last_launches = launches;
     return COARSE_OK;
 }
 

@@ -1,0 +1,133 @@
+"""GPU parity for CA-GCR(s) against the oracle's definition
+(least squares over the Krylov space, tests/test_oracle_cagcr_pins.py).
+
+What is compared, and why: the minimised residual is what the method defines stably,
+so ||b - A x_gpu|| (evaluated by the fp64 oracle apply) must match the oracle's optimum to 1e-4
+relative, and the norms the solve kernel reports must match the true ones.  The iterate x itself is
+compared too, with a bound that carries the conditioning of the power basis: the fp32 applies perturb
+each basis vector by ~2e-7, and the least-squares coefficients amplify that by cond(Q)."""
+import numpy as np
+import pytest
+import torch
+
+import synth
+import paper_2212_12559_b200 as cop
+from tests.helpers import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_cuda():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests selected but no CUDA device is visible (there is no CPU fallback)")
+    torch.cuda.set_device(0)
+
+
+def _case(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero, shift=12.0, seed=101):
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, seed, device="cuda")
+    links[:, 0] += shift * torch.eye(Nc, dtype=torch.complex64, device="cuda")
+    scales = scales_h = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+        scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        torch.cuda.synchronize()
+        links, scales_h = q, scales.cpu().numpy()
+    links_h = links.cpu().numpy()
+    b = synth.make_vectors(dims, Nc, 1, seed + 1, device="cuda")
+    x = torch.zeros_like(b) if x_is_zero else 0.05 * synth.make_vectors(dims, Nc, 1, seed + 2, device="cuda")
+    x0_h = x.cpu().numpy().reshape(-1)
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    info = torch.zeros((cycles, 3), dtype=torch.float64, device="cuda")
+    op.cagcr(b, x, s=s, cycles=cycles, x_is_zero=x_is_zero, info=info)
+    torch.cuda.synchronize()
+    assert op.last_launches == cycles * (s + 3) + (0 if x_is_zero else 2)
+    apply_fn = lambda v: oracle_lib.coarse_apply(dims, Nc, links_h, v.reshape(V, Nc, 1), link_precision=prec,
+                                                 scales=scales_h).reshape(-1)
+    b_h = b.cpu().numpy().reshape(-1)
+    x_ref, norms = oracle_lib.cagcr(apply_fn, b_h, x0_h, s, cycles)
+    x_gpu = x.cpu().numpy().reshape(-1)
+    r_gpu = np.linalg.norm(b_h.astype(np.complex128) - apply_fn(x_gpu))
+    info_h = info.cpu().numpy()
+    # conditioning of the first cycle's basis (for the bound on x)
+    P = [(b_h.astype(np.complex128) - (apply_fn(x0_h.astype(np.complex64)) if not x_is_zero else 0)).astype(np.complex64)]
+    for _ in range(s):
+        P.append(apply_fn(P[-1]).astype(np.complex64))
+    condQ = np.linalg.cond(np.stack(P[1:], axis=1).astype(np.complex128))
+    op.close()
+    return dict(x_err=rel_l2(x_gpu, x_ref), r_gpu=r_gpu, norms=norms, info=info_h, condQ=condQ)
+
+
+@pytest.mark.parametrize("dims,Nc", [((4, 4, 4, 4), 48), ((3, 2, 2, 4), 64), ((2, 2, 2, 2), 128)])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("s,cycles", [(8, 1), (4, 3), (1, 2), (16, 1)])
+@pytest.mark.parametrize("x_is_zero", [True, False])
+def test_cagcr_against_oracle(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero):
+    res = _case(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero)
+    norms, info = res["norms"], res["info"]
+    # Noise floor of the comparison, relative to ||r0||: complex64 basis vectors (6e-8) times the growth
+    # of the power basis.  For s <= 8 that is ~1e-6.  At s = 16 the power basis (cond > 1e20) is beyond
+    # fp64 normal equations: the factorisation truncates it and the residual stalls at a few 1e-5 of
+    # ||r0|| - which is why the paper's CA-GCR(16) uses a Chebyshev basis, not built here.
+    floor = (2e-6 if s <= 8 else 5e-5) * norms[0]
+    # the residual the GPU iterate really has is the oracle's optimum
+    assert abs(res["r_gpu"] - norms[-1]) <= 1e-4 * norms[-1] + floor, (res["r_gpu"], norms)
+    # what the solve kernel reports: ||r0||^2 per cycle and the predicted ||r||^2 after it
+    for c in range(cycles):
+        assert abs(np.sqrt(info[c, 0]) - norms[c]) <= 1e-4 * norms[c] + floor
+        assert info[c, 2] == s if s <= 8 else info[c, 2] >= 8          # whole basis kept up to s = 8
+    assert abs(np.sqrt(max(info[-1, 1], 0.0)) - norms[-1]) <= 1e-3 * norms[-1] + 5 * floor
+    # the iterate itself, with the basis conditioning in the bound
+    assert res["x_err"] <= 1e-5 + 20 * res["condQ"] * 2e-7, (res["x_err"], res["condQ"])
+
+
+def test_cagcr_reduces_the_residual_on_a_baseline_shaped_operator(oracle_lib):
+    """C1's generator (Gamma-Hermitian links) with a diagonal shift that makes it smoother-friendly."""
+    res = _case(oracle_lib, (4, 4, 4, 4), 48, cop.LINK_C64, 8, 2, True, shift=10.0, seed=20221201)
+    assert res["norms"][-1] < 0.05 * res["norms"][0]
+    # two cycles take the fp64 oracle to 1e-6 of ||r0||; the complex64 iterate and residual recurrence of the
+    # CUDA path stall at its single-precision floor (a few 1e-5): a smoother, not a solver
+    assert res["r_gpu"] <= 1e-4 * res["norms"][0]
+
+
+def test_cagcr_is_bit_reproducible():
+    dims, Nc = (4, 4, 2, 2), 48
+    links = synth.make_arbitrary_links(dims, Nc, 1, device="cuda")
+    links[:, 0] += 12.0 * torch.eye(Nc, dtype=torch.complex64, device="cuda")
+    b = synth.make_vectors(dims, Nc, 1, 2, device="cuda")
+    op = cop.CoarseOp(dims, Nc).set_links(links)
+    outs = []
+    for _ in range(2):
+        x = torch.empty_like(b)
+        op.cagcr(b, x, s=8, cycles=2)
+        torch.cuda.synchronize()
+        outs.append(x)
+    assert torch.equal(torch.view_as_real(outs[0]), torch.view_as_real(outs[1]))
+    op.close()
+
+
+def test_cagcr_argument_errors():
+    L = cop.lib()
+    dims, Nc, V = (2, 2, 2, 2), 48, 16
+    h = cop.coarse_op_create(dims, Nc, cop.LINK_C64)
+    assert cop.coarse_op_cagcr_work_bytes(h, 8) >= 10 * V * Nc * 8
+    assert cop.coarse_op_cagcr_work_bytes(h, 0) == 0 and cop.coarse_op_cagcr_work_bytes(h, 17) == 0
+    b = torch.zeros((V, Nc, 1), dtype=torch.complex64, device="cuda")
+    x = torch.zeros_like(b)
+    w = torch.zeros(cop.coarse_op_cagcr_work_bytes(h, 8), dtype=torch.uint8, device="cuda")
+    assert L.coarse_op_cagcr(h, b.data_ptr(), x.data_ptr(), 8, 1, 1, w.data_ptr(), None, None) == cop.ENOTREADY
+    links = torch.zeros((V, 9, Nc, Nc), dtype=torch.complex64, device="cuda")
+    assert L.coarse_op_set_links(h, links.data_ptr(), None) == cop.OK
+    assert L.coarse_op_cagcr(h, b.data_ptr(), x.data_ptr(), 0, 1, 1, w.data_ptr(), None, None) == cop.EINVAL
+    assert L.coarse_op_cagcr(h, b.data_ptr(), x.data_ptr(), 17, 1, 1, w.data_ptr(), None, None) == cop.EINVAL
+    assert L.coarse_op_cagcr(h, b.data_ptr(), x.data_ptr(), 8, 0, 1, w.data_ptr(), None, None) == cop.EINVAL
+    assert L.coarse_op_cagcr(h, None, x.data_ptr(), 8, 1, 1, w.data_ptr(), None, None) == cop.EINVAL
+    # a zero operator: the Gram matrix is singular, the basis truncates to nothing and x stays 0
+    info = torch.zeros(3, dtype=torch.float64, device="cuda")
+    b.fill_(1.0)
+    assert L.coarse_op_cagcr(h, b.data_ptr(), x.data_ptr(), 8, 1, 1, w.data_ptr(), info.data_ptr(), None) == cop.OK
+    torch.cuda.synchronize()
+    assert info[2].item() == 0 and torch.all(x == 0)
+    cop.coarse_op_destroy(h)
