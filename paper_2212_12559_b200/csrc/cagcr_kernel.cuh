@@ -17,54 +17,74 @@
 namespace coarse {
 
 constexpr int CAGCR_MAX_S = 16;
-constexpr int CAGCR_GRAM_BLOCKS = 148;
+constexpr int CAGCR_GRAM_BLOCKS = 296;
 
 struct CagcrVecs {
     const float2* p[CAGCR_MAX_S + 1];   // p_0 .. p_s
 };
 
-// grid (CAGCR_GRAM_BLOCKS, s+1): block (bx, j) accumulates sum_i conj(p_j[i]) p_k[i] for k = j..s over
-// its slice of i, and writes partial[bx][j][k].
+// Fused block inner products: every CTA walks tiles of CAGCR_TILE lattice elements, stages the s+1
+// basis vectors of the tile in shared memory ONCE (each vector is read from global memory exactly once
+// per cycle) and its 8 warps share out the (s+1)(s+2)/2 pairs (j <= k), pair index cyclic over warps;
+// a lane accumulates conj(p_j[e]) p_k[e] in fp64 over the elements e = lane, lane + 32, ... of the tile.
+// partial[block][pair] is written once per CTA; the solve kernel adds the blocks in order.
+constexpr int CAGCR_TILE = 256;
+constexpr int CAGCR_MAX_PAIRS = (CAGCR_MAX_S + 1) * (CAGCR_MAX_S + 2) / 2;     // 153
+constexpr int CAGCR_PAIRS_PER_WARP = (CAGCR_MAX_PAIRS + 7) / 8;                // 20
+
+__host__ __device__ inline int cagcr_pair_index(int j, int k, int S1) { return j * S1 - j * (j - 1) / 2 + (k - j); }
+
 __global__ void __launch_bounds__(256) cagcr_gram_kernel(CagcrVecs v, long long n, int s, double2* partial) {
-    const int j = blockIdx.y;
-    double2 acc[CAGCR_MAX_S + 1];
+    __shared__ float2 tile[CAGCR_MAX_S + 1][CAGCR_TILE];
+    __shared__ unsigned char pj[CAGCR_MAX_PAIRS], pk[CAGCR_MAX_PAIRS];
+    const int S1 = s + 1;
+    const int npairs = S1 * (S1 + 1) / 2;
+    for (int t = threadIdx.x; t < S1 * S1; t += blockDim.x) {
+        const int a = t / S1, b = t % S1;
+        if (b >= a) {
+            pj[cagcr_pair_index(a, b, S1)] = (unsigned char)a;
+            pk[cagcr_pair_index(a, b, S1)] = (unsigned char)b;
+        }
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double2 acc[CAGCR_PAIRS_PER_WARP];
 #pragma unroll
-    for (int k = 0; k <= CAGCR_MAX_S; ++k) acc[k] = make_double2(0.0, 0.0);
-    const float2* pj = v.p[j];
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const float2 a = pj[i];
+    for (int q = 0; q < CAGCR_PAIRS_PER_WARP; ++q) acc[q] = make_double2(0.0, 0.0);
+    const long long ntiles = (n + CAGCR_TILE - 1) / CAGCR_TILE;
+    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const long long i = t * CAGCR_TILE + threadIdx.x;
+        __syncthreads();                       // previous tile fully consumed (and pj/pk written)
+        for (int k = 0; k < S1; ++k) tile[k][threadIdx.x] = i < n ? v.p[k][i] : make_float2(0.f, 0.f);
+        __syncthreads();
 #pragma unroll
-        for (int k = 0; k <= CAGCR_MAX_S; ++k) {
-            if (k + j <= s) {
-                const float2 b = v.p[k + j][i];
-                acc[k].x += (double)a.x * (double)b.x + (double)a.y * (double)b.y;
-                acc[k].y += (double)a.x * (double)b.y - (double)a.y * (double)b.x;
+        for (int q = 0; q < CAGCR_PAIRS_PER_WARP; ++q) {
+            const int pidx = warp + 8 * q;
+            if (pidx < npairs) {
+                const float2* a = tile[pj[pidx]];
+                const float2* b = tile[pk[pidx]];
+                double2 t2 = acc[q];
+#pragma unroll
+                for (int e = 0; e < CAGCR_TILE / 32; ++e) {
+                    const float2 x = a[lane + 32 * e], y = b[lane + 32 * e];
+                    t2.x += (double)x.x * (double)y.x + (double)x.y * (double)y.y;
+                    t2.y += (double)x.x * (double)y.y - (double)x.y * (double)y.x;
+                }
+                acc[q] = t2;
             }
         }
     }
-    __shared__ double2 red[8][CAGCR_MAX_S + 1];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #pragma unroll
-    for (int k = 0; k <= CAGCR_MAX_S; ++k) {
-        if (k + j <= s) {
-            double2 t = acc[k];
+    for (int q = 0; q < CAGCR_PAIRS_PER_WARP; ++q) {
+        const int pidx = warp + 8 * q;
+        if (pidx < npairs) {
+            double2 t2 = acc[q];
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
-                t.x += __shfl_xor_sync(0xffffffffu, t.x, o);
-                t.y += __shfl_xor_sync(0xffffffffu, t.y, o);
+                t2.x += __shfl_xor_sync(0xffffffffu, t2.x, o);
+                t2.y += __shfl_xor_sync(0xffffffffu, t2.y, o);
             }
-            if (lane == 0) red[warp][k] = t;
+            if (lane == 0) partial[(long long)blockIdx.x * npairs + pidx] = t2;
         }
-    }
-    __syncthreads();
-    if (threadIdx.x <= CAGCR_MAX_S && threadIdx.x + j <= s) {
-        double2 t = make_double2(0.0, 0.0);
-        for (int w = 0; w < 8; ++w) {
-            t.x += red[w][threadIdx.x].x;
-            t.y += red[w][threadIdx.x].y;
-        }
-        const int S1 = s + 1;
-        partial[((long long)blockIdx.x * S1 + j) * S1 + j + threadIdx.x] = t;
     }
 }
 
@@ -81,7 +101,7 @@ __global__ void __launch_bounds__(320) cagcr_solve_kernel(const double2* partial
         if (k >= j) {
             double2 t = make_double2(0.0, 0.0);
             for (int b = 0; b < nblocks; ++b) {
-                const double2 x = partial[((long long)b * S1 + j) * S1 + k];
+                const double2 x = partial[(long long)b * (S1 * (S1 + 1) / 2) + cagcr_pair_index(j, k, S1)];
                 t.x += x.x;
                 t.y += x.y;
             }

@@ -719,7 +719,7 @@ int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int 
             if (rc != COARSE_OK) return rc;
             ++launches;
         }
-        cagcr_gram_kernel<<<dim3(CAGCR_GRAM_BLOCKS, S1), 256, 0, st>>>(v, n, s, partial);
+        cagcr_gram_kernel<<<CAGCR_GRAM_BLOCKS, 256, 0, st>>>(v, n, s, partial);
         cagcr_solve_kernel<<<1, 320, 0, st>>>(partial, CAGCR_GRAM_BLOCKS, s, alpha, info_dev ? info_dev + 3 * c : nullptr);
         cagcr_update_kernel<<<vgrid, 256, 0, st>>>(v, n, s, alpha, static_cast<float2*>(x_dev), r_out);
         launches += 3;
