@@ -176,7 +176,14 @@ int coarse_op_quantize_i16(const void* links_c64_dev, int64_t n_matrices, int Nc
  *                  cycle, and the number of basis vectors the factorisation kept (s unless the Gram
  *                  matrix lost positive definiteness).
  * 1 <= s <= 16.  Enqueues s + 3 kernels per cycle and returns; never synchronises. */
+/* coarse_op_cagcr_schur: the same smoother on the left-preconditioned even/odd Schur operator
+ * Shat_p v = v - Dhat_pq Dhat_qp v of a handle whose links are block-preconditioned (Yhat = X^-1 Y;
+ * PAPER.md:L87, Table 1 L127/L135: the levels the paper smooths with CA-GCR(8) are Schur-preconditioned).
+ * b and x are full-lattice vectors whose entries on the other parity must be zero (x is kept so);
+ * every operator application is two parity-restricted launches (coarse_op_apply_parts). */
 size_t coarse_op_cagcr_work_bytes(const coarse_op_t* op, int s);
+int coarse_op_cagcr_schur(coarse_op_t* op_hat, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                          int parity, void* work_dev, double* info_dev, void* stream);
 int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
                     void* work_dev, double* info_dev, void* stream);
 

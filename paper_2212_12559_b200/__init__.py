@@ -28,7 +28,7 @@ EXPORTS = (
     "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_parts", "coarse_op_apply_hvec",
     "coarse_op_quantize_vec_i16", "coarse_op_apply_host",
     "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_probe_read", "coarse_op_cagcr_work_bytes",
-    "coarse_op_cagcr", "coarse_op_destroy",
+    "coarse_op_cagcr", "coarse_op_cagcr_schur", "coarse_op_destroy",
     "coarse_op_last_error",
 )
 
@@ -83,6 +83,8 @@ def lib() -> ctypes.CDLL:
     L.coarse_op_cagcr_work_bytes.argtypes = [vp, ci]
     L.coarse_op_cagcr.restype = ci
     L.coarse_op_cagcr.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp, vp]
+    L.coarse_op_cagcr_schur.restype = ci
+    L.coarse_op_cagcr_schur.argtypes = [vp, vp, vp, ci, ci, ci, ci, vp, vp, vp]
     L.coarse_op_probe_read.restype = ci
     L.coarse_op_probe_read.argtypes = [vp, sz, ci, ci, vp]
     L.coarse_op_destroy.restype = None
@@ -242,7 +244,7 @@ def coarse_op_cagcr_work_bytes(op: int, s: int) -> int:
 
 
 def coarse_op_cagcr(op: int, b, x, s: int, cycles: int = 1, x_is_zero: bool = True, work=None, info=None,
-                    stream=None) -> None:
+                    stream=None, schur_parity: Optional[int] = None) -> None:
     """CA-GCR(s) smoother cycles on CUDA complex64 vectors b, x [V][Nc]; work: CUDA uint8 tensor of at
     least coarse_op_cagcr_work_bytes(op, s) bytes; info: optional CUDA float64 tensor [cycles][3]."""
     for t in (b, x, work):
@@ -254,8 +256,12 @@ def coarse_op_cagcr(op: int, b, x, s: int, cycles: int = 1, x_is_zero: bool = Tr
         raise ValueError("cagcr: b / x have the wrong size (1 RHS)")
     if info is not None and (info.numel() < 3 * cycles or info.element_size() != 8 or not info.is_cuda):
         raise ValueError("cagcr: info must be a CUDA float64 tensor with 3 * cycles entries")
-    _check(lib().coarse_op_cagcr(op, _ptr(b), _ptr(x), int(s), int(cycles), 1 if x_is_zero else 0, _ptr(work),
-                                 _ptr(info), _stream_handle(stream)))
+    if schur_parity is None:
+        _check(lib().coarse_op_cagcr(op, _ptr(b), _ptr(x), int(s), int(cycles), 1 if x_is_zero else 0, _ptr(work),
+                                     _ptr(info), _stream_handle(stream)))
+    else:
+        _check(lib().coarse_op_cagcr_schur(op, _ptr(b), _ptr(x), int(s), int(cycles), 1 if x_is_zero else 0,
+                                           int(schur_parity), _ptr(work), _ptr(info), _stream_handle(stream)))
 
 
 def coarse_op_probe_read(src, stage_bytes: int = 16384, stages: int = 6, stream=None) -> int:
@@ -303,11 +309,12 @@ class CoarseOp:
     def apply_hvec(self, vin_q, vin_norms, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
         coarse_op_apply_hvec(self._h, vin_q, vin_norms, vout, nrhs, dagger, stream)
 
-    def cagcr(self, b, x, s: int = 8, cycles: int = 1, x_is_zero: bool = True, work=None, info=None, stream=None):
+    def cagcr(self, b, x, s: int = 8, cycles: int = 1, x_is_zero: bool = True, work=None, info=None, stream=None,
+              schur_parity: Optional[int] = None):
         import torch
         if work is None:
             work = torch.empty(coarse_op_cagcr_work_bytes(self._h, s), dtype=torch.uint8, device=b.device)
-        coarse_op_cagcr(self._h, b, x, s, cycles, x_is_zero, work, info, stream)
+        coarse_op_cagcr(self._h, b, x, s, cycles, x_is_zero, work, info, stream, schur_parity)
         return work
 
     def apply_host(self, vin_host, vout_host, nrhs: int = 1, dagger: int = 0, stream=None) -> None:

@@ -670,11 +670,14 @@ size_t coarse_op_cagcr_work_bytes(const coarse_op_t* op, int s) {
     if (!op || s < 1 || s > CAGCR_MAX_S) return 0;
     const size_t vec = coarse_op_vector_bytes(op, 1);
     const size_t S1 = (size_t)s + 1;
-    return (S1 + 1) * vec + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1 * sizeof(double2) + (size_t)CAGCR_MAX_S * sizeof(double2) + 64;
+    return (S1 + 2) * vec + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1 * sizeof(double2) + (size_t)CAGCR_MAX_S * sizeof(double2) + 256;
 }
 
-int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
-                    void* work_dev, double* info_dev, void* stream) {
+// schur_parity < 0: the operator is A (coarse_op_apply).  schur_parity = 0 | 1: the operator is the
+// left-preconditioned Schur operator on that parity, Shat_p v = v - Dhat_pq Dhat_qp v, two
+// parity-restricted launches on this handle's (block-preconditioned) links.
+static int cagcr_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                      int schur_parity, void* work_dev, double* info_dev, void* stream) {
     if (!op) return fail(COARSE_EINVAL, "cagcr: op is NULL");
     if (!op->links) return fail(COARSE_ENOTREADY, "cagcr: coarse_op_set_links has not been called");
     if (!b_dev || !x_dev || !work_dev) return fail(COARSE_EINVAL, "cagcr: NULL pointer");
@@ -692,6 +695,25 @@ int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int 
     double2* alpha = partial + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1;
     const int vgrid = op->num_sms * 4;
     int launches = 0, rc;
+    float2* tmp = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(alpha + CAGCR_MAX_S) + 64);
+    tmp = reinterpret_cast<float2*>((reinterpret_cast<uintptr_t>(tmp) + 15) & ~(uintptr_t)15);
+    if (schur_parity >= 0) {
+        for (int mu = 0; mu < 4; ++mu)
+            if (op->lat.L[mu] & 1) return fail(COARSE_EINVAL, "cagcr_schur: the even/odd decomposition needs even extents");
+        // sites of the other parity are never written by the parity-restricted applies: they must read as zero
+        cudaError_t e = cudaMemsetAsync(work_dev, 0, (size_t)(S1 + 1) * vec, st);
+        if (e != cudaSuccess) return cuda_fail(e, "cagcr_schur: memset work");
+    }
+    auto apply_op = [&](const void* in, void* out) -> int {
+        if (schur_parity < 0) {
+            ++launches;
+            return coarse_op_apply(op, in, out, 1, 0, stream);
+        }
+        launches += 2;
+        int r = coarse_op_apply_parts(op, nullptr, in, tmp, 1, 0, 1 - schur_parity, COARSE_LOCAL_NONE, 0.f, 1.f, stream);
+        if (r != COARSE_OK) return r;
+        return coarse_op_apply_parts(op, in, tmp, out, 1, 0, schur_parity, COARSE_LOCAL_IDENTITY, 1.f, -1.f, stream);
+    };
     // s + 2 slots used as a ring: p_k = slot[(base + k) % (s+2)], k = 0..s, and the update writes the new
     // residual into slot[(base + s + 1) % (s+2)], which is p_0 of the next cycle.  In the first cycle
     // with x = 0 the residual is b itself (no copy): p_0 points at b and slot[base] stays unused.
@@ -703,9 +725,8 @@ int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int 
         if (e != cudaSuccess) return cuda_fail(e, "cagcr: memset x");
         p0_is_b = true;
     } else {
-        rc = coarse_op_apply(op, x_dev, slot[1], 1, 0, stream);
+        rc = apply_op(x_dev, slot[1]);
         if (rc != COARSE_OK) return rc;
-        ++launches;
         cagcr_residual_kernel<<<vgrid, 256, 0, st>>>(static_cast<const float2*>(b_dev), slot[1], n, slot[0]);
         ++launches;
     }
@@ -715,9 +736,8 @@ int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int 
         if (p0_is_b) v.p[0] = static_cast<const float2*>(b_dev);
         float2* r_out = slot[(base + s + 1) % NS];
         for (int k = 0; k < s; ++k) {
-            rc = coarse_op_apply(op, v.p[k], const_cast<float2*>(v.p[k + 1]), 1, 0, stream);
+            rc = apply_op(v.p[k], const_cast<float2*>(v.p[k + 1]));
             if (rc != COARSE_OK) return rc;
-            ++launches;
         }
         cagcr_gram_kernel<<<CAGCR_GRAM_BLOCKS, 256, 0, st>>>(v, n, s, partial);
         cagcr_solve_kernel<<<1, 320, 0, st>>>(partial, CAGCR_GRAM_BLOCKS, s, alpha, info_dev ? info_dev + 3 * c : nullptr);
@@ -730,6 +750,17 @@ int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int 
     if (e != cudaSuccess) return cuda_fail(e, "cagcr kernel launch");
     op->last_launches = launches;
     return COARSE_OK;
+}
+
+int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                    void* work_dev, double* info_dev, void* stream) {
+    return cagcr_impl(op, b_dev, x_dev, s, cycles, x_is_zero, -1, work_dev, info_dev, stream);
+}
+
+int coarse_op_cagcr_schur(coarse_op_t* op_hat, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                          int parity, void* work_dev, double* info_dev, void* stream) {
+    if (parity != 0 && parity != 1) return fail(COARSE_EINVAL, "cagcr_schur: parity must be 0 (even) or 1 (odd)");
+    return cagcr_impl(op_hat, b_dev, x_dev, s, cycles, x_is_zero, parity, work_dev, info_dev, stream);
 }
 
 int coarse_op_probe_read(const void* src_dev, size_t bytes, int stage_bytes, int stages, void* stream) {

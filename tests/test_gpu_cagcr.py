@@ -92,6 +92,40 @@ def test_cagcr_reduces_the_residual_on_a_baseline_shaped_operator(oracle_lib):
     assert res["r_gpu"] <= 1e-4 * res["norms"][0]
 
 
+@pytest.mark.parametrize("dims,Nc", [((4, 4, 4, 4), 48), ((2, 4, 2, 4), 128)])
+@pytest.mark.parametrize("parity", [0, 1])
+@pytest.mark.parametrize("x_is_zero", [True, False])
+def test_cagcr_on_the_schur_hat_operator(oracle_lib, dims, Nc, parity, x_is_zero):
+    """The paper's level-2/3 combination (Table 1): CA-GCR(8) on the Schur-preconditioned operator."""
+    V, s, cycles = synth.lattice_volume(dims), 8, 2
+    links = synth.make_arbitrary_links(dims, Nc, 7).numpy()
+    links[:, 0] += 6.0 * np.eye(Nc, dtype=np.complex64)
+    hat = oracle_lib.hat_links(links).astype(np.complex64)
+    par = oracle_lib.site_parities(dims)
+    mask = torch.as_tensor(par == parity, device="cuda")
+    b = synth.make_vectors(dims, Nc, 1, 8, device="cuda")
+    b[~mask] = 0
+    x = torch.zeros_like(b) if x_is_zero else 0.05 * synth.make_vectors(dims, Nc, 1, 9, device="cuda")
+    x[~mask] = 0
+    x0_h = x.cpu().numpy().reshape(-1)
+    op = cop.CoarseOp(dims, Nc).set_links(torch.as_tensor(hat, device="cuda"))
+    info = torch.zeros((cycles, 3), dtype=torch.float64, device="cuda")
+    op.cagcr(b, x, s=s, cycles=cycles, x_is_zero=x_is_zero, info=info, schur_parity=parity)
+    torch.cuda.synchronize()
+    assert op.last_launches == cycles * (2 * s + 3) + (0 if x_is_zero else 3)
+    f = lambda v: oracle_lib.schur_hat_apply(dims, Nc, hat, v.reshape(V, Nc, 1), parity).reshape(-1)
+    b_h = b.cpu().numpy().reshape(-1)
+    x_ref, norms = oracle_lib.cagcr(f, b_h, x0_h, s, cycles)
+    x_gpu = x.cpu().numpy().reshape(-1)
+    assert np.all(x_gpu.reshape(V, Nc)[par != parity] == 0)
+    r_gpu = np.linalg.norm(b_h.astype(np.complex128) - f(x_gpu))
+    assert abs(r_gpu - norms[-1]) <= 1e-4 * norms[-1] + 5e-5 * norms[0], (r_gpu, norms)
+    assert norms[-1] < 0.1 * norms[0]
+    info_h = info.cpu().numpy()
+    assert abs(np.sqrt(info_h[0, 0]) - norms[0]) <= 1e-5 * norms[0]
+    op.close()
+
+
 def test_cagcr_is_bit_reproducible():
     dims, Nc = (4, 4, 2, 2), 48
     links = synth.make_arbitrary_links(dims, Nc, 1, device="cuda")
