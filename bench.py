@@ -660,12 +660,15 @@ def main():
     ap.add_argument("--keep-links", type=int, default=0, help="COARSE_OPT_KEEP_LINKS override (0 auto, 1 never, 2 always)")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="time all K steps as one CUDA graph (auto: when the links fit 2x L2)")
+    ap.add_argument("--nrhs", type=int, default=0, help="override the config's number of right-hand sides")
     ap.add_argument("--hvec", action="store_true",
                     help="half-precision INPUT vectors (int16 + per-site norm, row f2) through coarse_op_apply_hvec")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     args = ap.parse_args()
     cfg = synth.config(args.config)
+    if args.nrhs:
+        cfg["nrhs"] = args.nrhs
     daggers = [0, 1] if args.dagger == "both" else [int(args.dagger)]
     if args.workload == "schur":
         return run_schur(args, cfg)

@@ -165,4 +165,20 @@ __device__ __forceinline__ float2 unpack_i16x2(uint32_t w) {
     return make_float2(__uint_as_float(lo) - 8421376.0f, __uint_as_float(hi) - 8421376.0f);
 }
 
+// The same decode through the conversion unit (I2F on the quarter-rate XU pipe).  The int16 STREAM
+// kernels decode XU of the 4 words of a link quad this way: with everything on the ALU/FMA pipes the
+// kernel is issue-bound (68 % of the issue slots, ncu) while the XU pipe idles, and with everything on
+// the XU pipe that pipe is the limiter (70 % busy).  Measured on C4 (sustained): dagger = 0
+// 2.29 / 2.25 / 2.16 / 2.30 ms for XU = 0 / 1 / 2 / 3, dagger = 1 2.42 / 2.31 / 2.39 / 2.40 ms.
+__device__ __forceinline__ float2 unpack_i16x2_xu(uint32_t w) {
+    return make_float2((float)(short)(w & 0xffffu), (float)(short)(w >> 16));
+}
+template <int XU>
+__device__ __forceinline__ void unpack_i16_quad(const uint4& t, float2& m0, float2& m1, float2& m2, float2& m3) {
+    m0 = unpack_i16x2(t.x);
+    m1 = XU >= 3 ? unpack_i16x2_xu(t.y) : unpack_i16x2(t.y);
+    m2 = XU >= 2 ? unpack_i16x2_xu(t.z) : unpack_i16x2(t.z);
+    m3 = XU >= 1 ? unpack_i16x2_xu(t.w) : unpack_i16x2(t.w);
+}
+
 }  // namespace coarse

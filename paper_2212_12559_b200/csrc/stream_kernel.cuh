@@ -295,8 +295,8 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                             const uint32_t a = lbase + rl * ROWBYTES + ps * QP * 16;
                             if constexpr (I16) {
                                 const uint4 t = ptx::lds128u(a);
-                                const float2 m0 = unpack_i16x2(t.x), m1 = unpack_i16x2(t.y);
-                                const float2 m2 = unpack_i16x2(t.z), m3 = unpack_i16x2(t.w);
+                                float2 m0, m1, m2, m3;
+                                unpack_i16_quad<2>(t, m0, m1, m2, m3);
                                 cmac<false>(acc[k], m0.x, m0.y, v[ps][0]);
                                 cmac<false>(acc[k], m1.x, m1.y, v[ps][1]);
                                 cmac<false>(acc[k], m2.x, m2.y, v[ps][2]);
@@ -372,8 +372,8 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                                 const uint32_t a = lbase + rl * ROWBYTES + ps * QP * 16;
                                 if constexpr (I16) {
                                     const uint4 t = ptx::lds128u(a);
-                                    const float2 m0 = unpack_i16x2(t.x), m1 = unpack_i16x2(t.y);
-                                    const float2 m2 = unpack_i16x2(t.z), m3 = unpack_i16x2(t.w);
+                                    float2 m0, m1, m2, m3;
+                                    unpack_i16_quad<1>(t, m0, m1, m2, m3);
                                     cmac<true>(acc[ps][0], m0.x, m0.y, vj);
                                     cmac<true>(acc[ps][1], m1.x, m1.y, vj);
                                     cmac<true>(acc[ps][2], m2.x, m2.y, vj);
