@@ -65,12 +65,12 @@ enum {
     COARSE_ENOMEM = -5
 };
 
-/* Kernel families.  AUTO picks STREAM for nrhs = 1, TENSOR for the block shapes it covers, BLOCK
+/* Kernel families.  AUTO picks STREAM for nrhs <= 4, TENSOR for the block shapes it covers, BLOCK
  * for the other nrhs <= 16, each when Nc is in the compiled set {32,48,64,96,128,192}; else SIMPLE.  Every family computes the same operation; tests run parity on each. */
 enum {
     COARSE_PATH_AUTO = 0,
     COARSE_PATH_SIMPLE = 1,  /* one thread per output element, any even Nc, any nrhs             */
-    COARSE_PATH_STREAM = 2,  /* persistent TMA-bulk -> smem ring -> CUDA-core consumers           */
+    COARSE_PATH_STREAM = 2,  /* persistent TMA-bulk -> smem ring -> CUDA-core consumers, nrhs <= 4 */
     COARSE_PATH_TENSOR = 3,  /* block apply on tcgen05 tensor cores (3xTF32), nrhs in {8,16}, c64   */
     COARSE_PATH_BLOCK = 4    /* block apply on the CUDA cores (same TMA ring), nrhs <= 16          */
 };

@@ -14,6 +14,7 @@
 #include "quantize_kernel.cuh"
 #include "simple_kernel.cuh"
 #include "stream_kernel.cuh"
+#include "stream_mr_kernel.cuh"
 #include "block_kernel.cuh"
 #include "tensor_kernel.cuh"
 #include "probe_kernel.cuh"
@@ -149,6 +150,72 @@ bool stream_supports(int Nc, int nrhs) {
     switch (Nc) {
         case 32: case 48: case 64: case 96: case 128: case 192: return true;
         default: return false;
+    }
+}
+
+bool stream_mr_supports(int Nc, int nrhs) { return stream_supports(Nc, 1) && nrhs >= 2 && nrhs <= 4; }
+
+// ---------------------------------------------------------------- STREAM-MR dispatch (2 <= nrhs <= 4)
+template <int NC, bool I16, bool DAG, int R>
+int launch_stream_mr_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
+    using Gm = StreamGeom<NC, I16, false, false>;
+    using Gr = StreamMrGeom<NC, I16, R>;
+    StreamParams p = base;
+    p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
+    int stages = (op->max_smem - Gr::fixed_bytes(DAG)) / (Gr::stage_bytes(DAG) + 16);
+    if (stages > 12) stages = 12;
+    if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM-MR: shared memory too small for Nc=%d nrhs=%d", NC, R);
+    int want = (114688 + Gr::stage_bytes(DAG) / 2) / Gr::stage_bytes(DAG);
+    if (want < 4) want = 4;
+    if (op->stages_opt > 0) want = op->stages_opt;
+    if (stages > want) stages = want;
+    p.stages = stages;
+    const int smem = Gr::smem_bytes(DAG, stages);
+    auto kern = coarse_apply_stream_mr<NC, I16, DAG, R>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream-mr kernel)");
+    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
+    if (grid > p.n_items) grid = p.n_items;
+    kern<<<grid, Gm::THREADS, smem, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "stream-mr kernel launch");
+    return COARSE_OK;
+}
+
+template <int NC, int R>
+int launch_stream_mr_r(const coarse_op* op, const StreamParams& p, int dagger, cudaStream_t stream) {
+    if (op->prec == COARSE_LINK_I16)
+        return dagger ? launch_stream_mr_t<NC, true, true, R>(op, p, stream) : launch_stream_mr_t<NC, true, false, R>(op, p, stream);
+    return dagger ? launch_stream_mr_t<NC, false, true, R>(op, p, stream) : launch_stream_mr_t<NC, false, false, R>(op, p, stream);
+}
+
+template <int NC>
+int launch_stream_mr_nc(const coarse_op* op, const StreamParams& p, int nrhs, int dagger, cudaStream_t stream) {
+    switch (nrhs) {
+        case 2: return launch_stream_mr_r<NC, 2>(op, p, dagger, stream);
+        case 3: return launch_stream_mr_r<NC, 3>(op, p, dagger, stream);
+        default: return launch_stream_mr_r<NC, 4>(op, p, dagger, stream);
+    }
+}
+
+int launch_stream_mr(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, cudaStream_t stream) {
+    StreamParams p = {};
+    p.lat = op->lat;
+    p.links = static_cast<const unsigned char*>(op->links);
+    p.scales = op->scales;
+    p.in = static_cast<const float2*>(in);
+    p.out = static_cast<float2*>(out);
+    p.keep_links = op->keep_opt == 2 || (op->keep_opt == 0 && coarse_op_link_bytes(op) <= (size_t)op->l2_bytes / 2);
+    p.parity = 2;
+    p.n_sites = op->lat.V;
+    switch (op->Nc) {
+        case 32: return launch_stream_mr_nc<32>(op, p, nrhs, dagger, stream);
+        case 48: return launch_stream_mr_nc<48>(op, p, nrhs, dagger, stream);
+        case 64: return launch_stream_mr_nc<64>(op, p, nrhs, dagger, stream);
+        case 96: return launch_stream_mr_nc<96>(op, p, nrhs, dagger, stream);
+        case 128: return launch_stream_mr_nc<128>(op, p, nrhs, dagger, stream);
+        case 192: return launch_stream_mr_nc<192>(op, p, nrhs, dagger, stream);
+        default: return fail(COARSE_EUNSUPPORTED, "STREAM path is not compiled for Nc=%d", op->Nc);
     }
 }
 
@@ -507,7 +574,7 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int path = op->path_opt;
     if (path == COARSE_PATH_AUTO)
-        path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM
+        path = (stream_supports(op->Nc, nrhs) || stream_mr_supports(op->Nc, nrhs)) ? COARSE_PATH_STREAM
                : (tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok) ? COARSE_PATH_TENSOR
                : block_supports(op->Nc, nrhs)                                  ? COARSE_PATH_BLOCK
                                                                                : COARSE_PATH_SIMPLE;
@@ -521,9 +588,12 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
             return fail(COARSE_EUNSUPPORTED, "apply: BLOCK path covers nrhs <= 16 (got Nc=%d nrhs=%d)", op->Nc, nrhs);
         rc = launch_block(op, in_dev, out_dev, nrhs, dagger, st);
     } else if (path == COARSE_PATH_STREAM) {
-        if (!stream_supports(op->Nc, nrhs))
-            return fail(COARSE_EUNSUPPORTED, "apply: STREAM path does not cover Nc=%d nrhs=%d", op->Nc, nrhs);
-        rc = launch_stream(op, in_dev, out_dev, dagger, kPlain, st);
+        if (stream_mr_supports(op->Nc, nrhs))
+            rc = launch_stream_mr(op, in_dev, out_dev, nrhs, dagger, st);
+        else if (!stream_supports(op->Nc, nrhs))
+            return fail(COARSE_EUNSUPPORTED, "apply: STREAM path covers nrhs <= 4 (got Nc=%d nrhs=%d)", op->Nc, nrhs);
+        else
+            rc = launch_stream(op, in_dev, out_dev, dagger, kPlain, st);
     } else {
         rc = launch_simple(op, in_dev, out_dev, nrhs, dagger, kPlain, st);
     }

@@ -114,6 +114,27 @@ def test_block_path_cuda_cores(oracle_lib, dims, Nc, prec, nrhs, dagger):
     _run(oracle_lib, dims, Nc, prec, nrhs, dagger, cop.PATH_BLOCK)
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (1, 1, 1, 1)])
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("nrhs", [2, 3, 4])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_stream_path_few_rhs(oracle_lib, dims, Nc, prec, nrhs, dagger):
+    """STREAM-MR: 2-4 right-hand sides on the streaming kernel (3 RHS = one propagator)."""
+    if Nc >= 128 and dims == (4, 4, 4, 4):
+        dims = (2, 4, 2, 2)
+    _run(oracle_lib, dims, Nc, prec, nrhs, dagger, cop.PATH_STREAM)
+
+
+@pytest.mark.parametrize("grid,stages", [(1, 2), (7, 3), (1000, 12)])
+def test_stream_few_rhs_any_grid(oracle_lib, grid, stages):
+    for dagger in (0, 1):
+        _run(oracle_lib, (5, 3, 4, 7), 48, cop.LINK_I16, 3, dagger, cop.PATH_STREAM, grid=grid,
+             opts={cop.OPT_STAGES: stages}, hermitian=False)
+        _run(oracle_lib, (3, 3, 2, 2), 128, cop.LINK_C64, 4, dagger, cop.PATH_STREAM, grid=grid,
+             opts={cop.OPT_STAGES: stages})
+
+
 @pytest.mark.parametrize("grid", [1, 7, 1000])
 def test_block_path_any_grid(oracle_lib, grid):
     for dagger in (0, 1):
@@ -125,7 +146,8 @@ def test_block_path_any_grid(oracle_lib, grid):
 def test_auto_path_selection():
     dims = (2, 2, 2, 2)
     cases = [(48, cop.LINK_C64, 1, cop.PATH_STREAM), (48, cop.LINK_C64, 16, cop.PATH_TENSOR),
-             (48, cop.LINK_C64, 3, cop.PATH_BLOCK), (64, cop.LINK_I16, 16, cop.PATH_BLOCK),
+             (48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_STREAM),
+             (48, cop.LINK_C64, 5, cop.PATH_BLOCK), (64, cop.LINK_I16, 16, cop.PATH_BLOCK),
              (96, cop.LINK_C64, 8, cop.PATH_BLOCK), (48, cop.LINK_C64, 17, cop.PATH_SIMPLE),
              (6, cop.LINK_C64, 2, cop.PATH_SIMPLE)]
     for Nc, prec, nrhs, want in cases:
