@@ -294,34 +294,52 @@ def coarse_apply_hvec(dims, Nc: int, links, vec_q, vec_norms, nrhs: int = 1, dag
 
 
 # ----------------------------------------------------------------------------- CA-GCR(s) (row f3)
+def _apply_fp64(apply_fn, v):
+    """A v for a complex128 v through an operator that takes complex64 input: A is linear, so
+    A v = A hi + A lo with hi = complex64(v), lo = complex64(v - hi) (error ~1e-15 |v|)."""
+    hi = v.astype(np.complex64)
+    lo = (v - hi.astype(np.complex128)).astype(np.complex64)
+    return apply_fn(hi) + apply_fn(lo)
+
+
 def cagcr(apply_fn, b, x0, s: int, cycles: int = 1):
-    """Communication-avoiding GCR(s), the paper's smoother ("CA-GCR(8)", Table 1 L116/L122/
-    L130), power basis (reading R23).  One cycle, by its definition:
-        r0 = b - A x0;   p_k = A^k r0, k = 0..s-1;   q_k = A p_k = p_{k+1}
-        alpha = argmin_a || r0 - sum_k a_k q_k ||_2          (numpy.linalg.lstsq on the tall matrix Q, columns
-                                                              scaled to unit norm, NO singular-value cut-off:
-                                                              the power basis reaches cond ~1e11 and the
-                                                              default rcond would silently shrink the space)
-        x = x0 + sum_k alpha_k p_k;   r = r0 - sum_k alpha_k q_k
-    i.e. the residual is minimised over x0 + K_s(A, r0), the iterate GMRES(s)/GCR(s) define.  The s+1
-    basis vectors are rounded to complex64 where the CUDA path stores them; everything else is fp64.
+    """Communication-avoiding GCR(s), the paper's smoother / coarsest-level solver ("CA-GCR(8)",
+    Table 1 L116/L122/L130, "Chebyshev-basis CA-GCR(16)" L134; reading R23).  One cycle, by its
+    definition, minimises the residual over the Krylov space:
+        r0 = b - A x0;    x = x0 + argmin_{z in K_s(A, r0)} || r0 - A z ||_2,   K_s = span{r0, A r0, .., A^(s-1) r0}
+    The definition names no basis (power, Chebyshev, ... span the same space), so the oracle evaluates it the
+    numerically safest way, entirely in fp64: an orthonormal basis of K_s by Arnoldi with re-orthogonalisation,
+    then a dense least-squares problem for the coefficients (numpy.linalg.lstsq, no cut-off).  A CUDA path
+    is free to build the space however it likes; how close it gets to this minimum is what is tested.
     apply_fn(v complex64 [n]) -> complex128 [n].  Returns (x complex128, [||r||_2 before each cycle and
     after the last])."""
     b = np.asarray(b).reshape(-1).astype(np.complex128)
     x = np.asarray(x0).reshape(-1).astype(np.complex128)
     norms = []
-    r = b - apply_fn(x.astype(np.complex64)) if np.any(x != 0) else b.copy()
+    r = b - _apply_fp64(apply_fn, x) if np.any(x != 0) else b.copy()
     for _ in range(cycles):
-        norms.append(float(np.linalg.norm(r)))
-        P = [r.astype(np.complex64)]
-        for _k in range(s):
-            P.append(apply_fn(P[-1]).astype(np.complex64))
-        Pm = np.stack([p.astype(np.complex128) for p in P], axis=1)       # n x (s+1)
-        Q = Pm[:, 1:]
-        d = np.linalg.norm(Q, axis=0)
-        d[d == 0] = 1.0
-        alpha = np.linalg.lstsq(Q / d, Pm[:, 0], rcond=1e-300)[0] / d
-        x = x + Pm[:, :s] @ alpha
-        r = Pm[:, 0] - Q @ alpha
+        beta = float(np.linalg.norm(r))
+        norms.append(beta)
+        if beta == 0.0:
+            continue
+        V = [r / beta]                       # orthonormal basis of K_s
+        AV = []                              # A V_k
+        for k in range(s):
+            w = _apply_fp64(apply_fn, V[k])
+            AV.append(w)
+            if k + 1 < s:
+                u = w.copy()
+                for _pass in range(2):       # modified Gram-Schmidt, twice
+                    for q in V:
+                        u -= np.vdot(q, u) * q
+                nu = float(np.linalg.norm(u))
+                if nu <= 1e-14 * float(np.linalg.norm(w)):
+                    break                    # the Krylov space is exhausted (invariant subspace)
+                V.append(u / nu)
+        Vm = np.stack(V, axis=1)
+        Qm = np.stack(AV[:Vm.shape[1]], axis=1)
+        y = np.linalg.lstsq(Qm, r, rcond=1e-300)[0]
+        x = x + Vm @ y
+        r = r - Qm @ y
     norms.append(float(np.linalg.norm(r)))
     return x, norms
