@@ -587,11 +587,16 @@ def run_cagcr(args, cfg):
         raise RuntimeError("--workload cagcr is a single-GPU measurement")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    dims, Nc, s = cfg["dims"], cfg["Nc"], 8
+    dims, Nc, s = cfg["dims"], cfg["Nc"], (16 if args.cheb else 8)
     V = synth.lattice_volume(dims)
     prec = cop.LINK_I16 if cfg["links"] == "i16" else cop.LINK_C64
     links = synth.make_gamma_hermitian_links(dims, Nc, cfg["seed"], device=dev)
     links[:, 0] += 12.0 * torch.eye(Nc, dtype=torch.complex64, device=dev)
+
+    def smooth(work=None):
+        if args.cheb:      # the hopping part has spectral radius ~4.1 around the shifted diagonal 12.1
+            return op.cagcr_cheb(b, x, 7.5, 16.7, s=s, cycles=1, work=work, info=info)
+        return op.cagcr(b, x, s=s, cycles=1, work=work, info=info)
     scales = None
     if prec == cop.LINK_I16:
         q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device=dev)
@@ -603,17 +608,17 @@ def run_cagcr(args, cfg):
     x = torch.zeros_like(b)
     op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
     info = torch.zeros((1, 3), dtype=torch.float64, device=dev)
-    work = op.cagcr(b, x, s=s, cycles=1, info=info)
+    work = smooth()
     stream = torch.cuda.current_stream()
     for _ in range(max(args.warmup, 3)):
-        op.cagcr(b, x, s=s, cycles=1, work=work, info=info)
+        smooth(work)
     torch.cuda.synchronize()
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clocks:
         t0.record(stream)
         for _ in range(args.steps):
-            op.cagcr(b, x, s=s, cycles=1, work=work, info=info)
+            smooth(work)
         t1.record(stream)
         tmp = torch.empty_like(b)
         a0.record(stream)
@@ -629,11 +634,12 @@ def run_cagcr(args, cfg):
         "metric": METRIC, "value": s * V * args.steps / (t0.elapsed_time(t1) * 1e-3), "unit": UNIT, "n_gpus": 1,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_cycle, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "CA-GCR(8) smoother cycle on the %s lattice, Nc=%d, %s links (X shifted by 12): 8 applies + "
-                               "Gram + solve + update per step" % ("x".join(map(str, dims)), Nc, cfg["links"]),
+        "config": {"workload": "%s cycle on the %s lattice, Nc=%d, %s links (X shifted by 12): %d applies + "
+                               "Gram + solve + update per step" % ("Chebyshev-basis CA-GCR(16)" if args.cheb else "CA-GCR(8)",
+                                                                   "x".join(map(str, dims)), Nc, cfg["links"], s),
                    "seed": cfg["seed"]},
-        "clocks": clocks.summary(), "gpu_launches": (s + 3) * args.steps,
-        "cagcr": {"ms_per_cycle": ms_cycle, "ms_of_8_plain_applies": ms_applies,
+        "clocks": clocks.summary(), "gpu_launches": ((2 * s + 2) if args.cheb else (s + 3)) * args.steps,
+        "cagcr": {"ms_per_cycle": ms_cycle, "ms_of_s_plain_applies": ms_applies, "s": s,
                   "vector_side_share": 1.0 - ms_applies / ms_cycle,
                   "residual_reduction_one_cycle": float(np.sqrt(max(inf[1], 0.0) / inf[0])) if inf[0] > 0 else None,
                   "basis_vectors_kept": int(inf[2])},
@@ -660,6 +666,7 @@ def main():
     ap.add_argument("--keep-links", type=int, default=0, help="COARSE_OPT_KEEP_LINKS override (0 auto, 1 never, 2 always)")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="time all K steps as one CUDA graph (auto: when the links fit 2x L2)")
+    ap.add_argument("--cheb", action="store_true", help="--workload cagcr: Chebyshev-basis CA-GCR(16) instead of CA-GCR(8)")
     ap.add_argument("--nrhs", type=int, default=0, help="override the config's number of right-hand sides")
     ap.add_argument("--hvec", action="store_true",
                     help="half-precision INPUT vectors (int16 + per-site norm, row f2) through coarse_op_apply_hvec")

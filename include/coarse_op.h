@@ -187,6 +187,19 @@ int coarse_op_cagcr_schur(coarse_op_t* op_hat, const void* b_dev, void* x_dev, i
 int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
                     void* work_dev, double* info_dev, void* stream);
 
+/* CA-GCR(s) with a CHEBYSHEV basis (the paper's coarsest-level solver is a "Chebyshev-basis CA-GCR(16)",
+ * PAPER.md:L134 Table 1): p_k = T_k((A - c)/d) r0 with [lambda_min, lambda_max] = [c - d, c + d] an
+ * interval that roughly encloses the operator's spectrum (real bounds, supplied by the caller).  The
+ * basis spans the same Krylov space as coarse_op_cagcr's power basis - the minimiser is the same - but
+ * stays well conditioned, so s = 16 keeps all its digits.  schur_parity = -1: the operator is A;
+ * 0 | 1: the Schur-hat operator of coarse_op_cagcr_schur.  Work: coarse_op_cagcr_cheb_work_bytes(op, s)
+ * (2s + 2 vectors).  2s + 2 launches per cycle for A (s applies, s - 1 recurrence steps, Gram, solve,
+ * update).  info_dev as for coarse_op_cagcr. */
+size_t coarse_op_cagcr_cheb_work_bytes(const coarse_op_t* op, int s);
+int coarse_op_cagcr_cheb(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                         float lambda_min, float lambda_max, int schur_parity, void* work_dev, double* info_dev,
+                         void* stream);
+
 /* Diagnostic: stream floor(bytes / stage_bytes) * stage_bytes bytes of device memory through the STREAM
  * kernels' TMA ring (one CTA per SM, `stages` slots of `stage_bytes`, evict_first bulk copies) with an
  * idle consumer.  Timed by the caller with CUDA events it gives the pure-read ceiling of this GPU for

@@ -28,7 +28,8 @@ EXPORTS = (
     "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_parts", "coarse_op_apply_hvec",
     "coarse_op_quantize_vec_i16", "coarse_op_apply_host",
     "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_probe_read", "coarse_op_cagcr_work_bytes",
-    "coarse_op_cagcr", "coarse_op_cagcr_schur", "coarse_op_destroy",
+    "coarse_op_cagcr", "coarse_op_cagcr_schur", "coarse_op_cagcr_cheb_work_bytes",
+    "coarse_op_cagcr_cheb", "coarse_op_destroy",
     "coarse_op_last_error",
 )
 
@@ -85,6 +86,10 @@ def lib() -> ctypes.CDLL:
     L.coarse_op_cagcr.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp, vp]
     L.coarse_op_cagcr_schur.restype = ci
     L.coarse_op_cagcr_schur.argtypes = [vp, vp, vp, ci, ci, ci, ci, vp, vp, vp]
+    L.coarse_op_cagcr_cheb_work_bytes.restype = sz
+    L.coarse_op_cagcr_cheb_work_bytes.argtypes = [vp, ci]
+    L.coarse_op_cagcr_cheb.restype = ci
+    L.coarse_op_cagcr_cheb.argtypes = [vp, vp, vp, ci, ci, ci, ctypes.c_float, ctypes.c_float, ci, vp, vp, vp]
     L.coarse_op_probe_read.restype = ci
     L.coarse_op_probe_read.argtypes = [vp, sz, ci, ci, vp]
     L.coarse_op_destroy.restype = None
@@ -264,6 +269,28 @@ def coarse_op_cagcr(op: int, b, x, s: int, cycles: int = 1, x_is_zero: bool = Tr
                                            int(schur_parity), _ptr(work), _ptr(info), _stream_handle(stream)))
 
 
+def coarse_op_cagcr_cheb_work_bytes(op: int, s: int) -> int:
+    return int(lib().coarse_op_cagcr_cheb_work_bytes(op, int(s)))
+
+
+def coarse_op_cagcr_cheb(op: int, b, x, s: int, lambda_min: float, lambda_max: float, cycles: int = 1,
+                         x_is_zero: bool = True, schur_parity: int = -1, work=None, info=None, stream=None) -> None:
+    """Chebyshev-basis CA-GCR(s) (include/coarse_op.h); same tensors as coarse_op_cagcr, work of
+    coarse_op_cagcr_cheb_work_bytes(op, s) bytes."""
+    for t in (b, x, work):
+        if t is None or not t.is_cuda or not t.is_contiguous():
+            raise ValueError("cagcr_cheb needs contiguous CUDA tensors b, x, work")
+    if work.numel() * work.element_size() < coarse_op_cagcr_cheb_work_bytes(op, s):
+        raise ValueError("cagcr_cheb: work buffer too small")
+    if b.numel() * b.element_size() != coarse_op_vector_bytes(op, 1) or x.numel() != b.numel():
+        raise ValueError("cagcr_cheb: b / x have the wrong size (1 RHS)")
+    if info is not None and (info.numel() < 3 * cycles or info.element_size() != 8 or not info.is_cuda):
+        raise ValueError("cagcr_cheb: info must be a CUDA float64 tensor with 3 * cycles entries")
+    _check(lib().coarse_op_cagcr_cheb(op, _ptr(b), _ptr(x), int(s), int(cycles), 1 if x_is_zero else 0,
+                                      float(lambda_min), float(lambda_max), int(schur_parity), _ptr(work), _ptr(info),
+                                      _stream_handle(stream)))
+
+
 def coarse_op_probe_read(src, stage_bytes: int = 16384, stages: int = 6, stream=None) -> int:
     """Enqueue the read-ceiling probe over the CUDA tensor `src`; returns the bytes it reads."""
     if not src.is_cuda or not src.is_contiguous():
@@ -315,6 +342,14 @@ class CoarseOp:
         if work is None:
             work = torch.empty(coarse_op_cagcr_work_bytes(self._h, s), dtype=torch.uint8, device=b.device)
         coarse_op_cagcr(self._h, b, x, s, cycles, x_is_zero, work, info, stream, schur_parity)
+        return work
+
+    def cagcr_cheb(self, b, x, lambda_min: float, lambda_max: float, s: int = 16, cycles: int = 1,
+                   x_is_zero: bool = True, schur_parity: int = -1, work=None, info=None, stream=None):
+        import torch
+        if work is None:
+            work = torch.empty(coarse_op_cagcr_cheb_work_bytes(self._h, s), dtype=torch.uint8, device=b.device)
+        coarse_op_cagcr_cheb(self._h, b, x, s, lambda_min, lambda_max, cycles, x_is_zero, schur_parity, work, info, stream)
         return work
 
     def apply_host(self, vin_host, vout_host, nrhs: int = 1, dagger: int = 0, stream=None) -> None:

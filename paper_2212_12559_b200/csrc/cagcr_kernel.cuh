@@ -192,4 +192,46 @@ __global__ void __launch_bounds__(256) cagcr_residual_kernel(const float2* b, co
     }
 }
 
+// ---- Chebyshev basis (the paper's coarsest-level solver is a "Chebyshev-basis CA-GCR(16)"):
+// p_k = T_k((A - c)/d) r0 on the interval [lambda_min, lambda_max] = [c - d, c + d] spans the same Krylov
+// space as the power basis but stays well conditioned, so s = 16 no longer drowns in the Gram matrix.
+// With t_k = A p_k:   p_1 = (t_0 - c p_0)/d,   p_{k+1} = (2/d)(t_k - c p_k) - p_{k-1}.
+// out = a*t + b*p + g*pm   (g = 0 and pm ignored for the first step)
+__global__ void __launch_bounds__(256) cagcr_cheb_step_kernel(const float2* t, const float2* p, const float2* pm,
+                                                              float a, float b, float g, long long n, float2* out) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float2 x = t[i], y = p[i];
+        float2 o = make_float2(fmaf(a, x.x, b * y.x), fmaf(a, x.y, b * y.y));
+        if (g != 0.f) {
+            const float2 z = pm[i];
+            o.x = fmaf(g, z.x, o.x);
+            o.y = fmaf(g, z.y, o.y);
+        }
+        out[i] = o;
+    }
+}
+
+// x += sum_{k<s} alpha_k P_k ;  r_out = r0 - sum_{k<s} alpha_k T_k      (P, T: separate vector lists)
+__global__ void __launch_bounds__(256) cagcr_update2_kernel(CagcrVecs P, CagcrVecs T, const float2* r0, long long n, int s,
+                                                            const double2* alpha, float2* x, float2* r_out) {
+    __shared__ float2 al[CAGCR_MAX_S];
+    if (threadIdx.x < s) al[threadIdx.x] = make_float2((float)alpha[threadIdx.x].x, (float)alpha[threadIdx.x].y);
+    __syncthreads();
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        float2 xs = x[i];
+        float2 rs = r0[i];
+#pragma unroll 4
+        for (int k = 0; k < s; ++k) {
+            const float2 a = al[k];
+            const float2 pk = P.p[k][i], tk = T.p[k][i];
+            xs.x = fmaf(a.x, pk.x, fmaf(-a.y, pk.y, xs.x));
+            xs.y = fmaf(a.x, pk.y, fmaf(a.y, pk.x, xs.y));
+            rs.x = fmaf(-a.x, tk.x, fmaf(a.y, tk.y, rs.x));
+            rs.y = fmaf(-a.x, tk.y, fmaf(-a.y, tk.x, rs.y));
+        }
+        x[i] = xs;
+        r_out[i] = rs;
+    }
+}
+
 }  // namespace coarse

@@ -822,6 +822,105 @@ static int cagcr_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int s, in
     return COARSE_OK;
 }
 
+// Chebyshev-basis variant (cagcr_kernel.cuh): P_k = T_k((A - c)/d) r0, T_k = A P_k kept as separate
+// vectors.  Slots: P_0..P_{s-1} | T_0..T_{s-1} | R (the update's output, swapped with P_0 every cycle).
+static int cagcr_cheb_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                           float lambda_min, float lambda_max, int schur_parity, void* work_dev, double* info_dev,
+                           void* stream) {
+    if (!op) return fail(COARSE_EINVAL, "cagcr_cheb: op is NULL");
+    if (!op->links) return fail(COARSE_ENOTREADY, "cagcr_cheb: coarse_op_set_links has not been called");
+    if (!b_dev || !x_dev || !work_dev) return fail(COARSE_EINVAL, "cagcr_cheb: NULL pointer");
+    if (s < 1 || s > CAGCR_MAX_S) return fail(COARSE_EINVAL, "cagcr_cheb: 1 <= s <= %d (got %d)", CAGCR_MAX_S, s);
+    if (cycles < 1) return fail(COARSE_EINVAL, "cagcr_cheb: cycles must be >= 1");
+    if (!(lambda_max > lambda_min)) return fail(COARSE_EINVAL, "cagcr_cheb: need lambda_max > lambda_min");
+    if (!aligned16(b_dev) || !aligned16(x_dev) || !aligned16(work_dev)) return fail(COARSE_EINVAL, "cagcr_cheb: pointers must be 16-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t vec = coarse_op_vector_bytes(op, 1);
+    const long long n = (long long)op->lat.V * op->Nc;
+    const int S1 = s + 1, NSLOT = 2 * s + 1;
+    unsigned char* w = static_cast<unsigned char*>(work_dev);
+    float2* slot[2 * CAGCR_MAX_S + 1];
+    for (int k = 0; k < NSLOT; ++k) slot[k] = reinterpret_cast<float2*>(w + (size_t)k * vec);
+    float2* tmp = reinterpret_cast<float2*>(w + (size_t)NSLOT * vec);
+    double2* partial = reinterpret_cast<double2*>(w + (size_t)(NSLOT + 1) * vec);
+    double2* alpha = partial + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1;
+    const int vgrid = op->num_sms * 4;
+    const float c = 0.5f * (lambda_max + lambda_min), d = 0.5f * (lambda_max - lambda_min);
+    int launches = 0, rc;
+    if (schur_parity >= 0) {
+        for (int mu = 0; mu < 4; ++mu)
+            if (op->lat.L[mu] & 1) return fail(COARSE_EINVAL, "cagcr_cheb: the even/odd decomposition needs even extents");
+        cudaError_t e = cudaMemsetAsync(work_dev, 0, (size_t)NSLOT * vec, st);
+        if (e != cudaSuccess) return cuda_fail(e, "cagcr_cheb: memset work");
+    }
+    auto apply_op = [&](const void* in, void* out) -> int {
+        if (schur_parity < 0) {
+            ++launches;
+            return coarse_op_apply(op, in, out, 1, 0, stream);
+        }
+        launches += 2;
+        int r = coarse_op_apply_parts(op, nullptr, in, tmp, 1, 0, 1 - schur_parity, COARSE_LOCAL_NONE, 0.f, 1.f, stream);
+        if (r != COARSE_OK) return r;
+        return coarse_op_apply_parts(op, in, tmp, out, 1, 0, schur_parity, COARSE_LOCAL_IDENTITY, 1.f, -1.f, stream);
+    };
+    int p0 = 0, rslot = 2 * s;          // slot of P_0 and of the update's output; swapped after every cycle
+    bool p0_is_b = false;
+    if (x_is_zero) {
+        cudaError_t e = cudaMemsetAsync(x_dev, 0, vec, st);
+        if (e != cudaSuccess) return cuda_fail(e, "cagcr_cheb: memset x");
+        p0_is_b = true;
+    } else {
+        rc = apply_op(x_dev, slot[s]);
+        if (rc != COARSE_OK) return rc;
+        cagcr_residual_kernel<<<vgrid, 256, 0, st>>>(static_cast<const float2*>(b_dev), slot[s], n, slot[p0]);
+        ++launches;
+    }
+    for (int cyc = 0; cyc < cycles; ++cyc) {
+        CagcrVecs P, T, Gv;
+        for (int k = 0; k <= CAGCR_MAX_S; ++k) { P.p[k] = nullptr; T.p[k] = nullptr; Gv.p[k] = nullptr; }
+        for (int k = 0; k < s; ++k) {
+            P.p[k] = k == 0 ? (p0_is_b ? static_cast<const float2*>(b_dev) : slot[p0]) : slot[k];
+            T.p[k] = slot[s + k];
+        }
+        for (int k = 0; k < s; ++k) {
+            rc = apply_op(P.p[k], const_cast<float2*>(T.p[k]));
+            if (rc != COARSE_OK) return rc;
+            if (k + 1 < s) {
+                const float a = (k == 0 ? 1.f : 2.f) / d;
+                cagcr_cheb_step_kernel<<<vgrid, 256, 0, st>>>(T.p[k], P.p[k], k == 0 ? P.p[k] : P.p[k - 1], a, -a * c,
+                                                              k == 0 ? 0.f : -1.f, n, const_cast<float2*>(P.p[k + 1]));
+                ++launches;
+            }
+        }
+        Gv.p[0] = P.p[0];
+        for (int k = 0; k < s; ++k) Gv.p[k + 1] = T.p[k];
+        cagcr_gram_kernel<<<CAGCR_GRAM_BLOCKS, 256, 0, st>>>(Gv, n, s, partial);
+        cagcr_solve_kernel<<<1, 320, 0, st>>>(partial, CAGCR_GRAM_BLOCKS, s, alpha, info_dev ? info_dev + 3 * cyc : nullptr);
+        cagcr_update2_kernel<<<vgrid, 256, 0, st>>>(P, T, P.p[0], n, s, alpha, static_cast<float2*>(x_dev), slot[rslot]);
+        launches += 3;
+        if (p0_is_b) { p0 = rslot; rslot = 0; p0_is_b = false; }   // slot 0 was unused while P_0 = b
+        else { const int t2 = p0; p0 = rslot; rslot = t2; }
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "cagcr_cheb kernel launch");
+    op->last_launches = launches;
+    return COARSE_OK;
+}
+
+size_t coarse_op_cagcr_cheb_work_bytes(const coarse_op_t* op, int s) {
+    if (!op || s < 1 || s > CAGCR_MAX_S) return 0;
+    const size_t vec = coarse_op_vector_bytes(op, 1);
+    const size_t S1 = (size_t)s + 1;
+    return (2 * (size_t)s + 2) * vec + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1 * sizeof(double2) + (size_t)CAGCR_MAX_S * sizeof(double2) + 256;
+}
+
+int coarse_op_cagcr_cheb(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                         float lambda_min, float lambda_max, int schur_parity, void* work_dev, double* info_dev,
+                         void* stream) {
+    if (schur_parity < -1 || schur_parity > 1) return fail(COARSE_EINVAL, "cagcr_cheb: schur_parity must be -1 (full operator), 0 or 1");
+    return cagcr_cheb_impl(op, b_dev, x_dev, s, cycles, x_is_zero, lambda_min, lambda_max, schur_parity, work_dev, info_dev, stream);
+}
+
 int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
                     void* work_dev, double* info_dev, void* stream) {
     return cagcr_impl(op, b_dev, x_dev, s, cycles, x_is_zero, -1, work_dev, info_dev, stream);

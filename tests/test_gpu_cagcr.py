@@ -67,11 +67,12 @@ def _case(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero, shift=12.0, seed=101
 def test_cagcr_against_oracle(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero):
     res = _case(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero)
     norms, info = res["norms"], res["info"]
-    # Noise floor of the comparison, relative to ||r0||: complex64 basis vectors (6e-8) times the growth
-    # of the power basis.  For s <= 8 that is ~1e-6.  At s = 16 the power basis (cond > 1e20) is beyond
-    # fp64 normal equations: the factorisation truncates it and the residual stalls at a few 1e-5 of
-    # ||r0|| - which is why the paper's CA-GCR(16) uses a Chebyshev basis, not built here.
-    floor = (2e-6 if s <= 8 else 5e-5) * norms[0]
+    # The oracle is the true minimiser (fp64 Arnoldi).  The CUDA power basis is stored in complex64 and its
+    # Gram matrix squares its conditioning, so how close it gets depends on s (measured on this operator:
+    # x off by 7e-7 / 1.3e-5 / 3.6e-5 and residual floors of 2e-9 / 5e-7 / 3e-5 ||r0|| at s = 4 / 8 / 16).
+    # The Chebyshev basis (test below) holds 3e-7 at every s; that is why the paper uses it at s = 16 (L134).
+    floor = {1: 2e-6, 4: 2e-6, 8: 1e-5, 16: 1e-4}[s] * norms[0]
+    x_bound = {1: 1e-5, 4: 1e-5, 8: 1e-4, 16: 1e-3}[s]
     # the residual the GPU iterate really has is the oracle's optimum
     assert abs(res["r_gpu"] - norms[-1]) <= 1e-4 * norms[-1] + floor, (res["r_gpu"], norms)
     # what the solve kernel reports: ||r0||^2 per cycle and the predicted ||r||^2 after it
@@ -79,8 +80,8 @@ def test_cagcr_against_oracle(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero):
         assert abs(np.sqrt(info[c, 0]) - norms[c]) <= 1e-4 * norms[c] + floor
         assert info[c, 2] == s if s <= 8 else info[c, 2] >= 8          # whole basis kept up to s = 8
     assert abs(np.sqrt(max(info[-1, 1], 0.0)) - norms[-1]) <= 1e-3 * norms[-1] + 5 * floor
-    # the iterate itself, with the basis conditioning in the bound
-    assert res["x_err"] <= 1e-5 + 20 * res["condQ"] * 2e-7, (res["x_err"], res["condQ"])
+    # the iterate itself
+    assert res["x_err"] <= x_bound * cycles, (res["x_err"], res["condQ"])
 
 
 def test_cagcr_reduces_the_residual_on_a_baseline_shaped_operator(oracle_lib):
@@ -123,6 +124,89 @@ def test_cagcr_on_the_schur_hat_operator(oracle_lib, dims, Nc, parity, x_is_zero
     assert norms[-1] < 0.1 * norms[0]
     info_h = info.cpu().numpy()
     assert abs(np.sqrt(info_h[0, 0]) - norms[0]) <= 1e-5 * norms[0]
+    op.close()
+
+
+def _cheb_case(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero, lam=(7.5, 16.5), shift=12.0, seed=201):
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, seed, device="cuda")
+    links[:, 0] += shift * torch.eye(Nc, dtype=torch.complex64, device="cuda")
+    scales = scales_h = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+        scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        torch.cuda.synchronize()
+        links, scales_h = q, scales.cpu().numpy()
+    links_h = links.cpu().numpy()
+    b = synth.make_vectors(dims, Nc, 1, seed + 1, device="cuda")
+    x = torch.zeros_like(b) if x_is_zero else 0.05 * synth.make_vectors(dims, Nc, 1, seed + 2, device="cuda")
+    x0_h = x.cpu().numpy().reshape(-1)
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    info = torch.zeros((cycles, 3), dtype=torch.float64, device="cuda")
+    op.cagcr_cheb(b, x, lam[0], lam[1], s=s, cycles=cycles, x_is_zero=x_is_zero, info=info)
+    torch.cuda.synchronize()
+    assert op.last_launches == cycles * (2 * s + 2) + (0 if x_is_zero else 2)
+    # the same start on the power basis, for comparison
+    xp = torch.zeros_like(b) if x_is_zero else torch.as_tensor(x0_h.reshape(V, Nc, 1), device="cuda").clone()
+    op.cagcr(b, xp, s=s, cycles=cycles, x_is_zero=x_is_zero)
+    torch.cuda.synchronize()
+    f = lambda v: oracle_lib.coarse_apply(dims, Nc, links_h, v.reshape(V, Nc, 1), link_precision=prec,
+                                          scales=scales_h).reshape(-1)
+    b_h = b.cpu().numpy().reshape(-1)
+    x_ref, norms = oracle_lib.cagcr(f, b_h, x0_h, s, cycles)
+    r_cheb = np.linalg.norm(b_h.astype(np.complex128) - f(x.cpu().numpy().reshape(-1)))
+    r_pow = np.linalg.norm(b_h.astype(np.complex128) - f(xp.cpu().numpy().reshape(-1)))
+    op.close()
+    return r_cheb, r_pow, norms, info.cpu().numpy(), rel_l2(x.cpu().numpy().reshape(-1), x_ref)
+
+
+@pytest.mark.parametrize("dims,Nc", [((4, 4, 4, 4), 48), ((2, 2, 2, 4), 128)])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("s,cycles", [(16, 1), (8, 2), (3, 2), (1, 1)])
+@pytest.mark.parametrize("x_is_zero", [True, False])
+def test_cagcr_chebyshev_basis(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero):
+    """Same minimiser as the power basis (the oracle's definition does not name a basis), reached with a
+    well-conditioned basis: the whole basis is kept at s = 16, the iterate matches the fp64 oracle to 1e-5
+    (measured 2-3e-7) and the residual to the single-precision floor, where the power basis stalls at 3e-5."""
+    r_cheb, r_pow, norms, info, x_err = _cheb_case(oracle_lib, dims, Nc, prec, s, cycles, x_is_zero)
+    assert np.all(info[:, 2] == s)                                    # no truncation, even at s = 16
+    assert abs(r_cheb - norms[-1]) <= 1e-4 * norms[-1] + 2e-6 * norms[0], (r_cheb, r_pow, norms)
+    assert r_cheb <= 1.05 * r_pow + 2e-6 * norms[0]                   # never worse than the power basis
+    assert abs(np.sqrt(info[0, 0]) - norms[0]) <= 1e-5 * norms[0]
+    assert x_err <= 1e-5, x_err                                       # the iterate itself, at every s
+
+
+def test_cagcr_chebyshev_on_schur_operator_and_errors(oracle_lib):
+    dims, Nc, parity, s = (4, 4, 4, 4), 48, 0, 12
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, 7).numpy()
+    links[:, 0] += 6.0 * np.eye(Nc, dtype=np.complex64)
+    hat = oracle_lib.hat_links(links).astype(np.complex64)
+    par = oracle_lib.site_parities(dims)
+    mask = torch.as_tensor(par == parity, device="cuda")
+    b = synth.make_vectors(dims, Nc, 1, 8, device="cuda")
+    b[~mask] = 0
+    x = torch.zeros_like(b)
+    op = cop.CoarseOp(dims, Nc).set_links(torch.as_tensor(hat, device="cuda"))
+    info = torch.zeros((1, 3), dtype=torch.float64, device="cuda")
+    op.cagcr_cheb(b, x, 0.3, 1.7, s=s, schur_parity=parity, info=info)       # Shat = 1 - Dhat Dhat: spectrum around 1
+    torch.cuda.synchronize()
+    f = lambda v: oracle_lib.schur_hat_apply(dims, Nc, hat, v.reshape(V, Nc, 1), parity).reshape(-1)
+    b_h = b.cpu().numpy().reshape(-1)
+    x_ref, norms = oracle_lib.cagcr(f, b_h, np.zeros_like(b_h), s, 1)
+    r_gpu = np.linalg.norm(b_h.astype(np.complex128) - f(x.cpu().numpy().reshape(-1)))
+    assert info[0, 2].item() == s
+    assert abs(r_gpu - norms[-1]) <= 1e-4 * norms[-1] + 2e-6 * norms[0], (r_gpu, norms)
+    assert rel_l2(x.cpu().numpy().reshape(-1), x_ref) <= 1e-5
+    L = cop.lib()
+    w = torch.zeros(cop.coarse_op_cagcr_cheb_work_bytes(op._h, s), dtype=torch.uint8, device="cuda")
+    args = lambda lo, hi, sp: (op._h, b.data_ptr(), x.data_ptr(), s, 1, 1, lo, hi, sp, w.data_ptr(), None, None)
+    assert L.coarse_op_cagcr_cheb(*args(2.0, 1.0, -1)) == cop.EINVAL
+    assert L.coarse_op_cagcr_cheb(*args(1.0, 2.0, 2)) == cop.EINVAL
+    assert L.coarse_op_cagcr_cheb(*args(1.0, 2.0, -1)) == cop.OK
+    torch.cuda.synchronize()
+    assert cop.coarse_op_cagcr_cheb_work_bytes(op._h, 17) == 0
     op.close()
 
 
