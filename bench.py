@@ -293,6 +293,8 @@ def run_ours(args, cfg, daggers):
         op.set_option(cop.OPT_FINE, args.fine)
     if args.keep_links:
         op.set_option(cop.OPT_KEEP_LINKS, args.keep_links)
+    if args.pdl:
+        op.set_option(cop.OPT_PDL, 1)
 
     vq = vnorm = None
     if args.hvec:
@@ -668,6 +670,7 @@ def main():
                     help="time all K steps as one CUDA graph (auto: when the links fit 2x L2)")
     ap.add_argument("--cheb", action="store_true", help="--workload cagcr: Chebyshev-basis CA-GCR(16) instead of CA-GCR(8)")
     ap.add_argument("--nrhs", type=int, default=0, help="override the config's number of right-hand sides")
+    ap.add_argument("--pdl", action="store_true", help="COARSE_OPT_PDL: programmatic dependent launch for chained applies")
     ap.add_argument("--hvec", action="store_true",
                     help="half-precision INPUT vectors (int16 + per-site norm, row f2) through coarse_op_apply_hvec")
     ap.add_argument("--no-cpu-baseline", action="store_true")

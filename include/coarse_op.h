@@ -80,7 +80,11 @@ enum {
     COARSE_OPT_GRID = 1,     /* persistent grid size for STREAM/TENSOR; 0 = one CTA per SM        */
     COARSE_OPT_STAGES = 2,   /* cap on the STREAM shared-memory ring depth; 0 = library default   */
     COARSE_OPT_FINE = 3,     /* STREAM dagger=0 small-lattice row-block split: 0 auto, 1 never, 2 always */
-    COARSE_OPT_KEEP_LINKS = 4 /* L2 policy of the link stream: 0 auto (keep if links <= L2/2), 1 evict_first, 2 keep */
+    COARSE_OPT_KEEP_LINKS = 4, /* L2 policy of the link stream: 0 auto (keep if links <= L2/2), 1 evict_first, 2 keep */
+    COARSE_OPT_PDL = 5       /* 1: launch the 1-RHS STREAM kernels with programmatic dependent launch: in a chain
+                                of applies on one stream the next kernel's CTAs start on SMs the previous one
+                                has left and prefetch their link stages before waiting for its output (the
+                                latency-limited small-lattice regime of PAPER.md:L99).  Default 0. */
 };
 
 /* Create an operator descriptor for a periodic lattice dims[0..3] (each >= 1), Nc even and

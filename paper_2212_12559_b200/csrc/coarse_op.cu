@@ -55,6 +55,7 @@ struct coarse_op {
     int stages_opt;
     int fine_opt;
     int keep_opt;
+    int pdl_opt;
     int l2_bytes;
     int last_launches;
     int last_path;
@@ -105,6 +106,24 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
     if (grid > p.n_items) grid = p.n_items;
+    p.pdl = op->pdl_opt ? 1 : 0;
+    if (p.pdl) {
+        // programmatic dependent launch: this kernel may start while the previous kernel of the stream
+        // drains; it orders itself against that kernel's memory with griddepcontrol.wait (stream_kernel.cuh)
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid);
+        cfg.blockDim = dim3(Gm::THREADS);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, kern, p);
+        if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch (PDL)");
+        return COARSE_OK;
+    }
     kern<<<grid, Gm::THREADS, smem, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch");
@@ -474,6 +493,7 @@ coarse_op_t* coarse_op_create(const int dims[4], int Nc, int link_precision) {
     op->stages_opt = 0;
     op->fine_opt = 0;
     op->keep_opt = 0;
+    op->pdl_opt = 0;
     { int l2 = 0; cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev); op->l2_bytes = l2; }
     op->last_launches = 0;
     op->last_path = 0;
@@ -553,6 +573,10 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value) {
         case COARSE_OPT_KEEP_LINKS:
             if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: keep_links must be 0 (auto), 1 (never) or 2 (always)");
             op->keep_opt = value;
+            return COARSE_OK;
+        case COARSE_OPT_PDL:
+            if (value != 0 && value != 1) return fail(COARSE_EINVAL, "set_option: pdl must be 0 or 1");
+            op->pdl_opt = value;
             return COARSE_OK;
         case COARSE_OPT_STAGES:
             if (value < 0 || value == 1) return fail(COARSE_EINVAL, "set_option: stages must be 0 (default) or >= 2");

@@ -51,6 +51,7 @@ struct StreamParams {
     int identity;             // 1: add alpha*u(x) to the result (local = identity)
     int parity;               // 0 even, 1 odd, 2 all sites
     int n_sites;              // sites in the parity set
+    int pdl;                  // 1: launched with programmatic stream serialization (COARSE_OPT_PDL)
     // HV (half-precision input vectors, coarse_op_apply_hvec): `in` points at int16 (re,im) entries
     const float* vnorms;      // fp32 norm per site (nrhs = 1)
 };
@@ -158,6 +159,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
         ptx::fence_mbar_init();
     }
     __syncthreads();
+    if (p.pdl) ptx::pdl_launch_dependents();   // the next kernel's CTAs may take SMs as ours exit
 
     if (warp == W) {
         // ------------------------------------------------------------------ producer
@@ -168,6 +170,21 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
         const uint32_t link_u32 = ptx::smem_u32(link_smem), vec_u32 = ptx::smem_u32(vec_smem);
         int slot = 0;
         uint32_t phase = 0;
+        // PDL: the links do not depend on the previous kernel of the stream, the vectors do.  The first S
+        // stages' LINK copies go out at once (they overlap the previous kernel's tail), their vector copies
+        // are queued; griddepcontrol.wait then makes the previous kernel's output visible and the queue
+        // is flushed.  Every store of this kernel comes after a vector copy, hence after the wait.
+        bool deferring = p.pdl != 0;
+        int n_def = 0;
+        const unsigned char* def_src[12];
+        auto flush_deferred = [&]() {
+            ptx::pdl_wait();
+            if (ptx::elect_one())
+                for (int q = 0; q < n_def; ++q)
+                    ptx::bulk_g2s(vec_u32 + q * VEC_STAGE, def_src[q], VEC_STAGE, full0 + 8u * q, pol_vec);
+            __syncwarp();
+            deferring = false;
+        };
         for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
             const int sidx = DAG ? item : item / NB;
             const int s = (GEN && p.parity != 2) ? parity_site(p.lat, sidx, p.parity) : sidx;
@@ -183,23 +200,28 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
 #pragma unroll 1
                 for (int c = 0; c < (DAG ? NB : 1); ++c) {
                     const int r0 = DAG ? c * RS : rb * RS;
+                    if (deferring && n_def == S) flush_deferred();    // the ring is full: the vectors are needed now
                     ptx::mbar_wait(empty0 + 8u * slot, phase ^ 1u);
+                    const unsigned char* vsrc = DAG ? (vec + r0 * VE) : vec;
                     if (ptx::elect_one()) {
                         ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE + VEC_STAGE);
                         ptx::bulk_g2s(link_u32 + slot * LINK_STAGE, mat + (int64_t)r0 * ROWBYTES, LINK_STAGE,
                                       full0 + 8u * slot, pol_links);
-                        ptx::bulk_g2s(vec_u32 + slot * VEC_STAGE, DAG ? (vec + r0 * VE) : vec, VEC_STAGE,
-                                      full0 + 8u * slot, pol_vec);
+                        if (!deferring)
+                            ptx::bulk_g2s(vec_u32 + slot * VEC_STAGE, vsrc, VEC_STAGE, full0 + 8u * slot, pol_vec);
                     }
+                    if (deferring) def_src[n_def++] = vsrc;            // slot index = position in the queue
                     __syncwarp();
                     if (++slot == S) { slot = 0; phase ^= 1u; }
                 }
             }
         }
+        if (deferring) flush_deferred();
         return;
     }
 
     // ---------------------------------------------------------------------- consumers
+    if ((GEN || HV) && p.pdl) ptx::pdl_wait();      // these variants read the input from global memory themselves
     const int grp = lane / G;          // which of the RPL rows of a warp-wide load
     const int qi = lane % G;           // quad index inside the pass
     const bool active = qi < QP;

@@ -273,6 +273,69 @@ def test_apply_is_graph_capturable(oracle_lib):
     op.close()
 
 
+@pytest.mark.parametrize("dims,Nc,prec", [((4, 4, 4, 4), 48, 0), ((2, 4, 2, 2), 192, 1), ((5, 3, 4, 7), 64, 1), ((1, 1, 1, 2), 32, 0)])
+def test_programmatic_dependent_launch_chain(oracle_lib, dims, Nc, prec):
+    """COARSE_OPT_PDL: a chain of applies where each kernel may start while its predecessor drains, including
+    the ping-pong a -> b -> a whose second kernel WRITES the buffer the first one reads.  Results must be
+    bit-identical to the same chain launched normally, and correct against the oracle."""
+    V = synth.lattice_volume(dims)
+    links, scales, links_h, scales_h = _links_for(dims, Nc, prec, 77, False, oracle_lib)
+    if prec == cop.LINK_C64:
+        links = links * 0.25                      # keep the 6-fold product's magnitude moderate
+        links_h = links.cpu().numpy()
+    else:
+        scales = scales * 0.25
+        scales_h = scales.cpu().numpy()
+    v0 = synth.make_vectors(dims, Nc, 1, 78, device="cuda")
+    outs = {}
+    for pdl in (0, 1):
+        op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales).set_option(cop.OPT_PDL, pdl)
+        a, b = v0.clone(), torch.empty_like(v0)
+        for k in range(6):
+            op.apply(a, b, dagger=k & 1)
+            a, b = b, a
+        torch.cuda.synchronize()
+        outs[pdl] = a.clone()
+        op.close()
+    assert torch.equal(torch.view_as_real(outs[0]), torch.view_as_real(outs[1]))
+    ref = v0.cpu().numpy()
+    for k in range(6):
+        ref = oracle_lib.coarse_apply(dims, Nc, links_h, ref.astype(np.complex64), dagger=k & 1, link_precision=prec,
+                                      scales=scales_h)
+    assert rel_l2_per_rhs(outs[1].cpu().numpy(), ref) <= 6 * TOL
+
+
+def test_pdl_with_parts_hvec_and_graph_capture(oracle_lib):
+    dims, Nc = (4, 4, 2, 2), 48
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, 5, device="cuda") * 0.25
+    v = synth.make_vectors(dims, Nc, 1, 6, device="cuda")
+    res = {}
+    for pdl in (0, 1):
+        op = cop.CoarseOp(dims, Nc).set_links(links).set_option(cop.OPT_PDL, pdl)
+        t, out = torch.zeros_like(v), torch.zeros_like(v)
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(3):
+                op.apply_parts(None, v, t, parity=cop.PARITY_ODD, local=cop.LOCAL_NONE, alpha=0.0, beta=1.0)
+                op.apply_parts(v, t, out, parity=cop.PARITY_EVEN, local=cop.LOCAL_IDENTITY, alpha=1.0, beta=-1.0)
+        torch.cuda.current_stream().wait_stream(side)
+        g.replay()
+        torch.cuda.synchronize()
+        q = torch.empty((V, Nc, 1, 2), dtype=torch.int16, device="cuda")
+        nm = torch.empty((V, 1), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_vec_i16(out, Nc, 1, q, nm)
+        o2 = torch.empty_like(v)
+        op.apply_hvec(q, nm, o2)
+        torch.cuda.synchronize()
+        res[pdl] = (out.clone(), o2.clone())
+        op.close()
+    assert torch.equal(torch.view_as_real(res[0][0]), torch.view_as_real(res[1][0]))
+    assert torch.equal(torch.view_as_real(res[0][1]), torch.view_as_real(res[1][1]))
+
+
 def test_read_probe_runs_and_validates_arguments():
     buf = torch.zeros(64 << 20, dtype=torch.uint8, device="cuda")
     assert cop.coarse_op_probe_read(buf, 16384, 6) == 64 << 20
