@@ -65,6 +65,9 @@ struct coarse_op {
     void* stage_in;
     void* stage_out;
     size_t stage_bytes;
+    cudaStream_t s_h2d, s_d2h;      // apply_host's copy streams and events (created on first use)
+    cudaEvent_t ev_up[4], ev_k[4], ev_done;
+    bool host_pipe_ok;
     CUtensorMap link_map;   // 2-D view of the link array for the TENSOR path (dagger = 0 slabs)
     bool link_map_ok;
 };
@@ -80,8 +83,9 @@ struct PartsSpec {
     int local;    // 0 none, 1 X, 2 identity
     float alpha, beta;
     const float* vnorms;   // non-NULL: half-precision input vectors (plain apply only)
+    int site_begin, site_end;   // output sites [site_begin, site_end) (plain apply only); end = 0: all
 };
-const PartsSpec kPlain = {false, nullptr, 2, 1, 1.f, 1.f, nullptr};
+const PartsSpec kPlain = {false, nullptr, 2, 1, 1.f, 1.f, nullptr, 0, 0};
 
 // ---------------------------------------------------------------- STREAM dispatch
 template <int NC, bool I16, bool DAG, bool FINE, bool GEN, bool HV = false>
@@ -90,6 +94,10 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     static_assert(Gm::OK, "unsupported STREAM geometry");
     StreamParams p = base;
     p.n_items = DAG ? p.n_sites : p.n_sites * Gm::NB;
+    if (base.n_items > 0) {                       // a site range [item_begin, n_items) was requested (in sites)
+        p.item_begin = DAG ? base.item_begin : base.item_begin * Gm::NB;
+        p.n_items = DAG ? base.n_items : base.n_items * Gm::NB;
+    }
     int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (Gm::stage_bytes(DAG) + 16);
     if (stages > 12) stages = 12;
     if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM: shared memory too small for Nc=%d", NC);
@@ -105,7 +113,8 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
-    if (grid > p.n_items) grid = p.n_items;
+    if (grid > p.n_items - p.item_begin) grid = p.n_items - p.item_begin;
+    if (grid < 1) return COARSE_OK;
     p.pdl = op->pdl_opt ? 1 : 0;
     if (p.pdl) {
         // programmatic dependent launch: this kernel may start while the previous kernel of the stream
@@ -245,7 +254,8 @@ int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, co
     p.scales = op->scales;
     p.in = static_cast<const float2*>(in);
     p.out = static_cast<float2*>(out);
-    p.n_items = 0;
+    p.n_items = ps.site_end > 0 ? ps.site_end : 0;
+    p.item_begin = ps.site_end > 0 ? ps.site_begin : 0;
     p.stages = 0;
     // links that fit L2 (with room for the vectors) are re-read from L2 by the next apply: keep them
     p.keep_links = op->keep_opt == 2 || (op->keep_opt == 0 && coarse_op_link_bytes(op) <= (size_t)op->l2_bytes / 2);
@@ -502,6 +512,8 @@ coarse_op_t* coarse_op_create(const int dims[4], int Nc, int link_precision) {
     op->max_smem = smem;
     op->stage_in = op->stage_out = nullptr;
     op->stage_bytes = 0;
+    op->s_h2d = op->s_d2h = nullptr;
+    op->host_pipe_ok = false;
     op->link_map_ok = false;
     g_last_error = "";
     return op;
@@ -647,7 +659,7 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
     // which the caller cannot express here, so overlap is always refused; u is read at x only and
     // may alias out.
     if (a < b + vb && b < a + vb) return fail(COARSE_EINVAL, "apply_parts: w and out overlap (the stencil reads neighbours)");
-    PartsSpec ps = {true, local != 0 ? u_dev : w_dev, parity, local, alpha, beta, nullptr};
+    PartsSpec ps = {true, local != 0 ? u_dev : w_dev, parity, local, alpha, beta, nullptr, 0, 0};
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int path = op->path_opt;
     if (path == COARSE_PATH_AUTO || path == COARSE_PATH_TENSOR || path == COARSE_PATH_BLOCK)
@@ -732,7 +744,71 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
         op->stage_bytes = vb;
     }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    cudaError_t e = cudaMemcpyAsync(op->stage_in, in_host, vb, cudaMemcpyHostToDevice, st);
+    cudaError_t e;
+    // Pipelined path (1 RHS on the STREAM kernels, at least 8 time slices): the lattice is cut into 4 ranges
+    // of x3-slices; range c is launched as soon as the slices it reads (its own and one on either side)
+    // are on the device, and its result goes back to the host while the next range computes.  H2D, the
+    // kernels and D2H run on three streams; nothing is reordered inside a range, so the result is
+    // bit-identical to the plain path.
+    const int T = op->lat.L[3];
+    const bool stream_1rhs = nrhs == 1 && stream_supports(op->Nc, 1) &&
+                             (op->path_opt == COARSE_PATH_AUTO || op->path_opt == COARSE_PATH_STREAM);
+    if (stream_1rhs && T >= 8 && vb >= ((size_t)1 << 22)) {
+        if (!op->host_pipe_ok) {
+            bool ok = cudaStreamCreateWithFlags(&op->s_h2d, cudaStreamNonBlocking) == cudaSuccess &&
+                      cudaStreamCreateWithFlags(&op->s_d2h, cudaStreamNonBlocking) == cudaSuccess;
+            for (int i = 0; ok && i < 4; ++i)
+                ok = cudaEventCreateWithFlags(&op->ev_up[i], cudaEventDisableTiming) == cudaSuccess &&
+                     cudaEventCreateWithFlags(&op->ev_k[i], cudaEventDisableTiming) == cudaSuccess;
+            ok = ok && cudaEventCreateWithFlags(&op->ev_done, cudaEventDisableTiming) == cudaSuccess;
+            if (!ok) { cudaGetLastError(); return fail(COARSE_ECUDA, "apply_host: cannot create copy streams/events"); }
+            op->host_pipe_ok = true;
+        }
+        const size_t plane = (size_t)(op->lat.V / T);               // sites per x3-slice
+        const size_t pb = plane * op->Nc * 8;                        // bytes per slice
+        const unsigned char* hin = static_cast<const unsigned char*>(in_host);
+        unsigned char* hout = static_cast<unsigned char*>(out_host);
+        unsigned char* din = static_cast<unsigned char*>(op->stage_in);
+        unsigned char* dout = static_cast<unsigned char*>(op->stage_out);
+        // the copy streams start after whatever the caller's stream has queued
+        if ((e = cudaEventRecord(op->ev_done, st)) != cudaSuccess) return cuda_fail(e, "apply_host: event record");
+        cudaStreamWaitEvent(op->s_h2d, op->ev_done, 0);
+        cudaStreamWaitEvent(op->s_d2h, op->ev_done, 0);
+        // slice T-1 first (range 0 reads it through the periodic wrap), then slices in order
+        if ((e = cudaMemcpyAsync(din + (size_t)(T - 1) * pb, hin + (size_t)(T - 1) * pb, pb, cudaMemcpyHostToDevice, op->s_h2d)) != cudaSuccess)
+            return cuda_fail(e, "apply_host: H2D copy");
+        int uploaded = 0;                                            // slices [0, uploaded) are queued
+        PartsSpec ps = kPlain;
+        op->last_launches = 0;
+        for (int c = 0; c < 4; ++c) {
+            const int t0 = (int)((long long)T * c / 4), t1 = (int)((long long)T * (c + 1) / 4);
+            int need = t1 + 1 < T - 1 ? t1 + 1 : T - 1;              // slices [0, need) plus slice T-1
+            if (need > uploaded) {
+                e = cudaMemcpyAsync(din + (size_t)uploaded * pb, hin + (size_t)uploaded * pb, (size_t)(need - uploaded) * pb,
+                                    cudaMemcpyHostToDevice, op->s_h2d);
+                if (e != cudaSuccess) return cuda_fail(e, "apply_host: H2D copy");
+                uploaded = need;
+            }
+            cudaEventRecord(op->ev_up[c], op->s_h2d);
+            cudaStreamWaitEvent(st, op->ev_up[c], 0);
+            ps.site_begin = (int)(plane * t0);
+            ps.site_end = (int)(plane * t1);
+            rc = launch_stream(op, op->stage_in, op->stage_out, dagger, ps, st);
+            if (rc != COARSE_OK) return rc;
+            op->last_launches += 1;
+            cudaEventRecord(op->ev_k[c], st);
+            cudaStreamWaitEvent(op->s_d2h, op->ev_k[c], 0);
+            e = cudaMemcpyAsync(hout + (size_t)t0 * pb, dout + (size_t)t0 * pb, (size_t)(t1 - t0) * pb, cudaMemcpyDeviceToHost, op->s_d2h);
+            if (e != cudaSuccess) return cuda_fail(e, "apply_host: D2H copy");
+        }
+        op->last_path = COARSE_PATH_STREAM;
+        cudaEventRecord(op->ev_done, op->s_d2h);
+        cudaStreamWaitEvent(st, op->ev_done, 0);
+        e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(e, "apply_host: stream synchronize");
+        return COARSE_OK;
+    }
+    e = cudaMemcpyAsync(op->stage_in, in_host, vb, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(e, "apply_host: H2D copy");
     rc = coarse_op_apply(op, op->stage_in, op->stage_out, nrhs, dagger, stream);
     if (rc != COARSE_OK) return rc;
@@ -983,6 +1059,12 @@ void coarse_op_destroy(coarse_op_t* op) {
     if (!op) return;
     if (op->stage_in) cudaFree(op->stage_in);
     if (op->stage_out) cudaFree(op->stage_out);
+    if (op->host_pipe_ok) {
+        for (int i = 0; i < 4; ++i) { cudaEventDestroy(op->ev_up[i]); cudaEventDestroy(op->ev_k[i]); }
+        cudaEventDestroy(op->ev_done);
+        cudaStreamDestroy(op->s_h2d);
+        cudaStreamDestroy(op->s_d2h);
+    }
     delete op;
 }
 

@@ -52,6 +52,7 @@ struct StreamParams {
     int parity;               // 0 even, 1 odd, 2 all sites
     int n_sites;              // sites in the parity set
     int pdl;                  // 1: launched with programmatic stream serialization (COARSE_OPT_PDL)
+    int item_begin;           // work items [item_begin, n_items): coarse_op_apply_host launches site ranges
     // HV (half-precision input vectors, coarse_op_apply_hvec): `in` points at int16 (re,im) entries
     const float* vnorms;      // fp32 norm per site (nrhs = 1)
 };
@@ -185,7 +186,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
             __syncwarp();
             deferring = false;
         };
-        for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+        for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
             const int sidx = DAG ? item : item / NB;
             const int s = (GEN && p.parity != 2) ? parity_site(p.lat, sidx, p.parity) : sidx;
             const int rb = DAG ? 0 : item % NB;
@@ -249,10 +250,10 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
         return f;
     };
     const int M0 = GEN ? p.m_begin : 0;
-    next_scale = fetch_scale(blockIdx.x);
-    next2_scale = fetch_scale(blockIdx.x + gridDim.x);
+    next_scale = fetch_scale(p.item_begin + blockIdx.x);
+    next2_scale = fetch_scale(p.item_begin + blockIdx.x + gridDim.x);
 
-    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+    for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
         const int s = site_of(item);
         const int rb = DAG ? 0 : item % NB;
         cur_scale = next_scale;

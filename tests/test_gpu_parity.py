@@ -376,6 +376,41 @@ def test_apply_host_matches_device_apply(oracle_lib):
         assert rel_l2_per_rhs(vout.numpy(), ref) <= TOL
 
 
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+def test_apply_host_pipelined_path_is_bit_identical(oracle_lib, prec):
+    """Large enough for coarse_op_apply_host's pipelined path (4 ranges of x3-slices, H2D / kernels / D2H on
+    three streams): must equal the plain device apply bit for bit, for both modes, and repeatedly."""
+    dims, Nc = (8, 8, 8, 24), 48
+    V = synth.lattice_volume(dims)
+    links, scales, _, _ = _links_for(dims, Nc, prec, 3, True, oracle_lib) if prec == cop.LINK_C64 else (None, None, None, None)
+    if prec == cop.LINK_I16:
+        lc = synth.make_gamma_hermitian_links(dims, Nc, 3, device="cuda")
+        links = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+        scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_i16(lc, Nc, links, scales)
+        del lc
+    vin_d = synth.make_vectors(dims, Nc, 1, 4, device="cuda")
+    vin = vin_d.cpu().pin_memory()
+    vout = torch.empty_like(vin).pin_memory()
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    for rep in range(2):
+        for dagger in (0, 1):
+            ref = torch.empty_like(vin_d)
+            op.apply(vin_d, ref, dagger=dagger)
+            torch.cuda.synchronize()
+            vout.fill_(float("nan"))
+            op.apply_host(vin, vout, dagger=dagger)
+            assert op.last_launches == 4 and op.last_path == cop.PATH_STREAM
+            assert torch.equal(torch.view_as_real(vout), torch.view_as_real(ref.cpu()))
+    # and against the oracle on sampled sites
+    sites = np.array([0, 1, 511, 512, V // 2, V - 513, V - 512, V - 1], dtype=np.int64)
+    got = vout.numpy()[sites]
+    refo = oracle_lib.coarse_apply_sites(dims, Nc, links.cpu().numpy(), vin.numpy(), sites, dagger=1,
+                                         link_precision=prec, scales=None if scales is None else scales.cpu().numpy())
+    assert rel_l2_per_rhs(got, refo) <= TOL
+    op.close()
+
+
 # ------------------------------------------------------------------ ABI behaviour
 def test_error_codes():
     dims, Nc = (2, 2, 2, 2), 48
