@@ -46,11 +46,11 @@ UNIT = "site-updates/s"
 # `ncu --set full` captures summarised under profiles/r01_ncu_full_*.md, keyed by
 # (config, path actually run, dagger); None for combinations that were not captured.
 NCU_TRAFFIC_BYTES = {
-    ("C2", 2, 0): 16361774080, ("C2", 2, 1): 16366542592,
-    ("C3", 2, 0): 7260963584, ("C3", 2, 1): 7260998144,
-    ("C4", 2, 0): 14582045952, ("C4", 2, 1): 14586587648,
-    ("C5", 3, 0): 7455878144, ("C5", 3, 1): 7442301440,
-    ("C5", 4, 0): 7446740992, ("C5", 4, 1): 7443230208,
+    ("C2", 2, 0): 16361995008, ("C2", 2, 1): 16367453696,
+    ("C3", 2, 0): 7260217344, ("C3", 2, 1): 7261264896,
+    ("C4", 2, 0): 14580726784, ("C4", 2, 1): 14584525824,
+    ("C5", 3, 0): 7481073920, ("C5", 3, 1): 7441391616,
+    ("C5", 4, 0): 7447821312, ("C5", 4, 1): 7443588096,
 }
 
 
