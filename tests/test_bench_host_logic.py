@@ -56,3 +56,20 @@ def test_two_rank_aggregation_gloo():
 
 def test_single_process_aggregation_is_identity():
     assert bench.reduce_max_sum(3.0, 7.0) == (3.0, 7.0)
+
+
+def test_paper_per_gpu_volume_configs_follow_from_table_1():
+    """synth.CONFIGS P2 / P3 are the paper's own per-GPU coarse volumes: derived here from the numbers the
+    paper prints (tests/golden/per_gpu_coarse_volumes.txt), not typed in twice."""
+    g = {}
+    for line in open(os.path.join(ROOT, "tests", "golden", "per_gpu_coarse_volumes.txt")):
+        if line.strip() and not line.startswith("#"):
+            k, v = line.split("=")
+            g[k.strip()] = [int(x) for x in v.split()]
+    local = [a // b for a, b in zip(g["global_lattice"], g["gpu_grid"])]
+    assert local == g["local_volume"]
+    lvl2 = [a // b for a, b in zip(local, g["aggregate_level2"])]
+    lvl3 = [a // b for a, b in zip(lvl2, g["aggregate_level3"])]
+    assert tuple(lvl2) == synth.config("P2")["dims"] and synth.config("P2")["Nc"] == g["Nc_level2"][0]
+    assert tuple(lvl3) == synth.config("P3")["dims"] and synth.config("P3")["Nc"] == g["Nc_level3"][0]
+    assert synth.lattice_volume(lvl2) == 1152 and synth.lattice_volume(lvl3) == 32
