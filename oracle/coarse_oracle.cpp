@@ -50,10 +50,13 @@
 //   C64: float[2] (re,im).  I16: int16_t[2] (re,im) + scales[s][m] float.
 //   vectors v[s][a][r] complex64 (float[2]), r innermost.  Output: complex128 (double[2]).
 //
-// Pins (tests/test_oracle_pins.py, -m "not gpu"): brute-force Galerkin P^H A P on tiny
-// lattices, unit-shift cases, X-only vs a library einsum, dense
-// assembly, adjoint identity, Gamma-Hermiticity, linearity, quantiser
-// bounds.  No function here is "parity unpinned".
+// Pins (-m "not gpu"): tests/test_oracle_pins.py - brute-force Galerkin P^H A P on tiny lattices
+// (PAPER.md:L43), unit-shift cases, X-only vs a library einsum, dense assembly, adjoint identity,
+// Gamma-Hermiticity, linearity, quantiser bounds; tests/test_oracle_evenodd_pins.py - O7
+// against dense X / hopping blocks with parity masks, the dense Schur complement, the solution property;
+// tests/test_oracle_hvec_pins.py - O8 against the complex64 apply on exactly representable data and the
+// dense matrix; tests/test_oracle_cagcr_pins.py - the CA-GCR iterate (oracle/__init__.py) against scipy
+// GMRES and the direct solve.  No function here or in oracle/__init__.py is "parity unpinned".
 
 #include <cmath>
 #include <cstdint>
