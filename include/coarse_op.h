@@ -84,7 +84,9 @@ enum {
     COARSE_OPT_PDL = 5       /* 1: launch the 1-RHS STREAM kernels with programmatic dependent launch: in a chain
                                 of applies on one stream the next kernel's CTAs start on SMs the previous one
                                 has left and prefetch their link stages before waiting for its output (the
-                                latency-limited small-lattice regime of PAPER.md:L99).  Default 0. */
+                                latency-limited small-lattice regime of PAPER.md:L99).  Default 0.  With it on,
+                                the LINK and scale arrays must not be written by work still in flight on the
+                                stream (they are read before the kernel orders itself against its predecessor). */
 };
 
 /* Create an operator descriptor for a periodic lattice dims[0..3] (each >= 1), Nc even and
