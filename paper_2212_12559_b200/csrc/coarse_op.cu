@@ -108,7 +108,12 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     if (op->stages_opt > 0) want = op->stages_opt;
     if (stages > want) stages = want;
     p.stages = stages;
-    const int smem = Gm::smem_bytes(DAG, stages);
+    int smem = Gm::smem_bytes(DAG, stages);
+    // PDL: a kernel whose shared-memory carve-out differs from its predecessor's cannot take over an SM
+    // before it has drained completely (measured: an alternating dagger 0 / dagger 1 chain gained nothing
+    // until both kernels asked for the same size), so under PDL both modes request the larger of the two.
+    if (op->pdl_opt && Gm::smem_bytes(!DAG, stages) > smem && Gm::smem_bytes(!DAG, stages) <= op->max_smem)
+        smem = Gm::smem_bytes(!DAG, stages);
     auto kern = coarse_apply_stream<NC, I16, DAG, FINE, GEN, HV>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
