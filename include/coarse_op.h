@@ -30,8 +30,8 @@
  *   vectors         v[s][a][r], float[2] = (re,im), a in [0,Nc) colour-spin (a = chi*N_vec + k),
  *                   r in [0,nrhs) innermost.
  *
- * OWNERSHIP  The handle owns metadata and (only if coarse_op_apply_host is used) two vector-sized
- *   staging buffers.  Link, scale, in and out buffers are the caller's; coarse_op_set_links borrows
+ * OWNERSHIP  The handle owns metadata, (only if coarse_op_apply_host is used) two vector-sized
+ *   staging buffers, and on lattices with fewer sites than SMs a few-MB workspace for the split dagger apply.  Link, scale, in and out buffers are the caller's; coarse_op_set_links borrows
  *   the pointers, which must stay valid and unchanged until destroy or the next set_links.
  *
  * ERRORS  int-returning calls return COARSE_OK (0) or a negative code; coarse_op_create returns
@@ -81,6 +81,9 @@ enum {
     COARSE_OPT_STAGES = 2,   /* cap on the STREAM shared-memory ring depth; 0 = library default   */
     COARSE_OPT_FINE = 3,     /* STREAM dagger=0 small-lattice row-block split: 0 auto, 1 never, 2 always */
     COARSE_OPT_KEEP_LINKS = 4, /* L2 policy of the link stream: 0 auto (keep if links <= L2/2), 1 evict_first, 2 keep */
+    COARSE_OPT_SPLIT_DAGGER = 6, /* dagger = 1, 1 RHS, lattices with fewer sites than SMs: split each site's
+                                contraction over its row chunks + a reduce kernel (2 launches): 0 auto, 1 never,
+                                2 always (needs the workspace coarse_op_set_links allocates on such lattices) */
     COARSE_OPT_PDL = 5       /* 1: launch the 1-RHS STREAM kernels with programmatic dependent launch: in a chain
                                 of applies on one stream the next kernel's CTAs start on SMs the previous one
                                 has left and prefetch their link stages before waiting for its output (the

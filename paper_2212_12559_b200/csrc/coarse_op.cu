@@ -56,6 +56,9 @@ struct coarse_op {
     int fine_opt;
     int keep_opt;
     int pdl_opt;
+    int split_opt;            // COARSE_OPT_SPLIT_DAGGER: 0 auto, 1 never, 2 always
+    float2* split_ws;         // partial vectors of the split dagger apply (allocated by set_links on tiny lattices)
+    size_t split_ws_bytes;
     int l2_bytes;
     int last_launches;
     int last_path;
@@ -98,6 +101,18 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
         p.item_begin = DAG ? base.item_begin : base.item_begin * Gm::NB;
         p.n_items = DAG ? base.n_items : base.n_items * Gm::NB;
     }
+    // dagger = 1 has one work item per site; on a lattice with fewer sites than SMs (the paper's level 3:
+    // 32 sites per GPU) the contraction of a site is split over its NB row chunks, one item each, and a
+    // small second kernel adds the NB partial vectors in order.
+    p.split = 0;
+    p.partial = nullptr;
+    if (DAG && !GEN && !HV && base.n_items == 0 && Gm::NB > 1 && op->split_ws &&
+        (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes &&
+        (op->split_opt == 2 || (op->split_opt == 0 && p.n_sites < op->num_sms))) {
+        p.split = 1;
+        p.partial = op->split_ws;
+        p.n_items = p.n_sites * Gm::NB;
+    }
     int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (Gm::stage_bytes(DAG) + 16);
     if (stages > 12) stages = 12;
     if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM: shared memory too small for Nc=%d", NC);
@@ -136,11 +151,18 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
         cfg.numAttrs = 1;
         e = cudaLaunchKernelEx(&cfg, kern, p);
         if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch (PDL)");
-        return COARSE_OK;
+    } else {
+        kern<<<grid, Gm::THREADS, smem, stream>>>(p);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch");
     }
-    kern<<<grid, Gm::THREADS, smem, stream>>>(p);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch");
+    if (p.split) {
+        const long long tot = (long long)p.n_sites * NC;
+        coarse_dagger_reduce_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(p.partial, p.n_sites, Gm::NB, NC, p.out);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "dagger reduce kernel launch");
+        return 1;      // one extra launch (coarse_op_apply adds it to last_launches)
+    }
     return COARSE_OK;
 }
 
@@ -509,6 +531,9 @@ coarse_op_t* coarse_op_create(const int dims[4], int Nc, int link_precision) {
     op->fine_opt = 0;
     op->keep_opt = 0;
     op->pdl_opt = 0;
+    op->split_opt = 0;
+    op->split_ws = nullptr;
+    op->split_ws_bytes = 0;
     { int l2 = 0; cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev); op->l2_bytes = l2; }
     op->last_launches = 0;
     op->last_path = 0;
@@ -552,6 +577,13 @@ int coarse_op_set_links(coarse_op_t* op, const void* links_dev, const float* sca
     }
     op->links = links_dev;
     op->scales = scales_dev;
+    // tiny lattices (fewer sites than SMs): workspace for the split dagger apply, V * (Nc/8) chunks * Nc
+    // complex numbers at most (a few MB); the only allocation the library makes besides apply_host's staging
+    if (!op->split_ws && op->lat.V < op->num_sms && stream_supports(op->Nc, 1)) {
+        const size_t bytes = (size_t)op->lat.V * (op->Nc / 8) * op->Nc * 8;
+        if (cudaMalloc(reinterpret_cast<void**>(&op->split_ws), bytes) == cudaSuccess) op->split_ws_bytes = bytes;
+        else { cudaGetLastError(); op->split_ws = nullptr; op->split_ws_bytes = 0; }
+    }
     return make_link_map(op);
 }
 
@@ -590,6 +622,10 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value) {
         case COARSE_OPT_KEEP_LINKS:
             if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: keep_links must be 0 (auto), 1 (never) or 2 (always)");
             op->keep_opt = value;
+            return COARSE_OK;
+        case COARSE_OPT_SPLIT_DAGGER:
+            if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: split_dagger must be 0 (auto), 1 (never) or 2 (always)");
+            op->split_opt = value;
             return COARSE_OK;
         case COARSE_OPT_PDL:
             if (value != 0 && value != 1) return fail(COARSE_EINVAL, "set_option: pdl must be 0 or 1");
@@ -638,8 +674,8 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
     } else {
         rc = launch_simple(op, in_dev, out_dev, nrhs, dagger, kPlain, st);
     }
-    if (rc != COARSE_OK) return rc;
-    op->last_launches = 1;
+    if (rc < 0) return rc;
+    op->last_launches = 1 + rc;      // the split dagger apply reports its second (reduce) launch as rc = 1
     op->last_path = path;
     return COARSE_OK;
 }
@@ -1064,6 +1100,7 @@ void coarse_op_destroy(coarse_op_t* op) {
     if (!op) return;
     if (op->stage_in) cudaFree(op->stage_in);
     if (op->stage_out) cudaFree(op->stage_out);
+    if (op->split_ws) cudaFree(op->split_ws);
     if (op->host_pipe_ok) {
         for (int i = 0; i < 4; ++i) { cudaEventDestroy(op->ev_up[i]); cudaEventDestroy(op->ev_k[i]); }
         cudaEventDestroy(op->ev_done);

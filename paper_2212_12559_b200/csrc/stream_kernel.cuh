@@ -53,6 +53,10 @@ struct StreamParams {
     int n_sites;              // sites in the parity set
     int pdl;                  // 1: launched with programmatic stream serialization (COARSE_OPT_PDL)
     int item_begin;           // work items [item_begin, n_items): coarse_op_apply_host launches site ranges
+    // dagger = 1 on a tiny lattice: split a site's contraction over its NB row chunks (item = (site, chunk)),
+    // partial vectors go to `partial` and coarse_dagger_reduce_kernel adds them in chunk order
+    int split;
+    float2* partial;          // [n_sites * NB][Nc]
     // HV (half-precision input vectors, coarse_op_apply_hvec): `in` points at int16 (re,im) entries
     const float* vnorms;      // fp32 norm per site (nrhs = 1)
 };
@@ -187,7 +191,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
             deferring = false;
         };
         for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
-            const int sidx = DAG ? item : item / NB;
+            const int sidx = (DAG && !p.split) ? item : item / NB;
             const int s = (GEN && p.parity != 2) ? parity_site(p.lat, sidx, p.parity) : sidx;
             const int rb = DAG ? 0 : item % NB;
             const SiteX cx = site_coords(p.lat, s);
@@ -198,8 +202,10 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                 const int sm = DAG ? sv : s;
                 const unsigned char* mat = p.links + ((int64_t)sm * 9 + m) * ((int64_t)NC * ROWBYTES);
                 const unsigned char* vec = reinterpret_cast<const unsigned char*>((GEN && m == 0) ? p.in_local : p.in) + (int64_t)sv * NC * VE;
+                const int c_begin = (DAG && p.split) ? item % NB : 0;
+                const int c_end = DAG ? (p.split ? c_begin + 1 : NB) : 1;
 #pragma unroll 1
-                for (int c = 0; c < (DAG ? NB : 1); ++c) {
+                for (int c = c_begin; c < c_end; ++c) {
                     const int r0 = DAG ? c * RS : rb * RS;
                     if (deferring && n_def == S) flush_deferred();    // the ring is full: the vectors are needed now
                     ptx::mbar_wait(empty0 + 8u * slot, phase ^ 1u);
@@ -236,7 +242,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
     // item (~3 us), and with a one-item lead ncu showed 12 % of the dagger = 1 samples waiting on it.
     float cur_scale = 1.f, next_scale = 1.f, next2_scale = 1.f;
     auto site_of = [&](int item) -> int {
-        const int sidx = DAG ? item : item / NB;
+        const int sidx = (DAG && !p.split) ? item : item / NB;
         return (GEN && p.parity != 2) ? parity_site(p.lat, sidx, p.parity) : sidx;
     };
     auto fetch_scale = [&](int item) -> float {
@@ -373,7 +379,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                 float sc = (I16 || HV) ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
                 if constexpr (GEN) sc *= (m == 0) ? p.alpha : p.beta;
 #pragma unroll 1
-                for (int c = 0; c < NB; ++c) {
+                for (int c = p.split ? item % NB : 0; c < (p.split ? item % NB + 1 : NB); ++c) {
                     ptx::mbar_wait(full0 + 8u * slot, phase);
                     const uint32_t lbase = link_u32 + slot * LINK_STAGE + qi * 16;
                     const uint32_t vbase = vec_u32 + slot * VEC_STAGE;
@@ -436,11 +442,27 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                     sum.x = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].x, sum.x);
                     sum.y = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].y, sum.y);
                 }
-                p.out[(int64_t)s * NC + t] = sum;
+                if (p.split) p.partial[(int64_t)item * NC + t] = sum;
+                else p.out[(int64_t)s * NC + t] = sum;
             }
             red_parity ^= 1;
         }
     }
+}
+
+// out[s][t] = sum_c partial[s*nb + c][t], chunks added in order (deterministic)
+__global__ void __launch_bounds__(256) coarse_dagger_reduce_kernel(const float2* partial, int n_sites, int nb, int nc, float2* out) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)n_sites * nc) return;
+    const long long s = idx / nc;
+    const int t = (int)(idx % nc);
+    float2 sum = make_float2(0.f, 0.f);
+    for (int c = 0; c < nb; ++c) {
+        const float2 x = partial[(s * nb + c) * nc + t];
+        sum.x += x.x;
+        sum.y += x.y;
+    }
+    out[idx] = sum;
 }
 
 }  // namespace coarse

@@ -336,6 +336,35 @@ def test_pdl_with_parts_hvec_and_graph_capture(oracle_lib):
     assert torch.equal(torch.view_as_real(res[0][1]), torch.view_as_real(res[1][1]))
 
 
+@pytest.mark.parametrize("dims", [(2, 4, 2, 2), (1, 1, 1, 1), (3, 2, 1, 4)])
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+def test_split_dagger_on_tiny_lattices(oracle_lib, dims, Nc, prec):
+    """dagger = 1 with fewer sites than SMs (the paper's level 3 has 32 sites per GPU): the contraction of
+    a site is split over its row chunks and reduced by a second kernel.  Auto picks it, forcing it off must
+    give the same numbers up to summation order, and both must match the oracle."""
+    V = synth.lattice_volume(dims)
+    links, scales, links_h, scales_h = _links_for(dims, Nc, prec, 61, False, oracle_lib)
+    vin = synth.make_vectors(dims, Nc, 1, 62, device="cuda")
+    ref = oracle_lib.coarse_apply(dims, Nc, links_h, vin.cpu().numpy(), dagger=1, link_precision=prec, scales=scales_h)
+    for mode, want_launches in ((0, None), (1, 1), (2, None)):
+        op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales).set_option(cop.OPT_SPLIT_DAGGER, mode)
+        out = torch.full_like(vin, float("nan"))
+        op.apply(vin, out, dagger=1)
+        torch.cuda.synchronize()
+        assert op.last_path == cop.PATH_STREAM
+        if want_launches:
+            assert op.last_launches == want_launches
+        else:
+            assert op.last_launches in (1, 2)          # 2 when the geometry has more than one row chunk
+        assert rel_l2_per_rhs(out.cpu().numpy(), ref) <= TOL
+        # dagger = 0 is untouched by the option
+        op.apply(vin, out, dagger=0)
+        torch.cuda.synchronize()
+        assert op.last_launches == 1
+        op.close()
+
+
 def test_read_probe_runs_and_validates_arguments():
     buf = torch.zeros(64 << 20, dtype=torch.uint8, device="cuda")
     assert cop.coarse_op_probe_read(buf, 16384, 6) == 64 << 20
