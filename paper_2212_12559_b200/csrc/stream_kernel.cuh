@@ -81,6 +81,14 @@ constexpr int stream_passes(int q) {
         if (q % p == 0 && q / p <= 32) return p;
     return 0;
 }
+// int16 links make the kernel issue-bound, so idle lanes cost time there: prefer a pass count that leaves
+// a power-of-two number of quads per pass (rows of 12 / 24 / 48 quads, Nc = 48 / 96 / 192, otherwise run
+// with 12 or 24 of every 16 or 32 lanes: measured 4.9-5.7 TB/s against 7.4 TB/s at Nc = 64).
+constexpr int stream_passes_full(int q) {
+    for (int p = 1; p <= 8; ++p)
+        if (q % p == 0 && q / p <= 32 && stream_pow2ceil(q / p) == q / p) return p;
+    return stream_passes(q);
+}
 constexpr int stream_rows_per_stage(int nc, int rowbytes, int unit, int max_bytes) {
     int best = 0;
     for (int d = unit; d <= nc; d += unit)
@@ -92,17 +100,23 @@ constexpr int stream_rows_per_stage(int nc, int rowbytes, int unit, int max_byte
 // allows, so that V * NB work items still fill 148 SMs when the local volume is a few hundred
 // sites or less ("additional parallelism is exposed in the matrix-vector application
 // to compensate for reduction in parallelism possible by the size of the local volume alone").
+// consumer warps: 8, or 6 when only a multiple of 6 warp-loads of rows divides Nc (Nc = 48 with 8 rows per load)
+constexpr int stream_warps(int nc, int rowbytes, int rpl) {
+    return stream_rows_per_stage(nc, rowbytes, 8 * rpl, 24576) > 0 ? 8
+           : stream_rows_per_stage(nc, rowbytes, 6 * rpl, 24576) > 0 ? 6 : 8;
+}
+
 template <int NC, bool I16, bool FINE = false, bool HV = false>
 struct StreamGeom {
-    static constexpr int W = 8;                                // consumer warps
     static constexpr int ENTRY_BYTES = I16 ? 4 : 8;            // one complex link entry
     static constexpr int ROWBYTES = NC * ENTRY_BYTES;
     static constexpr int Q = ROWBYTES / 16;                    // 16-byte quads per row
     static constexpr int CPQ = 16 / ENTRY_BYTES;               // complex entries per quad
-    static constexpr int PASSES = stream_passes(Q);
+    static constexpr int PASSES = I16 ? stream_passes_full(Q) : stream_passes(Q);
     static constexpr int QP = Q / PASSES;                      // quads per row per pass (<= 32)
     static constexpr int G = stream_pow2ceil(QP);              // lanes that share one row
     static constexpr int RPL = 32 / G;                         // rows per warp-wide load
+    static constexpr int W = stream_warps(NC, ROWBYTES, RPL);  // consumer warps
     static constexpr int RS = stream_rows_per_stage(NC, ROWBYTES, W * RPL, FINE ? (W * RPL * ROWBYTES) : 24576);
     static constexpr int NB = NC / RS;                         // row blocks per matrix
     static constexpr int WL = RS / (W * RPL);                  // warp-wide loads per warp, stage, pass
