@@ -213,7 +213,7 @@ bool stream_mr_supports(int Nc, int nrhs) { return stream_supports(Nc, 1) && nrh
 // ---------------------------------------------------------------- STREAM-MR dispatch (2 <= nrhs <= 4)
 template <int NC, bool I16, bool DAG, int R>
 int launch_stream_mr_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
-    using Gm = StreamGeom<NC, I16, false, false>;
+    using Gm = StreamGeom<NC, I16, false, false, true>;
     using Gr = StreamMrGeom<NC, I16, R>;
     StreamParams p = base;
     p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;

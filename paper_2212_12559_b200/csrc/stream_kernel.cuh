@@ -106,13 +106,13 @@ constexpr int stream_warps(int nc, int rowbytes, int rpl) {
            : stream_rows_per_stage(nc, rowbytes, 6 * rpl, 24576) > 0 ? 6 : 8;
 }
 
-template <int NC, bool I16, bool FINE = false, bool HV = false>
+template <int NC, bool I16, bool FINE = false, bool HV = false, bool FULL = I16>
 struct StreamGeom {
     static constexpr int ENTRY_BYTES = I16 ? 4 : 8;            // one complex link entry
     static constexpr int ROWBYTES = NC * ENTRY_BYTES;
     static constexpr int Q = ROWBYTES / 16;                    // 16-byte quads per row
     static constexpr int CPQ = 16 / ENTRY_BYTES;               // complex entries per quad
-    static constexpr int PASSES = I16 ? stream_passes_full(Q) : stream_passes(Q);
+    static constexpr int PASSES = FULL ? stream_passes_full(Q) : stream_passes(Q);   // FULL: all 32 lanes busy
     static constexpr int QP = Q / PASSES;                      // quads per row per pass (<= 32)
     static constexpr int G = stream_pow2ceil(QP);              // lanes that share one row
     static constexpr int RPL = 32 / G;                         // rows per warp-wide load

@@ -20,7 +20,7 @@ namespace coarse {
 
 template <int NC, bool I16, int R>
 struct StreamMrGeom {
-    using G1 = StreamGeom<NC, I16, false, false>;
+    using G1 = StreamGeom<NC, I16, false, false, true>;
     static constexpr int VEC_STAGE_N = NC * R * 8;
     static constexpr int VEC_STAGE_D = G1::RS * R * 8;
     static constexpr int RED_BYTES = G1::W * G1::RPL * NC * R * 8;   // dagger = 1, single buffer (two barriers per item)
@@ -42,8 +42,8 @@ struct StreamMrGeom {
 };
 
 template <int NC, bool I16, bool DAG, int R>
-__global__ void __launch_bounds__(StreamGeom<NC, I16, false, false>::THREADS, 1) coarse_apply_stream_mr(StreamParams p) {
-    using Gm = StreamGeom<NC, I16, false, false>;
+__global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREADS, 1) coarse_apply_stream_mr(StreamParams p) {
+    using Gm = StreamGeom<NC, I16, false, false, true>;
     using Gr = StreamMrGeom<NC, I16, R>;
     static_assert(Gr::OK, "unsupported STREAM-MR geometry");
     constexpr int W = Gm::W, RS = Gm::RS, NB = Gm::NB, WL = Gm::WL, QP = Gm::QP, G = Gm::G, RPL = Gm::RPL;
