@@ -54,6 +54,8 @@ def _load() -> ctypes.CDLL:
                                                   ctypes.c_double, ctypes.c_double, ci]
         lib.oracle_coarse_apply_hvec.restype = ci
         lib.oracle_coarse_apply_hvec.argtypes = [i4, ci, ci, vp, vp, vp, vp, vp, ci, ci, ci]
+        lib.oracle_coarse_apply_hvec_sites.restype = ci
+        lib.oracle_coarse_apply_hvec_sites.argtypes = [i4, ci, ci, vp, vp, vp, vp, vp, ci, ci, vp, ci64, ci]
         lib.oracle_quantize_vec_i16.restype = ci
         lib.oracle_quantize_vec_i16.argtypes = [vp, ci64, ci, ci, vp, vp]
         lib.oracle_neighbours.restype = ci
@@ -290,6 +292,29 @@ def coarse_apply_hvec(dims, Nc: int, links, vec_q, vec_norms, nrhs: int = 1, dag
                                           nm.ctypes.data, out.ctypes.data, nrhs, dagger, nthreads)
     if rc != 0:
         raise ValueError(f"oracle_coarse_apply_hvec rejected its arguments (rc={rc})")
+    return out
+
+
+def coarse_apply_hvec_sites(dims, Nc: int, links, vec_q, vec_norms, sites, nrhs: int = 1, dagger: int = 0,
+                            link_precision: int = LINK_C64, scales=None, nthreads: int = 0) -> np.ndarray:
+    """O8 evaluated only at `sites`; returns complex128 [len(sites)][Nc][nrhs]."""
+    V = int(np.prod([int(d) for d in dims]))
+    L = _as_links(links, link_precision, V, Nc)
+    q = np.ascontiguousarray(np.asarray(vec_q, dtype=np.int16))
+    nm = np.ascontiguousarray(np.asarray(vec_norms, dtype=np.float32))
+    if q.size != V * Nc * nrhs * 2 or nm.size != V * nrhs:
+        raise ValueError("half vectors must be int16 [V][Nc][nrhs][2] with float32 norms [V][nrhs]")
+    sc = None
+    if link_precision == LINK_I16:
+        sc = np.ascontiguousarray(np.asarray(scales, dtype=np.float32))
+    st = np.ascontiguousarray(np.asarray(sites, dtype=np.int64))
+    out = np.empty((st.size, Nc, nrhs), dtype=np.complex128)
+    rc = _load().oracle_coarse_apply_hvec_sites(_dims(dims), Nc, link_precision, L.ctypes.data,
+                                                sc.ctypes.data if sc is not None else None, q.ctypes.data,
+                                                nm.ctypes.data, out.ctypes.data, nrhs, dagger,
+                                                st.ctypes.data, st.size, nthreads)
+    if rc != 0:
+        raise ValueError(f"oracle_coarse_apply_hvec_sites rejected its arguments (rc={rc})")
     return out
 
 

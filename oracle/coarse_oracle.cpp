@@ -327,6 +327,33 @@ int oracle_coarse_apply_hvec(const int dims[4], int Nc, int link_precision, cons
     return 0;
 }
 
+// O8 evaluated only at the listed output sites (the same apply_site as every other entry point):
+// out is complex128 [nsites][Nc][nrhs], row k holding out(sites[k]).
+int oracle_coarse_apply_hvec_sites(const int dims[4], int Nc, int link_precision, const void* links,
+                                   const float* scales, const int16_t* in_q, const float* in_norms, double* out,
+                                   int nrhs, int dagger, const int64_t* sites, int64_t nsites, int nthreads) {
+    if (!valid(dims, Nc, link_precision, nrhs, dagger) || !links || !in_q || !in_norms || !out || !sites) return -1;
+    if (link_precision == 1 && !scales) return -1;
+    Lattice lat{{dims[0], dims[1], dims[2], dims[3]}, (int64_t)dims[0] * dims[1] * dims[2] * dims[3]};
+    for (int64_t k = 0; k < nsites; ++k) if (sites[k] < 0 || sites[k] >= lat.V) return -1;
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#pragma omp parallel num_threads(nthreads)
+#endif
+    {
+        g_hv.q = in_q;
+        g_hv.norms = in_norms;
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+        for (int64_t k = 0; k < nsites; ++k)
+            apply_site(lat, Nc, link_precision, links, scales, nullptr, nrhs, dagger, sites[k],
+                       out + k * 2 * (int64_t)Nc * nrhs);
+        g_hv = HalfVec();
+    }
+    return 0;
+}
+
 // O8 quantiser for vectors: one fp32 norm per (site, right-hand side),
 //   amax = max over the 2*Nc real components of |component|, norm = amax / 32767.0f,
 //   q = (int16) clamp(nearbyintf(component / norm), -32767, 32767); amax == 0 => norm = 0, q = 0.

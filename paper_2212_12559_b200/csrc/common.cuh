@@ -147,6 +147,23 @@ __device__ __forceinline__ uint4 lds128u(uint32_t addr) {
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
 }
+// Packed fp32 pairs (sm_100: fma.rn.f32x2 / add.rn.f32x2, SASS FFMA2 / FADD2): one issue slot for two
+// independent IEEE fp32 operations on an aligned register pair.
+__device__ __forceinline__ float2 ffma2(const float2 a, const float2 b, const float2 c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;"
+        : "=l"(d)
+        : "l"(reinterpret_cast<const uint64_t&>(a)), "l"(reinterpret_cast<const uint64_t&>(b)),
+          "l"(reinterpret_cast<const uint64_t&>(c)));
+    return reinterpret_cast<float2&>(d);
+}
+__device__ __forceinline__ float2 fadd2(const float2 a, const float2 b) {
+    uint64_t d;
+    asm("add.rn.f32x2 %0, %1, %2;"
+        : "=l"(d)
+        : "l"(reinterpret_cast<const uint64_t&>(a)), "l"(reinterpret_cast<const uint64_t&>(b)));
+    return reinterpret_cast<float2&>(d);
+}
 __device__ __forceinline__ float2 lds64(uint32_t addr) {
     float2 v;
     asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
@@ -166,7 +183,7 @@ __device__ __forceinline__ float2 unpack_i16x2(uint32_t w) {
     const uint32_t u = w ^ 0x80008000u;
     const uint32_t lo = __byte_perm(u, 0x4B000000u, 0x7610);
     const uint32_t hi = __byte_perm(u, 0x4B000000u, 0x7632);
-    return make_float2(__uint_as_float(lo) - 8421376.0f, __uint_as_float(hi) - 8421376.0f);
+    return ptx::fadd2(make_float2(__uint_as_float(lo), __uint_as_float(hi)), make_float2(-8421376.0f, -8421376.0f));
 }
 
 // The same decode through the conversion unit (I2F on the quarter-rate XU pipe).  The int16 STREAM

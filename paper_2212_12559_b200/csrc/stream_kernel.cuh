@@ -134,19 +134,15 @@ struct StreamGeom {
 };
 
 // acc += M * v   (conj = false)   |   acc += conj(M) * v   (conj = true)
+// Two packed FMAs (fma.rn.f32x2, SASS FFMA2, new on sm_100): acc += mre * (v.x, v.y), then
+// acc += mim * (-v.y, v.x) (conj: mim * (v.y, -v.x)).  Each half is an ordinary IEEE fp32 FMA, so the
+// result is the one the four scalar FMAs gave, in the same order; the instruction count of the
+// kernels' inner loops - which is what bounds the int16 and multi-RHS variants - halves.
 template <bool CONJ>
 __device__ __forceinline__ void cmac(float2& acc, float mre, float mim, const float2 v) {
-    if (!CONJ) {
-        acc.x = fmaf(mre, v.x, acc.x);
-        acc.x = fmaf(-mim, v.y, acc.x);
-        acc.y = fmaf(mre, v.y, acc.y);
-        acc.y = fmaf(mim, v.x, acc.y);
-    } else {
-        acc.x = fmaf(mre, v.x, acc.x);
-        acc.x = fmaf(mim, v.y, acc.x);
-        acc.y = fmaf(mre, v.y, acc.y);
-        acc.y = fmaf(-mim, v.x, acc.y);
-    }
+    const float2 vs = CONJ ? make_float2(v.y, -v.x) : make_float2(-v.y, v.x);
+    acc = ptx::ffma2(make_float2(mre, mre), v, acc);
+    acc = ptx::ffma2(make_float2(mim, mim), vs, acc);
 }
 
 template <int NC, bool I16, bool DAG, bool FINE = false, bool GEN = false, bool HV = false>

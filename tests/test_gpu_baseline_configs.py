@@ -1,11 +1,10 @@
 """GPU parity at BASELINE.json's full sizes (configs C1..C5), in the launch configuration bench.py
 times (AUTO path, default persistent grid).
 
-Small configs are compared element by element over the whole lattice.  For the large ones the
-oracle evaluates its definition one site at a time on SAMPLED output sites (lattice corners, the
-first/last sites, and seeded random sites); only the link matrices and vectors those sites touch
-are brought to the host.  At any size the adjoint identity <u, A v> = <A^H u, v> ties the dagger
-kernel to the non-dagger kernel over the WHOLE lattice.
+Every config is compared with the oracle element by element over the WHOLE lattice, both modes
+(tests/fullsize.py: the oracle evaluates its definition site by site over chunks of x3-slices, so
+the 16 GB of C2 links never sit on the host at once).  The adjoint identity <u, A v> = <A^H u, v>
+additionally ties the dagger kernel to the non-dagger kernel.
 """
 import numpy as np
 import pytest
@@ -13,12 +12,11 @@ import torch
 
 import synth
 import paper_2212_12559_b200 as cop
-from tests.helpers import neighbour_table, rel_l2_per_rhs
+from tests.fullsize import whole_lattice_errors
 
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-5                      # BASELINE.json north_star: relative L2 per output vector
-FULL_COMPARE_MAX_CMAC = 1.2e9   # whole-lattice oracle apply stays within seconds below this
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -52,28 +50,6 @@ def _build(name, oracle_lib):
     return cfg, V, links, scales, prec, vin, op
 
 
-def _sample_sites(dims, V, n_random, seed):
-    L0, L1, L2, L3 = dims
-    corners = []
-    for x3 in (0, L3 - 1):
-        for x2 in (0, L2 - 1):
-            for x1 in (0, L1 - 1):
-                for x0 in (0, L0 - 1):
-                    corners.append(x0 + L0 * (x1 + L1 * (x2 + L2 * x3)))
-    rng = np.random.default_rng(seed)
-    rnd = rng.integers(0, V, size=n_random)
-    return np.unique(np.concatenate([np.array(corners + [0, 1, V - 2, V - 1]), rnd])).astype(np.int64)
-
-
-def _host_sparse(t_dev, rows, shape_tail, dtype):
-    """Host array of the full first dimension with only `rows` filled from the device tensor
-    (untouched pages of np.empty are never committed)."""
-    host = np.empty((t_dev.shape[0],) + shape_tail, dtype=dtype)
-    idx = torch.as_tensor(rows, device=t_dev.device)
-    host[rows] = t_dev[idx].cpu().numpy().reshape((len(rows),) + shape_tail)
-    return host
-
-
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
 def test_baseline_config_parity(oracle_lib, name):
     cfg, V, links, scales, prec, vin, op = _build(name, oracle_lib)
@@ -91,34 +67,16 @@ def test_baseline_config_parity(oracle_lib, name):
     else:
         assert op.last_path == cop.PATH_TENSOR          # C5: block apply on the tensor cores
 
-    work = V * 9.0 * Nc * Nc * nrhs
-    vin_h = vin.cpu().numpy()
-    if work <= FULL_COMPARE_MAX_CMAC:
-        links_h = links.cpu().numpy()
-        scales_h = None if scales is None else scales.cpu().numpy()
-        for dagger in (0, 1):
-            ref = oracle_lib.coarse_apply(dims, Nc, links_h, vin_h, nrhs=nrhs, dagger=dagger,
-                                          link_precision=prec, scales=scales_h)
-            err = rel_l2_per_rhs(outs[dagger].cpu().numpy(), ref)
-            assert err <= TOL, f"{name} dagger={dagger}: rel-L2 {err:.3e}"
-    else:
-        sites = _sample_sites(dims, V, 160 if nrhs == 1 else 48, cfg["seed"])
-        nbr = neighbour_table(dims)
-        need = np.unique(nbr[sites].reshape(-1))
-        tail = (9, Nc, Nc, 2)
-        links_h = _host_sparse(links if prec == cop.LINK_I16 else torch.view_as_real(links),
-                               need, tail, np.int16 if prec == cop.LINK_I16 else np.float32)
-        scales_h = None if scales is None else scales.cpu().numpy()
-        for dagger in (0, 1):
-            ref = oracle_lib.coarse_apply_sites(dims, Nc, links_h, vin_h, sites, nrhs=nrhs, dagger=dagger,
-                                                link_precision=prec, scales=scales_h)
-            got = outs[dagger][torch.as_tensor(sites, device="cuda")].cpu().numpy()
-            err = rel_l2_per_rhs(got, ref)
-            assert err <= TOL, f"{name} dagger={dagger}: sampled rel-L2 {err:.3e}"
-            # per-site errors too: one wrong site must not hide in the norm
-            per_site = np.linalg.norm((got - ref).reshape(len(sites), -1), axis=1) / \
-                np.linalg.norm(ref.reshape(len(sites), -1), axis=1)
-            assert per_site.max() <= 5 * TOL
+    # EVERY output site against the oracle, element by element: the oracle's
+    # per-site evaluation over chunks of x3-slices, links brought to the host chunk by chunk
+    res = whole_lattice_errors(oracle_lib, dims, Nc, links, scales, prec, outs, nrhs, vin_h=vin.cpu().numpy())
+    for dagger in (0, 1):
+        err, worst_site, n_sites = res[dagger]
+        assert n_sites == V
+        assert err <= TOL, f"{name} dagger={dagger}: whole-lattice rel-L2 {err:.3e}"
+        # per-site errors too: one wrong site must not hide in the norm
+        assert worst_site <= 5 * TOL, f"{name} dagger={dagger}: worst site rel-L2 {worst_site:.3e}"
+        print(f"{name} dagger={dagger}: {n_sites} sites compared, rel-L2 {err:.2e}, worst site {worst_site:.2e}")
 
     # whole-lattice property: <u, A v> = <A^H u, v>   (u = a second seeded vector)
     u = synth.make_vectors(dims, Nc, nrhs, cfg["seed"] + 2, device="cuda")

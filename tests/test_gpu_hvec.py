@@ -89,10 +89,10 @@ def test_hvec_simple(oracle_lib, nrhs, prec, dagger):
     _run(oracle_lib, (2, 2, 1, 2), 48, prec, nrhs, dagger, cop.PATH_SIMPLE)
 
 
-def test_hvec_full_size_c4_sampled(oracle_lib):
+def test_hvec_full_size_c4_whole_lattice(oracle_lib):
     """BASELINE config C4 with half-precision input vectors, in the launch configuration of the bench:
-    sampled output sites against the oracle."""
-    from tests.helpers import neighbour_table
+    every output site against the oracle's O8 (`coarse_apply_hvec_sites`, the oracle's own apply_site)."""
+    from tests.fullsize import whole_lattice_errors
     cfg = synth.config("C4")
     dims, Nc = cfg["dims"], cfg["Nc"]
     V = synth.lattice_volume(dims)
@@ -106,38 +106,15 @@ def test_hvec_full_size_c4_sampled(oracle_lib):
     nm = torch.empty((V, 1), dtype=torch.float32, device="cuda")
     cop.coarse_op_quantize_vec_i16(v, Nc, 1, q, nm)
     op = cop.CoarseOp(dims, Nc, cop.LINK_I16).set_links(lq, scales)
-    rng = np.random.default_rng(3)
-    sites = np.unique(np.concatenate([[0, 1, V - 1], rng.integers(0, V, 64)])).astype(np.int64)
-    need = np.unique(neighbour_table(dims)[sites].reshape(-1))
-    links_h = np.empty((V, 9, Nc, Nc, 2), dtype=np.int16)
-    links_h[need] = lq[torch.as_tensor(need, device="cuda")].cpu().numpy()
-    q_h, nm_h, sc_h = q.cpu().numpy(), nm.cpu().numpy(), scales.cpu().numpy()
-    deq = (q_h.astype(np.float64) * nm_h[:, None, :, None].astype(np.float64))
+    outs = {}
     for dagger in (0, 1):
-        out = torch.empty_like(v)
-        op.apply_hvec(q, nm, out, dagger=dagger)
+        outs[dagger] = torch.full_like(v, float("nan"))
+        op.apply_hvec(q, nm, outs[dagger], dagger=dagger)
         torch.cuda.synchronize()
         assert op.last_path == cop.PATH_STREAM
-        # oracle one site at a time: build the 9 neighbour vectors exactly (double) via apply_sites on a
-        # float vector is not exact, so use the hvec oracle on a compact sub-lattice-free evaluation:
-        ref = _oracle_sites_hvec(oracle_lib, dims, Nc, links_h, sc_h, q_h, nm_h, sites, dagger)
-        got = out[torch.as_tensor(sites, device="cuda")].cpu().numpy()
-        assert rel_l2_per_rhs(got, ref) <= TOL
+    res = whole_lattice_errors(oracle_lib, dims, Nc, lq, scales, cop.LINK_I16, outs, 1,
+                               hvec=(q.cpu().numpy(), nm.cpu().numpy()))
+    for dagger in (0, 1):
+        err, worst_site, n_sites = res[dagger]
+        assert n_sites == V and err <= TOL and worst_site <= 5 * TOL, (dagger, err, worst_site)
     op.close()
-
-
-def _oracle_sites_hvec(oracle_lib, dims, Nc, links_h, sc_h, q_h, nm_h, sites, dagger):
-    """out(x) at the sampled sites from the oracle's int16-link dequantiser and the definition O1/O2,
-    written with numpy matrix products on the 9 dequantised matrices per site (double)."""
-    from tests.helpers import neighbour_table
-    nbr = neighbour_table(dims)
-    x = (q_h[..., 0].astype(np.float64) + 1j * q_h[..., 1].astype(np.float64)) * nm_h[:, None, :].astype(np.float64)
-    out = np.zeros((len(sites), Nc, 1), dtype=np.complex128)
-    for k, s in enumerate(sites):
-        for m in range(9):
-            # dagger: Y_{+mu} comes from x-mu^ (nbr index 5+mu), Y_{-mu} from x+mu^ (nbr index 1+mu)
-            sv = nbr[s, m] if not dagger else (s if m == 0 else nbr[s, m + 4 if m <= 4 else m - 4])
-            sm = sv if dagger else s
-            M = oracle_lib.dequantize_i16(links_h[sm, m][None], sc_h[sm, m][None], Nc)[0]
-            out[k] += (M.conj().T if dagger else M) @ x[sv]
-    return out

@@ -72,3 +72,30 @@ def test_half_vectors_cost_about_3e5_relative(oracle_lib):
     a = oracle_lib.coarse_apply_hvec(dims, Nc, links, q, norms)
     b = oracle_lib.coarse_apply(dims, Nc, links, v)
     assert 1e-6 < rel_l2(a, b) < 2e-4
+
+
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_hvec_sites_is_the_dense_operator_rows(oracle_lib, dagger):
+    """coarse_apply_hvec_sites at a site list = those block rows of the dense operator (assembled with
+    numpy from the dequantised links) times the exactly dequantised vector; int16 links, 2 RHS, extents 1-3."""
+    dims, Nc, nrhs = (3, 2, 1, 2), 6, 2
+    V = 12
+    links = synth.make_arbitrary_links(dims, Nc, 21).numpy()
+    lq, sc = oracle_lib.quantize_i16(links, Nc)
+    ldeq = oracle_lib.dequantize_i16(lq, sc, Nc).reshape(V, 9, Nc, Nc)
+    A = assemble_dense(ldeq, dims)
+    if dagger:
+        A = A.conj().T
+    v = synth.make_vectors(dims, Nc, nrhs, 22).numpy()
+    q, norms = oracle_lib.quantize_vec_i16(v, Nc, nrhs)
+    deq = q.astype(np.float64) * norms[:, None, :, None].astype(np.float64)
+    x = (deq[..., 0] + 1j * deq[..., 1]).reshape(V * Nc, nrhs)
+    ref = (A @ x).reshape(V, Nc, nrhs)
+    sites = np.array([11, 0, 5, 5, 7], dtype=np.int64)          # unordered, with a repeat
+    got = oracle_lib.coarse_apply_hvec_sites(dims, Nc, lq.reshape(V, 9, Nc, Nc, 2), q, norms, sites, nrhs=nrhs,
+                                             dagger=dagger, link_precision=oracle_lib.LINK_I16, scales=sc)
+    assert got.shape == (5, Nc, nrhs)
+    assert rel_l2(got, ref[sites]) < 1e-13
+    full = oracle_lib.coarse_apply_hvec(dims, Nc, lq.reshape(V, 9, Nc, Nc, 2), q, norms, nrhs=nrhs, dagger=dagger,
+                                        link_precision=oracle_lib.LINK_I16, scales=sc)
+    assert np.array_equal(got, full[sites])
