@@ -77,6 +77,7 @@ class ClockSampler:
 
     def __init__(self, index: int, period_s: float = 0.02):
         self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.power_w = []
         self._stop = threading.Event()
         self._thread = None
         self._period = period_s
@@ -101,6 +102,10 @@ class ClockSampler:
         while not self._stop.is_set():
             try:
                 self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                try:
+                    self.power_w.append(nv.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
+                except Exception:
+                    pass
                 try:
                     mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
                 except Exception:
@@ -127,8 +132,13 @@ class ClockSampler:
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
         s = sorted(self.samples)
-        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(s)}
+        out = {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+               "samples": len(s), "sm_mhz_min": s[0]}
+        if self.power_w:
+            pw = sorted(self.power_w)
+            out["power_w"] = pw[len(pw) // 2]
+            out["power_w_max"] = pw[-1]
+        return out
 
 
 def dist_env():
@@ -295,6 +305,8 @@ def run_ours(args, cfg, daggers):
         op.set_option(cop.OPT_KEEP_LINKS, args.keep_links)
     if args.pdl:
         op.set_option(cop.OPT_PDL, 1)
+    if args.warp_items:
+        op.set_option(cop.OPT_WARP_ITEMS, args.warp_items)
 
     vq = vnorm = None
     if args.hvec:
@@ -670,6 +682,11 @@ def main():
                     help="time all K steps as one CUDA graph (auto: when the links fit 2x L2)")
     ap.add_argument("--cheb", action="store_true", help="--workload cagcr: Chebyshev-basis CA-GCR(16) instead of CA-GCR(8)")
     ap.add_argument("--nrhs", type=int, default=0, help="override the config's number of right-hand sides")
+    ap.add_argument("--nc", type=int, default=0, help="override the config's colour-spin size Nc (other compiled shapes)")
+    ap.add_argument("--dims", default="", help="override the config's lattice, e.g. 16,16,8,12")
+    ap.add_argument("--links", default="", choices=["", "c64", "i16"], help="override the config's link storage")
+    ap.add_argument("--warp-items", type=int, default=0,
+                    help="COARSE_OPT_WARP_ITEMS override (0 auto, 1 never, 2 always, 11/12/14: 1/2/4 warps per team)")
     ap.add_argument("--pdl", action="store_true", help="COARSE_OPT_PDL: programmatic dependent launch for chained applies")
     ap.add_argument("--hvec", action="store_true",
                     help="half-precision INPUT vectors (int16 + per-site norm, row f2) through coarse_op_apply_hvec")
@@ -679,6 +696,14 @@ def main():
     cfg = synth.config(args.config)
     if args.nrhs:
         cfg["nrhs"] = args.nrhs
+    if args.nc:
+        cfg["Nc"] = args.nc
+    if args.dims:
+        cfg["dims"] = tuple(int(x) for x in args.dims.split(","))
+    if args.links:
+        cfg["links"] = args.links
+    if args.nrhs or args.nc or args.dims or args.links:
+        args.config = args.config + "*"          # not the BASELINE config any more: keyed tables do not apply
     daggers = [0, 1] if args.dagger == "both" else [int(args.dagger)]
     if args.workload == "schur":
         return run_schur(args, cfg)

@@ -81,15 +81,20 @@ enum {
     COARSE_OPT_STAGES = 2,   /* cap on the STREAM shared-memory ring depth; 0 = library default   */
     COARSE_OPT_FINE = 3,     /* STREAM dagger=0 small-lattice row-block split: 0 auto, 1 never, 2 always */
     COARSE_OPT_KEEP_LINKS = 4, /* L2 policy of the link stream: 0 auto (keep if links <= L2/2), 1 evict_first, 2 keep */
-    COARSE_OPT_SPLIT_DAGGER = 6, /* dagger = 1, 1 RHS, lattices with fewer sites than SMs: split each site's
-                                contraction over its row chunks + a reduce kernel (2 launches): 0 auto, 1 never,
-                                2 always (needs the workspace coarse_op_set_links allocates on such lattices) */
-    COARSE_OPT_PDL = 5       /* 1: launch the 1-RHS STREAM kernels with programmatic dependent launch: in a chain
+    COARSE_OPT_PDL = 5,      /* 1: launch the 1-RHS STREAM kernels with programmatic dependent launch: in a chain
                                 of applies on one stream the next kernel's CTAs start on SMs the previous one
                                 has left and prefetch their link stages before waiting for its output (the
                                 latency-limited small-lattice regime of PAPER.md:L99).  Default 0.  With it on,
                                 the LINK and scale arrays must not be written by work still in flight on the
                                 stream (they are read before the kernel orders itself against its predecessor). */
+    COARSE_OPT_SPLIT_DAGGER = 6, /* dagger = 1, 1 RHS, lattices with fewer sites than SMs: split each site's
+                                contraction over its row chunks + a reduce kernel (2 launches): 0 auto, 1 never,
+                                2 always (needs the workspace coarse_op_set_links allocates on such lattices) */
+    COARSE_OPT_WARP_ITEMS = 7 /* 1-RHS plain apply: the STREAM variant in which small teams of consumer warps own
+                                whole work items and every stage of theirs (csrc/stream2_kernel.cuh) instead of all
+                                eight warps sharing every stage: 0 auto (int16 links on lattices with at least 4
+                                items per team of the chip), 1 never, 2 always, 12 / 14 always with 2 / 4 warps per
+                                team (2 = 14).  With it COARSE_OPT_STAGES is the ring's slot count. */
 };
 
 /* Create an operator descriptor for a periodic lattice dims[0..3] (each >= 1), Nc even and

@@ -1,8 +1,6 @@
 // coarse_op.cu — C ABI of libcoarseop (include/coarse_op.h): argument checking, kernel selection
 // and launches.  All arithmetic of the coarse-op apply lives in the kernels included below.
-#include "../../include/coarse_op.h"
-
-#include <cuda_runtime.h>
+#include "internal.h"
 
 #include <cstdarg>
 #include <cstdio>
@@ -14,17 +12,17 @@
 #include "quantize_kernel.cuh"
 #include "simple_kernel.cuh"
 #include "stream_kernel.cuh"
-#include "stream_mr_kernel.cuh"
 #include "block_kernel.cuh"
-#include "tensor_kernel.cuh"
 #include "probe_kernel.cuh"
 #include "cagcr_kernel.cuh"
 
 using namespace coarse;
 
 namespace {
-
 thread_local std::string g_last_error = "";
+}
+
+namespace coarse {
 
 int fail(int code, const char* fmt, ...) {
     char buf[512];
@@ -40,165 +38,17 @@ int cuda_fail(cudaError_t e, const char* what) {
     return fail(COARSE_ECUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
+}  // namespace coarse
+
+namespace {
+
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 }  // namespace
 
-struct coarse_op {
-    Lat lat;
-    int Nc;
-    int prec;
-    const void* links;
-    const float* scales;
-    int path_opt;
-    int grid_opt;
-    int stages_opt;
-    int fine_opt;
-    int keep_opt;
-    int pdl_opt;
-    int split_opt;            // COARSE_OPT_SPLIT_DAGGER: 0 auto, 1 never, 2 always
-    float2* split_ws;         // partial vectors of the split dagger apply (allocated by set_links on tiny lattices)
-    size_t split_ws_bytes;
-    int l2_bytes;
-    int last_launches;
-    int last_path;
-    int device;
-    int num_sms;
-    int max_smem;
-    void* stage_in;
-    void* stage_out;
-    size_t stage_bytes;
-    cudaStream_t s_h2d, s_d2h;      // apply_host's copy streams and events (created on first use)
-    cudaEvent_t ev_up[4], ev_k[4], ev_done;
-    bool host_pipe_ok;
-    CUtensorMap link_map;   // 2-D view of the link array for the TENSOR path (dagger = 0 slabs)
-    bool link_map_ok;
-};
-
 namespace {
 
-// Parts apply (coarse_op_apply_parts): out = alpha*Loc(u) + beta*Hop(w) on one parity.  The plain
-// apply is the special case gen = false (u = w, local = X, alpha = beta = 1, all sites).
-struct PartsSpec {
-    bool gen;
-    const void* u;
-    int parity;   // 0 even, 1 odd, 2 all
-    int local;    // 0 none, 1 X, 2 identity
-    float alpha, beta;
-    const float* vnorms;   // non-NULL: half-precision input vectors (plain apply only)
-    int site_begin, site_end;   // output sites [site_begin, site_end) (plain apply only); end = 0: all
-};
 const PartsSpec kPlain = {false, nullptr, 2, 1, 1.f, 1.f, nullptr, 0, 0};
-
-// ---------------------------------------------------------------- STREAM dispatch
-template <int NC, bool I16, bool DAG, bool FINE, bool GEN, bool HV = false>
-int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
-    using Gm = StreamGeom<NC, I16, FINE, HV>;
-    static_assert(Gm::OK, "unsupported STREAM geometry");
-    StreamParams p = base;
-    p.n_items = DAG ? p.n_sites : p.n_sites * Gm::NB;
-    if (base.n_items > 0) {                       // a site range [item_begin, n_items) was requested (in sites)
-        p.item_begin = DAG ? base.item_begin : base.item_begin * Gm::NB;
-        p.n_items = DAG ? base.n_items : base.n_items * Gm::NB;
-    }
-    // dagger = 1 has one work item per site; on a lattice with fewer sites than SMs (the paper's level 3:
-    // 32 sites per GPU) the contraction of a site is split over its NB row chunks, one item each, and a
-    // small second kernel adds the NB partial vectors in order.
-    p.split = 0;
-    p.partial = nullptr;
-    if (DAG && !GEN && !HV && base.n_items == 0 && Gm::NB > 1 && op->split_ws &&
-        (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes &&
-        (op->split_opt == 2 || (op->split_opt == 0 && p.n_sites < op->num_sms))) {
-        p.split = 1;
-        p.partial = op->split_ws;
-        p.n_items = p.n_sites * Gm::NB;
-    }
-    int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (Gm::stage_bytes(DAG) + 16);
-    if (stages > 12) stages = 12;
-    if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM: shared memory too small for Nc=%d", NC);
-    // Default depth: ~112 KB in flight per SM (the measured optimum, see stream_kernel.cuh), at
-    // least 4 stages; COARSE_OPT_STAGES overrides.
-    int want = (114688 + Gm::stage_bytes(DAG) / 2) / Gm::stage_bytes(DAG);
-    if (want < 4) want = 4;
-    if (op->stages_opt > 0) want = op->stages_opt;
-    if (stages > want) stages = want;
-    p.stages = stages;
-    int smem = Gm::smem_bytes(DAG, stages);
-    // PDL: a kernel whose shared-memory carve-out differs from its predecessor's cannot take over an SM
-    // before it has drained completely (measured: an alternating dagger 0 / dagger 1 chain gained nothing
-    // until both kernels asked for the same size), so under PDL both modes request the larger of the two.
-    if (op->pdl_opt && Gm::smem_bytes(!DAG, stages) > smem && Gm::smem_bytes(!DAG, stages) <= op->max_smem)
-        smem = Gm::smem_bytes(!DAG, stages);
-    auto kern = coarse_apply_stream<NC, I16, DAG, FINE, GEN, HV>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
-    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
-    if (grid > p.n_items - p.item_begin) grid = p.n_items - p.item_begin;
-    if (grid < 1) return COARSE_OK;
-    p.pdl = op->pdl_opt ? 1 : 0;
-    if (p.pdl) {
-        // programmatic dependent launch: this kernel may start while the previous kernel of the stream
-        // drains; it orders itself against that kernel's memory with griddepcontrol.wait (stream_kernel.cuh)
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(grid);
-        cfg.blockDim = dim3(Gm::THREADS);
-        cfg.dynamicSmemBytes = smem;
-        cfg.stream = stream;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        e = cudaLaunchKernelEx(&cfg, kern, p);
-        if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch (PDL)");
-    } else {
-        kern<<<grid, Gm::THREADS, smem, stream>>>(p);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch");
-    }
-    if (p.split) {
-        const long long tot = (long long)p.n_sites * NC;
-        coarse_dagger_reduce_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(p.partial, p.n_sites, Gm::NB, NC, p.out);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return cuda_fail(e, "dagger reduce kernel launch");
-        return 1;      // one extra launch (coarse_op_apply adds it to last_launches)
-    }
-    return COARSE_OK;
-}
-
-// dagger = 0 on a tiny lattice: switch to the fine row-block geometry when the regular one gives
-// fewer work items than SMs (COARSE_OPT_FINE: 0 auto, 1 never, 2 always).  Measured on C1
-// (256 sites, Nc = 48: 256 regular items on 148 SMs) the regular geometry is 2.8x faster (5.6 us
-// vs 15.4 us warm): 3 KB stages pay the per-stage handshake 6x more often, so the fine split only
-// pays when SMs would otherwise sit idle.
-template <int NC, bool I16, bool GEN>
-int launch_stream_n(const coarse_op* op, const StreamParams& p, cudaStream_t stream) {
-    constexpr bool HAS_FINE = StreamGeom<NC, I16, true>::NB > StreamGeom<NC, I16, false>::NB;
-    if constexpr (HAS_FINE) {
-        const bool few = (int64_t)p.n_sites * StreamGeom<NC, I16, false>::NB < (int64_t)op->num_sms;
-        if (op->fine_opt == 2 || (op->fine_opt == 0 && few)) return launch_stream_t<NC, I16, false, true, GEN>(op, p, stream);
-    }
-    return launch_stream_t<NC, I16, false, false, GEN>(op, p, stream);
-}
-
-template <int NC, bool GEN>
-int launch_stream_nc(const coarse_op* op, const StreamParams& p, int dagger, cudaStream_t stream) {
-    if (op->prec == COARSE_LINK_I16)
-        return dagger ? launch_stream_t<NC, true, true, false, GEN>(op, p, stream) : launch_stream_n<NC, true, GEN>(op, p, stream);
-    return dagger ? launch_stream_t<NC, false, true, false, GEN>(op, p, stream) : launch_stream_n<NC, false, GEN>(op, p, stream);
-}
-
-template <int NC>
-int launch_stream_g(const coarse_op* op, const StreamParams& p, int dagger, bool gen, cudaStream_t stream) {
-    if (p.vnorms) {   // half-precision input vectors: regular geometry, plain apply
-        if (op->prec == COARSE_LINK_I16)
-            return dagger ? launch_stream_t<NC, true, true, false, false, true>(op, p, stream)
-                          : launch_stream_t<NC, true, false, false, false, true>(op, p, stream);
-        return dagger ? launch_stream_t<NC, false, true, false, false, true>(op, p, stream)
-                      : launch_stream_t<NC, false, false, false, false, true>(op, p, stream);
-    }
-    return gen ? launch_stream_nc<NC, true>(op, p, dagger, stream) : launch_stream_nc<NC, false>(op, p, dagger, stream);
-}
 
 bool stream_supports(int Nc, int nrhs) {
     if (nrhs != 1) return false;
@@ -209,49 +59,6 @@ bool stream_supports(int Nc, int nrhs) {
 }
 
 bool stream_mr_supports(int Nc, int nrhs) { return stream_supports(Nc, 1) && nrhs >= 2 && nrhs <= 4; }
-
-// ---------------------------------------------------------------- STREAM-MR dispatch (2 <= nrhs <= 4)
-template <int NC, bool I16, bool DAG, int R>
-int launch_stream_mr_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
-    using Gm = StreamGeom<NC, I16, false, false, true>;
-    using Gr = StreamMrGeom<NC, I16, R>;
-    StreamParams p = base;
-    p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
-    int stages = (op->max_smem - Gr::fixed_bytes(DAG)) / (Gr::stage_bytes(DAG) + 16);
-    if (stages > 12) stages = 12;
-    if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM-MR: shared memory too small for Nc=%d nrhs=%d", NC, R);
-    int want = (114688 + Gr::stage_bytes(DAG) / 2) / Gr::stage_bytes(DAG);
-    if (want < 4) want = 4;
-    if (op->stages_opt > 0) want = op->stages_opt;
-    if (stages > want) stages = want;
-    p.stages = stages;
-    const int smem = Gr::smem_bytes(DAG, stages);
-    auto kern = coarse_apply_stream_mr<NC, I16, DAG, R>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream-mr kernel)");
-    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
-    if (grid > p.n_items) grid = p.n_items;
-    kern<<<grid, Gm::THREADS, smem, stream>>>(p);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "stream-mr kernel launch");
-    return COARSE_OK;
-}
-
-template <int NC, int R>
-int launch_stream_mr_r(const coarse_op* op, const StreamParams& p, int dagger, cudaStream_t stream) {
-    if (op->prec == COARSE_LINK_I16)
-        return dagger ? launch_stream_mr_t<NC, true, true, R>(op, p, stream) : launch_stream_mr_t<NC, true, false, R>(op, p, stream);
-    return dagger ? launch_stream_mr_t<NC, false, true, R>(op, p, stream) : launch_stream_mr_t<NC, false, false, R>(op, p, stream);
-}
-
-template <int NC>
-int launch_stream_mr_nc(const coarse_op* op, const StreamParams& p, int nrhs, int dagger, cudaStream_t stream) {
-    switch (nrhs) {
-        case 2: return launch_stream_mr_r<NC, 2>(op, p, dagger, stream);
-        case 3: return launch_stream_mr_r<NC, 3>(op, p, dagger, stream);
-        default: return launch_stream_mr_r<NC, 4>(op, p, dagger, stream);
-    }
-}
 
 int launch_stream_mr(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, cudaStream_t stream) {
     StreamParams p = {};
@@ -264,12 +71,9 @@ int launch_stream_mr(const coarse_op* op, const void* in, void* out, int nrhs, i
     p.parity = 2;
     p.n_sites = op->lat.V;
     switch (op->Nc) {
-        case 32: return launch_stream_mr_nc<32>(op, p, nrhs, dagger, stream);
-        case 48: return launch_stream_mr_nc<48>(op, p, nrhs, dagger, stream);
-        case 64: return launch_stream_mr_nc<64>(op, p, nrhs, dagger, stream);
-        case 96: return launch_stream_mr_nc<96>(op, p, nrhs, dagger, stream);
-        case 128: return launch_stream_mr_nc<128>(op, p, nrhs, dagger, stream);
-        case 192: return launch_stream_mr_nc<192>(op, p, nrhs, dagger, stream);
+#define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_stream_mr_nc, NC)(op, p, nrhs, dagger, stream);
+        COARSE_FOR_EACH_NC(COARSE_CASE_NC)
+#undef COARSE_CASE_NC
         default: return fail(COARSE_EUNSUPPORTED, "STREAM path is not compiled for Nc=%d", op->Nc);
     }
 }
@@ -295,51 +99,11 @@ int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, co
     p.n_sites = ps.parity == 2 ? op->lat.V : op->lat.V / 2;
     p.vnorms = ps.vnorms;
     switch (op->Nc) {
-        case 32: return launch_stream_g<32>(op, p, dagger, ps.gen, stream);
-        case 48: return launch_stream_g<48>(op, p, dagger, ps.gen, stream);
-        case 64: return launch_stream_g<64>(op, p, dagger, ps.gen, stream);
-        case 96: return launch_stream_g<96>(op, p, dagger, ps.gen, stream);
-        case 128: return launch_stream_g<128>(op, p, dagger, ps.gen, stream);
-        case 192: return launch_stream_g<192>(op, p, dagger, ps.gen, stream);
+#define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_stream_nc, NC)(op, p, dagger, ps.gen, stream);
+        COARSE_FOR_EACH_NC(COARSE_CASE_NC)
+#undef COARSE_CASE_NC
         default: return fail(COARSE_EUNSUPPORTED, "STREAM path is not compiled for Nc=%d", op->Nc);
     }
-}
-
-// ---------------------------------------------------------------- BLOCK dispatch
-template <int NC, bool I16, bool DAG, int RP>
-int launch_block_t(const coarse_op* op, const BlockParams& base, cudaStream_t stream) {
-    using Gm = BlockGeom<NC, I16, RP>;
-    BlockParams p = base;
-    p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
-    const int sb = Gm::stage_bytes(DAG, p.nrhs);
-    int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (sb + 16);
-    if (stages < 2) return fail(COARSE_EUNSUPPORTED, "BLOCK: shared memory too small for Nc=%d nrhs=%d", NC, p.nrhs);
-    int want = (114688 + sb / 2) / sb;
-    if (want < 3) want = 3;
-    if (op->stages_opt > 0) want = op->stages_opt;
-    if (stages > want) stages = want;
-    p.stages = stages;
-    const int smem = Gm::smem_bytes(DAG, p.nrhs, stages);
-    auto kern = coarse_apply_block<NC, I16, DAG, RP>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(block kernel)");
-    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
-    if (grid > p.n_items) grid = p.n_items;
-    kern<<<grid, Gm::THREADS, smem, stream>>>(p);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "block kernel launch");
-    return COARSE_OK;
-}
-
-template <int NC>
-int launch_block_nc(const coarse_op* op, const BlockParams& p, int dagger, cudaStream_t stream) {
-    const bool i16 = op->prec == COARSE_LINK_I16;
-    if (p.nrhs <= 8) {
-        if (i16) return dagger ? launch_block_t<NC, true, true, 8>(op, p, stream) : launch_block_t<NC, true, false, 8>(op, p, stream);
-        return dagger ? launch_block_t<NC, false, true, 8>(op, p, stream) : launch_block_t<NC, false, false, 8>(op, p, stream);
-    }
-    if (i16) return dagger ? launch_block_t<NC, true, true, 16>(op, p, stream) : launch_block_t<NC, true, false, 16>(op, p, stream);
-    return dagger ? launch_block_t<NC, false, true, 16>(op, p, stream) : launch_block_t<NC, false, false, 16>(op, p, stream);
 }
 
 bool block_supports_nc(int Nc) { return stream_supports(Nc, 1); }
@@ -357,93 +121,10 @@ int launch_block(const coarse_op* op, const void* in, void* out, int nrhs, int d
     p.nrhs = nrhs;
     p.keep_links = op->keep_opt == 2 || (op->keep_opt == 0 && coarse_op_link_bytes(op) <= (size_t)op->l2_bytes / 2);
     switch (op->Nc) {
-        case 32: return launch_block_nc<32>(op, p, dagger, stream);
-        case 48: return launch_block_nc<48>(op, p, dagger, stream);
-        case 64: return launch_block_nc<64>(op, p, dagger, stream);
-        case 96: return launch_block_nc<96>(op, p, dagger, stream);
-        case 128: return launch_block_nc<128>(op, p, dagger, stream);
-        case 192: return launch_block_nc<192>(op, p, dagger, stream);
+#define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_block_nc, NC)(op, p, dagger, stream);
+        COARSE_FOR_EACH_NC(COARSE_CASE_NC)
+#undef COARSE_CASE_NC
         default: return fail(COARSE_EUNSUPPORTED, "BLOCK path is not compiled for Nc=%d", op->Nc);
-    }
-}
-
-// ---------------------------------------------------------------- TENSOR dispatch
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_tiled_fn() {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void* sym = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
-            qres == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(sym);
-        else
-            cudaGetLastError();
-    }
-    return fn;
-}
-
-bool tensor_supports_nc(int Nc, int prec) {
-    return prec == COARSE_LINK_C64 && (Nc == 48 || Nc == 64 || Nc == 128);
-}
-bool tensor_supports(int Nc, int prec, int nrhs) { return tensor_supports_nc(Nc, prec) && (nrhs == 8 || nrhs == 16); }
-
-// links[V*9*Nc rows][2*Nc floats]; box = Nc rows x 32 floats (128 B), SWIZZLE_128B.
-int make_link_map(coarse_op* op) {
-    op->link_map_ok = false;
-    if (!tensor_supports_nc(op->Nc, op->prec)) return COARSE_OK;
-    EncodeTiledFn fn = encode_tiled_fn();
-    if (!fn) return COARSE_OK;   // TENSOR path stays unavailable; apply reports it if it is requested
-    const cuuint64_t gdim[2] = {(cuuint64_t)2 * op->Nc, (cuuint64_t)op->lat.V * 9 * op->Nc};
-    const cuuint64_t gstride[1] = {(cuuint64_t)op->Nc * 8};
-    const cuuint32_t box[2] = {32, (cuuint32_t)op->Nc};
-    const cuuint32_t estr[2] = {1, 1};
-    CUresult r = fn(&op->link_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(op->links), gdim, gstride, box,
-                    estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    op->link_map_ok = (r == CUDA_SUCCESS);
-    return COARSE_OK;
-}
-
-template <int NC, int NRHS, bool DAG>
-int launch_tensor_t(const coarse_op* op, const TensorParams& p, cudaStream_t stream) {
-    using Gm = TensorGeom<NC, NRHS>;
-    auto kern = coarse_apply_tensor<NC, NRHS, DAG>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Gm::SMEM_BYTES);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(tensor kernel)");
-    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
-    if (grid > p.n_sites) grid = p.n_sites;
-    kern<<<grid, Gm::THREADS, Gm::SMEM_BYTES, stream>>>(op->link_map, p);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "tensor kernel launch");
-    return COARSE_OK;
-}
-
-template <int NC>
-int launch_tensor_nc(const coarse_op* op, const TensorParams& p, int nrhs, int dagger, cudaStream_t stream) {
-    if (nrhs == 8)
-        return dagger ? launch_tensor_t<NC, 8, true>(op, p, stream) : launch_tensor_t<NC, 8, false>(op, p, stream);
-    return dagger ? launch_tensor_t<NC, 16, true>(op, p, stream) : launch_tensor_t<NC, 16, false>(op, p, stream);
-}
-
-int launch_tensor(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, cudaStream_t stream) {
-    if (!op->link_map_ok) return fail(COARSE_EUNSUPPORTED, "TENSOR path: no tensor map for these links");
-    TensorParams p;
-    p.lat = op->lat;
-    p.links = static_cast<const unsigned char*>(op->links);
-    p.in = static_cast<const float2*>(in);
-    p.out = static_cast<float2*>(out);
-    p.n_sites = op->lat.V;
-    switch (op->Nc) {
-        case 48: return launch_tensor_nc<48>(op, p, nrhs, dagger, stream);
-        case 64: return launch_tensor_nc<64>(op, p, nrhs, dagger, stream);
-        case 128: return launch_tensor_nc<128>(op, p, nrhs, dagger, stream);
-        default: return fail(COARSE_EUNSUPPORTED, "TENSOR path is not compiled for Nc=%d", op->Nc);
     }
 }
 
@@ -532,6 +213,7 @@ coarse_op_t* coarse_op_create(const int dims[4], int Nc, int link_precision) {
     op->keep_opt = 0;
     op->pdl_opt = 0;
     op->split_opt = 0;
+    op->warp_items_opt = 0;
     op->split_ws = nullptr;
     op->split_ws_bytes = 0;
     { int l2 = 0; cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev); op->l2_bytes = l2; }
@@ -626,6 +308,11 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value) {
         case COARSE_OPT_SPLIT_DAGGER:
             if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: split_dagger must be 0 (auto), 1 (never) or 2 (always)");
             op->split_opt = value;
+            return COARSE_OK;
+        case COARSE_OPT_WARP_ITEMS:
+            if (!(value >= 0 && value <= 2) && value != 12 && value != 14)
+                return fail(COARSE_EINVAL, "set_option: warp_items must be 0 (auto), 1 (never), 2 (always) or 12 / 14 (always, 2 / 4 warps per team)");
+            op->warp_items_opt = value;
             return COARSE_OK;
         case COARSE_OPT_PDL:
             if (value != 0 && value != 1) return fail(COARSE_EINVAL, "set_option: pdl must be 0 or 1");
@@ -1086,7 +773,8 @@ int coarse_op_probe_read(const void* src_dev, size_t bytes, int stage_bytes, int
     if (smem > max_smem) return fail(COARSE_EINVAL, "probe_read: %d stages of %d bytes do not fit shared memory", stages, stage_bytes);
     const unsigned long long n_stages = bytes / (size_t)stage_bytes;
     if (n_stages < 1) return fail(COARSE_EINVAL, "probe_read: fewer bytes than one stage");
-    e = cudaFuncSetAttribute(probe_read_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    static SmemAttrCache attr_cache;
+    e = ensure_dynamic_smem(probe_read_kernel, dev, smem, attr_cache);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(probe kernel)");
     const int grid = n_stages < (unsigned long long)sms ? (int)n_stages : sms;
     probe_read_kernel<<<grid, 64, smem, static_cast<cudaStream_t>(stream)>>>(static_cast<const unsigned char*>(src_dev),

@@ -196,7 +196,7 @@ __device__ __forceinline__ float2 unpack_i16x2_xu(uint32_t w) {
 }
 template <int XU>
 __device__ __forceinline__ void unpack_i16_quad(const uint4& t, float2& m0, float2& m1, float2& m2, float2& m3) {
-    m0 = unpack_i16x2(t.x);
+    m0 = XU >= 4 ? unpack_i16x2_xu(t.x) : unpack_i16x2(t.x);
     m1 = XU >= 3 ? unpack_i16x2_xu(t.y) : unpack_i16x2(t.y);
     m2 = XU >= 2 ? unpack_i16x2_xu(t.z) : unpack_i16x2(t.z);
     m3 = XU >= 1 ? unpack_i16x2_xu(t.w) : unpack_i16x2(t.w);

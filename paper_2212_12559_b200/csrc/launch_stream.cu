@@ -1,0 +1,198 @@
+// launch_stream.cu — kernel selection and launch of the 1-RHS STREAM kernels for ONE colour-spin size
+// (compiled once per Nc with -DCOARSE_NC=<Nc>; see internal.h).
+#include "internal.h"
+#include "stream_kernel.cuh"
+#include "stream2_kernel.cuh"
+
+#ifndef COARSE_NC
+#error "compile with -DCOARSE_NC=<Nc>"
+#endif
+
+namespace coarse {
+namespace {
+
+// ---------------------------------------------------------------- STREAM dispatch
+template <int NC, bool I16, bool DAG, bool FINE, bool GEN, bool HV = false>
+int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
+    using Gm = StreamGeom<NC, I16, FINE, HV>;
+    static_assert(Gm::OK, "unsupported STREAM geometry");
+    StreamParams p = base;
+    p.n_items = DAG ? p.n_sites : p.n_sites * Gm::NB;
+    if (base.n_items > 0) {                       // a site range [item_begin, n_items) was requested (in sites)
+        p.item_begin = DAG ? base.item_begin : base.item_begin * Gm::NB;
+        p.n_items = DAG ? base.n_items : base.n_items * Gm::NB;
+    }
+    // dagger = 1 has one work item per site; on a lattice with fewer sites than SMs (the paper's level 3:
+    // 32 sites per GPU) the contraction of a site is split over its NB row chunks, one item each, and a
+    // small second kernel adds the NB partial vectors in order.
+    p.split = 0;
+    p.partial = nullptr;
+    if (DAG && !GEN && !HV && base.n_items == 0 && Gm::NB > 1 && op->split_ws &&
+        (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes &&
+        (op->split_opt == 2 || (op->split_opt == 0 && p.n_sites < op->num_sms))) {
+        p.split = 1;
+        p.partial = op->split_ws;
+        p.n_items = p.n_sites * Gm::NB;
+    }
+    int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (Gm::stage_bytes(DAG) + 16);
+    if (stages > 12) stages = 12;
+    if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM: shared memory too small for Nc=%d", NC);
+    // Default depth: ~112 KB in flight per SM (the measured optimum, see stream_kernel.cuh), at
+    // least 4 stages; COARSE_OPT_STAGES overrides.
+    int want = (114688 + Gm::stage_bytes(DAG) / 2) / Gm::stage_bytes(DAG);
+    if (want < 4) want = 4;
+    if (op->stages_opt > 0) want = op->stages_opt;
+    if (stages > want) stages = want;
+    p.stages = stages;
+    int smem = Gm::smem_bytes(DAG, stages);
+    // PDL: a kernel whose shared-memory carve-out differs from its predecessor's cannot take over an SM
+    // before it has drained completely (measured: an alternating dagger 0 / dagger 1 chain gained nothing
+    // until both kernels asked for the same size), so under PDL both modes request the larger of the two.
+    if (op->pdl_opt && Gm::smem_bytes(!DAG, stages) > smem && Gm::smem_bytes(!DAG, stages) <= op->max_smem)
+        smem = Gm::smem_bytes(!DAG, stages);
+    auto kern = coarse_apply_stream<NC, I16, DAG, FINE, GEN, HV>;
+    static SmemAttrCache attr_cache;
+    cudaError_t e = ensure_dynamic_smem(kern, op->device, smem, attr_cache);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
+    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
+    if (grid > p.n_items - p.item_begin) grid = p.n_items - p.item_begin;
+    if (grid < 1) return COARSE_OK;
+    p.pdl = op->pdl_opt ? 1 : 0;
+    if (p.pdl) {
+        // programmatic dependent launch: this kernel may start while the previous kernel of the stream
+        // drains; it orders itself against that kernel's memory with griddepcontrol.wait (stream_kernel.cuh)
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid);
+        cfg.blockDim = dim3(Gm::THREADS);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, kern, p);
+        if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch (PDL)");
+    } else {
+        kern<<<grid, Gm::THREADS, smem, stream>>>(p);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch");
+    }
+    if (p.split) {
+        const long long tot = (long long)p.n_sites * NC;
+        coarse_dagger_reduce_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(p.partial, p.n_sites, Gm::NB, NC, p.out);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "dagger reduce kernel launch");
+        return 1;      // one extra launch (coarse_op_apply adds it to last_launches)
+    }
+    return COARSE_OK;
+}
+
+// Team-owned stages (stream2_kernel.cuh): plain apply on the whole lattice, no PDL.
+template <int NC, bool I16, bool DAG, int TW>
+int launch_stream2_w(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
+    using Gm = Stream2Geom<NC, I16, TW>;
+    if constexpr (!Gm::OK) {
+        return fail(COARSE_EUNSUPPORTED, "STREAM (warp teams): no geometry for Nc=%d with %d warps per team", NC, TW);
+    } else {
+        StreamParams p = base;
+        p.n_items = DAG ? p.n_sites : p.n_sites * Gm::NB;
+        p.item_begin = 0;
+        // ring: one slot per team being read + ~104 KB in flight (the measured optimum of the read stream),
+        // a multiple of the team count so that every slot has a fixed owner; COARSE_OPT_STAGES overrides
+        const int sb = Gm::stage_bytes(DAG);
+        int slots = Gm::T + (106496 + sb / 2) / sb;
+        if (op->stages_opt > 0) slots = op->stages_opt;
+        const int fit = (op->max_smem - Gm::fixed_bytes(DAG)) / (sb + 16);
+        if (slots > fit) slots = fit;
+        slots = (slots + Gm::T / 2) / Gm::T * Gm::T;
+        if (slots > fit) slots -= Gm::T;
+        if (slots < 2 * Gm::T) slots = 2 * Gm::T;
+        if (slots > fit) return fail(COARSE_EUNSUPPORTED, "STREAM (warp teams): shared memory too small for Nc=%d", NC);
+        p.stages = slots;
+        const int smem = Gm::smem_bytes(DAG, slots);
+        auto kern = coarse_apply_stream2<NC, I16, DAG, TW>;
+        static SmemAttrCache attr_cache;
+        cudaError_t e = ensure_dynamic_smem(kern, op->device, smem, attr_cache);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream2 kernel)");
+        int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
+        const int need = (p.n_items + Gm::T - 1) / Gm::T;
+        if (grid > need) grid = need;
+        if (grid < 1) return COARSE_OK;
+        kern<<<grid, Gm::THREADS, smem, stream>>>(p);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "stream2 kernel launch");
+        return COARSE_OK;
+    }
+}
+
+// COARSE_OPT_WARP_ITEMS: 2 = default team width (4 warps: two teams; measured best on C4 and P2, where
+// its default ring of 8 slots has the 6 x 16 KB in flight the read stream peaks at), 12 / 14 = 2 / 4 warps
+template <int NC, bool I16, bool DAG>
+int launch_stream2_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
+    // rows of 24 / 48 quads (Nc = 96 / 192 int16) run best with 2 warps per team (measured: Nc 96 6.6 / 6.8 TB/s
+    // against 6.0 / 6.7 with 4 and 5.4 / 5.4 on the cooperative kernel), the others with 4
+    const bool two = op->warp_items_opt == 12 || (op->warp_items_opt != 14 && NC % 3 == 0);
+    if (two) return launch_stream2_w<NC, I16, DAG, 2>(op, base, stream);
+    return launch_stream2_w<NC, I16, DAG, 4>(op, base, stream);
+}
+
+template <int NC, bool I16>
+bool use_warp_items(const coarse_op* op, const StreamParams& p, int dagger, bool gen) {
+    if (gen || p.vnorms || p.n_items > 0 || op->pdl_opt || op->warp_items_opt == 1) return false;
+    if (op->warp_items_opt >= 2) return true;
+    const int64_t items = dagger ? (int64_t)p.n_sites : (int64_t)p.n_sites * Stream2Geom<NC, I16, 4>::NB;
+    return I16 && NC >= 64 && items >= (int64_t)4 * Stream2Geom<NC, I16, 4>::T * op->num_sms;
+}
+
+// dagger = 0 on a tiny lattice: switch to the fine row-block geometry when the regular one gives
+// fewer work items than SMs (COARSE_OPT_FINE: 0 auto, 1 never, 2 always).  Measured on C1
+// (256 sites, Nc = 48: 256 regular items on 148 SMs) the regular geometry is 2.8x faster (5.6 us
+// vs 15.4 us warm): 3 KB stages pay the per-stage handshake 6x more often, so the fine split only
+// pays when SMs would otherwise sit idle.
+template <int NC, bool I16, bool GEN>
+int launch_stream_n(const coarse_op* op, const StreamParams& p, cudaStream_t stream) {
+    constexpr bool HAS_FINE = StreamGeom<NC, I16, true>::NB > StreamGeom<NC, I16, false>::NB;
+    if constexpr (HAS_FINE) {
+        const bool few = (int64_t)p.n_sites * StreamGeom<NC, I16, false>::NB < (int64_t)op->num_sms;
+        if (op->fine_opt == 2 || (op->fine_opt == 0 && few)) return launch_stream_t<NC, I16, false, true, GEN>(op, p, stream);
+    }
+    return launch_stream_t<NC, I16, false, false, GEN>(op, p, stream);
+}
+
+template <int NC, bool GEN>
+int launch_stream_nc(const coarse_op* op, const StreamParams& p, int dagger, cudaStream_t stream) {
+    if (op->prec == COARSE_LINK_I16)
+        return dagger ? launch_stream_t<NC, true, true, false, GEN>(op, p, stream) : launch_stream_n<NC, true, GEN>(op, p, stream);
+    return dagger ? launch_stream_t<NC, false, true, false, GEN>(op, p, stream) : launch_stream_n<NC, false, GEN>(op, p, stream);
+}
+
+template <int NC>
+int launch_stream_g(const coarse_op* op, const StreamParams& p, int dagger, bool gen, cudaStream_t stream) {
+    if (p.vnorms) {   // half-precision input vectors: regular geometry, plain apply
+        if (op->prec == COARSE_LINK_I16)
+            return dagger ? launch_stream_t<NC, true, true, false, false, true>(op, p, stream)
+                          : launch_stream_t<NC, true, false, false, false, true>(op, p, stream);
+        return dagger ? launch_stream_t<NC, false, true, false, false, true>(op, p, stream)
+                      : launch_stream_t<NC, false, false, false, false, true>(op, p, stream);
+    }
+    if (op->prec == COARSE_LINK_I16) {
+        if constexpr (Stream2Geom<NC, true, 4>::OK)
+            if (use_warp_items<NC, true>(op, p, dagger, gen))
+                return dagger ? launch_stream2_t<NC, true, true>(op, p, stream) : launch_stream2_t<NC, true, false>(op, p, stream);
+    } else {
+        if constexpr (Stream2Geom<NC, false, 4>::OK)
+            if (use_warp_items<NC, false>(op, p, dagger, gen))
+                return dagger ? launch_stream2_t<NC, false, true>(op, p, stream) : launch_stream2_t<NC, false, false>(op, p, stream);
+    }
+    return gen ? launch_stream_nc<NC, true>(op, p, dagger, stream) : launch_stream_nc<NC, false>(op, p, dagger, stream);
+}
+
+}  // namespace
+
+int COARSE_CAT(launch_stream_nc, COARSE_NC)(const coarse_op* op, const StreamParams& p, int dagger, bool gen,
+                                            cudaStream_t stream) {
+    return launch_stream_g<COARSE_NC>(op, p, dagger, gen, stream);
+}
+
+}  // namespace coarse

@@ -1,0 +1,63 @@
+// launch_stream_mr.cu — launch of the 2-4 RHS STREAM-MR kernels for ONE colour-spin size (-DCOARSE_NC=<Nc>).
+#include "internal.h"
+#include "stream_mr_kernel.cuh"
+
+#ifndef COARSE_NC
+#error "compile with -DCOARSE_NC=<Nc>"
+#endif
+
+namespace coarse {
+namespace {
+
+// ---------------------------------------------------------------- STREAM-MR dispatch (2 <= nrhs <= 4)
+template <int NC, bool I16, bool DAG, int R>
+int launch_stream_mr_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
+    using Gm = StreamGeom<NC, I16, false, false, true>;
+    using Gr = StreamMrGeom<NC, I16, R>;
+    StreamParams p = base;
+    p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
+    int stages = (op->max_smem - Gr::fixed_bytes(DAG)) / (Gr::stage_bytes(DAG) + 16);
+    if (stages > 12) stages = 12;
+    if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM-MR: shared memory too small for Nc=%d nrhs=%d", NC, R);
+    int want = (114688 + Gr::stage_bytes(DAG) / 2) / Gr::stage_bytes(DAG);
+    if (want < 4) want = 4;
+    if (op->stages_opt > 0) want = op->stages_opt;
+    if (stages > want) stages = want;
+    p.stages = stages;
+    const int smem = Gr::smem_bytes(DAG, stages);
+    auto kern = coarse_apply_stream_mr<NC, I16, DAG, R>;
+    static SmemAttrCache attr_cache;
+    cudaError_t e = ensure_dynamic_smem(kern, op->device, smem, attr_cache);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream-mr kernel)");
+    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
+    if (grid > p.n_items) grid = p.n_items;
+    kern<<<grid, Gm::THREADS, smem, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "stream-mr kernel launch");
+    return COARSE_OK;
+}
+
+template <int NC, int R>
+int launch_stream_mr_r(const coarse_op* op, const StreamParams& p, int dagger, cudaStream_t stream) {
+    if (op->prec == COARSE_LINK_I16)
+        return dagger ? launch_stream_mr_t<NC, true, true, R>(op, p, stream) : launch_stream_mr_t<NC, true, false, R>(op, p, stream);
+    return dagger ? launch_stream_mr_t<NC, false, true, R>(op, p, stream) : launch_stream_mr_t<NC, false, false, R>(op, p, stream);
+}
+
+template <int NC>
+int launch_stream_mr_nc(const coarse_op* op, const StreamParams& p, int nrhs, int dagger, cudaStream_t stream) {
+    switch (nrhs) {
+        case 2: return launch_stream_mr_r<NC, 2>(op, p, dagger, stream);
+        case 3: return launch_stream_mr_r<NC, 3>(op, p, dagger, stream);
+        default: return launch_stream_mr_r<NC, 4>(op, p, dagger, stream);
+    }
+}
+
+}  // namespace
+
+int COARSE_CAT(launch_stream_mr_nc, COARSE_NC)(const coarse_op* op, const StreamParams& p, int nrhs, int dagger,
+                                               cudaStream_t stream) {
+    return launch_stream_mr_nc<COARSE_NC>(op, p, nrhs, dagger, stream);
+}
+
+}  // namespace coarse

@@ -460,8 +460,9 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
     }
 }
 
-// out[s][t] = sum_c partial[s*nb + c][t], chunks added in order (deterministic)
-__global__ void __launch_bounds__(256) coarse_dagger_reduce_kernel(const float2* partial, int n_sites, int nb, int nc, float2* out) {
+// out[s][t] = sum_c partial[s*nb + c][t], chunks added in order (deterministic).  static: this header is
+// compiled into one translation unit per Nc.
+static __global__ void __launch_bounds__(256) coarse_dagger_reduce_kernel(const float2* partial, int n_sites, int nb, int nc, float2* out) {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long long)n_sites * nc) return;
     const long long s = idx / nc;

@@ -82,6 +82,31 @@ def test_stream_path_single_rhs(oracle_lib, dims, Nc, prec, dagger):
     _run(oracle_lib, dims, Nc, prec, 1, dagger, cop.PATH_STREAM)
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (1, 1, 1, 1), (5, 3, 4, 7)])
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("dagger", [0, 1])
+@pytest.mark.parametrize("team", [12, 14])
+def test_stream_warp_teams_single_rhs(oracle_lib, dims, Nc, prec, dagger, team):
+    """The team-owned-stages STREAM variant (csrc/stream2_kernel.cuh), forced on every shape with 2 and 4
+    warps per team: ragged item counts (fewer items than teams, ragged last round), extents 1 and 2,
+    arbitrary links."""
+    if Nc >= 128 and dims == (5, 3, 4, 7):
+        dims = (5, 3, 2, 3)
+    _run(oracle_lib, dims, Nc, prec, 1, dagger, cop.PATH_STREAM, opts={cop.OPT_WARP_ITEMS: team}, hermitian=False)
+
+
+@pytest.mark.parametrize("grid,stages", [(1, 4), (3, 9), (2, 16), (1000, 0)])
+def test_stream_warp_teams_any_grid(oracle_lib, grid, stages):
+    """Many rounds per CTA (the multi-round ring bookkeeping), every ring depth the host may pick."""
+    for dagger in (0, 1):
+        for Nc, prec, team in ((64, cop.LINK_I16, 12), (48, cop.LINK_C64, 14), (192, cop.LINK_I16, 14), (128, cop.LINK_I16, 2)):
+            opts = {cop.OPT_WARP_ITEMS: team}
+            if stages:
+                opts[cop.OPT_STAGES] = stages
+            _run(oracle_lib, (5, 3, 2, 3), Nc, prec, 1, dagger, cop.PATH_STREAM, grid=grid, opts=opts)
+
+
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (1, 1, 1, 1)])
 @pytest.mark.parametrize("Nc", [6, 8, 48, 64])
 @pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
