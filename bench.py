@@ -42,16 +42,23 @@ import synth
 METRIC = "coarse-op site-updates/s"
 UNIT = "site-updates/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-# `ncu --set full` captures summarised under profiles/r01_ncu_full_*.md, keyed by
-# (config, path actually run, dagger); None for combinations that were not captured.
-NCU_TRAFFIC_BYTES = {
-    ("C2", 2, 0): 16361995008, ("C2", 2, 1): 16367453696,
-    ("C3", 2, 0): 7260217344, ("C3", 2, 1): 7261264896,
-    ("C4", 2, 0): 14580726784, ("C4", 2, 1): 14584525824,
-    ("C5", 3, 0): 7481073920, ("C5", 3, 1): 7441391616,
-    ("C5", 4, 0): 7447821312, ("C5", 4, 1): 7443588096,
-}
+def ncu_traffic_bytes(config: str, path: int, dagger: int, links: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, read from the newest
+    `profiles/r*_ncu_traffic.csv` (written by `python -m paper_2212_12559_b200.ncu_summary` from the
+    `ncu --set full` captures summarised beside it); None when that launch was not captured."""
+    import csv
+    import glob
+    best = None
+    for fn in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_ncu_traffic.csv"))):
+        try:
+            with open(fn) as f:
+                for row in csv.DictReader(f):
+                    if (row["config"] == config and int(row["path"]) == path and int(row["dagger"]) == dagger
+                            and row["links"] == links):
+                        best = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+        except Exception:
+            continue
+    return best
 
 
 def compulsory_bytes_per_site(Nc: int, links: str, nrhs: int, hvec: bool = False) -> int:
@@ -173,12 +180,12 @@ def oracle_sample_dims(cfg):
     d = list(cfg["dims"])
     per_site = 9 * cfg["Nc"] ** 2 * cfg["nrhs"]
     budget = 4.0e7 * 1.0            # complex MACs per apply (~0.05-0.5 s on 8-64 host cores)
-    while d[0] * d[1] * d[2] * d[3] * per_site > budget and d[3] > 2:
-        d[3] = max(2, d[3] // 2)
-    while d[0] * d[1] * d[2] * d[3] * per_site > budget and d[2] > 2:
-        d[2] = max(2, d[2] // 2)
-    while d[0] * d[1] * d[2] * d[3] * per_site > budget and d[1] > 2:
-        d[1] = max(2, d[1] // 2)
+    # halve the currently LONGEST extent (last index first) while over budget: extents stay >= 4 as long as
+    # possible, so x+mu and x-mu remain distinct sites as in the workload (two extent-2 directions would be
+    # friendlier to the CPU caches than the real lattice)
+    while d[0] * d[1] * d[2] * d[3] * per_site > budget and max(d) > 2:
+        mu = max(range(4), key=lambda k: (d[k], k))
+        d[mu] = max(2, d[mu] // 2)
     return tuple(d)
 
 
@@ -195,30 +202,30 @@ def make_oracle_sample(cfg, device):
     return dims, links, scales, prec, vin
 
 
-def oracle_step(sample, cfg, daggers):
+def oracle_step(sample, cfg, daggers, nthreads=0):
     import oracle
     dims, links, scales, prec, vin = sample
     for dg in daggers:
         oracle.coarse_apply(dims, cfg["Nc"], links, vin, nrhs=cfg["nrhs"], dagger=dg,
-                            link_precision=prec, scales=scales)
+                            link_precision=prec, scales=scales, nthreads=nthreads)
 
 
-def time_oracle(cfg, daggers, device, min_seconds=10.0, max_steps=100000):
+def time_oracle(cfg, daggers, device, min_seconds=10.0, max_steps=100000, nthreads=0):
     import oracle
     oracle.build()
     sample = make_oracle_sample(cfg, device)
     V = synth.lattice_volume(sample[0])
-    oracle_step(sample, cfg, daggers)                      # warm-up (page-in, thread pool)
+    oracle_step(sample, cfg, daggers, nthreads)            # warm-up (page-in, thread pool)
     t0 = time.perf_counter()
     n = 0
     while n < max_steps and (time.perf_counter() - t0 < min_seconds or n < 3):
-        oracle_step(sample, cfg, daggers)
+        oracle_step(sample, cfg, daggers, nthreads)
         n += 1
     dt = time.perf_counter() - t0
     return {
         "value": V * len(daggers) * n / dt,
         "unit": UNIT,
-        "cores": oracle.max_threads(),
+        "cores": nthreads if nthreads > 0 else oracle.max_threads(),
         "kind": "oracle",
         "sample": f"{n} steps on a {'x'.join(map(str, sample[0]))} slab of the workload lattice "
                   f"({V} sites, same Nc/links/nrhs/generator, periodic on its own), {dt:.1f} s of CPU time",
@@ -265,6 +272,150 @@ def workload_name(name, cfg, hvec=False):
             f"nrhs={cfg['nrhs']}")
 
 
+# ------------------------------------------------------------------------------- in-run parity
+def parity_sample_sites(dims, n_random, seed):
+    """Corners, first/last sites and seeded random sites of the lattice (sorted, unique)."""
+    L0, L1, L2, L3 = dims
+    V = L0 * L1 * L2 * L3
+    pts = [0, 1 % V, V - 2 if V > 1 else 0, V - 1]
+    for x3 in (0, L3 - 1):
+        for x2 in (0, L2 - 1):
+            for x1 in (0, L1 - 1):
+                for x0 in (0, L0 - 1):
+                    pts.append(x0 + L0 * (x1 + L1 * (x2 + L2 * x3)))
+    rnd = np.random.default_rng(seed).integers(0, V, size=n_random)
+    return np.unique(np.concatenate([np.asarray(pts, dtype=np.int64), rnd])).astype(np.int64)
+
+
+def parity_check(cfg, links, scales, vin, outs, n_random=64):
+    """"parity is checked in the same run, before timing, on the same buffers".  The device
+    buffers the timed loop is about to use hold one apply per dagger; the CPU oracle (its per-site
+    evaluation, `oracle.coarse_apply_sites`) recomputes >= 64 sampled output sites from the links and
+    vectors those sites touch.  Returns the worst relative L2 error over daggers and right-hand sides.
+    (Part of the oracle legs of this script, like cpu_baseline: the product path never calls it.)"""
+    import oracle
+    oracle.build()
+    dims, Nc, nrhs = cfg["dims"], cfg["Nc"], cfg["nrhs"]
+    V = synth.lattice_volume(dims)
+    i16 = cfg["links"] == "i16"
+    sites = parity_sample_sites(dims, n_random, cfg["seed"])
+    need = np.unique(np.concatenate([oracle.neighbours(dims, int(s)) for s in sites]))
+    flat = links if i16 else torch.view_as_real(links)
+    links_h = np.empty((V, 9, Nc, Nc, 2), dtype=np.int16 if i16 else np.float32)   # only the needed sites are touched
+    idx = torch.as_tensor(need, device=flat.device)
+    links_h[need] = flat[idx].cpu().numpy().reshape(len(need), 9, Nc, Nc, 2)
+    scales_h = None if scales is None else scales.cpu().numpy()
+    vin_h = vin.cpu().numpy()
+    worst, worst_site = 0.0, 0.0
+    sidx = torch.as_tensor(sites, device=flat.device)
+    for dg, out in outs.items():
+        ref = oracle.coarse_apply_sites(dims, Nc, links_h, vin_h, sites, nrhs=nrhs, dagger=dg,
+                                        link_precision=oracle.LINK_I16 if i16 else oracle.LINK_C64, scales=scales_h)
+        got = out[sidx].cpu().numpy().astype(np.complex128)
+        for r in range(nrhs):
+            worst = max(worst, float(np.linalg.norm(got[..., r] - ref[..., r]) / np.linalg.norm(ref[..., r])))
+        per_site = np.linalg.norm((got - ref).reshape(len(sites), -1), axis=1) / np.linalg.norm(ref.reshape(len(sites), -1), axis=1)
+        worst_site = max(worst_site, float(per_site.max()))
+    return {"rel_l2": worst, "worst_site_rel_l2": worst_site, "sites": int(len(sites)), "tolerance": 1e-5,
+            "ok": bool(worst <= 1e-5 and worst_site <= 5e-5)}
+
+
+def measure_config(name, steps, local, dev, read_ceiling=None):
+    """One BASELINE config on the AUTO path: in-run parity on sampled sites, then `steps` applies per dagger
+    timed with CUDA events (L2-resident lattices: one CUDA graph per dagger, warm, plus a cold number over
+    rotating link copies).  Sub-record of the default bench line (`configs`)."""
+    import paper_2212_12559_b200 as cop
+    cfg = synth.config(name)
+    dims, Nc, nrhs = cfg["dims"], cfg["Nc"], cfg["nrhs"]
+    V = synth.lattice_volume(dims)
+    prec = cop.LINK_I16 if cfg["links"] == "i16" else cop.LINK_C64
+    links = synth.make_gamma_hermitian_links(dims, Nc, cfg["seed"], device=dev)
+    scales = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device=dev)
+        scales = torch.empty((V, 9), dtype=torch.float32, device=dev)
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        torch.cuda.synchronize()
+        links = q
+    vin = synth.make_vectors(dims, Nc, nrhs, cfg["seed"] + 1, device=dev)
+    outs = {dg: torch.full_like(vin, float("nan")) for dg in (0, 1)}
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    stream = torch.cuda.current_stream()
+    for dg in (0, 1):
+        op.apply(vin, outs[dg], nrhs=nrhs, dagger=dg)
+    torch.cuda.synchronize()
+    path = op.last_path
+    parity = parity_check(cfg, links, scales, vin, outs)
+    link_bytes = links.numel() * links.element_size()
+    l2_bytes = torch.cuda.get_device_properties(dev).L2_cache_size
+    bps = compulsory_bytes_per_site(Nc, cfg["links"], nrhs)
+    peak, _ = measured_peak_gbs()
+    rec = {"workload": workload_name(name, cfg), "path": path, "steps": steps, "parity": parity,
+           "algorithmic_bytes_per_launch": bps * V}
+
+    def graph_of(fn):
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.graph(g, stream=side):
+            fn()
+        torch.cuda.current_stream().wait_stream(side)
+        g.replay()
+        torch.cuda.synchronize()
+        return g
+
+    def time_graph(g):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        g.replay()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b)
+
+    with ClockSampler(local) as clocks:
+        if link_bytes <= 2 * l2_bytes:
+            reps = max(steps, 50)
+            warm = {dg: time_graph(graph_of(lambda dg=dg: [op.apply(vin, outs[dg], nrhs=nrhs, dagger=dg) for _ in range(reps)])) / reps
+                    for dg in (0, 1)}
+            n_copies = int(3 * l2_bytes // max(1, link_bytes)) + 2
+            copies = [(links.clone(), None if scales is None else scales.clone()) for _ in range(n_copies)]
+            ops = [cop.CoarseOp(dims, Nc, prec).set_links(l, sc).set_option(cop.OPT_KEEP_LINKS, 1) for l, sc in copies]
+            creps = max(reps, 2 * n_copies)
+            ms = {dg: time_graph(graph_of(lambda dg=dg: [ops[r % n_copies].apply(vin, outs[dg], nrhs=nrhs, dagger=dg)
+                                                         for r in range(creps)])) / creps for dg in (0, 1)}
+            for o in ops:
+                o.close()
+            del ops, copies
+            rec["timing"] = "CUDA graph of %d applies per dagger; ms = COLD (links rotated over %d copies > L2), warm-L2 beside" % (creps, n_copies)
+            rec["warm_l2_ms"] = {str(dg): warm[dg] for dg in (0, 1)}
+        else:
+            for _ in range(3):
+                for dg in (0, 1):
+                    op.apply(vin, outs[dg], nrhs=nrhs, dagger=dg)
+            ev = {dg: [] for dg in (0, 1)}
+            for _ in range(steps):
+                for dg in (0, 1):
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream)
+                    op.apply(vin, outs[dg], nrhs=nrhs, dagger=dg)
+                    b.record(stream)
+                    ev[dg].append((a, b))
+            torch.cuda.synchronize()
+            ms = {dg: sum(a.elapsed_time(b) for a, b in ev[dg]) / steps for dg in (0, 1)}
+            rec["timing"] = "CUDA events around each of %d applies per dagger (dagger 0 / 1 alternating), mean" % steps
+    rec["ms"] = {str(dg): ms[dg] for dg in (0, 1)}
+    rec["gbs"] = {str(dg): bps * V / (ms[dg] * 1e-3) / 1e9 for dg in (0, 1)}
+    rec["frac"] = {str(dg): rec["gbs"][str(dg)] / peak for dg in (0, 1)}
+    rec["frac_of_nominal_8000"] = {str(dg): rec["gbs"][str(dg)] / 8000.0 for dg in (0, 1)}
+    if read_ceiling:
+        rec["frac_of_read_ceiling"] = {str(dg): rec["gbs"][str(dg)] / read_ceiling for dg in (0, 1)}
+    rec["msite_updates_per_s"] = {str(dg): V / (ms[dg] * 1e-3) / 1e6 for dg in (0, 1)}
+    rec["clocks"] = clocks.summary()
+    rec["traffic"] = {str(dg): ncu_traffic_bytes(name, path, dg, cfg["links"]) for dg in (0, 1)}
+    op.close()
+    return rec
+
+
 # ------------------------------------------------------------------------------- GPU arm
 def run_ours(args, cfg, daggers):
     import paper_2212_12559_b200 as cop
@@ -290,6 +441,7 @@ def run_ours(args, cfg, daggers):
         cop.coarse_op_quantize_i16(links, Nc, q, scales)
         torch.cuda.synchronize()
         links = q
+        del q
     vin = synth.make_vectors(dims, Nc, nrhs, cfg["seed"] + 1, device=dev)
     vouts = [torch.empty_like(vin) for _ in daggers]
     op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
@@ -366,6 +518,13 @@ def run_ours(args, cfg, daggers):
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
+    # parity in the same run, before timing, on the buffers the timed loop writes
+    parity = None
+    if rank == 0 and not args.hvec and not args.no_parity:
+        parity = parity_check(cfg, links, scales, vin, {dg: vouts[k] for k, dg in enumerate(daggers)})
+        if not parity["ok"]:
+            raise RuntimeError("bench.py: the GPU result does not match the CPU oracle on the sampled sites: %r" % (parity,))
+    barrier()
     cold = None
     if use_graph:
         launches = 0
@@ -463,7 +622,7 @@ def run_ours(args, cfg, daggers):
     achieved = bps * V / (kernel_ms[dom] * 1e-3) / 1e9
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": None if args.hvec else NCU_TRAFFIC_BYTES.get((args.config, op.last_path, dom)),
+        "traffic": None if args.hvec else ncu_traffic_bytes(args.config, op.last_path, dom, cfg["links"]),
         "kernel": "coarse_apply_%s<Nc=%d,%s,dagger=%d%s>" % (
             {cop.PATH_SIMPLE: "simple", cop.PATH_STREAM: "stream", cop.PATH_TENSOR: "tensor",
              cop.PATH_BLOCK: "block"}.get(op.last_path, "?"), Nc, "i16" if prec else "c64", dom,
@@ -515,12 +674,27 @@ def run_ours(args, cfg, daggers):
         "gpu_launches": gpu_launches,
         "roofline": roofline,
     }
-    if world == 1 and not args.no_cpu_baseline:
-        op.close()
-        del links, vin, vouts
-        line["cpu_baseline"] = time_oracle(cfg, daggers, dev, min_seconds=args.cpu_seconds)
-    print(json.dumps(line), flush=True)
+    if parity is not None:
+        line["parity"] = parity
     op.close()
+    del links, vin, vouts, op
+    if scales is not None:
+        del scales
+    torch.cuda.empty_cache()
+    # The other BASELINE configs as sub-records of the default line (the driver runs one line): AUTO path,
+    # in-run parity, 20 applies per dagger each.  Their launches are not part of `gpu_launches`/`value`.
+    if world == 1 and args.all_configs and args.config == "C2" and not args.hvec:
+        line["configs"] = {}
+        for name in ("C1", "C3", "C4", "C5"):
+            line["configs"][name] = measure_config(name, args.config_steps, local, dev, read_ceiling)
+            torch.cuda.empty_cache()
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = time_oracle(cfg, daggers, dev, min_seconds=args.cpu_seconds)
+        if args.all_configs and args.config == "C2":
+            # "plus a 1-thread number on C1 and C3"
+            line["cpu_baseline"]["one_thread"] = {
+                name: time_oracle(synth.config(name), daggers, dev, min_seconds=2.0, nthreads=1) for name in ("C1", "C3")}
+    print(json.dumps(line), flush=True)
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
@@ -691,6 +865,10 @@ def main():
     ap.add_argument("--hvec", action="store_true",
                     help="half-precision INPUT vectors (int16 + per-site norm, row f2) through coarse_op_apply_hvec")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-parity", action="store_true", help="skip the in-run oracle comparison of sampled sites")
+    ap.add_argument("--no-all-configs", dest="all_configs", action="store_false",
+                    help="default C2 line only: do not attach the C1/C3/C4/C5 sub-records")
+    ap.add_argument("--config-steps", type=int, default=20, help="applies per dagger for each sub-record")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     args = ap.parse_args()
     cfg = synth.config(args.config)

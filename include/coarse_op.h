@@ -30,9 +30,14 @@
  *   vectors         v[s][a][r], float[2] = (re,im), a in [0,Nc) colour-spin (a = chi*N_vec + k),
  *                   r in [0,nrhs) innermost.
  *
- * OWNERSHIP  The handle owns metadata, (only if coarse_op_apply_host is used) two vector-sized
- *   staging buffers, and on lattices with fewer sites than SMs a few-MB workspace for the split dagger apply.  Link, scale, in and out buffers are the caller's; coarse_op_set_links borrows
- *   the pointers, which must stay valid and unchanged until destroy or the next set_links.
+ * OWNERSHIP  Link, scale, in and out buffers are the caller's.  coarse_op_set_links borrows the link and
+ *   scale pointers, which must stay valid and unchanged until destroy or the next set_links.  The handle
+ *   owns its metadata and two kinds of device scratch: two vector-sized staging buffers plus two copy
+ *   streams (only if coarse_op_apply_host is used), and, on lattices with fewer sites than SMs, a few-MB
+ *   workspace for the split dagger apply.  Because of that scratch a handle may have work in flight on
+ *   ONE stream at a time; use one handle per stream for concurrent solves on the same links (handles
+ *   are cheap and may share link buffers).  A handle belongs to the device that was current in
+ *   coarse_op_create; calls made with another device current return COARSE_EINVAL.
  *
  * ERRORS  int-returning calls return COARSE_OK (0) or a negative code; coarse_op_create returns
  *   NULL.  coarse_op_last_error() gives a thread-local message.  No exception crosses the ABI.
@@ -131,7 +136,10 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
  *
  * and for dagger = 1 the same split of the adjoint (X(x)^H.u(x) and the adjoint hop of
  * coarse_op_apply).  Sites of the other parity are NOT written.  u_dev may be NULL for
- * COARSE_LOCAL_NONE and may alias out_dev (it is read at x only); w_dev must not overlap out_dev.
+ * COARSE_LOCAL_NONE.  Aliasing: w_dev must never overlap out_dev (the stencil reads neighbours).  With
+ * COARSE_LOCAL_IDENTITY u_dev may be the SAME pointer as out_dev (in place: every output element reads
+ * only its own u element first); a partial overlap, or any overlap with COARSE_LOCAL_X (X.u reads all of
+ * u(x) while other work items write out(x)), returns COARSE_EINVAL.
  * COARSE_PARITY_EVEN/ODD need every extent even (COARSE_EINVAL otherwise).
  * Examples (hat = an operator whose links are Yhat_m = X^{-1} Y_m):
  *     t_o   = Dhat_oe v_e           : apply_parts(hat, NULL, v, t, .., COARSE_PARITY_ODD, COARSE_LOCAL_NONE, 0, 1)

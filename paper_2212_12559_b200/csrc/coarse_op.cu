@@ -44,6 +44,22 @@ namespace {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
+    const uintptr_t x = reinterpret_cast<uintptr_t>(a), y = reinterpret_cast<uintptr_t>(b);
+    return x < y + nb && y < x + na;
+}
+
+// The handle belongs to the device that was current in coarse_op_create: launches and allocations made
+// with another device current would go to the wrong GPU with this one's pointers.
+int check_device(const coarse_op* op, const char* who) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (dev != op->device)
+        return fail(COARSE_EINVAL, "%s: the handle was created on device %d but device %d is current", who, op->device, dev);
+    return COARSE_OK;
+}
+
 }  // namespace
 
 namespace {
@@ -162,7 +178,7 @@ int check_apply_args(const coarse_op* op, const void* in, const void* out, int n
     if (!in || !out) return fail(COARSE_EINVAL, "apply: in/out is NULL");
     if (nrhs < 1) return fail(COARSE_EINVAL, "apply: nrhs must be >= 1 (got %d)", nrhs);
     if (dagger != 0 && dagger != 1) return fail(COARSE_EINVAL, "apply: dagger must be 0 or 1 (got %d)", dagger);
-    return COARSE_OK;
+    return check_device(op, "apply");
 }
 
 }  // namespace
@@ -250,6 +266,7 @@ int coarse_op_set_links(coarse_op_t* op, const void* links_dev, const float* sca
     if (!op) return fail(COARSE_EINVAL, "set_links: op is NULL");
     if (!links_dev) return fail(COARSE_EINVAL, "set_links: links_dev is NULL");
     if (!aligned16(links_dev)) return fail(COARSE_EINVAL, "set_links: links_dev must be 16-byte aligned");
+    { int rc = check_device(op, "set_links"); if (rc != COARSE_OK) return rc; }
     if (op->prec == COARSE_LINK_I16) {
         if (!scales_dev) return fail(COARSE_EINVAL, "set_links: I16 links need scales_dev");
         if ((reinterpret_cast<uintptr_t>(scales_dev) & 3u) != 0)
@@ -384,9 +401,17 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
     const uintptr_t b = reinterpret_cast<uintptr_t>(out_dev);
     const uintptr_t a = reinterpret_cast<uintptr_t>(w_dev);
     // w is read at neighbours: it may share a buffer with out only when the two parities are disjoint,
-    // which the caller cannot express here, so overlap is always refused; u is read at x only and
-    // may alias out.
+    // which the caller cannot express here, so overlap is always refused.
     if (a < b + vb && b < a + vb) return fail(COARSE_EINVAL, "apply_parts: w and out overlap (the stencil reads neighbours)");
+    // u: with the identity local term every output element reads exactly its own u element first, so
+    // u == out (in place) is safe; a shifted overlap is not.  With LOCAL_X the whole vector u(x) is read by
+    // work items that run concurrently with the writers of out(x): any overlap is refused.
+    if (local != COARSE_LOCAL_NONE && overlaps(u_dev, vb, out_dev, vb)) {
+        if (local == COARSE_LOCAL_X)
+            return fail(COARSE_EINVAL, "apply_parts: u and out overlap with COARSE_LOCAL_X (X.u reads all of u(x) while out(x) is written)");
+        if (u_dev != out_dev)
+            return fail(COARSE_EINVAL, "apply_parts: u and out overlap partially (only u == out is allowed, with COARSE_LOCAL_IDENTITY)");
+    }
     PartsSpec ps = {true, local != 0 ? u_dev : w_dev, parity, local, alpha, beta, nullptr, 0, 0};
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int path = op->path_opt;
@@ -483,13 +508,22 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
                              (op->path_opt == COARSE_PATH_AUTO || op->path_opt == COARSE_PATH_STREAM);
     if (stream_1rhs && T >= 8 && vb >= ((size_t)1 << 22)) {
         if (!op->host_pipe_ok) {
-            bool ok = cudaStreamCreateWithFlags(&op->s_h2d, cudaStreamNonBlocking) == cudaSuccess &&
-                      cudaStreamCreateWithFlags(&op->s_d2h, cudaStreamNonBlocking) == cudaSuccess;
-            for (int i = 0; ok && i < 4; ++i)
-                ok = cudaEventCreateWithFlags(&op->ev_up[i], cudaEventDisableTiming) == cudaSuccess &&
-                     cudaEventCreateWithFlags(&op->ev_k[i], cudaEventDisableTiming) == cudaSuccess;
-            ok = ok && cudaEventCreateWithFlags(&op->ev_done, cudaEventDisableTiming) == cudaSuccess;
-            if (!ok) { cudaGetLastError(); return fail(COARSE_ECUDA, "apply_host: cannot create copy streams/events"); }
+            // create the two copy streams and nine events; on a partial failure destroy what exists
+            cudaStream_t ss[2] = {nullptr, nullptr};
+            cudaEvent_t ev[9] = {};
+            bool ok = true;
+            for (int i = 0; ok && i < 2; ++i) ok = cudaStreamCreateWithFlags(&ss[i], cudaStreamNonBlocking) == cudaSuccess;
+            for (int i = 0; ok && i < 9; ++i) ok = cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming) == cudaSuccess;
+            if (!ok) {
+                cudaGetLastError();
+                for (int i = 0; i < 9; ++i) if (ev[i]) cudaEventDestroy(ev[i]);
+                for (int i = 0; i < 2; ++i) if (ss[i]) cudaStreamDestroy(ss[i]);
+                return fail(COARSE_ECUDA, "apply_host: cannot create copy streams/events");
+            }
+            op->s_h2d = ss[0];
+            op->s_d2h = ss[1];
+            for (int i = 0; i < 4; ++i) { op->ev_up[i] = ev[i]; op->ev_k[i] = ev[4 + i]; }
+            op->ev_done = ev[8];
             op->host_pipe_ok = true;
         }
         const size_t plane = (size_t)(op->lat.V / T);               // sites per x3-slice
@@ -498,13 +532,21 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
         unsigned char* hout = static_cast<unsigned char*>(out_host);
         unsigned char* din = static_cast<unsigned char*>(op->stage_in);
         unsigned char* dout = static_cast<unsigned char*>(op->stage_out);
+        // Once a copy is queued the host buffers are in use by the device: every exit, error or not,
+        // first drains the three streams (the header promises the call has synchronised when it returns).
+        auto drain = [&]() {
+            cudaStreamSynchronize(op->s_h2d);
+            cudaStreamSynchronize(st);
+            cudaStreamSynchronize(op->s_d2h);
+        };
+        auto bail_cuda = [&](cudaError_t err, const char* what) { drain(); cudaGetLastError(); return cuda_fail(err, what); };
         // the copy streams start after whatever the caller's stream has queued
         if ((e = cudaEventRecord(op->ev_done, st)) != cudaSuccess) return cuda_fail(e, "apply_host: event record");
-        cudaStreamWaitEvent(op->s_h2d, op->ev_done, 0);
-        cudaStreamWaitEvent(op->s_d2h, op->ev_done, 0);
+        if ((e = cudaStreamWaitEvent(op->s_h2d, op->ev_done, 0)) != cudaSuccess) return cuda_fail(e, "apply_host: stream wait");
+        if ((e = cudaStreamWaitEvent(op->s_d2h, op->ev_done, 0)) != cudaSuccess) return cuda_fail(e, "apply_host: stream wait");
         // slice T-1 first (range 0 reads it through the periodic wrap), then slices in order
         if ((e = cudaMemcpyAsync(din + (size_t)(T - 1) * pb, hin + (size_t)(T - 1) * pb, pb, cudaMemcpyHostToDevice, op->s_h2d)) != cudaSuccess)
-            return cuda_fail(e, "apply_host: H2D copy");
+            return bail_cuda(e, "apply_host: H2D copy");
         int uploaded = 0;                                            // slices [0, uploaded) are queued
         PartsSpec ps = kPlain;
         op->last_launches = 0;
@@ -514,24 +556,24 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
             if (need > uploaded) {
                 e = cudaMemcpyAsync(din + (size_t)uploaded * pb, hin + (size_t)uploaded * pb, (size_t)(need - uploaded) * pb,
                                     cudaMemcpyHostToDevice, op->s_h2d);
-                if (e != cudaSuccess) return cuda_fail(e, "apply_host: H2D copy");
+                if (e != cudaSuccess) return bail_cuda(e, "apply_host: H2D copy");
                 uploaded = need;
             }
-            cudaEventRecord(op->ev_up[c], op->s_h2d);
-            cudaStreamWaitEvent(st, op->ev_up[c], 0);
+            if ((e = cudaEventRecord(op->ev_up[c], op->s_h2d)) != cudaSuccess) return bail_cuda(e, "apply_host: event record");
+            if ((e = cudaStreamWaitEvent(st, op->ev_up[c], 0)) != cudaSuccess) return bail_cuda(e, "apply_host: stream wait");
             ps.site_begin = (int)(plane * t0);
             ps.site_end = (int)(plane * t1);
             rc = launch_stream(op, op->stage_in, op->stage_out, dagger, ps, st);
-            if (rc != COARSE_OK) return rc;
+            if (rc != COARSE_OK) { drain(); return rc; }
             op->last_launches += 1;
-            cudaEventRecord(op->ev_k[c], st);
-            cudaStreamWaitEvent(op->s_d2h, op->ev_k[c], 0);
+            if ((e = cudaEventRecord(op->ev_k[c], st)) != cudaSuccess) return bail_cuda(e, "apply_host: event record");
+            if ((e = cudaStreamWaitEvent(op->s_d2h, op->ev_k[c], 0)) != cudaSuccess) return bail_cuda(e, "apply_host: stream wait");
             e = cudaMemcpyAsync(hout + (size_t)t0 * pb, dout + (size_t)t0 * pb, (size_t)(t1 - t0) * pb, cudaMemcpyDeviceToHost, op->s_d2h);
-            if (e != cudaSuccess) return cuda_fail(e, "apply_host: D2H copy");
+            if (e != cudaSuccess) return bail_cuda(e, "apply_host: D2H copy");
         }
         op->last_path = COARSE_PATH_STREAM;
-        cudaEventRecord(op->ev_done, op->s_d2h);
-        cudaStreamWaitEvent(st, op->ev_done, 0);
+        if ((e = cudaEventRecord(op->ev_done, op->s_d2h)) != cudaSuccess) return bail_cuda(e, "apply_host: event record");
+        if ((e = cudaStreamWaitEvent(st, op->ev_done, 0)) != cudaSuccess) return bail_cuda(e, "apply_host: stream wait");
         e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) return cuda_fail(e, "apply_host: stream synchronize");
         return COARSE_OK;
@@ -539,9 +581,9 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
     e = cudaMemcpyAsync(op->stage_in, in_host, vb, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(e, "apply_host: H2D copy");
     rc = coarse_op_apply(op, op->stage_in, op->stage_out, nrhs, dagger, stream);
-    if (rc != COARSE_OK) return rc;
+    if (rc != COARSE_OK) { cudaStreamSynchronize(st); return rc; }      // the H2D copy reads in_host until then
     e = cudaMemcpyAsync(out_host, op->stage_out, vb, cudaMemcpyDeviceToHost, st);
-    if (e != cudaSuccess) return cuda_fail(e, "apply_host: D2H copy");
+    if (e != cudaSuccess) { cudaStreamSynchronize(st); cudaGetLastError(); return cuda_fail(e, "apply_host: D2H copy"); }
     e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return cuda_fail(e, "apply_host: stream synchronize");
     return COARSE_OK;
@@ -582,8 +624,17 @@ static int cagcr_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int s, in
     if (s < 1 || s > CAGCR_MAX_S) return fail(COARSE_EINVAL, "cagcr: 1 <= s <= %d (got %d)", CAGCR_MAX_S, s);
     if (cycles < 1) return fail(COARSE_EINVAL, "cagcr: cycles must be >= 1");
     if (!aligned16(b_dev) || !aligned16(x_dev) || !aligned16(work_dev)) return fail(COARSE_EINVAL, "cagcr: pointers must be 16-byte aligned");
+    { int rc0 = check_device(op, "cagcr"); if (rc0 != COARSE_OK) return rc0; }
+    if (op->path_opt == COARSE_PATH_TENSOR || op->path_opt == COARSE_PATH_BLOCK)
+        return fail(COARSE_EUNSUPPORTED, "cagcr: the handle is pinned to a block-apply path; the smoother applies 1 RHS");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t vec = coarse_op_vector_bytes(op, 1);
+    {
+        const size_t wb = coarse_op_cagcr_work_bytes(op, s);
+        if (overlaps(b_dev, vec, x_dev, vec) || overlaps(b_dev, vec, work_dev, wb) || overlaps(x_dev, vec, work_dev, wb))
+            return fail(COARSE_EINVAL, "cagcr: b, x and work must not overlap");
+    }
+    op->last_launches = 0;
     const long long n = (long long)op->lat.V * op->Nc;
     const int S1 = s + 1;
     unsigned char* w = static_cast<unsigned char*>(work_dev);
@@ -624,7 +675,7 @@ static int cagcr_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int s, in
         p0_is_b = true;
     } else {
         rc = apply_op(x_dev, slot[1]);
-        if (rc != COARSE_OK) return rc;
+        if (rc != COARSE_OK) { op->last_launches = launches; return rc; }
         cagcr_residual_kernel<<<vgrid, 256, 0, st>>>(static_cast<const float2*>(b_dev), slot[1], n, slot[0]);
         ++launches;
     }
@@ -635,12 +686,16 @@ static int cagcr_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int s, in
         float2* r_out = slot[(base + s + 1) % NS];
         for (int k = 0; k < s; ++k) {
             rc = apply_op(v.p[k], const_cast<float2*>(v.p[k + 1]));
-            if (rc != COARSE_OK) return rc;
+            if (rc != COARSE_OK) { op->last_launches = launches; return rc; }
         }
         cagcr_gram_kernel<<<CAGCR_GRAM_BLOCKS, 256, 0, st>>>(v, n, s, partial);
         cagcr_solve_kernel<<<1, 320, 0, st>>>(partial, CAGCR_GRAM_BLOCKS, s, alpha, info_dev ? info_dev + 3 * c : nullptr);
         cagcr_update_kernel<<<vgrid, 256, 0, st>>>(v, n, s, alpha, static_cast<float2*>(x_dev), r_out);
         launches += 3;
+        {
+            cudaError_t ec = cudaGetLastError();
+            if (ec != cudaSuccess) { op->last_launches = launches; return cuda_fail(ec, "cagcr kernel launch"); }
+        }
         base = (base + s + 1) % NS;
         p0_is_b = false;
     }
@@ -662,8 +717,17 @@ static int cagcr_cheb_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int 
     if (cycles < 1) return fail(COARSE_EINVAL, "cagcr_cheb: cycles must be >= 1");
     if (!(lambda_max > lambda_min)) return fail(COARSE_EINVAL, "cagcr_cheb: need lambda_max > lambda_min");
     if (!aligned16(b_dev) || !aligned16(x_dev) || !aligned16(work_dev)) return fail(COARSE_EINVAL, "cagcr_cheb: pointers must be 16-byte aligned");
+    { int rc0 = check_device(op, "cagcr_cheb"); if (rc0 != COARSE_OK) return rc0; }
+    if (op->path_opt == COARSE_PATH_TENSOR || op->path_opt == COARSE_PATH_BLOCK)
+        return fail(COARSE_EUNSUPPORTED, "cagcr_cheb: the handle is pinned to a block-apply path; the smoother applies 1 RHS");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t vec = coarse_op_vector_bytes(op, 1);
+    {
+        const size_t wb = coarse_op_cagcr_cheb_work_bytes(op, s);
+        if (overlaps(b_dev, vec, x_dev, vec) || overlaps(b_dev, vec, work_dev, wb) || overlaps(x_dev, vec, work_dev, wb))
+            return fail(COARSE_EINVAL, "cagcr_cheb: b, x and work must not overlap");
+    }
+    op->last_launches = 0;
     const long long n = (long long)op->lat.V * op->Nc;
     const int S1 = s + 1, NSLOT = 2 * s + 1;
     unsigned char* w = static_cast<unsigned char*>(work_dev);
@@ -712,7 +776,7 @@ static int cagcr_cheb_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int 
         }
         for (int k = 0; k < s; ++k) {
             rc = apply_op(P.p[k], const_cast<float2*>(T.p[k]));
-            if (rc != COARSE_OK) return rc;
+            if (rc != COARSE_OK) { op->last_launches = launches; return rc; }
             if (k + 1 < s) {
                 const float a = (k == 0 ? 1.f : 2.f) / d;
                 cagcr_cheb_step_kernel<<<vgrid, 256, 0, st>>>(T.p[k], P.p[k], k == 0 ? P.p[k] : P.p[k - 1], a, -a * c,
@@ -726,6 +790,10 @@ static int cagcr_cheb_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int 
         cagcr_solve_kernel<<<1, 320, 0, st>>>(partial, CAGCR_GRAM_BLOCKS, s, alpha, info_dev ? info_dev + 3 * cyc : nullptr);
         cagcr_update2_kernel<<<vgrid, 256, 0, st>>>(P, T, P.p[0], n, s, alpha, static_cast<float2*>(x_dev), slot[rslot]);
         launches += 3;
+        {
+            cudaError_t ec = cudaGetLastError();
+            if (ec != cudaSuccess) { op->last_launches = launches; return cuda_fail(ec, "cagcr_cheb kernel launch"); }
+        }
         if (p0_is_b) { p0 = rslot; rslot = 0; p0_is_b = false; }   // slot 0 was unused while P_0 = b
         else { const int t2 = p0; p0 = rslot; rslot = t2; }
     }

@@ -173,7 +173,33 @@ def test_parts_argument_errors():
     assert L.coarse_op_apply_parts(*args(v.data_ptr(), v.data_ptr(), o.data_ptr(), 2, 5)) == cop.EINVAL
     assert L.coarse_op_apply_parts(*args(None, v.data_ptr(), o.data_ptr(), 2, 1)) == cop.EINVAL           # local term without u
     assert L.coarse_op_apply_parts(*args(v.data_ptr(), o.data_ptr(), o.data_ptr(), 2, 1)) == cop.EINVAL   # w overlaps out
-    assert L.coarse_op_apply_parts(*args(o.data_ptr(), v.data_ptr(), o.data_ptr(), 2, 2)) == cop.OK       # u may alias out
+    assert L.coarse_op_apply_parts(*args(o.data_ptr(), v.data_ptr(), o.data_ptr(), 2, 2)) == cop.OK       # identity: u == out is allowed
+    assert L.coarse_op_apply_parts(*args(o.data_ptr(), v.data_ptr(), o.data_ptr(), 2, 1)) == cop.EINVAL   # X.u in place is a race
+    assert "COARSE_LOCAL_X" in cop.coarse_op_last_error()
+    big = torch.zeros((2 * V, 48, 1), dtype=torch.complex64, device="cuda")
+    shifted = big.data_ptr() + 48 * 8                                                                       # overlaps big[:V] by all but one site
+    assert L.coarse_op_apply_parts(*args(shifted, v.data_ptr(), big.data_ptr(), 2, 2)) == cop.EINVAL      # partial overlap
+    assert "partially" in cop.coarse_op_last_error()
     assert L.coarse_op_apply_parts(*args(None, v.data_ptr(), o.data_ptr(), 2, 0)) == cop.OK
     torch.cuda.synchronize()
     cop.coarse_op_destroy(h)
+
+
+@pytest.mark.parametrize("Nc,prec", [(96, cop.LINK_C64), (128, cop.LINK_I16), (48, cop.LINK_C64)])
+@pytest.mark.parametrize("dagger", [0, 1])
+@pytest.mark.parametrize("path", [cop.PATH_STREAM, cop.PATH_SIMPLE])
+def test_parts_identity_in_place_values(oracle_lib, Nc, prec, dagger, path):
+    """out = u - Hop(w) computed IN PLACE (u_dev == out_dev, COARSE_LOCAL_IDENTITY) on shapes whose sites
+    are split over several (site, row-block) work items (Nc = 96 / 128, dagger = 0): every output element
+    reads only its own u element, so the values must equal the out-of-place result of the oracle."""
+    dims = (2, 4, 2, 2)
+    V = synth.lattice_volume(dims)
+    links_d, scales_d, links_h, scales_h, u, w = _make(oracle_lib, dims, Nc, prec, 977, 1)
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links_d, scales_d).set_option(cop.OPT_PATH, path)
+    buf = u.clone()
+    op.apply_parts(buf, w, buf, dagger=dagger, parity=cop.PARITY_ALL, local=cop.LOCAL_IDENTITY, alpha=1.0, beta=-1.0)
+    torch.cuda.synchronize()
+    ref = oracle_lib.coarse_apply_parts(dims, Nc, links_h, u.cpu().numpy(), w.cpu().numpy(), dagger=dagger, parity=2,
+                                        local=2, alpha=1.0, beta=-1.0, link_precision=prec, scales=scales_h)
+    assert rel_l2_per_rhs(buf.cpu().numpy(), ref) <= TOL
+    op.close()
