@@ -765,6 +765,90 @@ def run_schur(args, cfg):
     return 0
 
 
+def run_hat(args, cfg):
+    """--workload hat: build the block-preconditioned links
+    Yhat_m = X^-1 Y_m of the config's operator on the device (coarse_op_build_hat_links) and quantise them
+    to int16 when the config stores int16 links.  A set-up step: one step = one build over the lattice.
+    Bound by fp64 FMA throughput (72 Nc^3 flops per site), not HBM; both fractions are reported."""
+    import paper_2212_12559_b200 as cop
+    world, rank, local = dist_env()
+    if world > 1:
+        raise RuntimeError("--workload hat is a single-GPU measurement")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dims, Nc = cfg["dims"], cfg["Nc"]
+    V = synth.lattice_volume(dims)
+    links = synth.make_gamma_hermitian_links(dims, Nc, cfg["seed"], device=dev)
+    op = cop.CoarseOp(dims, Nc, cop.LINK_C64).set_links(links)
+    hat = torch.empty_like(links)
+    info = torch.zeros((1,), dtype=torch.int32, device=dev)
+    work = op.build_hat_links(hat, info=info)
+    torch.cuda.synchronize()
+    parity = None
+    if not args.no_parity:
+        import oracle
+        sites = parity_sample_sites(dims, 24, cfg["seed"])
+        ref = oracle.hat_links(links[torch.as_tensor(sites, device=dev)].cpu().numpy())
+        got = hat[torch.as_tensor(sites, device=dev)].cpu().numpy().astype(np.complex128)
+        err = np.linalg.norm((got - ref).reshape(len(sites), 9, -1), axis=2) / np.linalg.norm(ref.reshape(len(sites), 9, -1), axis=2)
+        parity = {"rel_l2_per_matrix_max": float(err.max()), "sites": int(len(sites)), "tolerance": 1e-6,
+                  "ok": bool(err.max() <= 1e-6), "singular_sites": int(info.item())}
+        if not parity["ok"]:
+            raise RuntimeError("bench.py --workload hat: device-built hat links differ from the oracle: %r" % (parity,))
+    stream = torch.cuda.current_stream()
+    q = sc = None
+    if cfg["links"] == "i16":
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device=dev)
+        sc = torch.empty((V, 9), dtype=torch.float32, device=dev)
+
+    def step():
+        op.build_hat_links(hat, work=work)
+        if q is not None:
+            cop.coarse_op_quantize_i16(hat, Nc, q, sc)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    steps = min(args.steps, 20)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(steps)]
+    with ClockSampler(local) as clocks:
+        for a, b, c in ev:
+            a.record(stream)
+            op.build_hat_links(hat, work=work)
+            b.record(stream)
+            if q is not None:
+                cop.coarse_op_quantize_i16(hat, Nc, q, sc)
+            c.record(stream)
+        torch.cuda.synchronize()
+    ms_build = sum(a.elapsed_time(b) for a, b, c in ev) / steps
+    ms_total = sum(a.elapsed_time(c) for a, b, c in ev) / steps
+    flops = 72.0 * Nc ** 3 * V                         # 8 Nc^3 (complex Gauss-Jordan) + 8 x 8 Nc^3 (products), real flops
+    bytes_alg = V * (9 + 9) * Nc * Nc * 8              # 9 matrices read, 9 written (slot 0 = identity)
+    peak, peak_src = measured_peak_gbs()
+    fp64_peak = 148 * 64 * 2 * 1.965e9 / 1e12          # 148 SMs x 64 DFMA lanes x 2 flop x 1.965 GHz = 37.2 TFLOP/s
+    line = {
+        "metric": "hat-link builds: coarse sites/s", "value": V * steps / (ms_total * steps * 1e-3), "unit": "sites/s", "n_gpus": 1,
+        "steps": steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "block-preconditioned links Yhat = X^-1 Y on the %s lattice, Nc=%d, complex64 in, %s out" %
+                               ("x".join(map(str, dims)), Nc, "int16 + scales" if q is not None else "complex64"),
+                   "seed": cfg["seed"]},
+        "clocks": clocks.summary(), "gpu_launches": (2 if q is not None else 1) * steps,
+        "roofline": {"bound": "alu", "achieved": flops / (ms_build * 1e-3) / 1e12, "peak": fp64_peak, "unit": "TFLOP/s",
+                     "frac": flops / (ms_build * 1e-3) / 1e12 / fp64_peak, "traffic": None,
+                     "peak_source": "fp64 FMA: 148 SMs x 64 lanes x 2 flop x 1.965 GHz (derived, DESIGN.md §10)",
+                     "kernel": "hat_links_kernel", "kernel_ms": ms_build, "quantize_ms": ms_total - ms_build,
+                     "algorithmic_flops_per_launch": flops, "algorithmic_bytes_per_launch": bytes_alg,
+                     "hbm_gbs": bytes_alg / (ms_build * 1e-3) / 1e9, "hbm_frac_of_measured": bytes_alg / (ms_build * 1e-3) / 1e9 / peak},
+    }
+    if parity is not None:
+        line["parity"] = parity
+    print(json.dumps(line), flush=True)
+    op.close()
+    return 0
+
+
 def run_cagcr(args, cfg):
     """--workload cagcr: CA-GCR(8) smoother cycles on the config's operator
     (diagonally shifted so that the smoother converges).  One step = one cycle = 8 chained applies + the
@@ -844,7 +928,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2", choices=sorted(synth.CONFIGS))
-    ap.add_argument("--workload", default="apply", choices=["apply", "schur", "cagcr"],
+    ap.add_argument("--workload", default="apply", choices=["apply", "schur", "cagcr", "hat"],
                     help="apply: the BASELINE metric (default); schur: the even/odd Schur-hat operator (row f1)")
     ap.add_argument("--dagger", default="both", choices=["0", "1", "both"])
     ap.add_argument("--path", type=int, default=0, help="COARSE_PATH_* override (0 = auto)")
@@ -887,6 +971,8 @@ def main():
         return run_schur(args, cfg)
     if args.workload == "cagcr":
         return run_cagcr(args, cfg)
+    if args.workload == "hat":
+        return run_hat(args, cfg)
     if args.impl == "reference":
         return run_reference(args, cfg, daggers)
     return run_ours(args, cfg, daggers)

@@ -191,6 +191,26 @@ int coarse_op_last_path(const coarse_op_t* op);
 int coarse_op_quantize_i16(const void* links_c64_dev, int64_t n_matrices, int Nc, void* q_dev,
                            float* scales_dev, void* stream);
 
+/* Block-preconditioned links ("coarsening the block-preconditioned operator"; the operator
+ * the paper's "Schur-preconditioned" levels iterate on, Table 1 L127/L135), built on the device from this
+ * handle's links (either precision; int16 is dequantised exactly):
+ *
+ *     out[s][m] = X(s)^-1 . Y_m(s)  for m = 1..8,     out[s][0] = identity (COARSE_HAT_SLOT0_IDENTITY)
+ *                                                              or X(s)^-1 (COARSE_HAT_SLOT0_XINV)
+ *
+ * out_links_c64_dev: complex64 [V][9][Nc][Nc] in the canonical link layout (V*9*Nc*Nc*8 bytes, caller
+ * owned, must not overlap the handle's links); hand it to a second COARSE_LINK_C64 handle, or quantise it
+ * with coarse_op_quantize_i16 for a COARSE_LINK_I16 one.  With X^-1 in slot 0, "apply X^-1" is
+ * coarse_op_apply_parts(.., COARSE_LOCAL_X, alpha = 1, beta = 0) on that handle.
+ * work_dev: coarse_op_hat_work_bytes(op) bytes of scratch (16-byte aligned).  info_dev: NULL or int[1], set
+ * to the number of sites whose X has a zero pivot (those sites' outputs are non-finite).
+ * All arithmetic is fp64 (Gauss-Jordan with partial pivoting + eight Nc^3 products per site), rounded to
+ * complex64 once.  Any even Nc.  One launch; enqueues and returns. */
+enum { COARSE_HAT_SLOT0_IDENTITY = 0, COARSE_HAT_SLOT0_XINV = 1 };
+size_t coarse_op_hat_work_bytes(const coarse_op_t* op);
+int coarse_op_build_hat_links(coarse_op_t* op, void* out_links_c64_dev, int slot0, void* work_dev, int* info_dev,
+                              void* stream);
+
 /* CA-GCR(s), the paper's smoother ("CA-GCR(8)", Table 1 L116/L122/L130), on this operator,
  * 1 RHS, power basis.  Each of `cycles` cycles: r0 = b - A x; p_k = A^k r0 (s chained coarse_op_apply);
  * ONE fused pass of block inner products G_jk = <p_j, p_k> (fp64, the single reduction per cycle);

@@ -235,14 +235,15 @@ def schur_apply(dims, Nc: int, links, v, parity: int, nrhs: int = 1) -> np.ndarr
     return coarse_apply_parts(dims, Nc, links, vp, t2.astype(np.complex64), nrhs, 0, parity, LOCAL_X, 1.0, -1.0)
 
 
-def hat_links(links) -> np.ndarray:
+def hat_links(links, slot0_inverse: bool = False) -> np.ndarray:
     """Block-preconditioned links: Yhat_m(x) = X(x)^{-1} Y_m(x), m = 1..8; slot 0
-    holds the identity.  complex128 [V][9][Nc][Nc] (cast to complex64 before use as an input)."""
+    holds the identity, or X(x)^{-1} when slot0_inverse.  complex128 [V][9][Nc][Nc] (cast to complex64
+    before use as an input)."""
     links = np.asarray(links).astype(np.complex128)
     out = np.empty_like(links)
     Nc = links.shape[-1]
     for s in range(links.shape[0]):
-        out[s, 0] = np.eye(Nc)
+        out[s, 0] = np.linalg.solve(links[s, 0], np.eye(Nc)) if slot0_inverse else np.eye(Nc)
         out[s, 1:] = np.linalg.solve(links[s, 0][None, :, :], links[s, 1:])
     return out
 

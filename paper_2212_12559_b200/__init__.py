@@ -29,7 +29,7 @@ EXPORTS = (
     "coarse_op_quantize_vec_i16", "coarse_op_apply_host",
     "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_probe_read", "coarse_op_cagcr_work_bytes",
     "coarse_op_cagcr", "coarse_op_cagcr_schur", "coarse_op_cagcr_cheb_work_bytes",
-    "coarse_op_cagcr_cheb", "coarse_op_destroy",
+    "coarse_op_cagcr_cheb", "coarse_op_hat_work_bytes", "coarse_op_build_hat_links", "coarse_op_destroy",
     "coarse_op_last_error",
 )
 
@@ -78,6 +78,10 @@ def lib() -> ctypes.CDLL:
     L.coarse_op_last_launches.argtypes = [vp]
     L.coarse_op_last_path.restype = ci
     L.coarse_op_last_path.argtypes = [vp]
+    L.coarse_op_hat_work_bytes.restype = sz
+    L.coarse_op_hat_work_bytes.argtypes = [vp]
+    L.coarse_op_build_hat_links.restype = ci
+    L.coarse_op_build_hat_links.argtypes = [vp, vp, ci, vp, vp, vp]
     L.coarse_op_quantize_i16.restype = ci
     L.coarse_op_quantize_i16.argtypes = [vp, ci64, ci, vp, vp, vp]
     L.coarse_op_cagcr_work_bytes.restype = sz
@@ -244,6 +248,31 @@ def coarse_op_quantize_i16(links_c64, Nc: int, q_out, scales_out, stream=None) -
                                         _stream_handle(stream)))
 
 
+HAT_SLOT0_IDENTITY, HAT_SLOT0_XINV = 0, 1
+
+
+def coarse_op_hat_work_bytes(op: int) -> int:
+    return int(lib().coarse_op_hat_work_bytes(op))
+
+
+def coarse_op_build_hat_links(op: int, out_links, slot0: int = HAT_SLOT0_IDENTITY, work=None, info=None, stream=None):
+    """out_links: CUDA complex64 [V][9][Nc][Nc]; work: CUDA uint8 tensor of coarse_op_hat_work_bytes(op)
+    bytes (allocated when None); info: optional CUDA int32 tensor [1].  Returns the work tensor."""
+    import torch
+    if work is None:
+        work = torch.empty(coarse_op_hat_work_bytes(op), dtype=torch.uint8, device=out_links.device)
+    for t in (out_links, work) + ((info,) if info is not None else ()):
+        if not t.is_cuda or not t.is_contiguous():
+            raise ValueError("build_hat_links needs contiguous CUDA tensors")
+    if out_links.dtype != torch.complex64:
+        raise ValueError("build_hat_links: out_links must be complex64")
+    if info is not None and (info.dtype != torch.int32 or info.numel() < 1):
+        raise ValueError("build_hat_links: info must be an int32 tensor")
+    _check(lib().coarse_op_build_hat_links(op, _ptr(out_links), int(slot0), _ptr(work),
+                                           _ptr(info) if info is not None else None, _stream_handle(stream)))
+    return work
+
+
 def coarse_op_cagcr_work_bytes(op: int, s: int) -> int:
     return int(lib().coarse_op_cagcr_work_bytes(op, int(s)))
 
@@ -332,6 +361,12 @@ class CoarseOp:
     def apply_parts(self, u, w, vout, nrhs: int = 1, dagger: int = 0, parity: int = PARITY_ALL,
                     local: int = LOCAL_X, alpha: float = 1.0, beta: float = 1.0, stream=None) -> None:
         coarse_op_apply_parts(self._h, u, w, vout, nrhs, dagger, parity, local, alpha, beta, stream)
+
+    def build_hat_links(self, out_links, slot0: int = HAT_SLOT0_IDENTITY, work=None, info=None, stream=None):
+        """Yhat_m = X^-1 Y_m (slot 0: identity or X^-1) into out_links (complex64 [V][9][Nc][Nc])."""
+        if out_links.numel() != self.V * 9 * self.Nc * self.Nc:
+            raise ValueError("build_hat_links: out_links must hold V*9*Nc*Nc complex64 entries")
+        return coarse_op_build_hat_links(self._h, out_links, slot0, work, info, stream)
 
     def apply_hvec(self, vin_q, vin_norms, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
         coarse_op_apply_hvec(self._h, vin_q, vin_norms, vout, nrhs, dagger, stream)

@@ -15,6 +15,7 @@
 #include "block_kernel.cuh"
 #include "probe_kernel.cuh"
 #include "cagcr_kernel.cuh"
+#include "hat_kernel.cuh"
 
 using namespace coarse;
 
@@ -826,6 +827,57 @@ int coarse_op_cagcr_schur(coarse_op_t* op_hat, const void* b_dev, void* x_dev, i
                           int parity, void* work_dev, double* info_dev, void* stream) {
     if (parity != 0 && parity != 1) return fail(COARSE_EINVAL, "cagcr_schur: parity must be 0 (even) or 1 (odd)");
     return cagcr_impl(op_hat, b_dev, x_dev, s, cycles, x_is_zero, parity, work_dev, info_dev, stream);
+}
+
+static int hat_grid(const coarse_op* op) {
+    const int g = 2 * op->num_sms;
+    return op->lat.V < g ? op->lat.V : g;
+}
+
+size_t coarse_op_hat_work_bytes(const coarse_op_t* op) {
+    if (!op) return 0;
+    return (size_t)hat_grid(op) * op->Nc * op->Nc * sizeof(double2);
+}
+
+int coarse_op_build_hat_links(coarse_op_t* op, void* out_links_c64_dev, int slot0, void* work_dev, int* info_dev,
+                              void* stream) {
+    if (!op) return fail(COARSE_EINVAL, "build_hat_links: op is NULL");
+    if (!op->links) return fail(COARSE_ENOTREADY, "build_hat_links: coarse_op_set_links has not been called");
+    if (!out_links_c64_dev || !work_dev) return fail(COARSE_EINVAL, "build_hat_links: NULL pointer");
+    if (slot0 != COARSE_HAT_SLOT0_IDENTITY && slot0 != COARSE_HAT_SLOT0_XINV)
+        return fail(COARSE_EINVAL, "build_hat_links: slot0 must be COARSE_HAT_SLOT0_IDENTITY or COARSE_HAT_SLOT0_XINV");
+    if (!aligned16(out_links_c64_dev) || !aligned16(work_dev)) return fail(COARSE_EINVAL, "build_hat_links: pointers must be 16-byte aligned");
+    int rc = check_device(op, "build_hat_links");
+    if (rc != COARSE_OK) return rc;
+    const size_t out_bytes = (size_t)op->lat.V * 9 * op->Nc * op->Nc * 8;
+    if (overlaps(out_links_c64_dev, out_bytes, op->links, coarse_op_link_bytes(op)))
+        return fail(COARSE_EINVAL, "build_hat_links: out_links overlaps the operator's own links (not an in-place operation)");
+    if (overlaps(work_dev, coarse_op_hat_work_bytes(op), out_links_c64_dev, out_bytes) ||
+        overlaps(work_dev, coarse_op_hat_work_bytes(op), op->links, coarse_op_link_bytes(op)))
+        return fail(COARSE_EINVAL, "build_hat_links: work overlaps the links");
+    if (op->lat.V == 0) return COARSE_OK;
+    HatParams p;
+    p.lat = op->lat;
+    p.Nc = op->Nc;
+    p.i16 = op->prec == COARSE_LINK_I16;
+    p.links = op->links;
+    p.scales = op->scales;
+    p.out = static_cast<float2*>(out_links_c64_dev);
+    p.work = static_cast<double2*>(work_dev);
+    p.slot0_inverse = slot0 == COARSE_HAT_SLOT0_XINV;
+    p.info = info_dev;
+    const size_t smem = hat_smem_bytes(op->Nc);
+    if (smem > (size_t)op->max_smem) return fail(COARSE_EUNSUPPORTED, "build_hat_links: Nc=%d needs %zu bytes of shared memory", op->Nc, smem);
+    static SmemAttrCache attr_cache;
+    cudaError_t e = ensure_dynamic_smem(hat_links_kernel, op->device, (int)smem, attr_cache);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(hat kernel)");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (info_dev && (e = cudaMemsetAsync(info_dev, 0, sizeof(int), st)) != cudaSuccess) return cuda_fail(e, "build_hat_links: memset info");
+    hat_links_kernel<<<hat_grid(op), HAT_THREADS, smem, st>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "hat kernel launch");
+    op->last_launches = 1;
+    return COARSE_OK;
 }
 
 int coarse_op_probe_read(const void* src_dev, size_t bytes, int stage_bytes, int stages, void* stream) {

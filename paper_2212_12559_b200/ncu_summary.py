@@ -33,8 +33,14 @@ METRICS = [
 
 
 def read_report(path: str):
-    out = subprocess.run(["ncu", "-i", path, "--page", "raw", "--csv", "--print-units", "base"],
-                         capture_output=True, text=True, check=True).stdout
+    """`path`: an .ncu-rep file, or the text of `ncu -i REPORT --page raw --csv --print-units base` saved as .csv
+    (reports of several captures exceed what gpurun brings back; the raw page is exported on the GPU box)."""
+    if path.endswith(".csv"):
+        with open(path) as f:
+            out = f.read()
+    else:
+        out = subprocess.run(["ncu", "-i", path, "--page", "raw", "--csv", "--print-units", "base"],
+                             capture_output=True, text=True, check=True).stdout
     rows = list(csv.reader(io.StringIO(out)))
     hdr, units, data = rows[0], rows[1], rows[2:]
     return hdr, units, data

@@ -1,4 +1,4 @@
-"""Small numpy helpers for the tests (no oracle/, no CUDA path)."""
+"""Small numpy helpers for the tests (no oracle/ import; only gpu_hat_links touches the CUDA path, lazily)."""
 from __future__ import annotations
 
 import numpy as np
@@ -55,3 +55,22 @@ def gamma_diag(Nc):
     g = np.ones(Nc)
     g[Nc // 2:] = -1.0
     return g
+
+
+def gpu_hat_links(oracle_lib, dims, Nc, links_np):
+    """Block-preconditioned links built by the PRODUCT (coarse_op_build_hat_links) from complex64 links on the
+    host; returns the device tensor and its host copy (the same bits go to the oracle's apply), after
+    checking them against the oracle's own fp64 solve at fp32 rounding level."""
+    import torch
+    import paper_2212_12559_b200 as cop
+    links_d = torch.as_tensor(links_np, device="cuda")
+    op = cop.CoarseOp(dims, Nc).set_links(links_d)
+    hat_d = torch.empty_like(links_d)
+    op.build_hat_links(hat_d)
+    torch.cuda.synchronize()
+    op.close()
+    hat = hat_d.cpu().numpy()
+    ref = oracle_lib.hat_links(links_np)
+    d = np.linalg.norm((hat - ref).reshape(hat.shape[0], 9, -1), axis=2) / np.linalg.norm(ref.reshape(hat.shape[0], 9, -1), axis=2)
+    assert d.max() <= 1e-6, f"device-built hat links differ from the oracle's: {d.max():.3e}"
+    return hat_d, hat

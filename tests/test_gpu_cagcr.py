@@ -12,7 +12,7 @@ import torch
 
 import synth
 import paper_2212_12559_b200 as cop
-from tests.helpers import rel_l2
+from tests.helpers import gpu_hat_links, rel_l2
 
 pytestmark = pytest.mark.gpu
 
@@ -101,7 +101,7 @@ def test_cagcr_on_the_schur_hat_operator(oracle_lib, dims, Nc, parity, x_is_zero
     V, s, cycles = synth.lattice_volume(dims), 8, 2
     links = synth.make_arbitrary_links(dims, Nc, 7).numpy()
     links[:, 0] += 6.0 * np.eye(Nc, dtype=np.complex64)
-    hat = oracle_lib.hat_links(links).astype(np.complex64)
+    hat_d, hat = gpu_hat_links(oracle_lib, dims, Nc, links)       # the block-preconditioned links come from the device
     par = oracle_lib.site_parities(dims)
     mask = torch.as_tensor(par == parity, device="cuda")
     b = synth.make_vectors(dims, Nc, 1, 8, device="cuda")
@@ -109,7 +109,7 @@ def test_cagcr_on_the_schur_hat_operator(oracle_lib, dims, Nc, parity, x_is_zero
     x = torch.zeros_like(b) if x_is_zero else 0.05 * synth.make_vectors(dims, Nc, 1, 9, device="cuda")
     x[~mask] = 0
     x0_h = x.cpu().numpy().reshape(-1)
-    op = cop.CoarseOp(dims, Nc).set_links(torch.as_tensor(hat, device="cuda"))
+    op = cop.CoarseOp(dims, Nc).set_links(hat_d)
     info = torch.zeros((cycles, 3), dtype=torch.float64, device="cuda")
     op.cagcr(b, x, s=s, cycles=cycles, x_is_zero=x_is_zero, info=info, schur_parity=parity)
     torch.cuda.synchronize()
@@ -182,13 +182,13 @@ def test_cagcr_chebyshev_on_schur_operator_and_errors(oracle_lib):
     V = synth.lattice_volume(dims)
     links = synth.make_arbitrary_links(dims, Nc, 7).numpy()
     links[:, 0] += 6.0 * np.eye(Nc, dtype=np.complex64)
-    hat = oracle_lib.hat_links(links).astype(np.complex64)
+    hat_d, hat = gpu_hat_links(oracle_lib, dims, Nc, links)
     par = oracle_lib.site_parities(dims)
     mask = torch.as_tensor(par == parity, device="cuda")
     b = synth.make_vectors(dims, Nc, 1, 8, device="cuda")
     b[~mask] = 0
     x = torch.zeros_like(b)
-    op = cop.CoarseOp(dims, Nc).set_links(torch.as_tensor(hat, device="cuda"))
+    op = cop.CoarseOp(dims, Nc).set_links(hat_d)
     info = torch.zeros((1, 3), dtype=torch.float64, device="cuda")
     op.cagcr_cheb(b, x, 0.3, 1.7, s=s, schur_parity=parity, info=info)       # Shat = 1 - Dhat Dhat: spectrum around 1
     torch.cuda.synchronize()

@@ -8,7 +8,7 @@ import torch
 
 import synth
 import paper_2212_12559_b200 as cop
-from tests.helpers import rel_l2_per_rhs
+from tests.helpers import gpu_hat_links, rel_l2_per_rhs
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-5
@@ -112,11 +112,10 @@ def test_schur_hat_operator_two_launches(oracle_lib, dims, Nc, parity, dagger):
     V = synth.lattice_volume(dims)
     links = synth.make_arbitrary_links(dims, Nc, 77).numpy()
     links[:, 0] += 2.0 * np.eye(Nc, dtype=np.complex64)
-    hat = oracle_lib.hat_links(links).astype(np.complex64)          # setup product, same bits for both sides
+    hat_d, hat = gpu_hat_links(oracle_lib, dims, Nc, links)       # built on the device; same bits for both sides
     v = synth.make_vectors(dims, Nc, 1, 78, device="cuda")
     par = torch.as_tensor(oracle_lib.site_parities(dims), device="cuda")
     v[par != parity] = 0
-    hat_d = torch.as_tensor(hat, device="cuda")
     op = cop.CoarseOp(dims, Nc).set_links(hat_d)
     t = torch.zeros_like(v)
     out = torch.full_like(v, float("nan"))
@@ -137,13 +136,14 @@ def test_schur_complement_three_launches(oracle_lib, parity):
     dims, Nc = (4, 2, 2, 4), 48
     links = synth.make_arbitrary_links(dims, Nc, 91).numpy()
     links[:, 0] += 2.0 * np.eye(Nc, dtype=np.complex64)
-    xinv = np.zeros_like(links)
-    xinv[:, 0] = np.linalg.inv(links[:, 0].astype(np.complex128)).astype(np.complex64)
     v = synth.make_vectors(dims, Nc, 1, 92, device="cuda")
     par = torch.as_tensor(oracle_lib.site_parities(dims), device="cuda")
     v[par != parity] = 0
     op = cop.CoarseOp(dims, Nc).set_links(torch.as_tensor(links, device="cuda"))
-    opi = cop.CoarseOp(dims, Nc).set_links(torch.as_tensor(xinv, device="cuda"))
+    xinv_d = torch.empty((synth.lattice_volume(dims), 9, Nc, Nc), dtype=torch.complex64, device="cuda")
+    op.build_hat_links(xinv_d, slot0=cop.HAT_SLOT0_XINV)          # X^-1 in slot 0, built on the device
+    torch.cuda.synchronize()
+    opi = cop.CoarseOp(dims, Nc).set_links(xinv_d)
     t, t2, out = torch.zeros_like(v), torch.zeros_like(v), torch.full_like(v, float("nan"))
     q = 1 - parity
     op.apply_parts(None, v, t, parity=q, local=cop.LOCAL_NONE, alpha=0.0, beta=1.0)

@@ -163,3 +163,20 @@ def test_parts_rejects_bad_arguments(oracle_lib):
         oracle_lib.coarse_apply_parts(dims, Nc, links, None, w, local=1)
     with pytest.raises(ValueError):
         oracle_lib.schur_apply((3, 2, 2, 2), Nc, np.zeros((24, 9, Nc, Nc), np.complex64), np.zeros((24, Nc, 1), np.complex64), 0)
+
+
+def test_hat_links_definition_by_multiplying_back(oracle_lib):
+    """Pin of oracle.hat_links against its definition without re-calling the solver: X . Yhat_m = Y_m for
+    m = 1..8, slot 0 = identity, or X . slot0 = identity with slot0_inverse (reading R21)."""
+    dims, Nc = (2, 2, 2, 2), 12
+    links = synth.make_gamma_hermitian_links(dims, Nc, 5).numpy().astype(np.complex128)
+    hat = oracle_lib.hat_links(links)
+    hat_inv = oracle_lib.hat_links(links, slot0_inverse=True)
+    eye = np.eye(Nc)
+    for s in range(links.shape[0]):
+        X = links[s, 0]
+        assert np.array_equal(hat[s, 0], eye)
+        assert np.abs(X @ hat_inv[s, 0] - eye).max() < 1e-12
+        for m in range(1, 9):
+            assert np.abs(X @ hat[s, m] - links[s, m]).max() < 1e-12 * max(1.0, np.abs(links[s, m]).max() * np.linalg.cond(X))
+            assert np.array_equal(hat[s, m], hat_inv[s, m])
