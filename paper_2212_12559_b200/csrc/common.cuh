@@ -67,6 +67,20 @@ __device__ __forceinline__ int stencil_site_x(const Lat& lat, int s, const SiteX
     return (x == 0) ? s + (Lmu - 1) * stride : s - stride;
 }
 
+// Site index of the h-th site of a parity (all extents even, checked by the host): consecutive
+// h walk along x0 in steps of 2, the offset in x0 alternates with x1+x2+x3.
+__device__ __forceinline__ int parity_site(const Lat& lat, int h, int parity) {
+    const unsigned half = (unsigned)lat.L[0] >> 1;
+    const unsigned q1 = (unsigned)h / half;            // = x1 + L1*(x2 + L2*x3)
+    const unsigned x0h = (unsigned)h - q1 * half;
+    const unsigned q2 = q1 / (unsigned)lat.L[1];
+    const unsigned x1 = q1 - q2 * (unsigned)lat.L[1];
+    const unsigned x3 = q2 / (unsigned)lat.L[2];
+    const unsigned x2 = q2 - x3 * (unsigned)lat.L[2];
+    const unsigned off = (x1 + x2 + x3 + (unsigned)parity) & 1u;
+    return (int)(q1 * (unsigned)lat.L[0] + 2u * x0h + off);
+}
+
 namespace ptx {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {

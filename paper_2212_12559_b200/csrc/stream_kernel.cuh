@@ -61,20 +61,6 @@ struct StreamParams {
     const float* vnorms;      // fp32 norm per site (nrhs = 1)
 };
 
-// Site index of the h-th site of a parity (all extents even, checked by the host): consecutive
-// h walk along x0 in steps of 2, the offset in x0 alternates with x1+x2+x3.
-__device__ __forceinline__ int parity_site(const Lat& lat, int h, int parity) {
-    const unsigned half = (unsigned)lat.L[0] >> 1;
-    const unsigned q1 = (unsigned)h / half;            // = x1 + L1*(x2 + L2*x3)
-    const unsigned x0h = (unsigned)h - q1 * half;
-    const unsigned q2 = q1 / (unsigned)lat.L[1];
-    const unsigned x1 = q1 - q2 * (unsigned)lat.L[1];
-    const unsigned x3 = q2 / (unsigned)lat.L[2];
-    const unsigned x2 = q2 - x3 * (unsigned)lat.L[2];
-    const unsigned off = (x1 + x2 + x3 + (unsigned)parity) & 1u;
-    return (int)(q1 * (unsigned)lat.L[0] + 2u * x0h + off);
-}
-
 constexpr int stream_pow2ceil(int v) { return v <= 1 ? 1 : v <= 2 ? 2 : v <= 4 ? 4 : v <= 8 ? 8 : v <= 16 ? 16 : 32; }
 constexpr int stream_passes(int q) {
     for (int p = 1; p <= 8; ++p)
