@@ -44,8 +44,8 @@ def sources():
 
 def units():
     """(object name, source file, extra defines) of every translation unit."""
-    out = [("coarse_op", "coarse_op.cu", []), ("launch_tensor", "launch_tensor.cu", [])]
-    for fam in ("launch_stream", "launch_stream_mr", "launch_block"):
+    out = [("coarse_op", "coarse_op.cu", []), ("link_map", "link_map.cu", [])]
+    for fam in ("launch_stream", "launch_stream_mr", "launch_block", "launch_tensor"):
         for nc in NC_SET:
             out.append((f"{fam}_nc{nc}", f"{fam}.cu", [f"-DCOARSE_NC={nc}"]))
     return out

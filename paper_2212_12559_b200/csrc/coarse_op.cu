@@ -13,6 +13,7 @@
 #include "simple_kernel.cuh"
 #include "stream_kernel.cuh"
 #include "block_kernel.cuh"
+#include "tensor_kernel.cuh"
 #include "probe_kernel.cuh"
 #include "cagcr_kernel.cuh"
 #include "hat_kernel.cuh"
@@ -142,6 +143,31 @@ int launch_block(const coarse_op* op, const void* in, void* out, int nrhs, int d
         COARSE_FOR_EACH_NC(COARSE_CASE_NC)
 #undef COARSE_CASE_NC
         default: return fail(COARSE_EUNSUPPORTED, "BLOCK path is not compiled for Nc=%d", op->Nc);
+    }
+}
+
+// TENSOR: any nrhs (groups of 16 / 8 columns, zero padded), both link formats, the parts apply included.
+// Returns the number of launches beyond the first, or a negative error code.
+int launch_tensor(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, const PartsSpec& ps, cudaStream_t stream) {
+    if (!op->link_map_ok) return fail(COARSE_EUNSUPPORTED, "TENSOR path: no tensor map for these links");
+    TensorParams p = {};
+    p.lat = op->lat;
+    p.scales = op->scales;
+    p.in = static_cast<const float2*>(in);
+    p.in_local = static_cast<const float2*>(ps.gen && ps.local != 0 ? ps.u : in);
+    p.out = static_cast<float2*>(out);
+    p.parity = ps.parity;
+    p.n_sites = ps.parity == 2 ? op->lat.V : op->lat.V / 2;
+    p.m_begin = ps.local == 1 ? 0 : 1;
+    p.identity = ps.local == 2 ? 1 : 0;
+    p.alpha = ps.alpha;
+    p.beta = ps.beta;
+    p.nrhs = nrhs;
+    switch (op->Nc) {
+#define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_tensor_nc, NC)(op, p, dagger, stream);
+        COARSE_FOR_EACH_NC(COARSE_CASE_NC)
+#undef COARSE_CASE_NC
+        default: return fail(COARSE_EUNSUPPORTED, "TENSOR path is not compiled for Nc=%d", op->Nc);
     }
 }
 
@@ -284,7 +310,7 @@ int coarse_op_set_links(coarse_op_t* op, const void* links_dev, const float* sca
         if (cudaMalloc(reinterpret_cast<void**>(&op->split_ws), bytes) == cudaSuccess) op->split_ws_bytes = bytes;
         else { cudaGetLastError(); op->split_ws = nullptr; op->split_ws_bytes = 0; }
     }
-    return make_link_map(op);
+    return make_link_maps(op);
 }
 
 int coarse_op_set_option(coarse_op_t* op, int option, int value) {
@@ -306,7 +332,7 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value) {
             }
             if (value == COARSE_PATH_TENSOR) {
                 if (!tensor_supports_nc(op->Nc, op->prec))
-                    return fail(COARSE_EUNSUPPORTED, "set_option: TENSOR path covers complex64 links with Nc in {48,64,128} (got Nc=%d, precision %d)", op->Nc, op->prec);
+                    return fail(COARSE_EUNSUPPORTED, "set_option: TENSOR path is compiled for Nc in {32,48,64,96,128,192} (got Nc=%d)", op->Nc);
                 op->path_opt = value;
                 return COARSE_OK;
             }
@@ -363,8 +389,8 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
     op->last_launches = 0;
     if (path == COARSE_PATH_TENSOR) {
         if (!tensor_supports(op->Nc, op->prec, nrhs))
-            return fail(COARSE_EUNSUPPORTED, "apply: TENSOR path covers nrhs in {8,16} (got Nc=%d nrhs=%d)", op->Nc, nrhs);
-        rc = launch_tensor(op, in_dev, out_dev, nrhs, dagger, st);
+            return fail(COARSE_EUNSUPPORTED, "apply: TENSOR path is not compiled for Nc=%d", op->Nc);
+        rc = launch_tensor(op, in_dev, out_dev, nrhs, dagger, kPlain, st);
     } else if (path == COARSE_PATH_BLOCK) {
         if (!block_supports(op->Nc, nrhs))
             return fail(COARSE_EUNSUPPORTED, "apply: BLOCK path covers nrhs <= 16 (got Nc=%d nrhs=%d)", op->Nc, nrhs);
@@ -415,19 +441,25 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
     }
     PartsSpec ps = {true, local != 0 ? u_dev : w_dev, parity, local, alpha, beta, nullptr, 0, 0};
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // 1 RHS: STREAM (GEN instantiations); more: the TENSOR kernel (parity list, alpha / beta folded into the
+    // B operand, identity term in the epilogue); shapes neither covers: SIMPLE.  BLOCK has no parts variant.
     int path = op->path_opt;
-    if (path == COARSE_PATH_AUTO || path == COARSE_PATH_TENSOR || path == COARSE_PATH_BLOCK)
-        path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM : COARSE_PATH_SIMPLE;
+    const bool tensor_ok = tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok;
+    if (path == COARSE_PATH_AUTO || path == COARSE_PATH_BLOCK || (path == COARSE_PATH_STREAM && nrhs != 1) ||
+        (path == COARSE_PATH_TENSOR && !tensor_ok))
+        path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM : tensor_ok ? COARSE_PATH_TENSOR : COARSE_PATH_SIMPLE;
     op->last_launches = 0;
     if (path == COARSE_PATH_STREAM) {
         if (!stream_supports(op->Nc, nrhs))
             return fail(COARSE_EUNSUPPORTED, "apply_parts: STREAM path does not cover Nc=%d nrhs=%d", op->Nc, nrhs);
         rc = launch_stream(op, w_dev, out_dev, dagger, ps, st);
+    } else if (path == COARSE_PATH_TENSOR) {
+        rc = launch_tensor(op, w_dev, out_dev, nrhs, dagger, ps, st);
     } else {
         rc = launch_simple(op, w_dev, out_dev, nrhs, dagger, ps, st);
     }
-    if (rc != COARSE_OK) return rc;
-    op->last_launches = 1;
+    if (rc < 0) return rc;
+    op->last_launches = 1 + rc;
     op->last_path = path;
     return COARSE_OK;
 }

@@ -1,7 +1,7 @@
 // internal.h — what the translation units of libcoarseop share: the handle, the error helpers and the
 // per-family launch entry points.  The library is built from several .cu files compiled in parallel
 // (paper_2212_12559_b200/build.py): coarse_op.cu holds the C ABI, launch_stream.cu / launch_stream_mr.cu /
-// launch_block.cu are compiled once per colour-spin size Nc (-DCOARSE_NC=...), launch_tensor.cu once.
+// launch_block.cu / launch_tensor.cu are compiled once per colour-spin size Nc (-DCOARSE_NC=...), link_map.cu once.
 #pragma once
 #include "../../include/coarse_op.h"
 
@@ -42,7 +42,7 @@ struct coarse_op {
     cudaStream_t s_h2d, s_d2h;      // apply_host's copy streams and events (created on first use)
     cudaEvent_t ev_up[4], ev_k[4], ev_done;
     bool host_pipe_ok;
-    CUtensorMap link_map;   // 2-D view of the link array for the TENSOR path (dagger = 0 slabs)
+    CUtensorMap link_map[2];   // 2-D views of the link array for the TENSOR path (dagger 0 / dagger 1 slabs, link_map.cu)
     bool link_map_ok;
 };
 
@@ -80,6 +80,7 @@ struct PartsSpec {
 
 struct StreamParams;
 struct BlockParams;
+struct TensorParams;
 
 // per-Nc entry points, one translation unit each
 #define COARSE_DECL_NC(NC)                                                                                          \
@@ -87,14 +88,14 @@ struct BlockParams;
                                          cudaStream_t stream);                                                       \
     int COARSE_CAT(launch_stream_mr_nc, NC)(const coarse_op* op, const StreamParams& p, int nrhs, int dagger,         \
                                             cudaStream_t stream);                                                    \
-    int COARSE_CAT(launch_block_nc, NC)(const coarse_op* op, const BlockParams& p, int dagger, cudaStream_t stream);
+    int COARSE_CAT(launch_block_nc, NC)(const coarse_op* op, const BlockParams& p, int dagger, cudaStream_t stream); \
+    int COARSE_CAT(launch_tensor_nc, NC)(const coarse_op* op, const TensorParams& p, int dagger, cudaStream_t stream);
 COARSE_FOR_EACH_NC(COARSE_DECL_NC)
 #undef COARSE_DECL_NC
 
-// launch_tensor.cu
+// link_map.cu
 bool tensor_supports_nc(int Nc, int prec);
 bool tensor_supports(int Nc, int prec, int nrhs);
-int make_link_map(coarse_op* op);
-int launch_tensor(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, cudaStream_t stream);
+int make_link_maps(coarse_op* op);
 
 }  // namespace coarse

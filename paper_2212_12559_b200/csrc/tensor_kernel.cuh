@@ -1,33 +1,43 @@
 // tensor_kernel.cuh — COARSE_PATH_TENSOR: the block (multi-RHS) coarse-op apply on the tcgen05
-// tensor cores, error-compensated 3xTF32.
+// tensor cores, error-compensated 3xTF32 (multi-RHS is the paper's stated
+// future work, its propagators are 3 right-hand sides at a time, L188, on 16-bit links, L99).
 //
 // Per site the block apply is a complex GEMM  out[Nc x nrhs] = [X Y...][Nc x 9Nc] . in[9Nc x nrhs].
 // A row-major interleaved-complex link matrix IS a real M = Nc x K = 2Nc operand as stored:
-//   A[i][2j] = Re M_ij, A[i][2j+1] = Im M_ij.  The vectors become a real K x N = 2Nc x 2nrhs
+//   A[i][2j] = Re M_ij, A[i][2j+1] = Im M_ij.  The vectors become a real K x N = 2Nc x 2NP
 //   operand B = [B1 | B2],   B1[2j][r] = Re v_jr, B1[2j+1][r] = -Im v_jr   (-> Re out)
 //                            B2[2j][r] = Im v_jr, B2[2j+1][r] =  Re v_jr   (-> Im out)
 // (dagger: A[i][2j] = Re M_ji, A[i][2j+1] = Im M_ji, B1 = (Re v, Im v), B2 = (Im v, -Re v)).
-// TF32 keeps 10 mantissa bits, so each fp32 operand is split x = hi + lo (hi = x with the low 13
+// TF32 keeps 11 significant bits, so each fp32 operand is split x = hi + lo (hi = x with the low 13
 // mantissa bits cleared, lo = x - hi, exact) and the product is hi.hi + hi.lo + lo.hi in fp32
-// accumulators: relative error ~2^-21 per term instead of 2^-11.
+// accumulators: relative error ~2^-21 per term instead of 2^-11.  int16 links decode
+// to 16-bit integers in fp32, for which the same split is EXACT in both halves (11 + 5 bits); the
+// per-matrix scale is folded into the B operand like the STREAM kernels fold it into the vector.
 //
 // Since the split has to touch every link entry with CUDA threads anyway, the kernel is a
-// four-role pipeline per SM (persistent, one CTA per SM, items = sites):
-//   producer (1 thread)     TMA: per stage one 16-complex-column slab of a link matrix
-//                           (dagger 0: 2-D tensor-map box Nc rows x 128 B, SWIZZLE_128B, so that
-//                            "lane = row" reads are bank-conflict free; dagger 1: 16 full rows, one
-//                            contiguous bulk copy) + the matching 16 x nrhs vector entries.
-//   converters (2 x 4 warps) read the slab (lane <-> matrix row for dagger 0, lane <-> matrix
-//                           column for dagger 1: TMEM transposes for free), split hi/lo and write
-//                           the A operand straight into TENSOR MEMORY (tcgen05.st), so the link
-//                           bytes cross shared memory exactly twice (TMA write + one LDS read);
-//                           build B hi/lo in shared memory in the canonical K-major UMMA layout.
-//   MMA issuer (1 thread)   tcgen05.mma kind::tf32, A from TMEM, B from smem, D (128 x 2nrhs fp32)
+// four-role pipeline per SM (persistent, one CTA per SM):
+//   producer (1 elected lane) TMA: per stage one slab of a link matrix = the MT output rows of the item x
+//                           16 contraction columns (dagger 0: box MT rows x 128 B | 64 B, SWIZZLE_128B |
+//                           64B, so that "lane = row" reads are bank-conflict free; dagger 1: box 16 rows x
+//                           MT entries, lane = column).
+//   converters (2 x 4 warps) read the slab (lane <-> output index: TMEM transposes for free), decode /
+//                           split hi/lo and write the A operand straight into TENSOR MEMORY (tcgen05.st),
+//                           so the link bytes cross shared memory exactly twice (TMA write + one LDS
+//                           read); fetch the 16 x NP vector entries of the stage from global memory (L2
+//                           resident, prefetched one stage ahead into registers: any nrhs, any row pitch,
+//                           zero padding for free), scale, split and store B hi/lo in shared memory in
+//                           the canonical K-major UMMA layout.
+//   MMA issuer (1 elected lane) tcgen05.mma kind::tf32, A from TMEM, B from smem, D (128 x 2NP fp32)
 //                           in TMEM, 8 MMAs per stage (4 k-steps x {A_hi.[B_hi|B_lo], A_lo.B_hi}), one accumulator
 //                           slot per link matrix; tcgen05.commit releases the operand slot / publishes D.
 //   epilogue (4 warps)      tcgen05.ld D -> registers, adds the nine per-matrix partial results in
 //                           round-to-nearest fp32 -> out[s][i][r]; a ring of 4 accumulator slots lets
 //                           the next matrices' MMAs overlap the read-out.
+// Work item = (site, tile of MT = Nc / NT output indices); NT = 2 for Nc = 192 (M = 128 per MMA).
+// One launch handles NP = 8 or 16 right-hand-side columns [r0, r0 + width) of vectors with `nrhs`
+// columns; columns >= width are zero-padded in B and not stored (nrhs = 3 runs as NP = 8, nrhs = 40 as
+// three launches).  The parts apply (coarse_op_apply_parts: parity-restricted site list, X stage on/off,
+// alpha / beta folded into B, identity term added in the epilogue) is the same kernel with runtime flags.
 // Summation order is fixed: results are bit-identical run to run.
 #pragma once
 #include <cuda.h>
@@ -38,22 +48,35 @@ namespace coarse {
 
 struct TensorParams {
     Lat lat;
-    const unsigned char* links;
-    const float2* in;
+    const float* scales;      // int16 links: fp32 scale per (site, matrix)
+    const float2* in;         // w: operand of the hopping terms (plain apply: the input vector)
+    const float2* in_local;   // u: operand of the X term and of the identity term (plain apply: = in)
     float2* out;
-    int n_sites;
+    int n_sites;              // sites of the parity set (plain apply: V)
+    int parity;               // 0 even, 1 odd, 2 all sites
+    int m_begin;              // 0: the X stage runs; 1: it is skipped (local = none | identity)
+    int identity;             // 1: add alpha * u(x) to the result
+    float alpha, beta;        // out = alpha * Loc + beta * Hop (plain apply: 1, 1)
+    int nrhs;                 // right-hand sides stored per vector entry (row pitch of in / out)
+    int r0, width;            // this launch computes columns [r0, r0 + width), width <= NP
 };
 
-template <int NC, int NRHS>
+constexpr int tensor_clamp(int v, int lo, int hi) { return v < lo ? lo : v > hi ? hi : v; }
+
+template <int NC, bool I16, int NP>
 struct TensorGeom {
+    static constexpr int NT = NC > 128 ? 2 : 1;         // output tiles per site
+    static constexpr int MT = NC / NT;                  // output indices per item (<= 128 TMEM lanes)
+    static constexpr int ENTRY = I16 ? 4 : 8;           // bytes per complex link entry
     static constexpr int KSTAGE = 32;                   // real k per stage = 16 complex columns
-    static constexpr int CHUNKS = 2 * NC / KSTAGE;      // stages per link matrix
-    static constexpr int LINK_STAGE = NC * 128;         // bytes per stage (both dagger modes)
-    static constexpr int VEC_STAGE = 16 * NRHS * 8;
-    static constexpr int N = 2 * NRHS;                  // MMA N: [Re out | Im out]
+    static constexpr int CHUNKS = NC / 16;              // stages per link matrix
+    static constexpr int SLAB_ROW = 16 * ENTRY;         // dagger 0: bytes per slab row (128 | 64)
+    static constexpr int LINK_STAGE = MT * 16 * ENTRY;  // bytes per stage (both dagger modes)
+    static constexpr int N = 2 * NP;                    // MMA N: [Re out | Im out]
+    static constexpr int NE = NP / 8;                   // B entries per converter thread and stage
     static constexpr int B_HALF = KSTAGE * N * 4;       // B hi (or lo) bytes per stage
     static constexpr int B_SBO = (KSTAGE / 4) * 128;    // byte stride between 8-column groups of n
-    static constexpr int LS = 8;                        // link ring depth (TMA -> converters)
+    static constexpr int LS = tensor_clamp(131072 / LINK_STAGE, 4, 16);   // link ring depth (TMA -> converters)
     static constexpr int AS = 4;                        // operand ring depth (converters -> MMA)
     static constexpr int A_COLS = 2 * KSTAGE;           // TMEM columns per operand stage: hi | lo
     static constexpr int D_COL0 = AS * A_COLS;
@@ -62,8 +85,8 @@ struct TensorGeom {
     static constexpr int TMEM_COLS = 512;
     static constexpr int THREADS = 16 * 32;
     static constexpr int NBAR = 2 * LS + 2 * AS + 2 * DS;
-    static constexpr int SMEM_BYTES = 1024 + LS * LINK_STAGE + LS * VEC_STAGE + AS * 2 * B_HALF + NBAR * 8 + 16;
-    static constexpr bool OK = (NC % 16 == 0) && NC <= 128 && (NRHS % 8 == 0) && NRHS <= 16 &&
+    static constexpr int SMEM_BYTES = 1024 + LS * LINK_STAGE + AS * 2 * B_HALF + NBAR * 8 + 16;
+    static constexpr bool OK = (NC % 16 == 0) && (MT % 8 == 0) && MT <= 128 && CHUNKS >= 2 && (NP == 8 || NP == 16) &&
                                (D_COL0 + DS * D_COLS <= TMEM_COLS) && SMEM_BYTES <= 232448;
 };
 
@@ -120,6 +143,11 @@ __device__ __forceinline__ void fence_cta() { asm volatile("fence.acq_rel.cta;" 
 __device__ __forceinline__ void sts64(uint32_t addr, float a, float b) {
     asm volatile("st.shared.v2.f32 [%0], {%1,%2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
 }
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
 
 }  // namespace ptx
 
@@ -140,14 +168,13 @@ __device__ __forceinline__ uint64_t umma_desc_kmajor(uint32_t smem_addr, uint32_
     return d;                // base_offset 0, layout_type 0 = SWIZZLE_NONE
 }
 
-template <int NC, int NRHS, bool DAG>
-__global__ void __launch_bounds__(TensorGeom<NC, NRHS>::THREADS, 1)
+template <int NC, bool I16, int NP, bool DAG>
+__global__ void __launch_bounds__(TensorGeom<NC, I16, NP>::THREADS, 1)
 coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p) {
-    using Gm = TensorGeom<NC, NRHS>;
+    using Gm = TensorGeom<NC, I16, NP>;
     static_assert(Gm::OK, "unsupported TENSOR geometry");
-    constexpr int LS = Gm::LS, AS = Gm::AS, DS = Gm::DS, CHUNKS = Gm::CHUNKS, N = Gm::N;
-    constexpr int LINK_STAGE = Gm::LINK_STAGE, VEC_STAGE = Gm::VEC_STAGE, B_HALF = Gm::B_HALF, B_SBO = Gm::B_SBO;
-    constexpr int STAGES_PER_SITE = 9 * CHUNKS;
+    constexpr int LS = Gm::LS, AS = Gm::AS, DS = Gm::DS, CHUNKS = Gm::CHUNKS, N = Gm::N, NT = Gm::NT, MT = Gm::MT, NE = Gm::NE;
+    constexpr int LINK_STAGE = Gm::LINK_STAGE, B_HALF = Gm::B_HALF, B_SBO = Gm::B_SBO, ENTRY = Gm::ENTRY;
     // instruction descriptor: D fp32, A/B tf32, both K-major, N, M = 128
     constexpr uint32_t IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
     constexpr uint32_t IDESC2 = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(2 * N >> 3) << 17) | ((128u >> 4) << 24);
@@ -156,8 +183,7 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
     extern __shared__ unsigned char smem_raw[];
     const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t link_u32 = base;
-    const uint32_t vec_u32 = link_u32 + LS * LINK_STAGE;
-    const uint32_t b_u32 = vec_u32 + LS * VEC_STAGE;
+    const uint32_t b_u32 = link_u32 + LS * LINK_STAGE;
     const uint32_t bar_u32 = b_u32 + AS * 2 * B_HALF;
     const uint32_t full0 = bar_u32, empty0 = full0 + 8u * LS;
     const uint32_t abfull0 = empty0 + 8u * LS, abempty0 = abfull0 + 8u * AS;
@@ -188,39 +214,43 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-    const int n_my = (p.n_sites > (int)blockIdx.x) ? (p.n_sites - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    const int n_items = p.n_sites * NT;
+    const int n_my = (n_items > (int)blockIdx.x) ? (n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    const int M0 = p.m_begin;
+    const int n_mat_item = 9 - M0;                                   // link matrices per item
+    auto site_of_item = [&](int item) -> int {
+        const int h = NT == 1 ? item : item / NT;
+        return p.parity != 2 ? parity_site(p.lat, h, p.parity) : h;
+    };
 
     if (warp == 0) {
         // ---------------------------------------------------------------- TMA producer
         // (whole warp in uniform control flow, one elected lane issues: see the MMA issuer below)
         const uint64_t pol_links = ptx::policy_evict_first();
-        const uint64_t pol_vec = ptx::policy_evict_last();
         uint32_t t = 0;
         for (int it = 0; it < n_my; ++it) {
-            const int s = blockIdx.x + it * gridDim.x;
+            const int item = blockIdx.x + it * gridDim.x;
+            const int s = site_of_item(item);
+            const int i0 = NT == 1 ? 0 : (item % NT) * MT;
             const SiteX cx = site_coords(p.lat, s);
 #pragma unroll
             for (int m = 0; m < 9; ++m) {
+                if (m < M0) continue;
                 const int sv = stencil_site_x(p.lat, s, cx, m, DAG ? 1 : 0);
                 const int sm = DAG ? sv : s;
-                const int64_t mat_row0 = ((int64_t)sm * 9 + m) * NC;
-                const float2* vec = p.in + (int64_t)sv * NC * NRHS;
+                const int mat_row0 = (sm * 9 + m) * NC;             // < 2^31: checked by the host (make_link_maps)
 #pragma unroll 1
                 for (int c = 0; c < CHUNKS; ++c, ++t) {
                     const uint32_t slot = t % LS, ph = (t / LS) & 1u;
                     ptx::mbar_wait(empty0 + 8u * slot, ph ^ 1u);
                     if (ptx::elect_one()) {
-                        ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE + VEC_STAGE);
-                        if (!DAG) {
-                            ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, c * 32, (int)mat_row0,
+                        ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE);
+                        if (!DAG)      // rows [i0, i0 + MT) x complex columns [16c, 16c + 16)
+                            ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, c * (16 * ENTRY / 4), mat_row0 + i0,
                                              full0 + 8u * slot, pol_links);
-                        } else {
-                            ptx::bulk_g2s(link_u32 + slot * LINK_STAGE,
-                                          p.links + (mat_row0 + 16 * c) * (int64_t)(NC * 8), LINK_STAGE,
-                                          full0 + 8u * slot, pol_links);
-                        }
-                        ptx::bulk_g2s(vec_u32 + slot * VEC_STAGE, vec + (int64_t)16 * c * NRHS, VEC_STAGE,
-                                      full0 + 8u * slot, pol_vec);
+                        else           // rows [16c, 16c + 16) x complex columns [i0, i0 + MT)
+                            ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, i0 * (ENTRY / 4), mat_row0 + 16 * c,
+                                             full0 + 8u * slot, pol_links);
                     }
                     __syncwarp();
                 }
@@ -235,11 +265,11 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
         //
         // One accumulator slot per link matrix: the tensor core truncates (rounds toward zero) when it
         // adds into the fp32 accumulator, a bias that grows linearly with the chain length, so the
-        // chains are kept short (32 MMAs for hi.hi, 64 for the two cross terms, which are 2^-11
-        // smaller and live in their own columns) and the nine partial results are added with
+        // chains are kept short (4 CHUNKS MMAs for hi.hi, 8 CHUNKS for the two cross terms, which are
+        // 2^-11 smaller and live in their own columns) and the nine partial results are added with
         // round-to-nearest fp32 in the epilogue.
         uint32_t t = 0;
-        const uint32_t n_mat = (uint32_t)n_my * 9u;
+        const uint32_t n_mat = (uint32_t)n_my * (uint32_t)n_mat_item;
         for (uint32_t tm = 0; tm < n_mat; ++tm) {
             const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
             ptx::mbar_wait(dempty0 + 8u * ds, dph ^ 1u);
@@ -271,46 +301,122 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
         // ---------------------------------------------------------------- converters
         const int grp = (warp - 4) >> 2;              // stages t with t % 2 == grp
         const int q = warp & 3;                       // TMEM lane quadrant of this warp
-        const int row = q * 32 + lane;                // A-operand row = output index i
+        const int row = q * 32 + lane;                // A-operand row = output index i (inside the item's tile)
         const int gtid = (warp & 3) * 32 + lane;      // 0..127 inside the group
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
-        const uint32_t total = (uint32_t)n_my * STAGES_PER_SITE;
+        const uint32_t total = (uint32_t)n_my * (uint32_t)(n_mat_item * CHUNKS);
+
+        // B entries of this thread, the same (contraction row j, column r) in every stage.  A half-warp
+        // covers the 16 distinct 8-byte bank slots (k mod 4 pair, n mod 8) of the K-major layout, so its
+        // stores are conflict-free (e = gtid + 128 x: r = e & 7 [+ 8], j = 2 (e >> 4 [>> 1]) + ((e >> 3) & 1)).
+        int b_off_vec[NE];           // element offset inside the stage's 16 x nrhs block
+        uint32_t b_o1[NE], b_o2[NE]; // byte offsets of the (n = r) and (n = NP + r) entries in the B tile
+        bool b_valid[NE];
+#pragma unroll
+        for (int x = 0; x < NE; ++x) {
+            const int e = gtid + 128 * x;
+            const int rest = e >> 4;
+            const int r = (e & 7) + (NP == 16 ? (rest & 1) * 8 : 0);
+            const int j = 2 * (NP == 16 ? rest >> 1 : rest) + ((e >> 3) & 1);
+            b_valid[x] = r < p.width;
+            b_off_vec[x] = j * p.nrhs + r;
+            const uint32_t koff = (uint32_t)(j >> 1) * 128u + (uint32_t)(j & 1) * 8u;
+            b_o1[x] = koff + (uint32_t)(r >> 3) * B_SBO + (uint32_t)(r & 7) * 16u;
+            b_o2[x] = koff + (uint32_t)((NP + r) >> 3) * B_SBO + (uint32_t)((NP + r) & 7) * 16u;
+        }
+
+        // cursor of the NEXT stage of this group (its vector entries are prefetched while the current
+        // stage is converted): item index, matrix, chunk, and what depends on them
+        int n_it = 0, n_m = M0, n_c = grp, n_s = 0;
+        SiteX n_cx = {};
+        const float2* n_vec = p.in;
+        float n_sc = 1.f;
+        auto load_item = [&]() {
+            if (n_it < n_my) {
+                n_s = site_of_item(blockIdx.x + n_it * gridDim.x);
+                n_cx = site_coords(p.lat, n_s);
+            }
+        };
+        auto load_matrix = [&]() {
+            if (n_it < n_my) {
+                const int sv = stencil_site_x(p.lat, n_s, n_cx, n_m, DAG ? 1 : 0);
+                const int sm = DAG ? sv : n_s;
+                n_vec = (n_m == 0 ? p.in_local : p.in) + (int64_t)sv * NC * p.nrhs + p.r0;
+                n_sc = n_m == 0 ? p.alpha : p.beta;
+                if constexpr (I16) n_sc *= __ldg(p.scales + (int64_t)sm * 9 + n_m);
+            }
+        };
+        float2 vn[NE];
+        auto fetch = [&]() {
+#pragma unroll
+            for (int x = 0; x < NE; ++x)
+                vn[x] = (n_it < n_my && b_valid[x]) ? __ldg(n_vec + (int64_t)(16 * n_c) * p.nrhs + b_off_vec[x]) : make_float2(0.f, 0.f);
+        };
+        load_item();
+        load_matrix();
+        fetch();
+
         for (uint32_t t = grp; t < total; t += 2) {
             const uint32_t slot = t % LS, ph = (t / LS) & 1u;
             const uint32_t as = t % AS, aph = (t / AS) & 1u;
+            // this stage's vector entries and scale; then move the cursor two stages on and prefetch
+            float2 v[NE];
+#pragma unroll
+            for (int x = 0; x < NE; ++x) v[x] = vn[x];
+            const float sc = n_sc;
+            n_c += 2;
+            if (n_c >= CHUNKS) {
+                n_c -= CHUNKS;
+                if (++n_m == 9) { n_m = M0; ++n_it; load_item(); }
+                load_matrix();
+            }
+            fetch();
+
             ptx::mbar_wait(full0 + 8u * slot, ph);
-            uint32_t a[32];
-            if (row < NC) {
-                if (!DAG) {
-                    const uint32_t rb = link_u32 + slot * LINK_STAGE + row * 128;
+            float a[32];
+            if (row < MT) {
+                const uint32_t sb = link_u32 + slot * LINK_STAGE;
+                if constexpr (!DAG && !I16) {
+                    const uint32_t rb = sb + row * 128;            // SWIZZLE_128B: chunk u of row at u ^ (row & 7)
 #pragma unroll
                     for (int u = 0; u < 8; ++u) {
-                        const uint4 x = ptx::lds128u(rb + (((uint32_t)u ^ ((uint32_t)row & 7u)) << 4));
+                        const float4 x = ptx::lds128(rb + (((uint32_t)u ^ ((uint32_t)row & 7u)) << 4));
                         a[4 * u] = x.x; a[4 * u + 1] = x.y; a[4 * u + 2] = x.z; a[4 * u + 3] = x.w;
                     }
-                } else {
-                    const uint32_t cb = link_u32 + slot * LINK_STAGE + row * 8;
+                } else if constexpr (!DAG && I16) {
+                    const uint32_t rb = sb + row * 64;             // SWIZZLE_64B: chunk u of row at u ^ ((row >> 1) & 3)
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const uint4 x = ptx::lds128u(rb + (((uint32_t)u ^ (((uint32_t)row >> 1) & 3u)) << 4));
+                        const float2 e0 = unpack_i16x2(x.x), e1 = unpack_i16x2(x.y), e2 = unpack_i16x2(x.z), e3 = unpack_i16x2(x.w);
+                        a[8 * u] = e0.x; a[8 * u + 1] = e0.y; a[8 * u + 2] = e1.x; a[8 * u + 3] = e1.y;
+                        a[8 * u + 4] = e2.x; a[8 * u + 5] = e2.y; a[8 * u + 6] = e3.x; a[8 * u + 7] = e3.y;
+                    }
+                } else if constexpr (DAG && !I16) {
+                    const uint32_t cb = sb + row * 8;              // [16 rows][MT entries], lane = column
 #pragma unroll
                     for (int jj = 0; jj < 16; ++jj) {
-                        const float2 x = ptx::lds64(cb + jj * (NC * 8));
-                        a[2 * jj] = __float_as_uint(x.x); a[2 * jj + 1] = __float_as_uint(x.y);
+                        const float2 x = ptx::lds64(cb + jj * (MT * 8));
+                        a[2 * jj] = x.x; a[2 * jj + 1] = x.y;
+                    }
+                } else {
+                    const uint32_t cb = sb + row * 4;
+#pragma unroll
+                    for (int jj = 0; jj < 16; ++jj) {
+                        const float2 x = unpack_i16x2(ptx::lds32(cb + jj * (MT * 4)));
+                        a[2 * jj] = x.x; a[2 * jj + 1] = x.y;
                     }
                 }
             } else {
 #pragma unroll
-                for (int u = 0; u < 32; ++u) a[u] = 0u;
+                for (int u = 0; u < 32; ++u) a[u] = 0.f;
             }
-            float2 v[NRHS / 8];
-#pragma unroll
-            for (int x = 0; x < NRHS / 8; ++x) v[x] = ptx::lds64(vec_u32 + slot * VEC_STAGE + (gtid + 128 * x) * 8);
-#ifndef COARSE_EXP_LATE_RELEASE
             // The loaded values are not consumed before the release below, and SYNCS.ARRIVE does not wait
             // for in-flight LDS: without this fence the producer's next TMA write into the slot can overtake
             // the reads (seen on B200 as sporadic stale 512-byte runs).  The fence completes the loads.
             ptx::fence_cta();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);      // link slot back to the producer
-#endif
 
             ptx::mbar_wait(abempty0 + 8u * as, aph ^ 1u);            // MMAs that read this operand slot are done
             ptx::tc_fence_after();
@@ -319,39 +425,32 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
 #pragma unroll
-                for (int u = 0; u < 16; ++u) split_tf32(__uint_as_float(a[16 * h + u]), hi[u], lo[u]);
+                for (int u = 0; u < 16; ++u) split_tf32(a[16 * h + u], hi[u], lo[u]);
                 ptx::tmem_st16(a_hi + 16 * h, hi);
                 ptx::tmem_st16(a_lo + 16 * h, lo);
             }
             const uint32_t b_hi = b_u32 + as * 2 * B_HALF, b_lo = b_hi + B_HALF;
 #pragma unroll
-            for (int x = 0; x < NRHS / 8; ++x) {
-                const int e = gtid + 128 * x;
-                const int j = e / NRHS, r = e % NRHS;
-                // k = 2j, 2j+1 -> one 8-byte store; n = r (-> Re out) and n = NRHS + r (-> Im out)
-                const uint32_t koff = (uint32_t)(j >> 1) * 128u + (uint32_t)(j & 1) * 8u;
-                const uint32_t o1 = koff + (uint32_t)(r >> 3) * B_SBO + (uint32_t)(r & 7) * 16u;
-                const uint32_t o2 = koff + (uint32_t)((NRHS + r) >> 3) * B_SBO + (uint32_t)((NRHS + r) & 7) * 16u;
-                const float b1x = v[x].x, b1y = DAG ? v[x].y : -v[x].y;
-                const float b2x = v[x].y, b2y = DAG ? -v[x].x : v[x].x;
+            for (int x = 0; x < NE; ++x) {
+                // k = 2j, 2j+1 -> one 8-byte store; n = r (-> Re out) and n = NP + r (-> Im out)
+                const float vx = v[x].x * sc, vy = v[x].y * sc;
+                const float b1x = vx, b1y = DAG ? vy : -vy;
+                const float b2x = vy, b2y = DAG ? -vx : vx;
                 uint32_t h0, l0, h1, l1;
                 split_tf32(b1x, h0, l0);
                 split_tf32(b1y, h1, l1);
-                ptx::sts64(b_hi + o1, __uint_as_float(h0), __uint_as_float(h1));
-                ptx::sts64(b_lo + o1, __uint_as_float(l0), __uint_as_float(l1));
+                ptx::sts64(b_hi + b_o1[x], __uint_as_float(h0), __uint_as_float(h1));
+                ptx::sts64(b_lo + b_o1[x], __uint_as_float(l0), __uint_as_float(l1));
                 split_tf32(b2x, h0, l0);
                 split_tf32(b2y, h1, l1);
-                ptx::sts64(b_hi + o2, __uint_as_float(h0), __uint_as_float(h1));
-                ptx::sts64(b_lo + o2, __uint_as_float(l0), __uint_as_float(l1));
+                ptx::sts64(b_hi + b_o2[x], __uint_as_float(h0), __uint_as_float(h1));
+                ptx::sts64(b_lo + b_o2[x], __uint_as_float(l0), __uint_as_float(l1));
             }
             ptx::tc_wait_st();
             ptx::fence_proxy_async();
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(abfull0 + 8u * as);
-#ifdef COARSE_EXP_LATE_RELEASE
-            if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
-#endif
         }
     } else if (warp >= 12) {
         // ---------------------------------------------------------------- epilogue
@@ -360,12 +459,14 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         uint32_t tm = 0;
         for (int it = 0; it < n_my; ++it) {
-            const int s = blockIdx.x + it * gridDim.x;
+            const int item = blockIdx.x + it * gridDim.x;
+            const int s = site_of_item(item);
+            const int i0 = NT == 1 ? 0 : (item % NT) * MT;
             float acc[N];
 #pragma unroll
             for (int n = 0; n < N; ++n) acc[n] = 0.f;
 #pragma unroll 1
-            for (int m = 0; m < 9; ++m, ++tm) {
+            for (int m = M0; m < 9; ++m, ++tm) {
                 const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
                 ptx::mbar_wait(dfull0 + 8u * ds, dph);
                 ptx::tc_fence_after();
@@ -380,11 +481,29 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
 #pragma unroll
                 for (int n = 0; n < N; ++n) acc[n] += __uint_as_float(d[n]) + __uint_as_float(d[N + n]);
             }
-            if (row < NC) {
-                float4* o = reinterpret_cast<float4*>(p.out + ((int64_t)s * NC + row) * NRHS);
+            if (row < MT) {
+                const int64_t o = ((int64_t)s * NC + i0 + row) * p.nrhs + p.r0;
+                if (p.identity) {
 #pragma unroll
-                for (int r = 0; r < NRHS; r += 2)
-                    o[r >> 1] = make_float4(acc[r], acc[NRHS + r], acc[r + 1], acc[NRHS + r + 1]);
+                    for (int r = 0; r < NP; ++r)
+                        if (r < p.width) {
+                            const float2 u = __ldg(p.in_local + o + r);
+                            acc[r] = fmaf(p.alpha, u.x, acc[r]);
+                            acc[NP + r] = fmaf(p.alpha, u.y, acc[NP + r]);
+                        }
+                }
+                if (((p.nrhs | p.r0) & 1) == 0) {
+                    float4* o4 = reinterpret_cast<float4*>(p.out + o);
+#pragma unroll
+                    for (int r = 0; r < NP; r += 2) {
+                        if (r + 1 < p.width) o4[r >> 1] = make_float4(acc[r], acc[NP + r], acc[r + 1], acc[NP + r + 1]);
+                        else if (r < p.width) p.out[o + r] = make_float2(acc[r], acc[NP + r]);
+                    }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < NP; ++r)
+                        if (r < p.width) p.out[o + r] = make_float2(acc[r], acc[NP + r]);
+                }
             }
         }
     }

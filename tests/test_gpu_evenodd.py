@@ -47,7 +47,7 @@ def _check_parts(oracle_lib, dims, Nc, prec, nrhs, dagger, parity, local, path, 
     op.apply_parts(u if local else None, w, out, nrhs=nrhs, dagger=dagger, parity=parity, local=local,
                    alpha=alpha, beta=beta)
     torch.cuda.synchronize()
-    assert op.last_path == path and op.last_launches == 1
+    assert op.last_path == path and op.last_launches == (1 if path != cop.PATH_TENSOR else (nrhs + 15) // 16)
     ref = oracle_lib.coarse_apply_parts(dims, Nc, links_h, u.cpu().numpy() if local else None, w.cpu().numpy(),
                                         nrhs=nrhs, dagger=dagger, parity=parity, local=local, alpha=alpha,
                                         beta=beta, link_precision=prec, scales=scales_h)
@@ -88,6 +88,32 @@ def test_parts_stream_other_nc_and_fine_geometry(oracle_lib, Nc, dagger):
 def test_parts_simple(oracle_lib, nrhs, dagger, parity, local):
     _check_parts(oracle_lib, (4, 2, 2, 4), 8, cop.LINK_C64, nrhs, dagger, parity, local, cop.PATH_SIMPLE)
     _check_parts(oracle_lib, (2, 2, 2, 2), 48, cop.LINK_I16, nrhs, dagger, parity, local, cop.PATH_SIMPLE)
+
+
+@pytest.mark.parametrize("Nc", [48, 64, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("nrhs", [3, 8, 16, 18])
+@pytest.mark.parametrize("dagger", [0, 1])
+@pytest.mark.parametrize("parity", [0, 1, 2])
+@pytest.mark.parametrize("local", [0, 1, 2])
+def test_parts_tensor(oracle_lib, Nc, prec, nrhs, dagger, parity, local):
+    """Multi-RHS parts apply on the TENSOR kernel: parity-restricted site list, X stage on / off, alpha and
+    beta folded into the B operand, identity term added in the epilogue (L127/L135 + L200)."""
+    dims = (2, 2, 4, 2) if Nc >= 128 else (4, 2, 2, 4)
+    _check_parts(oracle_lib, dims, Nc, prec, nrhs, dagger, parity, local, cop.PATH_TENSOR)
+
+
+def test_parts_auto_routes_multi_rhs_to_tensor():
+    dims, Nc, nrhs = (2, 2, 2, 2), 48, 5
+    links = synth.make_arbitrary_links(dims, Nc, 5, device="cuda")
+    u = synth.make_vectors(dims, Nc, nrhs, 6, device="cuda")
+    w = synth.make_vectors(dims, Nc, nrhs, 7, device="cuda")
+    out = torch.zeros_like(u)
+    op = cop.CoarseOp(dims, Nc).set_links(links)
+    op.apply_parts(u, w, out, nrhs=nrhs, parity=cop.PARITY_EVEN, local=cop.LOCAL_X, alpha=1.0, beta=-1.0)
+    torch.cuda.synchronize()
+    assert op.last_path == cop.PATH_TENSOR
+    op.close()
 
 
 def test_parts_all_sites_equals_plain_apply():

@@ -129,6 +129,23 @@ def test_tensor_path_block_apply(oracle_lib, dims, Nc, nrhs, dagger):
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (1, 1, 1, 1)])
 @pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
 @pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("nrhs", [1, 3, 7, 8, 11, 16, 19, 40])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_tensor_path_every_shape(oracle_lib, dims, Nc, prec, nrhs, dagger):
+    """The TENSOR kernel on every compiled Nc (Nc = 192: two output tiles per site), both link formats
+    (int16: the paper's storage, decoded and split exactly), any nrhs: zero-padded 8- / 16-wide
+    column tiles (3 = one propagator; odd row pitches), several launches beyond 16."""
+    if Nc >= 128 and dims == (4, 4, 4, 4):
+        dims = (2, 4, 2, 2)               # keep the oracle's run time in seconds
+    if nrhs == 40 and dims == (4, 4, 4, 4):
+        dims = (2, 2, 2, 4)
+    err = _run(oracle_lib, dims, Nc, prec, nrhs, dagger, cop.PATH_TENSOR, hermitian=(nrhs != 7))
+    assert err <= 3e-6, f"3xTF32 with per-matrix accumulator chains should sit near 1e-6, got {err:.2e}"
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (1, 1, 1, 1)])
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
 @pytest.mark.parametrize("nrhs", [2, 3, 8, 11, 16])
 @pytest.mark.parametrize("dagger", [0, 1])
 def test_block_path_cuda_cores(oracle_lib, dims, Nc, prec, nrhs, dagger):
@@ -172,9 +189,9 @@ def test_auto_path_selection():
     dims = (2, 2, 2, 2)
     cases = [(48, cop.LINK_C64, 1, cop.PATH_STREAM), (48, cop.LINK_C64, 16, cop.PATH_TENSOR),
              (48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_STREAM),
-             (48, cop.LINK_C64, 5, cop.PATH_BLOCK), (64, cop.LINK_I16, 16, cop.PATH_BLOCK),
-             (96, cop.LINK_C64, 8, cop.PATH_BLOCK), (48, cop.LINK_C64, 17, cop.PATH_SIMPLE),
-             (6, cop.LINK_C64, 2, cop.PATH_SIMPLE)]
+             (48, cop.LINK_C64, 5, cop.PATH_TENSOR), (64, cop.LINK_I16, 16, cop.PATH_TENSOR),
+             (96, cop.LINK_C64, 8, cop.PATH_TENSOR), (48, cop.LINK_C64, 17, cop.PATH_TENSOR),
+             (192, cop.LINK_I16, 12, cop.PATH_TENSOR), (6, cop.LINK_C64, 2, cop.PATH_SIMPLE)]
     for Nc, prec, nrhs, want in cases:
         V = 16
         if prec == cop.LINK_C64:
@@ -220,17 +237,21 @@ def test_tensor_path_matches_cuda_core_path_and_is_reproducible():
 
 def test_tensor_path_unsupported_shapes():
     L = cop.lib()
-    h = cop.coarse_op_create((2, 2, 2, 2), 128, cop.LINK_I16)
+    h = cop.coarse_op_create((2, 2, 2, 2), 80, cop.LINK_I16)          # Nc outside the compiled set
     assert L.coarse_op_set_option(h, cop.OPT_PATH, cop.PATH_TENSOR) == cop.EUNSUPPORTED
     cop.coarse_op_destroy(h)
+
+
+def test_tensor_launch_count_beyond_16_rhs():
     dims, Nc = (2, 2, 2, 2), 64
     links = synth.make_arbitrary_links(dims, Nc, 3, device="cuda")
-    vin = synth.make_vectors(dims, Nc, 3, 4, device="cuda")
-    vout = torch.empty_like(vin)
     op = cop.CoarseOp(dims, Nc).set_links(links).set_option(cop.OPT_PATH, cop.PATH_TENSOR)
-    with pytest.raises(cop.CoarseOpError) as e:
-        op.apply(vin, vout, nrhs=3)
-    assert e.value.code == cop.EUNSUPPORTED
+    for nrhs, want in ((3, 1), (16, 1), (17, 2), (40, 3)):
+        vin = synth.make_vectors(dims, Nc, nrhs, 4, device="cuda")
+        vout = torch.empty_like(vin)
+        op.apply(vin, vout, nrhs=nrhs)
+        torch.cuda.synchronize()
+        assert op.last_launches == want and op.last_path == cop.PATH_TENSOR
     op.close()
 
 
