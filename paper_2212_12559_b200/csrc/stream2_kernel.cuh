@@ -47,6 +47,20 @@
 #define COARSE_S2_XU_D 1
 #endif
 
+// Complex MAC formulation (stream_kernel.cuh): 1 = matrix entry as the packed FFMA2 operand with two packed partial
+// sums per accumulator (cmacp: no register-pair duplication MOVs, 300 -> 246 instructions per stage and lane),
+// 0 = cmac<> (vector as the packed operand).  A/B in one gpurun call, 100-step loops, two repetitions each, int16
+// links: dagger = 0 is SLOWER with the shorter instruction stream (C4 2.19 -> 2.27 ms, Nc = 128 0.513 -> 0.539 ms:
+// 16 more live registers for the duplicated vector pairs and no issue-slot shortage left to relieve), dagger = 1 is
+// 1 % faster (C4 2.235 -> 2.209 ms, Nc = 128 0.5072 -> 0.5026 ms).  The multi-RHS kernel (stream_mr_kernel.cuh),
+// which IS issue-bound, gains 6-19 % from it in both modes.
+#ifndef COARSE_S2_PACKED_N
+#define COARSE_S2_PACKED_N 0
+#endif
+#ifndef COARSE_S2_PACKED_D
+#define COARSE_S2_PACKED_D 1
+#endif
+
 namespace coarse {
 
 constexpr int stream2_rows(int nc, int rowbytes, int unit, int max_bytes, int max_loads) {
@@ -242,6 +256,56 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
         next2_scale = fetch_scale(item + 2 * item_stride);
 
         if constexpr (!DAG) {
+#if COARSE_S2_PACKED_N
+            CAcc pacc[WL];
+#pragma unroll
+            for (int k = 0; k < WL; ++k) pacc[k].a = pacc[k].b = make_float2(0.f, 0.f);
+#pragma unroll 1
+            for (int m = 0; m < 9; ++m) {
+                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                ptx::mbar_wait(full0 + 8u * slot, phase);
+                const uint32_t lbase = link_u32 + slot * LINK_STAGE + (row0 * ROWBYTES + qi * 16);
+                const uint32_t vbase = vec_u32 + slot * VEC_STAGE;
+                VDup v[PASSES][CPQ];
+#pragma unroll
+                for (int ps = 0; ps < PASSES; ++ps) {
+                    const int col0 = (ps * QP + qi) * CPQ;
+#pragma unroll
+                    for (int h = 0; h < CPQ / 2; ++h) {
+                        float4 t = ptx::lds128(vbase + (col0 + 2 * h) * 8);
+                        if constexpr (I16) { t.x *= sc; t.y *= sc; t.z *= sc; t.w *= sc; }
+                        v[ps][2 * h] = vdup(make_float2(t.x, t.y));
+                        v[ps][2 * h + 1] = vdup(make_float2(t.z, t.w));
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < WL; ++k) {
+#pragma unroll
+                    for (int ps = 0; ps < PASSES; ++ps) {
+                        const uint32_t a = lbase + k * (RPL * ROWBYTES) + ps * QP * 16;
+                        if constexpr (I16) {
+                            const uint4 t = ptx::lds128u(a);
+                            float2 m0, m1, m2, m3;
+                            unpack_i16_quad<COARSE_S2_XU_N>(t, m0, m1, m2, m3);
+                            cmacp(pacc[k], m0, v[ps][0]);
+                            cmacp(pacc[k], m1, v[ps][1]);
+                            cmacp(pacc[k], m2, v[ps][2]);
+                            cmacp(pacc[k], m3, v[ps][3]);
+                        } else {
+                            const float4 t = ptx::lds128(a);
+                            cmacp(pacc[k], make_float2(t.x, t.y), v[ps][0]);
+                            cmacp(pacc[k], make_float2(t.z, t.w), v[ps][1]);
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
+                next_slot();
+            }
+            float2 acc[WL];
+#pragma unroll
+            for (int k = 0; k < WL; ++k) acc[k] = cfinal<false>(pacc[k]);
+#else
             float2 acc[WL];
 #pragma unroll
             for (int k = 0; k < WL; ++k) acc[k] = make_float2(0.f, 0.f);
@@ -290,6 +354,7 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
                 if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
                 next_slot();
             }
+#endif
             // a6: combine the column-slice partial sums, once per item
             const int k0 = transpose_reduce<WL, G / 2, WL>(acc, qi, 0);
             constexpr int NF = tr_final_n(WL, G / 2);
@@ -299,6 +364,54 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
                 for (int j = 0; j < NF; ++j) p.out[(int64_t)s * NC + rb * RS + row0 + (k0 + j) * RPL] = acc[j];
             }
         } else {
+#if COARSE_S2_PACKED_D
+            CAcc pacc[PASSES][CPQ];
+#pragma unroll
+            for (int ps = 0; ps < PASSES; ++ps)
+#pragma unroll
+                for (int e = 0; e < CPQ; ++e) pacc[ps][e].a = pacc[ps][e].b = make_float2(0.f, 0.f);
+#pragma unroll 1
+            for (int m = 0; m < 9; ++m) {
+                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+#pragma unroll 1
+                for (int c = 0; c < NB; ++c) {
+                    ptx::mbar_wait(full0 + 8u * slot, phase);
+                    const uint32_t lbase = link_u32 + slot * LINK_STAGE + (row0 * ROWBYTES + qi * 16);
+                    const uint32_t vbase = vec_u32 + slot * VEC_STAGE + row0 * 8;
+#pragma unroll
+                    for (int k = 0; k < WL; ++k) {
+                        float2 vj = ptx::lds64(vbase + k * (RPL * 8));
+                        if constexpr (I16) { vj.x *= sc; vj.y *= sc; }
+                        const VDup vd = vdup(vj);
+#pragma unroll
+                        for (int ps = 0; ps < PASSES; ++ps) {
+                            const uint32_t a = lbase + k * (RPL * ROWBYTES) + ps * QP * 16;
+                            if constexpr (I16) {
+                                const uint4 t = ptx::lds128u(a);
+                                float2 m0, m1, m2, m3;
+                                unpack_i16_quad<COARSE_S2_XU_D>(t, m0, m1, m2, m3);
+                                cmacp(pacc[ps][0], m0, vd);
+                                cmacp(pacc[ps][1], m1, vd);
+                                cmacp(pacc[ps][2], m2, vd);
+                                cmacp(pacc[ps][3], m3, vd);
+                            } else {
+                                const float4 t = ptx::lds128(a);
+                                cmacp(pacc[ps][0], make_float2(t.x, t.y), vd);
+                                cmacp(pacc[ps][1], make_float2(t.z, t.w), vd);
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
+                    next_slot();
+                }
+            }
+            float2 acc[PASSES][CPQ];
+#pragma unroll
+            for (int ps = 0; ps < PASSES; ++ps)
+#pragma unroll
+                for (int e = 0; e < CPQ; ++e) acc[ps][e] = cfinal<true>(pacc[ps][e]);
+#else
             float2 acc[PASSES][CPQ];
 #pragma unroll
             for (int ps = 0; ps < PASSES; ++ps)
@@ -339,6 +452,7 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
                     next_slot();
                 }
             }
+#endif
             // a6: combine the RPL row-group partial sums of the warp (lanes qi, qi + G, ...), then the TW warps'
 #pragma unroll
             for (int ps = 0; ps < PASSES; ++ps)

@@ -131,6 +131,35 @@ __device__ __forceinline__ void cmac(float2& acc, float mre, float mim, const fl
     acc = ptx::ffma2(make_float2(mim, mim), vs, acc);
 }
 
+// The same complex MAC with the MATRIX entry as the packed operand, for the kernels whose issue slots
+// are what bounds them (int16 links, several right-hand sides).  cmac<> needs (mre, mre) and (mim, mim)
+// as register pairs - two MOVs per link entry (ncu / SASS: 28 IMAD.MOV of 300 instructions per stage and
+// lane in the int16 kernel, 40 of 260 with 3 right-hand sides).  Here the decoded entry (re, im) IS the
+// packed operand, the duplicated pairs (v.re, v.re), (v.im, v.im) are built once per stage and reused for
+// every row, and the accumulator is kept as two packed partial sums
+//     a = sum (m.re, m.im) * v.re,    b = sum (m.re, m.im) * v.im
+// that are combined once per item: M.v = (a.x - b.y, a.y + b.x), conj(M).v = (a.x + b.y, b.x - a.y).
+struct CAcc {
+    float2 a, b;
+};
+struct VDup {
+    float2 re, im;
+};
+__device__ __forceinline__ VDup vdup(const float2 v) {
+    VDup d;
+    d.re = make_float2(v.x, v.x);
+    d.im = make_float2(v.y, v.y);
+    return d;
+}
+__device__ __forceinline__ void cmacp(CAcc& acc, const float2 m, const VDup& v) {
+    acc.a = ptx::ffma2(m, v.re, acc.a);
+    acc.b = ptx::ffma2(m, v.im, acc.b);
+}
+template <bool CONJ>
+__device__ __forceinline__ float2 cfinal(const CAcc& acc) {
+    return CONJ ? make_float2(acc.a.x + acc.b.y, acc.b.x - acc.a.y) : make_float2(acc.a.x - acc.b.y, acc.a.y + acc.b.x);
+}
+
 template <int NC, bool I16, bool DAG, bool FINE = false, bool GEN = false, bool HV = false>
 __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coarse_apply_stream(StreamParams p) {
     static_assert(!(DAG && FINE), "the fine geometry splits output rows: dagger = 0 only");

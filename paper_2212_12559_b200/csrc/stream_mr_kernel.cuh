@@ -131,11 +131,11 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
         next2_scale = fetch_scale(item + 2 * gridDim.x);
 
         if (!DAG) {
-            float2 acc[WL][R];
+            CAcc pacc[WL][R];
 #pragma unroll
             for (int k = 0; k < WL; ++k)
 #pragma unroll
-                for (int r = 0; r < R; ++r) acc[k][r] = make_float2(0.f, 0.f);
+                for (int r = 0; r < R; ++r) pacc[k][r].a = pacc[k][r].b = make_float2(0.f, 0.f);
 #pragma unroll 1
             for (int m = 0; m < 9; ++m) {
                 const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
@@ -158,17 +158,14 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
 #pragma unroll
                     for (int ps = 0; ps < PASSES; ++ps) {
                         // the lane's CPQ columns x R right-hand sides: CPQ*R contiguous complex numbers
-                        float2 v[CPQ * R];
+                        VDup v[CPQ * R];
                         const uint32_t va = vbase + (ps * QP + qi) * PITCH;
 #pragma unroll
                         for (int h = 0; h < CPQ * R / 2; ++h) {
-                            const float4 t = ptx::lds128(va + h * 16);
-                            v[2 * h] = make_float2(t.x, t.y);
-                            v[2 * h + 1] = make_float2(t.z, t.w);
-                        }
-                        if constexpr (I16) {
-#pragma unroll
-                            for (int e = 0; e < CPQ * R; ++e) { v[e].x *= sc; v[e].y *= sc; }
+                            float4 t = ptx::lds128(va + h * 16);
+                            if constexpr (I16) { t.x *= sc; t.y *= sc; t.z *= sc; t.w *= sc; }
+                            v[2 * h] = vdup(make_float2(t.x, t.y));
+                            v[2 * h + 1] = vdup(make_float2(t.z, t.w));
                         }
 #pragma unroll
                         for (int k = 0; k < WL; ++k) {
@@ -186,7 +183,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
 #pragma unroll
                             for (int e = 0; e < CPQ; ++e)
 #pragma unroll
-                                for (int r = 0; r < R; ++r) cmac<false>(acc[k][r], mm[e].x, mm[e].y, v[e * R + r]);
+                                for (int r = 0; r < R; ++r) cmacp(pacc[k][r], mm[e], v[e * R + r]);
                         }
                     }
                 }
@@ -195,6 +192,11 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                 if (++slot == S) { slot = 0; phase ^= 1u; }
             }
             // a6: combine the column-slice partial sums, once per item
+            float2 acc[WL][R];
+#pragma unroll
+            for (int k = 0; k < WL; ++k)
+#pragma unroll
+                for (int r = 0; r < R; ++r) acc[k][r] = cfinal<false>(pacc[k][r]);
 #pragma unroll
             for (int k = 0; k < WL; ++k) {
 #pragma unroll
@@ -212,13 +214,13 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                 }
             }
         } else {
-            float2 acc[PASSES][CPQ][R];
+            CAcc pacc[PASSES][CPQ][R];
 #pragma unroll
             for (int ps = 0; ps < PASSES; ++ps)
 #pragma unroll
                 for (int e = 0; e < CPQ; ++e)
 #pragma unroll
-                    for (int r = 0; r < R; ++r) acc[ps][e][r] = make_float2(0.f, 0.f);
+                    for (int r = 0; r < R; ++r) pacc[ps][e][r].a = pacc[ps][e][r].b = make_float2(0.f, 0.f);
 #pragma unroll 1
             for (int m = 0; m < 9; ++m) {
                 const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
@@ -231,11 +233,12 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
 #pragma unroll
                         for (int k = 0; k < WL; ++k) {
                             const int rl = (k * W + warp) * RPL + grp;
-                            float2 vj[R];
+                            VDup vj[R];
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
-                                vj[r] = ptx::lds64(vbase + (rl * R + r) * 8);
-                                if constexpr (I16) { vj[r].x *= sc; vj[r].y *= sc; }
+                                float2 t = ptx::lds64(vbase + (rl * R + r) * 8);
+                                if constexpr (I16) { t.x *= sc; t.y *= sc; }
+                                vj[r] = vdup(t);
                             }
 #pragma unroll
                             for (int ps = 0; ps < PASSES; ++ps) {
@@ -252,7 +255,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
 #pragma unroll
                                 for (int e = 0; e < CPQ; ++e)
 #pragma unroll
-                                    for (int r = 0; r < R; ++r) cmac<true>(acc[ps][e][r], mm[e].x, mm[e].y, vj[r]);
+                                    for (int r = 0; r < R; ++r) cmacp(pacc[ps][e][r], mm[e], vj[r]);
                             }
                         }
                     }
@@ -270,7 +273,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                     for (int e = 0; e < CPQ; ++e)
 #pragma unroll
                         for (int r = 0; r < R; ++r)
-                            red[((warp * RPL + grp) * NC + (ps * QP + qi) * CPQ + e) * R + r] = acc[ps][e][r];
+                            red[((warp * RPL + grp) * NC + (ps * QP + qi) * CPQ + e) * R + r] = cfinal<true>(pacc[ps][e][r]);
             }
             ptx::named_bar_sync(1, W * 32);
             for (int t = threadIdx.x; t < NC * R; t += W * 32) {
