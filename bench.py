@@ -374,7 +374,7 @@ def measure_config(name, steps, local, dev, read_ceiling=None):
 
     with ClockSampler(local) as clocks:
         if link_bytes <= 2 * l2_bytes:
-            reps = max(steps, 50)
+            reps = max(steps, 400)          # a graph launch costs tens of us: amortise it over many 6-10 us applies
             warm = {dg: time_graph(graph_of(lambda dg=dg: [op.apply(vin, outs[dg], nrhs=nrhs, dagger=dg) for _ in range(reps)])) / reps
                     for dg in (0, 1)}
             n_copies = int(3 * l2_bytes // max(1, link_bytes)) + 2
@@ -456,7 +456,7 @@ def run_ours(args, cfg, daggers):
     if args.keep_links:
         op.set_option(cop.OPT_KEEP_LINKS, args.keep_links)
     if args.pdl:
-        op.set_option(cop.OPT_PDL, 1)
+        op.set_option(cop.OPT_PDL, args.pdl)
     if args.warp_items:
         op.set_option(cop.OPT_WARP_ITEMS, args.warp_items)
 
@@ -945,7 +945,7 @@ def main():
     ap.add_argument("--links", default="", choices=["", "c64", "i16"], help="override the config's link storage")
     ap.add_argument("--warp-items", type=int, default=0,
                     help="COARSE_OPT_WARP_ITEMS override (0 auto, 1 never, 2 always, 11/12/14: 1/2/4 warps per team)")
-    ap.add_argument("--pdl", action="store_true", help="COARSE_OPT_PDL: programmatic dependent launch for chained applies")
+    ap.add_argument("--pdl", type=int, default=0, help="COARSE_OPT_PDL: programmatic dependent launch for chained applies (0 auto, 1 always, 2 never)")
     ap.add_argument("--hvec", action="store_true",
                     help="half-precision INPUT vectors (int16 + per-site norm, row f2) through coarse_op_apply_hvec")
     ap.add_argument("--no-cpu-baseline", action="store_true")

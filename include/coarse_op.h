@@ -35,7 +35,7 @@
  *   owns its metadata and two kinds of device scratch: two vector-sized staging buffers plus two copy
  *   streams (only if coarse_op_apply_host is used), and, on lattices with fewer sites than SMs, a few-MB
  *   workspace for the split dagger apply.  Because of that scratch a handle may have work in flight on
- *   ONE stream at a time; use one handle per stream for concurrent solves on the same links (handles
+ *   ONE stream at a time (two concurrent split applies would share the workspace and its counters); use one handle per stream for concurrent solves on the same links (handles
  *   are cheap and may share link buffers).  A handle belongs to the device that was current in
  *   coarse_op_create; calls made with another device current return COARSE_EINVAL.
  *
@@ -86,14 +86,17 @@ enum {
     COARSE_OPT_STAGES = 2,   /* cap on the STREAM shared-memory ring depth; 0 = library default   */
     COARSE_OPT_FINE = 3,     /* STREAM dagger=0 small-lattice row-block split: 0 auto, 1 never, 2 always */
     COARSE_OPT_KEEP_LINKS = 4, /* L2 policy of the link stream: 0 auto (keep if links <= L2/2), 1 evict_first, 2 keep */
-    COARSE_OPT_PDL = 5,      /* 1: launch the 1-RHS STREAM kernels with programmatic dependent launch: in a chain
-                                of applies on one stream the next kernel's CTAs start on SMs the previous one
-                                has left and prefetch their link stages before waiting for its output (the
-                                latency-limited small-lattice regime of PAPER.md:L99).  Default 0.  With it on,
-                                the LINK and scale arrays must not be written by work still in flight on the
-                                stream (they are read before the kernel orders itself against its predecessor). */
+    COARSE_OPT_PDL = 5,      /* programmatic dependent launch of the 1-RHS STREAM kernels: in a chain of applies on one
+                                stream the next kernel's CTAs start on SMs the previous one has left and prefetch
+                                their link stages before waiting for its output (the latency-limited small-lattice
+                                regime of PAPER.md:L99).  0 (default) auto: when the links fit L2, for every apply but
+                                the first after coarse_op_set_links (work that produced the links may still be in
+                                flight in front of that one); 1 always: the LINK and scale arrays must then not be
+                                written by work still in flight on the stream (they are read before the kernel orders
+                                itself against its predecessor); 2 never.  Results are bit-identical either way. */
     COARSE_OPT_SPLIT_DAGGER = 6, /* dagger = 1, 1 RHS, lattices with fewer sites than SMs: split each site's
-                                contraction over its row chunks + a reduce kernel (2 launches): 0 auto, 1 never,
+                                contraction over its row chunks, the CTA that finishes a site's last chunk adds the
+                                partial vectors in chunk order (one launch, deterministic): 0 auto, 1 never,
                                 2 always (needs the workspace coarse_op_set_links allocates on such lattices) */
     COARSE_OPT_WARP_ITEMS = 7 /* 1-RHS plain apply: the STREAM variant in which small teams of consumer warps own
                                 whole work items and every stage of theirs (csrc/stream2_kernel.cuh) instead of all

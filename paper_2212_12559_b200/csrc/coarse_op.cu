@@ -116,6 +116,12 @@ int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, co
     p.parity = ps.parity;
     p.n_sites = ps.parity == 2 ? op->lat.V : op->lat.V / 2;
     p.vnorms = ps.vnorms;
+    // Programmatic dependent launch: always (1), never (2), or auto (0): in the latency-limited regime (links
+    // resident in L2), for every launch but the first after coarse_op_set_links - work that PRODUCED the links
+    // may still be in flight on the stream in front of that one, and the link stages are read before the
+    // kernel orders itself against its predecessor.  Site-range launches (apply_host) never use it.
+    p.pdl = (op->pdl_opt == 1 || (op->pdl_opt == 0 && !op->links_fresh && ps.site_end == 0 &&
+                                  coarse_op_link_bytes(op) <= (size_t)op->l2_bytes)) ? 1 : 0;
     switch (op->Nc) {
 #define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_stream_nc, NC)(op, p, dagger, ps.gen, stream);
         COARSE_FOR_EACH_NC(COARSE_CASE_NC)
@@ -255,9 +261,11 @@ coarse_op_t* coarse_op_create(const int dims[4], int Nc, int link_precision) {
     op->fine_opt = 0;
     op->keep_opt = 0;
     op->pdl_opt = 0;
+    op->links_fresh = true;
     op->split_opt = 0;
     op->warp_items_opt = 0;
     op->split_ws = nullptr;
+    op->split_count = nullptr;
     op->split_ws_bytes = 0;
     { int l2 = 0; cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev); op->l2_bytes = l2; }
     op->last_launches = 0;
@@ -303,12 +311,29 @@ int coarse_op_set_links(coarse_op_t* op, const void* links_dev, const float* sca
     }
     op->links = links_dev;
     op->scales = scales_dev;
+    op->links_fresh = true;
     // tiny lattices (fewer sites than SMs): workspace for the split dagger apply, V * (Nc/8) chunks * Nc
     // complex numbers at most (a few MB); the only allocation the library makes besides apply_host's staging
     if (!op->split_ws && op->lat.V < op->num_sms && stream_supports(op->Nc, 1)) {
         const size_t bytes = (size_t)op->lat.V * (op->Nc / 8) * op->Nc * 8;
-        if (cudaMalloc(reinterpret_cast<void**>(&op->split_ws), bytes) == cudaSuccess) op->split_ws_bytes = bytes;
-        else { cudaGetLastError(); op->split_ws = nullptr; op->split_ws_bytes = 0; }
+        const size_t cbytes = (size_t)op->lat.V * sizeof(unsigned int);
+        if (cudaMalloc(reinterpret_cast<void**>(&op->split_ws), bytes + cbytes) == cudaSuccess) {
+            op->split_count = reinterpret_cast<unsigned int*>(reinterpret_cast<unsigned char*>(op->split_ws) + bytes);
+            // the counters start at zero and every launch leaves them at zero; the clear is complete before any
+            // stream can use them (one synchronisation per handle, at set-up time)
+            if (cudaMemset(op->split_count, 0, cbytes) == cudaSuccess && cudaDeviceSynchronize() == cudaSuccess) {
+                op->split_ws_bytes = bytes;
+            } else {
+                cudaGetLastError();
+                cudaFree(op->split_ws);
+                op->split_ws = nullptr;
+                op->split_count = nullptr;
+            }
+        } else {
+            cudaGetLastError();
+            op->split_ws = nullptr;
+            op->split_ws_bytes = 0;
+        }
     }
     return make_link_maps(op);
 }
@@ -359,7 +384,7 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value) {
             op->warp_items_opt = value;
             return COARSE_OK;
         case COARSE_OPT_PDL:
-            if (value != 0 && value != 1) return fail(COARSE_EINVAL, "set_option: pdl must be 0 or 1");
+            if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: pdl must be 0 (auto), 1 (always) or 2 (never)");
             op->pdl_opt = value;
             return COARSE_OK;
         case COARSE_OPT_STAGES:
@@ -408,6 +433,7 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
     if (rc < 0) return rc;
     op->last_launches = 1 + rc;      // the split dagger apply reports its second (reduce) launch as rc = 1
     op->last_path = path;
+    op->links_fresh = false;
     return COARSE_OK;
 }
 
@@ -461,6 +487,7 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
     if (rc < 0) return rc;
     op->last_launches = 1 + rc;
     op->last_path = path;
+    op->links_fresh = false;
     return COARSE_OK;
 }
 
@@ -492,6 +519,7 @@ int coarse_op_apply_hvec(coarse_op_t* op, const void* in_q_dev, const float* in_
     if (rc != COARSE_OK) return rc;
     op->last_launches = 1;
     op->last_path = path;
+    op->links_fresh = false;
     return COARSE_OK;
 }
 

@@ -25,11 +25,13 @@ struct coarse_op {
     int stages_opt;
     int fine_opt;
     int keep_opt;
-    int pdl_opt;
+    int pdl_opt;              // COARSE_OPT_PDL: 0 auto, 1 always, 2 never
+    bool links_fresh;         // no apply has been enqueued since coarse_op_set_links (auto PDL skips that launch)
     int split_opt;            // COARSE_OPT_SPLIT_DAGGER: 0 auto, 1 never, 2 always
     int warp_items_opt;       // COARSE_OPT_WARP_ITEMS: 0 auto, 1 never, 2 always
     float2* split_ws;         // partial vectors of the split dagger apply (allocated by set_links on tiny lattices)
     size_t split_ws_bytes;
+    unsigned int* split_count; // per-site chunk counters of the split dagger apply (zero between launches)
     int l2_bytes;
     int last_launches;
     int last_path;

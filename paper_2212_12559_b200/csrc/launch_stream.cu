@@ -23,15 +23,17 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
         p.n_items = DAG ? base.n_items : base.n_items * Gm::NB;
     }
     // dagger = 1 has one work item per site; on a lattice with fewer sites than SMs (the paper's level 3:
-    // 32 sites per GPU) the contraction of a site is split over its NB row chunks, one item each, and a
-    // small second kernel adds the NB partial vectors in order.
+    // 32 sites per GPU) the contraction of a site is split over its NB row chunks, one item each, and the
+    // CTA that finishes a site's last chunk adds the NB partial vectors in order (stream_kernel.cuh).
     p.split = 0;
     p.partial = nullptr;
+    p.split_count = nullptr;
     if (DAG && !GEN && !HV && base.n_items == 0 && Gm::NB > 1 && op->split_ws &&
         (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes &&
         (op->split_opt == 2 || (op->split_opt == 0 && p.n_sites < op->num_sms))) {
         p.split = 1;
         p.partial = op->split_ws;
+        p.split_count = op->split_count;
         p.n_items = p.n_sites * Gm::NB;
     }
     int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (Gm::stage_bytes(DAG) + 16);
@@ -48,7 +50,7 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     // PDL: a kernel whose shared-memory carve-out differs from its predecessor's cannot take over an SM
     // before it has drained completely (measured: an alternating dagger 0 / dagger 1 chain gained nothing
     // until both kernels asked for the same size), so under PDL both modes request the larger of the two.
-    if (op->pdl_opt && Gm::smem_bytes(!DAG, stages) > smem && Gm::smem_bytes(!DAG, stages) <= op->max_smem)
+    if (base.pdl && Gm::smem_bytes(!DAG, stages) > smem && Gm::smem_bytes(!DAG, stages) <= op->max_smem)
         smem = Gm::smem_bytes(!DAG, stages);
     auto kern = coarse_apply_stream<NC, I16, DAG, FINE, GEN, HV>;
     static SmemAttrCache attr_cache;
@@ -57,7 +59,7 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
     if (grid > p.n_items - p.item_begin) grid = p.n_items - p.item_begin;
     if (grid < 1) return COARSE_OK;
-    p.pdl = op->pdl_opt ? 1 : 0;
+    p.pdl = base.pdl;
     if (p.pdl) {
         // programmatic dependent launch: this kernel may start while the previous kernel of the stream
         // drains; it orders itself against that kernel's memory with griddepcontrol.wait (stream_kernel.cuh)
@@ -77,13 +79,6 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
         kern<<<grid, Gm::THREADS, smem, stream>>>(p);
         e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e, "stream kernel launch");
-    }
-    if (p.split) {
-        const long long tot = (long long)p.n_sites * NC;
-        coarse_dagger_reduce_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(p.partial, p.n_sites, Gm::NB, NC, p.out);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return cuda_fail(e, "dagger reduce kernel launch");
-        return 1;      // one extra launch (coarse_op_apply adds it to last_launches)
     }
     return COARSE_OK;
 }
@@ -139,7 +134,7 @@ int launch_stream2_t(const coarse_op* op, const StreamParams& base, cudaStream_t
 
 template <int NC, bool I16>
 bool use_warp_items(const coarse_op* op, const StreamParams& p, int dagger, bool gen) {
-    if (gen || p.vnorms || p.n_items > 0 || op->pdl_opt || op->warp_items_opt == 1) return false;
+    if (gen || p.vnorms || p.n_items > 0 || p.pdl || op->warp_items_opt == 1) return false;
     if (op->warp_items_opt >= 2) return true;
     const int64_t items = dagger ? (int64_t)p.n_sites : (int64_t)p.n_sites * Stream2Geom<NC, I16, 4>::NB;
     return I16 && NC >= 64 && items >= (int64_t)4 * Stream2Geom<NC, I16, 4>::T * op->num_sms;

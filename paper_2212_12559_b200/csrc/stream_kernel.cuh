@@ -53,10 +53,12 @@ struct StreamParams {
     int n_sites;              // sites in the parity set
     int pdl;                  // 1: launched with programmatic stream serialization (COARSE_OPT_PDL)
     int item_begin;           // work items [item_begin, n_items): coarse_op_apply_host launches site ranges
-    // dagger = 1 on a tiny lattice: split a site's contraction over its NB row chunks (item = (site, chunk)),
-    // partial vectors go to `partial` and coarse_dagger_reduce_kernel adds them in chunk order
+    // dagger = 1 on a tiny lattice: split a site's contraction over its NB row chunks (item = (site, chunk)):
+    // partial vectors go to `partial`, and the CTA that finishes a site's LAST chunk (split_count) adds the NB
+    // partial vectors in chunk order - one launch, and the sum does not depend on which CTA that is
     int split;
     float2* partial;          // [n_sites * NB][Nc]
+    unsigned int* split_count;   // [n_sites], zero between launches (the reducing CTA resets its site's counter)
     // HV (half-precision input vectors, coarse_op_apply_hvec): `in` points at int16 (re,im) entries
     const float* vnorms;      // fp32 norm per site (nrhs = 1)
 };
@@ -470,25 +472,34 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                 if (p.split) p.partial[(int64_t)item * NC + t] = sum;
                 else p.out[(int64_t)s * NC + t] = sum;
             }
+            if (p.split) {
+                // last-arriver reduction: every consumer thread publishes its part of the partial vector, one
+                // thread counts the chunk in; the CTA that counted the NB-th chunk of the site sums all of them
+                uint32_t* last_flag = reinterpret_cast<uint32_t*>(bars + 2 * S);
+                __threadfence();
+                ptx::named_bar_sync(1, W * 32);
+                if (threadIdx.x == 0) {
+                    const unsigned int old = atomicAdd(p.split_count + s, 1u);
+                    *last_flag = (old == (unsigned int)(NB - 1)) ? 1u : 0u;
+                    if (old == (unsigned int)(NB - 1)) p.split_count[s] = 0u;      // all NB arrivals are in: reset for the next launch
+                }
+                ptx::named_bar_sync(1, W * 32);
+                if (*last_flag) {
+                    __threadfence();
+                    for (int t = threadIdx.x; t < NC; t += W * 32) {
+                        float2 sum = make_float2(0.f, 0.f);
+                        for (int c = 0; c < NB; ++c) {
+                            const float2 x = __ldcg(p.partial + ((int64_t)s * NB + c) * NC + t);
+                            sum.x += x.x;
+                            sum.y += x.y;
+                        }
+                        p.out[(int64_t)s * NC + t] = sum;
+                    }
+                }
+            }
             red_parity ^= 1;
         }
     }
-}
-
-// out[s][t] = sum_c partial[s*nb + c][t], chunks added in order (deterministic).  static: this header is
-// compiled into one translation unit per Nc.
-static __global__ void __launch_bounds__(256) coarse_dagger_reduce_kernel(const float2* partial, int n_sites, int nb, int nc, float2* out) {
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (long long)n_sites * nc) return;
-    const long long s = idx / nc;
-    const int t = (int)(idx % nc);
-    float2 sum = make_float2(0.f, 0.f);
-    for (int c = 0; c < nb; ++c) {
-        const float2 x = partial[(s * nb + c) * nc + t];
-        sum.x += x.x;
-        sum.y += x.y;
-    }
-    out[idx] = sum;
 }
 
 }  // namespace coarse

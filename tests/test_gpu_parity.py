@@ -387,23 +387,28 @@ def test_pdl_with_parts_hvec_and_graph_capture(oracle_lib):
 @pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
 def test_split_dagger_on_tiny_lattices(oracle_lib, dims, Nc, prec):
     """dagger = 1 with fewer sites than SMs (the paper's level 3 has 32 sites per GPU): the contraction of
-    a site is split over its row chunks and reduced by a second kernel.  Auto picks it, forcing it off must
-    give the same numbers up to summation order, and both must match the oracle."""
+    a site is split over its row chunks and the CTA that finishes a site's last chunk adds the partial vectors
+    (one launch).  Auto picks it, forcing it off must give the same numbers up to summation order, both must
+    match the oracle, and repeated launches must be bit-identical (the chunk counters reset themselves)."""
     V = synth.lattice_volume(dims)
     links, scales, links_h, scales_h = _links_for(dims, Nc, prec, 61, False, oracle_lib)
     vin = synth.make_vectors(dims, Nc, 1, 62, device="cuda")
     ref = oracle_lib.coarse_apply(dims, Nc, links_h, vin.cpu().numpy(), dagger=1, link_precision=prec, scales=scales_h)
-    for mode, want_launches in ((0, None), (1, 1), (2, None)):
+    for mode in (0, 1, 2):
         op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales).set_option(cop.OPT_SPLIT_DAGGER, mode)
         out = torch.full_like(vin, float("nan"))
         op.apply(vin, out, dagger=1)
         torch.cuda.synchronize()
-        assert op.last_path == cop.PATH_STREAM
-        if want_launches:
-            assert op.last_launches == want_launches
-        else:
-            assert op.last_launches in (1, 2)          # 2 when the geometry has more than one row chunk
+        assert op.last_path == cop.PATH_STREAM and op.last_launches == 1
         assert rel_l2_per_rhs(out.cpu().numpy(), ref) <= TOL
+        for grid in (0, 1, 5):                          # many launches, also with every chunk of a site on one CTA
+            op.set_option(cop.OPT_GRID, grid)
+            for _ in range(3):
+                again = torch.full_like(vin, float("nan"))
+                op.apply(vin, again, dagger=1)
+                torch.cuda.synchronize()
+                assert torch.equal(torch.view_as_real(again), torch.view_as_real(out))
+        op.set_option(cop.OPT_GRID, 0)
         # dagger = 0 is untouched by the option
         op.apply(vin, out, dagger=0)
         torch.cuda.synchronize()
