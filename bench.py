@@ -851,8 +851,8 @@ def run_hat(args, cfg):
 
 def run_cagcr(args, cfg):
     """--workload cagcr: CA-GCR(8) smoother cycles on the config's operator
-    (diagonally shifted so that the smoother converges).  One step = one cycle = 8 chained applies + the
-    fused Gram pass + the 8x8 solve + the fused update = 11 launches."""
+    (diagonally shifted so that the smoother converges).  One step = one cycle = 8 applies + 7 fused
+    Chebyshev recurrence steps + the fused Gram pass + the 8x8 solve + the fused update (+ the interval estimate)."""
     import paper_2212_12559_b200 as cop
     world, rank, local = dist_env()
     if world > 1:
@@ -865,10 +865,15 @@ def run_cagcr(args, cfg):
     links = synth.make_gamma_hermitian_links(dims, Nc, cfg["seed"], device=dev)
     links[:, 0] += 12.0 * torch.eye(Nc, dtype=torch.complex64, device=dev)
 
+    n_launch = [0]
+
     def smooth(work=None):
-        if args.cheb:      # the hopping part has spectral radius ~4.1 around the shifted diagonal 12.1
-            return op.cagcr_cheb(b, x, 7.5, 16.7, s=s, cycles=1, work=work, info=info)
-        return op.cagcr(b, x, s=s, cycles=1, work=work, info=info)
+        if args.cheb:      # caller-supplied interval: the hopping part has spectral radius ~4.1 around the shifted diagonal 12.1
+            w = op.cagcr_cheb(b, x, 7.5, 16.7, s=s, cycles=1, work=work, info=info)
+        else:              # the default: interval estimated on the device from the first residual
+            w = op.cagcr(b, x, s=s, cycles=1, work=work, info=info)
+        n_launch[0] += op.last_launches
+        return w
     scales = None
     if prec == cop.LINK_I16:
         q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device=dev)
@@ -888,10 +893,12 @@ def run_cagcr(args, cfg):
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clocks:
+        n_launch[0] = 0
         t0.record(stream)
         for _ in range(args.steps):
             smooth(work)
         t1.record(stream)
+        timed_launches = n_launch[0]
         tmp = torch.empty_like(b)
         a0.record(stream)
         for _ in range(args.steps):
@@ -907,10 +914,10 @@ def run_cagcr(args, cfg):
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_cycle, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": "%s cycle on the %s lattice, Nc=%d, %s links (X shifted by 12): %d applies + "
-                               "Gram + solve + update per step" % ("Chebyshev-basis CA-GCR(16)" if args.cheb else "CA-GCR(8)",
+                               "recurrence steps + Gram + solve + update per step" % ("Chebyshev-basis CA-GCR(16), given interval" if args.cheb else "CA-GCR(8), estimated interval",
                                                                    "x".join(map(str, dims)), Nc, cfg["links"], s),
                    "seed": cfg["seed"]},
-        "clocks": clocks.summary(), "gpu_launches": ((2 * s + 2) if args.cheb else (s + 3)) * args.steps,
+        "clocks": clocks.summary(), "gpu_launches": timed_launches,
         "cagcr": {"ms_per_cycle": ms_cycle, "ms_of_s_plain_applies": ms_applies, "s": s,
                   "vector_side_share": 1.0 - ms_applies / ms_cycle,
                   "residual_reduction_one_cycle": float(np.sqrt(max(inf[1], 0.0) / inf[0])) if inf[0] > 0 else None,

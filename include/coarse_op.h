@@ -214,37 +214,37 @@ size_t coarse_op_hat_work_bytes(const coarse_op_t* op);
 int coarse_op_build_hat_links(coarse_op_t* op, void* out_links_c64_dev, int slot0, void* work_dev, int* info_dev,
                               void* stream);
 
-/* CA-GCR(s), the paper's smoother ("CA-GCR(8)", Table 1 L116/L122/L130), on this operator,
- * 1 RHS, power basis.  Each of `cycles` cycles: r0 = b - A x; p_k = A^k r0 (s chained coarse_op_apply);
- * ONE fused pass of block inner products G_jk = <p_j, p_k> (fp64, the single reduction per cycle);
- * alpha = argmin || r0 - sum_k alpha_k A p_k || from the s x s normal equations (fp64 Cholesky on the
- * device); x += sum_k alpha_k p_k, r = r0 - sum_k alpha_k A p_k in one fused update pass.
+/* CA-GCR(s), the paper's smoother ("CA-GCR(8)", Table 1 L116/L122/L130; its coarsest-level solver is a
+ * "Chebyshev-basis CA-GCR(16)", L134), on this operator, 1 RHS.  Each of `cycles` cycles minimises the residual
+ * over x + K_s(A, r0), r0 = b - A x, the communication-avoiding way: the whole basis first - the Chebyshev basis
+ * p_k = T_k((A - c)/d) r0 with t_k = A p_k kept beside it (s chained coarse_op_apply + s - 1 fused recurrence
+ * steps) - then ONE fused pass of block inner products (fp64, the single reduction per cycle), the s x s normal
+ * equations (fp64 Cholesky on the device) and one fused update x += sum_k alpha_k p_k, r = r0 - sum_k alpha_k t_k.
+ * The basis spans the same Krylov space as the power basis A^k r0 - the minimiser is the same - but stays well
+ * conditioned at every s <= 16.
+ *   interval       coarse_op_cagcr / coarse_op_cagcr_schur estimate [c - d, c + d] on the device, in the first
+ *                  cycle, from the moments of r0 (c = Re <r0, A r0>/<r0, r0>, d = twice the spread of A as r0 sees
+ *                  it): no caller-supplied bounds, no host round trip.  coarse_op_cagcr_cheb takes real bounds
+ *                  [lambda_min, lambda_max] that roughly enclose the spectrum (both 0: estimate as above).
  *   b_dev, x_dev   complex64 [V][Nc]; x_is_zero != 0: x is cleared first and b is used as r0 directly.
- *   work_dev       coarse_op_cagcr_work_bytes(op, s) bytes of caller-owned scratch (16-byte aligned).
+ *   work_dev       coarse_op_cagcr_work_bytes(op, s) bytes of caller-owned scratch (16-byte aligned): 2s + 2 vectors.
  *   info_dev       NULL, or double[3 * cycles]: per cycle ||r0||^2, the predicted ||r||^2 after the
  *                  cycle, and the number of basis vectors the factorisation kept (s unless the Gram
  *                  matrix lost positive definiteness).
- * 1 <= s <= 16.  Enqueues s + 3 kernels per cycle and returns; never synchronises. */
-/* coarse_op_cagcr_schur: the same smoother on the left-preconditioned even/odd Schur operator
- * Shat_p v = v - Dhat_pq Dhat_qp v of a handle whose links are block-preconditioned (Yhat = X^-1 Y;
- * PAPER.md:L87, Table 1 L127/L135: the levels the paper smooths with CA-GCR(8) are Schur-preconditioned).
- * b and x are full-lattice vectors whose entries on the other parity must be zero (x is kept so);
- * every operator application is two parity-restricted launches (coarse_op_apply_parts). */
+ * 1 <= s <= 16.  Enqueues 2s + 2 kernels per cycle for A (s applies, s - 1 recurrence steps, Gram, solve, update)
+ * plus 2 for the interval estimate (1 when the bounds are given); never synchronises.
+ * coarse_op_cagcr_schur (and schur_parity = 0 | 1 of coarse_op_cagcr_cheb): the same smoother on the
+ * left-preconditioned even/odd Schur operator Shat_p v = v - Dhat_pq Dhat_qp v of a handle whose links are
+ * block-preconditioned (Yhat = X^-1 Y; Table 1 L127/L135: the levels the paper smooths with
+ * CA-GCR(8) are Schur-preconditioned).  b and x are full-lattice vectors whose entries on the other parity must
+ * be zero (x is kept so); every operator application is two parity-restricted launches (coarse_op_apply_parts).
+ * schur_parity = -1: the operator is A. */
 size_t coarse_op_cagcr_work_bytes(const coarse_op_t* op, int s);
-int coarse_op_cagcr_schur(coarse_op_t* op_hat, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
-                          int parity, void* work_dev, double* info_dev, void* stream);
+size_t coarse_op_cagcr_cheb_work_bytes(const coarse_op_t* op, int s);   /* the same number */
 int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
                     void* work_dev, double* info_dev, void* stream);
-
-/* CA-GCR(s) with a CHEBYSHEV basis (the paper's coarsest-level solver is a "Chebyshev-basis CA-GCR(16)",
- * PAPER.md:L134 Table 1): p_k = T_k((A - c)/d) r0 with [lambda_min, lambda_max] = [c - d, c + d] an
- * interval that roughly encloses the operator's spectrum (real bounds, supplied by the caller).  The
- * basis spans the same Krylov space as coarse_op_cagcr's power basis - the minimiser is the same - but
- * stays well conditioned, so s = 16 keeps all its digits.  schur_parity = -1: the operator is A;
- * 0 | 1: the Schur-hat operator of coarse_op_cagcr_schur.  Work: coarse_op_cagcr_cheb_work_bytes(op, s)
- * (2s + 2 vectors).  2s + 2 launches per cycle for A (s applies, s - 1 recurrence steps, Gram, solve,
- * update).  info_dev as for coarse_op_cagcr. */
-size_t coarse_op_cagcr_cheb_work_bytes(const coarse_op_t* op, int s);
+int coarse_op_cagcr_schur(coarse_op_t* op_hat, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
+                          int parity, void* work_dev, double* info_dev, void* stream);
 int coarse_op_cagcr_cheb(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
                          float lambda_min, float lambda_max, int schur_parity, void* work_dev, double* info_dev,
                          void* stream);

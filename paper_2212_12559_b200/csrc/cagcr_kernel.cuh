@@ -1,16 +1,20 @@
 // cagcr_kernel.cuh — the vector side of CA-GCR(s), the paper's smoother ("CA-GCR(8)",
 // Table 1 L116/L122/L130), around s chained coarse-op applies:
 //
-//   p_0 = r0,  p_{k+1} = A p_k  (k < s)          s applies (stream_kernel.cuh), 98 % of the time
-//   G_jk = <p_j, p_k>,  0 <= j <= k <= s          ONE fused pass of block inner products (this file);
+//   p_k = T_k((A - c)/d) r0, t_k = A p_k (k < s)   s applies (stream_kernel.cuh, 95 % of the time) and s - 1
+//                                                 fused three-term recurrence steps: the Chebyshev basis of
+//                                                 the Krylov space K_s(A, r0) on [c - d, c + d]
+//   G = Gram matrix of (r0, t_0 .. t_{s-1})       ONE fused pass of block inner products (this file);
 //                                                 on a partitioned lattice this is the single
 //                                                 all-reduce per cycle that makes the method
 //                                                 "communication avoiding"
-//   (Q^H Q) alpha = Q^H r0 with q_k = p_{k+1}     s x s Hermitian solve, fp64 Cholesky, one thread
-//   x += sum_k alpha_k p_k,  r = p_0 - sum_k alpha_k p_{k+1}      one fused update pass
+//   (T^H T) alpha = T^H r0                        s x s Hermitian solve, fp64 Cholesky, one thread
+//   x += sum_k alpha_k p_k,  r = r0 - sum_k alpha_k t_k      one fused update pass
 //
-// The Gram matrix is accumulated in fp64 (the power basis is ill conditioned; the normal equations
-// square that) with a fixed two-level summation order: bit-identical run to run.
+// The interval is either the caller's or estimated on the device, without a host round trip, from the
+// moments of the first residual: m1 = <r0, A r0>/<r0, r0>, m2 = <A r0, A r0>/<r0, r0>,
+// c = Re m1, d = 2 sqrt(m2 - (Re m1)^2) (twice the spread of the spectrum as r0 sees it).
+// The Gram matrix is accumulated in fp64 with a fixed two-level summation order: bit-identical run to run.
 #pragma once
 #include "common.cuh"
 
@@ -159,31 +163,6 @@ __global__ void __launch_bounds__(320) cagcr_solve_kernel(const double2* partial
     }
 }
 
-// x += sum_{k<s} alpha_k p_k ;  r_out = p_0 - sum_{k<s} alpha_k p_{k+1}
-__global__ void __launch_bounds__(256) cagcr_update_kernel(CagcrVecs v, long long n, int s, const double2* alpha,
-                                                           float2* x, float2* r_out) {
-    __shared__ float2 al[CAGCR_MAX_S];
-    if (threadIdx.x < s) al[threadIdx.x] = make_float2((float)alpha[threadIdx.x].x, (float)alpha[threadIdx.x].y);
-    __syncthreads();
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        float2 xs = x[i];
-        float2 prev = v.p[0][i];
-        float2 rs = prev;
-#pragma unroll 4
-        for (int k = 0; k < s; ++k) {
-            const float2 a = al[k];
-            xs.x = fmaf(a.x, prev.x, fmaf(-a.y, prev.y, xs.x));
-            xs.y = fmaf(a.x, prev.y, fmaf(a.y, prev.x, xs.y));
-            const float2 next = v.p[k + 1][i];
-            rs.x = fmaf(-a.x, next.x, fmaf(a.y, next.y, rs.x));
-            rs.y = fmaf(-a.x, next.y, fmaf(-a.y, next.x, rs.y));
-            prev = next;
-        }
-        x[i] = xs;
-        r_out[i] = rs;
-    }
-}
-
 // r = b - t
 __global__ void __launch_bounds__(256) cagcr_residual_kernel(const float2* b, const float2* t, long long n, float2* r) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
@@ -194,21 +173,53 @@ __global__ void __launch_bounds__(256) cagcr_residual_kernel(const float2* b, co
 
 // ---- Chebyshev basis (the paper's coarsest-level solver is a "Chebyshev-basis CA-GCR(16)"):
 // p_k = T_k((A - c)/d) r0 on the interval [lambda_min, lambda_max] = [c - d, c + d] spans the same Krylov
-// space as the power basis but stays well conditioned, so s = 16 no longer drowns in the Gram matrix.
+// space as the power basis A^k r0 but stays well conditioned (the power basis, stored in complex64 with a Gram
+// matrix that squares its conditioning, lost the iterate's 5th digit at s = 8 and truncated itself at s = 16).
 // With t_k = A p_k:   p_1 = (t_0 - c p_0)/d,   p_{k+1} = (2/d)(t_k - c p_k) - p_{k-1}.
-// out = a*t + b*p + g*pm   (g = 0 and pm ignored for the first step)
+// cd = {c, d} lives in device memory (written by one of the two kernels below).
 __global__ void __launch_bounds__(256) cagcr_cheb_step_kernel(const float2* t, const float2* p, const float2* pm,
-                                                              float a, float b, float g, long long n, float2* out) {
+                                                              const double* cd, int first, long long n, float2* out) {
+    const float a = (float)((first ? 1.0 : 2.0) / cd[1]);
+    const float b = (float)(-(first ? 1.0 : 2.0) * cd[0] / cd[1]);
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         const float2 x = t[i], y = p[i];
         float2 o = make_float2(fmaf(a, x.x, b * y.x), fmaf(a, x.y, b * y.y));
-        if (g != 0.f) {
+        if (!first) {
             const float2 z = pm[i];
-            o.x = fmaf(g, z.x, o.x);
-            o.y = fmaf(g, z.y, o.y);
+            o.x -= z.x;
+            o.y -= z.y;
         }
         out[i] = o;
     }
+}
+
+__global__ void cagcr_set_interval_kernel(double c, double d, double* cd) {
+    cd[0] = c;
+    cd[1] = d;
+}
+
+// Interval from the Gram partials of (r0, A r0) (cagcr_gram_kernel with s = 1: pairs (0,0), (0,1), (1,1)).
+__global__ void __launch_bounds__(32) cagcr_interval_kernel(const double2* partial, int nblocks, double* cd) {
+    if (threadIdx.x != 0) return;
+    double g00 = 0.0, g11 = 0.0;
+    double2 g01 = make_double2(0.0, 0.0);
+    for (int b = 0; b < nblocks; ++b) {
+        g00 += partial[(long long)b * 3 + 0].x;
+        g01.x += partial[(long long)b * 3 + 1].x;
+        g01.y += partial[(long long)b * 3 + 1].y;
+        g11 += partial[(long long)b * 3 + 2].x;
+    }
+    double c = 0.0, d = 1.0;
+    if (g00 > 0.0) {
+        c = g01.x / g00;
+        const double var = g11 / g00 - c * c;                 // includes the imaginary spread of the spectrum
+        d = 2.0 * sqrt(var > 0.0 ? var : 0.0);
+        const double floor_d = 1e-3 * fabs(c);
+        if (!(d > floor_d)) d = floor_d;
+        if (!(d > 0.0)) d = 1.0;
+    }
+    cd[0] = c;
+    cd[1] = d;
 }
 
 // x += sum_{k<s} alpha_k P_k ;  r_out = r0 - sum_{k<s} alpha_k T_k      (P, T: separate vector lists)

@@ -667,107 +667,14 @@ int coarse_op_quantize_i16(const void* links_c64_dev, int64_t n_matrices, int Nc
     return COARSE_OK;
 }
 
-size_t coarse_op_cagcr_work_bytes(const coarse_op_t* op, int s) {
-    if (!op || s < 1 || s > CAGCR_MAX_S) return 0;
-    const size_t vec = coarse_op_vector_bytes(op, 1);
-    const size_t S1 = (size_t)s + 1;
-    return (S1 + 2) * vec + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1 * sizeof(double2) + (size_t)CAGCR_MAX_S * sizeof(double2) + 256;
-}
+size_t coarse_op_cagcr_work_bytes(const coarse_op_t* op, int s) { return coarse_op_cagcr_cheb_work_bytes(op, s); }
 
+// CA-GCR(s) on the Chebyshev basis (cagcr_kernel.cuh): P_k = T_k((A - c)/d) r0, T_k = A P_k kept as separate
+// vectors.  Slots: P_0..P_{s-1} | T_0..T_{s-1} | R (the update's output, swapped with P_0 every cycle).
+// lambda_min = lambda_max = 0: the interval is estimated on the device in the first cycle.
 // schur_parity < 0: the operator is A (coarse_op_apply).  schur_parity = 0 | 1: the operator is the
 // left-preconditioned Schur operator on that parity, Shat_p v = v - Dhat_pq Dhat_qp v, two
 // parity-restricted launches on this handle's (block-preconditioned) links.
-static int cagcr_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
-                      int schur_parity, void* work_dev, double* info_dev, void* stream) {
-    if (!op) return fail(COARSE_EINVAL, "cagcr: op is NULL");
-    if (!op->links) return fail(COARSE_ENOTREADY, "cagcr: coarse_op_set_links has not been called");
-    if (!b_dev || !x_dev || !work_dev) return fail(COARSE_EINVAL, "cagcr: NULL pointer");
-    if (s < 1 || s > CAGCR_MAX_S) return fail(COARSE_EINVAL, "cagcr: 1 <= s <= %d (got %d)", CAGCR_MAX_S, s);
-    if (cycles < 1) return fail(COARSE_EINVAL, "cagcr: cycles must be >= 1");
-    if (!aligned16(b_dev) || !aligned16(x_dev) || !aligned16(work_dev)) return fail(COARSE_EINVAL, "cagcr: pointers must be 16-byte aligned");
-    { int rc0 = check_device(op, "cagcr"); if (rc0 != COARSE_OK) return rc0; }
-    if (op->path_opt == COARSE_PATH_TENSOR || op->path_opt == COARSE_PATH_BLOCK)
-        return fail(COARSE_EUNSUPPORTED, "cagcr: the handle is pinned to a block-apply path; the smoother applies 1 RHS");
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t vec = coarse_op_vector_bytes(op, 1);
-    {
-        const size_t wb = coarse_op_cagcr_work_bytes(op, s);
-        if (overlaps(b_dev, vec, x_dev, vec) || overlaps(b_dev, vec, work_dev, wb) || overlaps(x_dev, vec, work_dev, wb))
-            return fail(COARSE_EINVAL, "cagcr: b, x and work must not overlap");
-    }
-    op->last_launches = 0;
-    const long long n = (long long)op->lat.V * op->Nc;
-    const int S1 = s + 1;
-    unsigned char* w = static_cast<unsigned char*>(work_dev);
-    float2* slot[CAGCR_MAX_S + 2];
-    for (int k = 0; k < S1 + 1; ++k) slot[k] = reinterpret_cast<float2*>(w + (size_t)k * vec);
-    double2* partial = reinterpret_cast<double2*>(w + (size_t)(S1 + 1) * vec);
-    double2* alpha = partial + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1;
-    const int vgrid = op->num_sms * 4;
-    int launches = 0, rc;
-    float2* tmp = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(alpha + CAGCR_MAX_S) + 64);
-    tmp = reinterpret_cast<float2*>((reinterpret_cast<uintptr_t>(tmp) + 15) & ~(uintptr_t)15);
-    if (schur_parity >= 0) {
-        for (int mu = 0; mu < 4; ++mu)
-            if (op->lat.L[mu] & 1) return fail(COARSE_EINVAL, "cagcr_schur: the even/odd decomposition needs even extents");
-        // sites of the other parity are never written by the parity-restricted applies: they must read as zero
-        cudaError_t e = cudaMemsetAsync(work_dev, 0, (size_t)(S1 + 1) * vec, st);
-        if (e != cudaSuccess) return cuda_fail(e, "cagcr_schur: memset work");
-    }
-    auto apply_op = [&](const void* in, void* out) -> int {
-        if (schur_parity < 0) {
-            ++launches;
-            return coarse_op_apply(op, in, out, 1, 0, stream);
-        }
-        launches += 2;
-        int r = coarse_op_apply_parts(op, nullptr, in, tmp, 1, 0, 1 - schur_parity, COARSE_LOCAL_NONE, 0.f, 1.f, stream);
-        if (r != COARSE_OK) return r;
-        return coarse_op_apply_parts(op, in, tmp, out, 1, 0, schur_parity, COARSE_LOCAL_IDENTITY, 1.f, -1.f, stream);
-    };
-    // s + 2 slots used as a ring: p_k = slot[(base + k) % (s+2)], k = 0..s, and the update writes the new
-    // residual into slot[(base + s + 1) % (s+2)], which is p_0 of the next cycle.  In the first cycle
-    // with x = 0 the residual is b itself (no copy): p_0 points at b and slot[base] stays unused.
-    const int NS = S1 + 1;
-    int base = 0;
-    bool p0_is_b = false;
-    if (x_is_zero) {
-        cudaError_t e = cudaMemsetAsync(x_dev, 0, vec, st);
-        if (e != cudaSuccess) return cuda_fail(e, "cagcr: memset x");
-        p0_is_b = true;
-    } else {
-        rc = apply_op(x_dev, slot[1]);
-        if (rc != COARSE_OK) { op->last_launches = launches; return rc; }
-        cagcr_residual_kernel<<<vgrid, 256, 0, st>>>(static_cast<const float2*>(b_dev), slot[1], n, slot[0]);
-        ++launches;
-    }
-    for (int c = 0; c < cycles; ++c) {
-        CagcrVecs v;
-        for (int k = 0; k <= CAGCR_MAX_S; ++k) v.p[k] = k <= s ? slot[(base + k) % NS] : nullptr;
-        if (p0_is_b) v.p[0] = static_cast<const float2*>(b_dev);
-        float2* r_out = slot[(base + s + 1) % NS];
-        for (int k = 0; k < s; ++k) {
-            rc = apply_op(v.p[k], const_cast<float2*>(v.p[k + 1]));
-            if (rc != COARSE_OK) { op->last_launches = launches; return rc; }
-        }
-        cagcr_gram_kernel<<<CAGCR_GRAM_BLOCKS, 256, 0, st>>>(v, n, s, partial);
-        cagcr_solve_kernel<<<1, 320, 0, st>>>(partial, CAGCR_GRAM_BLOCKS, s, alpha, info_dev ? info_dev + 3 * c : nullptr);
-        cagcr_update_kernel<<<vgrid, 256, 0, st>>>(v, n, s, alpha, static_cast<float2*>(x_dev), r_out);
-        launches += 3;
-        {
-            cudaError_t ec = cudaGetLastError();
-            if (ec != cudaSuccess) { op->last_launches = launches; return cuda_fail(ec, "cagcr kernel launch"); }
-        }
-        base = (base + s + 1) % NS;
-        p0_is_b = false;
-    }
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "cagcr kernel launch");
-    op->last_launches = launches;
-    return COARSE_OK;
-}
-
-// Chebyshev-basis variant (cagcr_kernel.cuh): P_k = T_k((A - c)/d) r0, T_k = A P_k kept as separate
-// vectors.  Slots: P_0..P_{s-1} | T_0..T_{s-1} | R (the update's output, swapped with P_0 every cycle).
 static int cagcr_cheb_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
                            float lambda_min, float lambda_max, int schur_parity, void* work_dev, double* info_dev,
                            void* stream) {
@@ -776,7 +683,9 @@ static int cagcr_cheb_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int 
     if (!b_dev || !x_dev || !work_dev) return fail(COARSE_EINVAL, "cagcr_cheb: NULL pointer");
     if (s < 1 || s > CAGCR_MAX_S) return fail(COARSE_EINVAL, "cagcr_cheb: 1 <= s <= %d (got %d)", CAGCR_MAX_S, s);
     if (cycles < 1) return fail(COARSE_EINVAL, "cagcr_cheb: cycles must be >= 1");
-    if (!(lambda_max > lambda_min)) return fail(COARSE_EINVAL, "cagcr_cheb: need lambda_max > lambda_min");
+    const bool auto_interval = lambda_min == 0.f && lambda_max == 0.f;
+    if (!auto_interval && !(lambda_max > lambda_min))
+        return fail(COARSE_EINVAL, "cagcr_cheb: need lambda_max > lambda_min (or both 0: estimate the interval)");
     if (!aligned16(b_dev) || !aligned16(x_dev) || !aligned16(work_dev)) return fail(COARSE_EINVAL, "cagcr_cheb: pointers must be 16-byte aligned");
     { int rc0 = check_device(op, "cagcr_cheb"); if (rc0 != COARSE_OK) return rc0; }
     if (op->path_opt == COARSE_PATH_TENSOR || op->path_opt == COARSE_PATH_BLOCK)
@@ -797,9 +706,14 @@ static int cagcr_cheb_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int 
     float2* tmp = reinterpret_cast<float2*>(w + (size_t)NSLOT * vec);
     double2* partial = reinterpret_cast<double2*>(w + (size_t)(NSLOT + 1) * vec);
     double2* alpha = partial + (size_t)CAGCR_GRAM_BLOCKS * S1 * S1;
+    double* cd = reinterpret_cast<double*>(alpha + CAGCR_MAX_S);          // {c, d} of the Chebyshev interval
     const int vgrid = op->num_sms * 4;
-    const float c = 0.5f * (lambda_max + lambda_min), d = 0.5f * (lambda_max - lambda_min);
     int launches = 0, rc;
+    if (!auto_interval) {
+        cagcr_set_interval_kernel<<<1, 1, 0, st>>>(0.5 * ((double)lambda_max + (double)lambda_min),
+                                                   0.5 * ((double)lambda_max - (double)lambda_min), cd);
+        ++launches;
+    }
     if (schur_parity >= 0) {
         for (int mu = 0; mu < 4; ++mu)
             if (op->lat.L[mu] & 1) return fail(COARSE_EINVAL, "cagcr_cheb: the even/odd decomposition needs even extents");
@@ -838,10 +752,19 @@ static int cagcr_cheb_impl(coarse_op_t* op, const void* b_dev, void* x_dev, int 
         for (int k = 0; k < s; ++k) {
             rc = apply_op(P.p[k], const_cast<float2*>(T.p[k]));
             if (rc != COARSE_OK) { op->last_launches = launches; return rc; }
+            if (k == 0 && cyc == 0 && auto_interval) {
+                // moments of the first residual -> interval, on the device (no host round trip)
+                CagcrVecs Mv;
+                for (int q = 0; q <= CAGCR_MAX_S; ++q) Mv.p[q] = nullptr;
+                Mv.p[0] = P.p[0];
+                Mv.p[1] = T.p[0];
+                cagcr_gram_kernel<<<CAGCR_GRAM_BLOCKS, 256, 0, st>>>(Mv, n, 1, partial);
+                cagcr_interval_kernel<<<1, 32, 0, st>>>(partial, CAGCR_GRAM_BLOCKS, cd);
+                launches += 2;
+            }
             if (k + 1 < s) {
-                const float a = (k == 0 ? 1.f : 2.f) / d;
-                cagcr_cheb_step_kernel<<<vgrid, 256, 0, st>>>(T.p[k], P.p[k], k == 0 ? P.p[k] : P.p[k - 1], a, -a * c,
-                                                              k == 0 ? 0.f : -1.f, n, const_cast<float2*>(P.p[k + 1]));
+                cagcr_cheb_step_kernel<<<vgrid, 256, 0, st>>>(T.p[k], P.p[k], k == 0 ? P.p[k] : P.p[k - 1], cd, k == 0 ? 1 : 0, n,
+                                                              const_cast<float2*>(P.p[k + 1]));
                 ++launches;
             }
         }
@@ -880,13 +803,13 @@ int coarse_op_cagcr_cheb(coarse_op_t* op, const void* b_dev, void* x_dev, int s,
 
 int coarse_op_cagcr(coarse_op_t* op, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
                     void* work_dev, double* info_dev, void* stream) {
-    return cagcr_impl(op, b_dev, x_dev, s, cycles, x_is_zero, -1, work_dev, info_dev, stream);
+    return cagcr_cheb_impl(op, b_dev, x_dev, s, cycles, x_is_zero, 0.f, 0.f, -1, work_dev, info_dev, stream);
 }
 
 int coarse_op_cagcr_schur(coarse_op_t* op_hat, const void* b_dev, void* x_dev, int s, int cycles, int x_is_zero,
                           int parity, void* work_dev, double* info_dev, void* stream) {
     if (parity != 0 && parity != 1) return fail(COARSE_EINVAL, "cagcr_schur: parity must be 0 (even) or 1 (odd)");
-    return cagcr_impl(op_hat, b_dev, x_dev, s, cycles, x_is_zero, parity, work_dev, info_dev, stream);
+    return cagcr_cheb_impl(op_hat, b_dev, x_dev, s, cycles, x_is_zero, 0.f, 0.f, parity, work_dev, info_dev, stream);
 }
 
 static int hat_grid(const coarse_op* op) {
