@@ -174,7 +174,7 @@ int coarse_op_quantize_vec_i16(const void* v_c64_dev, int64_t n_sites, int Nc, i
 /* Same operation on HOST vectors: copies in_host to a device staging buffer owned by the handle
  * (allocated on first use, grown when nrhs grows), applies, copies the result to out_host and
  * synchronises the stream before returning.  Pinned host memory gives full PCIe rate.
- * For 1 RHS on the STREAM kernels with dims[3] >= 8 and vectors of at least 4 MiB the call is
+ * On the STREAM (1-4 RHS) and TENSOR kernels, with dims[3] >= 8 and vectors of at least 4 MiB, the call is
  * pipelined: the lattice is cut into 4 ranges of x3-slices, each launched as soon as the slices it
  * reads are on the device, its result copied back while the next range computes (H2D, kernels and
  * D2H on three streams, two of them owned by the handle); the result is bit-identical. */

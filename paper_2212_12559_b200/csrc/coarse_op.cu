@@ -78,7 +78,7 @@ bool stream_supports(int Nc, int nrhs) {
 
 bool stream_mr_supports(int Nc, int nrhs) { return stream_supports(Nc, 1) && nrhs >= 2 && nrhs <= 4; }
 
-int launch_stream_mr(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, cudaStream_t stream) {
+int launch_stream_mr(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, const PartsSpec& ps, cudaStream_t stream) {
     StreamParams p = {};
     p.lat = op->lat;
     p.links = static_cast<const unsigned char*>(op->links);
@@ -88,6 +88,8 @@ int launch_stream_mr(const coarse_op* op, const void* in, void* out, int nrhs, i
     p.keep_links = op->keep_opt == 2 || (op->keep_opt == 0 && coarse_op_link_bytes(op) <= (size_t)op->l2_bytes / 2);
     p.parity = 2;
     p.n_sites = op->lat.V;
+    p.n_items = ps.site_end > 0 ? ps.site_end : 0;
+    p.item_begin = ps.site_end > 0 ? ps.site_begin : 0;
     switch (op->Nc) {
 #define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_stream_mr_nc, NC)(op, p, nrhs, dagger, stream);
         COARSE_FOR_EACH_NC(COARSE_CASE_NC)
@@ -164,6 +166,11 @@ int launch_tensor(const coarse_op* op, const void* in, void* out, int nrhs, int 
     p.out = static_cast<float2*>(out);
     p.parity = ps.parity;
     p.n_sites = ps.parity == 2 ? op->lat.V : op->lat.V / 2;
+    p.site_begin = 0;
+    if (ps.site_end > 0) {
+        p.site_begin = ps.site_begin;
+        p.n_sites = ps.site_end - ps.site_begin;
+    }
     p.m_begin = ps.local == 1 ? 0 : 1;
     p.identity = ps.local == 2 ? 1 : 0;
     p.alpha = ps.alpha;
@@ -422,7 +429,7 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
         rc = launch_block(op, in_dev, out_dev, nrhs, dagger, st);
     } else if (path == COARSE_PATH_STREAM) {
         if (stream_mr_supports(op->Nc, nrhs))
-            rc = launch_stream_mr(op, in_dev, out_dev, nrhs, dagger, st);
+            rc = launch_stream_mr(op, in_dev, out_dev, nrhs, dagger, kPlain, st);
         else if (!stream_supports(op->Nc, nrhs))
             return fail(COARSE_EUNSUPPORTED, "apply: STREAM path covers nrhs <= 4 (got Nc=%d nrhs=%d)", op->Nc, nrhs);
         else
@@ -559,15 +566,22 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
     }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     cudaError_t e;
-    // Pipelined path (1 RHS on the STREAM kernels, at least 8 time slices): the lattice is cut into 4 ranges
+    // Pipelined path (STREAM kernels for 1-4 RHS, TENSOR kernel beyond; at least 8 time slices): the lattice is cut into 4 ranges
     // of x3-slices; range c is launched as soon as the slices it reads (its own and one on either side)
     // are on the device, and its result goes back to the host while the next range computes.  H2D, the
     // kernels and D2H run on three streams; nothing is reordered inside a range, so the result is
     // bit-identical to the plain path.
     const int T = op->lat.L[3];
-    const bool stream_1rhs = nrhs == 1 && stream_supports(op->Nc, 1) &&
-                             (op->path_opt == COARSE_PATH_AUTO || op->path_opt == COARSE_PATH_STREAM);
-    if (stream_1rhs && T >= 8 && vb >= ((size_t)1 << 22)) {
+    // the family coarse_op_apply would pick; STREAM (1-4 RHS) and TENSOR launch site ranges
+    int hpath = op->path_opt;
+    if (hpath == COARSE_PATH_AUTO)
+        hpath = (stream_supports(op->Nc, nrhs) || stream_mr_supports(op->Nc, nrhs)) ? COARSE_PATH_STREAM
+                : (tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok) ? COARSE_PATH_TENSOR
+                : block_supports(op->Nc, nrhs)                                  ? COARSE_PATH_BLOCK
+                                                                                : COARSE_PATH_SIMPLE;
+    const bool ranged = (hpath == COARSE_PATH_STREAM && (stream_supports(op->Nc, nrhs) || stream_mr_supports(op->Nc, nrhs))) ||
+                        (hpath == COARSE_PATH_TENSOR && tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok);
+    if (ranged && T >= 8 && vb >= ((size_t)1 << 22)) {
         if (!op->host_pipe_ok) {
             // create the two copy streams and nine events; on a partial failure destroy what exists
             cudaStream_t ss[2] = {nullptr, nullptr};
@@ -588,7 +602,7 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
             op->host_pipe_ok = true;
         }
         const size_t plane = (size_t)(op->lat.V / T);               // sites per x3-slice
-        const size_t pb = plane * op->Nc * 8;                        // bytes per slice
+        const size_t pb = plane * op->Nc * nrhs * 8;                 // bytes per slice
         const unsigned char* hin = static_cast<const unsigned char*>(in_host);
         unsigned char* hout = static_cast<unsigned char*>(out_host);
         unsigned char* din = static_cast<unsigned char*>(op->stage_in);
@@ -624,15 +638,18 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
             if ((e = cudaStreamWaitEvent(st, op->ev_up[c], 0)) != cudaSuccess) return bail_cuda(e, "apply_host: stream wait");
             ps.site_begin = (int)(plane * t0);
             ps.site_end = (int)(plane * t1);
-            rc = launch_stream(op, op->stage_in, op->stage_out, dagger, ps, st);
-            if (rc != COARSE_OK) { drain(); return rc; }
-            op->last_launches += 1;
+            if (hpath == COARSE_PATH_TENSOR) rc = launch_tensor(op, op->stage_in, op->stage_out, nrhs, dagger, ps, st);
+            else if (nrhs == 1) rc = launch_stream(op, op->stage_in, op->stage_out, dagger, ps, st);
+            else rc = launch_stream_mr(op, op->stage_in, op->stage_out, nrhs, dagger, ps, st);
+            if (rc < 0) { drain(); return rc; }
+            op->last_launches += 1 + rc;
             if ((e = cudaEventRecord(op->ev_k[c], st)) != cudaSuccess) return bail_cuda(e, "apply_host: event record");
             if ((e = cudaStreamWaitEvent(op->s_d2h, op->ev_k[c], 0)) != cudaSuccess) return bail_cuda(e, "apply_host: stream wait");
             e = cudaMemcpyAsync(hout + (size_t)t0 * pb, dout + (size_t)t0 * pb, (size_t)(t1 - t0) * pb, cudaMemcpyDeviceToHost, op->s_d2h);
             if (e != cudaSuccess) return bail_cuda(e, "apply_host: D2H copy");
         }
-        op->last_path = COARSE_PATH_STREAM;
+        op->last_path = hpath;
+        op->links_fresh = false;
         if ((e = cudaEventRecord(op->ev_done, op->s_d2h)) != cudaSuccess) return bail_cuda(e, "apply_host: event record");
         if ((e = cudaStreamWaitEvent(st, op->ev_done, 0)) != cudaSuccess) return bail_cuda(e, "apply_host: stream wait");
         e = cudaStreamSynchronize(st);

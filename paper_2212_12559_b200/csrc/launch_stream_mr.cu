@@ -16,6 +16,11 @@ int launch_stream_mr_t(const coarse_op* op, const StreamParams& base, cudaStream
     using Gr = StreamMrGeom<NC, I16, R>;
     StreamParams p = base;
     p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
+    p.item_begin = 0;
+    if (base.n_items > 0) {                       // a site range [item_begin, n_items) was requested (in sites)
+        p.item_begin = DAG ? base.item_begin : base.item_begin * Gm::NB;
+        p.n_items = DAG ? base.n_items : base.n_items * Gm::NB;
+    }
     int stages = (op->max_smem - Gr::fixed_bytes(DAG)) / (Gr::stage_bytes(DAG) + 16);
     if (stages > 12) stages = 12;
     if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM-MR: shared memory too small for Nc=%d nrhs=%d", NC, R);
@@ -30,7 +35,8 @@ int launch_stream_mr_t(const coarse_op* op, const StreamParams& base, cudaStream
     cudaError_t e = ensure_dynamic_smem(kern, op->device, smem, attr_cache);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream-mr kernel)");
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
-    if (grid > p.n_items) grid = p.n_items;
+    if (grid > p.n_items - p.item_begin) grid = p.n_items - p.item_begin;
+    if (grid < 1) return COARSE_OK;
     kern<<<grid, Gm::THREADS, smem, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "stream-mr kernel launch");

@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
         const uint32_t link_u32 = ptx::smem_u32(link_smem), vec_u32 = ptx::smem_u32(vec_smem);
         int slot = 0;
         uint32_t phase = 0;
-        for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+        for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
             const int s = DAG ? item : item / NB;
             const int rb = DAG ? 0 : item % NB;
             const SiteX cx = site_coords(p.lat, s);
@@ -120,10 +120,10 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
         const int sm = DAG ? stencil_site(p.lat, s, lane, 1) : s;
         return __ldg(p.scales + (int64_t)sm * 9 + lane);
     };
-    next_scale = fetch_scale(blockIdx.x);
-    next2_scale = fetch_scale(blockIdx.x + gridDim.x);
+    next_scale = fetch_scale(p.item_begin + blockIdx.x);
+    next2_scale = fetch_scale(p.item_begin + blockIdx.x + gridDim.x);
 
-    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+    for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
         const int s = DAG ? item : item / NB;
         const int rb = DAG ? 0 : item % NB;
         cur_scale = next_scale;

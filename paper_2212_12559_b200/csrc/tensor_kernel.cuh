@@ -52,7 +52,8 @@ struct TensorParams {
     const float2* in;         // w: operand of the hopping terms (plain apply: the input vector)
     const float2* in_local;   // u: operand of the X term and of the identity term (plain apply: = in)
     float2* out;
-    int n_sites;              // sites of the parity set (plain apply: V)
+    int n_sites;              // sites of the parity set (plain apply: V), or of the site range
+    int site_begin;           // first site (index in the parity list) of this launch: coarse_op_apply_host launches ranges
     int parity;               // 0 even, 1 odd, 2 all sites
     int m_begin;              // 0: the X stage runs; 1: it is skipped (local = none | identity)
     int identity;             // 1: add alpha * u(x) to the result
@@ -219,7 +220,7 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
     const int M0 = p.m_begin;
     const int n_mat_item = 9 - M0;                                   // link matrices per item
     auto site_of_item = [&](int item) -> int {
-        const int h = NT == 1 ? item : item / NT;
+        const int h = (NT == 1 ? item : item / NT) + p.site_begin;
         return p.parity != 2 ? parity_site(p.lat, h, p.parity) : h;
     };
 

@@ -491,6 +491,37 @@ def test_apply_host_pipelined_path_is_bit_identical(oracle_lib, prec):
     op.close()
 
 
+@pytest.mark.parametrize("Nc,prec,nrhs,want_path,launches", [
+    (48, cop.LINK_I16, 3, cop.PATH_STREAM, 4), (64, cop.LINK_C64, 16, cop.PATH_TENSOR, 4),
+    (48, cop.LINK_I16, 20, cop.PATH_TENSOR, 8)])
+def test_apply_host_pipelined_multi_rhs_is_bit_identical(oracle_lib, Nc, prec, nrhs, want_path, launches):
+    """The pipelined host path for several right-hand sides: STREAM-MR (3 = one propagator) and
+    TENSOR launch ranges of x3-slices too; results must equal the device-resident apply bit for bit."""
+    dims = (8, 8, 8, 16)                      # vectors of at least 4 MiB: the pipelined path
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, 5, device="cuda")
+    scales = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+        scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        torch.cuda.synchronize()
+        links = q
+    vin_d = synth.make_vectors(dims, Nc, nrhs, 6, device="cuda")
+    vin = vin_d.cpu().pin_memory()
+    vout = torch.empty_like(vin).pin_memory()
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    for dagger in (0, 1):
+        ref = torch.empty_like(vin_d)
+        op.apply(vin_d, ref, nrhs=nrhs, dagger=dagger)
+        torch.cuda.synchronize()
+        vout.fill_(float("nan"))
+        op.apply_host(vin, vout, nrhs=nrhs, dagger=dagger)
+        assert op.last_launches == launches and op.last_path == want_path
+        assert torch.equal(torch.view_as_real(vout), torch.view_as_real(ref.cpu()))
+    op.close()
+
+
 # ------------------------------------------------------------------ ABI behaviour
 def test_error_codes():
     dims, Nc = (2, 2, 2, 2), 48
