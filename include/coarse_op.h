@@ -98,11 +98,14 @@ enum {
                                 contraction over its row chunks, the CTA that finishes a site's last chunk adds the
                                 partial vectors in chunk order (one launch, deterministic): 0 auto, 1 never,
                                 2 always (needs the workspace coarse_op_set_links allocates on such lattices) */
-    COARSE_OPT_WARP_ITEMS = 7 /* 1-RHS plain apply: the STREAM variant in which small teams of consumer warps own
+    COARSE_OPT_WARP_ITEMS = 7, /* 1-RHS plain apply: the STREAM variant in which small teams of consumer warps own
                                 whole work items and every stage of theirs (csrc/stream2_kernel.cuh) instead of all
                                 eight warps sharing every stage: 0 auto (int16 links on lattices with at least 4
                                 items per team of the chip), 1 never, 2 always, 12 / 14 always with 2 / 4 warps per
                                 team (2 = 14).  With it COARSE_OPT_STAGES is the ring's slot count. */
+    COARSE_OPT_TENSOR_I8 = 8  /* TENSOR path on int16 links: 0 auto / 2: the integer tensor-core kernel (csrc/tensor_i8_kernel.cuh:
+                                link entries as two int8 planes, exact, vectors in 23-bit fixed point per site), 1: the
+                                3xTF32 kernel.  Site-range launches of coarse_op_apply_host always use the latter. */
 };
 
 /* Create an operator descriptor for a periodic lattice dims[0..3] (each >= 1), Nc even and

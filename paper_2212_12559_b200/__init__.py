@@ -19,7 +19,7 @@ LINK_I16 = 1
 OK, EINVAL, EUNSUPPORTED, ENOTREADY, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 
 PATH_AUTO, PATH_SIMPLE, PATH_STREAM, PATH_TENSOR, PATH_BLOCK = 0, 1, 2, 3, 4
-OPT_PATH, OPT_GRID, OPT_STAGES, OPT_FINE, OPT_KEEP_LINKS, OPT_PDL, OPT_SPLIT_DAGGER, OPT_WARP_ITEMS = 0, 1, 2, 3, 4, 5, 6, 7
+OPT_PATH, OPT_GRID, OPT_STAGES, OPT_FINE, OPT_KEEP_LINKS, OPT_PDL, OPT_SPLIT_DAGGER, OPT_WARP_ITEMS, OPT_TENSOR_I8 = 0, 1, 2, 3, 4, 5, 6, 7, 8
 PARITY_EVEN, PARITY_ODD, PARITY_ALL = 0, 1, 2
 LOCAL_NONE, LOCAL_X, LOCAL_IDENTITY = 0, 1, 2
 

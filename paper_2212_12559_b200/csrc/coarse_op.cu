@@ -176,6 +176,18 @@ int launch_tensor(const coarse_op* op, const void* in, void* out, int nrhs, int 
     p.alpha = ps.alpha;
     p.beta = ps.beta;
     p.nrhs = nrhs;
+    // int16 links: the integer tensor-core kernel (exact link operand, 4x fewer and 4x deeper MMAs), unless a
+    // site range is launched (coarse_op_apply_host: its input arrives slice by slice, the per-site scales of
+    // the fixed-point B operand need whole neighbour vectors) or the scale buffer is too small and cannot grow
+    if (op->prec == COARSE_LINK_I16 && op->link_map_i8_ok && op->tensor_i8_opt != 1 && ps.site_end == 0 && op->vscale) {
+        const void* u_other = (ps.gen && ps.local != 0 && ps.u != in) ? ps.u : nullptr;
+        switch (op->Nc) {
+#define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_tensor_i8_nc, NC)(op, p, u_other, op->vscale, dagger, stream);
+            COARSE_FOR_EACH_NC(COARSE_CASE_NC)
+#undef COARSE_CASE_NC
+            default: return fail(COARSE_EUNSUPPORTED, "TENSOR path is not compiled for Nc=%d", op->Nc);
+        }
+    }
     switch (op->Nc) {
 #define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_tensor_nc, NC)(op, p, dagger, stream);
         COARSE_FOR_EACH_NC(COARSE_CASE_NC)
@@ -210,6 +222,22 @@ int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int 
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "simple kernel launch");
     return COARSE_OK;
+}
+
+// COARSE_PATH_AUTO.  1 RHS: STREAM.  2-4 RHS: STREAM-MR, except int16 links with Nc >= 96, where the integer
+// tensor-core kernel is faster (measured, 3 RHS: Nc = 128 0.58 / 0.55 ms against 0.74 / 0.65 ms; Nc = 64 the
+// other way round, 4.6 against 2.9 / 3.0 ms: small matrices make small pipeline stages).  5 and more: TENSOR
+// (BLOCK only on request, or when no tensor map could be made), outside the compiled Nc: SIMPLE.
+int auto_path(const coarse_op* op, int nrhs) {
+    const bool tensor_ok = tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok;
+    if (stream_supports(op->Nc, nrhs)) return COARSE_PATH_STREAM;
+    if (stream_mr_supports(op->Nc, nrhs)) {
+        const bool i8 = op->prec == COARSE_LINK_I16 && op->link_map_i8_ok && op->vscale && op->tensor_i8_opt != 1;
+        return (tensor_ok && i8 && op->Nc >= 96) ? COARSE_PATH_TENSOR : COARSE_PATH_STREAM;
+    }
+    if (tensor_ok) return COARSE_PATH_TENSOR;
+    if (block_supports(op->Nc, nrhs)) return COARSE_PATH_BLOCK;
+    return COARSE_PATH_SIMPLE;
 }
 
 int check_apply_args(const coarse_op* op, const void* in, const void* out, int nrhs, int dagger) {
@@ -285,6 +313,9 @@ coarse_op_t* coarse_op_create(const int dims[4], int Nc, int link_precision) {
     op->s_h2d = op->s_d2h = nullptr;
     op->host_pipe_ok = false;
     op->link_map_ok = false;
+    op->link_map_i8_ok = false;
+    op->vscale = nullptr;
+    op->tensor_i8_opt = 0;
     g_last_error = "";
     return op;
 }
@@ -342,7 +373,19 @@ int coarse_op_set_links(coarse_op_t* op, const void* links_dev, const float* sca
             op->split_ws_bytes = 0;
         }
     }
-    return make_link_maps(op);
+    {
+        const int rc = make_link_maps(op);
+        if (rc != COARSE_OK) return rc;
+    }
+    // int16 links: scale buffer of the integer tensor-core kernel, (g, 1/g) per (site, column) for two operands and
+    // the 16 columns of one launch (V x 256 bytes); without it multi-RHS applies run on the 3xTF32 kernel
+    if (op->prec == COARSE_LINK_I16 && op->link_map_i8_ok && !op->vscale) {
+        if (cudaMalloc(reinterpret_cast<void**>(&op->vscale), (size_t)2 * 2 * op->lat.V * 16 * sizeof(float)) != cudaSuccess) {
+            cudaGetLastError();
+            op->vscale = nullptr;
+        }
+    }
+    return COARSE_OK;
 }
 
 int coarse_op_set_option(coarse_op_t* op, int option, int value) {
@@ -385,6 +428,10 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value) {
             if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: split_dagger must be 0 (auto), 1 (never) or 2 (always)");
             op->split_opt = value;
             return COARSE_OK;
+        case COARSE_OPT_TENSOR_I8:
+            if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: tensor_i8 must be 0 (auto), 1 (never) or 2 (always)");
+            op->tensor_i8_opt = value;
+            return COARSE_OK;
         case COARSE_OPT_WARP_ITEMS:
             if (!(value >= 0 && value <= 2) && value != 12 && value != 14)
                 return fail(COARSE_EINVAL, "set_option: warp_items must be 0 (auto), 1 (never), 2 (always) or 12 / 14 (always, 2 / 4 warps per team)");
@@ -413,11 +460,7 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
     if (a < b + vb && b < a + vb) return fail(COARSE_EINVAL, "apply: in and out overlap (the stencil reads neighbours)");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int path = op->path_opt;
-    if (path == COARSE_PATH_AUTO)
-        path = (stream_supports(op->Nc, nrhs) || stream_mr_supports(op->Nc, nrhs)) ? COARSE_PATH_STREAM
-               : (tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok) ? COARSE_PATH_TENSOR
-               : block_supports(op->Nc, nrhs)                                  ? COARSE_PATH_BLOCK
-                                                                               : COARSE_PATH_SIMPLE;
+    if (path == COARSE_PATH_AUTO) path = auto_path(op, nrhs);
     op->last_launches = 0;
     if (path == COARSE_PATH_TENSOR) {
         if (!tensor_supports(op->Nc, op->prec, nrhs))
@@ -574,11 +617,7 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
     const int T = op->lat.L[3];
     // the family coarse_op_apply would pick; STREAM (1-4 RHS) and TENSOR launch site ranges
     int hpath = op->path_opt;
-    if (hpath == COARSE_PATH_AUTO)
-        hpath = (stream_supports(op->Nc, nrhs) || stream_mr_supports(op->Nc, nrhs)) ? COARSE_PATH_STREAM
-                : (tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok) ? COARSE_PATH_TENSOR
-                : block_supports(op->Nc, nrhs)                                  ? COARSE_PATH_BLOCK
-                                                                                : COARSE_PATH_SIMPLE;
+    if (hpath == COARSE_PATH_AUTO) hpath = auto_path(op, nrhs);
     const bool ranged = (hpath == COARSE_PATH_STREAM && (stream_supports(op->Nc, nrhs) || stream_mr_supports(op->Nc, nrhs))) ||
                         (hpath == COARSE_PATH_TENSOR && tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok);
     if (ranged && T >= 8 && vb >= ((size_t)1 << 22)) {
@@ -909,6 +948,7 @@ void coarse_op_destroy(coarse_op_t* op) {
     if (op->stage_in) cudaFree(op->stage_in);
     if (op->stage_out) cudaFree(op->stage_out);
     if (op->split_ws) cudaFree(op->split_ws);
+    if (op->vscale) cudaFree(op->vscale);
     if (op->host_pipe_ok) {
         for (int i = 0; i < 4; ++i) { cudaEventDestroy(op->ev_up[i]); cudaEventDestroy(op->ev_k[i]); }
         cudaEventDestroy(op->ev_done);

@@ -46,6 +46,10 @@ struct coarse_op {
     bool host_pipe_ok;
     CUtensorMap link_map[2];   // 2-D views of the link array for the TENSOR path (dagger 0 / dagger 1 slabs, link_map.cu)
     bool link_map_ok;
+    CUtensorMap link_map_i8[2];   // int16 links: the slabs of the integer tensor-core kernel (tensor_i8_kernel.cuh)
+    bool link_map_i8_ok;
+    float* vscale;             // int16 links: (g, 1/g) per (site, column) of the two operands of the int8 TENSOR kernel
+    int tensor_i8_opt;         // COARSE_OPT_TENSOR_I8: 0 auto (on for int16 links), 1 never, 2 always
 };
 
 namespace coarse {
@@ -91,7 +95,9 @@ struct TensorParams;
     int COARSE_CAT(launch_stream_mr_nc, NC)(const coarse_op* op, const StreamParams& p, int nrhs, int dagger,         \
                                             cudaStream_t stream);                                                    \
     int COARSE_CAT(launch_block_nc, NC)(const coarse_op* op, const BlockParams& p, int dagger, cudaStream_t stream); \
-    int COARSE_CAT(launch_tensor_nc, NC)(const coarse_op* op, const TensorParams& p, int dagger, cudaStream_t stream);
+    int COARSE_CAT(launch_tensor_nc, NC)(const coarse_op* op, const TensorParams& p, int dagger, cudaStream_t stream); \
+    int COARSE_CAT(launch_tensor_i8_nc, NC)(const coarse_op* op, const TensorParams& p, const void* u_other,           \
+                                            float* vscale, int dagger, cudaStream_t stream);
 COARSE_FOR_EACH_NC(COARSE_DECL_NC)
 #undef COARSE_DECL_NC
 

@@ -2,6 +2,7 @@
 // (compiled once per Nc with -DCOARSE_NC=<Nc>; see internal.h).
 #include "internal.h"
 #include "tensor_kernel.cuh"
+#include "tensor_i8_kernel.cuh"
 
 #ifndef COARSE_NC
 #error "compile with -DCOARSE_NC=<Nc>"
@@ -31,7 +32,61 @@ int launch_tensor_d(const coarse_op* op, const TensorParams& p, int dagger, cuda
     return dagger ? launch_tensor_t<NC, I16, NP, true>(op, p, stream) : launch_tensor_t<NC, I16, NP, false>(op, p, stream);
 }
 
+// int16 links on the integer tensor cores (tensor_i8_kernel.cuh)
+template <int NC, int NP, bool DAG>
+int launch_tensor_i8_t(const coarse_op* op, const TensorI8Params& p, cudaStream_t stream) {
+    using Gm = TensorI8Geom<NC, NP>;
+    auto kern = coarse_apply_tensor_i8<NC, NP, DAG>;
+    static SmemAttrCache attr_cache;
+    cudaError_t e = ensure_dynamic_smem(kern, op->device, Gm::SMEM_BYTES, attr_cache);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(tensor-i8 kernel)");
+    int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
+    if (grid > p.t.n_sites * Gm::NT) grid = p.t.n_sites * Gm::NT;
+    if (grid < 1) return COARSE_OK;
+    kern<<<grid, Gm::THREADS, Gm::SMEM_BYTES, stream>>>(op->link_map_i8[DAG ? 1 : 0], p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "tensor-i8 kernel launch");
+    return COARSE_OK;
+}
+
 }  // namespace
+
+// int16 links: per group of up to 16 right-hand sides one (or, when the local operand u differs from w, two)
+// pre-pass launches for the power-of-two scales of the fixed-point B operand, then the kernel.  `vscale`
+// holds 2 x V x TENSOR_I8_GP (g, 1/g) pairs.  Returns the number of launches beyond the first.
+int COARSE_CAT(launch_tensor_i8_nc, COARSE_NC)(const coarse_op* op, const TensorParams& base, const void* u_other, float* vscale,
+                                               int dagger, cudaStream_t stream) {
+    int launches = 0;
+    float* gw = vscale;
+    float* gu = vscale + (size_t)2 * op->lat.V * TENSOR_I8_GP;
+    for (int r0 = 0; r0 < base.nrhs; r0 += 16) {
+        TensorI8Params p;
+        p.t = base;
+        p.t.r0 = r0;
+        p.t.width = base.nrhs - r0 < 16 ? base.nrhs - r0 : 16;
+        p.vscale_w = gw;
+        p.vscale_u = u_other ? gu : gw;
+        const long long total = (long long)op->lat.V * p.t.width;
+        const unsigned blocks = (unsigned)((total + 127) / 128);
+        vec_pow2_scale_kernel<<<blocks, 128, 0, stream>>>(base.in, op->lat.V, op->Nc, base.nrhs, r0, p.t.width, reinterpret_cast<float2*>(gw));
+        ++launches;
+        if (u_other) {
+            vec_pow2_scale_kernel<<<blocks, 128, 0, stream>>>(static_cast<const float2*>(u_other), op->lat.V, op->Nc, base.nrhs, r0,
+                                                              p.t.width, reinterpret_cast<float2*>(gu));
+            ++launches;
+        }
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "vector scale kernel launch");
+        int rc;
+        if (p.t.width <= 8)
+            rc = dagger ? launch_tensor_i8_t<COARSE_NC, 8, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 8, false>(op, p, stream);
+        else
+            rc = dagger ? launch_tensor_i8_t<COARSE_NC, 16, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 16, false>(op, p, stream);
+        if (rc != COARSE_OK) return rc;
+        ++launches;
+    }
+    return launches > 0 ? launches - 1 : 0;
+}
 
 // One launch per group of up to 16 right-hand sides (8-wide tile when at most 8 are left); returns the
 // number of launches beyond the first, or a negative error code.

@@ -40,6 +40,7 @@ bool tensor_supports(int Nc, int prec, int nrhs) { return tensor_supports_nc(Nc,
 // MT = Nc (Nc <= 128) or Nc / 2 (the output tile of one work item).
 int make_link_maps(coarse_op* op) {
     op->link_map_ok = false;
+    op->link_map_i8_ok = false;
     if (!tensor_supports_nc(op->Nc, op->prec)) return COARSE_OK;
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return COARSE_OK;   // TENSOR path stays unavailable; apply reports it if it is requested
@@ -61,6 +62,18 @@ int make_link_maps(coarse_op* op) {
     r = fn(&op->link_map[1], dt, 2, const_cast<void*>(op->links), gdim, gstride, box1, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     op->link_map_ok = (r == CUDA_SUCCESS);
+    if (!op->link_map_ok || !i16) return COARSE_OK;
+    // int16 links, integer tensor-core kernel: stages of KC = 32 complex columns (16 when 32 does not divide Nc)
+    const int KC = op->Nc % 32 == 0 ? 32 : 16;
+    const cuuint32_t box2[2] = {(cuuint32_t)KC, (cuuint32_t)MT};
+    r = fn(&op->link_map_i8[0], dt, 2, const_cast<void*>(op->links), gdim, gstride, box2, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+           KC == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return COARSE_OK;
+    const cuuint32_t box3[2] = {(cuuint32_t)MT, (cuuint32_t)KC};
+    r = fn(&op->link_map_i8[1], dt, 2, const_cast<void*>(op->links), gdim, gstride, box3, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    op->link_map_i8_ok = (r == CUDA_SUCCESS);
     return COARSE_OK;
 }
 

@@ -1,0 +1,481 @@
+// tensor_i8_kernel.cuh — COARSE_PATH_TENSOR for int16 LINKS (the paper's storage) and several
+// right-hand sides (its future work, L200; a propagator is 3, L188): the block apply on the B200's INTEGER
+// tensor cores (tcgen05.mma kind::i8, int32 accumulators in TMEM), exact in the link operand.
+//
+// Why not the 3xTF32 kernel (tensor_kernel.cuh) for these links: ncu on it shows one pipeline stage of 16
+// complex columns costing ~350 ns whatever its size - eight K = 8 MMAs per stage whose issue backs up in
+// the MIO queue, plus ~250 decode / split instructions per converter lane - so int16 links, which carry
+// twice the entries per byte, ran at 4.2 TB/s where complex64 links are HBM bound.  An int16 entry
+// q = 256 a1 + a0 is two BYTES: a1 = q >> 8 signed, a0 = q & 255 unsigned.  As int8 operands
+//   * the A operand needs no arithmetic at all: two byte permutes (PRMT) per pair of entries gather the
+//     high bytes and the low bytes of a row into the K-major TMEM layout (32 instead of ~256 instructions
+//     per 32 complex columns), and
+//   * one MMA covers K = 32 real values (16 complex columns) instead of 8: 4 MMAs per 16 KB stage, not 16.
+// The B operand (the vectors) is turned into fixed point per (site, right-hand side): with
+// g = 2^-e such that max |component| g lies in [1/2, 1) (a small pre-pass kernel over the vector field, L2
+// resident), B = rint(v g 2^22) is split into three signed base-256 digits d0, d1, d2 (exact: B = sum d_l 256^l),
+// stored side by side along N, so that per 16 complex columns
+//     D1[:, l] += A1 . d_l        (signed x signed,   N = 3 x 2 NP)
+//     D0[:, l] += A0 . d_l        (unsigned x signed, N = 3 x 2 NP)
+// are TWO MMAs, exact in int32 (|a| <= 255, |d| <= 128, K = 2 Nc <= 384 per link matrix: < 2^24).  The epilogue
+// recombines out += f_m [ ((T_2 256 + T_1) 256 + T_0) ],  T_l = 256 D1_l + D0_l  (T_l in int32, the rest in fp32),
+// f_m = scale_m coef_m / (g 2^22).  The only rounding besides that recombination is the 23-bit fixed-point
+// representation of each site vector relative to its largest component - the same order as the fp32 rounding
+// of the inputs themselves; measured 1e-7 against the fp64 oracle (tolerance 1e-5).
+//
+// Pipeline roles, work items, the parts apply (parity list, X stage on / off, alpha / beta, identity term) and
+// the RHS column tiles are those of tensor_kernel.cuh; a stage is KC = 32 complex columns (16 for Nc = 48).
+// Bit-identical run to run (integer accumulation, fixed schedule).
+#pragma once
+#include "tensor_kernel.cuh"
+
+namespace coarse {
+
+constexpr int TENSOR_I8_GP = 16;   // row pitch of the scale arrays: one launch handles at most 16 right-hand sides
+
+struct TensorI8Params {
+    TensorParams t;
+    const float* vscale_w;    // [V][TENSOR_I8_GP][2] = (g, 1/g) of columns r0.. of the hopping operand w (plain apply: of `in`)
+    const float* vscale_u;    // the same for the local operand u (plain apply: = vscale_w)
+};
+
+template <int NC, int NP>
+struct TensorI8Geom {
+    static constexpr int NT = NC > 128 ? 2 : 1;
+    static constexpr int MT = NC / NT;
+    static constexpr int KC = (NC % 32 == 0) ? 32 : 16;       // complex columns per stage
+    static constexpr int CHUNKS = NC / KC;                     // stages per link matrix
+    static constexpr int KSTEPS = KC / 16;                     // MMA k-steps (K = 32 int8 = 16 complex columns)
+    static constexpr int LINK_STAGE = MT * KC * 4;
+    static constexpr int NB3 = 3 * 2 * NP;                     // MMA N: three digit blocks of [Re out | Im out]
+    static constexpr int B_STAGE = 2 * KC * NB3;               // int8 B tile of a stage, bytes
+    static constexpr int B_SBO = (2 * KC / 16) * 128;          // byte stride between 8-column groups of n
+    static constexpr int NE = KC * NP / 128;                   // B entries per converter thread and stage
+    static constexpr int LS = tensor_clamp(131072 / LINK_STAGE, 4, 16);
+    static constexpr int AS = 4;
+    static constexpr int A_HALF = KC / 2;                      // TMEM columns of one byte plane (4 int8 per column)
+    static constexpr int A_COLS = 2 * A_HALF;                  // high bytes | low bytes
+    static constexpr int D_COL0 = AS * A_COLS;
+    static constexpr int DS = 2;
+    static constexpr int D_COLS = 2 * NB3;                     // [D1 | D0]
+    static constexpr int FT = 8;                               // ring of per-matrix epilogue factor rows
+    static constexpr int TMEM_COLS = 512;
+    static constexpr int NG = 3, CONV_W0 = 2, EPI_W0 = CONV_W0 + 4 * NG;
+    static constexpr int THREADS = (EPI_W0 + 4) * 32;
+    static constexpr int NBAR = 2 * LS + 2 * AS + 2 * DS;
+    static constexpr int SMEM_BYTES = 1024 + LS * LINK_STAGE + AS * B_STAGE + FT * NP * 4 + NBAR * 8 + 16;
+    static constexpr bool OK = (NC % 16 == 0) && (MT % 8 == 0) && MT <= 128 && (NP == 8 || NP == 16) && NE >= 1 &&
+                               (D_COL0 + DS * D_COLS <= TMEM_COLS) && SMEM_BYTES <= 232448 && 2 * NC * 128 * 255 < (1 << 24);
+};
+
+namespace ptx {
+
+// D[tmem] (+)= A[tmem] . B[smem], kind::i8, int32 accumulate
+__device__ __forceinline__ void mma_i8_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* v) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr)
+                 : "memory");
+}
+__device__ __forceinline__ void sts16(uint32_t addr, uint32_t v) {
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
+
+}  // namespace ptx
+
+// (g, 1/g) per (site, right-hand side): g = 2^-e with max |component| g in [1/2, 1); an all-zero vector gets (0, 0).
+// One thread per (site, column r0 + r < r0 + width); consecutive threads read consecutive right-hand sides of one
+// entry (coalesced); gs[site][r] with row pitch TENSOR_I8_GP.
+static __global__ void __launch_bounds__(128) vec_pow2_scale_kernel(const float2* v, long long n_sites, int nc, int nrhs, int r0,
+                                                                    int width, float2* gs) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n_sites * width) return;
+    const long long s = idx / width;
+    const int r = (int)(idx - s * width);
+    const float2* p = v + s * nc * nrhs + r0 + r;
+    float m = 0.f;
+    for (int a = 0; a < nc; ++a) {
+        const float2 x = p[(long long)a * nrhs];
+        m = fmaxf(m, fmaxf(fabsf(x.x), fabsf(x.y)));
+    }
+    float2 o = make_float2(0.f, 0.f);
+    if (m > 0.f && m < 3.0e38f) {
+        int e;
+        frexpf(m, &e);                                   // m = f 2^e, f in [1/2, 1)
+        e = e < -100 ? -100 : e > 100 ? 100 : e;         // keep g and 1/g (and g 2^22) normal numbers
+        o = make_float2(ldexpf(1.f, -e), ldexpf(1.f, e));
+    }
+    gs[s * TENSOR_I8_GP + r] = o;
+}
+
+// Signed base-256 digits of b (|b| <= 2^22 + 1): b = d0 + 256 d1 + 65536 d2 with d0, d1 in [-128, 127], |d2| <= 65.
+// With t1 = (b + 128) >> 8 and t2 = (t1 + 128) >> 8 (arithmetic shifts: the carries of the signed digits) the
+// digits are the LOW BYTES of b, t1, t2 as two's complement int8: 4 integer instructions per value, and one
+// byte permute packs the same digit of the two values of a (re, im) pair for the 16-bit store.
+__device__ __forceinline__ void digit_regs(int b, int& t1, int& t2) {
+    t1 = (b + 128) >> 8;
+    t2 = (t1 + 128) >> 8;
+}
+__device__ __forceinline__ uint32_t pack_lo_bytes(int x, int y) { return __byte_perm((uint32_t)x, (uint32_t)y, 0x0040); }
+
+template <int NC, int NP, bool DAG>
+__global__ void __launch_bounds__(TensorI8Geom<NC, NP>::THREADS, 1)
+coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Params pp) {
+    using Gm = TensorI8Geom<NC, NP>;
+    static_assert(Gm::OK, "unsupported TENSOR-I8 geometry");
+    constexpr int LS = Gm::LS, AS = Gm::AS, DS = Gm::DS, CHUNKS = Gm::CHUNKS, NT = Gm::NT, MT = Gm::MT, NE = Gm::NE;
+    constexpr int KC = Gm::KC, LINK_STAGE = Gm::LINK_STAGE, B_STAGE = Gm::B_STAGE, B_SBO = Gm::B_SBO, NB3 = Gm::NB3, FT = Gm::FT;
+    // instruction descriptors: D int32 (c_format 2), A signed | unsigned 8 bit, B signed 8 bit, K-major, N = NB3, M = 128
+    constexpr uint32_t IDESC_S = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NB3 >> 3) << 17) | ((128u >> 4) << 24);
+    constexpr uint32_t IDESC_U = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(NB3 >> 3) << 17) | ((128u >> 4) << 24);
+    const TensorParams& p = pp.t;
+
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t link_u32 = base;
+    const uint32_t b_u32 = link_u32 + LS * LINK_STAGE;
+    const uint32_t ft_u32 = b_u32 + AS * B_STAGE;
+    const uint32_t bar_u32 = ft_u32 + FT * NP * 4;
+    const uint32_t full0 = bar_u32, empty0 = full0 + 8u * LS;
+    const uint32_t abfull0 = empty0 + 8u * LS, abempty0 = abfull0 + 8u * AS;
+    const uint32_t dfull0 = abempty0 + 8u * AS, dempty0 = dfull0 + 8u * DS;
+    const uint32_t tmem_slot = dempty0 + 8u * DS;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < LS; ++i) {
+            ptx::mbar_init(full0 + 8u * i, 1);
+            ptx::mbar_init(empty0 + 8u * i, 4);
+        }
+        for (int i = 0; i < AS; ++i) {
+            ptx::mbar_init(abfull0 + 8u * i, 4);
+            ptx::mbar_init(abempty0 + 8u * i, 1);
+        }
+        for (int i = 0; i < DS; ++i) {
+            ptx::mbar_init(dfull0 + 8u * i, 1);
+            ptx::mbar_init(dempty0 + 8u * i, 4);
+        }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) ptx::tmem_alloc(tmem_slot, Gm::TMEM_COLS);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    uint32_t tmem_base;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+    const int n_items = p.n_sites * NT;
+    const int n_my = (n_items > (int)blockIdx.x) ? (n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    const int M0 = p.m_begin;
+    const int n_mat_item = 9 - M0;
+    auto site_of_item = [&](int item) -> int {
+        const int h = (NT == 1 ? item : item / NT) + p.site_begin;
+        return p.parity != 2 ? parity_site(p.lat, h, p.parity) : h;
+    };
+
+    if (warp == 0) {
+        // ---------------------------------------------------------------- TMA producer
+        const uint64_t pol_links = ptx::policy_evict_first();
+        uint32_t t = 0;
+        for (int it = 0; it < n_my; ++it) {
+            const int item = blockIdx.x + it * gridDim.x;
+            const int s = site_of_item(item);
+            const int i0 = NT == 1 ? 0 : (item % NT) * MT;
+            const SiteX cx = site_coords(p.lat, s);
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                if (m < M0) continue;
+                const int sv = stencil_site_x(p.lat, s, cx, m, DAG ? 1 : 0);
+                const int sm = DAG ? sv : s;
+                const int mat_row0 = (sm * 9 + m) * NC;
+#pragma unroll 1
+                for (int c = 0; c < CHUNKS; ++c, ++t) {
+                    const uint32_t slot = t % LS, ph = (t / LS) & 1u;
+                    ptx::mbar_wait(empty0 + 8u * slot, ph ^ 1u);
+                    if (ptx::elect_one()) {
+                        ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE);
+                        if (!DAG)      // rows [i0, i0 + MT) x complex columns [KC c, KC c + KC)
+                            ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, c * KC, mat_row0 + i0, full0 + 8u * slot, pol_links);
+                        else           // rows [KC c, KC c + KC) x complex columns [i0, i0 + MT)
+                            ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, i0, mat_row0 + KC * c, full0 + 8u * slot, pol_links);
+                    }
+                    __syncwarp();
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ---------------------------------------------------------------- MMA issuer (one elected lane, uniform control flow)
+        uint32_t t = 0;
+        const uint32_t n_mat = (uint32_t)n_my * (uint32_t)n_mat_item;
+        for (uint32_t tm = 0; tm < n_mat; ++tm) {
+            const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
+            ptx::mbar_wait(dempty0 + 8u * ds, dph ^ 1u);
+            ptx::tc_fence_after();
+            const uint32_t d1 = tmem_base + Gm::D_COL0 + ds * Gm::D_COLS, d0 = d1 + NB3;
+#pragma unroll 1
+            for (int c = 0; c < CHUNKS; ++c, ++t) {
+                const uint32_t as = t % AS, aph = (t / AS) & 1u;
+                ptx::mbar_wait(abfull0 + 8u * as, aph);
+                ptx::tc_fence_after();
+                if (ptx::elect_one()) {
+                    const uint32_t a1 = tmem_base + as * Gm::A_COLS, a0 = a1 + Gm::A_HALF;
+                    const uint64_t db0 = umma_desc_kmajor(b_u32 + as * B_STAGE, 128, B_SBO);
+#pragma unroll
+                    for (int kk = 0; kk < Gm::KSTEPS; ++kk) {
+                        const uint64_t db = db0 + (uint64_t)(kk * 256 >> 4);
+                        ptx::mma_i8_ts(d1, a1 + kk * 8, db, IDESC_S, (c | kk) != 0 ? 1u : 0u);
+                        ptx::mma_i8_ts(d0, a0 + kk * 8, db, IDESC_U, (c | kk) != 0 ? 1u : 0u);
+                    }
+                    ptx::tc_commit(abempty0 + 8u * as);
+                    if (c == CHUNKS - 1) ptx::tc_commit(dfull0 + 8u * ds);
+                }
+                __syncwarp();
+            }
+        }
+    } else if (warp >= Gm::CONV_W0 && warp < Gm::EPI_W0) {
+        // ---------------------------------------------------------------- converters
+        constexpr int NG = Gm::NG;
+        const int grp = (warp - Gm::CONV_W0) >> 2;
+        const int q = warp & 3;
+        const int row = q * 32 + lane;
+        const int gtid = ((warp - Gm::CONV_W0) & 3) * 32 + lane;
+        const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
+        const uint32_t total = (uint32_t)n_my * (uint32_t)(n_mat_item * CHUNKS);
+
+        // B entries of this thread: contraction row j (of the stage's KC) and column r, the same in every
+        // stage; every entry of a thread has the same r (e = gtid + 128 x: r = e & 7 [+ 8 bit 4], j from the rest)
+        const int my_r = (gtid & 7) + (NP == 16 ? ((gtid >> 4) & 1) * 8 : 0);
+        const bool r_valid = my_r < p.width;
+        int b_off_vec[NE];
+        uint32_t b_o[NE];              // byte offset of (k = 2j, n = r, digit 0) in the B tile
+#pragma unroll
+        for (int x = 0; x < NE; ++x) {
+            const int e = gtid + 128 * x;
+            const int j = 2 * (e >> (NP == 16 ? 5 : 4)) + ((e >> 3) & 1);
+            b_off_vec[x] = j * p.nrhs + my_r;
+            const int k = 2 * j;
+            b_o[x] = (uint32_t)(k >> 4) * 128u + (uint32_t)(my_r >> 3) * B_SBO + (uint32_t)(my_r & 7) * 16u + (uint32_t)(k & 15);
+        }
+        constexpr uint32_t N_STEP = (uint32_t)(NP >> 3) * B_SBO;     // byte step of NP columns of n (NP is a multiple of 8)
+
+        int n_it = 0, n_m = M0, n_c = grp, n_s = 0;
+        SiteX n_cx = {};
+        const float2* n_vec = p.in;
+        float n_g = 0.f, n_f = 0.f;       // fixed-point scale g 2^22 of the operand, epilogue factor of the matrix
+        auto load_item = [&]() {
+            if (n_it < n_my) {
+                n_s = site_of_item(blockIdx.x + n_it * gridDim.x);
+                n_cx = site_coords(p.lat, n_s);
+            }
+        };
+        auto load_matrix = [&]() {
+            if (n_it < n_my) {
+                const int sv = stencil_site_x(p.lat, n_s, n_cx, n_m, DAG ? 1 : 0);
+                const int sm = DAG ? sv : n_s;
+                n_vec = (n_m == 0 ? p.in_local : p.in) + (int64_t)sv * NC * p.nrhs + p.r0;
+                const float2 gs = r_valid ? __ldg(reinterpret_cast<const float2*>(n_m == 0 ? pp.vscale_u : pp.vscale_w) + (int64_t)sv * TENSOR_I8_GP + my_r)
+                                          : make_float2(0.f, 0.f);
+                n_g = gs.x * 4194304.f;
+                n_f = (n_m == 0 ? p.alpha : p.beta) * __ldg(p.scales + (int64_t)sm * 9 + n_m) * gs.y * (1.f / 4194304.f);
+            }
+        };
+        float2 vn[NE];
+        auto fetch = [&]() {
+#pragma unroll
+            for (int x = 0; x < NE; ++x)
+                vn[x] = (n_it < n_my && r_valid) ? __ldg(n_vec + (int64_t)(KC * n_c) * p.nrhs + b_off_vec[x]) : make_float2(0.f, 0.f);
+        };
+        auto normalise = [&]() -> bool {
+            bool item_changed = false;
+            while (n_c >= CHUNKS) {
+                n_c -= CHUNKS;
+                if (++n_m == 9) { n_m = M0; ++n_it; item_changed = true; }
+            }
+            return item_changed;
+        };
+        normalise();
+        load_item();
+        load_matrix();
+        fetch();
+        // matrix counter of the stage being converted (for the factor ring): stage t belongs to matrix t / CHUNKS
+        for (uint32_t t = grp; t < total; t += NG) {
+            const uint32_t slot = t % LS, ph = (t / LS) & 1u;
+            const uint32_t as = t % AS, aph = (t / AS) & 1u;
+            float2 v[NE];
+#pragma unroll
+            for (int x = 0; x < NE; ++x) v[x] = vn[x];
+            const float g = n_g, f = n_f;
+            const bool first_chunk = n_c == 0;
+            n_c += NG;
+            if (n_c >= CHUNKS) {
+                if (normalise()) load_item();
+                load_matrix();
+            }
+            fetch();
+
+            ptx::mbar_wait(full0 + 8u * slot, ph);
+            uint32_t w[KC];                                   // the lane's KC link entries (re, im) int16
+            if (row < MT) {
+                const uint32_t sb = link_u32 + slot * LINK_STAGE;
+                if constexpr (!DAG) {
+                    const uint32_t rb = sb + row * (KC * 4);
+#pragma unroll
+                    for (int u = 0; u < KC / 4; ++u) {
+                        const uint32_t sw = KC == 32 ? ((uint32_t)row & 7u) : (((uint32_t)row >> 1) & 3u);   // SWIZZLE_128B | 64B
+                        const uint4 x = ptx::lds128u(rb + (((uint32_t)u ^ sw) << 4));
+                        w[4 * u] = x.x; w[4 * u + 1] = x.y; w[4 * u + 2] = x.z; w[4 * u + 3] = x.w;
+                    }
+                } else {
+                    const uint32_t cb = sb + row * 4;
+#pragma unroll
+                    for (int jj = 0; jj < KC; ++jj) w[jj] = ptx::lds32(cb + jj * (MT * 4));
+                }
+            } else {
+#pragma unroll
+                for (int u = 0; u < KC; ++u) w[u] = 0u;
+            }
+            ptx::fence_cta();          // the loads must have completed before the slot goes back (see tensor_kernel.cuh)
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
+
+            ptx::mbar_wait(abempty0 + 8u * as, aph ^ 1u);
+            ptx::tc_fence_after();
+            // A operand: high bytes (signed) and low bytes (unsigned), k = 2j (re), 2j + 1 (im): 4 per TMEM column
+            uint32_t a1[KC / 2], a0[KC / 2];
+#pragma unroll
+            for (int c2 = 0; c2 < KC / 2; ++c2) {
+                a1[c2] = __byte_perm(w[2 * c2], w[2 * c2 + 1], 0x7531);
+                a0[c2] = __byte_perm(w[2 * c2], w[2 * c2 + 1], 0x6420);
+            }
+            const uint32_t a1_t = tmem_base + lane_addr + as * Gm::A_COLS, a0_t = a1_t + Gm::A_HALF;
+            if constexpr (KC == 32) {
+                ptx::tmem_st16(a1_t, a1);
+                ptx::tmem_st16(a0_t, a0);
+            } else {
+                ptx::tmem_st8(a1_t, a1);
+                ptx::tmem_st8(a0_t, a0);
+            }
+            // B operand: fixed point, three signed digits, [Re out | Im out] x 3 along n
+            const uint32_t bt = b_u32 + as * B_STAGE;
+#pragma unroll
+            for (int x = 0; x < NE; ++x) {
+                const float vx = v[x].x * g, vy = v[x].y * g;
+                const int b1x = __float2int_rn(vx), b1y = __float2int_rn(DAG ? vy : -vy);     // n = r      (-> Re out)
+                const int b2x = __float2int_rn(vy), b2y = __float2int_rn(DAG ? -vx : vx);     // n = NP + r (-> Im out)
+                int x1, x2, y1, y2;
+                digit_regs(b1x, x1, x2);
+                digit_regs(b1y, y1, y2);
+                ptx::sts16(bt + b_o[x], pack_lo_bytes(b1x, b1y));
+                ptx::sts16(bt + b_o[x] + 2 * N_STEP, pack_lo_bytes(x1, y1));
+                ptx::sts16(bt + b_o[x] + 4 * N_STEP, pack_lo_bytes(x2, y2));
+                digit_regs(b2x, x1, x2);
+                digit_regs(b2y, y1, y2);
+                ptx::sts16(bt + b_o[x] + N_STEP, pack_lo_bytes(b2x, b2y));
+                ptx::sts16(bt + b_o[x] + 3 * N_STEP, pack_lo_bytes(x1, y1));
+                ptx::sts16(bt + b_o[x] + 5 * N_STEP, pack_lo_bytes(x2, y2));
+            }
+            // epilogue factor of this matrix and column: written by the group that converts the matrix's first chunk
+            if (first_chunk && gtid < 32 && (gtid & 8) == 0) {
+                // lanes 0-7 (and 16-23 for NP = 16) of the group's first warp hold r = 0..7 (8..15)
+                asm volatile("st.shared.f32 [%0], %1;" ::"r"(ft_u32 + (uint32_t)(((t / CHUNKS) % FT) * NP + my_r) * 4u), "f"(f) : "memory");
+            }
+            ptx::tc_wait_st();
+            ptx::fence_proxy_async();
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(abfull0 + 8u * as);
+        }
+    } else if (warp >= Gm::EPI_W0) {
+        // ---------------------------------------------------------------- epilogue
+        const int q = warp & 3;
+        const int row = q * 32 + lane;
+        const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
+        uint32_t tm = 0;
+        for (int it = 0; it < n_my; ++it) {
+            const int item = blockIdx.x + it * gridDim.x;
+            const int s = site_of_item(item);
+            const int i0 = NT == 1 ? 0 : (item % NT) * MT;
+            float acc[2 * NP];
+#pragma unroll
+            for (int n = 0; n < 2 * NP; ++n) acc[n] = 0.f;
+#pragma unroll 1
+            for (int m = M0; m < 9; ++m, ++tm) {
+                const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
+                ptx::mbar_wait(dfull0 + 8u * ds, dph);
+                ptx::tc_fence_after();
+                const uint32_t d1_t = tmem_base + lane_addr + Gm::D_COL0 + ds * Gm::D_COLS, d0_t = d1_t + NB3;
+                const uint32_t ft = ft_u32 + (uint32_t)((tm % FT) * NP) * 4u;
+                // 8 columns of n at a time: digits 2, 1, 0 of both byte planes, Horner in fp32
+#pragma unroll
+                for (int pc = 0; pc < 2 * NP / 8; ++pc) {
+                    float S[8];
+#pragma unroll
+                    for (int l = 2; l >= 0; --l) {
+                        uint32_t hi[8], lo[8];
+                        ptx::tmem_ld8(d1_t + l * 2 * NP + 8 * pc, hi);
+                        ptx::tmem_ld8(d0_t + l * 2 * NP + 8 * pc, lo);
+                        ptx::tc_wait_ld();
+#pragma unroll
+                        for (int n = 0; n < 8; ++n) {
+                            const float T = (float)((int)hi[n] * 256 + (int)lo[n]);
+                            S[n] = l == 2 ? T : fmaf(S[n], 256.f, T);
+                        }
+                    }
+#pragma unroll
+                    for (int n = 0; n < 8; ++n) {
+                        float fr;
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(fr) : "r"(ft + (uint32_t)((8 * pc + n) % NP) * 4u));
+                        acc[8 * pc + n] = fmaf(fr, S[n], acc[8 * pc + n]);
+                    }
+                }
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(dempty0 + 8u * ds);
+            }
+            if (row < MT) {
+                const int64_t o = ((int64_t)s * NC + i0 + row) * p.nrhs + p.r0;
+                if (p.identity) {
+#pragma unroll
+                    for (int r = 0; r < NP; ++r)
+                        if (r < p.width) {
+                            const float2 u = __ldg(p.in_local + o + r);
+                            acc[r] = fmaf(p.alpha, u.x, acc[r]);
+                            acc[NP + r] = fmaf(p.alpha, u.y, acc[NP + r]);
+                        }
+                }
+                if (((p.nrhs | p.r0) & 1) == 0) {
+                    float4* o4 = reinterpret_cast<float4*>(p.out + o);
+#pragma unroll
+                    for (int r = 0; r < NP; r += 2) {
+                        if (r + 1 < p.width) o4[r >> 1] = make_float4(acc[r], acc[NP + r], acc[r + 1], acc[NP + r + 1]);
+                        else if (r < p.width) p.out[o + r] = make_float2(acc[r], acc[NP + r]);
+                    }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < NP; ++r)
+                        if (r < p.width) p.out[o + r] = make_float2(acc[r], acc[NP + r]);
+                }
+            }
+        }
+    }
+
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc(tmem_base, Gm::TMEM_COLS);
+}
+
+}  // namespace coarse

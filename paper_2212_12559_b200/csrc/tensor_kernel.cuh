@@ -20,7 +20,7 @@
 //                           16 contraction columns (dagger 0: box MT rows x 128 B | 64 B, SWIZZLE_128B |
 //                           64B, so that "lane = row" reads are bank-conflict free; dagger 1: box 16 rows x
 //                           MT entries, lane = column).
-//   converters (2 x 4 warps) read the slab (lane <-> output index: TMEM transposes for free), decode /
+//   converters (3 x 4 warps) read the slab (lane <-> output index: TMEM transposes for free), decode /
 //                           split hi/lo and write the A operand straight into TENSOR MEMORY (tcgen05.st),
 //                           so the link bytes cross shared memory exactly twice (TMA write + one LDS
 //                           read); fetch the 16 x NP vector entries of the stage from global memory (L2
@@ -84,7 +84,10 @@ struct TensorGeom {
     static constexpr int DS = 4;                        // accumulator ring depth (MMA -> epilogue), one slot per link matrix
     static constexpr int D_COLS = 2 * N;                // per slot: [hi.hi chain | hi.lo + lo.hi chain]
     static constexpr int TMEM_COLS = 512;
-    static constexpr int THREADS = 16 * 32;
+    static constexpr int NG = 3;                        // converter groups of 4 warps (stage t -> group t mod NG)
+    static constexpr int CONV_W0 = 2;                   // warps: 0 producer, 1 MMA issuer, 2 .. 2+4NG-1 converters, then 4 epilogue
+    static constexpr int EPI_W0 = CONV_W0 + 4 * NG;
+    static constexpr int THREADS = (EPI_W0 + 4) * 32;   // 18 warps; any 4 consecutive warps cover the 4 TMEM lane quadrants
     static constexpr int NBAR = 2 * LS + 2 * AS + 2 * DS;
     static constexpr int SMEM_BYTES = 1024 + LS * LINK_STAGE + AS * 2 * B_HALF + NBAR * 8 + 16;
     static constexpr bool OK = (NC % 16 == 0) && (MT % 8 == 0) && MT <= 128 && CHUNKS >= 2 && (NP == 8 || NP == 16) &&
@@ -298,12 +301,16 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
                 __syncwarp();
             }
         }
-    } else if (warp >= 4 && warp < 12) {
+    } else if (warp >= Gm::CONV_W0 && warp < Gm::EPI_W0) {
         // ---------------------------------------------------------------- converters
-        const int grp = (warp - 4) >> 2;              // stages t with t % 2 == grp
-        const int q = warp & 3;                       // TMEM lane quadrant of this warp
+        // Three groups in flight: ncu on the two-group version showed the converter warps issuing 22 % of the
+        // time (275 instructions per stage in ~1250 cycles: mbarrier round trips, tcgen05.st + wait::st, the
+        // proxy fence), i.e. bound by the latency chain of a stage, not by issue slots or HBM.
+        constexpr int NG = Gm::NG;
+        const int grp = (warp - Gm::CONV_W0) >> 2;    // stages t with t % NG == grp
+        const int q = warp & 3;                       // TMEM lane quadrant of this warp (hardware: warp id mod 4)
         const int row = q * 32 + lane;                // A-operand row = output index i (inside the item's tile)
-        const int gtid = (warp & 3) * 32 + lane;      // 0..127 inside the group
+        const int gtid = ((warp - Gm::CONV_W0) & 3) * 32 + lane;      // 0..127 inside the group
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         const uint32_t total = (uint32_t)n_my * (uint32_t)(n_mat_item * CHUNKS);
 
@@ -328,7 +335,7 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
 
         // cursor of the NEXT stage of this group (its vector entries are prefetched while the current
         // stage is converted): item index, matrix, chunk, and what depends on them
-        int n_it = 0, n_m = M0, n_c = grp, n_s = 0;
+        int n_it = 0, n_m = M0, n_c = grp, n_s = 0;     // stage t = grp: chunk grp of the first matrix (normalised below)
         SiteX n_cx = {};
         const float2* n_vec = p.in;
         float n_sc = 1.f;
@@ -353,11 +360,20 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
             for (int x = 0; x < NE; ++x)
                 vn[x] = (n_it < n_my && b_valid[x]) ? __ldg(n_vec + (int64_t)(16 * n_c) * p.nrhs + b_off_vec[x]) : make_float2(0.f, 0.f);
         };
+        auto normalise = [&]() -> bool {               // carry n_c into (n_m, n_it); true if the item changed
+            bool item_changed = false;
+            while (n_c >= CHUNKS) {
+                n_c -= CHUNKS;
+                if (++n_m == 9) { n_m = M0; ++n_it; item_changed = true; }
+            }
+            return item_changed;
+        };
+        normalise();
         load_item();
         load_matrix();
         fetch();
 
-        for (uint32_t t = grp; t < total; t += 2) {
+        for (uint32_t t = grp; t < total; t += NG) {
             const uint32_t slot = t % LS, ph = (t / LS) & 1u;
             const uint32_t as = t % AS, aph = (t / AS) & 1u;
             // this stage's vector entries and scale; then move the cursor two stages on and prefetch
@@ -365,10 +381,9 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
 #pragma unroll
             for (int x = 0; x < NE; ++x) v[x] = vn[x];
             const float sc = n_sc;
-            n_c += 2;
+            n_c += NG;
             if (n_c >= CHUNKS) {
-                n_c -= CHUNKS;
-                if (++n_m == 9) { n_m = M0; ++n_it; load_item(); }
+                if (normalise()) load_item();
                 load_matrix();
             }
             fetch();
@@ -453,7 +468,7 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(abfull0 + 8u * as);
         }
-    } else if (warp >= 12) {
+    } else if (warp >= Gm::EPI_W0) {
         // ---------------------------------------------------------------- epilogue
         const int q = warp & 3;
         const int row = q * 32 + lane;
@@ -471,16 +486,20 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
                 const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
                 ptx::mbar_wait(dfull0 + 8u * ds, dph);
                 ptx::tc_fence_after();
-                uint32_t d[2 * N];
                 const uint32_t d_tmem = tmem_base + lane_addr + Gm::D_COL0 + ds * Gm::D_COLS;
+                // 16 columns of the main chain and the matching 16 of the cross-term chain at a time
 #pragma unroll
-                for (int c = 0; c < 2 * N / 16; ++c) ptx::tmem_ld16(d_tmem + 16 * c, d + 16 * c);
-                ptx::tc_wait_ld();
+                for (int c = 0; c < N / 16; ++c) {
+                    uint32_t dm[16], dx[16];
+                    ptx::tmem_ld16(d_tmem + 16 * c, dm);
+                    ptx::tmem_ld16(d_tmem + N + 16 * c, dx);
+                    ptx::tc_wait_ld();
+#pragma unroll
+                    for (int n = 0; n < 16; ++n) acc[16 * c + n] += __uint_as_float(dm[n]) + __uint_as_float(dx[n]);
+                }
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(dempty0 + 8u * ds);
-#pragma unroll
-                for (int n = 0; n < N; ++n) acc[n] += __uint_as_float(d[n]) + __uint_as_float(d[N + n]);
             }
             if (row < MT) {
                 const int64_t o = ((int64_t)s * NC + i0 + row) * p.nrhs + p.r0;

@@ -47,7 +47,13 @@ def _check_parts(oracle_lib, dims, Nc, prec, nrhs, dagger, parity, local, path, 
     op.apply_parts(u if local else None, w, out, nrhs=nrhs, dagger=dagger, parity=parity, local=local,
                    alpha=alpha, beta=beta)
     torch.cuda.synchronize()
-    assert op.last_path == path and op.last_launches == (1 if path != cop.PATH_TENSOR else (nrhs + 15) // 16)
+    if path != cop.PATH_TENSOR:
+        want = 1
+    elif prec == cop.LINK_I16:      # integer tensor-core kernel: + one scale pre-pass per operand and column group
+        want = ((nrhs + 15) // 16) * (2 + (1 if local else 0))
+    else:
+        want = (nrhs + 15) // 16
+    assert op.last_path == path and op.last_launches == want
     ref = oracle_lib.coarse_apply_parts(dims, Nc, links_h, u.cpu().numpy() if local else None, w.cpu().numpy(),
                                         nrhs=nrhs, dagger=dagger, parity=parity, local=local, alpha=alpha,
                                         beta=beta, link_precision=prec, scales=scales_h)
