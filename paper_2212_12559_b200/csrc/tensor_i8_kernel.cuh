@@ -256,16 +256,18 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         const uint32_t total = (uint32_t)n_my * (uint32_t)(n_mat_item * CHUNKS);
 
-        // B entries of this thread: contraction row j (of the stage's KC) and column r, the same in every
-        // stage; every entry of a thread has the same r (e = gtid + 128 x: r = e & 7 [+ 8 bit 4], j from the rest)
-        const int my_r = (gtid & 7) + (NP == 16 ? ((gtid >> 4) & 1) * 8 : 0);
+        // B entries of this thread: contraction row j (of the stage's KC) and column r, the same in every stage;
+        // every entry of a thread has the same r.  e = gtid + 128 x: bits 0-2 = r mod 8 (16-byte rows of the K-major
+        // layout: banks 4 apart), bits 3-4 = j mod 4 (bytes 2 apart / next word), bit 5 = r div 8 (NP = 16), rest = j div 4:
+        // the 32 lanes of a 16-bit store touch 16 distinct words in 16 distinct banks (conflict-free).
+        const int my_r = (gtid & 7) + (NP == 16 ? ((gtid >> 5) & 1) * 8 : 0);
         const bool r_valid = my_r < p.width;
         int b_off_vec[NE];
         uint32_t b_o[NE];              // byte offset of (k = 2j, n = r, digit 0) in the B tile
 #pragma unroll
         for (int x = 0; x < NE; ++x) {
             const int e = gtid + 128 * x;
-            const int j = 2 * (e >> (NP == 16 ? 5 : 4)) + ((e >> 3) & 1);
+            const int j = ((e >> 3) & 3) + 4 * (e >> (NP == 16 ? 6 : 5));
             b_off_vec[x] = j * p.nrhs + my_r;
             const int k = 2 * j;
             b_o[x] = (uint32_t)(k >> 4) * 128u + (uint32_t)(my_r >> 3) * B_SBO + (uint32_t)(my_r & 7) * 16u + (uint32_t)(k & 15);
@@ -389,8 +391,8 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                 ptx::sts16(bt + b_o[x] + 5 * N_STEP, pack_lo_bytes(x2, y2));
             }
             // epilogue factor of this matrix and column: written by the group that converts the matrix's first chunk
-            if (first_chunk && gtid < 32 && (gtid & 8) == 0) {
-                // lanes 0-7 (and 16-23 for NP = 16) of the group's first warp hold r = 0..7 (8..15)
+            if (first_chunk && (gtid & 0x18) == 0 && gtid < 64) {
+                // threads 0-7 (and 32-39 for NP = 16) of the group hold r = 0..7 (8..15)
                 asm volatile("st.shared.f32 [%0], %1;" ::"r"(ft_u32 + (uint32_t)(((t / CHUNKS) % FT) * NP + my_r) * 4u), "f"(f) : "memory");
             }
             ptx::tc_wait_st();

@@ -511,14 +511,24 @@ def test_apply_host_pipelined_multi_rhs_is_bit_identical(oracle_lib, Nc, prec, n
     vin = vin_d.cpu().pin_memory()
     vout = torch.empty_like(vin).pin_memory()
     op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    i8 = prec == cop.LINK_I16 and want_path == cop.PATH_TENSOR
     for dagger in (0, 1):
-        ref = torch.empty_like(vin_d)
-        op.apply(vin_d, ref, nrhs=nrhs, dagger=dagger)
+        ref_default = torch.empty_like(vin_d)
+        op.apply(vin_d, ref_default, nrhs=nrhs, dagger=dagger)
+        ref = ref_default
+        if i8:
+            # the device-resident apply runs int16 links on the integer tensor-core kernel; the site-range launches of
+            # apply_host use the 3xTF32 kernel (include/coarse_op.h): bit-identical to THAT kernel, 1e-5 to the other
+            op.set_option(cop.OPT_TENSOR_I8, 1)
+            ref = torch.empty_like(vin_d)
+            op.apply(vin_d, ref, nrhs=nrhs, dagger=dagger)
+            op.set_option(cop.OPT_TENSOR_I8, 0)
         torch.cuda.synchronize()
         vout.fill_(float("nan"))
         op.apply_host(vin, vout, nrhs=nrhs, dagger=dagger)
         assert op.last_launches == launches and op.last_path == want_path
         assert torch.equal(torch.view_as_real(vout), torch.view_as_real(ref.cpu()))
+        assert rel_l2_per_rhs(vout.numpy(), ref_default.cpu().numpy()) <= 3e-6
     op.close()
 
 
