@@ -459,6 +459,8 @@ def run_ours(args, cfg, daggers):
         op.set_option(cop.OPT_PDL, args.pdl)
     if args.warp_items:
         op.set_option(cop.OPT_WARP_ITEMS, args.warp_items)
+    if args.tensor_i8:
+        op.set_option(cop.OPT_TENSOR_I8, args.tensor_i8)
 
     vq = vnorm = None
     if args.hvec:
@@ -952,6 +954,8 @@ def main():
     ap.add_argument("--links", default="", choices=["", "c64", "i16"], help="override the config's link storage")
     ap.add_argument("--warp-items", type=int, default=0,
                     help="COARSE_OPT_WARP_ITEMS override (0 auto, 1 never, 2 always, 11/12/14: 1/2/4 warps per team)")
+    ap.add_argument("--tensor-i8", type=int, default=0,
+                    help="COARSE_OPT_TENSOR_I8: int16 links on the TENSOR path (0 auto = integer tensor cores, 1 = the 3xTF32 kernel)")
     ap.add_argument("--pdl", type=int, default=0, help="COARSE_OPT_PDL: programmatic dependent launch for chained applies (0 auto, 1 always, 2 never)")
     ap.add_argument("--hvec", action="store_true",
                     help="half-precision INPUT vectors (int16 + per-site norm, row f2) through coarse_op_apply_hvec")
