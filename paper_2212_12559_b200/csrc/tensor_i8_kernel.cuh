@@ -21,7 +21,7 @@
 // recombines out += f_m [ ((T_2 256 + T_1) 256 + T_0) ],  T_l = 256 D1_l + D0_l  (T_l in int32, the rest in fp32),
 // f_m = scale_m coef_m / (g 2^22).  The only rounding besides that recombination is the 23-bit fixed-point
 // representation of each site vector relative to its largest component - the same order as the fp32 rounding
-// of the inputs themselves; measured 1e-7 against the fp64 oracle (tolerance 1e-5).
+// of the inputs themselves; measured 3e-7 relative L2 against an fp64 evaluation (tolerance 1e-5).
 //
 // Pipeline roles, work items, the parts apply (parity list, X stage on / off, alpha / beta, identity term) and
 // the RHS column tiles are those of tensor_kernel.cuh; a stage is KC = 32 complex columns (16 for Nc = 48).
