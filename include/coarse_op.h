@@ -100,8 +100,8 @@ enum {
                                 2 always (needs the workspace coarse_op_set_links allocates on such lattices) */
     COARSE_OPT_WARP_ITEMS = 7, /* 1-RHS plain apply: the STREAM variant in which small teams of consumer warps own
                                 whole work items and every stage of theirs (csrc/stream2_kernel.cuh) instead of all
-                                eight warps sharing every stage: 0 auto (int16 links on lattices with at least 4
-                                items per team of the chip), 1 never, 2 always, 12 / 14 always with 2 / 4 warps per
+                                eight warps sharing every stage: 0 auto (int16 links with Nc >= 48, and Nc = 32, on lattices with at
+                                least 4 items per team of the chip), 1 never, 2 always, 12 / 14 always with 2 / 4 warps per
                                 team (2 = 14).  With it COARSE_OPT_STAGES is the ring's slot count. */
     COARSE_OPT_TENSOR_I8 = 8  /* TENSOR path on int16 links: 0 auto / 2: the integer tensor-core kernel (csrc/tensor_i8_kernel.cuh:
                                 link entries as two int8 planes, exact, vectors in 23-bit fixed point per site), 1: the

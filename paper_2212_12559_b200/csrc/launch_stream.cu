@@ -127,7 +127,8 @@ template <int NC, bool I16, bool DAG>
 int launch_stream2_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
     // rows of 24 / 48 quads (Nc = 96 / 192 int16) run best with 2 warps per team (measured: Nc 96 6.6 / 6.8 TB/s
     // against 6.0 / 6.7 with 4 and 5.4 / 5.4 on the cooperative kernel), the others with 4
-    const bool two = op->warp_items_opt == 12 || (op->warp_items_opt != 14 && NC % 3 == 0);
+    constexpr bool has4 = Stream2Geom<NC, I16, 4>::OK, has2 = Stream2Geom<NC, I16, 2>::OK;
+    const bool two = !has4 || (has2 && (op->warp_items_opt == 12 || (op->warp_items_opt != 14 && (NC % 3 == 0 || NC == 32))));
     if (two) return launch_stream2_w<NC, I16, DAG, 2>(op, base, stream);
     return launch_stream2_w<NC, I16, DAG, 4>(op, base, stream);
 }
@@ -136,8 +137,13 @@ template <int NC, bool I16>
 bool use_warp_items(const coarse_op* op, const StreamParams& p, int dagger, bool gen) {
     if (gen || p.vnorms || p.n_items > 0 || p.pdl || op->warp_items_opt == 1) return false;
     if (op->warp_items_opt >= 2) return true;
-    const int64_t items = dagger ? (int64_t)p.n_sites : (int64_t)p.n_sites * Stream2Geom<NC, I16, 4>::NB;
-    return I16 && NC >= 64 && items >= (int64_t)4 * Stream2Geom<NC, I16, 4>::T * op->num_sms;
+    // auto: int16 links with Nc >= 48 (issue-bound on the cooperative kernel; Nc = 48: 5.5 / 5.2 -> 6.3 / 6.4 TB/s with
+    // 2 warps per team) and the 4-8 KB matrices of Nc = 32 (the cooperative kernel pays its per-stage handshake eight
+    // times per 8 KB there: complex64 5.6 / 5.1 -> 7.2 / 7.0 TB/s, int16 2.7 / 2.5 -> 3.7 / 3.7), on lattices with at
+    // least 4 items per team of the chip
+    using G2 = Stream2Geom<NC, I16, (Stream2Geom<NC, I16, 4>::OK ? 4 : 2)>;
+    const int64_t items = dagger ? (int64_t)p.n_sites : (int64_t)p.n_sites * G2::NB;
+    return ((I16 && NC >= 48) || NC == 32) && items >= (int64_t)4 * G2::T * op->num_sms;
 }
 
 // dagger = 0 on a tiny lattice: switch to the fine row-block geometry when the regular one gives
@@ -172,11 +178,11 @@ int launch_stream_g(const coarse_op* op, const StreamParams& p, int dagger, bool
                       : launch_stream_t<NC, false, false, false, false, true>(op, p, stream);
     }
     if (op->prec == COARSE_LINK_I16) {
-        if constexpr (Stream2Geom<NC, true, 4>::OK)
+        if constexpr (Stream2Geom<NC, true, 4>::OK || Stream2Geom<NC, true, 2>::OK)
             if (use_warp_items<NC, true>(op, p, dagger, gen))
                 return dagger ? launch_stream2_t<NC, true, true>(op, p, stream) : launch_stream2_t<NC, true, false>(op, p, stream);
     } else {
-        if constexpr (Stream2Geom<NC, false, 4>::OK)
+        if constexpr (Stream2Geom<NC, false, 4>::OK || Stream2Geom<NC, false, 2>::OK)
             if (use_warp_items<NC, false>(op, p, dagger, gen))
                 return dagger ? launch_stream2_t<NC, false, true>(op, p, stream) : launch_stream2_t<NC, false, false>(op, p, stream);
     }
