@@ -180,7 +180,7 @@ int launch_tensor(const coarse_op* op, const void* in, void* out, int nrhs, int 
     // site range is launched (coarse_op_apply_host: its input arrives slice by slice, the per-site scales of
     // the fixed-point B operand need whole neighbour vectors) or the scale buffer is too small and cannot grow
     if (op->prec == COARSE_LINK_I16 && op->link_map_i8_ok && op->tensor_i8_opt != 1 && ps.site_end == 0 && op->vscale) {
-        const void* u_other = (ps.gen && ps.local != 0 && ps.u != in) ? ps.u : nullptr;
+        const void* u_other = (ps.gen && ps.local == 1 && ps.u != in) ? ps.u : nullptr;   // X.u needs u's scales; the identity term does not
         switch (op->Nc) {
 #define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_tensor_i8_nc, NC)(op, p, u_other, op->vscale, dagger, stream);
             COARSE_FOR_EACH_NC(COARSE_CASE_NC)

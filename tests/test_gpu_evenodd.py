@@ -50,7 +50,7 @@ def _check_parts(oracle_lib, dims, Nc, prec, nrhs, dagger, parity, local, path, 
     if path != cop.PATH_TENSOR:
         want = 1
     elif prec == cop.LINK_I16:      # integer tensor-core kernel: + one scale pre-pass per operand and column group
-        want = ((nrhs + 15) // 16) * (2 + (1 if local else 0))
+        want = ((nrhs + 15) // 16) * (2 + (1 if local == 1 else 0))
     else:
         want = (nrhs + 15) // 16
     assert op.last_path == path and op.last_launches == want
@@ -232,6 +232,24 @@ def test_parts_identity_in_place_values(oracle_lib, Nc, prec, dagger, path):
     op.apply_parts(buf, w, buf, dagger=dagger, parity=cop.PARITY_ALL, local=cop.LOCAL_IDENTITY, alpha=1.0, beta=-1.0)
     torch.cuda.synchronize()
     ref = oracle_lib.coarse_apply_parts(dims, Nc, links_h, u.cpu().numpy(), w.cpu().numpy(), dagger=dagger, parity=2,
+                                        local=2, alpha=1.0, beta=-1.0, link_precision=prec, scales=scales_h)
+    assert rel_l2_per_rhs(buf.cpu().numpy(), ref) <= TOL
+    op.close()
+
+
+@pytest.mark.parametrize("Nc,prec", [(96, cop.LINK_C64), (128, cop.LINK_I16), (192, cop.LINK_I16)])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_parts_identity_in_place_values_multi_rhs(oracle_lib, Nc, prec, dagger):
+    """The same in-place update with several right-hand sides, on the tensor kernels (the identity term is read in
+    the epilogue by the thread that then stores the element)."""
+    dims, nrhs = (2, 4, 2, 2), 5
+    links_d, scales_d, links_h, scales_h, u, w = _make(oracle_lib, dims, Nc, prec, 978, nrhs)
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links_d, scales_d)
+    buf = u.clone()
+    op.apply_parts(buf, w, buf, nrhs=nrhs, dagger=dagger, parity=cop.PARITY_ALL, local=cop.LOCAL_IDENTITY, alpha=1.0, beta=-1.0)
+    torch.cuda.synchronize()
+    assert op.last_path == cop.PATH_TENSOR
+    ref = oracle_lib.coarse_apply_parts(dims, Nc, links_h, u.cpu().numpy(), w.cpu().numpy(), nrhs=nrhs, dagger=dagger, parity=2,
                                         local=2, alpha=1.0, beta=-1.0, link_precision=prec, scales=scales_h)
     assert rel_l2_per_rhs(buf.cpu().numpy(), ref) <= TOL
     op.close()
