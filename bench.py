@@ -320,12 +320,14 @@ def parity_check(cfg, links, scales, vin, outs, n_random=64):
             "ok": bool(worst <= 1e-5 and worst_site <= 5e-5)}
 
 
-def measure_config(name, steps, local, dev, read_ceiling=None):
+def measure_config(name, steps, local, dev, read_ceiling=None, override=None):
     """One BASELINE config on the AUTO path: in-run parity on sampled sites, then `steps` applies per dagger
     timed with CUDA events (L2-resident lattices: one CUDA graph per dagger, warm, plus a cold number over
-    rotating link copies).  Sub-record of the default bench line (`configs`)."""
+    rotating link copies).  Sub-record of the default bench line (`configs`; `override` changes links / nrhs
+    for the `extras` records)."""
     import paper_2212_12559_b200 as cop
     cfg = synth.config(name)
+    cfg.update(override or {})
     dims, Nc, nrhs = cfg["dims"], cfg["Nc"], cfg["nrhs"]
     V = synth.lattice_volume(dims)
     prec = cop.LINK_I16 if cfg["links"] == "i16" else cop.LINK_C64
@@ -411,7 +413,7 @@ def measure_config(name, steps, local, dev, read_ceiling=None):
         rec["frac_of_read_ceiling"] = {str(dg): rec["gbs"][str(dg)] / read_ceiling for dg in (0, 1)}
     rec["msite_updates_per_s"] = {str(dg): V / (ms[dg] * 1e-3) / 1e6 for dg in (0, 1)}
     rec["clocks"] = clocks.summary()
-    rec["traffic"] = {str(dg): ncu_traffic_bytes(name, path, dg, cfg["links"]) for dg in (0, 1)}
+    rec["traffic"] = None if override else {str(dg): ncu_traffic_bytes(name, path, dg, cfg["links"]) for dg in (0, 1)}
     op.close()
     return rec
 
@@ -689,6 +691,13 @@ def run_ours(args, cfg, daggers):
         line["configs"] = {}
         for name in ("C1", "C3", "C4", "C5"):
             line["configs"][name] = measure_config(name, args.config_steps, local, dev, read_ceiling)
+            torch.cuda.empty_cache()
+        # the paper's storage format (int16 links) with several right-hand sides (its future work, L200;
+        # 3 = one propagator): not BASELINE configs, reported beside them
+        line["extras"] = {}
+        for key, name, ov in (("C5_int16_nrhs16", "C5", {"links": "i16"}), ("C5_int16_nrhs3", "C5", {"links": "i16", "nrhs": 3}),
+                              ("C4_nrhs3", "C4", {"nrhs": 3})):
+            line["extras"][key] = measure_config(name, args.config_steps, local, dev, read_ceiling, override=ov)
             torch.cuda.empty_cache()
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = time_oracle(cfg, daggers, dev, min_seconds=args.cpu_seconds)
