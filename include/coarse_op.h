@@ -160,13 +160,22 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
 
 /* The plain apply on HALF-PRECISION input vectors ("half precision" = 16-bit fixed
  * point with a per-site fp32 norm): in(x)_jr = in_norms[x][r] * (q_re + i q_im), in_q_dev =
- * int16_t[V][Nc][nrhs][2], in_norms_dev = float[V][nrhs].  The output stays complex64 (a site's rows
- * are produced by several CTAs, so the per-site norm of the result is taken by a separate
- * coarse_op_quantize_vec_i16 when a half-precision result is wanted).  Nc % 4 == 0.
+ * int16_t[V][Nc][nrhs][2], in_norms_dev = float[V][nrhs].  The output is complex64 (coarse_op_apply_hout adds the
+ * half-precision result).  Nc % 4 == 0.
  * nrhs = 1 runs on the STREAM kernels (the norm is folded into the vector operand like the int16
  * link scale), other nrhs on SIMPLE. */
 int coarse_op_apply_hvec(coarse_op_t* op, const void* in_q_dev, const float* in_norms_dev, void* out_dev, int nrhs,
                          int dagger, void* stream);
+
+/* The apply with a HALF-PRECISION RESULT: out_c64_dev receives the complex64 result as coarse_op_apply
+ * would write it, and (out_q_dev, out_norms_dev) the same vector as 16-bit fixed point with a per-(site, rhs) fp32 norm,
+ * exactly what coarse_op_quantize_vec_i16 makes of out_c64_dev (norm = max|component| / 32767, q = clamp(rint(component /
+ * norm))).  in_norms_dev = NULL: in_dev is a complex64 vector; else the half-precision input of coarse_op_apply_hvec.
+ * For 1 RHS on the STREAM kernels it is ONE launch: a CTA owns whole sites (all row blocks of a site in a row), keeps
+ * the site's rows in shared memory and ends each site with a CTA-local epilogue (norm, 16-bit vector).  Other
+ * nrhs / shapes: the apply followed by the vector quantiser.  The three vector buffers must not overlap. */
+int coarse_op_apply_hout(coarse_op_t* op, const void* in_dev, const float* in_norms_dev, void* out_c64_dev, void* out_q_dev,
+                         float* out_norms_dev, int nrhs, int dagger, void* stream);
 
 /* Vector quantiser: for each (site, rhs) norm = max|component|/32767 (fp32 division) and
  * q = clamp(rint(component/norm), -32767, 32767); an all-zero vector gets norm 0 and q = 0.

@@ -26,6 +26,7 @@ LOCAL_NONE, LOCAL_X, LOCAL_IDENTITY = 0, 1, 2
 EXPORTS = (
     "coarse_op_create", "coarse_op_link_bytes", "coarse_op_scale_bytes", "coarse_op_vector_bytes",
     "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_parts", "coarse_op_apply_hvec",
+    "coarse_op_apply_hout",
     "coarse_op_quantize_vec_i16", "coarse_op_apply_host",
     "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_probe_read", "coarse_op_cagcr_work_bytes",
     "coarse_op_cagcr", "coarse_op_cagcr_schur", "coarse_op_cagcr_cheb_work_bytes",
@@ -70,6 +71,8 @@ def lib() -> ctypes.CDLL:
     L.coarse_op_apply_parts.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ctypes.c_float, ctypes.c_float, vp]
     L.coarse_op_apply_hvec.restype = ci
     L.coarse_op_apply_hvec.argtypes = [vp, vp, vp, vp, ci, ci, vp]
+    L.coarse_op_apply_hout.restype = ci
+    L.coarse_op_apply_hout.argtypes = [vp, vp, vp, vp, vp, vp, ci, ci, vp]
     L.coarse_op_quantize_vec_i16.restype = ci
     L.coarse_op_quantize_vec_i16.argtypes = [vp, ci64, ci, ci, vp, vp, vp]
     L.coarse_op_apply_host.restype = ci
@@ -201,6 +204,24 @@ def coarse_op_apply_hvec(op: int, vin_q, vin_norms, vout, nrhs: int = 1, dagger:
         raise ValueError("vin_norms must hold one float32 per (site, rhs)")
     _check(lib().coarse_op_apply_hvec(op, _ptr(vin_q), _ptr(vin_norms), _ptr(vout), int(nrhs), int(dagger),
                                       _stream_handle(stream)))
+
+
+def coarse_op_apply_hout(op: int, vin, vin_norms, vout, vout_q, vout_norms, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+    """The apply with a half-precision result beside the complex64 one.  vin: CUDA complex64 [V][Nc][nrhs] (vin_norms None)
+    or int16 [V][Nc][nrhs][2] with vin_norms float32 [V][nrhs]; vout complex64 [V][Nc][nrhs]; vout_q int16 [V][Nc][nrhs][2];
+    vout_norms float32 [V][nrhs]."""
+    for t in (vin, vout, vout_q, vout_norms) + ((vin_norms,) if vin_norms is not None else ()):
+        if not t.is_cuda or not t.is_contiguous():
+            raise ValueError("apply_hout needs contiguous CUDA tensors")
+    vb = coarse_op_vector_bytes(op, nrhs)
+    if vout.numel() * vout.element_size() != vb or vout_q.numel() * vout_q.element_size() * 2 != vb:
+        raise ValueError("output tensors have the wrong number of bytes for this operator/nrhs")
+    if vin.numel() * vin.element_size() != (vb // 2 if vin_norms is not None else vb):
+        raise ValueError("input tensor has the wrong number of bytes for this operator/nrhs")
+    if vout_norms.element_size() != 4 or vout_norms.numel() % nrhs:
+        raise ValueError("vout_norms must hold one float32 per (site, rhs)")
+    _check(lib().coarse_op_apply_hout(op, _ptr(vin), _ptr(vin_norms) if vin_norms is not None else None, _ptr(vout), _ptr(vout_q),
+                                      _ptr(vout_norms), int(nrhs), int(dagger), _stream_handle(stream)))
 
 
 def coarse_op_quantize_vec_i16(v_c64, Nc: int, nrhs: int, q_out, norms_out, stream=None) -> None:
@@ -370,6 +391,9 @@ class CoarseOp:
 
     def apply_hvec(self, vin_q, vin_norms, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
         coarse_op_apply_hvec(self._h, vin_q, vin_norms, vout, nrhs, dagger, stream)
+
+    def apply_hout(self, vin, vin_norms, vout, vout_q, vout_norms, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+        coarse_op_apply_hout(self._h, vin, vin_norms, vout, vout_q, vout_norms, nrhs, dagger, stream)
 
     def cagcr(self, b, x, s: int = 8, cycles: int = 1, x_is_zero: bool = True, work=None, info=None, stream=None,
               schur_parity: Optional[int] = None):

@@ -118,6 +118,8 @@ int launch_stream(const coarse_op* op, const void* in, void* out, int dagger, co
     p.parity = ps.parity;
     p.n_sites = ps.parity == 2 ? op->lat.V : op->lat.V / 2;
     p.vnorms = ps.vnorms;
+    p.hout_q = static_cast<short2*>(ps.hout_q);
+    p.hout_norms = ps.hout_norms;
     // Programmatic dependent launch: always (1), never (2), or auto (0): in the latency-limited regime (links
     // resident in L2), for every launch but the first after coarse_op_set_links - work that PRODUCED the links
     // may still be in flight on the stream in front of that one, and the link stages are read before the
@@ -570,6 +572,46 @@ int coarse_op_apply_hvec(coarse_op_t* op, const void* in_q_dev, const float* in_
     op->last_launches = 1;
     op->last_path = path;
     op->links_fresh = false;
+    return COARSE_OK;
+}
+
+int coarse_op_apply_hout(coarse_op_t* op, const void* in_dev, const float* in_norms_dev, void* out_c64_dev, void* out_q_dev,
+                         float* out_norms_dev, int nrhs, int dagger, void* stream) {
+    int rc = check_apply_args(op, in_dev, out_c64_dev, nrhs, dagger);
+    if (rc != COARSE_OK) return rc;
+    if (!out_q_dev || !out_norms_dev) return fail(COARSE_EINVAL, "apply_hout: out_q_dev / out_norms_dev is NULL");
+    if (!aligned16(in_dev) || !aligned16(out_c64_dev) || !aligned16(out_q_dev) || (reinterpret_cast<uintptr_t>(out_norms_dev) & 3u) ||
+        (in_norms_dev && (reinterpret_cast<uintptr_t>(in_norms_dev) & 3u)))
+        return fail(COARSE_EINVAL, "apply_hout: vectors must be 16-byte aligned, norm arrays 4-byte aligned");
+    const size_t vb = coarse_op_vector_bytes(op, nrhs);
+    const size_t in_b = in_norms_dev ? vb / 2 : vb;
+    if (overlaps(in_dev, in_b, out_c64_dev, vb) || overlaps(in_dev, in_b, out_q_dev, vb / 2) || overlaps(out_c64_dev, vb, out_q_dev, vb / 2))
+        return fail(COARSE_EINVAL, "apply_hout: in, out_c64 and out_q must not overlap");
+    if (in_norms_dev && op->Nc % 4) return fail(COARSE_EUNSUPPORTED, "apply_hout: half-precision input needs Nc % 4 == 0 (got %d)", op->Nc);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool fused = nrhs == 1 && stream_supports(op->Nc, 1) &&
+                       (op->path_opt == COARSE_PATH_AUTO || op->path_opt == COARSE_PATH_STREAM);
+    if (fused) {
+        PartsSpec ps = kPlain;
+        ps.vnorms = in_norms_dev;
+        ps.hout_q = out_q_dev;
+        ps.hout_norms = out_norms_dev;
+        op->last_launches = 0;
+        rc = launch_stream(op, in_dev, out_c64_dev, dagger, ps, st);
+        if (rc < 0) return rc;
+        op->last_launches = 1 + rc;
+        op->last_path = COARSE_PATH_STREAM;
+        op->links_fresh = false;
+        return COARSE_OK;
+    }
+    // several right-hand sides, or a shape outside the STREAM kernels: the apply, then the vector quantiser
+    rc = in_norms_dev ? coarse_op_apply_hvec(op, in_dev, in_norms_dev, out_c64_dev, nrhs, dagger, stream)
+                      : coarse_op_apply(op, in_dev, out_c64_dev, nrhs, dagger, stream);
+    if (rc != COARSE_OK) return rc;
+    const int launches = op->last_launches;
+    rc = coarse_op_quantize_vec_i16(out_c64_dev, op->lat.V, op->Nc, nrhs, out_q_dev, out_norms_dev, stream);
+    if (rc != COARSE_OK) return rc;
+    op->last_launches = launches + 1;
     return COARSE_OK;
 }
 

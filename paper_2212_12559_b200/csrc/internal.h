@@ -82,6 +82,8 @@ struct PartsSpec {
     float alpha, beta;
     const float* vnorms;   // non-NULL: half-precision input vectors (plain apply only)
     int site_begin, site_end;   // output sites [site_begin, site_end) (plain apply only); end = 0: all
+    void* hout_q;               // non-NULL: also write the result as int16 + per-site norm (coarse_op_apply_hout, 1 RHS)
+    float* hout_norms;
 };
 
 struct StreamParams;

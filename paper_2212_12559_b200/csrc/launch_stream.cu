@@ -28,7 +28,7 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     p.split = 0;
     p.partial = nullptr;
     p.split_count = nullptr;
-    if (DAG && !GEN && !HV && base.n_items == 0 && Gm::NB > 1 && op->split_ws &&
+    if (DAG && !GEN && !HV && base.n_items == 0 && !base.hout_q && Gm::NB > 1 && op->split_ws &&
         (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes &&
         (op->split_opt == 2 || (op->split_opt == 0 && p.n_sites < op->num_sms))) {
         p.split = 1;
@@ -83,7 +83,7 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     return COARSE_OK;
 }
 
-// Team-owned stages (stream2_kernel.cuh): plain apply on the whole lattice, no PDL.
+// Team-owned stages (stream2_kernel.cuh): plain apply on the whole lattice or a site range, no PDL.
 template <int NC, bool I16, bool DAG, int TW>
 int launch_stream2_w(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
     using Gm = Stream2Geom<NC, I16, TW>;
@@ -93,6 +93,10 @@ int launch_stream2_w(const coarse_op* op, const StreamParams& base, cudaStream_t
         StreamParams p = base;
         p.n_items = DAG ? p.n_sites : p.n_sites * Gm::NB;
         p.item_begin = 0;
+        if (base.n_items > 0) {                       // a site range [item_begin, n_items) was requested (in sites)
+            p.item_begin = DAG ? base.item_begin : base.item_begin * Gm::NB;
+            p.n_items = DAG ? base.n_items : base.n_items * Gm::NB;
+        }
         // ring: one slot per team being read + ~104 KB in flight (the measured optimum of the read stream),
         // a multiple of the team count so that every slot has a fixed owner; COARSE_OPT_STAGES overrides
         const int sb = Gm::stage_bytes(DAG);
@@ -111,7 +115,7 @@ int launch_stream2_w(const coarse_op* op, const StreamParams& base, cudaStream_t
         cudaError_t e = ensure_dynamic_smem(kern, op->device, smem, attr_cache);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream2 kernel)");
         int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
-        const int need = (p.n_items + Gm::T - 1) / Gm::T;
+        const int need = (p.n_items - p.item_begin + Gm::T - 1) / Gm::T;
         if (grid > need) grid = need;
         if (grid < 1) return COARSE_OK;
         kern<<<grid, Gm::THREADS, smem, stream>>>(p);
@@ -135,7 +139,9 @@ int launch_stream2_t(const coarse_op* op, const StreamParams& base, cudaStream_t
 
 template <int NC, bool I16>
 bool use_warp_items(const coarse_op* op, const StreamParams& p, int dagger, bool gen) {
-    if (gen || p.vnorms || p.n_items > 0 || p.pdl || op->warp_items_opt == 1) return false;
+    // (site-range launches take the decision the full-lattice apply takes, so that coarse_op_apply_host stays
+    // bit-identical to coarse_op_apply)
+    if (gen || p.vnorms || p.hout_q || p.pdl || op->warp_items_opt == 1) return false;
     if (op->warp_items_opt >= 2) return true;
     // auto: int16 links with Nc >= 48 (issue-bound on the cooperative kernel; Nc = 48: 5.5 / 5.2 -> 6.3 / 6.4 TB/s with
     // 2 warps per team) and the 4-8 KB matrices of Nc = 32 (the cooperative kernel pays its per-stage handshake eight

@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
         const uint64_t pol_links = p.keep_links ? pol_vec : ptx::policy_evict_first();
         int slot = 0;
         uint32_t phase = 0;
-        for (int base = blockIdx.x * T; base < p.n_items; base += item_stride) {
+        for (int base = p.item_begin + blockIdx.x * T; base < p.n_items; base += item_stride) {
             const int my_item = base + (lane % T);
             int svh[NH];
 #pragma unroll
@@ -228,7 +228,7 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
     const int grp = lane / G;          // which of the RPL rows of a warp-wide load
     const int qi = lane % G;           // quad index inside the pass
     const int row0 = wi * (WL * RPL) + grp;     // this lane's first row of a stage; further rows every RPL
-    const int item0 = blockIdx.x * T + team;
+    const int item0 = p.item_begin + blockIdx.x * T + team;     // item_begin: site-range launches (coarse_op_apply_host)
     int slot = team;                   // this team's slots: team, team + T, ..
     uint32_t phase = 0;
     auto next_slot = [&]() {

@@ -61,6 +61,13 @@ struct StreamParams {
     unsigned int* split_count;   // [n_sites], zero between launches (the reducing CTA resets its site's counter)
     // HV (half-precision input vectors, coarse_op_apply_hvec): `in` points at int16 (re,im) entries
     const float* vnorms;      // fp32 norm per site (nrhs = 1)
+    // Half-precision OUTPUT (coarse_op_apply_hout): besides the complex64 result in `out`, the CTA takes
+    // the site's norm max|component| / 32767 and writes the 16-bit fixed-point vector.  For that a CTA OWNS whole
+    // sites: with several row blocks per site (dagger = 0) its work items are walked site-major (all row blocks of a
+    // site in a row), the rows are kept in a small shared-memory buffer and the epilogue is CTA-local
+    // (two named barriers per site; a first version with a global counter per site cost 1.7 us per item).
+    short2* hout_q;           // NULL: off
+    float* hout_norms;        // [V]
 };
 
 constexpr int stream_pow2ceil(int v) { return v <= 1 ? 1 : v <= 2 ? 2 : v <= 4 ? 4 : v <= 8 ? 8 : v <= 16 ? 16 : 32; }
@@ -117,7 +124,8 @@ struct StreamGeom {
     static constexpr int THREADS = (W + 1) * 32;
 
     static constexpr int stage_bytes(bool dag) { return LINK_STAGE + (dag ? VEC_STAGE_D : VEC_STAGE_N); }
-    static constexpr int fixed_bytes(bool dag) { return (dag ? RED_BYTES : 0) + 128; }
+    static constexpr int SITE_BYTES = NC * 8;                  // half-precision output: the site's complex64 rows
+    static constexpr int fixed_bytes(bool dag) { return (dag ? RED_BYTES : 0) + 128 + SITE_BYTES; }
     static int smem_bytes(bool dag, int stages) { return stages * (stage_bytes(dag) + 16) + fixed_bytes(dag); }
 };
 
@@ -162,6 +170,38 @@ __device__ __forceinline__ float2 cfinal(const CAcc& acc) {
     return CONJ ? make_float2(acc.a.x + acc.b.y, acc.b.x - acc.a.y) : make_float2(acc.a.x - acc.b.y, acc.a.y + acc.b.x);
 }
 
+// Per-site half-precision epilogue, called by all consumer threads of the CTA that owns site s once its NC result
+// entries are in `sbuf` (shared memory).  scratch: 9 words of shared memory.  The arithmetic is that of
+// quantize_vec_i16_kernel (R22): norm = amax / 32767 (fp32 division), q = clamp(rint(component / norm)).
+template <int NC, int NTHREADS>
+__device__ __forceinline__ void half_out_epilogue(const StreamParams& p, int s, const float2* sbuf, uint32_t* scratch) {
+    ptx::named_bar_sync(1, NTHREADS);                    // every row of the site is in sbuf
+    float amax = 0.f;
+    for (int t = threadIdx.x; t < NC; t += NTHREADS) {
+        const float2 x = sbuf[t];
+        amax = fmaxf(amax, fmaxf(fabsf(x.x), fabsf(x.y)));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    if ((threadIdx.x & 31) == 0) scratch[1 + (threadIdx.x >> 5)] = __float_as_uint(amax);
+    ptx::named_bar_sync(1, NTHREADS);
+    amax = 0.f;
+#pragma unroll
+    for (int w = 0; w < NTHREADS / 32; ++w) amax = fmaxf(amax, __uint_as_float(scratch[1 + w]));
+    const float norm = amax == 0.f ? 0.f : __fdiv_rn(amax, 32767.0f);
+    if (threadIdx.x == 0) p.hout_norms[s] = norm;
+    for (int t = threadIdx.x; t < NC; t += NTHREADS) {
+        short2 o = make_short2(0, 0);
+        if (amax != 0.f) {
+            const float2 x = sbuf[t];
+            o.x = (short)fminf(32767.f, fmaxf(-32767.f, rintf(__fdiv_rn(x.x, norm))));
+            o.y = (short)fminf(32767.f, fmaxf(-32767.f, rintf(__fdiv_rn(x.y, norm))));
+        }
+        p.hout_q[(int64_t)s * NC + t] = o;
+    }
+    ptx::named_bar_sync(1, NTHREADS);                    // sbuf and scratch are reused by the next site
+}
+
 template <int NC, bool I16, bool DAG, bool FINE = false, bool GEN = false, bool HV = false>
 __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coarse_apply_stream(StreamParams p) {
     static_assert(!(DAG && FINE), "the fine geometry splits output rows: dagger = 0 only");
@@ -193,6 +233,14 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
     __syncthreads();
     if (p.pdl) ptx::pdl_launch_dependents();   // the next kernel's CTAs may take SMs as ours exit
 
+    // The it-th work item of this CTA.  Default: items blockIdx.x, blockIdx.x + gridDim.x, ...  Half-precision output
+    // with several row blocks per site: site-major, the NB items of a site in a row (the CTA owns the site).
+    const bool site_major = !DAG && NB > 1 && p.hout_q != nullptr;
+    auto item_at = [&](int it) -> int {
+        if (site_major) return p.item_begin + ((int)blockIdx.x + (it / NB) * (int)gridDim.x) * NB + it % NB;
+        return p.item_begin + (int)blockIdx.x + it * (int)gridDim.x;
+    };
+
     if (warp == W) {
         // ------------------------------------------------------------------ producer
         // The whole warp walks the loop (uniform control flow, so the bulk copies are not wrapped
@@ -217,7 +265,9 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
             __syncwarp();
             deferring = false;
         };
-        for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
+        for (int it = 0;; ++it) {
+            const int item = item_at(it);
+            if (item >= p.n_items) break;
             const int sidx = (DAG && !p.split) ? item : item / NB;
             const int s = (GEN && p.parity != 2) ? parity_site(p.lat, sidx, p.parity) : sidx;
             const int rb = DAG ? 0 : item % NB;
@@ -283,15 +333,19 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
         return f;
     };
     const int M0 = GEN ? p.m_begin : 0;
-    next_scale = fetch_scale(p.item_begin + blockIdx.x);
-    next2_scale = fetch_scale(p.item_begin + blockIdx.x + gridDim.x);
+    next_scale = fetch_scale(item_at(0));
+    next2_scale = fetch_scale(item_at(1));
+    float2* sbuf = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(bars + 2 * S) + 128);     // half-precision output
+    uint32_t* hscratch = reinterpret_cast<uint32_t*>(bars + 2 * S);
 
-    for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
+    for (int it = 0;; ++it) {
+        const int item = item_at(it);
+        if (item >= p.n_items) break;
         const int s = site_of(item);
         const int rb = DAG ? 0 : item % NB;
         cur_scale = next_scale;
         next_scale = next2_scale;
-        next2_scale = fetch_scale(item + 2 * gridDim.x);
+        next2_scale = fetch_scale(item_at(it + 2));
 
         if (!DAG) {
             float2 acc[WL];
@@ -384,8 +438,10 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                         acc[k].y = fmaf(p.alpha, uloc[k].y, acc[k].y);
                     }
                     p.out[(int64_t)s * NC + row] = acc[k];
+                    if (p.hout_q) sbuf[row] = acc[k];
                 }
             }
+            if (p.hout_q && rb == NB - 1) half_out_epilogue<NC, W * 32>(p, s, sbuf, hscratch);
         } else {
             constexpr int UL = (NC + W * 32 - 1) / (W * 32);
             float2 uloc[GEN ? UL : 1];
@@ -471,6 +527,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                 }
                 if (p.split) p.partial[(int64_t)item * NC + t] = sum;
                 else p.out[(int64_t)s * NC + t] = sum;
+                if (p.hout_q) sbuf[t] = sum;
             }
             if (p.split) {
                 // last-arriver reduction: every consumer thread publishes its part of the partial vector, one
@@ -497,6 +554,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                     }
                 }
             }
+            if (p.hout_q) half_out_epilogue<NC, W * 32>(p, s, sbuf, hscratch);
             red_parity ^= 1;
         }
     }

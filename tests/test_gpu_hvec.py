@@ -118,3 +118,93 @@ def test_hvec_full_size_c4_whole_lattice(oracle_lib):
         err, worst_site, n_sites = res[dagger]
         assert n_sites == V and err <= TOL and worst_site <= 5 * TOL, (dagger, err, worst_site)
     op.close()
+
+
+# ------------------------------------------------------------------ half-precision OUTPUT (coarse_op_apply_hout)
+def _run_hout(oracle_lib, dims, Nc, prec, nrhs, dagger, half_in, opts=None, want_launches=None):
+    """The complex64 result must match the oracle's apply (1e-5); the 16-bit result must be EXACTLY what the oracle's
+    vector quantiser (pinned in tests/test_oracle_hvec_pins.py) makes of that complex64 result - the rounding decision is
+    taken in fp32 on the same numbers on both sides - and must dequantise to the oracle's apply within half a step."""
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, 65, device="cuda")
+    scales = scales_h = None
+    if prec == cop.LINK_I16:
+        lq = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+        scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_i16(links, Nc, lq, scales)
+        torch.cuda.synchronize()
+        links, scales_h = lq, scales.cpu().numpy()
+    v = synth.make_vectors(dims, Nc, nrhs, 66, device="cuda")
+    if V > 1:
+        v[1] *= 1e-6
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    for k, val in (opts or {}).items():
+        op.set_option(k, val)
+    out = torch.full((V, Nc, nrhs), complex(float("nan"), float("nan")), dtype=torch.complex64, device="cuda")
+    oq = torch.full((V, Nc, nrhs, 2), -7, dtype=torch.int16, device="cuda")
+    on = torch.full((V, nrhs), float("nan"), dtype=torch.float32, device="cuda")
+    if half_in:
+        q, nm, q_h, nm_h = _quantise(oracle_lib, v, Nc, nrhs)
+        ref = oracle_lib.coarse_apply_hvec(dims, Nc, links.cpu().numpy(), q_h, nm_h, nrhs=nrhs, dagger=dagger,
+                                           link_precision=prec, scales=scales_h)
+    else:
+        q, nm = v, None
+        ref = oracle_lib.coarse_apply(dims, Nc, links.cpu().numpy(), v.cpu().numpy(), nrhs=nrhs, dagger=dagger,
+                                      link_precision=prec, scales=scales_h)
+    for rep in range(2):                       # twice: the per-site counters must be back at zero
+        oq.fill_(-7)
+        op.apply_hout(q, nm, out, oq, on, nrhs=nrhs, dagger=dagger)
+        torch.cuda.synchronize()
+        if want_launches is not None:
+            assert op.last_launches == want_launches
+        got = out.cpu().numpy()
+        assert rel_l2_per_rhs(got, ref) <= TOL
+        q_ref, n_ref = oracle_lib.quantize_vec_i16(got, Nc, nrhs)
+        assert np.array_equal(on.cpu().numpy(), n_ref)
+        assert np.array_equal(oq.cpu().numpy(), q_ref)
+        deq = on.cpu().numpy()[:, None, :] * (oq.cpu().numpy()[..., 0].astype(np.float64) + 1j * oq.cpu().numpy()[..., 1])
+        step = on.cpu().numpy()[:, None, :]
+        assert np.all(np.abs(deq - ref) <= 0.75 * step * np.sqrt(2) + 1e-5 * np.abs(ref).max())
+    op.close()
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (1, 1, 1, 1)])
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("dagger", [0, 1])
+@pytest.mark.parametrize("half_in", [False, True])
+def test_half_precision_output_fused_epilogue(oracle_lib, dims, Nc, prec, dagger, half_in):
+    """1 RHS: ONE launch; the CTA that finishes a site's last (site, row-block) item takes the norm and writes the int16
+    vector (Nc >= 96 in dagger 0: several CTAs per site; dagger 1: one)."""
+    if Nc >= 128 and dims == (4, 4, 4, 4):
+        dims = (2, 4, 2, 2)
+    _run_hout(oracle_lib, dims, Nc, prec, 1, dagger, half_in, want_launches=1)
+
+
+@pytest.mark.parametrize("grid,fine", [(1, 0), (5, 2), (1000, 0)])
+def test_half_precision_output_any_grid(oracle_lib, grid, fine):
+    for dagger in (0, 1):
+        _run_hout(oracle_lib, (3, 2, 2, 4), 128, cop.LINK_I16, 1, dagger, False, opts={cop.OPT_GRID: grid, cop.OPT_FINE: fine})
+        _run_hout(oracle_lib, (5, 3, 2, 3), 48, cop.LINK_C64, 1, dagger, True, opts={cop.OPT_GRID: grid})
+
+
+@pytest.mark.parametrize("nrhs", [3, 16])
+def test_half_precision_output_multi_rhs_two_pass(oracle_lib, nrhs):
+    """Several right-hand sides: the apply (STREAM-MR / tensor kernels), then the vector quantiser."""
+    _run_hout(oracle_lib, (4, 2, 2, 2), 64, cop.LINK_C64, nrhs, 0, False, want_launches=2)
+    _run_hout(oracle_lib, (2, 2, 2, 2), 128, cop.LINK_I16, nrhs, 1, False)
+
+
+def test_half_precision_output_argument_errors():
+    dims, Nc, V = (2, 2, 2, 2), 48, 16
+    links = torch.zeros((V, 9, Nc, Nc), dtype=torch.complex64, device="cuda")
+    v = torch.zeros((V, Nc, 1), dtype=torch.complex64, device="cuda")
+    out, oq, on = torch.zeros_like(v), torch.zeros((V, Nc, 1, 2), dtype=torch.int16, device="cuda"), torch.zeros((V, 1), device="cuda")
+    op = cop.CoarseOp(dims, Nc).set_links(links)
+    L = cop.lib()
+    assert L.coarse_op_apply_hout(op._h, v.data_ptr(), None, out.data_ptr(), None, on.data_ptr(), 1, 0, None) == cop.EINVAL
+    assert L.coarse_op_apply_hout(op._h, v.data_ptr(), None, v.data_ptr(), oq.data_ptr(), on.data_ptr(), 1, 0, None) == cop.EINVAL
+    assert L.coarse_op_apply_hout(op._h, v.data_ptr(), None, out.data_ptr(), oq.data_ptr(), on.data_ptr(), 1, 0, None) == cop.OK
+    torch.cuda.synchronize()
+    assert torch.all(oq == 0) and torch.all(on == 0)          # a zero operator: norm 0, q 0
+    op.close()
