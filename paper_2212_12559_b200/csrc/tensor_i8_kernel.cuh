@@ -109,10 +109,15 @@ static __global__ void __launch_bounds__(128) vec_pow2_scale_kernel(const float2
     float m = 0.f;
     for (int a = 0; a < nc; ++a) {
         const float2 x = p[(long long)a * nrhs];
-        m = fmaxf(m, fmaxf(fabsf(x.x), fabsf(x.y)));
+        const float ax = fmaxf(fabsf(x.x), fabsf(x.y));
+        m = (x.x != x.x || x.y != x.y || m != m) ? __int_as_float(0x7fc00000) : fmaxf(m, ax);      // fmaxf drops NaN: keep it
     }
     float2 o = make_float2(0.f, 0.f);
-    if (m > 0.f && m < 3.0e38f) {
+    if (!(m <= 3.0e38f)) {
+        // Inf or NaN in the vector: fixed point cannot carry it, so the column's epilogue factor becomes NaN and every
+        // output that reads this site is NaN, as IEEE arithmetic on the complex64 path would make it (or Inf)
+        o = make_float2(0.f, __int_as_float(0x7fc00000));
+    } else if (m > 0.f) {
         int e;
         frexpf(m, &e);                                   // m = f 2^e, f in [1/2, 1)
         e = e < -100 ? -100 : e > 100 ? 100 : e;         // keep g and 1/g (and g 2^22) normal numbers

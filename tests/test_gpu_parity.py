@@ -242,6 +242,34 @@ def test_tensor_path_unsupported_shapes():
     cop.coarse_op_destroy(h)
 
 
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("bad", [float("nan"), float("inf")])
+def test_tensor_paths_propagate_non_finite_inputs(prec, bad):
+    """A NaN / Inf in one input vector entry must reach every output that reads it (a solver detects divergence that
+    way), also on the integer tensor-core kernel whose fixed-point operand cannot represent it; other columns and
+    sites that do not touch the entry stay finite."""
+    dims, Nc, nrhs = (4, 4, 2, 2), 64, 8
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, 31, device="cuda")
+    scales = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+        scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        links = q
+    vin = synth.make_vectors(dims, Nc, nrhs, 32, device="cuda")
+    vin[5, 7, 2] = complex(bad, 0.0)
+    vout = torch.empty_like(vin)
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales).set_option(cop.OPT_PATH, cop.PATH_TENSOR)
+    op.apply(vin, vout, nrhs=nrhs)
+    torch.cuda.synchronize()
+    fin = torch.isfinite(torch.view_as_real(vout)).all(dim=-1)          # [V][Nc][nrhs]
+    assert not fin[5, :, 2].any()                                        # the site itself (X term), column 2
+    assert fin[:, :, [0, 1, 3, 4, 5, 6, 7]].all()                        # other columns untouched
+    assert fin[:, :, 2].any()                                            # sites that are no neighbours of site 5
+    op.close()
+
+
 def test_tensor_launch_count_beyond_16_rhs():
     dims, Nc = (2, 2, 2, 2), 64
     links = synth.make_arbitrary_links(dims, Nc, 3, device="cuda")
