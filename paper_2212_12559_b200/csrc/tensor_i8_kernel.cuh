@@ -17,9 +17,10 @@
 // stored side by side along N, so that per 16 complex columns
 //     D1[:, l] += A1 . d_l        (signed x signed,   N = 3 x 2 NP)
 //     D0[:, l] += A0 . d_l        (unsigned x signed, N = 3 x 2 NP)
-// are TWO MMAs, exact in int32 (|a| <= 255, |d| <= 128, K = 2 Nc <= 384 per link matrix: < 2^24).  The epilogue
-// recombines out += f_m [ ((T_2 256 + T_1) 256 + T_0) ],  T_l = 256 D1_l + D0_l  (T_l in int32, the rest in fp32),
-// f_m = scale_m coef_m / (g 2^22).  The only rounding besides that recombination is the 23-bit fixed-point
+// are TWO MMAs, exact in int32 (|a| <= 255, |d| <= 128, K = 2 Nc <= 384 per link matrix: < 2^24).  Products of equal
+// weight share accumulator columns: D1 is written ONE digit block higher than D0, so that the slot holds
+// W_0 = D0_0, W_1 = D1_0 + D0_1, W_2 = D1_1 + D0_2, W_3 = D1_2 (four blocks instead of six), and the epilogue
+// recombines out += f_m (((W_3 256 + W_2) 256 + W_1) 256 + W_0) in fp32, f_m = scale_m coef_m / (g 2^22).  The only rounding besides that recombination is the 23-bit fixed-point
 // representation of each site vector relative to its largest component - the same order as the fp32 rounding
 // of the inputs themselves; measured 3e-7 relative L2 against an fp64 evaluation (tolerance 1e-5).
 //
@@ -31,6 +32,9 @@
 
 namespace coarse {
 
+#ifndef COARSE_I8_NG
+#define COARSE_I8_NG 3
+#endif
 constexpr int TENSOR_I8_GP = 16;   // row pitch of the scale arrays: one launch handles at most 16 right-hand sides
 
 struct TensorI8Params {
@@ -56,11 +60,11 @@ struct TensorI8Geom {
     static constexpr int A_HALF = KC / 2;                      // TMEM columns of one byte plane (4 int8 per column)
     static constexpr int A_COLS = 2 * A_HALF;                  // high bytes | low bytes
     static constexpr int D_COL0 = AS * A_COLS;
-    static constexpr int DS = 2;
-    static constexpr int D_COLS = 2 * NB3;                     // [D1 | D0]
+    static constexpr int DS = 3;
+    static constexpr int D_COLS = 4 * 2 * NP;                  // W_0 .. W_3, each [Re out | Im out]
     static constexpr int FT = 8;                               // ring of per-matrix epilogue factor rows
     static constexpr int TMEM_COLS = 512;
-    static constexpr int NG = 3, CONV_W0 = 2, EPI_W0 = CONV_W0 + 4 * NG;
+    static constexpr int NG = COARSE_I8_NG, CONV_W0 = 2, EPI_W0 = CONV_W0 + 4 * NG;
     static constexpr int THREADS = (EPI_W0 + 4) * 32;
     static constexpr int NBAR = 2 * LS + 2 * AS + 2 * DS;
     static constexpr int SMEM_BYTES = 1024 + LS * LINK_STAGE + AS * B_STAGE + FT * NP * 4 + NBAR * 8 + 16;
@@ -146,6 +150,8 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
     // instruction descriptors: D int32 (c_format 2), A signed | unsigned 8 bit, B signed 8 bit, K-major, N = NB3, M = 128
     constexpr uint32_t IDESC_S = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NB3 >> 3) << 17) | ((128u >> 4) << 24);
     constexpr uint32_t IDESC_U = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(NB3 >> 3) << 17) | ((128u >> 4) << 24);
+    constexpr uint32_t IDESC_U1 = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(2 * NP >> 3) << 17) | ((128u >> 4) << 24);   // one digit block
+    constexpr uint32_t IDESC_U2 = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(4 * NP >> 3) << 17) | ((128u >> 4) << 24);   // two digit blocks
     const TensorParams& p = pp.t;
 
     extern __shared__ unsigned char smem_raw[];
@@ -230,7 +236,8 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
             const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
             ptx::mbar_wait(dempty0 + 8u * ds, dph ^ 1u);
             ptx::tc_fence_after();
-            const uint32_t d1 = tmem_base + Gm::D_COL0 + ds * Gm::D_COLS, d0 = d1 + NB3;
+            // high-byte plane one digit block above the low-byte plane: equal weights share columns
+            const uint32_t d0 = tmem_base + Gm::D_COL0 + ds * Gm::D_COLS, d1 = d0 + 2 * NP;
 #pragma unroll 1
             for (int c = 0; c < CHUNKS; ++c, ++t) {
                 const uint32_t as = t % AS, aph = (t / AS) & 1u;
@@ -242,8 +249,16 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
 #pragma unroll
                     for (int kk = 0; kk < Gm::KSTEPS; ++kk) {
                         const uint64_t db = db0 + (uint64_t)(kk * 256 >> 4);
-                        ptx::mma_i8_ts(d1, a1 + kk * 8, db, IDESC_S, (c | kk) != 0 ? 1u : 0u);
-                        ptx::mma_i8_ts(d0, a0 + kk * 8, db, IDESC_U, (c | kk) != 0 ? 1u : 0u);
+                        if (c == 0 && kk == 0) {
+                            // first k-step of the matrix: W_1 .. W_3 = high plane (overwrite), W_0 = low plane digit 0
+                            // (overwrite), W_1, W_2 += low plane digits 1, 2
+                            ptx::mma_i8_ts(d1, a1, db, IDESC_S, 0u);
+                            ptx::mma_i8_ts(d0, a0, db, IDESC_U1, 0u);
+                            ptx::mma_i8_ts(d1, a0, db + (uint64_t)((2 * (NP >> 3) * B_SBO) >> 4), IDESC_U2, 1u);
+                        } else {
+                            ptx::mma_i8_ts(d1, a1 + kk * 8, db, IDESC_S, 1u);
+                            ptx::mma_i8_ts(d0, a0 + kk * 8, db, IDESC_U, 1u);
+                        }
                     }
                     ptx::tc_commit(abempty0 + 8u * as);
                     if (c == CHUNKS - 1) ptx::tc_commit(dfull0 + 8u * ds);
@@ -424,29 +439,25 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                 const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
                 ptx::mbar_wait(dfull0 + 8u * ds, dph);
                 ptx::tc_fence_after();
-                const uint32_t d1_t = tmem_base + lane_addr + Gm::D_COL0 + ds * Gm::D_COLS, d0_t = d1_t + NB3;
+                const uint32_t d_t = tmem_base + lane_addr + Gm::D_COL0 + ds * Gm::D_COLS;
                 const uint32_t ft = ft_u32 + (uint32_t)((tm % FT) * NP) * 4u;
-                // 8 columns of n at a time: digits 2, 1, 0 of both byte planes, Horner in fp32
+                // 8 columns of n at a time: the four weight blocks W_3 .. W_0, Horner in fp32
 #pragma unroll
                 for (int pc = 0; pc < 2 * NP / 8; ++pc) {
-                    float S[8];
-#pragma unroll
-                    for (int l = 2; l >= 0; --l) {
-                        uint32_t hi[8], lo[8];
-                        ptx::tmem_ld8(d1_t + l * 2 * NP + 8 * pc, hi);
-                        ptx::tmem_ld8(d0_t + l * 2 * NP + 8 * pc, lo);
-                        ptx::tc_wait_ld();
-#pragma unroll
-                        for (int n = 0; n < 8; ++n) {
-                            const float T = (float)((int)hi[n] * 256 + (int)lo[n]);
-                            S[n] = l == 2 ? T : fmaf(S[n], 256.f, T);
-                        }
-                    }
+                    uint32_t w3[8], w2[8], w1[8], w0[8];
+                    ptx::tmem_ld8(d_t + 3 * 2 * NP + 8 * pc, w3);
+                    ptx::tmem_ld8(d_t + 2 * 2 * NP + 8 * pc, w2);
+                    ptx::tmem_ld8(d_t + 1 * 2 * NP + 8 * pc, w1);
+                    ptx::tmem_ld8(d_t + 8 * pc, w0);
+                    ptx::tc_wait_ld();
 #pragma unroll
                     for (int n = 0; n < 8; ++n) {
+                        float S = fmaf((float)(int)w3[n], 256.f, (float)(int)w2[n]);
+                        S = fmaf(S, 256.f, (float)(int)w1[n]);
+                        S = fmaf(S, 256.f, (float)(int)w0[n]);
                         float fr;
                         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(fr) : "r"(ft + (uint32_t)((8 * pc + n) % NP) * 4u));
-                        acc[8 * pc + n] = fmaf(fr, S[n], acc[8 * pc + n]);
+                        acc[8 * pc + n] = fmaf(fr, S, acc[8 * pc + n]);
                     }
                 }
                 ptx::tc_fence_before();
