@@ -703,7 +703,9 @@ def run_ours(args, cfg, daggers):
         # 3 = one propagator): not BASELINE configs, reported beside them
         line["extras"] = {}
         for key, name, ov in (("C5_int16_nrhs16", "C5", {"links": "i16"}), ("C5_int16_nrhs3", "C5", {"links": "i16", "nrhs": 3}),
-                              ("C4_nrhs3", "C4", {"nrhs": 3})):
+                              ("C4_nrhs3", "C4", {"nrhs": 3}),
+                              # the paper's own per-GPU coarse volumes (PAPER.md:L117/L125/L133): level 2 and level 3, int16
+                              ("P2_paper_level2_per_gpu", "P2", None), ("P3_paper_level3_per_gpu", "P3", None)):
             line["extras"][key] = measure_config(name, args.config_steps, local, dev, read_ceiling, override=ov)
             torch.cuda.empty_cache()
     if world == 1 and not args.no_cpu_baseline:
