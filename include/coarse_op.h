@@ -70,14 +70,18 @@ enum {
     COARSE_ENOMEM = -5
 };
 
-/* Kernel families.  AUTO picks STREAM for nrhs <= 4, TENSOR for the block shapes it covers, BLOCK
- * for the other nrhs <= 16, each when Nc is in the compiled set {32,48,64,96,128,192}; else SIMPLE.  Every family computes the same operation; tests run parity on each. */
+/* Kernel families, each compiled for Nc in {32,48,64,96,128,192}; every family computes the same operation and the
+ * tests run parity on each.  AUTO: 1 RHS -> STREAM; 2-4 RHS -> STREAM (its multi-RHS kernel), except int16 links with
+ * Nc >= 96 -> TENSOR; 5 RHS and more -> TENSOR; BLOCK only on request (or when no tensor map can be made for the links);
+ * Nc outside the compiled set -> SIMPLE. */
 enum {
     COARSE_PATH_AUTO = 0,
-    COARSE_PATH_SIMPLE = 1,  /* one thread per output element, any even Nc, any nrhs             */
-    COARSE_PATH_STREAM = 2,  /* persistent TMA-bulk -> smem ring -> CUDA-core consumers, nrhs <= 4 */
-    COARSE_PATH_TENSOR = 3,  /* block apply on tcgen05 tensor cores (3xTF32), nrhs in {8,16}, c64   */
-    COARSE_PATH_BLOCK = 4    /* block apply on the CUDA cores (same TMA ring), nrhs <= 16          */
+    COARSE_PATH_SIMPLE = 1,  /* one thread per output element, any even Nc, any nrhs                           */
+    COARSE_PATH_STREAM = 2,  /* persistent TMA-bulk -> smem ring -> CUDA-core consumers, nrhs <= 4              */
+    COARSE_PATH_TENSOR = 3,  /* block apply on the tcgen05 tensor cores, any nrhs (column tiles of 8 / 16, one launch
+                                per 16): complex64 links as 3xTF32, int16 links on the integer tensor cores (int8
+                                planes, exact), see COARSE_OPT_TENSOR_I8                                         */
+    COARSE_PATH_BLOCK = 4    /* block apply on the CUDA cores (same TMA ring), nrhs <= 16: the comparison arm    */
 };
 
 enum {
@@ -151,8 +155,8 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
  *     t_o   = Dhat_oe v_e           : apply_parts(hat, NULL, v, t, .., COARSE_PARITY_ODD, COARSE_LOCAL_NONE, 0, 1)
  *     out_e = v_e - Dhat_eo t_o     : apply_parts(hat, v, t, out, .., COARSE_PARITY_EVEN, COARSE_LOCAL_IDENTITY, 1, -1)
  *     out_e = X_e v_e - D_eo t_o    : apply_parts(op, v, t, out, .., COARSE_PARITY_EVEN, COARSE_LOCAL_X, 1, -1)
- * nrhs = 1 runs on the STREAM kernels (8 or 9 link matrices streamed per site of the parity),
- * other nrhs on SIMPLE. */
+ * nrhs = 1 runs on the STREAM kernels (8 or 9 link matrices streamed per site of the parity), several right-hand
+ * sides on the TENSOR kernels (SIMPLE outside the compiled Nc). */
 enum { COARSE_PARITY_EVEN = 0, COARSE_PARITY_ODD = 1, COARSE_PARITY_ALL = 2 };
 enum { COARSE_LOCAL_NONE = 0, COARSE_LOCAL_X = 1, COARSE_LOCAL_IDENTITY = 2 };
 int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev, void* out_dev, int nrhs,
