@@ -161,6 +161,15 @@ __device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) 
     lo = __float_as_uint(x - __uint_as_float(hi));
 }
 
+// The same for a pair: the two low parts come from ONE packed FMA, lo = x - hi = fma(hi, -1, x) (exact).
+__device__ __forceinline__ void split_tf32_pair(float x0, float x1, uint32_t& hi0, uint32_t& hi1, uint32_t& lo0, uint32_t& lo1) {
+    hi0 = __float_as_uint(x0) & 0xffffe000u;
+    hi1 = __float_as_uint(x1) & 0xffffe000u;
+    const float2 lo = ptx::ffma2(make_float2(__uint_as_float(hi0), __uint_as_float(hi1)), make_float2(-1.f, -1.f), make_float2(x0, x1));
+    lo0 = __float_as_uint(lo.x);
+    lo1 = __float_as_uint(lo.y);
+}
+
 // K-major, no-swizzle UMMA shared-memory descriptor (SM100 format): 8 x 16-byte core matrices,
 // LBO = byte step between the two k-halves of one MMA (128), SBO = byte step between 8-wide n groups.
 __device__ __forceinline__ uint64_t umma_desc_kmajor(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
@@ -441,7 +450,7 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
 #pragma unroll
-                for (int u = 0; u < 16; ++u) split_tf32(a[16 * h + u], hi[u], lo[u]);
+                for (int u = 0; u < 16; u += 2) split_tf32_pair(a[16 * h + u], a[16 * h + u + 1], hi[u], hi[u + 1], lo[u], lo[u + 1]);
                 ptx::tmem_st16(a_hi + 16 * h, hi);
                 ptx::tmem_st16(a_lo + 16 * h, lo);
             }
@@ -453,12 +462,10 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
                 const float b1x = vx, b1y = DAG ? vy : -vy;
                 const float b2x = vy, b2y = DAG ? -vx : vx;
                 uint32_t h0, l0, h1, l1;
-                split_tf32(b1x, h0, l0);
-                split_tf32(b1y, h1, l1);
+                split_tf32_pair(b1x, b1y, h0, h1, l0, l1);
                 ptx::sts64(b_hi + b_o1[x], __uint_as_float(h0), __uint_as_float(h1));
                 ptx::sts64(b_lo + b_o1[x], __uint_as_float(l0), __uint_as_float(l1));
-                split_tf32(b2x, h0, l0);
-                split_tf32(b2y, h1, l1);
+                split_tf32_pair(b2x, b2y, h0, h1, l0, l1);
                 ptx::sts64(b_hi + b_o2[x], __uint_as_float(h0), __uint_as_float(h1));
                 ptx::sts64(b_lo + b_o2[x], __uint_as_float(l0), __uint_as_float(l1));
             }
