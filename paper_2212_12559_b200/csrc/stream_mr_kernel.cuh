@@ -16,6 +16,14 @@
 #pragma once
 #include "stream_kernel.cuh"
 
+// Words (of the 4) of every int16 link quad decoded through the conversion unit (see stream2_kernel.cuh)
+#ifndef COARSE_MR_XU_N
+#define COARSE_MR_XU_N 2
+#endif
+#ifndef COARSE_MR_XU_D
+#define COARSE_MR_XU_D 1
+#endif
+
 namespace coarse {
 
 template <int NC, bool I16, int R>
@@ -174,7 +182,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                             float2 mm[CPQ];
                             if constexpr (I16) {
                                 const uint4 t = ptx::lds128u(a);
-                                unpack_i16_quad<2>(t, mm[0], mm[1], mm[CPQ - 2], mm[CPQ - 1]);
+                                unpack_i16_quad<COARSE_MR_XU_N>(t, mm[0], mm[1], mm[CPQ - 2], mm[CPQ - 1]);
                             } else {
                                 const float4 t = ptx::lds128(a);
                                 mm[0] = make_float2(t.x, t.y);
@@ -246,7 +254,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                                 float2 mm[CPQ];
                                 if constexpr (I16) {
                                     const uint4 t = ptx::lds128u(a);
-                                    unpack_i16_quad<1>(t, mm[0], mm[1], mm[CPQ - 2], mm[CPQ - 1]);
+                                    unpack_i16_quad<COARSE_MR_XU_D>(t, mm[0], mm[1], mm[CPQ - 2], mm[CPQ - 1]);
                                 } else {
                                     const float4 t = ptx::lds128(a);
                                     mm[0] = make_float2(t.x, t.y);
