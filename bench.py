@@ -708,6 +708,15 @@ def run_ours(args, cfg, daggers):
                               ("P2_paper_level2_per_gpu", "P2", None), ("P3_paper_level3_per_gpu", "P3", None)):
             line["extras"][key] = measure_config(name, args.config_steps, local, dev, read_ceiling, override=ov)
             torch.cuda.empty_cache()
+        # the SURVEY.md §8(f) rows on the C3 shape (the paper's level-2 operator): the even/odd Schur-hat operator (f1), one
+        # CA-GCR(8) smoother cycle (f3), and the device build of the block-preconditioned links on C1's lattice (f1)
+        sub = argparse.Namespace(**vars(args))
+        sub.steps, sub.warmup, sub.cheb = 10, 3, False
+        for key, fn, cname in (("schur_C3", run_schur, "C3"), ("cagcr8_C3", run_cagcr, "C3"), ("hat_links_C1", run_hat, "C1")):
+            rec = fn(sub, synth.config(cname), emit=False)
+            line["extras"][key] = {k: rec[k] for k in ("metric", "value", "unit", "ms_per_step", "config", "clocks", "gpu_launches",
+                                                       "roofline", "cagcr", "parity") if k in rec}
+            torch.cuda.empty_cache()
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = time_oracle(cfg, daggers, dev, min_seconds=args.cpu_seconds)
         if args.all_configs and args.config == "C2":
@@ -722,7 +731,7 @@ def run_ours(args, cfg, daggers):
 
 
 # ------------------------------------------------------------------------------- even/odd workload
-def run_schur(args, cfg):
+def run_schur(args, cfg, emit=True):
     """--workload schur (not the default bench line): the left-preconditioned
     Schur operator on block-preconditioned links, Shat_e v = v - Dhat_eo Dhat_oe v, and its adjoint.
     One step = Shat_e.v then Shat_e^H.v = 4 parity-restricted hop launches of V/2 sites each."""
@@ -780,12 +789,15 @@ def run_schur(args, cfg):
                      "schur_ms": ms0, "schur_dagger_ms": ms1, "algorithmic_bytes_per_schur_apply": bytes_schur,
                      "dagger_achieved": bytes_schur / (ms1 * 1e-3) / 1e9},
     }
+    if not emit:
+        op.close()
+        return line
     print(json.dumps(line), flush=True)
     op.close()
     return 0
 
 
-def run_hat(args, cfg):
+def run_hat(args, cfg, emit=True):
     """--workload hat: build the block-preconditioned links
     Yhat_m = X^-1 Y_m of the config's operator on the device (coarse_op_build_hat_links) and quantise them
     to int16 when the config stores int16 links.  A set-up step: one step = one build over the lattice.
@@ -864,12 +876,15 @@ def run_hat(args, cfg):
     }
     if parity is not None:
         line["parity"] = parity
+    if not emit:
+        op.close()
+        return line
     print(json.dumps(line), flush=True)
     op.close()
     return 0
 
 
-def run_cagcr(args, cfg):
+def run_cagcr(args, cfg, emit=True):
     """--workload cagcr: CA-GCR(8) smoother cycles on the config's operator
     (diagonally shifted so that the smoother converges).  One step = one cycle = 8 applies + 7 fused
     Chebyshev recurrence steps + the fused Gram pass + the 8x8 solve + the fused update (+ the interval estimate)."""
@@ -943,6 +958,9 @@ def run_cagcr(args, cfg):
                   "residual_reduction_one_cycle": float(np.sqrt(max(inf[1], 0.0) / inf[0])) if inf[0] > 0 else None,
                   "basis_vectors_kept": int(inf[2])},
     }
+    if not emit:
+        op.close()
+        return line
     print(json.dumps(line), flush=True)
     op.close()
     return 0
