@@ -24,7 +24,7 @@ def family(mangled: str) -> str:
     m = re.search(r"coarse\d+(coarse_apply_[a-z0-9_]+?)I", mangled)
     if m:
         return m.group(1)
-    m = re.search(r"\d+([a-z_0-9]+kernel)", mangled)
+    m = re.search(r"coarse\d+([a-z_0-9]+kernel)", mangled)
     return m.group(1) if m else mangled[:40]
 
 
