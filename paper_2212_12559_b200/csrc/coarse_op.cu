@@ -86,10 +86,16 @@ int launch_stream_mr(const coarse_op* op, const void* in, void* out, int nrhs, i
     p.in = static_cast<const float2*>(in);
     p.out = static_cast<float2*>(out);
     p.keep_links = op->keep_opt == 2 || (op->keep_opt == 0 && coarse_op_link_bytes(op) <= (size_t)op->l2_bytes / 2);
-    p.parity = 2;
-    p.n_sites = op->lat.V;
+    p.parity = ps.parity;
+    p.n_sites = ps.parity == 2 ? op->lat.V : op->lat.V / 2;
     p.n_items = ps.site_end > 0 ? ps.site_end : 0;
     p.item_begin = ps.site_end > 0 ? ps.site_begin : 0;
+    p.gen = ps.gen ? 1 : 0;                                    // parts apply: runtime flags of the multi-RHS kernel
+    p.in_local = static_cast<const float2*>(ps.gen && ps.local != 0 ? ps.u : in);
+    p.alpha = ps.alpha;
+    p.beta = ps.beta;
+    p.m_begin = ps.local == 1 ? 0 : 1;
+    p.identity = ps.local == 2 ? 1 : 0;
     switch (op->Nc) {
 #define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_stream_mr_nc, NC)(op, p, nrhs, dagger, stream);
         COARSE_FOR_EACH_NC(COARSE_CASE_NC)
@@ -519,18 +525,21 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
     }
     PartsSpec ps = {true, local != 0 ? u_dev : w_dev, parity, local, alpha, beta, nullptr, 0, 0};
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    // 1 RHS: STREAM (GEN instantiations); more: the TENSOR kernel (parity list, alpha / beta folded into the
-    // B operand, identity term in the epilogue); shapes neither covers: SIMPLE.  BLOCK has no parts variant.
+    // 1 RHS: STREAM (GEN instantiations); 2-4: STREAM-MR (runtime flags), except int16 links with Nc >= 96; more: the
+    // TENSOR kernels (parity list, alpha / beta folded into the B operand, identity term in the epilogue); shapes none of
+    // them covers: SIMPLE.
     int path = op->path_opt;
     const bool tensor_ok = tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok;
-    if (path == COARSE_PATH_AUTO || path == COARSE_PATH_BLOCK || (path == COARSE_PATH_STREAM && nrhs != 1) ||
-        (path == COARSE_PATH_TENSOR && !tensor_ok))
-        path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM : tensor_ok ? COARSE_PATH_TENSOR : COARSE_PATH_SIMPLE;
+    const bool stream_ok = stream_supports(op->Nc, nrhs) || stream_mr_supports(op->Nc, nrhs);
+    if (path == COARSE_PATH_AUTO || path == COARSE_PATH_BLOCK) {
+        path = auto_path(op, nrhs);                                     // the plain apply's rule; BLOCK has no parts variant
+        if (path == COARSE_PATH_BLOCK) path = COARSE_PATH_SIMPLE;
+    } else if ((path == COARSE_PATH_STREAM && !stream_ok) || (path == COARSE_PATH_TENSOR && !tensor_ok)) {
+        path = stream_ok ? COARSE_PATH_STREAM : tensor_ok ? COARSE_PATH_TENSOR : COARSE_PATH_SIMPLE;
+    }
     op->last_launches = 0;
     if (path == COARSE_PATH_STREAM) {
-        if (!stream_supports(op->Nc, nrhs))
-            return fail(COARSE_EUNSUPPORTED, "apply_parts: STREAM path does not cover Nc=%d nrhs=%d", op->Nc, nrhs);
-        rc = launch_stream(op, w_dev, out_dev, dagger, ps, st);
+        rc = nrhs == 1 ? launch_stream(op, w_dev, out_dev, dagger, ps, st) : launch_stream_mr(op, w_dev, out_dev, nrhs, dagger, ps, st);
     } else if (path == COARSE_PATH_TENSOR) {
         rc = launch_tensor(op, w_dev, out_dev, nrhs, dagger, ps, st);
     } else {

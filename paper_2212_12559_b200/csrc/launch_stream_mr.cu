@@ -15,7 +15,7 @@ int launch_stream_mr_t(const coarse_op* op, const StreamParams& base, cudaStream
     using Gm = StreamGeom<NC, I16, false, false, true>;
     using Gr = StreamMrGeom<NC, I16, R>;
     StreamParams p = base;
-    p.n_items = DAG ? op->lat.V : op->lat.V * Gm::NB;
+    p.n_items = DAG ? base.n_sites : base.n_sites * Gm::NB;      // n_sites: the parity set of a parts apply, else V
     p.item_begin = 0;
     if (base.n_items > 0) {                       // a site range [item_begin, n_items) was requested (in sites)
         p.item_begin = DAG ? base.item_begin : base.item_begin * Gm::NB;

@@ -51,6 +51,7 @@ struct StreamParams {
     int identity;             // 1: add alpha*u(x) to the result (local = identity)
     int parity;               // 0 even, 1 odd, 2 all sites
     int n_sites;              // sites in the parity set
+    int gen;                  // STREAM-MR only (runtime flag there): 1 = parts apply (the 1-RHS kernels use the GEN template)
     int pdl;                  // 1: launched with programmatic stream serialization (COARSE_OPT_PDL)
     int item_begin;           // work items [item_begin, n_items): coarse_op_apply_host launches site ranges
     // dagger = 1 on a tiny lattice: split a site's contraction over its NB row chunks (item = (site, chunk)):

@@ -85,15 +85,17 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
         int slot = 0;
         uint32_t phase = 0;
         for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
-            const int s = DAG ? item : item / NB;
+            const int sidx = DAG ? item : item / NB;
+            const int s = p.parity != 2 ? parity_site(p.lat, sidx, p.parity) : sidx;      // parts apply: one parity
             const int rb = DAG ? 0 : item % NB;
             const SiteX cx = site_coords(p.lat, s);
 #pragma unroll
             for (int m = 0; m < 9; ++m) {
+                if (m < p.m_begin) continue;                                              // parts apply: no X stage
                 const int sv = stencil_site_x(p.lat, s, cx, m, DAG ? 1 : 0);
                 const int sm = DAG ? sv : s;
                 const unsigned char* mat = p.links + ((int64_t)sm * 9 + m) * ((int64_t)NC * ROWBYTES);
-                const float2* vec = p.in + (int64_t)sv * NC * R;
+                const float2* vec = (m == 0 ? p.in_local : p.in) + (int64_t)sv * NC * R;
 #pragma unroll 1
                 for (int c = 0; c < (DAG ? NB : 1); ++c) {
                     const int r0 = DAG ? c * RS : rb * RS;
@@ -122,17 +124,22 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
     uint32_t phase = 0;
 
     float cur_scale = 1.f, next_scale = 1.f, next2_scale = 1.f;
+    auto site_of = [&](int item) -> int {
+        const int sidx = DAG ? item : item / NB;
+        return p.parity != 2 ? parity_site(p.lat, sidx, p.parity) : sidx;
+    };
     auto fetch_scale = [&](int item) -> float {
         if (!I16 || lane >= 9 || item >= p.n_items) return 1.f;
-        const int s = DAG ? item : item / NB;
+        const int s = site_of(item);
         const int sm = DAG ? stencil_site(p.lat, s, lane, 1) : s;
         return __ldg(p.scales + (int64_t)sm * 9 + lane);
     };
+    const bool scale_v = I16 || p.gen != 0;        // the vector operand carries the link scale and / or alpha, beta
     next_scale = fetch_scale(p.item_begin + blockIdx.x);
     next2_scale = fetch_scale(p.item_begin + blockIdx.x + gridDim.x);
 
     for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
-        const int s = DAG ? item : item / NB;
+        const int s = site_of(item);
         const int rb = DAG ? 0 : item % NB;
         cur_scale = next_scale;
         next_scale = next2_scale;
@@ -145,8 +152,9 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
 #pragma unroll
                 for (int r = 0; r < R; ++r) pacc[k][r].a = pacc[k][r].b = make_float2(0.f, 0.f);
 #pragma unroll 1
-            for (int m = 0; m < 9; ++m) {
-                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+            for (int m = p.m_begin; m < 9; ++m) {
+                float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                if (p.gen) sc *= (m == 0) ? p.alpha : p.beta;
                 ptx::mbar_wait(full0 + 8u * slot, phase);
                 const uint32_t lbase = link_u32 + slot * LINK_STAGE + qi * 16;
                 uint32_t vbase = vec_u32 + slot * VEC_STAGE;
@@ -171,7 +179,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
 #pragma unroll
                         for (int h = 0; h < CPQ * R / 2; ++h) {
                             float4 t = ptx::lds128(va + h * 16);
-                            if constexpr (I16) { t.x *= sc; t.y *= sc; t.z *= sc; t.w *= sc; }
+                            if (scale_v) { t.x *= sc; t.y *= sc; t.z *= sc; t.w *= sc; }
                             v[2 * h] = vdup(make_float2(t.x, t.y));
                             v[2 * h + 1] = vdup(make_float2(t.z, t.w));
                         }
@@ -218,7 +226,15 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                 if (qi == 0) {
                     const int row = rb * RS + (k * W + warp) * RPL + grp;
 #pragma unroll
-                    for (int r = 0; r < R; ++r) p.out[((int64_t)s * NC + row) * R + r] = acc[k][r];
+                    for (int r = 0; r < R; ++r) {
+                        float2 o = acc[k][r];
+                        if (p.identity) {           // parts apply: + alpha u(x); each element reads only its own u element
+                            const float2 u = __ldg(p.in_local + ((int64_t)s * NC + row) * R + r);
+                            o.x = fmaf(p.alpha, u.x, o.x);
+                            o.y = fmaf(p.alpha, u.y, o.y);
+                        }
+                        p.out[((int64_t)s * NC + row) * R + r] = o;
+                    }
                 }
             }
         } else {
@@ -230,8 +246,9 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
 #pragma unroll
                     for (int r = 0; r < R; ++r) pacc[ps][e][r].a = pacc[ps][e][r].b = make_float2(0.f, 0.f);
 #pragma unroll 1
-            for (int m = 0; m < 9; ++m) {
-                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+            for (int m = p.m_begin; m < 9; ++m) {
+                float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                if (p.gen) sc *= (m == 0) ? p.alpha : p.beta;
 #pragma unroll 1
                 for (int c = 0; c < NB; ++c) {
                     ptx::mbar_wait(full0 + 8u * slot, phase);
@@ -245,7 +262,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
                                 float2 t = ptx::lds64(vbase + (rl * R + r) * 8);
-                                if constexpr (I16) { t.x *= sc; t.y *= sc; }
+                                if (scale_v) { t.x *= sc; t.y *= sc; }
                                 vj[r] = vdup(t);
                             }
 #pragma unroll
@@ -291,6 +308,11 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                     const float2 x = red[g * NC * R + t];
                     sum.x += x.x;
                     sum.y += x.y;
+                }
+                if (p.identity) {
+                    const float2 u = __ldg(p.in_local + (int64_t)s * NC * R + t);
+                    sum.x = fmaf(p.alpha, u.x, sum.x);
+                    sum.y = fmaf(p.alpha, u.y, sum.y);
                 }
                 p.out[(int64_t)s * NC * R + t] = sum;
             }

@@ -370,9 +370,6 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
 #pragma unroll
                 for (int u = 0; u < KC; ++u) w[u] = 0u;
             }
-            ptx::fence_cta();          // the loads must have completed before the slot goes back (see tensor_kernel.cuh)
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
 
             ptx::mbar_wait(abempty0 + 8u * as, aph ^ 1u);
             ptx::tc_fence_after();
@@ -420,6 +417,8 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(abfull0 + 8u * as);
+            // link slot back to the producer: after the loaded entries have gone into tensor memory (see tensor_kernel.cuh)
+            if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
         }
     } else if (warp >= Gm::EPI_W0) {
         // ---------------------------------------------------------------- epilogue

@@ -436,12 +436,6 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
 #pragma unroll
                 for (int u = 0; u < 32; ++u) a[u] = 0.f;
             }
-            // The loaded values are not consumed before the release below, and SYNCS.ARRIVE does not wait
-            // for in-flight LDS: without this fence the producer's next TMA write into the slot can overtake
-            // the reads (seen on B200 as sporadic stale 512-byte runs).  The fence completes the loads.
-            ptx::fence_cta();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);      // link slot back to the producer
 
             ptx::mbar_wait(abempty0 + 8u * as, aph ^ 1u);            // MMAs that read this operand slot are done
             ptx::tc_fence_after();
@@ -474,6 +468,11 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(abfull0 + 8u * as);
+            // Link slot back to the producer - only HERE, after the loaded values have gone through the split into
+            // tensor memory (wait::st above): the release must come after a CONSUMER of the loads in program order.
+            // Releasing right after the loads behind a fence.acq_rel.cta (rounds 1 and 2 until a stress run) let the
+            // producer's next TMA write overtake the reads once in ~600-2000 applies (a few wrong rows at one site).
+            if (lane == 0) ptx::mbar_arrive(empty0 + 8u * slot);
         }
     } else if (warp >= Gm::EPI_W0) {
         // ---------------------------------------------------------------- epilogue

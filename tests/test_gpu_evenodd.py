@@ -109,6 +109,37 @@ def test_parts_tensor(oracle_lib, Nc, prec, nrhs, dagger, parity, local):
     _check_parts(oracle_lib, dims, Nc, prec, nrhs, dagger, parity, local, cop.PATH_TENSOR)
 
 
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("nrhs", [2, 3, 4])
+@pytest.mark.parametrize("dagger", [0, 1])
+@pytest.mark.parametrize("parity,local", [(0, 0), (1, 1), (2, 2), (0, 2), (1, 0), (2, 1)])
+def test_parts_stream_few_rhs(oracle_lib, Nc, prec, nrhs, dagger, parity, local):
+    """2-4 right-hand sides (3 = one propagator) of the parts apply on the STREAM-MR kernel: parity list,
+    X stage on / off, alpha / beta folded into the vector operand, identity term added at the store."""
+    dims = (2, 2, 4, 2) if Nc >= 128 else (4, 2, 2, 4)
+    _check_parts(oracle_lib, dims, Nc, prec, nrhs, dagger, parity, local, cop.PATH_STREAM)
+
+
+def test_parts_auto_routes_few_rhs():
+    dims = (2, 2, 2, 2)
+    for Nc, prec, nrhs, want in ((48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_STREAM),
+                                 (128, cop.LINK_I16, 3, cop.PATH_TENSOR), (128, cop.LINK_C64, 2, cop.PATH_STREAM)):
+        V = 16
+        if prec == cop.LINK_C64:
+            links, scales = torch.zeros((V, 9, Nc, Nc), dtype=torch.complex64, device="cuda"), None
+        else:
+            links = torch.zeros((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+            scales = torch.ones((V, 9), dtype=torch.float32, device="cuda")
+        u = torch.zeros((V, Nc, nrhs), dtype=torch.complex64, device="cuda")
+        w, out = torch.zeros_like(u), torch.zeros_like(u)
+        op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+        op.apply_parts(u, w, out, nrhs=nrhs, parity=cop.PARITY_ODD, local=cop.LOCAL_IDENTITY, alpha=1.0, beta=-1.0)
+        torch.cuda.synchronize()
+        assert op.last_path == want, (Nc, prec, nrhs, op.last_path)
+        op.close()
+
+
 def test_parts_auto_routes_multi_rhs_to_tensor():
     dims, Nc, nrhs = (2, 2, 2, 2), 48, 5
     links = synth.make_arbitrary_links(dims, Nc, 5, device="cuda")
@@ -241,15 +272,16 @@ def test_parts_identity_in_place_values(oracle_lib, Nc, prec, dagger, path):
 @pytest.mark.parametrize("dagger", [0, 1])
 def test_parts_identity_in_place_values_multi_rhs(oracle_lib, Nc, prec, dagger):
     """The same in-place update with several right-hand sides, on the tensor kernels (the identity term is read in
-    the epilogue by the thread that then stores the element)."""
-    dims, nrhs = (2, 4, 2, 2), 5
-    links_d, scales_d, links_h, scales_h, u, w = _make(oracle_lib, dims, Nc, prec, 978, nrhs)
-    op = cop.CoarseOp(dims, Nc, prec).set_links(links_d, scales_d)
-    buf = u.clone()
-    op.apply_parts(buf, w, buf, nrhs=nrhs, dagger=dagger, parity=cop.PARITY_ALL, local=cop.LOCAL_IDENTITY, alpha=1.0, beta=-1.0)
-    torch.cuda.synchronize()
-    assert op.last_path == cop.PATH_TENSOR
-    ref = oracle_lib.coarse_apply_parts(dims, Nc, links_h, u.cpu().numpy(), w.cpu().numpy(), nrhs=nrhs, dagger=dagger, parity=2,
-                                        local=2, alpha=1.0, beta=-1.0, link_precision=prec, scales=scales_h)
-    assert rel_l2_per_rhs(buf.cpu().numpy(), ref) <= TOL
-    op.close()
+    the epilogue by the thread that then stores the element) and on STREAM-MR (read at the store)."""
+    dims = (2, 4, 2, 2)
+    for nrhs, want in ((5, cop.PATH_TENSOR), (3, cop.PATH_TENSOR if (prec == cop.LINK_I16 and Nc >= 96) else cop.PATH_STREAM)):
+        links_d, scales_d, links_h, scales_h, u, w = _make(oracle_lib, dims, Nc, prec, 978, nrhs)
+        op = cop.CoarseOp(dims, Nc, prec).set_links(links_d, scales_d)
+        buf = u.clone()
+        op.apply_parts(buf, w, buf, nrhs=nrhs, dagger=dagger, parity=cop.PARITY_ALL, local=cop.LOCAL_IDENTITY, alpha=1.0, beta=-1.0)
+        torch.cuda.synchronize()
+        assert op.last_path == want
+        ref = oracle_lib.coarse_apply_parts(dims, Nc, links_h, u.cpu().numpy(), w.cpu().numpy(), nrhs=nrhs, dagger=dagger, parity=2,
+                                            local=2, alpha=1.0, beta=-1.0, link_precision=prec, scales=scales_h)
+        assert rel_l2_per_rhs(buf.cpu().numpy(), ref) <= TOL
+        op.close()

@@ -235,6 +235,35 @@ def test_tensor_path_matches_cuda_core_path_and_is_reproducible():
     op.close()
 
 
+@pytest.mark.parametrize("Nc,prec,applies", [(64, cop.LINK_C64, 1200), (128, cop.LINK_I16, 600)])
+def test_tensor_kernels_bit_reproducible_under_stress(Nc, prec, applies):
+    """Many applies on a lattice with ~55 work items per CTA: every result must equal the first one bit for bit.  (An
+    earlier version released a link slot right after loading it, behind a fence only; the producer's next TMA write
+    overtook the reads once in 600-2000 applies and a few rows of one site came out wrong.)"""
+    dims, nrhs = (8, 8, 8, 16), 16
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, 5, device="cuda")
+    scales = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+        scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        links = q
+    vin = synth.make_vectors(dims, Nc, nrhs, 6, device="cuda")
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales).set_option(cop.OPT_PATH, cop.PATH_TENSOR)
+    refs = {}
+    for dagger in (0, 1):
+        refs[dagger] = torch.empty_like(vin)
+        op.apply(vin, refs[dagger], nrhs=nrhs, dagger=dagger)
+    out = torch.empty_like(vin)
+    bad = 0
+    for it in range(applies):
+        op.apply(vin, out, nrhs=nrhs, dagger=it % 2)
+        bad += int(not torch.equal(torch.view_as_real(out), torch.view_as_real(refs[it % 2])))
+    assert bad == 0, f"{bad} of {applies} applies differ from the first one"
+    op.close()
+
+
 def test_tensor_path_unsupported_shapes():
     L = cop.lib()
     h = cop.coarse_op_create((2, 2, 2, 2), 80, cop.LINK_I16)          # Nc outside the compiled set
