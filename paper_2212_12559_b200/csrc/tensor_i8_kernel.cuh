@@ -30,6 +30,10 @@
 #pragma once
 #include "tensor_kernel.cuh"
 
+#ifndef COARSE_TENSOR_RING_BYTES
+#define COARSE_TENSOR_RING_BYTES 131072      // link bytes in the TMA ring per SM (slots being converted included)
+#endif
+
 namespace coarse {
 
 #ifndef COARSE_I8_NG
@@ -55,7 +59,7 @@ struct TensorI8Geom {
     static constexpr int B_STAGE = 2 * KC * NB3;               // int8 B tile of a stage, bytes
     static constexpr int B_SBO = (2 * KC / 16) * 128;          // byte stride between 8-column groups of n
     static constexpr int NE = KC * NP / 128;                   // B entries per converter thread and stage
-    static constexpr int LS = tensor_clamp(131072 / LINK_STAGE, 4, 16);
+    static constexpr int LS = tensor_clamp(COARSE_TENSOR_RING_BYTES / LINK_STAGE, 4, 20);
     static constexpr int AS = 4;
     static constexpr int A_HALF = KC / 2;                      // TMEM columns of one byte plane (4 int8 per column)
     static constexpr int A_COLS = 2 * A_HALF;                  // high bytes | low bytes

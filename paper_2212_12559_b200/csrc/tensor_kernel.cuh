@@ -44,6 +44,10 @@
 
 #include "common.cuh"
 
+#ifndef COARSE_TENSOR_RING_BYTES
+#define COARSE_TENSOR_RING_BYTES 131072      // link bytes in the TMA ring per SM (slots being converted included)
+#endif
+
 namespace coarse {
 
 struct TensorParams {
@@ -77,7 +81,7 @@ struct TensorGeom {
     static constexpr int NE = NP / 8;                   // B entries per converter thread and stage
     static constexpr int B_HALF = KSTAGE * N * 4;       // B hi (or lo) bytes per stage
     static constexpr int B_SBO = (KSTAGE / 4) * 128;    // byte stride between 8-column groups of n
-    static constexpr int LS = tensor_clamp(131072 / LINK_STAGE, 4, 16);   // link ring depth (TMA -> converters)
+    static constexpr int LS = tensor_clamp(COARSE_TENSOR_RING_BYTES / LINK_STAGE, 4, 20);   // link ring depth (TMA -> converters)
     static constexpr int AS = 4;                        // operand ring depth (converters -> MMA)
     static constexpr int A_COLS = 2 * KSTAGE;           // TMEM columns per operand stage: hi | lo
     static constexpr int D_COL0 = AS * A_COLS;
