@@ -264,6 +264,39 @@ def test_tensor_kernels_bit_reproducible_under_stress(Nc, prec, applies):
     op.close()
 
 
+@pytest.mark.parametrize("Nc,prec,nrhs,opts", [
+    (48, cop.LINK_C64, 1, {}), (128, cop.LINK_C64, 1, {}), (64, cop.LINK_I16, 1, {}), (48, cop.LINK_I16, 1, {}),
+    (64, cop.LINK_I16, 1, {cop.OPT_WARP_ITEMS: 1}), (64, cop.LINK_I16, 3, {}), (48, cop.LINK_C64, 4, {}),
+    (64, cop.LINK_I16, 5, {cop.OPT_PATH: cop.PATH_BLOCK})])
+def test_streaming_kernels_bit_reproducible_under_stress(Nc, prec, nrhs, opts):
+    """The same watch on the TMA-ring kernels that run on the CUDA cores (cooperative and warp-team STREAM, STREAM-MR,
+    BLOCK): 1000 applies on a lattice with ~55 work items per CTA, each equal to the first bit for bit."""
+    dims = (8, 8, 8, 16)
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, 5, device="cuda")
+    scales = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+        scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        links = q
+    vin = synth.make_vectors(dims, Nc, nrhs, 6, device="cuda")
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    for k, v in opts.items():
+        op.set_option(k, v)
+    refs = {}
+    for dagger in (0, 1):
+        refs[dagger] = torch.empty_like(vin)
+        op.apply(vin, refs[dagger], nrhs=nrhs, dagger=dagger)
+    out = torch.empty_like(vin)
+    bad = 0
+    for it in range(1000):
+        op.apply(vin, out, nrhs=nrhs, dagger=it % 2)
+        bad += int(not torch.equal(torch.view_as_real(out), torch.view_as_real(refs[it % 2])))
+    assert bad == 0, f"{bad} of 1000 applies differ from the first one"
+    op.close()
+
+
 def test_tensor_path_unsupported_shapes():
     L = cop.lib()
     h = cop.coarse_op_create((2, 2, 2, 2), 80, cop.LINK_I16)          # Nc outside the compiled set
