@@ -660,7 +660,7 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
     }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     cudaError_t e;
-    // Pipelined path (STREAM kernels for 1-4 RHS, TENSOR kernel beyond; at least 8 time slices): the lattice is cut into 4 ranges
+    // Pipelined path (STREAM kernels for 1-4 RHS, TENSOR kernel beyond; at least 8 time slices): the lattice is cut into 4 (or 8) ranges
     // of x3-slices; range c is launched as soon as the slices it reads (its own and one on either side)
     // are on the device, and its result goes back to the host while the next range computes.  H2D, the
     // kernels and D2H run on three streams; nothing is reordered inside a range, so the result is
@@ -675,20 +675,20 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
         if (!op->host_pipe_ok) {
             // create the two copy streams and nine events; on a partial failure destroy what exists
             cudaStream_t ss[2] = {nullptr, nullptr};
-            cudaEvent_t ev[9] = {};
+            cudaEvent_t ev[17] = {};
             bool ok = true;
             for (int i = 0; ok && i < 2; ++i) ok = cudaStreamCreateWithFlags(&ss[i], cudaStreamNonBlocking) == cudaSuccess;
-            for (int i = 0; ok && i < 9; ++i) ok = cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming) == cudaSuccess;
+            for (int i = 0; ok && i < 17; ++i) ok = cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming) == cudaSuccess;
             if (!ok) {
                 cudaGetLastError();
-                for (int i = 0; i < 9; ++i) if (ev[i]) cudaEventDestroy(ev[i]);
+                for (int i = 0; i < 17; ++i) if (ev[i]) cudaEventDestroy(ev[i]);
                 for (int i = 0; i < 2; ++i) if (ss[i]) cudaStreamDestroy(ss[i]);
                 return fail(COARSE_ECUDA, "apply_host: cannot create copy streams/events");
             }
             op->s_h2d = ss[0];
             op->s_d2h = ss[1];
-            for (int i = 0; i < 4; ++i) { op->ev_up[i] = ev[i]; op->ev_k[i] = ev[4 + i]; }
-            op->ev_done = ev[8];
+            for (int i = 0; i < 8; ++i) { op->ev_up[i] = ev[i]; op->ev_k[i] = ev[8 + i]; }
+            op->ev_done = ev[16];
             op->host_pipe_ok = true;
         }
         const size_t plane = (size_t)(op->lat.V / T);               // sites per x3-slice
@@ -715,8 +715,11 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
         int uploaded = 0;                                            // slices [0, uploaded) are queued
         PartsSpec ps = kPlain;
         op->last_launches = 0;
-        for (int c = 0; c < 4; ++c) {
-            const int t0 = (int)((long long)T * c / 4), t1 = (int)((long long)T * (c + 1) / 4);
+        // 4 ranges; 8 when the copies dominate (vectors of 32 MiB and more: several right-hand sides), so that less of the
+        // first upload and the last download is exposed
+        const int NR = (vb >= ((size_t)1 << 25) && T >= 8) ? 8 : 4;
+        for (int c = 0; c < NR; ++c) {
+            const int t0 = (int)((long long)T * c / NR), t1 = (int)((long long)T * (c + 1) / NR);
             int need = t1 + 1 < T - 1 ? t1 + 1 : T - 1;              // slices [0, need) plus slice T-1
             if (need > uploaded) {
                 e = cudaMemcpyAsync(din + (size_t)uploaded * pb, hin + (size_t)uploaded * pb, (size_t)(need - uploaded) * pb,
@@ -1001,7 +1004,7 @@ void coarse_op_destroy(coarse_op_t* op) {
     if (op->split_ws) cudaFree(op->split_ws);
     if (op->vscale) cudaFree(op->vscale);
     if (op->host_pipe_ok) {
-        for (int i = 0; i < 4; ++i) { cudaEventDestroy(op->ev_up[i]); cudaEventDestroy(op->ev_k[i]); }
+        for (int i = 0; i < 8; ++i) { cudaEventDestroy(op->ev_up[i]); cudaEventDestroy(op->ev_k[i]); }
         cudaEventDestroy(op->ev_done);
         cudaStreamDestroy(op->s_h2d);
         cudaStreamDestroy(op->s_d2h);

@@ -42,7 +42,7 @@ struct coarse_op {
     void* stage_out;
     size_t stage_bytes;
     cudaStream_t s_h2d, s_d2h;      // apply_host's copy streams and events (created on first use)
-    cudaEvent_t ev_up[4], ev_k[4], ev_done;
+    cudaEvent_t ev_up[8], ev_k[8], ev_done;   // up to 8 ranges of x3-slices
     bool host_pipe_ok;
     CUtensorMap link_map[2];   // 2-D views of the link array for the TENSOR path (dagger 0 / dagger 1 slabs, link_map.cu)
     bool link_map_ok;

@@ -582,8 +582,8 @@ def test_apply_host_pipelined_path_is_bit_identical(oracle_lib, prec):
 
 
 @pytest.mark.parametrize("Nc,prec,nrhs,want_path,launches", [
-    (48, cop.LINK_I16, 3, cop.PATH_STREAM, 4), (64, cop.LINK_C64, 16, cop.PATH_TENSOR, 4),
-    (48, cop.LINK_I16, 20, cop.PATH_TENSOR, 8)])
+    (48, cop.LINK_I16, 3, cop.PATH_STREAM, 4), (64, cop.LINK_C64, 16, cop.PATH_TENSOR, 8),
+    (48, cop.LINK_I16, 20, cop.PATH_TENSOR, 16)])
 def test_apply_host_pipelined_multi_rhs_is_bit_identical(oracle_lib, Nc, prec, nrhs, want_path, launches):
     """The pipelined host path for several right-hand sides: STREAM-MR (3 = one propagator) and
     TENSOR launch ranges of x3-slices too; results must equal the device-resident apply bit for bit."""
