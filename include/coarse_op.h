@@ -192,9 +192,9 @@ int coarse_op_quantize_vec_i16(const void* v_c64_dev, int64_t n_sites, int Nc, i
  * synchronises the stream before returning.  Pinned host memory gives full PCIe rate.
  * On the STREAM (1-4 RHS) and TENSOR kernels, with dims[3] >= 8 and vectors of at least 4 MiB, the call is
  * pipelined: the lattice is cut into 4 ranges of x3-slices (8 when the vectors are 32 MiB or more), each launched as
- * soon as the slices it
- * reads are on the device, its result copied back while the next range computes (H2D, kernels and
- * D2H on three streams, two of them owned by the handle); the result is bit-identical. */
+ * soon as the slices it reads are on the device, its result copied back while the next range computes (H2D, kernels
+ * and D2H on three streams, two of them owned by the handle); the result is bit-identical to coarse_op_apply's (int16
+ * links with 5 or more right-hand sides: to its result with COARSE_OPT_TENSOR_I8 = 1, see there). */
 int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, int nrhs, int dagger,
                          void* stream);
 
