@@ -33,7 +33,8 @@
 //   epilogue (4 warps)      tcgen05.ld D -> registers, adds the nine per-matrix partial results in
 //                           round-to-nearest fp32 -> out[s][i][r]; a ring of 4 accumulator slots lets
 //                           the next matrices' MMAs overlap the read-out.
-// Work item = (site, tile of MT = Nc / NT output indices); NT = 2 for Nc = 192 (M = 128 per MMA).
+// Work item = (site, tile of MT = Nc / NT output indices); NT = 2 for Nc = 192 (M = 128 per MMA); for Nc <= 64 a work
+// item is a PAIR of sites sharing the 128-lane tile (TensorGeom::NS).
 // One launch handles NP = 8 or 16 right-hand-side columns [r0, r0 + width) of vectors with `nrhs`
 // columns; columns >= width are zero-padded in B and not stored (nrhs = 3 runs as NP = 8, nrhs = 40 as
 // three launches).  The parts apply (coarse_op_apply_parts: parity-restricted site list, X stage on/off,
@@ -76,17 +77,24 @@ struct TensorGeom {
     static constexpr int KSTAGE = 32;                   // real k per stage = 16 complex columns
     static constexpr int CHUNKS = NC / 16;              // stages per link matrix
     static constexpr int SLAB_ROW = 16 * ENTRY;         // dagger 0: bytes per slab row (128 | 64)
-    static constexpr int LINK_STAGE = MT * 16 * ENTRY;  // bytes per stage (both dagger modes)
-    static constexpr int N = 2 * NP;                    // MMA N: [Re out | Im out]
-    static constexpr int NE = NP / 8;                   // B entries per converter thread and stage
+    // Matrices of at most 64 rows (Nc <= 64) would leave half of the 128-lane MMA tile idle while the kernel is bound by
+    // the NUMBER of MMAs and pipeline stages (a stage costs ~350 ns whatever its size): a work item then holds TWO
+    // sites - site 0 in lanes 0.., site 1 in lanes 64.. - whose B operands sit side by side along N; each MMA computes both
+    // (the two off-diagonal blocks of its result are never read).  Half the stages and MMAs per site.
+    static constexpr int NS = MT <= 64 ? 2 : 1;         // sites per work item
+    static constexpr int SLAB_BYTES = MT * 16 * ENTRY;  // one site's slab of a stage (both dagger modes)
+    static constexpr int SLAB_PITCH = NS == 2 ? 64 * SLAB_ROW : SLAB_BYTES;   // smem distance between the two sites' slabs
+    static constexpr int LINK_STAGE = NS * SLAB_PITCH;  // smem bytes per stage
+    static constexpr int N = 2 * NP * NS;               // MMA N: per site [Re out | Im out]
+    static constexpr int NE = NS * NP / 8;              // B entries per converter thread and stage
     static constexpr int B_HALF = KSTAGE * N * 4;       // B hi (or lo) bytes per stage
     static constexpr int B_SBO = (KSTAGE / 4) * 128;    // byte stride between 8-column groups of n
     static constexpr int LS = tensor_clamp(COARSE_TENSOR_RING_BYTES / LINK_STAGE, 4, 20);   // link ring depth (TMA -> converters)
     static constexpr int AS = 4;                        // operand ring depth (converters -> MMA)
     static constexpr int A_COLS = 2 * KSTAGE;           // TMEM columns per operand stage: hi | lo
     static constexpr int D_COL0 = AS * A_COLS;
-    static constexpr int DS = 4;                        // accumulator ring depth (MMA -> epilogue), one slot per link matrix
     static constexpr int D_COLS = 2 * N;                // per slot: [hi.hi chain | hi.lo + lo.hi chain]
+    static constexpr int DS = tensor_clamp((512 - D_COL0) / D_COLS, 2, 4);   // accumulator ring depth (MMA -> epilogue), one slot per link matrix
     static constexpr int TMEM_COLS = 512;
     static constexpr int NG = 3;                        // converter groups of 4 warps (stage t -> group t mod NG)
     static constexpr int CONV_W0 = 2;                   // warps: 0 producer, 1 MMA issuer, 2 .. 2+4NG-1 converters, then 4 epilogue
@@ -191,6 +199,7 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
     using Gm = TensorGeom<NC, I16, NP>;
     static_assert(Gm::OK, "unsupported TENSOR geometry");
     constexpr int LS = Gm::LS, AS = Gm::AS, DS = Gm::DS, CHUNKS = Gm::CHUNKS, N = Gm::N, NT = Gm::NT, MT = Gm::MT, NE = Gm::NE;
+    constexpr int NS = Gm::NS, SLAB_BYTES = Gm::SLAB_BYTES, SLAB_PITCH = Gm::SLAB_PITCH;
     constexpr int LINK_STAGE = Gm::LINK_STAGE, B_HALF = Gm::B_HALF, B_SBO = Gm::B_SBO, ENTRY = Gm::ENTRY;
     // instruction descriptor: D fp32, A/B tf32, both K-major, N, M = 128
     constexpr uint32_t IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
@@ -231,12 +240,16 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-    const int n_items = p.n_sites * NT;
+    const int n_items = NS == 2 ? (p.n_sites + 1) / 2 : p.n_sites * NT;
     const int n_my = (n_items > (int)blockIdx.x) ? (n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
     const int M0 = p.m_begin;
     const int n_mat_item = 9 - M0;                                   // link matrices per item
-    auto site_of_item = [&](int item) -> int {
-        const int h = (NT == 1 ? item : item / NT) + p.site_begin;
+    // site sg (0 | 1) of a work item; an odd site count leaves the last item's second half without a site: it
+    // re-computes the first one (valid memory, constant byte counts) and does not store
+    auto site_valid = [&](int item, int sg) -> bool { return NS == 1 || 2 * item + sg < p.n_sites; };
+    auto site_of_item = [&](int item, int sg = 0) -> int {
+        int h = NS == 2 ? 2 * item + (site_valid(item, sg) ? sg : 0) : (NT == 1 ? item : item / NT);
+        h += p.site_begin;
         return p.parity != 2 ? parity_site(p.lat, h, p.parity) : h;
     };
 
@@ -247,27 +260,38 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
         uint32_t t = 0;
         for (int it = 0; it < n_my; ++it) {
             const int item = blockIdx.x + it * gridDim.x;
-            const int s = site_of_item(item);
             const int i0 = NT == 1 ? 0 : (item % NT) * MT;
-            const SiteX cx = site_coords(p.lat, s);
+            int s[NS];
+            SiteX cx[NS];
+#pragma unroll
+            for (int sg = 0; sg < NS; ++sg) {
+                s[sg] = site_of_item(item, sg);
+                cx[sg] = site_coords(p.lat, s[sg]);
+            }
 #pragma unroll
             for (int m = 0; m < 9; ++m) {
                 if (m < M0) continue;
-                const int sv = stencil_site_x(p.lat, s, cx, m, DAG ? 1 : 0);
-                const int sm = DAG ? sv : s;
-                const int mat_row0 = (sm * 9 + m) * NC;             // < 2^31: checked by the host (make_link_maps)
+                int mat_row0[NS];
+#pragma unroll
+                for (int sg = 0; sg < NS; ++sg) {
+                    const int sv = stencil_site_x(p.lat, s[sg], cx[sg], m, DAG ? 1 : 0);
+                    const int sm = DAG ? sv : s[sg];
+                    mat_row0[sg] = (sm * 9 + m) * NC;               // < 2^31: checked by the host (make_link_maps)
+                }
 #pragma unroll 1
                 for (int c = 0; c < CHUNKS; ++c, ++t) {
                     const uint32_t slot = t % LS, ph = (t / LS) & 1u;
                     ptx::mbar_wait(empty0 + 8u * slot, ph ^ 1u);
                     if (ptx::elect_one()) {
-                        ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE);
-                        if (!DAG)      // rows [i0, i0 + MT) x complex columns [16c, 16c + 16)
-                            ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, c * (16 * ENTRY / 4), mat_row0 + i0,
-                                             full0 + 8u * slot, pol_links);
-                        else           // rows [16c, 16c + 16) x complex columns [i0, i0 + MT)
-                            ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, i0 * (ENTRY / 4), mat_row0 + 16 * c,
-                                             full0 + 8u * slot, pol_links);
+                        ptx::mbar_arrive_expect_tx(full0 + 8u * slot, NS * SLAB_BYTES);
+#pragma unroll
+                        for (int sg = 0; sg < NS; ++sg) {
+                            const uint32_t dst = link_u32 + slot * LINK_STAGE + sg * SLAB_PITCH;
+                            if (!DAG)      // rows [i0, i0 + MT) x complex columns [16c, 16c + 16)
+                                ptx::tma_load_2d(dst, &link_map, c * (16 * ENTRY / 4), mat_row0[sg] + i0, full0 + 8u * slot, pol_links);
+                            else           // rows [16c, 16c + 16) x complex columns [i0, i0 + MT)
+                                ptx::tma_load_2d(dst, &link_map, i0 * (ENTRY / 4), mat_row0[sg] + 16 * c, full0 + 8u * slot, pol_links);
+                        }
                     }
                     __syncwarp();
                 }
@@ -322,7 +346,9 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
         constexpr int NG = Gm::NG;
         const int grp = (warp - Gm::CONV_W0) >> 2;    // stages t with t % NG == grp
         const int q = warp & 3;                       // TMEM lane quadrant of this warp (hardware: warp id mod 4)
-        const int row = q * 32 + lane;                // A-operand row = output index i (inside the item's tile)
+        const int lane_row = q * 32 + lane;           // TMEM lane
+        const int sg_row = NS == 2 ? lane_row >> 6 : 0;               // which site of the item this lane serves
+        const int row = NS == 2 ? lane_row & 63 : lane_row;           // A-operand row = output index i of that site
         const int gtid = ((warp - Gm::CONV_W0) & 3) * 32 + lane;      // 0..127 inside the group
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         const uint32_t total = (uint32_t)n_my * (uint32_t)(n_mat_item * CHUNKS);
@@ -331,47 +357,63 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
         // covers the 16 distinct 8-byte bank slots (k mod 4 pair, n mod 8) of the K-major layout, so its
         // stores are conflict-free (e = gtid + 128 x: r = e & 7 [+ 8], j = 2 (e >> 4 [>> 1]) + ((e >> 3) & 1)).
         int b_off_vec[NE];           // element offset inside the stage's 16 x nrhs block
+        int b_sg[NE];                // site of the item the entry belongs to
         uint32_t b_o1[NE], b_o2[NE]; // byte offsets of the (n = r) and (n = NP + r) entries in the B tile
         bool b_valid[NE];
 #pragma unroll
         for (int x = 0; x < NE; ++x) {
             const int e = gtid + 128 * x;
-            const int rest = e >> 4;
-            const int r = (e & 7) + (NP == 16 ? (rest & 1) * 8 : 0);
-            const int j = 2 * (NP == 16 ? rest >> 1 : rest) + ((e >> 3) & 1);
+            int rest = e >> 4;
+            int r = e & 7;
+            if (NP == 16) { r += (rest & 1) * 8; rest >>= 1; }
+            int sg = 0;
+            if (NS == 2) { sg = rest & 1; rest >>= 1; }
+            const int j = 2 * rest + ((e >> 3) & 1);
             b_valid[x] = r < p.width;
+            b_sg[x] = sg;
             b_off_vec[x] = j * p.nrhs + r;
             const uint32_t koff = (uint32_t)(j >> 1) * 128u + (uint32_t)(j & 1) * 8u;
-            b_o1[x] = koff + (uint32_t)(r >> 3) * B_SBO + (uint32_t)(r & 7) * 16u;
-            b_o2[x] = koff + (uint32_t)((NP + r) >> 3) * B_SBO + (uint32_t)((NP + r) & 7) * 16u;
+            const int n1 = sg * 2 * NP + r, n2 = n1 + NP;
+            b_o1[x] = koff + (uint32_t)(n1 >> 3) * B_SBO + (uint32_t)(n1 & 7) * 16u;
+            b_o2[x] = koff + (uint32_t)(n2 >> 3) * B_SBO + (uint32_t)(n2 & 7) * 16u;
         }
 
         // cursor of the NEXT stage of this group (its vector entries are prefetched while the current
         // stage is converted): item index, matrix, chunk, and what depends on them
-        int n_it = 0, n_m = M0, n_c = grp, n_s = 0;     // stage t = grp: chunk grp of the first matrix (normalised below)
-        SiteX n_cx = {};
-        const float2* n_vec = p.in;
-        float n_sc = 1.f;
+        int n_it = 0, n_m = M0, n_c = grp;              // stage t = grp: chunk grp of the first matrix (normalised below)
+        int n_s[NS];
+        SiteX n_cx[NS];
+        const float2* n_vec[NS];
+        float n_sc[NS];
+#pragma unroll
+        for (int sg = 0; sg < NS; ++sg) { n_s[sg] = 0; n_cx[sg] = SiteX{}; n_vec[sg] = p.in; n_sc[sg] = 1.f; }
         auto load_item = [&]() {
             if (n_it < n_my) {
-                n_s = site_of_item(blockIdx.x + n_it * gridDim.x);
-                n_cx = site_coords(p.lat, n_s);
+#pragma unroll
+                for (int sg = 0; sg < NS; ++sg) {
+                    n_s[sg] = site_of_item(blockIdx.x + n_it * gridDim.x, sg);
+                    n_cx[sg] = site_coords(p.lat, n_s[sg]);
+                }
             }
         };
         auto load_matrix = [&]() {
             if (n_it < n_my) {
-                const int sv = stencil_site_x(p.lat, n_s, n_cx, n_m, DAG ? 1 : 0);
-                const int sm = DAG ? sv : n_s;
-                n_vec = (n_m == 0 ? p.in_local : p.in) + (int64_t)sv * NC * p.nrhs + p.r0;
-                n_sc = n_m == 0 ? p.alpha : p.beta;
-                if constexpr (I16) n_sc *= __ldg(p.scales + (int64_t)sm * 9 + n_m);
+#pragma unroll
+                for (int sg = 0; sg < NS; ++sg) {
+                    const int sv = stencil_site_x(p.lat, n_s[sg], n_cx[sg], n_m, DAG ? 1 : 0);
+                    const int sm = DAG ? sv : n_s[sg];
+                    n_vec[sg] = (n_m == 0 ? p.in_local : p.in) + (int64_t)sv * NC * p.nrhs + p.r0;
+                    n_sc[sg] = n_m == 0 ? p.alpha : p.beta;
+                    if constexpr (I16) n_sc[sg] *= __ldg(p.scales + (int64_t)sm * 9 + n_m);
+                }
             }
         };
         float2 vn[NE];
         auto fetch = [&]() {
 #pragma unroll
             for (int x = 0; x < NE; ++x)
-                vn[x] = (n_it < n_my && b_valid[x]) ? __ldg(n_vec + (int64_t)(16 * n_c) * p.nrhs + b_off_vec[x]) : make_float2(0.f, 0.f);
+                vn[x] = (n_it < n_my && b_valid[x]) ? __ldg(n_vec[NS == 2 ? b_sg[x] : 0] + (int64_t)(16 * n_c) * p.nrhs + b_off_vec[x])
+                                                    : make_float2(0.f, 0.f);
         };
         auto normalise = [&]() -> bool {               // carry n_c into (n_m, n_it); true if the item changed
             bool item_changed = false;
@@ -393,7 +435,9 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
             float2 v[NE];
 #pragma unroll
             for (int x = 0; x < NE; ++x) v[x] = vn[x];
-            const float sc = n_sc;
+            float sc[NS];
+#pragma unroll
+            for (int sg = 0; sg < NS; ++sg) sc[sg] = n_sc[sg];
             n_c += NG;
             if (n_c >= CHUNKS) {
                 if (normalise()) load_item();
@@ -404,7 +448,7 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
             ptx::mbar_wait(full0 + 8u * slot, ph);
             float a[32];
             if (row < MT) {
-                const uint32_t sb = link_u32 + slot * LINK_STAGE;
+                const uint32_t sb = link_u32 + slot * LINK_STAGE + sg_row * SLAB_PITCH;
                 if constexpr (!DAG && !I16) {
                     const uint32_t rb = sb + row * 128;            // SWIZZLE_128B: chunk u of row at u ^ (row & 7)
 #pragma unroll
@@ -456,7 +500,8 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
 #pragma unroll
             for (int x = 0; x < NE; ++x) {
                 // k = 2j, 2j+1 -> one 8-byte store; n = r (-> Re out) and n = NP + r (-> Im out)
-                const float vx = v[x].x * sc, vy = v[x].y * sc;
+                const float scx = sc[NS == 2 ? b_sg[x] : 0];
+                const float vx = v[x].x * scx, vy = v[x].y * scx;
                 const float b1x = vx, b1y = DAG ? vy : -vy;
                 const float b2x = vy, b2y = DAG ? -vx : vx;
                 uint32_t h0, l0, h1, l1;
@@ -481,25 +526,29 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
     } else if (warp >= Gm::EPI_W0) {
         // ---------------------------------------------------------------- epilogue
         const int q = warp & 3;
-        const int row = q * 32 + lane;
+        const int lane_row = q * 32 + lane;
+        const int sg_row = NS == 2 ? lane_row >> 6 : 0;       // site of the item this lane's row belongs to (warp-uniform)
+        const int row = NS == 2 ? lane_row & 63 : lane_row;
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
+        constexpr int NA = 2 * NP;                             // accumulators of a row: [Re out | Im out] of ITS site
         uint32_t tm = 0;
         for (int it = 0; it < n_my; ++it) {
             const int item = blockIdx.x + it * gridDim.x;
-            const int s = site_of_item(item);
+            const int s = site_of_item(item, sg_row);
             const int i0 = NT == 1 ? 0 : (item % NT) * MT;
-            float acc[N];
+            float acc[NA];
 #pragma unroll
-            for (int n = 0; n < N; ++n) acc[n] = 0.f;
+            for (int n = 0; n < NA; ++n) acc[n] = 0.f;
 #pragma unroll 1
             for (int m = M0; m < 9; ++m, ++tm) {
                 const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
                 ptx::mbar_wait(dfull0 + 8u * ds, dph);
                 ptx::tc_fence_after();
-                const uint32_t d_tmem = tmem_base + lane_addr + Gm::D_COL0 + ds * Gm::D_COLS;
+                // this row's site: columns [sg NA, sg NA + NA) of the main chain and of the cross-term chain
+                const uint32_t d_tmem = tmem_base + lane_addr + Gm::D_COL0 + ds * Gm::D_COLS + sg_row * NA;
                 // 16 columns of the main chain and the matching 16 of the cross-term chain at a time
 #pragma unroll
-                for (int c = 0; c < N / 16; ++c) {
+                for (int c = 0; c < NA / 16; ++c) {
                     uint32_t dm[16], dx[16];
                     ptx::tmem_ld16(d_tmem + 16 * c, dm);
                     ptx::tmem_ld16(d_tmem + N + 16 * c, dx);
@@ -511,7 +560,7 @@ coarse_apply_tensor(const __grid_constant__ CUtensorMap link_map, TensorParams p
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(dempty0 + 8u * ds);
             }
-            if (row < MT) {
+            if (row < MT && site_valid(item, sg_row)) {
                 const int64_t o = ((int64_t)s * NC + i0 + row) * p.nrhs + p.r0;
                 if (p.identity) {
 #pragma unroll
