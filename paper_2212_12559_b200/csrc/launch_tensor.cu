@@ -42,7 +42,8 @@ int launch_tensor_i8_t(const coarse_op* op, const TensorI8Params& p, cudaStream_
     cudaError_t e = ensure_dynamic_smem(kern, op->device, Gm::SMEM_BYTES, attr_cache);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(tensor-i8 kernel)");
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
-    if (grid > p.t.n_sites * Gm::NT) grid = p.t.n_sites * Gm::NT;
+    const int n_items = Gm::NS == 2 ? (p.t.n_sites + 1) / 2 : p.t.n_sites * Gm::NT;
+    if (grid > n_items) grid = n_items;
     if (grid < 1) return COARSE_OK;
     kern<<<grid, Gm::THREADS, Gm::SMEM_BYTES, stream>>>(op->link_map_i8[DAG ? 1 : 0], p);
     e = cudaGetLastError();

@@ -54,24 +54,31 @@ struct TensorI8Geom {
     static constexpr int KC = (NC % 32 == 0) ? 32 : 16;       // complex columns per stage
     static constexpr int CHUNKS = NC / KC;                     // stages per link matrix
     static constexpr int KSTEPS = KC / 16;                     // MMA k-steps (K = 32 int8 = 16 complex columns)
-    static constexpr int LINK_STAGE = MT * KC * 4;
-    static constexpr int NB3 = 3 * 2 * NP;                     // MMA N: three digit blocks of [Re out | Im out]
+    // Two sites per work item when the matrices have at most 64 rows and the 8-wide column tile is in use (the
+    // accumulator ring of the 16-wide tile would not fit tensor memory): site 0 in TMEM lanes 0.., site 1 in lanes
+    // 64.., their B operands side by side along N inside every digit block (see TensorGeom::NS in tensor_kernel.cuh).
+    static constexpr int NS = (MT <= 64 && NP == 8) ? 2 : 1;
+    static constexpr int NPS = NP * NS;                        // right-hand-side columns of an item (all its sites)
+    static constexpr int SLAB_BYTES = MT * KC * 4;             // one site's slab of a stage
+    static constexpr int SLAB_PITCH = NS == 2 ? 64 * KC * 4 : SLAB_BYTES;
+    static constexpr int LINK_STAGE = NS * SLAB_PITCH;
+    static constexpr int NB3 = 3 * 2 * NPS;                    // MMA N: three digit blocks of (per site) [Re out | Im out]
     static constexpr int B_STAGE = 2 * KC * NB3;               // int8 B tile of a stage, bytes
     static constexpr int B_SBO = (2 * KC / 16) * 128;          // byte stride between 8-column groups of n
-    static constexpr int NE = KC * NP / 128;                   // B entries per converter thread and stage
+    static constexpr int NE = KC * NPS / 128;                  // B entries per converter thread and stage
     static constexpr int LS = tensor_clamp(COARSE_TENSOR_RING_BYTES / LINK_STAGE, 4, 20);
     static constexpr int AS = 4;
     static constexpr int A_HALF = KC / 2;                      // TMEM columns of one byte plane (4 int8 per column)
     static constexpr int A_COLS = 2 * A_HALF;                  // high bytes | low bytes
     static constexpr int D_COL0 = AS * A_COLS;
     static constexpr int DS = 3;
-    static constexpr int D_COLS = 4 * 2 * NP;                  // W_0 .. W_3, each [Re out | Im out]
+    static constexpr int D_COLS = 4 * 2 * NPS;                 // W_0 .. W_3, each (per site) [Re out | Im out]
     static constexpr int FT = 8;                               // ring of per-matrix epilogue factor rows
     static constexpr int TMEM_COLS = 512;
     static constexpr int NG = COARSE_I8_NG, CONV_W0 = 2, EPI_W0 = CONV_W0 + 4 * NG;
     static constexpr int THREADS = (EPI_W0 + 4) * 32;
     static constexpr int NBAR = 2 * LS + 2 * AS + 2 * DS;
-    static constexpr int SMEM_BYTES = 1024 + LS * LINK_STAGE + AS * B_STAGE + FT * NP * 4 + NBAR * 8 + 16;
+    static constexpr int SMEM_BYTES = 1024 + LS * LINK_STAGE + AS * B_STAGE + FT * NPS * 4 + NBAR * 8 + 16;
     static constexpr bool OK = (NC % 16 == 0) && (MT % 8 == 0) && MT <= 128 && (NP == 8 || NP == 16) && NE >= 1 &&
                                (D_COL0 + DS * D_COLS <= TMEM_COLS) && SMEM_BYTES <= 232448 && 2 * NC * 128 * 255 < (1 << 24);
 };
@@ -151,11 +158,12 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
     static_assert(Gm::OK, "unsupported TENSOR-I8 geometry");
     constexpr int LS = Gm::LS, AS = Gm::AS, DS = Gm::DS, CHUNKS = Gm::CHUNKS, NT = Gm::NT, MT = Gm::MT, NE = Gm::NE;
     constexpr int KC = Gm::KC, LINK_STAGE = Gm::LINK_STAGE, B_STAGE = Gm::B_STAGE, B_SBO = Gm::B_SBO, NB3 = Gm::NB3, FT = Gm::FT;
+    constexpr int NS = Gm::NS, NPS = Gm::NPS, SLAB_BYTES = Gm::SLAB_BYTES, SLAB_PITCH = Gm::SLAB_PITCH;
     // instruction descriptors: D int32 (c_format 2), A signed | unsigned 8 bit, B signed 8 bit, K-major, N = NB3, M = 128
     constexpr uint32_t IDESC_S = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NB3 >> 3) << 17) | ((128u >> 4) << 24);
     constexpr uint32_t IDESC_U = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(NB3 >> 3) << 17) | ((128u >> 4) << 24);
-    constexpr uint32_t IDESC_U1 = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(2 * NP >> 3) << 17) | ((128u >> 4) << 24);   // one digit block
-    constexpr uint32_t IDESC_U2 = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(4 * NP >> 3) << 17) | ((128u >> 4) << 24);   // two digit blocks
+    constexpr uint32_t IDESC_U1 = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(2 * NPS >> 3) << 17) | ((128u >> 4) << 24);   // one digit block
+    constexpr uint32_t IDESC_U2 = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(4 * NPS >> 3) << 17) | ((128u >> 4) << 24);   // two digit blocks
     const TensorParams& p = pp.t;
 
     extern __shared__ unsigned char smem_raw[];
@@ -163,7 +171,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
     const uint32_t link_u32 = base;
     const uint32_t b_u32 = link_u32 + LS * LINK_STAGE;
     const uint32_t ft_u32 = b_u32 + AS * B_STAGE;
-    const uint32_t bar_u32 = ft_u32 + FT * NP * 4;
+    const uint32_t bar_u32 = ft_u32 + FT * NPS * 4;
     const uint32_t full0 = bar_u32, empty0 = full0 + 8u * LS;
     const uint32_t abfull0 = empty0 + 8u * LS, abempty0 = abfull0 + 8u * AS;
     const uint32_t dfull0 = abempty0 + 8u * AS, dempty0 = dfull0 + 8u * DS;
@@ -193,12 +201,16 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-    const int n_items = p.n_sites * NT;
+    const int n_items = NS == 2 ? (p.n_sites + 1) / 2 : p.n_sites * NT;
     const int n_my = (n_items > (int)blockIdx.x) ? (n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
     const int M0 = p.m_begin;
     const int n_mat_item = 9 - M0;
-    auto site_of_item = [&](int item) -> int {
-        const int h = (NT == 1 ? item : item / NT) + p.site_begin;
+    // site sg (0 | 1) of a work item; the second half of the last item of an odd site count re-computes the first
+    // site (valid memory, constant byte counts) and does not store
+    auto site_valid = [&](int item, int sg) -> bool { return NS == 1 || 2 * item + sg < p.n_sites; };
+    auto site_of_item = [&](int item, int sg = 0) -> int {
+        int h = NS == 2 ? 2 * item + (site_valid(item, sg) ? sg : 0) : (NT == 1 ? item : item / NT);
+        h += p.site_begin;
         return p.parity != 2 ? parity_site(p.lat, h, p.parity) : h;
     };
 
@@ -208,25 +220,38 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
         uint32_t t = 0;
         for (int it = 0; it < n_my; ++it) {
             const int item = blockIdx.x + it * gridDim.x;
-            const int s = site_of_item(item);
             const int i0 = NT == 1 ? 0 : (item % NT) * MT;
-            const SiteX cx = site_coords(p.lat, s);
+            int s[NS];
+            SiteX cx[NS];
+#pragma unroll
+            for (int sg = 0; sg < NS; ++sg) {
+                s[sg] = site_of_item(item, sg);
+                cx[sg] = site_coords(p.lat, s[sg]);
+            }
 #pragma unroll
             for (int m = 0; m < 9; ++m) {
                 if (m < M0) continue;
-                const int sv = stencil_site_x(p.lat, s, cx, m, DAG ? 1 : 0);
-                const int sm = DAG ? sv : s;
-                const int mat_row0 = (sm * 9 + m) * NC;
+                int mat_row0[NS];
+#pragma unroll
+                for (int sg = 0; sg < NS; ++sg) {
+                    const int sv = stencil_site_x(p.lat, s[sg], cx[sg], m, DAG ? 1 : 0);
+                    const int sm = DAG ? sv : s[sg];
+                    mat_row0[sg] = (sm * 9 + m) * NC;
+                }
 #pragma unroll 1
                 for (int c = 0; c < CHUNKS; ++c, ++t) {
                     const uint32_t slot = t % LS, ph = (t / LS) & 1u;
                     ptx::mbar_wait(empty0 + 8u * slot, ph ^ 1u);
                     if (ptx::elect_one()) {
-                        ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE);
-                        if (!DAG)      // rows [i0, i0 + MT) x complex columns [KC c, KC c + KC)
-                            ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, c * KC, mat_row0 + i0, full0 + 8u * slot, pol_links);
-                        else           // rows [KC c, KC c + KC) x complex columns [i0, i0 + MT)
-                            ptx::tma_load_2d(link_u32 + slot * LINK_STAGE, &link_map, i0, mat_row0 + KC * c, full0 + 8u * slot, pol_links);
+                        ptx::mbar_arrive_expect_tx(full0 + 8u * slot, NS * SLAB_BYTES);
+#pragma unroll
+                        for (int sg = 0; sg < NS; ++sg) {
+                            const uint32_t dst = link_u32 + slot * LINK_STAGE + sg * SLAB_PITCH;
+                            if (!DAG)      // rows [i0, i0 + MT) x complex columns [KC c, KC c + KC)
+                                ptx::tma_load_2d(dst, &link_map, c * KC, mat_row0[sg] + i0, full0 + 8u * slot, pol_links);
+                            else           // rows [KC c, KC c + KC) x complex columns [i0, i0 + MT)
+                                ptx::tma_load_2d(dst, &link_map, i0, mat_row0[sg] + KC * c, full0 + 8u * slot, pol_links);
+                        }
                     }
                     __syncwarp();
                 }
@@ -241,7 +266,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
             ptx::mbar_wait(dempty0 + 8u * ds, dph ^ 1u);
             ptx::tc_fence_after();
             // high-byte plane one digit block above the low-byte plane: equal weights share columns
-            const uint32_t d0 = tmem_base + Gm::D_COL0 + ds * Gm::D_COLS, d1 = d0 + 2 * NP;
+            const uint32_t d0 = tmem_base + Gm::D_COL0 + ds * Gm::D_COLS, d1 = d0 + 2 * NPS;
 #pragma unroll 1
             for (int c = 0; c < CHUNKS; ++c, ++t) {
                 const uint32_t as = t % AS, aph = (t / AS) & 1u;
@@ -258,7 +283,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                             // (overwrite), W_1, W_2 += low plane digits 1, 2
                             ptx::mma_i8_ts(d1, a1, db, IDESC_S, 0u);
                             ptx::mma_i8_ts(d0, a0, db, IDESC_U1, 0u);
-                            ptx::mma_i8_ts(d1, a0, db + (uint64_t)((2 * (NP >> 3) * B_SBO) >> 4), IDESC_U2, 1u);
+                            ptx::mma_i8_ts(d1, a0, db + (uint64_t)((2 * (NPS >> 3) * B_SBO) >> 4), IDESC_U2, 1u);
                         } else {
                             ptx::mma_i8_ts(d1, a1 + kk * 8, db, IDESC_S, 1u);
                             ptx::mma_i8_ts(d0, a0 + kk * 8, db, IDESC_U, 1u);
@@ -275,28 +300,33 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
         constexpr int NG = Gm::NG;
         const int grp = (warp - Gm::CONV_W0) >> 2;
         const int q = warp & 3;
-        const int row = q * 32 + lane;
+        const int lane_row = q * 32 + lane;                           // TMEM lane
+        const int sg_row = NS == 2 ? lane_row >> 6 : 0;               // site of the item whose matrix row this lane converts
+        const int row = NS == 2 ? lane_row & 63 : lane_row;
         const int gtid = ((warp - Gm::CONV_W0) & 3) * 32 + lane;
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         const uint32_t total = (uint32_t)n_my * (uint32_t)(n_mat_item * CHUNKS);
 
         // B entries of this thread: contraction row j (of the stage's KC) and column r, the same in every stage;
         // every entry of a thread has the same r.  e = gtid + 128 x: bits 0-2 = r mod 8 (16-byte rows of the K-major
-        // layout: banks 4 apart), bits 3-4 = j mod 4 (bytes 2 apart / next word), bit 5 = r div 8 (NP = 16), rest = j div 4:
+        // layout: banks 4 apart), bits 3-4 = j mod 4 (bytes 2 apart / next word), bit 5 = r div 8 (NP = 16) or the site sg (two sites per item), rest = j div 4:
         // the 32 lanes of a 16-bit store touch 16 distinct words in 16 distinct banks (conflict-free).
         const int my_r = (gtid & 7) + (NP == 16 ? ((gtid >> 5) & 1) * 8 : 0);
+        const int my_sg = NS == 2 ? (gtid >> 5) & 1 : 0;              // every B entry of a thread belongs to ONE site of the item
+        const int my_n = my_sg * 2 * NP + my_r;                       // column inside a digit block
         const bool r_valid = my_r < p.width;
         int b_off_vec[NE];
         uint32_t b_o[NE];              // byte offset of (k = 2j, n = r, digit 0) in the B tile
 #pragma unroll
         for (int x = 0; x < NE; ++x) {
             const int e = gtid + 128 * x;
-            const int j = ((e >> 3) & 3) + 4 * (e >> (NP == 16 ? 6 : 5));
+            const int j = ((e >> 3) & 3) + 4 * (e >> (NPS == 16 ? 6 : 5));
             b_off_vec[x] = j * p.nrhs + my_r;
             const int k = 2 * j;
-            b_o[x] = (uint32_t)(k >> 4) * 128u + (uint32_t)(my_r >> 3) * B_SBO + (uint32_t)(my_r & 7) * 16u + (uint32_t)(k & 15);
+            b_o[x] = (uint32_t)(k >> 4) * 128u + (uint32_t)(my_n >> 3) * B_SBO + (uint32_t)(my_n & 7) * 16u + (uint32_t)(k & 15);
         }
         constexpr uint32_t N_STEP = (uint32_t)(NP >> 3) * B_SBO;     // byte step of NP columns of n (NP is a multiple of 8)
+        constexpr uint32_t D_STEP = 2 * NS * N_STEP;                 // byte step of one digit block
 
         int n_it = 0, n_m = M0, n_c = grp, n_s = 0;
         SiteX n_cx = {};
@@ -304,7 +334,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
         float n_g = 0.f, n_f = 0.f;       // fixed-point scale g 2^22 of the operand, epilogue factor of the matrix
         auto load_item = [&]() {
             if (n_it < n_my) {
-                n_s = site_of_item(blockIdx.x + n_it * gridDim.x);
+                n_s = site_of_item(blockIdx.x + n_it * gridDim.x, my_sg);
                 n_cx = site_coords(p.lat, n_s);
             }
         };
@@ -356,7 +386,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
             ptx::mbar_wait(full0 + 8u * slot, ph);
             uint32_t w[KC];                                   // the lane's KC link entries (re, im) int16
             if (row < MT) {
-                const uint32_t sb = link_u32 + slot * LINK_STAGE;
+                const uint32_t sb = link_u32 + slot * LINK_STAGE + sg_row * SLAB_PITCH;
                 if constexpr (!DAG) {
                     const uint32_t rb = sb + row * (KC * 4);
 #pragma unroll
@@ -403,18 +433,18 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                 digit_regs(b1x, x1, x2);
                 digit_regs(b1y, y1, y2);
                 ptx::sts16(bt + b_o[x], pack_lo_bytes(b1x, b1y));
-                ptx::sts16(bt + b_o[x] + 2 * N_STEP, pack_lo_bytes(x1, y1));
-                ptx::sts16(bt + b_o[x] + 4 * N_STEP, pack_lo_bytes(x2, y2));
+                ptx::sts16(bt + b_o[x] + D_STEP, pack_lo_bytes(x1, y1));
+                ptx::sts16(bt + b_o[x] + 2 * D_STEP, pack_lo_bytes(x2, y2));
                 digit_regs(b2x, x1, x2);
                 digit_regs(b2y, y1, y2);
                 ptx::sts16(bt + b_o[x] + N_STEP, pack_lo_bytes(b2x, b2y));
-                ptx::sts16(bt + b_o[x] + 3 * N_STEP, pack_lo_bytes(x1, y1));
-                ptx::sts16(bt + b_o[x] + 5 * N_STEP, pack_lo_bytes(x2, y2));
+                ptx::sts16(bt + b_o[x] + N_STEP + D_STEP, pack_lo_bytes(x1, y1));
+                ptx::sts16(bt + b_o[x] + N_STEP + 2 * D_STEP, pack_lo_bytes(x2, y2));
             }
             // epilogue factor of this matrix and column: written by the group that converts the matrix's first chunk
             if (first_chunk && (gtid & 0x18) == 0 && gtid < 64) {
-                // threads 0-7 (and 32-39 for NP = 16) of the group hold r = 0..7 (8..15)
-                asm volatile("st.shared.f32 [%0], %1;" ::"r"(ft_u32 + (uint32_t)(((t / CHUNKS) % FT) * NP + my_r) * 4u), "f"(f) : "memory");
+                // threads 0-7 (and 32-39 for NP = 16 / the second site) of the group hold r = 0..7 (8..15 / r = 0..7 of site 1)
+                asm volatile("st.shared.f32 [%0], %1;" ::"r"(ft_u32 + (uint32_t)(((t / CHUNKS) % FT) * NPS + my_sg * NP + my_r) * 4u), "f"(f) : "memory");
             }
             ptx::tc_wait_st();
             ptx::fence_proxy_async();
@@ -427,12 +457,14 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
     } else if (warp >= Gm::EPI_W0) {
         // ---------------------------------------------------------------- epilogue
         const int q = warp & 3;
-        const int row = q * 32 + lane;
+        const int lane_row = q * 32 + lane;
+        const int sg_row = NS == 2 ? lane_row >> 6 : 0;               // warp-uniform
+        const int row = NS == 2 ? lane_row & 63 : lane_row;
         const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
         uint32_t tm = 0;
         for (int it = 0; it < n_my; ++it) {
             const int item = blockIdx.x + it * gridDim.x;
-            const int s = site_of_item(item);
+            const int s = site_of_item(item, sg_row);
             const int i0 = NT == 1 ? 0 : (item % NT) * MT;
             float acc[2 * NP];
 #pragma unroll
@@ -442,15 +474,15 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                 const uint32_t ds = tm % DS, dph = (tm / DS) & 1u;
                 ptx::mbar_wait(dfull0 + 8u * ds, dph);
                 ptx::tc_fence_after();
-                const uint32_t d_t = tmem_base + lane_addr + Gm::D_COL0 + ds * Gm::D_COLS;
-                const uint32_t ft = ft_u32 + (uint32_t)((tm % FT) * NP) * 4u;
+                const uint32_t d_t = tmem_base + lane_addr + Gm::D_COL0 + ds * Gm::D_COLS + sg_row * 2 * NP;   // this row's site
+                const uint32_t ft = ft_u32 + (uint32_t)((tm % FT) * NPS + sg_row * NP) * 4u;
                 // 8 columns of n at a time: the four weight blocks W_3 .. W_0, Horner in fp32
 #pragma unroll
                 for (int pc = 0; pc < 2 * NP / 8; ++pc) {
                     uint32_t w3[8], w2[8], w1[8], w0[8];
-                    ptx::tmem_ld8(d_t + 3 * 2 * NP + 8 * pc, w3);
-                    ptx::tmem_ld8(d_t + 2 * 2 * NP + 8 * pc, w2);
-                    ptx::tmem_ld8(d_t + 1 * 2 * NP + 8 * pc, w1);
+                    ptx::tmem_ld8(d_t + 3 * 2 * NPS + 8 * pc, w3);
+                    ptx::tmem_ld8(d_t + 2 * 2 * NPS + 8 * pc, w2);
+                    ptx::tmem_ld8(d_t + 1 * 2 * NPS + 8 * pc, w1);
                     ptx::tmem_ld8(d_t + 8 * pc, w0);
                     ptx::tc_wait_ld();
 #pragma unroll
@@ -467,7 +499,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive(dempty0 + 8u * ds);
             }
-            if (row < MT) {
+            if (row < MT && site_valid(item, sg_row)) {
                 const int64_t o = ((int64_t)s * NC + i0 + row) * p.nrhs + p.r0;
                 if (p.identity) {
 #pragma unroll
