@@ -232,16 +232,20 @@ int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int 
     return COARSE_OK;
 }
 
-// COARSE_PATH_AUTO.  1 RHS: STREAM.  2-4 RHS: STREAM-MR, except int16 links with Nc >= 96, where the integer
-// tensor-core kernel is faster (measured, 3 RHS: Nc = 128 0.58 / 0.55 ms against 0.74 / 0.65 ms; Nc = 64 the
-// other way round, 4.6 against 2.9 / 3.0 ms: small matrices make small pipeline stages).  5 and more: TENSOR
-// (BLOCK only on request, or when no tensor map could be made), outside the compiled Nc: SIMPLE.
+// COARSE_PATH_AUTO.  1 RHS: STREAM.  2-4 RHS: STREAM-MR, except int16 links where the integer tensor-core kernel
+// is faster - from 2 RHS for Nc >= 96 and Nc = 32, from 3 for Nc = 64, at 4 for Nc = 48 (measured ms, dagger 0 / 1,
+// HBM-sized lattices, STREAM-MR against TENSOR: Nc = 128, 3 RHS 0.74 / 0.65 against 0.58 / 0.55; Nc = 64, 3 RHS 3.11 / 3.05
+// against 2.97 / 2.94, 4 RHS 4.47 / 4.17 against 3.04 / 3.00, 2 RHS 2.93 / 2.56 against 2.93 / 2.89; Nc = 48, 3 RHS 2.57 /
+// 2.63 against 3.30 / 3.33, 4 RHS 3.59 / 4.63 against 3.33 / 3.34; Nc = 32, 2 RHS 4.35 / 2.95 against 2.82 / 2.92).  5 and
+// more: TENSOR (BLOCK only on request, or when no tensor map could be made), outside the compiled Nc: SIMPLE.
+int tensor_i8_min_nrhs(int Nc) { return Nc >= 96 ? 2 : Nc == 64 ? 3 : Nc == 48 ? 4 : 2; }
+
 int auto_path(const coarse_op* op, int nrhs) {
     const bool tensor_ok = tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok;
     if (stream_supports(op->Nc, nrhs)) return COARSE_PATH_STREAM;
     if (stream_mr_supports(op->Nc, nrhs)) {
         const bool i8 = op->prec == COARSE_LINK_I16 && op->link_map_i8_ok && op->vscale && op->tensor_i8_opt != 1;
-        return (tensor_ok && i8 && op->Nc >= 96) ? COARSE_PATH_TENSOR : COARSE_PATH_STREAM;
+        return (tensor_ok && i8 && nrhs >= tensor_i8_min_nrhs(op->Nc)) ? COARSE_PATH_TENSOR : COARSE_PATH_STREAM;
     }
     if (tensor_ok) return COARSE_PATH_TENSOR;
     if (block_supports(op->Nc, nrhs)) return COARSE_PATH_BLOCK;

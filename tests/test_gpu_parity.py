@@ -188,7 +188,9 @@ def test_block_path_any_grid(oracle_lib, grid):
 def test_auto_path_selection():
     dims = (2, 2, 2, 2)
     cases = [(48, cop.LINK_C64, 1, cop.PATH_STREAM), (48, cop.LINK_C64, 16, cop.PATH_TENSOR),
-             (48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_STREAM),
+             (48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_TENSOR),
+             (64, cop.LINK_I16, 2, cop.PATH_STREAM), (48, cop.LINK_I16, 3, cop.PATH_STREAM), (48, cop.LINK_I16, 4, cop.PATH_TENSOR),
+             (32, cop.LINK_I16, 2, cop.PATH_TENSOR), (64, cop.LINK_C64, 4, cop.PATH_STREAM),
              (48, cop.LINK_C64, 5, cop.PATH_TENSOR), (64, cop.LINK_I16, 16, cop.PATH_TENSOR),
              (96, cop.LINK_C64, 8, cop.PATH_TENSOR), (48, cop.LINK_C64, 17, cop.PATH_TENSOR),
              (192, cop.LINK_I16, 12, cop.PATH_TENSOR), (6, cop.LINK_C64, 2, cop.PATH_SIMPLE)]
@@ -583,7 +585,7 @@ def test_apply_host_pipelined_path_is_bit_identical(oracle_lib, prec):
 
 @pytest.mark.parametrize("Nc,prec,nrhs,want_path,launches", [
     (48, cop.LINK_I16, 3, cop.PATH_STREAM, 4), (64, cop.LINK_C64, 16, cop.PATH_TENSOR, 8),
-    (48, cop.LINK_I16, 20, cop.PATH_TENSOR, 16)])
+    (48, cop.LINK_I16, 20, cop.PATH_TENSOR, 16), (64, cop.LINK_I16, 4, cop.PATH_TENSOR, 4)])
 def test_apply_host_pipelined_multi_rhs_is_bit_identical(oracle_lib, Nc, prec, nrhs, want_path, launches):
     """The pipelined host path for several right-hand sides: STREAM-MR (3 = one propagator) and
     TENSOR launch ranges of x3-slices too; results must equal the device-resident apply bit for bit."""
@@ -609,10 +611,13 @@ def test_apply_host_pipelined_multi_rhs_is_bit_identical(oracle_lib, Nc, prec, n
         if i8:
             # the device-resident apply runs int16 links on the integer tensor-core kernel; the site-range launches of
             # apply_host use the 3xTF32 kernel (include/coarse_op.h): bit-identical to THAT kernel, 1e-5 to the other
+            # (the path is pinned for the comparison run: with the integer kernel switched off AUTO sends 2-4 RHS to STREAM)
             op.set_option(cop.OPT_TENSOR_I8, 1)
+            op.set_option(cop.OPT_PATH, cop.PATH_TENSOR)
             ref = torch.empty_like(vin_d)
             op.apply(vin_d, ref, nrhs=nrhs, dagger=dagger)
             op.set_option(cop.OPT_TENSOR_I8, 0)
+            op.set_option(cop.OPT_PATH, cop.PATH_AUTO)
         torch.cuda.synchronize()
         vout.fill_(float("nan"))
         op.apply_host(vin, vout, nrhs=nrhs, dagger=dagger)
