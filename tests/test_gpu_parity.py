@@ -143,6 +143,18 @@ def test_tensor_path_every_shape(oracle_lib, dims, Nc, prec, nrhs, dagger):
     assert err <= 3e-6, f"3xTF32 with per-matrix accumulator chains should sit near 1e-6, got {err:.2e}"
 
 
+@pytest.mark.parametrize("Nc", [32, 48, 64])
+@pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
+@pytest.mark.parametrize("nrhs", [3, 8, 16])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_tensor_two_sites_per_tile_odd_site_count(oracle_lib, Nc, prec, nrhs, dagger):
+    """Nc <= 64: a work item of the tensor kernels is a PAIR of sites sharing the 128-lane MMA tile.  135 sites: the
+    last item has one site only (its second half must not store), with one CTA per item, several items per CTA and a
+    single CTA walking all 68 items (rings wrap many times)."""
+    for grid in (0, 7, 1):
+        _run(oracle_lib, (3, 3, 3, 5), Nc, prec, nrhs, dagger, cop.PATH_TENSOR, seed=77 + grid, hermitian=False, grid=grid)
+
+
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (1, 1, 1, 1)])
 @pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
 @pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
