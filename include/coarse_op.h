@@ -71,8 +71,8 @@ enum {
 };
 
 /* Kernel families, each compiled for Nc in {32,48,64,96,128,192}; every family computes the same operation and the
- * tests run parity on each.  AUTO: 1 RHS -> STREAM; 2-4 RHS -> STREAM (its multi-RHS kernel), except int16 links from
- * 2 RHS (Nc >= 96, Nc = 32), 3 RHS (Nc = 64) or 4 RHS (Nc = 48) -> TENSOR; 5 RHS and more -> TENSOR; BLOCK only on request (or when no tensor map can be made for the links);
+ * tests run parity on each.  AUTO: 1 RHS -> STREAM; 2-4 RHS -> STREAM (its multi-RHS kernel), except int16 links
+ * (Nc = 48: only at 4 RHS) -> TENSOR; 5 RHS and more -> TENSOR; BLOCK only on request (or when no tensor map can be made for the links);
  * Nc outside the compiled set -> SIMPLE. */
 enum {
     COARSE_PATH_AUTO = 0,

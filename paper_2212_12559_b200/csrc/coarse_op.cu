@@ -232,13 +232,14 @@ int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int 
     return COARSE_OK;
 }
 
-// COARSE_PATH_AUTO.  1 RHS: STREAM.  2-4 RHS: STREAM-MR, except int16 links where the integer tensor-core kernel
-// is faster - from 2 RHS for Nc >= 96 and Nc = 32, from 3 for Nc = 64, at 4 for Nc = 48 (measured ms, dagger 0 / 1,
-// HBM-sized lattices, STREAM-MR against TENSOR: Nc = 128, 3 RHS 0.74 / 0.65 against 0.58 / 0.55; Nc = 64, 3 RHS 3.11 / 3.05
-// against 2.97 / 2.94, 4 RHS 4.47 / 4.17 against 3.04 / 3.00, 2 RHS 2.93 / 2.56 against 2.93 / 2.89; Nc = 48, 3 RHS 2.57 /
-// 2.63 against 3.30 / 3.33, 4 RHS 3.59 / 4.63 against 3.33 / 3.34; Nc = 32, 2 RHS 4.35 / 2.95 against 2.82 / 2.92).  5 and
-// more: TENSOR (BLOCK only on request, or when no tensor map could be made), outside the compiled Nc: SIMPLE.
-int tensor_i8_min_nrhs(int Nc) { return Nc >= 96 ? 2 : Nc == 64 ? 3 : Nc == 48 ? 4 : 2; }
+// COARSE_PATH_AUTO.  1 RHS: STREAM.  2-4 RHS: STREAM-MR, except int16 links, where the integer tensor-core kernel
+// (4-wide column tile, two sites per MMA tile for Nc <= 64) is faster from 2 RHS on - Nc = 48 only at 4 (measured ms,
+// dagger 0 / 1, HBM-sized lattices, STREAM-MR against TENSOR: Nc = 128, 3 RHS 0.74 / 0.65 against 0.58 / 0.55; Nc = 64,
+// 2 RHS 3.07 / 2.68 against 2.59 / 2.61, 3 RHS 3.26 / 3.20 against 2.66 / 2.67, 4 RHS 4.46 / 4.17 against 2.67 / 2.68;
+// Nc = 48, 2 RHS 2.20 / 2.45 against 2.77 / 2.90, 3 RHS 2.57 / 2.63 against 2.79 / 2.92, 4 RHS 3.60 / 4.61 against 2.80 / 2.93;
+// Nc = 32, 2 RHS 4.28 / 2.95 against 2.32 / 2.41).  5 and more: TENSOR (BLOCK only on request, or when no tensor map
+// could be made), outside the compiled Nc: SIMPLE.
+int tensor_i8_min_nrhs(int Nc) { return Nc == 48 ? 4 : 2; }
 
 int auto_path(const coarse_op* op, int nrhs) {
     const bool tensor_ok = tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok;

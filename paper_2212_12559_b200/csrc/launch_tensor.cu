@@ -79,8 +79,17 @@ int COARSE_CAT(launch_tensor_i8_nc, COARSE_NC)(const coarse_op* op, const Tensor
         }
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e, "vector scale kernel launch");
-        int rc;
-        if (p.t.width <= 8)
+        int rc = COARSE_OK;
+        bool done = false;
+        if constexpr (TensorI8Geom<COARSE_NC, 4>::OK) {      // Nc <= 64: 4-wide tile (two sites per item) for 2-4 right-hand sides
+            if (p.t.width <= 4) {
+                rc = dagger ? launch_tensor_i8_t<COARSE_NC, 4, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 4, false>(op, p, stream);
+                done = true;
+            }
+        }
+        if (done)
+            ;
+        else if (p.t.width <= 8)
             rc = dagger ? launch_tensor_i8_t<COARSE_NC, 8, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 8, false>(op, p, stream);
         else
             rc = dagger ? launch_tensor_i8_t<COARSE_NC, 16, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 16, false>(op, p, stream);

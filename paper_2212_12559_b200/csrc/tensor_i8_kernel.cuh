@@ -57,7 +57,7 @@ struct TensorI8Geom {
     // Two sites per work item when the matrices have at most 64 rows and the 8-wide column tile is in use (the
     // accumulator ring of the 16-wide tile would not fit tensor memory): site 0 in TMEM lanes 0.., site 1 in lanes
     // 64.., their B operands side by side along N inside every digit block (see TensorGeom::NS in tensor_kernel.cuh).
-    static constexpr int NS = (MT <= 64 && NP == 8) ? 2 : 1;
+    static constexpr int NS = (MT <= 64 && NP <= 8) ? 2 : 1;     // (a 4-wide column tile for 2-4 right-hand sides exists in this mode only)
     static constexpr int NPS = NP * NS;                        // right-hand-side columns of an item (all its sites)
     static constexpr int SLAB_BYTES = MT * KC * 4;             // one site's slab of a stage
     static constexpr int SLAB_PITCH = NS == 2 ? 64 * KC * 4 : SLAB_BYTES;
@@ -79,7 +79,7 @@ struct TensorI8Geom {
     static constexpr int THREADS = (EPI_W0 + 4) * 32;
     static constexpr int NBAR = 2 * LS + 2 * AS + 2 * DS;
     static constexpr int SMEM_BYTES = 1024 + LS * LINK_STAGE + AS * B_STAGE + FT * NPS * 4 + NBAR * 8 + 16;
-    static constexpr bool OK = (NC % 16 == 0) && (MT % 8 == 0) && MT <= 128 && (NP == 8 || NP == 16) && NE >= 1 &&
+    static constexpr bool OK = (NC % 16 == 0) && (MT % 8 == 0) && MT <= 128 && (NP == 4 || NP == 8 || NP == 16) && NE >= 1 && NB3 % 16 == 0 &&
                                (D_COL0 + DS * D_COLS <= TMEM_COLS) && SMEM_BYTES <= 232448 && 2 * NC * 128 * 255 < (1 << 24);
 };
 
@@ -283,7 +283,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                             // (overwrite), W_1, W_2 += low plane digits 1, 2
                             ptx::mma_i8_ts(d1, a1, db, IDESC_S, 0u);
                             ptx::mma_i8_ts(d0, a0, db, IDESC_U1, 0u);
-                            ptx::mma_i8_ts(d1, a0, db + (uint64_t)((2 * (NPS >> 3) * B_SBO) >> 4), IDESC_U2, 1u);
+                            ptx::mma_i8_ts(d1, a0, db + (uint64_t)(((2 * NPS >> 3) * B_SBO) >> 4), IDESC_U2, 1u);
                         } else {
                             ptx::mma_i8_ts(d1, a1 + kk * 8, db, IDESC_S, 1u);
                             ptx::mma_i8_ts(d0, a0 + kk * 8, db, IDESC_U, 1u);
@@ -309,9 +309,11 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
 
         // B entries of this thread: contraction row j (of the stage's KC) and column r, the same in every stage;
         // every entry of a thread has the same r.  e = gtid + 128 x: bits 0-2 = r mod 8 (16-byte rows of the K-major
-        // layout: banks 4 apart), bits 3-4 = j mod 4 (bytes 2 apart / next word), bit 5 = r div 8 (NP = 16) or the site sg (two sites per item), rest = j div 4:
+        // layout: banks 4 apart), bits 3-4 = j mod 4 (bytes 2 apart / next word) - for the 4-wide tile bits 0-1 = r and
+        // bits 2-4 = j mod 8 -, bit 5 = r div 8 (NP = 16) or the site sg (two sites per item), rest = the high part of j:
         // the 32 lanes of a 16-bit store touch 16 distinct words in 16 distinct banks (conflict-free).
-        const int my_r = (gtid & 7) + (NP == 16 ? ((gtid >> 5) & 1) * 8 : 0);
+        constexpr int RB = NP >= 8 ? 3 : 2, JB = 5 - RB;              // lane bits of r and of j
+        const int my_r = (gtid & ((1 << RB) - 1)) + (NP == 16 ? ((gtid >> 5) & 1) * 8 : 0);
         const int my_sg = NS == 2 ? (gtid >> 5) & 1 : 0;              // every B entry of a thread belongs to ONE site of the item
         const int my_n = my_sg * 2 * NP + my_r;                       // column inside a digit block
         const bool r_valid = my_r < p.width;
@@ -320,13 +322,13 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
 #pragma unroll
         for (int x = 0; x < NE; ++x) {
             const int e = gtid + 128 * x;
-            const int j = ((e >> 3) & 3) + 4 * (e >> (NPS == 16 ? 6 : 5));
+            const int j = ((e >> RB) & ((1 << JB) - 1)) + (1 << JB) * (e >> ((NP == 16 || NS == 2) ? 6 : 5));
             b_off_vec[x] = j * p.nrhs + my_r;
             const int k = 2 * j;
             b_o[x] = (uint32_t)(k >> 4) * 128u + (uint32_t)(my_n >> 3) * B_SBO + (uint32_t)(my_n & 7) * 16u + (uint32_t)(k & 15);
         }
-        constexpr uint32_t N_STEP = (uint32_t)(NP >> 3) * B_SBO;     // byte step of NP columns of n (NP is a multiple of 8)
-        constexpr uint32_t D_STEP = 2 * NS * N_STEP;                 // byte step of one digit block
+        constexpr uint32_t N_STEP = (uint32_t)(NP >> 3) * B_SBO + (uint32_t)(NP & 7) * 16u;   // byte step of NP columns of n (Re -> Im block)
+        constexpr uint32_t D_STEP = (uint32_t)(2 * NPS >> 3) * B_SBO;                          // byte step of one digit block (2 NPS columns)
 
         int n_it = 0, n_m = M0, n_c = grp, n_s = 0;
         SiteX n_cx = {};
@@ -442,8 +444,9 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                 ptx::sts16(bt + b_o[x] + N_STEP + 2 * D_STEP, pack_lo_bytes(x2, y2));
             }
             // epilogue factor of this matrix and column: written by the group that converts the matrix's first chunk
-            if (first_chunk && (gtid & 0x18) == 0 && gtid < 64) {
-                // threads 0-7 (and 32-39 for NP = 16 / the second site) of the group hold r = 0..7 (8..15 / r = 0..7 of site 1)
+            if (first_chunk && (gtid & (0x1f & ~((1 << RB) - 1))) == 0 && gtid < 64) {
+                // threads 0-7 (and 32-39 for NP = 16 / the second site) of the group hold r = 0..7 (8..15 / r = 0..7 of site 1);
+                // 4-wide tile: threads 0-3 and 32-35
                 asm volatile("st.shared.f32 [%0], %1;" ::"r"(ft_u32 + (uint32_t)(((t / CHUNKS) % FT) * NPS + my_sg * NP + my_r) * 4u), "f"(f) : "memory");
             }
             ptx::tc_wait_st();

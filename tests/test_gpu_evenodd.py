@@ -123,7 +123,7 @@ def test_parts_stream_few_rhs(oracle_lib, Nc, prec, nrhs, dagger, parity, local)
 
 def test_parts_auto_routes_few_rhs():
     dims = (2, 2, 2, 2)
-    for Nc, prec, nrhs, want in ((48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_TENSOR), (64, cop.LINK_I16, 2, cop.PATH_STREAM),
+    for Nc, prec, nrhs, want in ((48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_TENSOR), (64, cop.LINK_I16, 2, cop.PATH_TENSOR), (48, cop.LINK_I16, 2, cop.PATH_STREAM),
                                  (128, cop.LINK_I16, 3, cop.PATH_TENSOR), (128, cop.LINK_C64, 2, cop.PATH_STREAM)):
         V = 16
         if prec == cop.LINK_C64:

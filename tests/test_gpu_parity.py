@@ -201,7 +201,7 @@ def test_auto_path_selection():
     dims = (2, 2, 2, 2)
     cases = [(48, cop.LINK_C64, 1, cop.PATH_STREAM), (48, cop.LINK_C64, 16, cop.PATH_TENSOR),
              (48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_TENSOR),
-             (64, cop.LINK_I16, 2, cop.PATH_STREAM), (48, cop.LINK_I16, 3, cop.PATH_STREAM), (48, cop.LINK_I16, 4, cop.PATH_TENSOR),
+             (64, cop.LINK_I16, 2, cop.PATH_TENSOR), (48, cop.LINK_I16, 3, cop.PATH_STREAM), (48, cop.LINK_I16, 4, cop.PATH_TENSOR),
              (32, cop.LINK_I16, 2, cop.PATH_TENSOR), (64, cop.LINK_C64, 4, cop.PATH_STREAM),
              (48, cop.LINK_C64, 5, cop.PATH_TENSOR), (64, cop.LINK_I16, 16, cop.PATH_TENSOR),
              (96, cop.LINK_C64, 8, cop.PATH_TENSOR), (48, cop.LINK_C64, 17, cop.PATH_TENSOR),
@@ -249,12 +249,13 @@ def test_tensor_path_matches_cuda_core_path_and_is_reproducible():
     op.close()
 
 
-@pytest.mark.parametrize("Nc,prec,applies", [(64, cop.LINK_C64, 1200), (128, cop.LINK_I16, 600)])
-def test_tensor_kernels_bit_reproducible_under_stress(Nc, prec, applies):
+@pytest.mark.parametrize("Nc,prec,nrhs,applies", [(64, cop.LINK_C64, 16, 1200), (128, cop.LINK_I16, 16, 600),
+                                                  (64, cop.LINK_I16, 8, 1200), (64, cop.LINK_I16, 3, 1200)])
+def test_tensor_kernels_bit_reproducible_under_stress(Nc, prec, nrhs, applies):
     """Many applies on a lattice with ~55 work items per CTA: every result must equal the first one bit for bit.  (An
     earlier version released a link slot right after loading it, behind a fence only; the producer's next TMA write
     overtook the reads once in 600-2000 applies and a few rows of one site came out wrong.)"""
-    dims, nrhs = (8, 8, 8, 16), 16
+    dims = (8, 8, 8, 16)                  # (Nc = 64 int16: two sites per MMA tile, 8- and 4-wide column tiles)
     V = synth.lattice_volume(dims)
     links = synth.make_arbitrary_links(dims, Nc, 5, device="cuda")
     scales = None
