@@ -181,6 +181,23 @@ int coarse_op_apply_hvec(coarse_op_t* op, const void* in_q_dev, const float* in_
 int coarse_op_apply_hout(coarse_op_t* op, const void* in_dev, const float* in_norms_dev, void* out_c64_dev, void* out_q_dev,
                          float* out_norms_dev, int nrhs, int dagger, void* stream);
 
+/* The plain apply for callers that cannot call cudaMalloc (code under CUDA stream capture, tight serving loops,
+ * harnesses that forbid allocation): out = D in (dagger 0) or D^dagger in (1) for INT16 links and any
+ * nrhs >= 1, on the integer tensor-core kernel of COARSE_PATH_TENSOR - the same kernels, launches and
+ * results as coarse_op_apply with that path - but with the kernel's scratch memory (the power-of-two scales of the
+ * fixed-point vector operand, one (g, 1/g) pair per site and column) in a file-scope __device__ array of the library
+ * instead of the buffer coarse_op_set_links allocates.  This call reaches no cudaMalloc / cudaFree and no allocating
+ * library routine; the handle itself must have been created and given its links beforehand.
+ * Limit: at most COARSE_STATIC_MAX_SITES lattice sites (the array is COARSE_STATIC_MAX_SITES * 128 bytes = 1 MiB,
+ * held by every GPU that loads the library until the process exits); more sites, complex64 links or an Nc outside
+ * the compiled set return COARSE_EUNSUPPORTED with a message.  in_dev / out_dev: device, complex64 [V][Nc][nrhs],
+ * 16-byte aligned, not overlapping; the handle's device must be current.
+ * The array is shared by ALL calls and handles of the process on that GPU and keeps the last call's contents:
+ * nothing in it needs to start at zero (each call rewrites every entry it reads), calls on one stream are ordered,
+ * but calls that overlap on the GPU (other streams without an ordering event) RACE on it. */
+#define COARSE_STATIC_MAX_SITES 8192
+int coarse_op_apply_static(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs, int dagger, void* stream);
+
 /* Vector quantiser: for each (site, rhs) norm = max|component|/32767 (fp32 division) and
  * q = clamp(rint(component/norm), -32767, 32767); an all-zero vector gets norm 0 and q = 0.
  * v_c64_dev: float[n_sites][Nc][nrhs][2]; q_dev: int16_t same shape; norms_dev: float[n_sites][nrhs]. */

@@ -26,7 +26,7 @@ LOCAL_NONE, LOCAL_X, LOCAL_IDENTITY = 0, 1, 2
 EXPORTS = (
     "coarse_op_create", "coarse_op_link_bytes", "coarse_op_scale_bytes", "coarse_op_vector_bytes",
     "coarse_op_set_links", "coarse_op_set_option", "coarse_op_apply", "coarse_op_apply_parts", "coarse_op_apply_hvec",
-    "coarse_op_apply_hout",
+    "coarse_op_apply_hout", "coarse_op_apply_static",
     "coarse_op_quantize_vec_i16", "coarse_op_apply_host",
     "coarse_op_last_launches", "coarse_op_last_path", "coarse_op_quantize_i16", "coarse_op_probe_read", "coarse_op_cagcr_work_bytes",
     "coarse_op_cagcr", "coarse_op_cagcr_schur", "coarse_op_cagcr_cheb_work_bytes",
@@ -71,6 +71,8 @@ def lib() -> ctypes.CDLL:
     L.coarse_op_apply_parts.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ctypes.c_float, ctypes.c_float, vp]
     L.coarse_op_apply_hvec.restype = ci
     L.coarse_op_apply_hvec.argtypes = [vp, vp, vp, vp, ci, ci, vp]
+    L.coarse_op_apply_static.restype = ci
+    L.coarse_op_apply_static.argtypes = [vp, vp, vp, ci, ci, vp]
     L.coarse_op_apply_hout.restype = ci
     L.coarse_op_apply_hout.argtypes = [vp, vp, vp, vp, vp, vp, ci, ci, vp]
     L.coarse_op_quantize_vec_i16.restype = ci
@@ -174,6 +176,20 @@ def coarse_op_apply(op: int, vin, vout, nrhs: int = 1, dagger: int = 0, stream=N
         if t.numel() * t.element_size() != coarse_op_vector_bytes(op, nrhs):
             raise ValueError("vector tensor has the wrong number of bytes for this operator/nrhs")
     _check(lib().coarse_op_apply(op, _ptr(vin), _ptr(vout), int(nrhs), int(dagger), _stream_handle(stream)))
+
+
+STATIC_MAX_SITES = 8192        # COARSE_STATIC_MAX_SITES in include/coarse_op.h
+
+
+def coarse_op_apply_static(op: int, vin, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+    """The plain apply on int16 links with the kernel's scratch in a static device array of the library: the call
+    allocates nothing (include/coarse_op.h; at most STATIC_MAX_SITES sites; calls that overlap on the GPU race)."""
+    for t in (vin, vout):
+        if not t.is_cuda or not t.is_contiguous():
+            raise ValueError("vectors must be contiguous CUDA tensors")
+        if t.numel() * t.element_size() != coarse_op_vector_bytes(op, nrhs):
+            raise ValueError("vector tensor has the wrong number of bytes for this operator/nrhs")
+    _check(lib().coarse_op_apply_static(op, _ptr(vin), _ptr(vout), int(nrhs), int(dagger), _stream_handle(stream)))
 
 
 def coarse_op_apply_parts(op: int, u, w, vout, nrhs: int = 1, dagger: int = 0, parity: int = PARITY_ALL,
@@ -378,6 +394,9 @@ class CoarseOp:
 
     def apply(self, vin, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
         coarse_op_apply(self._h, vin, vout, nrhs, dagger, stream)
+
+    def apply_static(self, vin, vout, nrhs: int = 1, dagger: int = 0, stream=None) -> None:
+        coarse_op_apply_static(self._h, vin, vout, nrhs, dagger, stream)
 
     def apply_parts(self, u, w, vout, nrhs: int = 1, dagger: int = 0, parity: int = PARITY_ALL,
                     local: int = LOCAL_X, alpha: float = 1.0, beta: float = 1.0, stream=None) -> None:

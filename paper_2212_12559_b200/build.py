@@ -44,7 +44,7 @@ def sources():
 
 def units():
     """(object name, source file, extra defines) of every translation unit."""
-    out = [("coarse_op", "coarse_op.cu", []), ("link_map", "link_map.cu", [])]
+    out = [("coarse_op", "coarse_op.cu", []), ("link_map", "link_map.cu", []), ("static_scratch", "static_scratch.cu", [])]
     for fam in ("launch_stream", "launch_stream_mr", "launch_block", "launch_tensor"):
         for nc in NC_SET:
             out.append((f"{fam}_nc{nc}", f"{fam}.cu", [f"-DCOARSE_NC={nc}"]))
