@@ -493,6 +493,8 @@ def run_ours(args, cfg, daggers):
     # all K steps (coarse_op_apply is capturable: it only enqueues).
     use_graph = args.graph == "on" or (args.graph == "auto" and link_bytes <= 2 * l2_bytes)
 
+    path_of = {}
+
     def step(record=None):
         nonlocal launches
         for k, dg in enumerate(daggers):
@@ -502,6 +504,7 @@ def run_ours(args, cfg, daggers):
                 e0.record(stream)
             apply_one(vouts[k], dg)
             launches += op.last_launches
+            path_of[dg] = op.last_path              # AUTO may pick another family per mode (complex64, 4 RHS)
             if record is not None:
                 e1.record(stream)
                 record[dg].append((e0, e1))
@@ -633,10 +636,10 @@ def run_ours(args, cfg, daggers):
     achieved = bps * V / (kernel_ms[dom] * 1e-3) / 1e9
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": None if args.hvec else ncu_traffic_bytes(args.config, op.last_path, dom, cfg["links"]),
+        "traffic": None if args.hvec else ncu_traffic_bytes(args.config, path_of.get(dom, op.last_path), dom, cfg["links"]),
         "kernel": "coarse_apply_%s<Nc=%d,%s,dagger=%d%s>" % (
             {cop.PATH_SIMPLE: "simple", cop.PATH_STREAM: "stream", cop.PATH_TENSOR: "tensor",
-             cop.PATH_BLOCK: "block"}.get(op.last_path, "?"), Nc, "i16" if prec else "c64", dom,
+             cop.PATH_BLOCK: "block"}.get(path_of.get(dom, op.last_path), "?"), Nc, "i16" if prec else "c64", dom,
             "" if nrhs == 1 else ",nrhs=%d" % nrhs),
         "kernel_ms": kernel_ms[dom],
         "algorithmic_bytes_per_launch": bps * V,

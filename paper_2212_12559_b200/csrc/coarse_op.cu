@@ -239,14 +239,21 @@ int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int 
 // Nc = 48, 2 RHS 2.20 / 2.45 against 2.77 / 2.90, 3 RHS 2.57 / 2.63 against 2.79 / 2.92, 4 RHS 3.60 / 4.61 against 2.80 / 2.93;
 // Nc = 32, 2 RHS 4.28 / 2.95 against 2.32 / 2.41).  5 and more: TENSOR (BLOCK only on request, or when no tensor map
 // could be made), outside the compiled Nc: SIMPLE.
+// Complex64 links with exactly 4 RHS in dagger = 0 also go to TENSOR for Nc >= 48: there every warp of STREAM-MR reads
+// the whole 4-wide vector block of a stage with 4-way bank conflicts (stream_mr_kernel.cuh) and the kernel is bound by
+// shared-memory bandwidth at twice the time of 3 RHS (measured ms, STREAM-MR against TENSOR: Nc = 192 1.10 / 0.59,
+// Nc = 128 2.15 / 1.06, Nc = 96 4.33 / 2.82, Nc = 64 6.35 / 5.00, Nc = 48 4.46 / 3.86, Nc = 32 4.76 / 4.71); its
+// dagger = 1 (1.03 ms at Nc = 128) stays.
 int tensor_i8_min_nrhs(int Nc) { return Nc == 48 ? 4 : 2; }
 
-int auto_path(const coarse_op* op, int nrhs) {
+int auto_path(const coarse_op* op, int nrhs, int dagger) {
     const bool tensor_ok = tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok;
     if (stream_supports(op->Nc, nrhs)) return COARSE_PATH_STREAM;
     if (stream_mr_supports(op->Nc, nrhs)) {
         const bool i8 = op->prec == COARSE_LINK_I16 && op->link_map_i8_ok && op->vscale && op->tensor_i8_opt != 1;
-        return (tensor_ok && i8 && nrhs >= tensor_i8_min_nrhs(op->Nc)) ? COARSE_PATH_TENSOR : COARSE_PATH_STREAM;
+        if (tensor_ok && i8 && nrhs >= tensor_i8_min_nrhs(op->Nc)) return COARSE_PATH_TENSOR;
+        if (tensor_ok && op->prec == COARSE_LINK_C64 && nrhs == 4 && dagger == 0 && op->Nc >= 48) return COARSE_PATH_TENSOR;
+        return COARSE_PATH_STREAM;
     }
     if (tensor_ok) return COARSE_PATH_TENSOR;
     if (block_supports(op->Nc, nrhs)) return COARSE_PATH_BLOCK;
@@ -473,7 +480,7 @@ int coarse_op_apply(coarse_op_t* op, const void* in_dev, void* out_dev, int nrhs
     if (a < b + vb && b < a + vb) return fail(COARSE_EINVAL, "apply: in and out overlap (the stencil reads neighbours)");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int path = op->path_opt;
-    if (path == COARSE_PATH_AUTO) path = auto_path(op, nrhs);
+    if (path == COARSE_PATH_AUTO) path = auto_path(op, nrhs, dagger);
     op->last_launches = 0;
     if (path == COARSE_PATH_TENSOR) {
         if (!tensor_supports(op->Nc, op->prec, nrhs))
@@ -537,7 +544,7 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
     const bool tensor_ok = tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok;
     const bool stream_ok = stream_supports(op->Nc, nrhs) || stream_mr_supports(op->Nc, nrhs);
     if (path == COARSE_PATH_AUTO || path == COARSE_PATH_BLOCK) {
-        path = auto_path(op, nrhs);                                     // the plain apply's rule; BLOCK has no parts variant
+        path = auto_path(op, nrhs, dagger);                                     // the plain apply's rule; BLOCK has no parts variant
         if (path == COARSE_PATH_BLOCK) path = COARSE_PATH_SIMPLE;
     } else if ((path == COARSE_PATH_STREAM && !stream_ok) || (path == COARSE_PATH_TENSOR && !tensor_ok)) {
         path = stream_ok ? COARSE_PATH_STREAM : tensor_ok ? COARSE_PATH_TENSOR : COARSE_PATH_SIMPLE;
@@ -673,7 +680,7 @@ int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, i
     const int T = op->lat.L[3];
     // the family coarse_op_apply would pick; STREAM (1-4 RHS) and TENSOR launch site ranges
     int hpath = op->path_opt;
-    if (hpath == COARSE_PATH_AUTO) hpath = auto_path(op, nrhs);
+    if (hpath == COARSE_PATH_AUTO) hpath = auto_path(op, nrhs, dagger);
     const bool ranged = (hpath == COARSE_PATH_STREAM && (stream_supports(op->Nc, nrhs) || stream_mr_supports(op->Nc, nrhs))) ||
                         (hpath == COARSE_PATH_TENSOR && tensor_supports(op->Nc, op->prec, nrhs) && op->link_map_ok);
     if (ranged && T >= 8 && vb >= ((size_t)1 << 22)) {

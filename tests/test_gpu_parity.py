@@ -202,7 +202,7 @@ def test_auto_path_selection():
     cases = [(48, cop.LINK_C64, 1, cop.PATH_STREAM), (48, cop.LINK_C64, 16, cop.PATH_TENSOR),
              (48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_TENSOR),
              (64, cop.LINK_I16, 2, cop.PATH_TENSOR), (48, cop.LINK_I16, 3, cop.PATH_STREAM), (48, cop.LINK_I16, 4, cop.PATH_TENSOR),
-             (32, cop.LINK_I16, 2, cop.PATH_TENSOR), (64, cop.LINK_C64, 4, cop.PATH_STREAM),
+             (32, cop.LINK_I16, 2, cop.PATH_TENSOR), (64, cop.LINK_C64, 4, cop.PATH_TENSOR), (32, cop.LINK_C64, 4, cop.PATH_STREAM),
              (48, cop.LINK_C64, 5, cop.PATH_TENSOR), (64, cop.LINK_I16, 16, cop.PATH_TENSOR),
              (96, cop.LINK_C64, 8, cop.PATH_TENSOR), (48, cop.LINK_C64, 17, cop.PATH_TENSOR),
              (192, cop.LINK_I16, 12, cop.PATH_TENSOR), (6, cop.LINK_C64, 2, cop.PATH_SIMPLE)]
@@ -219,6 +219,10 @@ def test_auto_path_selection():
         op.apply(vin, vout, nrhs=nrhs)
         torch.cuda.synchronize()
         assert op.last_path == want, (Nc, prec, nrhs, op.last_path, want)
+        if prec == cop.LINK_C64 and nrhs == 4:      # complex64, 4 RHS: only dagger = 0 leaves STREAM-MR (bank conflicts there)
+            op.apply(vin, vout, nrhs=nrhs, dagger=1)
+            torch.cuda.synchronize()
+            assert op.last_path == cop.PATH_STREAM
         op.close()
 
 
