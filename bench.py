@@ -287,11 +287,13 @@ def parity_sample_sites(dims, n_random, seed):
     return np.unique(np.concatenate([np.asarray(pts, dtype=np.int64), rnd])).astype(np.int64)
 
 
-def parity_check(cfg, links, scales, vin, outs, n_random=64):
+def parity_check(cfg, links, scales, vin, outs, n_random=64, hvec=None):
     """"parity is checked in the same run, before timing, on the same buffers".  The device
     buffers the timed loop is about to use hold one apply per dagger; the CPU oracle (its per-site
     evaluation, `oracle.coarse_apply_sites`) recomputes >= 64 sampled output sites from the links and
     vectors those sites touch.  Returns the worst relative L2 error over daggers and right-hand sides.
+    `hvec` = (int16 vector, norms): the run applies the operator to half-precision vectors (--hvec), and the oracle
+    evaluates the same int16 + norm arrays.
     (Part of the oracle legs of this script, like cpu_baseline: the product path never calls it.)"""
     import oracle
     oracle.build()
@@ -305,12 +307,17 @@ def parity_check(cfg, links, scales, vin, outs, n_random=64):
     idx = torch.as_tensor(need, device=flat.device)
     links_h[need] = flat[idx].cpu().numpy().reshape(len(need), 9, Nc, Nc, 2)
     scales_h = None if scales is None else scales.cpu().numpy()
-    vin_h = vin.cpu().numpy()
+    vin_h = vin.cpu().numpy() if hvec is None else None
+    hq_h, hn_h = (hvec[0].cpu().numpy(), hvec[1].cpu().numpy()) if hvec is not None else (None, None)
     worst, worst_site = 0.0, 0.0
     sidx = torch.as_tensor(sites, device=flat.device)
     for dg, out in outs.items():
-        ref = oracle.coarse_apply_sites(dims, Nc, links_h, vin_h, sites, nrhs=nrhs, dagger=dg,
-                                        link_precision=oracle.LINK_I16 if i16 else oracle.LINK_C64, scales=scales_h)
+        if hvec is not None:
+            ref = oracle.coarse_apply_hvec_sites(dims, Nc, links_h, hq_h, hn_h, sites, nrhs=nrhs, dagger=dg,
+                                                 link_precision=oracle.LINK_I16 if i16 else oracle.LINK_C64, scales=scales_h)
+        else:
+            ref = oracle.coarse_apply_sites(dims, Nc, links_h, vin_h, sites, nrhs=nrhs, dagger=dg,
+                                            link_precision=oracle.LINK_I16 if i16 else oracle.LINK_C64, scales=scales_h)
         got = out[sidx].cpu().numpy().astype(np.complex128)
         for r in range(nrhs):
             worst = max(worst, float(np.linalg.norm(got[..., r] - ref[..., r]) / np.linalg.norm(ref[..., r])))
@@ -343,16 +350,29 @@ def measure_config(name, steps, local, dev, read_ceiling=None, override=None):
     outs = {dg: torch.full_like(vin, float("nan")) for dg in (0, 1)}
     op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
     stream = torch.cuda.current_stream()
+    hvec = bool(cfg.get("hvec"))        # half-precision input vectors: int16 + per-site norm
+    vq = vnorm = None
+    if hvec:
+        vq = torch.empty((V, Nc, nrhs, 2), dtype=torch.int16, device=dev)
+        vnorm = torch.empty((V, nrhs), dtype=torch.float32, device=dev)
+        cop.coarse_op_quantize_vec_i16(vin, Nc, nrhs, vq, vnorm)
+
+    def apply(o, out, dg):
+        if hvec:
+            o.apply_hvec(vq, vnorm, out, nrhs=nrhs, dagger=dg)
+        else:
+            o.apply(vin, out, nrhs=nrhs, dagger=dg)
+
     for dg in (0, 1):
-        op.apply(vin, outs[dg], nrhs=nrhs, dagger=dg)
+        apply(op, outs[dg], dg)
     torch.cuda.synchronize()
     path = op.last_path
-    parity = parity_check(cfg, links, scales, vin, outs)
+    parity = parity_check(cfg, links, scales, vin, outs, hvec=(vq, vnorm) if hvec else None)
     link_bytes = links.numel() * links.element_size()
     l2_bytes = torch.cuda.get_device_properties(dev).L2_cache_size
-    bps = compulsory_bytes_per_site(Nc, cfg["links"], nrhs)
+    bps = compulsory_bytes_per_site(Nc, cfg["links"], nrhs, hvec)
     peak, _ = measured_peak_gbs()
-    rec = {"workload": workload_name(name, cfg), "path": path, "steps": steps, "parity": parity,
+    rec = {"workload": workload_name(name, cfg, hvec), "path": path, "steps": steps, "parity": parity,
            "algorithmic_bytes_per_launch": bps * V}
 
     def graph_of(fn):
@@ -377,13 +397,13 @@ def measure_config(name, steps, local, dev, read_ceiling=None, override=None):
     with ClockSampler(local) as clocks:
         if link_bytes <= 2 * l2_bytes:
             reps = max(steps, 400)          # a graph launch costs tens of us: amortise it over many 6-10 us applies
-            warm = {dg: time_graph(graph_of(lambda dg=dg: [op.apply(vin, outs[dg], nrhs=nrhs, dagger=dg) for _ in range(reps)])) / reps
+            warm = {dg: time_graph(graph_of(lambda dg=dg: [apply(op, outs[dg], dg) for _ in range(reps)])) / reps
                     for dg in (0, 1)}
             n_copies = int(3 * l2_bytes // max(1, link_bytes)) + 2
             copies = [(links.clone(), None if scales is None else scales.clone()) for _ in range(n_copies)]
             ops = [cop.CoarseOp(dims, Nc, prec).set_links(l, sc).set_option(cop.OPT_KEEP_LINKS, 1) for l, sc in copies]
             creps = max(reps, 2 * n_copies)
-            ms = {dg: time_graph(graph_of(lambda dg=dg: [ops[r % n_copies].apply(vin, outs[dg], nrhs=nrhs, dagger=dg)
+            ms = {dg: time_graph(graph_of(lambda dg=dg: [apply(ops[r % n_copies], outs[dg], dg)
                                                          for r in range(creps)])) / creps for dg in (0, 1)}
             for o in ops:
                 o.close()
@@ -393,13 +413,13 @@ def measure_config(name, steps, local, dev, read_ceiling=None, override=None):
         else:
             for _ in range(3):
                 for dg in (0, 1):
-                    op.apply(vin, outs[dg], nrhs=nrhs, dagger=dg)
+                    apply(op, outs[dg], dg)
             ev = {dg: [] for dg in (0, 1)}
             for _ in range(steps):
                 for dg in (0, 1):
                     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                     a.record(stream)
-                    op.apply(vin, outs[dg], nrhs=nrhs, dagger=dg)
+                    apply(op, outs[dg], dg)
                     b.record(stream)
                     ev[dg].append((a, b))
             torch.cuda.synchronize()
@@ -534,8 +554,9 @@ def run_ours(args, cfg, daggers):
     torch.cuda.synchronize()
     # parity in the same run, before timing, on the buffers the timed loop writes
     parity = None
-    if rank == 0 and not args.hvec and not args.no_parity:      # (with --hout the complex64 result is what is checked)
-        parity = parity_check(cfg, links, scales, vin, {dg: vouts[k] for k, dg in enumerate(daggers)})
+    if rank == 0 and not args.no_parity:      # (with --hout the complex64 result is what is checked)
+        parity = parity_check(cfg, links, scales, vin, {dg: vouts[k] for k, dg in enumerate(daggers)},
+                              hvec=(vq, vnorm) if args.hvec else None)
         if not parity["ok"]:
             raise RuntimeError("bench.py: the GPU result does not match the CPU oracle on the sampled sites: %r" % (parity,))
     barrier()
@@ -707,6 +728,9 @@ def run_ours(args, cfg, daggers):
         line["extras"] = {}
         for key, name, ov in (("C5_int16_nrhs16", "C5", {"links": "i16"}), ("C5_int16_nrhs3", "C5", {"links": "i16", "nrhs": 3}),
                               ("C4_nrhs3", "C4", {"nrhs": 3}),
+                              # ... and with the paper's half-precision VECTORS too (L97): both operands 16-bit fixed point
+                              ("C5_int16_hvec_nrhs16", "C5", {"links": "i16", "hvec": True}),
+                              ("C4_hvec_nrhs3", "C4", {"nrhs": 3, "hvec": True}),
                               # the paper's own per-GPU coarse volumes (PAPER.md:L117/L125/L133): level 2 and level 3, int16
                               ("P2_paper_level2_per_gpu", "P2", None), ("P3_paper_level3_per_gpu", "P3", None)):
             line["extras"][key] = measure_config(name, args.config_steps, local, dev, read_ceiling, override=ov)

@@ -204,6 +204,35 @@ int launch_tensor(const coarse_op* op, const void* in, void* out, int nrhs, int 
     }
 }
 
+// TENSOR on int16 links with HALF-PRECISION vectors (int16 pairs + fp32 norm per (site, rhs)): the plain apply only.
+// Returns the number of launches beyond the first, or a negative error code.
+bool tensor_hvec_supports(const coarse_op* op, int nrhs) {
+    return op->prec == COARSE_LINK_I16 && op->link_map_i8_ok && tensor_supports(op->Nc, op->prec, nrhs);
+}
+
+int launch_tensor_hvec(const coarse_op* op, const void* in_q, const float* in_norms, void* out, int nrhs, int dagger, cudaStream_t stream) {
+    TensorParams p = {};
+    p.lat = op->lat;
+    p.scales = op->scales;
+    p.in = static_cast<const float2*>(in_q);        // int16 (re, im) pairs; the HV kernels re-type the pointer
+    p.in_local = p.in;
+    p.out = static_cast<float2*>(out);
+    p.parity = 2;
+    p.n_sites = op->lat.V;
+    p.site_begin = 0;
+    p.m_begin = 0;
+    p.identity = 0;
+    p.alpha = 1.f;
+    p.beta = 1.f;
+    p.nrhs = nrhs;
+    switch (op->Nc) {
+#define COARSE_CASE_NC(NC) case NC: return COARSE_CAT(launch_tensor_i8h_nc, NC)(op, p, in_norms, dagger, stream);
+        COARSE_FOR_EACH_NC(COARSE_CASE_NC)
+#undef COARSE_CASE_NC
+        default: return fail(COARSE_EUNSUPPORTED, "TENSOR path is not compiled for Nc=%d", op->Nc);
+    }
+}
+
 int launch_simple(const coarse_op* op, const void* in, void* out, int nrhs, int dagger, const PartsSpec& ps, cudaStream_t stream) {
     SimpleParams p;
     p.lat = op->lat;
@@ -578,10 +607,21 @@ int coarse_op_apply_hvec(coarse_op_t* op, const void* in_q_dev, const float* in_
     PartsSpec ps = kPlain;
     ps.vnorms = in_norms_dev;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // 1 RHS: STREAM (the norm folded into the vector operand); several right-hand sides on int16 links: the integer
+    // tensor-core kernel, both operands exact int8 planes (tensor_i8_kernel.cuh, HV); otherwise SIMPLE
     int path = op->path_opt;
-    if (path == COARSE_PATH_AUTO || path == COARSE_PATH_TENSOR || path == COARSE_PATH_BLOCK)
-        path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM : COARSE_PATH_SIMPLE;
+    if (path == COARSE_PATH_TENSOR && !tensor_hvec_supports(op, nrhs)) path = COARSE_PATH_AUTO;
+    if (path == COARSE_PATH_AUTO || path == COARSE_PATH_BLOCK)
+        path = stream_supports(op->Nc, nrhs) ? COARSE_PATH_STREAM : tensor_hvec_supports(op, nrhs) ? COARSE_PATH_TENSOR : COARSE_PATH_SIMPLE;
     op->last_launches = 0;
+    if (path == COARSE_PATH_TENSOR) {
+        rc = launch_tensor_hvec(op, in_q_dev, in_norms_dev, out_dev, nrhs, dagger, st);
+        if (rc < 0) return rc;
+        op->last_launches = 1 + rc;
+        op->last_path = path;
+        op->links_fresh = false;
+        return COARSE_OK;
+    }
     if (path == COARSE_PATH_STREAM) {
         if (!stream_supports(op->Nc, nrhs))
             return fail(COARSE_EUNSUPPORTED, "apply_hvec: STREAM path does not cover Nc=%d nrhs=%d", op->Nc, nrhs);

@@ -99,7 +99,9 @@ struct TensorParams;
     int COARSE_CAT(launch_block_nc, NC)(const coarse_op* op, const BlockParams& p, int dagger, cudaStream_t stream); \
     int COARSE_CAT(launch_tensor_nc, NC)(const coarse_op* op, const TensorParams& p, int dagger, cudaStream_t stream); \
     int COARSE_CAT(launch_tensor_i8_nc, NC)(const coarse_op* op, const TensorParams& p, const void* u_other,           \
-                                            float* vscale, int dagger, cudaStream_t stream);
+                                            float* vscale, int dagger, cudaStream_t stream);                        \
+    int COARSE_CAT(launch_tensor_i8h_nc, NC)(const coarse_op* op, const TensorParams& p, const float* vnorms,          \
+                                             int dagger, cudaStream_t stream);
 COARSE_FOR_EACH_NC(COARSE_DECL_NC)
 #undef COARSE_DECL_NC
 

@@ -34,10 +34,10 @@ int launch_tensor_d(const coarse_op* op, const TensorParams& p, int dagger, cuda
 }
 
 // int16 links on the integer tensor cores (tensor_i8_kernel.cuh)
-template <int NC, int NP, bool DAG>
+template <int NC, int NP, bool DAG, bool HV = false>
 int launch_tensor_i8_t(const coarse_op* op, const TensorI8Params& p, cudaStream_t stream) {
-    using Gm = TensorI8Geom<NC, NP>;
-    auto kern = coarse_apply_tensor_i8<NC, NP, DAG>;
+    using Gm = TensorI8Geom<NC, NP, HV>;
+    auto kern = coarse_apply_tensor_i8<NC, NP, DAG, HV>;
     static SmemAttrCache attr_cache;
     cudaError_t e = ensure_dynamic_smem(kern, op->device, Gm::SMEM_BYTES, attr_cache);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(tensor-i8 kernel)");
@@ -68,6 +68,7 @@ int COARSE_CAT(launch_tensor_i8_nc, COARSE_NC)(const coarse_op* op, const Tensor
         p.t.width = base.nrhs - r0 < 16 ? base.nrhs - r0 : 16;
         p.vscale_w = gw;
         p.vscale_u = u_other ? gu : gw;
+        p.vnorms = nullptr;
         const long long total = (long long)op->lat.V * p.t.width;
         const unsigned blocks = (unsigned)((total + 127) / 128);
         vec_pow2_scale_kernel<<<blocks, 128, 0, stream>>>(base.in, op->lat.V, op->Nc, base.nrhs, r0, p.t.width, reinterpret_cast<float2*>(gw));
@@ -93,6 +94,39 @@ int COARSE_CAT(launch_tensor_i8_nc, COARSE_NC)(const coarse_op* op, const Tensor
             rc = dagger ? launch_tensor_i8_t<COARSE_NC, 8, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 8, false>(op, p, stream);
         else
             rc = dagger ? launch_tensor_i8_t<COARSE_NC, 16, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 16, false>(op, p, stream);
+        if (rc != COARSE_OK) return rc;
+        ++launches;
+    }
+    return launches > 0 ? launches - 1 : 0;
+}
+
+// int16 links AND int16 + norm vectors (coarse_op_apply_hvec with several right-hand sides): base.in holds int16 pairs,
+// no pre-pass (the components are the fixed-point operand).  One launch per group of up to 16 right-hand sides; returns
+// the number of launches beyond the first.
+int COARSE_CAT(launch_tensor_i8h_nc, COARSE_NC)(const coarse_op* op, const TensorParams& base, const float* vnorms, int dagger,
+                                                cudaStream_t stream) {
+    int launches = 0;
+    for (int r0 = 0; r0 < base.nrhs; r0 += 16) {
+        TensorI8Params p;
+        p.t = base;
+        p.t.r0 = r0;
+        p.t.width = base.nrhs - r0 < 16 ? base.nrhs - r0 : 16;
+        p.vscale_w = p.vscale_u = nullptr;
+        p.vnorms = vnorms;
+        int rc = COARSE_OK;
+        bool done = false;
+        if constexpr (TensorI8Geom<COARSE_NC, 4, true>::OK) {
+            if (p.t.width <= 4) {
+                rc = dagger ? launch_tensor_i8_t<COARSE_NC, 4, true, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 4, false, true>(op, p, stream);
+                done = true;
+            }
+        }
+        if (done)
+            ;
+        else if (p.t.width <= 8)
+            rc = dagger ? launch_tensor_i8_t<COARSE_NC, 8, true, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 8, false, true>(op, p, stream);
+        else
+            rc = dagger ? launch_tensor_i8_t<COARSE_NC, 16, true, true>(op, p, stream) : launch_tensor_i8_t<COARSE_NC, 16, false, true>(op, p, stream);
         if (rc != COARSE_OK) return rc;
         ++launches;
     }

@@ -28,6 +28,8 @@
 // the RHS column tiles are those of tensor_kernel.cuh; a stage is KC = 32 complex columns (16 for Nc = 48).
 // Bit-identical run to run (integer accumulation, fixed schedule).
 #pragma once
+#include <type_traits>
+
 #include "tensor_kernel.cuh"
 
 #ifndef COARSE_TENSOR_RING_BYTES
@@ -45,9 +47,18 @@ struct TensorI8Params {
     TensorParams t;
     const float* vscale_w;    // [V][TENSOR_I8_GP][2] = (g, 1/g) of columns r0.. of the hopping operand w (plain apply: of `in`)
     const float* vscale_u;    // the same for the local operand u (plain apply: = vscale_w)
+    const float* vnorms;      // HV kernels: `t.in` holds int16 (re, im) pairs [V][Nc][nrhs] and this the fp32 norm per (site, rhs)
 };
 
-template <int NC, int NP>
+// HV = half-precision VECTORS (16-bit fixed point with a per-site fp32 norm) on top of the 16-bit links
+// (L99) - the paper's own storage for both operands.  An int16 vector component q = 256 b1 + b0 is already fixed point:
+// its two bytes ARE the digits (b1 signed, b0 unsigned), so the B operand needs no arithmetic either (two byte permutes per
+// entry, against 4 F2I + 16 integer instructions for three signed digits of an fp32 value), and there are two digit blocks
+// instead of three.  The two blocks differ in signedness, which an MMA fixes per operand: four MMAs per k-step
+//     W_0 = A0.B0 (u8 x u8)   W_1 = A0.B1 (u8 x s8) + A1.B0 (s8 x u8)   W_2 = A1.B1 (s8 x s8)
+// into three accumulator blocks; out += f_m ((W_2 256 + W_1) 256 + W_0), f_m = link scale x coefficient x vector norm.
+// Both operands enter the tensor core exactly; the only rounding is the fp32 recombination in the epilogue.
+template <int NC, int NP, bool HV = false>
 struct TensorI8Geom {
     static constexpr int NT = NC > 128 ? 2 : 1;
     static constexpr int MT = NC / NT;
@@ -62,7 +73,8 @@ struct TensorI8Geom {
     static constexpr int SLAB_BYTES = MT * KC * 4;             // one site's slab of a stage
     static constexpr int SLAB_PITCH = NS == 2 ? 64 * KC * 4 : SLAB_BYTES;
     static constexpr int LINK_STAGE = NS * SLAB_PITCH;
-    static constexpr int NB3 = 3 * 2 * NPS;                    // MMA N: three digit blocks of (per site) [Re out | Im out]
+    static constexpr int NDIG = HV ? 2 : 3;                    // digit blocks of the B operand
+    static constexpr int NB3 = NDIG * 2 * NPS;                 // B tile columns: NDIG digit blocks of (per site) [Re out | Im out]
     static constexpr int B_STAGE = 2 * KC * NB3;               // int8 B tile of a stage, bytes
     static constexpr int B_SBO = (2 * KC / 16) * 128;          // byte stride between 8-column groups of n
     static constexpr int NE = KC * NPS / 128;                  // B entries per converter thread and stage
@@ -72,7 +84,7 @@ struct TensorI8Geom {
     static constexpr int A_COLS = 2 * A_HALF;                  // high bytes | low bytes
     static constexpr int D_COL0 = AS * A_COLS;
     static constexpr int DS = 3;
-    static constexpr int D_COLS = 4 * 2 * NPS;                 // W_0 .. W_3, each (per site) [Re out | Im out]
+    static constexpr int D_COLS = (NDIG + 1) * 2 * NPS;        // W_0 .. W_NDIG, each (per site) [Re out | Im out]
     static constexpr int FT = 8;                               // ring of per-matrix epilogue factor rows
     static constexpr int TMEM_COLS = 512;
     static constexpr int NG = COARSE_I8_NG, CONV_W0 = 2, EPI_W0 = CONV_W0 + 4 * NG;
@@ -80,7 +92,8 @@ struct TensorI8Geom {
     static constexpr int NBAR = 2 * LS + 2 * AS + 2 * DS;
     static constexpr int SMEM_BYTES = 1024 + LS * LINK_STAGE + AS * B_STAGE + FT * NPS * 4 + NBAR * 8 + 16;
     static constexpr bool OK = (NC % 16 == 0) && (MT % 8 == 0) && MT <= 128 && (NP == 4 || NP == 8 || NP == 16) && NE >= 1 && NB3 % 16 == 0 &&
-                               (D_COL0 + DS * D_COLS <= TMEM_COLS) && SMEM_BYTES <= 232448 && 2 * NC * 128 * 255 < (1 << 24);
+                               (D_COL0 + DS * D_COLS <= TMEM_COLS) && SMEM_BYTES <= 232448 &&
+                               (HV ? ((2 * NPS) % 16 == 0 && 2 * NC * 2 * 255 * 255 < (1 << 30)) : (2 * NC * 128 * 255 < (1 << 24)));
 };
 
 namespace ptx {
@@ -151,10 +164,11 @@ __device__ __forceinline__ void digit_regs(int b, int& t1, int& t2) {
 }
 __device__ __forceinline__ uint32_t pack_lo_bytes(int x, int y) { return __byte_perm((uint32_t)x, (uint32_t)y, 0x0040); }
 
-template <int NC, int NP, bool DAG>
-__global__ void __launch_bounds__(TensorI8Geom<NC, NP>::THREADS, 1)
+template <int NC, int NP, bool DAG, bool HV = false>
+__global__ void __launch_bounds__(TensorI8Geom<NC, NP, HV>::THREADS, 1)
 coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Params pp) {
-    using Gm = TensorI8Geom<NC, NP>;
+    using Gm = TensorI8Geom<NC, NP, HV>;
+    using VecT = typename std::conditional<HV, uint32_t, float2>::type;      // one complex vector component in memory
     static_assert(Gm::OK, "unsupported TENSOR-I8 geometry");
     constexpr int LS = Gm::LS, AS = Gm::AS, DS = Gm::DS, CHUNKS = Gm::CHUNKS, NT = Gm::NT, MT = Gm::MT, NE = Gm::NE;
     constexpr int KC = Gm::KC, LINK_STAGE = Gm::LINK_STAGE, B_STAGE = Gm::B_STAGE, B_SBO = Gm::B_SBO, NB3 = Gm::NB3, FT = Gm::FT;
@@ -164,6 +178,10 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
     constexpr uint32_t IDESC_U = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(NB3 >> 3) << 17) | ((128u >> 4) << 24);
     constexpr uint32_t IDESC_U1 = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(2 * NPS >> 3) << 17) | ((128u >> 4) << 24);   // one digit block
     constexpr uint32_t IDESC_U2 = (2u << 4) | (0u << 7) | (1u << 10) | ((uint32_t)(4 * NPS >> 3) << 17) | ((128u >> 4) << 24);   // two digit blocks
+    // HV: one digit block (N = 2 NPS) per MMA, every signedness combination of (A plane, B digit)
+    constexpr uint32_t IDESC_H0 = (2u << 4) | ((uint32_t)(2 * NPS >> 3) << 17) | ((128u >> 4) << 24);
+    constexpr uint32_t IDESC_UU = IDESC_H0, IDESC_US = IDESC_H0 | (1u << 10), IDESC_SU = IDESC_H0 | (1u << 7),
+                       IDESC_SS = IDESC_H0 | (1u << 7) | (1u << 10);
     const TensorParams& p = pp.t;
 
     extern __shared__ unsigned char smem_raw[];
@@ -278,7 +296,14 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
 #pragma unroll
                     for (int kk = 0; kk < Gm::KSTEPS; ++kk) {
                         const uint64_t db = db0 + (uint64_t)(kk * 256 >> 4);
-                        if (c == 0 && kk == 0) {
+                        if constexpr (HV) {
+                            const uint64_t db_hi = db + (uint64_t)(((2 * NPS >> 3) * B_SBO) >> 4);     // second digit block: high bytes
+                            const uint32_t acc = (c == 0 && kk == 0) ? 0u : 1u;                         // first k-step of the matrix overwrites
+                            ptx::mma_i8_ts(d0, a0 + kk * 8, db, IDESC_UU, acc);                         // W_0  = A0.B0
+                            ptx::mma_i8_ts(d0 + 2 * NPS, a0 + kk * 8, db_hi, IDESC_US, acc);            // W_1  = A0.B1
+                            ptx::mma_i8_ts(d0 + 2 * NPS, a1 + kk * 8, db, IDESC_SU, 1u);                // W_1 += A1.B0
+                            ptx::mma_i8_ts(d0 + 4 * NPS, a1 + kk * 8, db_hi, IDESC_SS, acc);            // W_2  = A1.B1
+                        } else if (c == 0 && kk == 0) {
                             // first k-step of the matrix: W_1 .. W_3 = high plane (overwrite), W_0 = low plane digit 0
                             // (overwrite), W_1, W_2 += low plane digits 1, 2
                             ptx::mma_i8_ts(d1, a1, db, IDESC_S, 0u);
@@ -332,7 +357,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
 
         int n_it = 0, n_m = M0, n_c = grp, n_s = 0;
         SiteX n_cx = {};
-        const float2* n_vec = p.in;
+        const VecT* n_vec = reinterpret_cast<const VecT*>(p.in);
         float n_g = 0.f, n_f = 0.f;       // fixed-point scale g 2^22 of the operand, epilogue factor of the matrix
         auto load_item = [&]() {
             if (n_it < n_my) {
@@ -344,18 +369,23 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
             if (n_it < n_my) {
                 const int sv = stencil_site_x(p.lat, n_s, n_cx, n_m, DAG ? 1 : 0);
                 const int sm = DAG ? sv : n_s;
-                n_vec = (n_m == 0 ? p.in_local : p.in) + (int64_t)sv * NC * p.nrhs + p.r0;
+                n_vec = reinterpret_cast<const VecT*>(n_m == 0 ? p.in_local : p.in) + (int64_t)sv * NC * p.nrhs + p.r0;
+                if constexpr (HV) {
+                    const float nm = r_valid ? __ldg(pp.vnorms + (int64_t)sv * p.nrhs + p.r0 + my_r) : 0.f;
+                    n_f = (n_m == 0 ? p.alpha : p.beta) * __ldg(p.scales + (int64_t)sm * 9 + n_m) * nm;
+                    return;
+                }
                 const float2 gs = r_valid ? __ldg(reinterpret_cast<const float2*>(n_m == 0 ? pp.vscale_u : pp.vscale_w) + (int64_t)sv * TENSOR_I8_GP + my_r)
                                           : make_float2(0.f, 0.f);
                 n_g = gs.x * 4194304.f;
                 n_f = (n_m == 0 ? p.alpha : p.beta) * __ldg(p.scales + (int64_t)sm * 9 + n_m) * gs.y * (1.f / 4194304.f);
             }
         };
-        float2 vn[NE];
+        VecT vn[NE];
         auto fetch = [&]() {
 #pragma unroll
             for (int x = 0; x < NE; ++x)
-                vn[x] = (n_it < n_my && r_valid) ? __ldg(n_vec + (int64_t)(KC * n_c) * p.nrhs + b_off_vec[x]) : make_float2(0.f, 0.f);
+                vn[x] = (n_it < n_my && r_valid) ? __ldg(n_vec + (int64_t)(KC * n_c) * p.nrhs + b_off_vec[x]) : VecT{};
         };
         auto normalise = [&]() -> bool {
             bool item_changed = false;
@@ -373,7 +403,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
         for (uint32_t t = grp; t < total; t += NG) {
             const uint32_t slot = t % LS, ph = (t / LS) & 1u;
             const uint32_t as = t % AS, aph = (t / AS) & 1u;
-            float2 v[NE];
+            VecT v[NE];
 #pragma unroll
             for (int x = 0; x < NE; ++x) v[x] = vn[x];
             const float g = n_g, f = n_f;
@@ -428,6 +458,19 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
             const uint32_t bt = b_u32 + as * B_STAGE;
 #pragma unroll
             for (int x = 0; x < NE; ++x) {
+                if constexpr (HV) {
+                    // the int16 components are the fixed-point operand: low bytes (unsigned) into block 0, high bytes
+                    // (signed) into block 1; -q is formed in 32 bits (|q| <= 32767 by the quantiser; -32768 would still be
+                    // exact here: its two's complement bytes are taken from the 32-bit negative)
+                    const uint32_t w = v[x];
+                    const int re = (int)(w << 16) >> 16, im = (int)w >> 16;
+                    const int b1x = re, b1y = DAG ? im : -im;                                  // n = r      (-> Re out)
+                    const int b2x = im, b2y = DAG ? -re : re;                                  // n = NP + r (-> Im out)
+                    ptx::sts16(bt + b_o[x], pack_lo_bytes(b1x, b1y));
+                    ptx::sts16(bt + b_o[x] + D_STEP, __byte_perm((uint32_t)b1x, (uint32_t)b1y, 0x0051));
+                    ptx::sts16(bt + b_o[x] + N_STEP, pack_lo_bytes(b2x, b2y));
+                    ptx::sts16(bt + b_o[x] + N_STEP + D_STEP, __byte_perm((uint32_t)b2x, (uint32_t)b2y, 0x0051));
+                } else {
                 const float vx = v[x].x * g, vy = v[x].y * g;
                 const int b1x = __float2int_rn(vx), b1y = __float2int_rn(DAG ? vy : -vy);     // n = r      (-> Re out)
                 const int b2x = __float2int_rn(vy), b2y = __float2int_rn(DAG ? -vx : vx);     // n = NP + r (-> Im out)
@@ -442,6 +485,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                 ptx::sts16(bt + b_o[x] + N_STEP, pack_lo_bytes(b2x, b2y));
                 ptx::sts16(bt + b_o[x] + N_STEP + D_STEP, pack_lo_bytes(x1, y1));
                 ptx::sts16(bt + b_o[x] + N_STEP + 2 * D_STEP, pack_lo_bytes(x2, y2));
+                }
             }
             // epilogue factor of this matrix and column: written by the group that converts the matrix's first chunk
             if (first_chunk && (gtid & (0x1f & ~((1 << RB) - 1))) == 0 && gtid < 64) {
@@ -483,14 +527,14 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
 #pragma unroll
                 for (int pc = 0; pc < 2 * NP / 8; ++pc) {
                     uint32_t w3[8], w2[8], w1[8], w0[8];
-                    ptx::tmem_ld8(d_t + 3 * 2 * NPS + 8 * pc, w3);
+                    if constexpr (!HV) ptx::tmem_ld8(d_t + 3 * 2 * NPS + 8 * pc, w3);
                     ptx::tmem_ld8(d_t + 2 * 2 * NPS + 8 * pc, w2);
                     ptx::tmem_ld8(d_t + 1 * 2 * NPS + 8 * pc, w1);
                     ptx::tmem_ld8(d_t + 8 * pc, w0);
                     ptx::tc_wait_ld();
 #pragma unroll
                     for (int n = 0; n < 8; ++n) {
-                        float S = fmaf((float)(int)w3[n], 256.f, (float)(int)w2[n]);
+                        float S = HV ? (float)(int)w2[n] : fmaf((float)(int)w3[n], 256.f, (float)(int)w2[n]);
                         S = fmaf(S, 256.f, (float)(int)w1[n]);
                         S = fmaf(S, 256.f, (float)(int)w0[n]);
                         float fr;

@@ -32,7 +32,7 @@ def _quantise(oracle_lib, v, Nc, nrhs):
     return q, nm, q_ref, nm_ref
 
 
-def _run(oracle_lib, dims, Nc, prec, nrhs, dagger, path, opts=None):
+def _run(oracle_lib, dims, Nc, prec, nrhs, dagger, path, opts=None, launches=1, pin_path=True):
     V = synth.lattice_volume(dims)
     links = synth.make_arbitrary_links(dims, Nc, 55, device="cuda")
     scales = scales_h = None
@@ -49,12 +49,14 @@ def _run(oracle_lib, dims, Nc, prec, nrhs, dagger, path, opts=None):
         v[2] = 0
     q, nm, q_h, nm_h = _quantise(oracle_lib, v, Nc, nrhs)
     out = torch.full((V, Nc, nrhs), complex(float("nan"), float("nan")), dtype=torch.complex64, device="cuda")
-    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales).set_option(cop.OPT_PATH, path)
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    if pin_path:
+        op.set_option(cop.OPT_PATH, path)
     for k, val in (opts or {}).items():
         op.set_option(k, val)
     op.apply_hvec(q, nm, out, nrhs=nrhs, dagger=dagger)
     torch.cuda.synchronize()
-    assert op.last_path == path and op.last_launches == 1
+    assert op.last_path == path and op.last_launches == launches
     ref = oracle_lib.coarse_apply_hvec(dims, Nc, links.cpu().numpy(), q_h, nm_h, nrhs=nrhs, dagger=dagger,
                                        link_precision=prec, scales=scales_h)
     got = out.cpu().numpy()
@@ -87,6 +89,63 @@ def test_hvec_stream_any_grid(oracle_lib, grid, stages):
 def test_hvec_simple(oracle_lib, nrhs, prec, dagger):
     _run(oracle_lib, (3, 2, 2, 2), 8, prec, nrhs, dagger, cop.PATH_SIMPLE)
     _run(oracle_lib, (2, 2, 1, 2), 48, prec, nrhs, dagger, cop.PATH_SIMPLE)
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 3, 3, 5), (1, 1, 1, 1)])
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("nrhs", [2, 3, 8, 11, 16, 19])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_hvec_tensor_int16_links_int16_vectors(oracle_lib, dims, Nc, nrhs, dagger):
+    """Several right-hand sides with the paper's storage for BOTH operands (16-bit links; 16-bit vectors
+    with a per-site norm, L97) on the integer tensor cores: link bytes and vector bytes are the int8 operands, int32
+    accumulation is exact.  Every compiled Nc (two sites per MMA tile at Nc <= 64: odd site count 135), 4-, 8- and
+    16-wide column tiles, ragged widths, more than 16 columns (two launches); AUTO picks this path."""
+    if Nc >= 96 and dims != (1, 1, 1, 1):
+        dims = (2, 4, 2, 2) if dims == (4, 4, 4, 4) else (3, 1, 3, 2)
+    _run(oracle_lib, dims, Nc, cop.LINK_I16, nrhs, dagger, cop.PATH_TENSOR, launches=(nrhs + 15) // 16, pin_path=False)
+
+
+@pytest.mark.parametrize("grid", [1, 7])
+def test_hvec_tensor_any_grid_and_single_rhs(oracle_lib, grid):
+    """One CTA walking every item (rings wrap many times) and a ragged grid; 1 RHS on the tensor kernel when pinned."""
+    for dagger in (0, 1):
+        _run(oracle_lib, (3, 3, 3, 5), 64, cop.LINK_I16, 8, dagger, cop.PATH_TENSOR, opts={cop.OPT_GRID: grid})
+        _run(oracle_lib, (5, 3, 2, 3), 128, cop.LINK_I16, 16, dagger, cop.PATH_TENSOR, opts={cop.OPT_GRID: grid})
+        _run(oracle_lib, (3, 2, 1, 4), 48, cop.LINK_I16, 1, dagger, cop.PATH_TENSOR, opts={cop.OPT_GRID: grid})
+
+
+@pytest.mark.parametrize("Nc,nrhs,applies", [(64, 8, 800), (128, 16, 400)])
+def test_hvec_tensor_bit_reproducible_under_stress(Nc, nrhs, applies):
+    """Integer accumulation and a fixed schedule: every apply must equal the first one bit for bit (~55 work items per
+    CTA; the link-slot release race of tests/test_gpu_parity.py's stress test would show up here the same way)."""
+    dims = (8, 8, 8, 16)
+    V = synth.lattice_volume(dims)
+    lc = synth.make_arbitrary_links(dims, Nc, 5, device="cuda")
+    lq = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+    scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+    cop.coarse_op_quantize_i16(lc, Nc, lq, scales)
+    del lc
+    v = synth.make_vectors(dims, Nc, nrhs, 6, device="cuda")
+    q = torch.empty((V, Nc, nrhs, 2), dtype=torch.int16, device="cuda")
+    nm = torch.empty((V, nrhs), dtype=torch.float32, device="cuda")
+    cop.coarse_op_quantize_vec_i16(v, Nc, nrhs, q, nm)
+    op = cop.CoarseOp(dims, Nc, cop.LINK_I16).set_links(lq, scales)
+    refs = {}
+    for dagger in (0, 1):
+        refs[dagger] = torch.empty_like(v)
+        op.apply_hvec(q, nm, refs[dagger], nrhs=nrhs, dagger=dagger)
+    assert op.last_path == cop.PATH_TENSOR
+    out = torch.empty_like(v)
+    bad = 0
+    for it in range(applies):
+        op.apply_hvec(q, nm, out, nrhs=nrhs, dagger=it % 2)
+        bad += int(not torch.equal(torch.view_as_real(out), torch.view_as_real(refs[it % 2])))
+    assert bad == 0, f"{bad} of {applies} applies differ from the first one"
+    op.close()
+
+
+def test_hvec_multi_rhs_complex64_links_stay_on_simple(oracle_lib):
+    _run(oracle_lib, (2, 2, 1, 2), 48, cop.LINK_C64, 3, 0, cop.PATH_SIMPLE, pin_path=False)
 
 
 def test_hvec_full_size_c4_whole_lattice(oracle_lib):
