@@ -68,7 +68,8 @@ struct TensorI8Geom {
     // Two sites per work item when the matrices have at most 64 rows and the 8-wide column tile is in use (the
     // accumulator ring of the 16-wide tile would not fit tensor memory): site 0 in TMEM lanes 0.., site 1 in lanes
     // 64.., their B operands side by side along N inside every digit block (see TensorGeom::NS in tensor_kernel.cuh).
-    static constexpr int NS = (MT <= 64 && NP <= 8) ? 2 : 1;     // (a 4-wide column tile for 2-4 right-hand sides exists in this mode only)
+    static constexpr int NS = (MT <= 64 && (NP <= 8 || HV)) ? 2 : 1;   // (a 4-wide column tile for 2-4 right-hand sides exists in this mode only;
+                                                                       //  HV: three accumulator blocks, so the 16-wide tile fits too, with a ring of 2)
     static constexpr int NPS = NP * NS;                        // right-hand-side columns of an item (all its sites)
     static constexpr int SLAB_BYTES = MT * KC * 4;             // one site's slab of a stage
     static constexpr int SLAB_PITCH = NS == 2 ? 64 * KC * 4 : SLAB_BYTES;
@@ -83,8 +84,8 @@ struct TensorI8Geom {
     static constexpr int A_HALF = KC / 2;                      // TMEM columns of one byte plane (4 int8 per column)
     static constexpr int A_COLS = 2 * A_HALF;                  // high bytes | low bytes
     static constexpr int D_COL0 = AS * A_COLS;
-    static constexpr int DS = 3;
     static constexpr int D_COLS = (NDIG + 1) * 2 * NPS;        // W_0 .. W_NDIG, each (per site) [Re out | Im out]
+    static constexpr int DS = tensor_clamp((512 - D_COL0) / D_COLS, 2, 3);   // accumulator ring depth
     static constexpr int FT = 8;                               // ring of per-matrix epilogue factor rows
     static constexpr int TMEM_COLS = 512;
     static constexpr int NG = COARSE_I8_NG, CONV_W0 = 2, EPI_W0 = CONV_W0 + 4 * NG;
@@ -338,8 +339,9 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
         // bits 2-4 = j mod 8 -, bit 5 = r div 8 (NP = 16) or the site sg (two sites per item), rest = the high part of j:
         // the 32 lanes of a 16-bit store touch 16 distinct words in 16 distinct banks (conflict-free).
         constexpr int RB = NP >= 8 ? 3 : 2, JB = 5 - RB;              // lane bits of r and of j
-        const int my_r = (gtid & ((1 << RB) - 1)) + (NP == 16 ? ((gtid >> 5) & 1) * 8 : 0);
-        const int my_sg = NS == 2 ? (gtid >> 5) & 1 : 0;              // every B entry of a thread belongs to ONE site of the item
+        constexpr int R8B = NP == 16 ? 1 : 0;                         // thread-index bit 5 = r div 8 (16-wide tile), the next bit = site
+        const int my_r = (gtid & ((1 << RB) - 1)) + (R8B ? ((gtid >> 5) & 1) * 8 : 0);
+        const int my_sg = NS == 2 ? (gtid >> (5 + R8B)) & 1 : 0;      // every B entry of a thread belongs to ONE site of the item
         const int my_n = my_sg * 2 * NP + my_r;                       // column inside a digit block
         const bool r_valid = my_r < p.width;
         int b_off_vec[NE];
@@ -347,7 +349,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
 #pragma unroll
         for (int x = 0; x < NE; ++x) {
             const int e = gtid + 128 * x;
-            const int j = ((e >> RB) & ((1 << JB) - 1)) + (1 << JB) * (e >> ((NP == 16 || NS == 2) ? 6 : 5));
+            const int j = ((e >> RB) & ((1 << JB) - 1)) + (1 << JB) * (e >> (5 + R8B + (NS == 2 ? 1 : 0)));
             b_off_vec[x] = j * p.nrhs + my_r;
             const int k = 2 * j;
             b_o[x] = (uint32_t)(k >> 4) * 128u + (uint32_t)(my_n >> 3) * B_SBO + (uint32_t)(my_n & 7) * 16u + (uint32_t)(k & 15);
@@ -488,7 +490,7 @@ coarse_apply_tensor_i8(const __grid_constant__ CUtensorMap link_map, TensorI8Par
                 }
             }
             // epilogue factor of this matrix and column: written by the group that converts the matrix's first chunk
-            if (first_chunk && (gtid & (0x1f & ~((1 << RB) - 1))) == 0 && gtid < 64) {
+            if (first_chunk && (gtid & (0x1f & ~((1 << RB) - 1))) == 0 && gtid < (32 << (R8B + (NS == 2 ? 1 : 0)))) {
                 // threads 0-7 (and 32-39 for NP = 16 / the second site) of the group hold r = 0..7 (8..15 / r = 0..7 of site 1);
                 // 4-wide tile: threads 0-3 and 32-35
                 asm volatile("st.shared.f32 [%0], %1;" ::"r"(ft_u32 + (uint32_t)(((t / CHUNKS) % FT) * NPS + my_sg * NP + my_r) * 4u), "f"(f) : "memory");
