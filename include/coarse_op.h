@@ -109,7 +109,8 @@ enum {
                                 team (2 = 14).  With it COARSE_OPT_STAGES is the ring's slot count. */
     COARSE_OPT_TENSOR_I8 = 8  /* TENSOR path on int16 links: 0 auto / 2: the integer tensor-core kernel (csrc/tensor_i8_kernel.cuh:
                                 link entries as two int8 planes, exact, vectors in 23-bit fixed point per site), 1: the
-                                3xTF32 kernel.  Site-range launches of coarse_op_apply_host always use the latter. */
+                                3xTF32 kernel.  Site-range launches of coarse_op_apply_host always use the latter;
+                                coarse_op_apply_hvec and coarse_op_apply_static (integer kernel only) ignore the option. */
 };
 
 /* Create an operator descriptor for a periodic lattice dims[0..3] (each >= 1), Nc even and
@@ -214,7 +215,8 @@ int coarse_op_quantize_vec_i16(const void* v_c64_dev, int64_t n_sites, int Nc, i
  * pipelined: the lattice is cut into 4 ranges of x3-slices (8 when the vectors are 32 MiB or more), each launched as
  * soon as the slices it reads are on the device, its result copied back while the next range computes (H2D, kernels
  * and D2H on three streams, two of them owned by the handle); the result is bit-identical to coarse_op_apply's (int16
- * links with 5 or more right-hand sides: to its result with COARSE_OPT_TENSOR_I8 = 1, see there). */
+ * links on the TENSOR path, i.e. several right-hand sides: to its result with COARSE_OPT_PATH = COARSE_PATH_TENSOR and
+ * COARSE_OPT_TENSOR_I8 = 1, see there). */
 int coarse_op_apply_host(coarse_op_t* op, const void* in_host, void* out_host, int nrhs, int dagger,
                          void* stream);
 
