@@ -168,7 +168,7 @@ int coarse_op_apply_parts(coarse_op_t* op, const void* u_dev, const void* w_dev,
  * int16_t[V][Nc][nrhs][2], in_norms_dev = float[V][nrhs].  The output is complex64 (coarse_op_apply_hout adds the
  * half-precision result).  Nc % 4 == 0.
  * nrhs = 1 runs on the STREAM kernels (the norm is folded into the vector operand like the int16
- * link scale).  Several right-hand sides on int16 links - the paper's storage for both operands (L97, L99) - run on
+ * link scale; int16 links on large lattices: the warp-team kernel, as for complex64 vectors).  Several right-hand sides on int16 links - the paper's storage for both operands (L97, L99) - run on
  * the integer tensor cores (COARSE_PATH_TENSOR; one launch per 16 columns): the two bytes of an int16 link entry and
  * of an int16 vector component are the int8 operands, int32 accumulation is exact, and the only rounding is the fp32
  * recombination by link scale x vector norm in the epilogue.  Complex64 links with several right-hand sides: SIMPLE. */

@@ -84,9 +84,9 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
 }
 
 // Team-owned stages (stream2_kernel.cuh): plain apply on the whole lattice or a site range, no PDL.
-template <int NC, bool I16, bool DAG, int TW>
+template <int NC, bool I16, bool DAG, int TW, bool HV = false>
 int launch_stream2_w(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
-    using Gm = Stream2Geom<NC, I16, TW>;
+    using Gm = Stream2Geom<NC, I16, TW, HV>;
     if constexpr (!Gm::OK) {
         return fail(COARSE_EUNSUPPORTED, "STREAM (warp teams): no geometry for Nc=%d with %d warps per team", NC, TW);
     } else {
@@ -110,7 +110,7 @@ int launch_stream2_w(const coarse_op* op, const StreamParams& base, cudaStream_t
         if (slots > fit) return fail(COARSE_EUNSUPPORTED, "STREAM (warp teams): shared memory too small for Nc=%d", NC);
         p.stages = slots;
         const int smem = Gm::smem_bytes(DAG, slots);
-        auto kern = coarse_apply_stream2<NC, I16, DAG, TW>;
+        auto kern = coarse_apply_stream2<NC, I16, DAG, TW, HV>;
         static SmemAttrCache attr_cache;
         cudaError_t e = ensure_dynamic_smem(kern, op->device, smem, attr_cache);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream2 kernel)");
@@ -127,21 +127,21 @@ int launch_stream2_w(const coarse_op* op, const StreamParams& base, cudaStream_t
 
 // COARSE_OPT_WARP_ITEMS: 2 = default team width (4 warps: two teams; measured best on C4 and P2, where
 // its default ring of 8 slots has the 6 x 16 KB in flight the read stream peaks at), 12 / 14 = 2 / 4 warps
-template <int NC, bool I16, bool DAG>
+template <int NC, bool I16, bool DAG, bool HV = false>
 int launch_stream2_t(const coarse_op* op, const StreamParams& base, cudaStream_t stream) {
     // rows of 24 / 48 quads (Nc = 96 / 192 int16) run best with 2 warps per team (measured: Nc 96 6.6 / 6.8 TB/s
     // against 6.0 / 6.7 with 4 and 5.4 / 5.4 on the cooperative kernel), the others with 4
     constexpr bool has4 = Stream2Geom<NC, I16, 4>::OK, has2 = Stream2Geom<NC, I16, 2>::OK;
     const bool two = !has4 || (has2 && (op->warp_items_opt == 12 || (op->warp_items_opt != 14 && (NC % 3 == 0 || NC == 32))));
-    if (two) return launch_stream2_w<NC, I16, DAG, 2>(op, base, stream);
-    return launch_stream2_w<NC, I16, DAG, 4>(op, base, stream);
+    if (two) return launch_stream2_w<NC, I16, DAG, 2, HV>(op, base, stream);
+    return launch_stream2_w<NC, I16, DAG, 4, HV>(op, base, stream);
 }
 
 template <int NC, bool I16>
 bool use_warp_items(const coarse_op* op, const StreamParams& p, int dagger, bool gen) {
     // (site-range launches take the decision the full-lattice apply takes, so that coarse_op_apply_host stays
     // bit-identical to coarse_op_apply)
-    if (gen || p.vnorms || p.hout_q || p.pdl || op->warp_items_opt == 1) return false;
+    if (gen || (p.vnorms && !I16) || p.hout_q || p.pdl || op->warp_items_opt == 1) return false;   // (half vectors: int16 links only)
     if (op->warp_items_opt >= 2) return true;
     // auto: int16 links with Nc >= 48 (issue-bound on the cooperative kernel; Nc = 48: 5.5 / 5.2 -> 6.3 / 6.4 TB/s with
     // 2 warps per team) and the 4-8 KB matrices of Nc = 32 (the cooperative kernel pays its per-stage handshake eight
@@ -177,6 +177,12 @@ int launch_stream_nc(const coarse_op* op, const StreamParams& p, int dagger, cud
 template <int NC>
 int launch_stream_g(const coarse_op* op, const StreamParams& p, int dagger, bool gen, cudaStream_t stream) {
     if (p.vnorms) {   // half-precision input vectors: regular geometry, plain apply
+        if (op->prec == COARSE_LINK_I16) {
+            // the paper's storage for both operands: warp teams on large lattices, as for complex64 vectors
+            if constexpr (Stream2Geom<NC, true, 4>::OK || Stream2Geom<NC, true, 2>::OK)
+                if (use_warp_items<NC, true>(op, p, dagger, gen))
+                    return dagger ? launch_stream2_t<NC, true, true, true>(op, p, stream) : launch_stream2_t<NC, true, false, true>(op, p, stream);
+        }
         if (op->prec == COARSE_LINK_I16)
             return dagger ? launch_stream_t<NC, true, true, false, false, true>(op, p, stream)
                           : launch_stream_t<NC, true, false, false, false, true>(op, p, stream);

@@ -70,7 +70,9 @@ constexpr int stream2_rows(int nc, int rowbytes, int unit, int max_bytes, int ma
     return best;
 }
 
-template <int NC, bool I16, int TW>
+// HV: half-precision input vectors (coarse_op_apply_hvec) - `in` holds int16 (re, im) pairs, the per-site
+// norm is folded into the per-matrix operand scale (as in stream_kernel.cuh), a vector stage is half the bytes.
+template <int NC, bool I16, int TW, bool HV = false>
 struct Stream2Geom {
     using G1 = StreamGeom<NC, I16, false, false, true>;      // all-lanes-busy lane mapping
     static constexpr int W = 8;                               // consumer warps
@@ -81,8 +83,9 @@ struct Stream2Geom {
     static constexpr int NB = NC / (RS > 0 ? RS : 1);
     static constexpr int WL = RS / (TW * RPL);                // warp-wide loads per warp, stage and pass
     static constexpr int LINK_STAGE = RS * ROWBYTES;
-    static constexpr int VEC_STAGE_N = NC * 8;
-    static constexpr int VEC_STAGE_D = RS * 8;
+    static constexpr int VEC_ENTRY = HV ? 4 : 8;
+    static constexpr int VEC_STAGE_N = NC * VEC_ENTRY;
+    static constexpr int VEC_STAGE_D = RS * VEC_ENTRY;
     static constexpr int RED_BYTES = T * 2 * (TW - 1) * NC * 8;               // dagger = 1 team reduction
     static constexpr bool OK = G1::OK && RS > 0 && QP == G && (TW == 2 || TW == 4);
     static constexpr int THREADS = (W + 1) * 32;
@@ -136,9 +139,11 @@ __device__ __forceinline__ int transpose_reduce(float2 (&acc)[NTOT], int lane_in
     }
 }
 
-template <int NC, bool I16, bool DAG, int TW>
-__global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_apply_stream2(StreamParams p) {
-    using Gm = Stream2Geom<NC, I16, TW>;
+template <int NC, bool I16, bool DAG, int TW, bool HV = false>
+__global__ void __launch_bounds__(Stream2Geom<NC, I16, TW, HV>::THREADS, 1) coarse_apply_stream2(StreamParams p) {
+    using Gm = Stream2Geom<NC, I16, TW, HV>;
+    constexpr int VE = Gm::VEC_ENTRY;
+    constexpr bool SCALED = I16 || HV;                    // the vector operand carries a per-matrix scale
     static_assert(Gm::OK, "unsupported STREAM2 geometry");
     constexpr int W = Gm::W, T = Gm::T, RS = Gm::RS, NB = Gm::NB, WL = Gm::WL, QP = Gm::QP, G = Gm::G, RPL = Gm::RPL;
     constexpr int PASSES = Gm::PASSES, CPQ = Gm::CPQ, ROWBYTES = Gm::ROWBYTES;
@@ -199,7 +204,7 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
                             const int sm = DAG ? sv : s;
                             const int r0 = DAG ? c * RS : (item % NB) * RS;
                             const unsigned char* mat = p.links + ((int64_t)sm * 9 + m) * ((int64_t)NC * ROWBYTES) + (int64_t)r0 * ROWBYTES;
-                            const unsigned char* vec = reinterpret_cast<const unsigned char*>(p.in) + ((int64_t)sv * NC + (DAG ? r0 : 0)) * 8;
+                            const unsigned char* vec = reinterpret_cast<const unsigned char*>(p.in) + ((int64_t)sv * NC + (DAG ? r0 : 0)) * VE;
                             if (ptx::elect_one()) {
                                 ptx::mbar_arrive_expect_tx(full0 + 8u * slot, LINK_STAGE + VEC_STAGE);
                                 ptx::bulk_g2s(link_u32 + slot * LINK_STAGE, mat, LINK_STAGE, full0 + 8u * slot, pol_links);
@@ -240,10 +245,14 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
     // int16: lane m (< 9) carries the fp32 scale of matrix m of the current item, fetched two items ahead
     float cur_scale = 1.f, next_scale = 1.f, next2_scale = 1.f;
     auto fetch_scale = [&](int item) -> float {
-        if (!I16 || lane >= 9 || item >= p.n_items) return 1.f;
+        if (!SCALED || lane >= 9 || item >= p.n_items) return 1.f;
         const int s = DAG ? item : item / NB;
-        const int sm = DAG ? stencil_site(p.lat, s, lane, 1) : s;
-        return __ldg(p.scales + (int64_t)sm * 9 + lane);
+        const int sv = (DAG || HV) ? stencil_site(p.lat, s, lane, DAG ? 1 : 0) : s;    // site of stage `lane`'s vector
+        const int sm = DAG ? sv : s;
+        float f = 1.f;
+        if constexpr (I16) f = __ldg(p.scales + (int64_t)sm * 9 + lane);
+        if constexpr (HV) f *= __ldg(p.vnorms + sv);                                  // half vectors: per-site norm folded in
+        return f;
     };
     next_scale = fetch_scale(item0);
     next2_scale = fetch_scale(item0 + item_stride);
@@ -257,12 +266,13 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
 
         if constexpr (!DAG) {
 #if COARSE_S2_PACKED_N
+            static_assert(!HV, "half vectors are implemented in the cmac<> formulation of dagger = 0");
             CAcc pacc[WL];
 #pragma unroll
             for (int k = 0; k < WL; ++k) pacc[k].a = pacc[k].b = make_float2(0.f, 0.f);
 #pragma unroll 1
             for (int m = 0; m < 9; ++m) {
-                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                const float sc = SCALED ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
                 ptx::mbar_wait(full0 + 8u * slot, phase);
                 const uint32_t lbase = link_u32 + slot * LINK_STAGE + (row0 * ROWBYTES + qi * 16);
                 const uint32_t vbase = vec_u32 + slot * VEC_STAGE;
@@ -311,7 +321,7 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
             for (int k = 0; k < WL; ++k) acc[k] = make_float2(0.f, 0.f);
 #pragma unroll 1
             for (int m = 0; m < 9; ++m) {
-                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                const float sc = SCALED ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
                 ptx::mbar_wait(full0 + 8u * slot, phase);
                 const uint32_t lbase = link_u32 + slot * LINK_STAGE + (row0 * ROWBYTES + qi * 16);
                 const uint32_t vbase = vec_u32 + slot * VEC_STAGE;
@@ -319,13 +329,27 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
 #pragma unroll
                 for (int ps = 0; ps < PASSES; ++ps) {
                     const int col0 = (ps * QP + qi) * CPQ;
+                    if constexpr (HV) {
+                        if constexpr (CPQ == 2) {
+                            const float2 t = ptx::lds64(vbase + col0 * 4);
+                            v[ps][0] = unpack_i16x2(__float_as_uint(t.x));
+                            v[ps][1] = unpack_i16x2(__float_as_uint(t.y));
+                        } else {
+                            const uint4 t = ptx::lds128u(vbase + col0 * 4);
+                            v[ps][0] = unpack_i16x2(t.x);
+                            v[ps][1] = unpack_i16x2(t.y);
+                            v[ps][2] = unpack_i16x2(t.z);
+                            v[ps][3] = unpack_i16x2(t.w);
+                        }
+                    } else {
 #pragma unroll
-                    for (int h = 0; h < CPQ / 2; ++h) {
-                        const float4 t = ptx::lds128(vbase + (col0 + 2 * h) * 8);
-                        v[ps][2 * h] = make_float2(t.x, t.y);
-                        v[ps][2 * h + 1] = make_float2(t.z, t.w);
+                        for (int h = 0; h < CPQ / 2; ++h) {
+                            const float4 t = ptx::lds128(vbase + (col0 + 2 * h) * 8);
+                            v[ps][2 * h] = make_float2(t.x, t.y);
+                            v[ps][2 * h + 1] = make_float2(t.z, t.w);
+                        }
                     }
-                    if constexpr (I16) {
+                    if constexpr (SCALED) {
 #pragma unroll
                         for (int e = 0; e < CPQ; ++e) { v[ps][e].x *= sc; v[ps][e].y *= sc; }
                     }
@@ -372,16 +396,23 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
                 for (int e = 0; e < CPQ; ++e) pacc[ps][e].a = pacc[ps][e].b = make_float2(0.f, 0.f);
 #pragma unroll 1
             for (int m = 0; m < 9; ++m) {
-                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                const float sc = SCALED ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
 #pragma unroll 1
                 for (int c = 0; c < NB; ++c) {
                     ptx::mbar_wait(full0 + 8u * slot, phase);
                     const uint32_t lbase = link_u32 + slot * LINK_STAGE + (row0 * ROWBYTES + qi * 16);
-                    const uint32_t vbase = vec_u32 + slot * VEC_STAGE + row0 * 8;
+                    const uint32_t vbase = vec_u32 + slot * VEC_STAGE + row0 * VE;
 #pragma unroll
                     for (int k = 0; k < WL; ++k) {
-                        float2 vj = ptx::lds64(vbase + k * (RPL * 8));
-                        if constexpr (I16) { vj.x *= sc; vj.y *= sc; }
+                        float2 vj;
+                        if constexpr (HV) {
+                            uint32_t w;
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w) : "r"(vbase + k * (RPL * 4)));
+                            vj = unpack_i16x2(w);
+                        } else {
+                            vj = ptx::lds64(vbase + k * (RPL * 8));
+                        }
+                        if constexpr (SCALED) { vj.x *= sc; vj.y *= sc; }
                         const VDup vd = vdup(vj);
 #pragma unroll
                         for (int ps = 0; ps < PASSES; ++ps) {
@@ -412,6 +443,7 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
 #pragma unroll
                 for (int e = 0; e < CPQ; ++e) acc[ps][e] = cfinal<true>(pacc[ps][e]);
 #else
+            static_assert(!HV, "half vectors are implemented in the packed formulation of dagger = 1");
             float2 acc[PASSES][CPQ];
 #pragma unroll
             for (int ps = 0; ps < PASSES; ++ps)
@@ -419,7 +451,7 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW>::THREADS, 1) coarse_a
                 for (int e = 0; e < CPQ; ++e) acc[ps][e] = make_float2(0.f, 0.f);
 #pragma unroll 1
             for (int m = 0; m < 9; ++m) {
-                const float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
+                const float sc = SCALED ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
 #pragma unroll 1
                 for (int c = 0; c < NB; ++c) {
                     ptx::mbar_wait(full0 + 8u * slot, phase);

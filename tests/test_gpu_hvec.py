@@ -76,6 +76,20 @@ def test_hvec_stream(oracle_lib, dims, Nc, prec, dagger):
     _run(oracle_lib, dims, Nc, prec, 1, dagger, cop.PATH_STREAM)
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (3, 2, 1, 4), (5, 3, 4, 7)])
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("team", [12, 14])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_hvec_stream_warp_teams(oracle_lib, dims, Nc, team, dagger):
+    """int16 links AND int16 + norm vectors (the paper's storage for both, PAPER.md:L97 / L99) on the warp-team kernel
+    (stream2_kernel.cuh, what AUTO runs on large lattices; forced here): 2 and 4 warps per team, ragged last round."""
+    if Nc >= 128 and dims == (5, 3, 4, 7):
+        dims = (5, 3, 2, 3)
+    _run(oracle_lib, dims, Nc, cop.LINK_I16, 1, dagger, cop.PATH_STREAM, opts={cop.OPT_WARP_ITEMS: team})
+    if dims == (3, 2, 1, 4):
+        _run(oracle_lib, (5, 3, 2, 3), Nc, cop.LINK_I16, 1, dagger, cop.PATH_STREAM, opts={cop.OPT_WARP_ITEMS: team, cop.OPT_GRID: 3})
+
+
 @pytest.mark.parametrize("grid,stages", [(1, 2), (7, 3), (1000, 12)])
 def test_hvec_stream_any_grid(oracle_lib, grid, stages):
     for dagger in (0, 1):
