@@ -180,7 +180,8 @@ int coarse_op_apply_hvec(coarse_op_t* op, const void* in_q_dev, const float* in_
  * exactly what coarse_op_quantize_vec_i16 makes of out_c64_dev (norm = max|component| / 32767, q = clamp(rint(component /
  * norm))).  in_norms_dev = NULL: in_dev is a complex64 vector; else the half-precision input of coarse_op_apply_hvec.
  * For 1 RHS on the STREAM kernels it is ONE launch: a CTA owns whole sites (all row blocks of a site in a row), keeps
- * the site's rows in shared memory and ends each site with a CTA-local epilogue (norm, 16-bit vector).  Other
+ * the site's rows in shared memory and ends each site with a CTA-local epilogue (norm, 16-bit vector); int16 links on
+ * large lattices: the warp-team kernel, where a team of warps holds a whole site (dagger 1; dagger 0 for Nc <= 64).  Other
  * nrhs / shapes: the apply followed by the vector quantiser.  The three vector buffers must not overlap. */
 int coarse_op_apply_hout(coarse_op_t* op, const void* in_dev, const float* in_norms_dev, void* out_c64_dev, void* out_q_dev,
                          float* out_norms_dev, int nrhs, int dagger, void* stream);

@@ -141,7 +141,14 @@ template <int NC, bool I16>
 bool use_warp_items(const coarse_op* op, const StreamParams& p, int dagger, bool gen) {
     // (site-range launches take the decision the full-lattice apply takes, so that coarse_op_apply_host stays
     // bit-identical to coarse_op_apply)
-    if (gen || (p.vnorms && !I16) || p.hout_q || p.pdl || op->warp_items_opt == 1) return false;   // (half vectors: int16 links only)
+    if (gen || (p.vnorms && !I16) || p.pdl || op->warp_items_opt == 1) return false;   // (half vectors: int16 links only)
+    if (p.hout_q) {
+        // half-precision output: int16 links, and in dagger = 0 only when a work item is a whole site (a team then holds
+        // all rows of the site; otherwise the cooperative kernel's site-owning CTAs do it)
+        constexpr int nb4 = Stream2Geom<NC, I16, 4>::OK ? Stream2Geom<NC, I16, 4>::NB : 1;
+        constexpr int nb2 = Stream2Geom<NC, I16, 2>::OK ? Stream2Geom<NC, I16, 2>::NB : 1;
+        if (!I16 || (!dagger && (nb4 > 1 || nb2 > 1))) return false;
+    }
     if (op->warp_items_opt >= 2) return true;
     // auto: int16 links with Nc >= 48 (issue-bound on the cooperative kernel; Nc = 48: 5.5 / 5.2 -> 6.3 / 6.4 TB/s with
     // 2 warps per team) and the 4-8 KB matrices of Nc = 32 (the cooperative kernel pays its per-stage handshake eight

@@ -90,7 +90,8 @@ struct Stream2Geom {
     static constexpr bool OK = G1::OK && RS > 0 && QP == G && (TW == 2 || TW == 4);
     static constexpr int THREADS = (W + 1) * 32;
     static constexpr int stage_bytes(bool dag) { return LINK_STAGE + (dag ? VEC_STAGE_D : VEC_STAGE_N); }
-    static constexpr int fixed_bytes(bool dag) { return (dag ? RED_BYTES : 0) + 128; }
+    static constexpr int HOUT_BYTES = 2 * W * 4;                              // half-precision output: per-warp maxima, double buffered
+    static constexpr int fixed_bytes(bool dag) { return (dag ? RED_BYTES : 0) + 128 + HOUT_BYTES; }
     static int smem_bytes(bool dag, int slots) { return slots * (stage_bytes(dag) + 16) + fixed_bytes(dag); }
 };
 
@@ -139,6 +140,17 @@ __device__ __forceinline__ int transpose_reduce(float2 (&acc)[NTOT], int lane_in
     }
 }
 
+// Half-precision output (coarse_op_apply_hout): 16-bit component of x for the site norm `norm` (amax = 32767 norm), the
+// arithmetic of quantize_vec_i16_kernel (R22).
+__device__ __forceinline__ short2 half_out_q(float2 x, float amax, float norm) {
+    short2 o = make_short2(0, 0);
+    if (amax != 0.f) {
+        o.x = (short)fminf(32767.f, fmaxf(-32767.f, rintf(__fdiv_rn(x.x, norm))));
+        o.y = (short)fminf(32767.f, fmaxf(-32767.f, rintf(__fdiv_rn(x.y, norm))));
+    }
+    return o;
+}
+
 template <int NC, bool I16, bool DAG, int TW, bool HV = false>
 __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW, HV>::THREADS, 1) coarse_apply_stream2(StreamParams p) {
     using Gm = Stream2Geom<NC, I16, TW, HV>;
@@ -158,6 +170,7 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW, HV>::THREADS, 1) coar
     uint64_t* bars = reinterpret_cast<uint64_t*>(red_smem + (DAG ? Gm::RED_BYTES : 0));
     const uint32_t full0 = ptx::smem_u32(bars);
     const uint32_t empty0 = full0 + 8u * S;
+    float* hmax = reinterpret_cast<float*>(bars + 2 * S);            // [2][W]: half-precision output (dagger = 0)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
@@ -387,6 +400,34 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW, HV>::THREADS, 1) coar
 #pragma unroll
                 for (int j = 0; j < NF; ++j) p.out[(int64_t)s * NC + rb * RS + row0 + (k0 + j) * RPL] = acc[j];
             }
+            if constexpr (NB == 1) {
+                // half-precision result beside it (the launcher sends hout here only when an item is a whole site): the
+                // site's rows are spread over the team's lanes, so the team takes the maximum through hmax[buf][warp]
+                // behind ONE team-wide named barrier (double buffered: the next item's barrier orders the reuse), then every
+                // lane quantises the rows it holds
+                if (p.hout_q) {
+                    float amax = 0.f;
+                    if ((qi & PLAIN) == 0) {
+#pragma unroll
+                        for (int j = 0; j < NF; ++j) amax = fmaxf(amax, fmaxf(fabsf(acc[j].x), fabsf(acc[j].y)));
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+                    if (lane == 0) hmax[red_buf * W + warp] = amax;
+                    ptx::named_bar_sync(1 + team, TW * 32);
+                    amax = 0.f;
+#pragma unroll
+                    for (int w = 0; w < TW; ++w) amax = fmaxf(amax, hmax[red_buf * W + team * TW + w]);
+                    red_buf ^= 1;
+                    const float norm = amax == 0.f ? 0.f : __fdiv_rn(amax, 32767.0f);
+                    if (wi == 0 && lane == 0) p.hout_norms[s] = norm;
+                    if ((qi & PLAIN) == 0) {
+                        short2* hq = p.hout_q;
+#pragma unroll
+                        for (int j = 0; j < NF; ++j) hq[(int64_t)s * NC + row0 + (k0 + j) * RPL] = half_out_q(acc[j], amax, norm);
+                    }
+                }
+            }
         } else {
 #if COARSE_S2_PACKED_D
             CAcc pacc[PASSES][CPQ];
@@ -529,6 +570,27 @@ __global__ void __launch_bounds__(Stream2Geom<NC, I16, TW, HV>::THREADS, 1) coar
 #pragma unroll
                     for (int h = 0; h < CPQ / 2; ++h)
                         dst[h] = make_float4(acc[ps][2 * h].x, acc[ps][2 * h].y, acc[ps][2 * h + 1].x, acc[ps][2 * h + 1].y);
+                }
+            }
+            // half-precision result: the whole site sits in the grp == 0 lanes of the team's first warp - one warp-wide maximum
+            if (p.hout_q && wi == 0) {
+                float amax = 0.f;
+                if (grp == 0) {
+#pragma unroll
+                    for (int ps = 0; ps < PASSES; ++ps)
+#pragma unroll
+                        for (int e = 0; e < CPQ; ++e) amax = fmaxf(amax, fmaxf(fabsf(acc[ps][e].x), fabsf(acc[ps][e].y)));
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+                const float norm = amax == 0.f ? 0.f : __fdiv_rn(amax, 32767.0f);
+                if (lane == 0) p.hout_norms[s] = norm;
+                if (grp == 0) {
+                    short2* hq = p.hout_q;
+#pragma unroll
+                    for (int ps = 0; ps < PASSES; ++ps)
+#pragma unroll
+                        for (int e = 0; e < CPQ; ++e) hq[(int64_t)s * NC + (ps * QP + qi) * CPQ + e] = half_out_q(acc[ps][e], amax, norm);
                 }
             }
         }

@@ -261,6 +261,20 @@ def test_half_precision_output_any_grid(oracle_lib, grid, fine):
         _run_hout(oracle_lib, (5, 3, 2, 3), 48, cop.LINK_C64, 1, dagger, True, opts={cop.OPT_GRID: grid})
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (5, 3, 2, 3)])
+@pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
+@pytest.mark.parametrize("team", [12, 14])
+@pytest.mark.parametrize("dagger", [0, 1])
+@pytest.mark.parametrize("half_in", [False, True])
+def test_half_precision_output_warp_teams(oracle_lib, dims, Nc, team, dagger, half_in):
+    """Half-precision output on the warp-team kernel (int16 links; what AUTO runs on large lattices): dagger 1 and, where a
+    work item is a whole site (Nc <= 64), dagger 0 - a team holds all rows of the site and takes the norm itself; the
+    other shapes fall back to the cooperative kernel's site-owning CTAs.  PDL off so that both repetitions take this path."""
+    if Nc >= 128 and dims == (4, 4, 4, 4):
+        dims = (2, 4, 2, 2)
+    _run_hout(oracle_lib, dims, Nc, cop.LINK_I16, 1, dagger, half_in, opts={cop.OPT_WARP_ITEMS: team, cop.OPT_PDL: 2}, want_launches=1)
+
+
 @pytest.mark.parametrize("nrhs", [3, 16])
 def test_half_precision_output_multi_rhs_two_pass(oracle_lib, nrhs):
     """Several right-hand sides: the apply (STREAM-MR / tensor kernels), then the vector quantiser."""
