@@ -158,6 +158,49 @@ def test_hvec_tensor_bit_reproducible_under_stress(Nc, nrhs, applies):
     op.close()
 
 
+@pytest.mark.parametrize("Nc,half_in", [(64, False), (64, True), (48, True), (128, False)])
+def test_half_output_warp_teams_bit_reproducible_under_stress(Nc, half_in):
+    """Half-precision output from the warp-team kernel on a lattice with many items per team: the 16-bit vectors, the norms
+    and the complex64 result of every apply must equal the first one's (the team-wide maximum goes through a double-buffered
+    shared-memory slot behind one named barrier per item)."""
+    dims, applies = (8, 8, 8, 16), 600
+    V = synth.lattice_volume(dims)
+    lc = synth.make_arbitrary_links(dims, Nc, 5, device="cuda")
+    lq = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+    scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+    cop.coarse_op_quantize_i16(lc, Nc, lq, scales)
+    del lc
+    v = synth.make_vectors(dims, Nc, 1, 6, device="cuda")
+    v[::7] *= 1e-3                                   # norms that differ from site to site
+    q = nm = None
+    if half_in:
+        q = torch.empty((V, Nc, 1, 2), dtype=torch.int16, device="cuda")
+        nm = torch.empty((V, 1), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_vec_i16(v, Nc, 1, q, nm)
+    op = cop.CoarseOp(dims, Nc, cop.LINK_I16).set_links(lq, scales)
+    src = q if half_in else v
+    refs = {}
+    for dagger in (0, 1):
+        refs[dagger] = (torch.empty_like(v), torch.empty((V, Nc, 1, 2), dtype=torch.int16, device="cuda"),
+                        torch.empty((V, 1), dtype=torch.float32, device="cuda"))
+        op.apply_hout(src, nm, *refs[dagger], dagger=dagger)
+    out, oq, on = torch.empty_like(v), torch.empty((V, Nc, 1, 2), dtype=torch.int16, device="cuda"), torch.empty((V, 1), dtype=torch.float32, device="cuda")
+    bad = 0
+    for it in range(applies):
+        dg = it % 2
+        op.apply_hout(src, nm, out, oq, on, dagger=dg)
+        ok = torch.equal(torch.view_as_real(out), torch.view_as_real(refs[dg][0])) and torch.equal(oq, refs[dg][1]) and torch.equal(on, refs[dg][2])
+        bad += int(not ok)
+    assert bad == 0, f"{bad} of {applies} applies differ from the first one"
+    # and the first one is right: the 16-bit result is the vector quantiser applied to the complex64 result
+    q2 = torch.empty_like(oq)
+    n2 = torch.empty_like(on)
+    cop.coarse_op_quantize_vec_i16(refs[1][0], Nc, 1, q2, n2)
+    torch.cuda.synchronize()
+    assert torch.equal(q2, refs[1][1]) and torch.equal(n2, refs[1][2])
+    op.close()
+
+
 def test_hvec_multi_rhs_complex64_links_stay_on_simple(oracle_lib):
     _run(oracle_lib, (2, 2, 1, 2), 48, cop.LINK_C64, 3, 0, cop.PATH_SIMPLE, pin_path=False)
 
