@@ -99,9 +99,13 @@ enum {
                                 written by work still in flight on the stream (they are read before the kernel orders
                                 itself against its predecessor); 2 never.  Results are bit-identical either way. */
     COARSE_OPT_SPLIT_DAGGER = 6, /* dagger = 1, 1 RHS, lattices with fewer sites than SMs: split each site's
-                                contraction over its row chunks, the CTA that finishes a site's last chunk adds the
-                                partial vectors in chunk order (one launch, deterministic): 0 auto, 1 never,
-                                2 always (needs the workspace coarse_op_set_links allocates on such lattices) */
+                                contraction over its row chunks.  The kernel is launched as thread-block clusters
+                                of 4 (2) CTAs, one site per cluster at a time; the partial vectors meet in the
+                                shared memory of the cluster's first CTA behind one cluster barrier (one launch,
+                                deterministic): 0 auto, 1 never, 2 always, 3 always with the global-memory scheme
+                                instead (partial vectors in a workspace coarse_op_set_links allocates on such
+                                lattices, the CTA that counts a site's last chunk in adds them in chunk order; also
+                                the fallback where clusters cannot be launched) */
     COARSE_OPT_WARP_ITEMS = 7, /* 1-RHS plain apply: the STREAM variant in which small teams of consumer warps own
                                 whole work items and every stage of theirs (csrc/stream2_kernel.cuh) instead of all
                                 eight warps sharing every stage: 0 auto (int16 links with Nc >= 48, and Nc = 32, on lattices with at

@@ -474,7 +474,7 @@ int coarse_op_set_option(coarse_op_t* op, int option, int value) {
             op->keep_opt = value;
             return COARSE_OK;
         case COARSE_OPT_SPLIT_DAGGER:
-            if (value < 0 || value > 2) return fail(COARSE_EINVAL, "set_option: split_dagger must be 0 (auto), 1 (never) or 2 (always)");
+            if (value < 0 || value > 3) return fail(COARSE_EINVAL, "set_option: split_dagger must be 0 (auto), 1 (never), 2 (always) or 3 (always, workspace scheme)");
             op->split_opt = value;
             return COARSE_OK;
         case COARSE_OPT_TENSOR_I8:

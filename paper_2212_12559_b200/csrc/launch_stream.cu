@@ -25,17 +25,28 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     // dagger = 1 has one work item per site; on a lattice with fewer sites than SMs (the paper's level 3:
     // 32 sites per GPU) the contraction of a site is split over its NB row chunks, one item each, and the
     // CTA that finishes a site's last chunk adds the NB partial vectors in order (stream_kernel.cuh).
+    // COARSE_OPT_SPLIT_DAGGER: 0 auto (clusters on lattices with fewer sites than SMs), 1 never, 2 always (clusters),
+    // 3 always with the global-memory scheme: partial vectors in a workspace, a per-site counter, the CTA that counts a
+    // site's last chunk in adds them (a device-scope fence, an atomic round trip and an L2 read at the end of the
+    // kernel: measured 3.7 us of a 12.2 us apply on the paper's level-3 volume, against ~1 us for the cluster barrier).
     p.split = 0;
     p.partial = nullptr;
     p.split_count = nullptr;
-    if (DAG && !GEN && !HV && base.n_items == 0 && !base.hout_q && Gm::NB > 1 && op->split_ws &&
-        (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes &&
-        (op->split_opt == 2 || (op->split_opt == 0 && p.n_sites < op->num_sms))) {
-        p.split = 1;
-        p.partial = op->split_ws;
-        p.split_count = op->split_count;
-        p.n_items = p.n_sites * Gm::NB;
-    }
+    p.cluster = 0;
+    const bool split_ok = DAG && !GEN && !HV && base.n_items == 0 && !base.hout_q && Gm::NB > 1;
+    const bool split_wanted = op->split_opt >= 2 || (op->split_opt == 0 && p.n_sites < op->num_sms);
+    if (split_ok && split_wanted && op->split_opt != 3)
+        p.cluster = Gm::NB >= STREAM_MAX_CLUSTER ? STREAM_MAX_CLUSTER : 2;
+    auto use_workspace_split = [&]() {
+        p.cluster = 0;
+        if (split_ok && split_wanted && op->split_ws && (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes) {
+            p.split = 1;
+            p.partial = op->split_ws;
+            p.split_count = op->split_count;
+            p.n_items = p.n_sites * Gm::NB;
+        }
+    };
+    if (!p.cluster) use_workspace_split();
     int stages = (op->max_smem - Gm::fixed_bytes(DAG)) / (Gm::stage_bytes(DAG) + 16);
     if (stages > 12) stages = 12;
     if (stages < 2) return fail(COARSE_EUNSUPPORTED, "STREAM: shared memory too small for Nc=%d", NC);
@@ -57,9 +68,34 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     cudaError_t e = ensure_dynamic_smem(kern, op->device, smem, attr_cache);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(stream kernel)");
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
+    p.pdl = base.pdl;
+    if (p.cluster) {
+        // one site per cluster at a time; as many clusters as the chip holds (or COARSE_OPT_GRID / cluster size)
+        int n_cl = grid / p.cluster;
+        if (n_cl < 1) n_cl = 1;
+        if (n_cl > p.n_sites) n_cl = p.n_sites;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(n_cl * p.cluster);
+        cfg.blockDim = dim3(Gm::THREADS);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[2];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = p.cluster;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[1].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = p.pdl ? 2 : 1;
+        if (n_cl < 1) return COARSE_OK;
+        e = cudaLaunchKernelEx(&cfg, kern, p);
+        if (e == cudaSuccess) return COARSE_OK;
+        cudaGetLastError();                  // clusters of this size cannot be scheduled here: the workspace scheme
+        use_workspace_split();
+    }
     if (grid > p.n_items - p.item_begin) grid = p.n_items - p.item_begin;
     if (grid < 1) return COARSE_OK;
-    p.pdl = base.pdl;
     if (p.pdl) {
         // programmatic dependent launch: this kernel may start while the previous kernel of the stream
         // drains; it orders itself against that kernel's memory with griddepcontrol.wait (stream_kernel.cuh)

@@ -60,6 +60,10 @@ struct StreamParams {
     int split;
     float2* partial;          // [n_sites * NB][Nc]
     unsigned int* split_count;   // [n_sites], zero between launches (the reducing CTA resets its site's counter)
+    // ... or, launched as thread-block CLUSTERS of `cluster` CTAs (one site per cluster, the CTA of rank r takes the
+    // chunks r, r + cluster, ..): the partial vectors meet in the shared memory of the rank-0 CTA (distributed shared
+    // memory stores, one cluster barrier per site) - no global round trip, no device-scope fence, no atomic
+    int cluster;
     // HV (half-precision input vectors, coarse_op_apply_hvec): `in` points at int16 (re,im) entries
     const float* vnorms;      // fp32 norm per site (nrhs = 1)
     // Half-precision OUTPUT (coarse_op_apply_hout): besides the complex64 result in `out`, the CTA takes
@@ -70,6 +74,10 @@ struct StreamParams {
     short2* hout_q;           // NULL: off
     float* hout_norms;        // [V]
 };
+
+// Split dagger apply in clusters (StreamParams::cluster): ranks 1.. of a cluster store their partial vector into the rank-0
+// CTA's buffer [2 site parities][STREAM_MAX_CLUSTER - 1][NC].
+constexpr int STREAM_MAX_CLUSTER = 4;
 
 constexpr int stream_pow2ceil(int v) { return v <= 1 ? 1 : v <= 2 ? 2 : v <= 4 ? 4 : v <= 8 ? 8 : v <= 16 ? 16 : 32; }
 constexpr int stream_passes(int q) {
@@ -126,7 +134,8 @@ struct StreamGeom {
 
     static constexpr int stage_bytes(bool dag) { return LINK_STAGE + (dag ? VEC_STAGE_D : VEC_STAGE_N); }
     static constexpr int SITE_BYTES = NC * 8;                  // half-precision output: the site's complex64 rows
-    static constexpr int fixed_bytes(bool dag) { return (dag ? RED_BYTES : 0) + 128 + SITE_BYTES; }
+    static constexpr int CL_BYTES = 2 * (STREAM_MAX_CLUSTER - 1) * NC * 8;   // split dagger apply in clusters (rank 0's inbox)
+    static constexpr int fixed_bytes(bool dag) { return (dag ? RED_BYTES + CL_BYTES : 0) + 128 + SITE_BYTES; }
     static int smem_bytes(bool dag, int stages) { return stages * (stage_bytes(dag) + 16) + fixed_bytes(dag); }
 };
 
@@ -174,6 +183,20 @@ __device__ __forceinline__ float2 cfinal(const CAcc& acc) {
 // Per-site half-precision epilogue, called by all consumer threads of the CTA that owns site s once its NC result
 // entries are in `sbuf` (shared memory).  scratch: 9 words of shared memory.  The arithmetic is that of
 // quantize_vec_i16_kernel (R22): norm = amax / 32767 (fp32 division), q = clamp(rint(component / norm)).
+namespace ptx {
+__device__ __forceinline__ uint32_t mapa_shared(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_f2(uint32_t addr, float2 v) {
+    asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+}  // namespace ptx
+
 template <int NC, int NTHREADS>
 __device__ __forceinline__ void half_out_epilogue(const StreamParams& p, int s, const float2* sbuf, uint32_t* scratch) {
     ptx::named_bar_sync(1, NTHREADS);                    // every row of the site is in sbuf
@@ -237,8 +260,12 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
     // The it-th work item of this CTA.  Default: items blockIdx.x, blockIdx.x + gridDim.x, ...  Half-precision output
     // with several row blocks per site: site-major, the NB items of a site in a row (the CTA owns the site).
     const bool site_major = !DAG && NB > 1 && p.hout_q != nullptr;
+    // cluster mode (split dagger apply): the CTAs of a cluster share their work items (sites); rank r takes the chunks r, r + CR, ..
+    const int CR = DAG ? p.cluster : 0;
+    const int crank = CR ? (int)blockIdx.x % CR : 0;
     auto item_at = [&](int it) -> int {
         if (site_major) return p.item_begin + ((int)blockIdx.x + (it / NB) * (int)gridDim.x) * NB + it % NB;
+        if (CR) return p.item_begin + (int)blockIdx.x / CR + it * ((int)gridDim.x / CR);
         return p.item_begin + (int)blockIdx.x + it * (int)gridDim.x;
     };
 
@@ -280,10 +307,11 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                 const int sm = DAG ? sv : s;
                 const unsigned char* mat = p.links + ((int64_t)sm * 9 + m) * ((int64_t)NC * ROWBYTES);
                 const unsigned char* vec = reinterpret_cast<const unsigned char*>((GEN && m == 0) ? p.in_local : p.in) + (int64_t)sv * NC * VE;
-                const int c_begin = (DAG && p.split) ? item % NB : 0;
+                const int c_begin = (DAG && p.split) ? item % NB : crank;
                 const int c_end = DAG ? (p.split ? c_begin + 1 : NB) : 1;
+                const int c_step = CR ? CR : 1;
 #pragma unroll 1
-                for (int c = c_begin; c < c_end; ++c) {
+                for (int c = c_begin; c < c_end; c += c_step) {
                     const int r0 = DAG ? c * RS : rb * RS;
                     if (deferring && n_def == S) flush_deferred();    // the ring is full: the vectors are needed now
                     ptx::mbar_wait(empty0 + 8u * slot, phase ^ 1u);
@@ -299,6 +327,12 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                     __syncwarp();
                     if (++slot == S) { slot = 0; phase ^= 1u; }
                 }
+            }
+            if (CR) {
+                // the site's cluster barrier counts every thread of the cluster: arrive with the consumers (queued vector
+                // copies must be out first, the consumers are waiting for them)
+                if (deferring) flush_deferred();
+                ptx::cluster_sync_all();
             }
         }
         if (deferring) flush_deferred();
@@ -338,6 +372,12 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
     next2_scale = fetch_scale(item_at(1));
     float2* sbuf = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(bars + 2 * S) + 128);     // half-precision output
     uint32_t* hscratch = reinterpret_cast<uint32_t*>(bars + 2 * S);
+    // cluster mode: rank 0's inbox [2][STREAM_MAX_CLUSTER - 1][NC] behind the half-output buffer; the other ranks address it
+    // through the cluster's shared-memory window
+    static_assert(NC <= W * 32, "cluster mode: one output column per consumer thread");
+    float2* cl_buf = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(bars + 2 * S) + 128 + Gm::SITE_BYTES);
+    const uint32_t cl_inbox = CR ? ptx::mapa_shared(ptx::smem_u32(cl_buf), 0u) : 0u;
+    float2 cl_keep = make_float2(0.f, 0.f);
 
     for (int it = 0;; ++it) {
         const int item = item_at(it);
@@ -463,7 +503,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                 float sc = (I16 || HV) ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
                 if constexpr (GEN) sc *= (m == 0) ? p.alpha : p.beta;
 #pragma unroll 1
-                for (int c = p.split ? item % NB : 0; c < (p.split ? item % NB + 1 : NB); ++c) {
+                for (int c = p.split ? item % NB : crank; c < (p.split ? item % NB + 1 : NB); c += (CR ? CR : 1)) {
                     ptx::mbar_wait(full0 + 8u * slot, phase);
                     const uint32_t lbase = link_u32 + slot * LINK_STAGE + qi * 16;
                     const uint32_t vbase = vec_u32 + slot * VEC_STAGE;
@@ -526,9 +566,26 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                     sum.x = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].x, sum.x);
                     sum.y = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].y, sum.y);
                 }
-                if (p.split) p.partial[(int64_t)item * NC + t] = sum;
+                if (CR) {
+                    // ranks 1.. send their partial sum to the rank-0 CTA's inbox (distributed shared memory); rank 0 keeps its
+                    // own in a register and adds the others, in rank order, behind the site's cluster barrier
+                    if (crank) ptx::st_cluster_f2(cl_inbox + (uint32_t)(((it & 1) * (STREAM_MAX_CLUSTER - 1) + crank - 1) * NC + t) * 8u, sum);
+                    else cl_keep = sum;
+                } else if (p.split) p.partial[(int64_t)item * NC + t] = sum;
                 else p.out[(int64_t)s * NC + t] = sum;
                 if (p.hout_q) sbuf[t] = sum;
+            }
+            if (CR) {
+                ptx::cluster_sync_all();
+                if (crank == 0 && threadIdx.x < NC) {
+                    float2 sum = cl_keep;
+                    for (int r = 1; r < CR; ++r) {
+                        const float2 x = cl_buf[((it & 1) * (STREAM_MAX_CLUSTER - 1) + r - 1) * NC + threadIdx.x];
+                        sum.x += x.x;
+                        sum.y += x.y;
+                    }
+                    p.out[(int64_t)s * NC + threadIdx.x] = sum;
+                }
             }
             if (p.split) {
                 // last-arriver reduction: every consumer thread publishes its part of the partial vector, one

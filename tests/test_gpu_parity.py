@@ -491,26 +491,28 @@ def test_pdl_with_parts_hvec_and_graph_capture(oracle_lib):
     assert torch.equal(torch.view_as_real(res[0][1]), torch.view_as_real(res[1][1]))
 
 
-@pytest.mark.parametrize("dims", [(2, 4, 2, 2), (1, 1, 1, 1), (3, 2, 1, 4)])
+@pytest.mark.parametrize("dims", [(2, 4, 2, 2), (1, 1, 1, 1), (3, 2, 1, 4), (3, 3, 3, 5)])
 @pytest.mark.parametrize("Nc", [32, 48, 64, 96, 128, 192])
 @pytest.mark.parametrize("prec", [cop.LINK_C64, cop.LINK_I16])
 def test_split_dagger_on_tiny_lattices(oracle_lib, dims, Nc, prec):
     """dagger = 1 with fewer sites than SMs (the paper's level 3 has 32 sites per GPU): the contraction of
-    a site is split over its row chunks and the CTA that finishes a site's last chunk adds the partial vectors
-    (one launch).  Auto picks it, forcing it off must give the same numbers up to summation order, both must
-    match the oracle, and repeated launches must be bit-identical (the chunk counters reset themselves)."""
+    a site is split over its row chunks - in thread-block clusters whose partial vectors meet in the first CTA's
+    shared memory (auto, 2), or through a global workspace with a per-site counter (3).  Forcing it off (1) must give
+    the same numbers up to summation order, all must match the oracle, and repeated launches must be bit-identical for
+    any grid (one cluster walking every site: the inbox is double buffered; the chunk counters reset themselves).
+    135 sites: several sites per cluster also in the default launch."""
     V = synth.lattice_volume(dims)
     links, scales, links_h, scales_h = _links_for(dims, Nc, prec, 61, False, oracle_lib)
     vin = synth.make_vectors(dims, Nc, 1, 62, device="cuda")
     ref = oracle_lib.coarse_apply(dims, Nc, links_h, vin.cpu().numpy(), dagger=1, link_precision=prec, scales=scales_h)
-    for mode in (0, 1, 2):
+    for mode in (0, 1, 2, 3):
         op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales).set_option(cop.OPT_SPLIT_DAGGER, mode)
         out = torch.full_like(vin, float("nan"))
         op.apply(vin, out, dagger=1)
         torch.cuda.synchronize()
         assert op.last_path == cop.PATH_STREAM and op.last_launches == 1
         assert rel_l2_per_rhs(out.cpu().numpy(), ref) <= TOL
-        for grid in (0, 1, 5):                          # many launches, also with every chunk of a site on one CTA
+        for grid in (0, 1, 5, 9):                       # many launches, also with every chunk of a site on one CTA
             op.set_option(cop.OPT_GRID, grid)
             for _ in range(3):
                 again = torch.full_like(vin, float("nan"))
@@ -523,6 +525,37 @@ def test_split_dagger_on_tiny_lattices(oracle_lib, dims, Nc, prec):
         torch.cuda.synchronize()
         assert op.last_launches == 1
         op.close()
+
+
+@pytest.mark.parametrize("Nc,prec", [(192, cop.LINK_I16), (128, cop.LINK_C64), (48, cop.LINK_C64)])
+def test_split_dagger_clusters_bit_reproducible_under_stress(Nc, prec):
+    """The paper's level-3 volume (32 sites): 3000 alternating A / A^H applies in one stream (PDL chain, cluster launches for
+    A^H), every result equal to the first one's bit for bit."""
+    dims = (2, 4, 2, 2)
+    V = synth.lattice_volume(dims)
+    links = synth.make_arbitrary_links(dims, Nc, 5, device="cuda")
+    scales = None
+    if prec == cop.LINK_I16:
+        q = torch.empty((V, 9, Nc, Nc, 2), dtype=torch.int16, device="cuda")
+        scales = torch.empty((V, 9), dtype=torch.float32, device="cuda")
+        cop.coarse_op_quantize_i16(links, Nc, q, scales)
+        links = q
+    vin = synth.make_vectors(dims, Nc, 1, 6, device="cuda")
+    op = cop.CoarseOp(dims, Nc, prec).set_links(links, scales)
+    refs = {}
+    for dagger in (0, 1):
+        refs[dagger] = torch.empty_like(vin)
+        op.apply(vin, refs[dagger], dagger=dagger)
+    outs = [torch.empty_like(vin) for _ in range(6)]
+    bad = 0
+    for rep in range(500):
+        for k in range(6):
+            op.apply(vin, outs[k], dagger=k % 2)
+        torch.cuda.synchronize()
+        for k in range(6):
+            bad += int(not torch.equal(torch.view_as_real(outs[k]), torch.view_as_real(refs[k % 2])))
+    assert bad == 0, f"{bad} of 3000 applies differ from the first one"
+    op.close()
 
 
 def test_read_probe_runs_and_validates_arguments():
