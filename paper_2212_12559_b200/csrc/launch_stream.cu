@@ -33,7 +33,7 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     p.partial = nullptr;
     p.split_count = nullptr;
     p.cluster = 0;
-    const bool split_ok = DAG && !GEN && !HV && base.n_items == 0 && !base.hout_q && Gm::NB > 1;
+    const bool split_ok = DAG && !FINE && !GEN && !HV && base.n_items == 0 && !base.hout_q && Gm::NB > 1;
     const bool split_wanted = op->split_opt >= 2 || (op->split_opt == 0 && p.n_sites < op->num_sms);
     if (split_ok && split_wanted && op->split_opt != 3)
         p.cluster = Gm::NB >= STREAM_MAX_CLUSTER ? STREAM_MAX_CLUSTER : 2;
@@ -88,10 +88,14 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
         attr[1].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr;
         cfg.numAttrs = p.pdl ? 2 : 1;
-        if (n_cl < 1) return COARSE_OK;
-        e = cudaLaunchKernelEx(&cfg, kern, p);
-        if (e == cudaSuccess) return COARSE_OK;
-        cudaGetLastError();                  // clusters of this size cannot be scheduled here: the workspace scheme
+        if constexpr (DAG && !FINE && !GEN && !HV) {
+            auto kern_cl = coarse_apply_stream<NC, I16, DAG, FINE, GEN, HV, true>;
+            static SmemAttrCache attr_cache_cl;
+            e = ensure_dynamic_smem(kern_cl, op->device, smem, attr_cache_cl);
+            if (e == cudaSuccess) e = cudaLaunchKernelEx(&cfg, kern_cl, p);
+            if (e == cudaSuccess) return COARSE_OK;
+            cudaGetLastError();              // clusters of this size cannot be scheduled here: the workspace scheme
+        }
         use_workspace_split();
     }
     if (grid > p.n_items - p.item_begin) grid = p.n_items - p.item_begin;

@@ -226,8 +226,12 @@ __device__ __forceinline__ void half_out_epilogue(const StreamParams& p, int s, 
     ptx::named_bar_sync(1, NTHREADS);                    // sbuf and scratch are reused by the next site
 }
 
-template <int NC, bool I16, bool DAG, bool FINE = false, bool GEN = false, bool HV = false>
+// CL: the instantiation launched as thread-block clusters (split dagger apply).  It is a separate kernel because the mere
+// presence of cluster instructions (mapa, barrier.cluster) in a kernel costs ~0.9 us per launch even when they are never
+// executed (measured on the 256-site C1 lattice: dagger = 1 6.4 -> 7.3 us warm with one kernel for both).
+template <int NC, bool I16, bool DAG, bool FINE = false, bool GEN = false, bool HV = false, bool CL = false>
 __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coarse_apply_stream(StreamParams p) {
+    static_assert(!CL || (DAG && !FINE && !GEN && !HV), "cluster launches: the plain dagger = 1 apply");
     static_assert(!(DAG && FINE), "the fine geometry splits output rows: dagger = 0 only");
     static_assert(!(GEN && HV), "half-precision input vectors are implemented for the plain apply");
     using Gm = StreamGeom<NC, I16, FINE, HV>;
@@ -261,7 +265,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
     // with several row blocks per site: site-major, the NB items of a site in a row (the CTA owns the site).
     const bool site_major = !DAG && NB > 1 && p.hout_q != nullptr;
     // cluster mode (split dagger apply): the CTAs of a cluster share their work items (sites); rank r takes the chunks r, r + CR, ..
-    const int CR = DAG ? p.cluster : 0;
+    const int CR = CL ? p.cluster : 0;
     const int crank = CR ? (int)blockIdx.x % CR : 0;
     auto item_at = [&](int it) -> int {
         if (site_major) return p.item_begin + ((int)blockIdx.x + (it / NB) * (int)gridDim.x) * NB + it % NB;
