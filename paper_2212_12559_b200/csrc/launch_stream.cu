@@ -33,13 +33,13 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     p.partial = nullptr;
     p.split_count = nullptr;
     p.cluster = 0;
-    const bool split_ok = DAG && !FINE && !GEN && base.n_items == 0 && !base.hout_q && Gm::NB > 1;     // (HV: clusters only)
+    const bool split_ok = DAG && !FINE && base.n_items == 0 && !base.hout_q && Gm::NB > 1;     // (HV, parts apply: clusters only)
     const bool split_wanted = op->split_opt >= 2 || (op->split_opt == 0 && p.n_sites < op->num_sms);
     if (split_ok && split_wanted && op->split_opt != 3)
         p.cluster = Gm::NB >= STREAM_MAX_CLUSTER ? STREAM_MAX_CLUSTER : 2;
     auto use_workspace_split = [&]() {
         p.cluster = 0;
-        if (split_ok && !HV && split_wanted && op->split_ws && (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes) {
+        if (split_ok && !HV && !GEN && split_wanted && op->split_ws && (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes) {
             p.split = 1;
             p.partial = op->split_ws;
             p.split_count = op->split_count;
@@ -88,7 +88,7 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
         attr[1].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr;
         cfg.numAttrs = p.pdl ? 2 : 1;
-        if constexpr (DAG && !FINE && !GEN) {
+        if constexpr (DAG && !FINE) {
             auto kern_cl = coarse_apply_stream<NC, I16, DAG, FINE, GEN, HV, true>;
             static SmemAttrCache attr_cache_cl;
             e = ensure_dynamic_smem(kern_cl, op->device, smem, attr_cache_cl);

@@ -231,7 +231,7 @@ __device__ __forceinline__ void half_out_epilogue(const StreamParams& p, int s, 
 // executed (measured on the 256-site C1 lattice: dagger = 1 6.4 -> 7.3 us warm with one kernel for both).
 template <int NC, bool I16, bool DAG, bool FINE = false, bool GEN = false, bool HV = false, bool CL = false>
 __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coarse_apply_stream(StreamParams p) {
-    static_assert(!CL || (DAG && !FINE && !GEN), "cluster launches: the plain dagger = 1 apply (complex64 or half-precision input)");
+    static_assert(!CL || (DAG && !FINE), "cluster launches: dagger = 1 (plain apply, half-precision input, parts apply)");
     static_assert(!(DAG && FINE), "the fine geometry splits output rows: dagger = 0 only");
     static_assert(!(GEN && HV), "half-precision input vectors are implemented for the plain apply");
     using Gm = StreamGeom<NC, I16, FINE, HV>;
@@ -567,8 +567,10 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                     sum.y += x.y;
                 }
                 if constexpr (GEN) {
-                    sum.x = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].x, sum.x);
-                    sum.y = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].y, sum.y);
+                    if (crank == 0) {                                  // (cluster mode: the identity term once per site)
+                        sum.x = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].x, sum.x);
+                        sum.y = fmaf(p.alpha, uloc[(GEN && UL > 1) ? ku : 0].y, sum.y);
+                    }
                 }
                 if (CR) {
                     // ranks 1.. send their partial sum to the rank-0 CTA's inbox (distributed shared memory); rank 0 keeps its
