@@ -72,7 +72,7 @@ enum {
 
 /* Kernel families, each compiled for Nc in {32,48,64,96,128,192}; every family computes the same operation and the
  * tests run parity on each.  AUTO: 1 RHS -> STREAM; 2-4 RHS -> STREAM (its multi-RHS kernel), except int16 links
- * (Nc = 48: only at 4 RHS) and complex64 links with exactly 4 RHS in dagger = 0 (Nc >= 48) -> TENSOR; 5 RHS and more -> TENSOR; BLOCK only on request (or when no tensor map can be made for the links);
+ * (Nc = 48: only at 4 RHS; 2-3 RHS only on lattices with at least two tensor work items per SM) and complex64 links with exactly 4 RHS in dagger = 0 (Nc >= 48) -> TENSOR; 5 RHS and more -> TENSOR; BLOCK only on request (or when no tensor map can be made for the links);
  * Nc outside the compiled set -> SIMPLE. */
 enum {
     COARSE_PATH_AUTO = 0,

@@ -280,7 +280,14 @@ int auto_path(const coarse_op* op, int nrhs, int dagger) {
     if (stream_supports(op->Nc, nrhs)) return COARSE_PATH_STREAM;
     if (stream_mr_supports(op->Nc, nrhs)) {
         const bool i8 = op->prec == COARSE_LINK_I16 && op->link_map_i8_ok && op->vscale && op->tensor_i8_opt != 1;
-        if (tensor_ok && i8 && nrhs >= tensor_i8_min_nrhs(op->Nc)) return COARSE_PATH_TENSOR;
+        // ... on lattices that give the tensor kernel at least two work items per SM.  Below that its long per-item chain
+        // (9 matrices x Nc / 32 stages) sets a floor of 15-30 us, and 2-3 right-hand sides are faster on STREAM-MR (measured
+        // us, dagger 0 / 1, STREAM-MR against TENSOR, 3 RHS: the paper's level-3 volume, 32 sites Nc = 192, 16 / 36 against
+        // 29 / 30; 32 sites Nc = 128 7 / 17 against 21 / 22; 256 sites Nc = 64 12 / 11 against 15 / 15; 1024 sites Nc = 64
+        // 37 / 34 against 35 / 36).  4 right-hand sides stay on TENSOR (some STREAM-MR int16 instantiations spill at 4).
+        const int64_t t_items = op->Nc <= 64 ? ((int64_t)op->lat.V + 1) / 2 : (int64_t)op->lat.V * (op->Nc > 128 ? 2 : 1);
+        const bool tiny = nrhs <= 3 && t_items < 2 * (int64_t)op->num_sms;
+        if (tensor_ok && i8 && !tiny && nrhs >= tensor_i8_min_nrhs(op->Nc)) return COARSE_PATH_TENSOR;
         if (tensor_ok && op->prec == COARSE_LINK_C64 && nrhs == 4 && dagger == 0 && op->Nc >= 48) return COARSE_PATH_TENSOR;
         return COARSE_PATH_STREAM;
     }

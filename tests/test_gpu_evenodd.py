@@ -122,10 +122,12 @@ def test_parts_stream_few_rhs(oracle_lib, Nc, prec, nrhs, dagger, parity, local)
 
 
 def test_parts_auto_routes_few_rhs():
-    dims = (2, 2, 2, 2)
-    for Nc, prec, nrhs, want in ((48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_TENSOR), (64, cop.LINK_I16, 2, cop.PATH_TENSOR), (48, cop.LINK_I16, 2, cop.PATH_STREAM),
-                                 (128, cop.LINK_I16, 3, cop.PATH_TENSOR), (128, cop.LINK_C64, 2, cop.PATH_STREAM)):
-        V = 16
+    small, large = (2, 2, 2, 2), (4, 4, 4, 10)        # int16, 2-3 RHS: TENSOR needs two work items per SM, else STREAM-MR
+    for dims, Nc, prec, nrhs, want in ((small, 48, cop.LINK_C64, 3, cop.PATH_STREAM), (small, 64, cop.LINK_I16, 4, cop.PATH_TENSOR),
+                                       (large, 64, cop.LINK_I16, 2, cop.PATH_TENSOR), (small, 64, cop.LINK_I16, 2, cop.PATH_STREAM),
+                                       (small, 48, cop.LINK_I16, 2, cop.PATH_STREAM), (large, 128, cop.LINK_I16, 3, cop.PATH_TENSOR),
+                                       (small, 128, cop.LINK_I16, 3, cop.PATH_STREAM), (small, 128, cop.LINK_C64, 2, cop.PATH_STREAM)):
+        V = synth.lattice_volume(dims)
         if prec == cop.LINK_C64:
             links, scales = torch.zeros((V, 9, Nc, Nc), dtype=torch.complex64, device="cuda"), None
         else:
@@ -274,7 +276,7 @@ def test_parts_identity_in_place_values_multi_rhs(oracle_lib, Nc, prec, dagger):
     """The same in-place update with several right-hand sides, on the tensor kernels (the identity term is read in
     the epilogue by the thread that then stores the element) and on STREAM-MR (read at the store)."""
     dims = (2, 4, 2, 2)
-    for nrhs, want in ((5, cop.PATH_TENSOR), (3, cop.PATH_TENSOR if (prec == cop.LINK_I16 and Nc >= 96) else cop.PATH_STREAM)):
+    for nrhs, want in ((5, cop.PATH_TENSOR), (3, cop.PATH_STREAM)):       # (32 sites: 2-3 RHS stay on STREAM-MR for int16 links too)
         links_d, scales_d, links_h, scales_h, u, w = _make(oracle_lib, dims, Nc, prec, 978, nrhs)
         op = cop.CoarseOp(dims, Nc, prec).set_links(links_d, scales_d)
         buf = u.clone()

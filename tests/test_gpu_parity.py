@@ -198,16 +198,20 @@ def test_block_path_any_grid(oracle_lib, grid):
 
 
 def test_auto_path_selection():
-    dims = (2, 2, 2, 2)
-    cases = [(48, cop.LINK_C64, 1, cop.PATH_STREAM), (48, cop.LINK_C64, 16, cop.PATH_TENSOR),
-             (48, cop.LINK_C64, 3, cop.PATH_STREAM), (64, cop.LINK_I16, 4, cop.PATH_TENSOR),
-             (64, cop.LINK_I16, 2, cop.PATH_TENSOR), (48, cop.LINK_I16, 3, cop.PATH_STREAM), (48, cop.LINK_I16, 4, cop.PATH_TENSOR),
-             (32, cop.LINK_I16, 2, cop.PATH_TENSOR), (64, cop.LINK_C64, 4, cop.PATH_TENSOR), (32, cop.LINK_C64, 4, cop.PATH_STREAM),
-             (48, cop.LINK_C64, 5, cop.PATH_TENSOR), (64, cop.LINK_I16, 16, cop.PATH_TENSOR),
-             (96, cop.LINK_C64, 8, cop.PATH_TENSOR), (48, cop.LINK_C64, 17, cop.PATH_TENSOR),
-             (192, cop.LINK_I16, 12, cop.PATH_TENSOR), (6, cop.LINK_C64, 2, cop.PATH_SIMPLE)]
-    for Nc, prec, nrhs, want in cases:
-        V = 16
+    small, large = (2, 2, 2, 2), (4, 4, 4, 10)       # 16 sites; 640 sites: at least two tensor work items per SM
+    cases = [(small, 48, cop.LINK_C64, 1, cop.PATH_STREAM), (small, 48, cop.LINK_C64, 16, cop.PATH_TENSOR),
+             (small, 48, cop.LINK_C64, 3, cop.PATH_STREAM), (small, 64, cop.LINK_I16, 4, cop.PATH_TENSOR),
+             # int16 links, 2-3 RHS: the integer tensor kernel on large lattices, STREAM-MR on tiny ones
+             (large, 64, cop.LINK_I16, 2, cop.PATH_TENSOR), (small, 64, cop.LINK_I16, 2, cop.PATH_STREAM),
+             (large, 128, cop.LINK_I16, 3, cop.PATH_TENSOR), (small, 128, cop.LINK_I16, 3, cop.PATH_STREAM),
+             (large, 48, cop.LINK_I16, 3, cop.PATH_STREAM), (small, 48, cop.LINK_I16, 4, cop.PATH_TENSOR),
+             (large, 32, cop.LINK_I16, 2, cop.PATH_TENSOR), (small, 64, cop.LINK_C64, 4, cop.PATH_TENSOR),
+             (small, 32, cop.LINK_C64, 4, cop.PATH_STREAM),
+             (small, 48, cop.LINK_C64, 5, cop.PATH_TENSOR), (small, 64, cop.LINK_I16, 16, cop.PATH_TENSOR),
+             (small, 96, cop.LINK_C64, 8, cop.PATH_TENSOR), (small, 48, cop.LINK_C64, 17, cop.PATH_TENSOR),
+             (small, 192, cop.LINK_I16, 12, cop.PATH_TENSOR), (small, 6, cop.LINK_C64, 2, cop.PATH_SIMPLE)]
+    for dims, Nc, prec, nrhs, want in cases:
+        V = synth.lattice_volume(dims)
         if prec == cop.LINK_C64:
             links, scales = torch.zeros((V, 9, Nc, Nc), dtype=torch.complex64, device="cuda"), None
         else:
