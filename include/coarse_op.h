@@ -98,7 +98,8 @@ enum {
                                 flight in front of that one); 1 always: the LINK and scale arrays must then not be
                                 written by work still in flight on the stream (they are read before the kernel orders
                                 itself against its predecessor); 2 never.  Results are bit-identical either way. */
-    COARSE_OPT_SPLIT_DAGGER = 6, /* dagger = 1, 1 RHS, lattices with fewer sites than SMs: split each site's
+    COARSE_OPT_SPLIT_DAGGER = 6, /* dagger = 1, 1-4 RHS on STREAM, lattices so small that every site can have a cluster of
+                                4 (2) CTAs to itself at once (sites x cluster size <= SMs): split each site's
                                 contraction over its row chunks.  The kernel is launched as thread-block clusters
                                 of 4 (2) CTAs, one site per cluster at a time; the partial vectors meet in the
                                 shared memory of the cluster's first CTA behind one cluster barrier (one launch,

@@ -34,9 +34,16 @@ int launch_stream_t(const coarse_op* op, const StreamParams& base, cudaStream_t 
     p.split_count = nullptr;
     p.cluster = 0;
     const bool split_ok = DAG && !FINE && base.n_items == 0 && !base.hout_q && Gm::NB > 1;     // (HV, parts apply: clusters only)
-    const bool split_wanted = op->split_opt >= 2 || (op->split_opt == 0 && p.n_sites < op->num_sms);
+    // auto: only when every site gets a cluster of its own at once - the largest cluster size (4, 2) with n_sites x size <= SMs.
+    // Measured on Nc = 192 int16 (us, clusters / workspace scheme / no split): 32 sites 10.1 / 12.6 / 20.7, 64 sites (size 4, two
+    // sites per cluster in turn) 19.5 / 18.8 / 21.0, 128 sites 57.7 / 40.7 / 27.0 - several sites per cluster, or chunks of
+    // several sites per CTA, lose against one CTA per site.
+    int auto_cluster = 0;
+    if (Gm::NB >= STREAM_MAX_CLUSTER && (int64_t)p.n_sites * STREAM_MAX_CLUSTER <= op->num_sms) auto_cluster = STREAM_MAX_CLUSTER;
+    else if ((int64_t)p.n_sites * 2 <= op->num_sms) auto_cluster = 2;
+    const bool split_wanted = op->split_opt >= 2 || (op->split_opt == 0 && auto_cluster > 0);
     if (split_ok && split_wanted && op->split_opt != 3)
-        p.cluster = Gm::NB >= STREAM_MAX_CLUSTER ? STREAM_MAX_CLUSTER : 2;
+        p.cluster = op->split_opt == 0 ? auto_cluster : (Gm::NB >= STREAM_MAX_CLUSTER ? STREAM_MAX_CLUSTER : 2);
     auto use_workspace_split = [&]() {
         p.cluster = 0;
         if (split_ok && !HV && !GEN && split_wanted && op->split_ws && (size_t)p.n_sites * Gm::NB * NC * 8 <= op->split_ws_bytes) {

@@ -15,6 +15,7 @@ int launch_stream_mr_t(const coarse_op* op, const StreamParams& base, cudaStream
     using Gm = StreamGeom<NC, I16, false, false, true>;
     using Gr = StreamMrGeom<NC, I16, R>;
     StreamParams p = base;
+    p.cluster = 0;
     p.n_items = DAG ? base.n_sites : base.n_sites * Gm::NB;      // n_sites: the parity set of a parts apply, else V
     p.item_begin = 0;
     if (base.n_items > 0) {                       // a site range [item_begin, n_items) was requested (in sites)
@@ -37,6 +38,40 @@ int launch_stream_mr_t(const coarse_op* op, const StreamParams& base, cudaStream
     int grid = op->grid_opt > 0 ? op->grid_opt : op->num_sms;
     if (grid > p.n_items - p.item_begin) grid = p.n_items - p.item_begin;
     if (grid < 1) return COARSE_OK;
+    // dagger = 1 on a lattice with fewer sites than SMs: thread-block clusters, one site per cluster, the contraction of a
+    // site split over the cluster's CTAs (COARSE_OPT_SPLIT_DAGGER 1 / 3: off); falls back to the plain launch
+    if constexpr (DAG) {
+        int auto_cluster = 0;                 // every site a cluster of its own at once (launch_stream.cu)
+        if (Gm::NB >= STREAM_MAX_CLUSTER && (int64_t)p.n_sites * STREAM_MAX_CLUSTER <= op->num_sms) auto_cluster = STREAM_MAX_CLUSTER;
+        else if ((int64_t)p.n_sites * 2 <= op->num_sms) auto_cluster = 2;
+        if (base.n_items == 0 && Gm::NB > 1 && op->split_opt != 1 && op->split_opt != 3 && (op->split_opt == 2 || auto_cluster > 0)) {
+            p.cluster = op->split_opt == 0 ? auto_cluster : (Gm::NB >= STREAM_MAX_CLUSTER ? STREAM_MAX_CLUSTER : 2);
+            int n_cl = (op->grid_opt > 0 ? op->grid_opt : op->num_sms) / p.cluster;
+            if (n_cl < 1) n_cl = 1;
+            if (n_cl > p.n_sites) n_cl = p.n_sites;
+            auto kern_cl = coarse_apply_stream_mr<NC, I16, DAG, R, true>;
+            static SmemAttrCache attr_cache_cl;
+            e = ensure_dynamic_smem(kern_cl, op->device, smem, attr_cache_cl);
+            if (e == cudaSuccess && n_cl >= 1) {
+                cudaLaunchConfig_t cfg = {};
+                cfg.gridDim = dim3(n_cl * p.cluster);
+                cfg.blockDim = dim3(Gm::THREADS);
+                cfg.dynamicSmemBytes = smem;
+                cfg.stream = stream;
+                cudaLaunchAttribute attr[1];
+                attr[0].id = cudaLaunchAttributeClusterDimension;
+                attr[0].val.clusterDim.x = p.cluster;
+                attr[0].val.clusterDim.y = 1;
+                attr[0].val.clusterDim.z = 1;
+                cfg.attrs = attr;
+                cfg.numAttrs = 1;
+                e = cudaLaunchKernelEx(&cfg, kern_cl, p);
+                if (e == cudaSuccess) return COARSE_OK;
+            }
+            cudaGetLastError();
+            p.cluster = 0;
+        }
+    }
     kern<<<grid, Gm::THREADS, smem, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "stream-mr kernel launch");

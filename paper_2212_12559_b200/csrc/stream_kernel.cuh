@@ -192,6 +192,8 @@ __device__ __forceinline__ uint32_t mapa_shared(uint32_t addr, uint32_t rank) {
 __device__ __forceinline__ void st_cluster_f2(uint32_t addr, float2 v) {
     asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
 }
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
@@ -286,6 +288,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
         // stages' LINK copies go out at once (they overlap the previous kernel's tail), their vector copies
         // are queued; griddepcontrol.wait then makes the previous kernel's output visible and the queue
         // is flushed.  Every store of this kernel comes after a vector copy, hence after the wait.
+        bool cl_pending = false;
         bool deferring = p.pdl != 0;
         int n_def = 0;
         const unsigned char* def_src[12];
@@ -333,13 +336,18 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, FINE, HV>::THREADS, 1) coa
                 }
             }
             if (CR) {
-                // the site's cluster barrier counts every thread of the cluster: arrive with the consumers (queued vector
-                // copies must be out first, the consumers are waiting for them)
+                // the site's cluster barrier counts every thread of the cluster.  The producer ARRIVES once the site's last
+                // stage is issued (queued vector copies must be out first, the consumers are waiting for them) and goes on
+                // with the next site's stages; it completes the barrier (wait) only before its next arrival, so the ring
+                // does not drain at site boundaries
                 if (deferring) flush_deferred();
-                ptx::cluster_sync_all();
+                if (cl_pending) ptx::cluster_wait();
+                ptx::cluster_arrive();
+                cl_pending = true;
             }
         }
         if (deferring) flush_deferred();
+        if (cl_pending) ptx::cluster_wait();
         return;
     }
 

@@ -45,12 +45,17 @@ struct StreamMrGeom {
     static constexpr int PRIV_BYTES = G1::W * PRIV_WARP;
     static constexpr bool OK = G1::OK && R >= 2 && R <= 4;
     static constexpr int stage_bytes(bool dag) { return G1::LINK_STAGE + (dag ? VEC_STAGE_D : VEC_STAGE_N); }
-    static constexpr int fixed_bytes(bool dag) { return (dag ? RED_BYTES : PRIV_BYTES) + 128; }
+    static constexpr int CL_BYTES = 2 * (STREAM_MAX_CLUSTER - 1) * NC * R * 8;   // dagger = 1 in clusters: rank 0's inbox (stream_kernel.cuh)
+    static constexpr int fixed_bytes(bool dag) { return (dag ? RED_BYTES + CL_BYTES : PRIV_BYTES) + 128; }
     static int smem_bytes(bool dag, int stages) { return stages * (stage_bytes(dag) + 16) + fixed_bytes(dag); }
 };
 
-template <int NC, bool I16, bool DAG, int R>
+// CL: launched as thread-block clusters on lattices with fewer sites than SMs (dagger = 1: one site per cluster, the CTA of rank r
+// contracts the row chunks r, r + cluster, .., the partial vectors meet in rank 0's shared memory) - its own instantiation, see
+// stream_kernel.cuh.
+template <int NC, bool I16, bool DAG, int R, bool CL = false>
 __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREADS, 1) coarse_apply_stream_mr(StreamParams p) {
+    static_assert(!CL || DAG, "cluster launches: dagger = 1");
     using Gm = StreamGeom<NC, I16, false, false, true>;
     using Gr = StreamMrGeom<NC, I16, R>;
     static_assert(Gr::OK, "unsupported STREAM-MR geometry");
@@ -68,6 +73,10 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
     const uint32_t empty0 = full0 + 8u * S;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int CR = CL ? p.cluster : 0;                                  // CTAs per cluster (0: plain launch)
+    const int crank = CR ? (int)blockIdx.x % CR : 0;
+    const int item0 = p.item_begin + (CR ? (int)blockIdx.x / CR : (int)blockIdx.x);
+    const int item_stride = CR ? (int)gridDim.x / CR : (int)gridDim.x;
     if (threadIdx.x == 0) {
         for (int i = 0; i < S; ++i) {
             ptx::mbar_init(full0 + 8u * i, 1);
@@ -84,7 +93,8 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
         const uint32_t link_u32 = ptx::smem_u32(link_smem), vec_u32 = ptx::smem_u32(vec_smem);
         int slot = 0;
         uint32_t phase = 0;
-        for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
+        bool cl_pending = false;
+        for (int item = item0; item < p.n_items; item += item_stride) {
             const int sidx = DAG ? item : item / NB;
             const int s = p.parity != 2 ? parity_site(p.lat, sidx, p.parity) : sidx;      // parts apply: one parity
             const int rb = DAG ? 0 : item % NB;
@@ -97,7 +107,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                 const unsigned char* mat = p.links + ((int64_t)sm * 9 + m) * ((int64_t)NC * ROWBYTES);
                 const float2* vec = (m == 0 ? p.in_local : p.in) + (int64_t)sv * NC * R;
 #pragma unroll 1
-                for (int c = 0; c < (DAG ? NB : 1); ++c) {
+                for (int c = crank; c < (DAG ? NB : 1); c += (CR ? CR : 1)) {
                     const int r0 = DAG ? c * RS : rb * RS;
                     ptx::mbar_wait(empty0 + 8u * slot, phase ^ 1u);
                     if (ptx::elect_one()) {
@@ -111,7 +121,13 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                     if (++slot == S) { slot = 0; phase ^= 1u; }
                 }
             }
+            if (CR) {                             // the site's cluster barrier counts every thread of the cluster: arrive now,
+                if (cl_pending) ptx::cluster_wait();  // complete it before the next arrival (no drain at site boundaries)
+                ptx::cluster_arrive();
+                cl_pending = true;
+            }
         }
+        if (cl_pending) ptx::cluster_wait();
         return;
     }
 
@@ -135,15 +151,20 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
         return __ldg(p.scales + (int64_t)sm * 9 + lane);
     };
     const bool scale_v = I16 || p.gen != 0;        // the vector operand carries the link scale and / or alpha, beta
-    next_scale = fetch_scale(p.item_begin + blockIdx.x);
-    next2_scale = fetch_scale(p.item_begin + blockIdx.x + gridDim.x);
+    next_scale = fetch_scale(item0);
+    next2_scale = fetch_scale(item0 + item_stride);
 
-    for (int item = p.item_begin + blockIdx.x; item < p.n_items; item += gridDim.x) {
+    // cluster mode: rank 0's inbox [2 site parities][STREAM_MAX_CLUSTER - 1][NC R] behind the barriers
+    float2* cl_buf = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(bars + 2 * S) + 128);
+    const uint32_t cl_inbox = CR ? ptx::mapa_shared(ptx::smem_u32(cl_buf), 0u) : 0u;
+    constexpr int UL = (NC * R + W * 32 - 1) / (W * 32);
+    int it = 0;
+    for (int item = item0; item < p.n_items; item += item_stride, ++it) {
         const int s = site_of(item);
         const int rb = DAG ? 0 : item % NB;
         cur_scale = next_scale;
         next_scale = next2_scale;
-        next2_scale = fetch_scale(item + 2 * gridDim.x);
+        next2_scale = fetch_scale(item + 2 * item_stride);
 
         if (!DAG) {
             CAcc pacc[WL][R];
@@ -250,7 +271,7 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                 float sc = I16 ? __shfl_sync(0xffffffffu, cur_scale, m) : 1.f;
                 if (p.gen) sc *= (m == 0) ? p.alpha : p.beta;
 #pragma unroll 1
-                for (int c = 0; c < NB; ++c) {
+                for (int c = crank; c < NB; c += (CR ? CR : 1)) {
                     ptx::mbar_wait(full0 + 8u * slot, phase);
                     const uint32_t lbase = link_u32 + slot * LINK_STAGE + qi * 16;
                     const uint32_t vbase = vec_u32 + slot * VEC_STAGE;
@@ -301,22 +322,49 @@ __global__ void __launch_bounds__(StreamGeom<NC, I16, false, false, true>::THREA
                             red[((warp * RPL + grp) * NC + (ps * QP + qi) * CPQ + e) * R + r] = cfinal<true>(pacc[ps][e][r]);
             }
             ptx::named_bar_sync(1, W * 32);
-            for (int t = threadIdx.x; t < NC * R; t += W * 32) {
-                float2 sum = make_float2(0.f, 0.f);
+            float2 cl_keep[UL];
 #pragma unroll
-                for (int g = 0; g < W * RPL; ++g) {
-                    const float2 x = red[g * NC * R + t];
-                    sum.x += x.x;
-                    sum.y += x.y;
+            for (int ku = 0; ku < UL; ++ku) {
+                const int t = (int)threadIdx.x + ku * W * 32;
+                cl_keep[ku] = make_float2(0.f, 0.f);
+                if (t < NC * R) {
+                    float2 sum = make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int g = 0; g < W * RPL; ++g) {
+                        const float2 x = red[g * NC * R + t];
+                        sum.x += x.x;
+                        sum.y += x.y;
+                    }
+                    if (p.identity && crank == 0) {
+                        const float2 u = __ldg(p.in_local + (int64_t)s * NC * R + t);
+                        sum.x = fmaf(p.alpha, u.x, sum.x);
+                        sum.y = fmaf(p.alpha, u.y, sum.y);
+                    }
+                    if (!CR) p.out[(int64_t)s * NC * R + t] = sum;
+                    else if (crank) ptx::st_cluster_f2(cl_inbox + (uint32_t)(((it & 1) * (STREAM_MAX_CLUSTER - 1) + crank - 1) * (NC * R) + t) * 8u, sum);
+                    else cl_keep[ku] = sum;
                 }
-                if (p.identity) {
-                    const float2 u = __ldg(p.in_local + (int64_t)s * NC * R + t);
-                    sum.x = fmaf(p.alpha, u.x, sum.x);
-                    sum.y = fmaf(p.alpha, u.y, sum.y);
-                }
-                p.out[(int64_t)s * NC * R + t] = sum;
             }
             ptx::named_bar_sync(1, W * 32);      // red is reused by the next item
+            if (CR) {
+                // the ranks' partial vectors are in rank 0's inbox behind the site's cluster barrier; rank 0 adds them in rank order
+                ptx::cluster_sync_all();
+                if (crank == 0) {
+#pragma unroll
+                    for (int ku = 0; ku < UL; ++ku) {
+                        const int t = (int)threadIdx.x + ku * W * 32;
+                        if (t < NC * R) {
+                            float2 sum = cl_keep[ku];
+                            for (int r = 1; r < CR; ++r) {
+                                const float2 x = cl_buf[((it & 1) * (STREAM_MAX_CLUSTER - 1) + r - 1) * (NC * R) + t];
+                                sum.x += x.x;
+                                sum.y += x.y;
+                            }
+                            p.out[(int64_t)s * NC * R + t] = sum;
+                        }
+                    }
+                }
+            }
         }
     }
 }
